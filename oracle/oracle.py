@@ -1,0 +1,341 @@
+"""OSOG forward-render ORACLE, Python side (test infrastructure, NOT the product).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this module.  It shares nothing with paper_2606_21381_b200/ (no kernels, headers, helpers, tables).
+
+Pieces, each following the passage it cites (line numbers are /root/reference/PAPER.md):
+  render_opd      float64 loop over pixels x particles in C (oracle/osog_oracle.c)   Eq. 1, 2, 7
+  field           U = exp(i 2 pi (OPD/lambda + fx0 x + fy0 y))                        Eq. 2 (A == 1), :113-115
+  pupil_mask      circ(|k| / k_NA) on the FFT grid, integer comparison                Eq. 3 (delta z = 0)
+  intensity       I = | IFFT2( FFT2(U) * P ) |^2                                      :90, :99
+  philox4x32_10   counter-based RNG, written from its published description
+  read_noise      z ~ N(0,1) per (seed, frame, pixel) by Box-Muller                   :126 (Gaussian term)
+  binning         bounding boxes -> tiles -> counts / offsets / ascending lists       DESIGN.md section 3 (B1-B4)
+
+Every reading of the paper taken here (units, pixel centres, quaternion convention, pupil edge,
+FFT normalisation, noise model ...) is listed in DESIGN.md section 3.  Pins: tests/test_oracle_*.py.
+"""
+from __future__ import annotations
+
+import ctypes
+import math
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_LIB = None
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        path = _build.build()
+        lib = ctypes.CDLL(path)
+        fp = ctypes.POINTER(ctypes.c_float)
+        u8p = ctypes.POINTER(ctypes.c_uint8)
+        dp = ctypes.POINTER(ctypes.c_double)
+        lib.osog_oracle_render_opd.argtypes = [ctypes.c_int64] + [fp] * 10 + [u8p] + [
+            ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, dp]
+        lib.osog_oracle_render_opd.restype = None
+        lib.osog_oracle_thickness.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double]
+        lib.osog_oracle_thickness.restype = ctypes.c_double
+        lib.osog_oracle_circumradius.argtypes = [ctypes.c_uint8] + [ctypes.c_float] * 3
+        lib.osog_oracle_circumradius.restype = ctypes.c_double
+        lib.osog_oracle_rot_from_quat.argtypes = [dp, dp]
+        lib.osog_oracle_rot_from_quat.restype = None
+        lib.osog_oracle_prism_planes.argtypes = [ctypes.c_double] * 3 + [dp, dp]
+        lib.osog_oracle_prism_planes.restype = ctypes.c_int
+        _LIB = lib
+    return _LIB
+
+
+_COLS = ("cx", "cy", "qw", "qx", "qy", "qz", "d0", "d1", "d2", "n_p")
+
+
+def _ptr(a, ct):
+    return a.ctypes.data_as(ctypes.POINTER(ct))
+
+
+# --------------------------------------------------------------------------------------------
+# geometry (C)
+# --------------------------------------------------------------------------------------------
+def rot_from_quat(q) -> np.ndarray:
+    """R(q), q = (w, x, y, z) Hamilton, active body->world; no renormalisation (reading A4)."""
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    R = np.empty(9, dtype=np.float64)
+    _lib().osog_oracle_rot_from_quat(_ptr(q, ctypes.c_double), _ptr(R, ctypes.c_double))
+    return R.reshape(3, 3)
+
+
+def prism_planes(s, L, hc):
+    """Body-frame (A[12,3], b[12]) of the capped tetragonal prism, Eq. 1 form A x <= b."""
+    A = np.zeros((16, 3), dtype=np.float64)
+    b = np.zeros(16, dtype=np.float64)
+    m = _lib().osog_oracle_prism_planes(float(s), float(L), float(hc), _ptr(A, ctypes.c_double), _ptr(b, ctypes.c_double))
+    return A[:m].copy(), b[:m].copy()
+
+
+def thickness(kind, q, dims, dx, dy, f32=False) -> float:
+    """Chord length along z of one particle at offset (dx, dy) from its centre.  With f32=True q and dims
+    are first rounded to float32, as the renderer sees them (the scene is float32)."""
+    q = np.asarray(q, dtype=np.float64)
+    d = np.asarray(dims, dtype=np.float64)
+    if f32:
+        q = q.astype(np.float32).astype(np.float64)
+        d = d.astype(np.float32).astype(np.float64)
+    q = np.ascontiguousarray(q)
+    d = np.ascontiguousarray(d)
+    return _lib().osog_oracle_thickness(int(kind), _ptr(q, ctypes.c_double), _ptr(d, ctypes.c_double),
+                                        float(dx), float(dy))
+
+
+def circumradius(kind, dims) -> float:
+    d = np.asarray(dims, dtype=np.float32)
+    return _lib().osog_oracle_circumradius(int(kind), float(d[0]), float(d[1]), float(d[2]))
+
+
+def render_opd_frame(cols, lo, hi, H, W, pitch, n_medium, mode="bcircle") -> np.ndarray:
+    """OPD [H, W] float64 of particles lo..hi-1 of the SoA `cols` (dict of float32 arrays + kind)."""
+    out = np.empty((H, W), dtype=np.float64)
+    arrs = [np.ascontiguousarray(cols[k][lo:hi], dtype=np.float32) for k in _COLS]
+    kind = np.ascontiguousarray(cols["kind"][lo:hi], dtype=np.uint8)
+    a = {k: v for k, v in zip(_COLS, arrs)}
+    f = ctypes.c_float
+    _lib().osog_oracle_render_opd(
+        hi - lo, _ptr(a["cx"], f), _ptr(a["cy"], f), _ptr(a["qw"], f), _ptr(a["qx"], f), _ptr(a["qy"], f),
+        _ptr(a["qz"], f), _ptr(a["d0"], f), _ptr(a["d1"], f), _ptr(a["d2"], f), _ptr(a["n_p"], f),
+        _ptr(kind, ctypes.c_uint8), H, W, float(pitch), float(n_medium),
+        {"full": 0, "bcircle": 1}[mode], _ptr(out, ctypes.c_double))
+    return out
+
+
+def render_opd(scene, mode="bcircle") -> np.ndarray:
+    """OPD [B, H, W] float64 for a workloads.Scene."""
+    fs = scene.frame_start
+    return np.stack([render_opd_frame(scene.cols, int(fs[b]), int(fs[b + 1]), scene.H, scene.W,
+                                      scene.pitch_um, scene.n_medium, mode) for b in range(scene.B)])
+
+
+# --------------------------------------------------------------------------------------------
+# optics (numpy, float64 / complex128)
+# --------------------------------------------------------------------------------------------
+def field(opd, lam, pitch, tilt_x=0.0, tilt_y=0.0) -> np.ndarray:
+    """Exit wave of Eq. 2 with A == 1 and phase sign +i, times the oblique-illumination ramp
+    exp(i 2 pi (fx0 x + fy0 y)), fx0 = sin(tilt_x)/lambda (reading A11), at pixel centres."""
+    H, W = opd.shape
+    x = (np.arange(W, dtype=np.float64) + 0.5) * pitch
+    y = (np.arange(H, dtype=np.float64) + 0.5) * pitch
+    fx0 = math.sin(tilt_x) / lam
+    fy0 = math.sin(tilt_y) / lam
+    turns = opd / lam + fx0 * x[None, :] + fy0 * y[:, None]
+    return np.exp(2j * np.pi * turns)
+
+
+def pupil_threshold(H, W, NA, pitch, lam) -> int:
+    """floor((NA p / lambda)^2 H^2 W^2): bin (my, mx) passes iff mx^2 H^2 + my^2 W^2 <= this (A10)."""
+    r = NA * pitch / lam
+    return int(math.floor(r * r * (float(H) * H) * (float(W) * W)))
+
+
+def pupil_mask(H, W, NA, pitch, lam) -> np.ndarray:
+    """circ(|k|/k_NA) of Eq. 3 on the FFT grid: spatial frequency of bin m is m/(W p) with m the signed
+    FFT index; inclusive edge; cutoff NA/lambda; compared in 64-bit integers."""
+    mx = np.fft.fftfreq(W, d=1.0 / W).round().astype(np.int64)
+    my = np.fft.fftfreq(H, d=1.0 / H).round().astype(np.int64)
+    lhs = (mx * mx)[None, :] * (H * H) + (my * my)[:, None] * (W * W)
+    return lhs <= pupil_threshold(H, W, NA, pitch, lam)
+
+
+def coherent_image(U, mask=None) -> np.ndarray:
+    """U * h_obj, h_obj = F^-1{P}: forward FFT, multiply by the pupil, inverse FFT
+    (normalised so that an all-pass pupil returns U)."""
+    F = np.fft.fft2(U)
+    if mask is not None:
+        F = F * mask
+    return np.fft.ifft2(F)
+
+
+def intensity(U, mask=None) -> np.ndarray:
+    """I_BF = |U * h_obj|^2."""
+    V = coherent_image(U, mask)
+    return V.real * V.real + V.imag * V.imag
+
+
+# --------------------------------------------------------------------------------------------
+# Philox4x32-10 and Gaussian read noise
+# --------------------------------------------------------------------------------------------
+_PHILOX_M0 = np.uint64(0xD2511F53)
+_PHILOX_M1 = np.uint64(0xCD9E8D57)
+_PHILOX_W0 = 0x9E3779B9
+_PHILOX_W1 = 0xBB67AE85
+_MASK32 = np.uint64(0xFFFFFFFF)
+
+
+def philox4x32_10(counter, key) -> np.ndarray:
+    """Philox-4x32 with 10 rounds (Salmon, Moraes, Dror, Shaw, SC'11).  counter: uint32 [..., 4],
+    key: (k0, k1).  One round maps (c0, c1, c2, c3) to (hi(M1 c2) ^ c1 ^ k0, lo(M1 c2),
+    hi(M0 c0) ^ c3 ^ k1, lo(M0 c0)); the key is bumped by the Weyl constants between rounds."""
+    c = np.asarray(counter, dtype=np.uint64) & _MASK32
+    c0, c1, c2, c3 = (c[..., k].copy() for k in range(4))
+    k0 = int(key[0]) & 0xFFFFFFFF
+    k1 = int(key[1]) & 0xFFFFFFFF
+    for _ in range(10):
+        p0 = _PHILOX_M0 * c0
+        p1 = _PHILOX_M1 * c2
+        n0 = (p1 >> np.uint64(32)) ^ c1 ^ np.uint64(k0)
+        n1 = p1 & _MASK32
+        n2 = (p0 >> np.uint64(32)) ^ c3 ^ np.uint64(k1)
+        n3 = p0 & _MASK32
+        c0, c1, c2, c3 = n0, n1, n2, n3
+        k0 = (k0 + _PHILOX_W0) & 0xFFFFFFFF
+        k1 = (k1 + _PHILOX_W1) & 0xFFFFFFFF
+    return np.stack([c0, c1, c2, c3], axis=-1).astype(np.uint32)
+
+
+def read_noise(seed, frame, H, W) -> np.ndarray:
+    """Standard normal z[i, j] for one frame (reading A13): Philox key = (seed low 32, seed high 32),
+    counter = (pixel = i W + j, frame, 0, 0); u1 = (r0 + 1) 2^-32 in (0, 1], u2 = r1 2^-32 in [0, 1);
+    z = sqrt(-2 ln u1) cos(2 pi u2) (Box-Muller)."""
+    pix = np.arange(H * W, dtype=np.uint64)
+    ctr = np.zeros((H * W, 4), dtype=np.uint64)
+    ctr[:, 0] = pix
+    ctr[:, 1] = np.uint64(frame)
+    r = philox4x32_10(ctr, (seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF))
+    u1 = (r[:, 0].astype(np.float64) + 1.0) * 2.0 ** -32
+    u2 = r[:, 1].astype(np.float64) * 2.0 ** -32
+    z = np.sqrt(-2.0 * np.log(u1)) * np.cos(2.0 * np.pi * u2)
+    return z.reshape(H, W)
+
+
+# --------------------------------------------------------------------------------------------
+# whole path for a Scene
+# --------------------------------------------------------------------------------------------
+def render_field(scene, opd=None, mode="bcircle") -> np.ndarray:
+    """complex128 [B, H, W]."""
+    if opd is None:
+        opd = render_opd(scene, mode)
+    return np.stack([field(opd[b], float(scene.lambda_um[b]), scene.pitch_um, scene.tilt_x_rad, scene.tilt_y_rad)
+                     for b in range(scene.B)])
+
+
+def render_intensity(scene, U=None, pupil_enabled=True, mode="bcircle") -> np.ndarray:
+    """float64 [B, H, W]: |coherent image|^2 + sigma * z."""
+    if U is None:
+        U = render_field(scene, mode=mode)
+    out = []
+    for b in range(scene.B):
+        mask = pupil_mask(scene.H, scene.W, float(scene.NA[b]), scene.pitch_um, float(scene.lambda_um[b])) \
+            if pupil_enabled else None
+        I = intensity(U[b], mask)
+        if scene.read_noise_sigma != 0.0:
+            I = I + scene.read_noise_sigma * read_noise(scene.seed, b, scene.H, scene.W)
+        out.append(I)
+    return np.stack(out)
+
+
+# --------------------------------------------------------------------------------------------
+# binning (float64 -> integers), B1-B4
+# --------------------------------------------------------------------------------------------
+BBOX_PAD_PX = 2.0 ** -10
+
+
+def _rot_all(cols):
+    w, x, y, z = (cols[k].astype(np.float64) for k in ("qw", "qx", "qy", "qz"))
+    R = np.empty((w.size, 3, 3), dtype=np.float64)
+    R[:, 0, 0] = 1.0 - 2.0 * (y * y + z * z); R[:, 0, 1] = 2.0 * (x * y - w * z); R[:, 0, 2] = 2.0 * (x * z + w * y)
+    R[:, 1, 0] = 2.0 * (x * y + w * z); R[:, 1, 1] = 1.0 - 2.0 * (x * x + z * z); R[:, 1, 2] = 2.0 * (y * z - w * x)
+    R[:, 2, 0] = 2.0 * (x * z - w * y); R[:, 2, 1] = 2.0 * (y * z + w * x); R[:, 2, 2] = 1.0 - 2.0 * (x * x + y * y)
+    return R
+
+
+def particle_valid(cols) -> np.ndarray:
+    ok = np.ones(cols["cx"].shape[0], dtype=bool)
+    for k in _COLS:
+        ok &= np.isfinite(cols[k])
+    for k in ("d0", "d1", "d2"):
+        ok &= cols[k] > 0
+    ok &= cols["kind"] <= 1
+    return ok
+
+
+def half_extents(cols):
+    """B1: half-extent of the body's projection along world x and y.
+    Ellipsoid: hx = sqrt(R_x0^2 a^2 + R_x1^2 b^2 + R_x2^2 c^2); prism: max over the 10 vertices
+    (+-s/2, +-s/2, +-L/2), (0, 0, +-(L/2 + hc)) of |(R v)_x|; same with row y."""
+    R = _rot_all(cols)
+    d0, d1, d2 = (cols[k].astype(np.float64) for k in ("d0", "d1", "d2"))
+    dims = np.stack([d0, d1, d2], axis=1)
+    he = np.sqrt(((R[:, 0:2, :] * dims[:, None, :]) ** 2).sum(axis=2))          # [N, 2]
+    s, L, hc = d0, d1, d2
+    verts = []
+    for sx in (1.0, -1.0):
+        for sy in (1.0, -1.0):
+            for sz in (1.0, -1.0):
+                verts.append(np.stack([sx * 0.5 * s, sy * 0.5 * s, sz * 0.5 * L], axis=1))
+    for sz in (1.0, -1.0):
+        verts.append(np.stack([0.0 * s, 0.0 * s, sz * (0.5 * L + hc)], axis=1))
+    V = np.stack(verts, axis=1)                                                   # [N, 10, 3]
+    RV = np.einsum("nrc,nvc->nvr", R, V)                                          # [N, 10, 3]
+    hp = np.abs(RV[:, :, 0:2]).max(axis=1)                                        # [N, 2]
+    isp = (cols["kind"] == 1)[:, None]
+    h = np.where(isp, hp, he)
+    return h[:, 0], h[:, 1]
+
+
+def bboxes(cols, H, W, pitch):
+    """B2: inclusive pixel range whose centres can lie inside the projection, padded by 2^-10 px,
+    clamped to the frame.  Returns int64 arrays j0, j1, i0, i1 and a bool `listed` (valid and not empty)."""
+    with np.errstate(invalid="ignore", over="ignore"):
+        hx, hy = half_extents(cols)
+        cx = cols["cx"].astype(np.float64)
+        cy = cols["cy"].astype(np.float64)
+        ok = particle_valid(cols)
+        fj0 = np.ceil((cx - hx) / pitch - 0.5 - BBOX_PAD_PX)
+        fj1 = np.floor((cx + hx) / pitch - 0.5 + BBOX_PAD_PX)
+        fi0 = np.ceil((cy - hy) / pitch - 0.5 - BBOX_PAD_PX)
+        fi1 = np.floor((cy + hy) / pitch - 0.5 + BBOX_PAD_PX)
+        ok &= np.isfinite(fj0) & np.isfinite(fj1) & np.isfinite(fi0) & np.isfinite(fi1)
+    big = 2.0 ** 30
+    def clampi(f, lo, hi):
+        f = np.where(ok, np.clip(f, -big, big), 0.0)
+        return np.clip(f.astype(np.int64), lo, hi)
+    j0 = clampi(fj0, 0, W); j1 = clampi(fj1, -1, W - 1)
+    i0 = clampi(fi0, 0, H); i1 = clampi(fi1, -1, H - 1)
+    listed = ok & (j0 <= j1) & (i0 <= i1)
+    return j0, j1, i0, i1, listed
+
+
+def binning(scene, T):
+    """B3-B4 for a Scene: tiles of T x T pixels, row-major per frame, frames concatenated
+    (global tile id = frame * tiles_per_frame + ty * ceil(W/T) + tx).  A particle is listed in every
+    tile its bounding box touches.  Returns (count uint32 [n_tiles], offset uint32 [n_tiles + 1],
+    list uint32 [pairs]) with each tile's segment in ascending GLOBAL particle index."""
+    H, W, B = scene.H, scene.W, scene.B
+    ntx = -(-W // T)
+    nty = -(-H // T)
+    tpf = ntx * nty
+    j0, j1, i0, i1, listed = bboxes(scene.cols, H, W, scene.pitch_um)
+    fs = scene.frame_start
+    frame_of = np.repeat(np.arange(B), np.diff(fs))
+    count = np.zeros(B * tpf, dtype=np.int64)
+    pairs_t = []
+    pairs_n = []
+    for n in np.nonzero(listed)[0]:
+        tx = np.arange(j0[n] // T, j1[n] // T + 1)
+        ty = np.arange(i0[n] // T, i1[n] // T + 1)
+        t = (frame_of[n] * tpf + ty[:, None] * ntx + tx[None, :]).ravel()
+        count[t] += 1
+        pairs_t.append(t)
+        pairs_n.append(np.full(t.size, n, dtype=np.int64))
+    offset = np.zeros(B * tpf + 1, dtype=np.int64)
+    np.cumsum(count, out=offset[1:])
+    if pairs_t:
+        pt = np.concatenate(pairs_t)
+        pn = np.concatenate(pairs_n)
+        order = np.lexsort((pn, pt))          # by tile, then ascending particle index
+        lst = pn[order]
+    else:
+        lst = np.zeros(0, dtype=np.int64)
+    return count.astype(np.uint32), offset.astype(np.uint32), lst.astype(np.uint32)

@@ -1,0 +1,192 @@
+/*
+ * OSOG forward-render ORACLE (test infrastructure, NOT the product).
+ *
+ * Plain, slow, float64 CPU restatement of what the hot path computes, written from the paper
+ * and the readings listed in DESIGN.md section 3.  It shares no code,
+ * header, table or helper with the CUDA path under paper_2606_21381_b200/csrc and is imported only
+ * by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs.
+ *
+ * What is computed (per frame, pixel (i,j) = row i, column j, centre x=(j+1/2)p, y=(i+1/2)p):
+ *
+ *   OPD[i,j] = sum over particles n, ascending n, of (n_p[n] - n_medium) * thickness_n(x-cx, y-cy)
+ *
+ * - the integrand of Eq. 2 ("integral of [n_p(z) - n_m] dz") for piecewise-constant
+ *   n_p, summed over particles as Eq. 7's accumulate=True does.  Off-canvas
+ *   pixels are simply not part of the frame ("strict boolean masking").
+ *
+ * thickness_n(dx,dy) = length of the intersection of the vertical line (dx,dy,.) with the body:
+ *   kind 0  ellipsoid  { q : q^T M q <= 1 },  M = R diag(1/a^2,1/b^2,1/c^2) R^T   (not in the paper:
+ *           BASELINE.json north_star, "ellipsoid quadratic"); solved as a quadratic in z.
+ *   kind 1  capped tetragonal prism = intersection of 12 half-spaces  A x <= b  (Eq. 1),
+ *           evaluated by the generic loop over planes: enter = max over planes with n_z<0 of g/n_z,
+ *           exit = min over planes with n_z>0 of g/n_z, g = b - n_x dx - n_y dy; a plane with n_z==0
+ *           empties the line when g<0.
+ *
+ * Precision: float64 throughout; the float32 inputs are promoted exactly.  No tiling, no bounding
+ * boxes; `mode` 1 ("bcircle") skips pixels farther from the centre than the body's circumradius,
+ * which is trivially conservative and is shown bit-identical to mode 0 ("full") by the tests.
+ *
+ * Pins (tests/test_oracle_*.py, run with -m "not gpu"): sphere closed form, axis-aligned ellipsoid,
+ * Schur-complement projection, prism closed forms, volume invariance, vertex/plane consistency,
+ * permutation invariance, integer translation, supersampled ray marching by inside-test only.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#define OSOG_ORACLE_MAX_PLANES 16
+
+/* Hamilton unit quaternion (w,x,y,z) -> active rotation matrix body->world, row-major R[3*r+c].
+ * No renormalisation (reading A4). */
+void osog_oracle_rot_from_quat(const double q[4], double R[9])
+{
+    const double w = q[0], x = q[1], y = q[2], z = q[3];
+    R[0] = 1.0 - 2.0 * (y * y + z * z); R[1] = 2.0 * (x * y - w * z);       R[2] = 2.0 * (x * z + w * y);
+    R[3] = 2.0 * (x * y + w * z);       R[4] = 1.0 - 2.0 * (x * x + z * z); R[5] = 2.0 * (y * z - w * x);
+    R[6] = 2.0 * (x * z - w * y);       R[7] = 2.0 * (y * z + w * x);       R[8] = 1.0 - 2.0 * (x * x + y * y);
+}
+
+/* Ellipsoid: points q with q^T M q <= 1, M = R D R^T, D = diag(1/a^2, 1/b^2, 1/c^2).
+ * On the line q = (dx, dy, z):  A z^2 + 2 Bq z + C <= 0  with
+ *   A = M_zz,  Bq = M_xz dx + M_yz dy,  C = M_xx dx^2 + 2 M_xy dx dy + M_yy dy^2 - 1,
+ * so the chord length is 2 sqrt(Bq^2 - A C) / A when the discriminant is positive, else 0. */
+double osog_oracle_thickness_ellipsoid(const double R[9], double a, double b, double c,
+                                       double dx, double dy)
+{
+    const double D[3] = { 1.0 / (a * a), 1.0 / (b * b), 1.0 / (c * c) };
+    double M[9];
+    for (int r = 0; r < 3; ++r)
+        for (int s = 0; s < 3; ++s) {
+            double acc = 0.0;
+            for (int k = 0; k < 3; ++k) acc += R[3 * r + k] * D[k] * R[3 * s + k];
+            M[3 * r + s] = acc;
+        }
+    const double A  = M[8];
+    const double Bq = M[2] * dx + M[5] * dy;
+    const double C  = M[0] * dx * dx + 2.0 * M[1] * dx * dy + M[4] * dy * dy - 1.0;
+    const double disc = Bq * Bq - A * C;
+    return disc > 0.0 ? 2.0 * sqrt(disc) / A : 0.0;
+}
+
+/* Body-frame half-spaces of the capped tetragonal prism (reading A5/A6): square
+ * cross-section of side s in body x,y; prismatic part |z| <= L/2; a four-sided pyramid of height hc
+ * on each end with apex (0,0,+-(L/2+hc)).  12 planes, un-normalised normals:
+ *   +-(1,0,0), +-(0,1,0)                      with b = s/2
+ *   (+-hc, 0, +-s/2), (0, +-hc, +-s/2)        with b = hc*s/2 + s*L/4     (all sign choices)
+ * Returns the number of planes (12). */
+int osog_oracle_prism_planes(double s, double L, double hc, double A[][3], double b[])
+{
+    int m = 0;
+    const double sgn[2] = { 1.0, -1.0 };
+    for (int k = 0; k < 2; ++k) { A[m][0] = sgn[k]; A[m][1] = 0.0; A[m][2] = 0.0; b[m] = 0.5 * s; ++m; }
+    for (int k = 0; k < 2; ++k) { A[m][0] = 0.0; A[m][1] = sgn[k]; A[m][2] = 0.0; b[m] = 0.5 * s; ++m; }
+    const double bc = hc * s * 0.5 + s * L * 0.25;
+    for (int kz = 0; kz < 2; ++kz)
+        for (int kx = 0; kx < 2; ++kx) { A[m][0] = sgn[kx] * hc; A[m][1] = 0.0; A[m][2] = sgn[kz] * 0.5 * s; b[m] = bc; ++m; }
+    for (int kz = 0; kz < 2; ++kz)
+        for (int ky = 0; ky < 2; ++ky) { A[m][0] = 0.0; A[m][1] = sgn[ky] * hc; A[m][2] = sgn[kz] * 0.5 * s; b[m] = bc; ++m; }
+    return m;
+}
+
+/* Eq. 1: P = { x | A x <= b }, planes given in WORLD axes relative to the centre.
+ * Length of { z : A (dx,dy,z) <= b }. */
+double osog_oracle_thickness_polyhedron(int M, const double A[][3], const double b[],
+                                        double dx, double dy)
+{
+    double enter = -INFINITY, exit_ = INFINITY;
+    for (int k = 0; k < M; ++k) {
+        const double g = b[k] - A[k][0] * dx - A[k][1] * dy;
+        const double nz = A[k][2];
+        if (nz > 0.0)      { const double z = g / nz; if (z < exit_) exit_ = z; }
+        else if (nz < 0.0) { const double z = g / nz; if (z > enter) enter = z; }
+        else if (g < 0.0)  return 0.0;
+    }
+    const double t = exit_ - enter;
+    return t > 0.0 ? t : 0.0;
+}
+
+/* World-frame planes of prism n: normal R n_hat, same offset b. */
+static int prism_world_planes(const double R[9], double s, double L, double hc,
+                              double Aw[][3], double b[])
+{
+    double Ab[OSOG_ORACLE_MAX_PLANES][3];
+    const int M = osog_oracle_prism_planes(s, L, hc, Ab, b);
+    for (int k = 0; k < M; ++k)
+        for (int r = 0; r < 3; ++r)
+            Aw[k][r] = R[3 * r + 0] * Ab[k][0] + R[3 * r + 1] * Ab[k][1] + R[3 * r + 2] * Ab[k][2];
+    return M;
+}
+
+/* A particle takes part iff every parameter is finite and all three dimensions are positive
+ * (error behaviour: others are skipped). */
+int osog_oracle_particle_valid(float cx, float cy, float qw, float qx, float qy, float qz,
+                               float d0, float d1, float d2, float n_p, uint8_t kind)
+{
+    const double v[10] = { cx, cy, qw, qx, qy, qz, d0, d1, d2, n_p };
+    for (int k = 0; k < 10; ++k) if (!isfinite(v[k])) return 0;
+    if (!(d0 > 0.0f) || !(d1 > 0.0f) || !(d2 > 0.0f)) return 0;
+    return kind <= 1;
+}
+
+/* Thickness of one particle at offset (dx,dy) from its centre; q = (w,x,y,z), dims = (d0,d1,d2). */
+double osog_oracle_thickness(uint8_t kind, const double q[4], const double dims[3], double dx, double dy)
+{
+    double R[9];
+    osog_oracle_rot_from_quat(q, R);
+    if (kind == 0) return osog_oracle_thickness_ellipsoid(R, dims[0], dims[1], dims[2], dx, dy);
+    double Aw[OSOG_ORACLE_MAX_PLANES][3], b[OSOG_ORACLE_MAX_PLANES];
+    const int M = prism_world_planes(R, dims[0], dims[1], dims[2], Aw, b);
+    return osog_oracle_thickness_polyhedron(M, Aw, b, dx, dy);
+}
+
+/* Circumradius of the body (largest distance of any of its points from the centre):
+ * ellipsoid: largest semi-axis; prism: largest vertex norm over (+-s/2,+-s/2,+-L/2), (0,0,+-(L/2+hc)). */
+double osog_oracle_circumradius(uint8_t kind, float d0, float d1, float d2)
+{
+    if (kind == 0) return fmax((double)d0, fmax((double)d1, (double)d2));
+    const double s = d0, L = d1, hc = d2;
+    return fmax(sqrt(0.5 * s * s + 0.25 * L * L), 0.5 * L + hc);
+}
+
+/* One frame of OPD.  Particle arrays hold this frame's N particles.  mode 0 = full, 1 = bcircle.
+ * opd is row-major [H*W], overwritten.  Rows are split over OpenMP threads; for each pixel the
+ * particle loop runs in ascending index, so the summation order is fixed. */
+void osog_oracle_render_opd(int64_t N,
+                            const float *cx, const float *cy,
+                            const float *qw, const float *qx, const float *qy, const float *qz,
+                            const float *d0, const float *d1, const float *d2,
+                            const float *n_p, const uint8_t *kind,
+                            int H, int W, double pitch, double n_medium, int mode, double *opd)
+{
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int i = 0; i < H; ++i) {
+        const double y = (i + 0.5) * pitch;
+        for (int j = 0; j < W; ++j) opd[(size_t)i * W + j] = 0.0;
+        for (int64_t n = 0; n < N; ++n) {
+            if (!osog_oracle_particle_valid(cx[n], cy[n], qw[n], qx[n], qy[n], qz[n],
+                                            d0[n], d1[n], d2[n], n_p[n], kind[n])) continue;
+            const double dy = y - (double)cy[n];
+            const double dn = (double)n_p[n] - n_medium;
+            const double q[4] = { qw[n], qx[n], qy[n], qz[n] };
+            double R[9];
+            osog_oracle_rot_from_quat(q, R);
+            double Aw[OSOG_ORACLE_MAX_PLANES][3], b[OSOG_ORACLE_MAX_PLANES];
+            int M = 0;
+            if (kind[n] == 1) M = prism_world_planes(R, d0[n], d1[n], d2[n], Aw, b);
+            double r2 = INFINITY;
+            if (mode == 1) {
+                const double r = osog_oracle_circumradius(kind[n], d0[n], d1[n], d2[n]) * (1.0 + 1e-9);
+                r2 = r * r;
+                if (dy * dy > r2) continue;
+            }
+            for (int j = 0; j < W; ++j) {
+                const double dx = (j + 0.5) * pitch - (double)cx[n];
+                if (dx * dx + dy * dy > r2) continue;
+                const double t = kind[n] == 0
+                    ? osog_oracle_thickness_ellipsoid(R, d0[n], d1[n], d2[n], dx, dy)
+                    : osog_oracle_thickness_polyhedron(M, Aw, b, dx, dy);
+                opd[(size_t)i * W + j] += dn * t;
+            }
+        }
+    }
+}
