@@ -1,0 +1,141 @@
+/*
+ * osog.h - C ABI of the B200-native OSOG forward-render hot path.
+ *
+ * What the library computes (citations: /root/reference/PAPER.md line numbers; readings A1-A19 and the
+ * binning spec B1-B4 are listed in DESIGN.md section 3):
+ *
+ *   For every frame b and pixel (i, j) (row i, column j, centre x = (j + 1/2) p, y = (i + 1/2) p):
+ *     OPD[b,i,j] = sum over the frame's particles n, ascending n, of (n_p[n] - n_medium) * thickness_n(x - cx, y - cy)
+ *                  - the integrand of Eq. 2 accumulated as Eq. 7 does;
+ *                  thickness = chord of the vertical line through the convex body: ellipsoid quadric, or the
+ *                  half-space intersection {x | A x <= b} of Eq. 1 for the capped tetragonal prism.
+ *     U[b,i,j]   = exp(i 2 pi (OPD / lambda_b + fx0 x + fy0 y)),  fx0 = sin(tilt_x) / lambda_b   (Eq. 2 with A == 1,
+ *                  oblique illumination as a phase ramp)
+ *     I[b]       = | IFFT2( FFT2(U[b]) * circ(|k| / (NA_b / lambda_b)) ) |^2  (+ sigma * z[b,i,j])
+ *                  (Eq. 3 with delta z = 0; I_BF; Gaussian read noise)
+ *
+ * Conventions
+ *   - One context per (device, stream).  Every render call ENQUEUES work on the context's stream and returns
+ *     without synchronising; outputs are valid once the caller has synchronised that stream.
+ *   - All particle arrays and all output buffers are DEVICE pointers, caller-owned, 16-byte aligned.  The
+ *     library reads the inputs, OVERWRITES the whole output (never accumulates into it) and owns only its own
+ *     scratch, allocated in osog_create and freed in osog_destroy.  No allocation happens in a render call.
+ *   - Results are bitwise reproducible from run to run: every pixel sums its particles in ascending index.
+ *   - There is no CPU fallback and no backend dispatch: without a CUDA device osog_create fails.
+ *   - Return value: 0 = OK, negative = error (see the enum).  Nothing is printed, nothing throws or aborts.
+ *   - Particles with a non-finite parameter, a non-positive dimension or kind > 1 are skipped (they join no
+ *     tile) and set the OSOG_WBADPARTICLE bit reported by osog_status.
+ */
+#ifndef OSOG_H_
+#define OSOG_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define OSOG_API_VERSION 1
+
+enum {
+    OSOG_OK = 0,
+    OSOG_EINVAL = -1,     /* null / misaligned pointer, bad size, N > max_particles, B > max_frames, bad optics */
+    OSOG_ECUDA = -2,      /* CUDA runtime, launch or cuFFT failure (osog_last_cuda_error gives the code)       */
+    OSOG_ECAPACITY = -3,  /* (particle, tile) pair list overflow: the frames of that call are zero-filled       */
+    OSOG_ENOMEM = -4      /* allocation failure in osog_create                                                 */
+};
+/* status bits returned by osog_status (sticky until the next render call) */
+#define OSOG_WBADPARTICLE 1u   /* at least one particle was skipped as invalid                    */
+#define OSOG_WOVERFLOW    2u   /* pair list overflow happened on the device (see OSOG_ECAPACITY) */
+
+typedef struct osog_ctx osog_ctx;   /* opaque: scratch buffers, tables, cuFFT plans */
+
+/* Sizes fixed at creation.  struct_size = sizeof(osog_config) (ABI check). */
+typedef struct {
+    uint32_t struct_size;
+    int32_t  device;         /* CUDA device ordinal                                                        */
+    void*    stream;         /* cudaStream_t the context enqueues on (0 = legacy default stream)           */
+    int32_t  H, W;           /* frame height / width in pixels, 1 .. 32768; need not be tile multiples     */
+    int32_t  max_frames;     /* largest batch B of one call, >= 1                                          */
+    int64_t  max_particles;  /* largest N (total over the batch) of one call, >= 0                         */
+    int64_t  max_pairs;      /* capacity of the (particle, tile) pair list; 0 = 64 * max_particles + 1024  */
+} osog_config;
+
+/* Particle state, Structure of Arrays ("S in R^{N x D}"): one DEVICE array of length N per
+ * column, const, caller-owned.  Frame b owns particles frame_start[b] .. frame_start[b+1]-1. */
+typedef struct {
+    uint32_t struct_size;
+    const float *cx, *cy, *cz;        /* centre, um; cz is accepted and unused (projection along z); may be NULL */
+    const float *qw, *qx, *qy, *qz;   /* unit quaternion (w, x, y, z), Hamilton, active body -> world, not renormalised */
+    const float *d0, *d1, *d2;        /* kind 0: semi-axes a, b, c;  kind 1: side s, length L, cap height hc (um) */
+    const float *n_p;                 /* refractive index of the particle                                    */
+    const uint8_t *kind;              /* 0 = ellipsoid (sphere = equal axes), 1 = capped tetragonal prism    */
+    const int32_t *frame_start;       /* DEVICE int32 [B + 1], ascending, [0] = 0, [B] = N; NULL iff B == 1 */
+} osog_particles;
+
+/* Optics of one call.  lambda_um and NA are HOST arrays of length B (read before the call returns). */
+typedef struct {
+    uint32_t struct_size;
+    int32_t  B;                       /* frames in this call, 1 .. max_frames                                */
+    double   pitch_um;                /* pixel pitch p > 0                                                    */
+    double   n_medium;                /* refractive index of the medium                                       */
+    const double *lambda_um;          /* [B] vacuum wavelength > 0                                            */
+    const double *NA;                 /* [B] numerical aperture > 0 (used by osog_render_intensity only)      */
+    double   tilt_x_rad, tilt_y_rad;  /* oblique illumination: phase ramp exp(i 2 pi sin(tilt)/lambda * x); 0 = none */
+    double   read_noise_sigma;        /* intensity only: I += sigma * z, z ~ N(0,1) Philox4x32-10 keyed (seed, frame, pixel); 0 = none */
+    uint64_t seed;
+    int32_t  pupil_enabled;           /* 0 = all-pass pupil (Parseval check), else circ(NA / lambda)          */
+} osog_optics;
+
+/* Create a context: allocates all scratch (records, bounding boxes, tile counts / offsets / lists, ramp
+ * tables, one complex frame batch and the cuFFT plans).  *out is set to NULL on failure. */
+int osog_create(osog_ctx** out, const osog_config* cfg);
+
+/* OPD frame(s): d_opd is DEVICE float [B, H, W], row-major, micrometres.  Steps H1-H6 of DESIGN.md:
+ * prepare + bounding box + tile count, scan, fill, per-tile ordered composition. */
+int osog_render_opd(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd);
+
+/* Complex exit wave: d_field is DEVICE float [B, H, W, 2] (interleaved re, im = complex64).  Same steps as
+ * osog_render_opd with the phase-to-complex conversion and the ramp fused into the tile write-out (H7). */
+int osog_render_field(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_field);
+
+/* Coherent intensity through the circular pupil: d_intensity is DEVICE float [B, H, W].  Runs the hot path
+ * into the context's own complex frame, then the library stage: cuFFT forward, pupil mask (integer
+ * comparison m_x^2 H^2 + m_y^2 W^2 <= floor((NA p / lambda)^2 H^2 W^2)) and 1/(HW), cuFFT inverse, |.|^2,
+ * optional read noise. */
+int osog_render_intensity(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_intensity);
+
+/* Library stage alone on a caller-supplied field (DEVICE complex64 [B, H, W], left untouched): used to time
+ * the cuFFT stage separately from the hot path. */
+int osog_field_to_intensity(osog_ctx* ctx, const osog_optics* o, const float* d_field, float* d_intensity);
+
+/* Measured alternative to the ordered tile composition (paper-style scatter-add): one warp
+ * per particle, global atomicAdd into d_opd.  NOT deterministic in the last bits; kept for comparison only. */
+int osog_render_opd_atomic(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd);
+
+int osog_destroy(osog_ctx* ctx);
+
+/* Synchronises the stream.  *status_bits = OSOG_W* bits of the last render call, *pairs = number of
+ * (particle, tile) pairs that call needed (compare with max_pairs).  Either pointer may be NULL.
+ * Returns OSOG_ECAPACITY if the last call overflowed, OSOG_ECUDA on a sticky CUDA error, else OSOG_OK. */
+int osog_status(osog_ctx* ctx, uint32_t* status_bits, int64_t* pairs);
+
+/* Test / diagnostics: synchronises, then copies the binning of the last render call to HOST arrays:
+ * h_offset [n_tiles + 1] (exclusive scan of the per-tile counts), h_list [min(pairs, cap)] (each tile's
+ * segment in ascending particle index).  Tile id = frame * tiles_per_frame + (i / T) * ceil(W / T) + (j / T).
+ * Any pointer may be NULL.  *n_tiles and *n_pairs are always written. */
+int osog_debug_bins(osog_ctx* ctx, uint32_t* h_offset, uint32_t* h_list, int64_t cap,
+                    int64_t* n_tiles, int64_t* n_pairs);
+
+/* Tile edge T in pixels (build-time constant of the binning, B3). */
+int osog_tile_size(void);
+
+/* Last CUDA / cuFFT error code seen by this context (0 = none). */
+int osog_last_cuda_error(const osog_ctx* ctx);
+
+const char* osog_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OSOG_H_ */

@@ -1,0 +1,234 @@
+"""Thin ctypes binding of libosog.so (include/osog.h).  Argument marshalling only: every step of the
+render path runs in the CUDA kernels of the library.  PyTorch supplies device memory and the stream.
+
+There is no CPU fallback: if libosog.so is missing and cannot be built, or no CUDA device is present,
+the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+OSOG_OK, OSOG_EINVAL, OSOG_ECUDA, OSOG_ECAPACITY, OSOG_ENOMEM = 0, -1, -2, -3, -4
+OSOG_WBADPARTICLE, OSOG_WOVERFLOW = 1, 2
+
+_F32_COLS = ("cx", "cy", "cz", "qw", "qx", "qy", "qz", "d0", "d1", "d2", "n_p")
+
+
+class osog_config(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("device", C.c_int32), ("stream", C.c_void_p),
+                ("H", C.c_int32), ("W", C.c_int32), ("max_frames", C.c_int32),
+                ("max_particles", C.c_int64), ("max_pairs", C.c_int64)]
+
+
+class osog_particles(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32)] + [(k, C.c_void_p) for k in _F32_COLS] + \
+               [("kind", C.c_void_p), ("frame_start", C.c_void_p)]
+
+
+class osog_optics(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("B", C.c_int32), ("pitch_um", C.c_double), ("n_medium", C.c_double),
+                ("lambda_um", C.POINTER(C.c_double)), ("NA", C.POINTER(C.c_double)),
+                ("tilt_x_rad", C.c_double), ("tilt_y_rad", C.c_double), ("read_noise_sigma", C.c_double),
+                ("seed", C.c_uint64), ("pupil_enabled", C.c_int32)]
+
+
+class OsogError(RuntimeError):
+    def __init__(self, code, what):
+        self.code = code
+        super().__init__(f"{what}: {lib().osog_strerror(code).decode()} ({code})")
+
+
+_LIB = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def lib():
+    """Load (building first if the sources are newer) libosog.so and declare every exported symbol."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = _build.LIB
+    if _build.needs_build():
+        path = _build.build()
+    L = C.CDLL(path)
+    ctx = C.c_void_p
+    L.osog_create.argtypes = [C.POINTER(ctx), C.POINTER(osog_config)]
+    for name in ("osog_render_opd", "osog_render_field", "osog_render_intensity", "osog_render_opd_atomic"):
+        getattr(L, name).argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p]
+    L.osog_field_to_intensity.argtypes = [ctx, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
+    L.osog_destroy.argtypes = [ctx]
+    L.osog_status.argtypes = [ctx, C.POINTER(C.c_uint32), C.POINTER(C.c_int64)]
+    L.osog_debug_bins.argtypes = [ctx, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    L.osog_tile_size.argtypes = []
+    L.osog_last_cuda_error.argtypes = [ctx]
+    L.osog_strerror.argtypes = [C.c_int]
+    L.osog_strerror.restype = C.c_char_p
+    for name in EXPORTS:
+        if name != "osog_strerror":
+            getattr(L, name).restype = C.c_int
+    _LIB = L
+    return L
+
+
+EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
+           "osog_field_to_intensity", "osog_render_opd_atomic", "osog_destroy", "osog_status",
+           "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
+
+
+def osog_tile_size() -> int:
+    return lib().osog_tile_size()
+
+
+class Particles:
+    """SoA particle state resident on the device (torch tensors), plus the osog_particles view of it."""
+
+    def __init__(self, cols: dict, frame_start=None, device="cuda:0"):
+        import torch
+        self.device = torch.device(device)
+        self.t = {}
+        for k in _F32_COLS:
+            if k in cols and cols[k] is not None:
+                self.t[k] = self._dev(cols[k], torch.float32)
+        self.t["kind"] = self._dev(cols["kind"], torch.uint8)
+        self.N = int(self.t["kind"].numel())
+        self.frame_start = None
+        if frame_start is not None:
+            self.frame_start = self._dev(np.asarray(frame_start, dtype=np.int32), torch.int32)
+        self.c = osog_particles()
+        self.c.struct_size = C.sizeof(osog_particles)
+        for k in _F32_COLS:
+            setattr(self.c, k, self.t[k].data_ptr() if k in self.t and self.N > 0 else None)
+        self.c.kind = self.t["kind"].data_ptr() if self.N > 0 else None
+        self.c.frame_start = self.frame_start.data_ptr() if self.frame_start is not None else None
+
+    def _dev(self, a, dtype):
+        import torch
+        if isinstance(a, torch.Tensor):
+            return a.to(device=self.device, dtype=dtype).contiguous()
+        return torch.from_numpy(np.ascontiguousarray(a)).to(dtype).to(self.device)
+
+    @classmethod
+    def from_scene(cls, scene, device="cuda:0"):
+        return cls(scene.cols, scene.frame_start if scene.B > 1 else None, device)
+
+
+def make_optics(B, pitch_um, n_medium, lambda_um, NA=None, tilt_x_rad=0.0, tilt_y_rad=0.0,
+                read_noise_sigma=0.0, seed=0, pupil_enabled=True):
+    """osog_optics plus the host arrays it points to (kept alive as attributes)."""
+    o = osog_optics()
+    o.struct_size = C.sizeof(osog_optics)
+    o.B = int(B)
+    o.pitch_um = float(pitch_um)
+    o.n_medium = float(n_medium)
+    lam = np.ascontiguousarray(np.broadcast_to(np.asarray(lambda_um, dtype=np.float64), (B,)))
+    o._lam = lam
+    o.lambda_um = lam.ctypes.data_as(C.POINTER(C.c_double))
+    if NA is not None:
+        na = np.ascontiguousarray(np.broadcast_to(np.asarray(NA, dtype=np.float64), (B,)))
+        o._na = na
+        o.NA = na.ctypes.data_as(C.POINTER(C.c_double))
+    o.tilt_x_rad = float(tilt_x_rad)
+    o.tilt_y_rad = float(tilt_y_rad)
+    o.read_noise_sigma = float(read_noise_sigma)
+    o.seed = int(seed) & 0xFFFFFFFFFFFFFFFF
+    o.pupil_enabled = 1 if pupil_enabled else 0
+    return o
+
+
+def optics_from_scene(scene, pupil_enabled=True):
+    return make_optics(scene.B, scene.pitch_um, scene.n_medium, scene.lambda_um, scene.NA, scene.tilt_x_rad,
+                       scene.tilt_y_rad, scene.read_noise_sigma, scene.seed, pupil_enabled)
+
+
+class Context:
+    """osog_ctx owner.  Methods mirror the C entry points and return torch tensors on the device."""
+
+    def __init__(self, H, W, max_particles, max_frames=1, max_pairs=0, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("osog: no CUDA device; this library has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.H, self.W, self.max_frames = int(H), int(W), int(max_frames)
+        cfg = osog_config()
+        cfg.struct_size = C.sizeof(osog_config)
+        cfg.device = self.device.index or 0
+        cfg.stream = self.stream.cuda_stream
+        cfg.H, cfg.W, cfg.max_frames = self.H, self.W, self.max_frames
+        cfg.max_particles = int(max_particles)
+        cfg.max_pairs = int(max_pairs)
+        self._ctx = C.c_void_p()
+        r = lib().osog_create(C.byref(self._ctx), C.byref(cfg))
+        if r != OSOG_OK:
+            self._ctx = None
+            raise OsogError(r, "osog_create")
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            lib().osog_destroy(self._ctx)
+            self._ctx = None
+
+    __del__ = close
+
+    def _out(self, B, *tail, out=None):
+        if out is not None:
+            return out
+        return self.torch.empty((B, self.H, self.W) + tail, dtype=self.torch.float32, device=self.device)
+
+    def _call(self, name, p, o, out):
+        r = getattr(lib(), name)(self._ctx, C.byref(p.c), p.N, C.byref(o), out.data_ptr())
+        if r != OSOG_OK:
+            raise OsogError(r, name)
+        return out
+
+    def render_opd(self, p: Particles, o, out=None):
+        """float32 [B, H, W] OPD in micrometres (osog_render_opd)."""
+        return self._call("osog_render_opd", p, o, self._out(o.B, out=out))
+
+    def render_opd_atomic(self, p: Particles, o, out=None):
+        return self._call("osog_render_opd_atomic", p, o, self._out(o.B, out=out))
+
+    def render_field(self, p: Particles, o, out=None):
+        """complex64 [B, H, W] exit wave (osog_render_field); `out` is a float32 [B, H, W, 2] buffer."""
+        buf = self._call("osog_render_field", p, o, self._out(o.B, 2, out=out))
+        return self.torch.view_as_complex(buf)
+
+    def render_intensity(self, p: Particles, o, out=None):
+        """float32 [B, H, W] coherent intensity (osog_render_intensity)."""
+        return self._call("osog_render_intensity", p, o, self._out(o.B, out=out))
+
+    def field_to_intensity(self, o, field, out=None):
+        out = self._out(o.B, out=out)
+        f = self.torch.view_as_real(field) if field.is_complex() else field
+        r = lib().osog_field_to_intensity(self._ctx, C.byref(o), f.data_ptr(), out.data_ptr())
+        if r != OSOG_OK:
+            raise OsogError(r, "osog_field_to_intensity")
+        return out
+
+    def status(self):
+        """(status bits, pairs needed) of the last render call; synchronises the stream."""
+        bits, pairs = C.c_uint32(0), C.c_int64(0)
+        r = lib().osog_status(self._ctx, C.byref(bits), C.byref(pairs))
+        return r, bits.value, pairs.value
+
+    def debug_bins(self):
+        """(count, offset, list) of the last render call as numpy uint32 arrays."""
+        nt, npairs = C.c_int64(0), C.c_int64(0)
+        r = lib().osog_debug_bins(self._ctx, None, None, 0, C.byref(nt), C.byref(npairs))
+        if r not in (OSOG_OK, OSOG_ECAPACITY):
+            raise OsogError(r, "osog_debug_bins")
+        offset = np.zeros(nt.value + 1, dtype=np.uint32)
+        lst = np.zeros(npairs.value, dtype=np.uint32)
+        r = lib().osog_debug_bins(self._ctx, offset.ctypes.data, lst.ctypes.data, lst.size, C.byref(nt), C.byref(npairs))
+        if r != OSOG_OK:
+            raise OsogError(r, "osog_debug_bins")
+        return np.diff(offset).astype(np.uint32), offset, lst

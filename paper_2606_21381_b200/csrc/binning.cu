@@ -1,0 +1,394 @@
+// H1-H4 of DESIGN.md: per-particle preparation (fp64), bounding box -> tile range -> per-tile count,
+// exclusive scan, fill of the per-tile particle lists.  Integer results must equal the oracle's binning
+// bit for bit (B1-B4); the canonical (ascending) order of each list is established by
+// the composition kernel, which sorts its own segment and writes it back (compose.cu).
+#include "osog_internal.cuh"
+
+namespace osog {
+
+struct PrepArgs {
+    const float *cx, *cy, *qw, *qx, *qy, *qz, *d0, *d1, *d2, *n_p;
+    const uint8_t* kind;
+    const int32_t* frame_start;   // device [B+1] or nullptr
+    long long N;
+    int B, H, W, ntx, nty;
+    double pitch, n_medium;
+    float* rec32;
+    double* rec64;
+    int4* tbox;
+    int* pframe;
+    uint32_t* count;
+    float2 *ramp_x, *ramp_y;
+    FrameOptics* optics;
+    DeviceStatus* status;
+    int has_ramp;
+    OpticsChunk oc;               // frames 0 .. min(B, kOpticsChunk)-1 by value
+};
+
+__device__ __forceinline__ bool finite_f(float v) { return fabsf(v) <= 3.402823466e38f; }   // false for NaN / inf
+
+// exp(i 2 pi t) for a double turn count, as float2
+__device__ __forceinline__ float2 cis_turns(double t)
+{
+    t -= rint(t);
+    double s, c;
+    sincospi(2.0 * t, &s, &c);
+    return make_float2((float)c, (float)s);
+}
+
+__global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
+{
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+
+    if (gid < a.B && gid < kOpticsChunk) a.optics[gid] = a.oc.f[gid];
+
+    if (gid >= a.N) {
+        // ---- phase-ramp tables exp(i 2 pi fx0 x_j), x_j = (j + 1/2) p  (oblique illumination)
+        if (!a.has_ramp) return;
+        long long r = gid - a.N;
+        const long long nx = (long long)a.B * a.W, ny = (long long)a.B * a.H;
+        if (r < nx) {
+            const int b = (int)(r / a.W), j = (int)(r % a.W);
+            const double f = b < kOpticsChunk ? a.oc.f[b].fx0_pitch : a.optics[b].fx0_pitch;
+            a.ramp_x[r] = cis_turns(f * (j + 0.5));
+        } else if (r - nx < ny) {
+            r -= nx;
+            const int b = (int)(r / a.H), i = (int)(r % a.H);
+            const double f = b < kOpticsChunk ? a.oc.f[b].fy0_pitch : a.optics[b].fy0_pitch;
+            a.ramp_y[r] = cis_turns(f * (i + 0.5));
+        }
+        return;
+    }
+
+    // ---- H1/H2: one particle ---------------------------------------------------------------------------------
+    const long long n = gid;
+    const float fcx = a.cx[n], fcy = a.cy[n], fqw = a.qw[n], fqx = a.qx[n], fqy = a.qy[n], fqz = a.qz[n];
+    const float fd0 = a.d0[n], fd1 = a.d1[n], fd2 = a.d2[n], fnp = a.n_p[n];
+    const unsigned kind = a.kind[n];
+    bool valid = finite_f(fcx) && finite_f(fcy) && finite_f(fqw) && finite_f(fqx) && finite_f(fqy) && finite_f(fqz) &&
+                 finite_f(fd0) && finite_f(fd1) && finite_f(fd2) && finite_f(fnp) &&
+                 fd0 > 0.0f && fd1 > 0.0f && fd2 > 0.0f && kind <= 1u;
+
+    int b = 0;
+    if (a.frame_start != nullptr) {              // largest b with frame_start[b] <= n
+        int lo = 0, hi = a.B;
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if ((long long)a.frame_start[mid] <= n) lo = mid; else hi = mid;
+        }
+        b = lo;
+    }
+    a.pframe[n] = b;
+
+    int4 tb = make_int4(1, 0, 1, 0);             // empty tile range
+    if (!valid) {
+        atomicOr(&a.status->bits, OSOG_WBADPARTICLE);
+        a.tbox[n] = tb;
+        return;
+    }
+
+    const double p = a.pitch;
+    const double cx = fcx, cy = fcy;
+    const double w = fqw, x = fqx, y = fqy, z = fqz;
+    // Hamilton active rotation body -> world, no renormalisation (reading A4)
+    const double R00 = 1.0 - 2.0 * (y * y + z * z), R01 = 2.0 * (x * y - w * z), R02 = 2.0 * (x * z + w * y);
+    const double R10 = 2.0 * (x * y + w * z), R11 = 1.0 - 2.0 * (x * x + z * z), R12 = 2.0 * (y * z - w * x);
+    const double R20 = 2.0 * (x * z - w * y), R21 = 2.0 * (y * z + w * x), R22 = 1.0 - 2.0 * (x * x + y * y);
+    const double e0 = fd0, e1 = fd1, e2 = fd2;
+
+    // B1: half extents of the projection
+    double hx, hy;
+    if (kind == 0u) {
+        hx = sqrt(R00 * R00 * e0 * e0 + R01 * R01 * e1 * e1 + R02 * R02 * e2 * e2);
+        hy = sqrt(R10 * R10 * e0 * e0 + R11 * R11 * e1 * e1 + R12 * R12 * e2 * e2);
+    } else {
+        const double hs = 0.5 * e0, hl = 0.5 * e1, ap = 0.5 * e1 + e2;
+        hx = fabs(R02 * ap);
+        hy = fabs(R12 * ap);
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {            // (+-s/2, +-s/2, +L/2); the -L/2 half mirrors it through the centre
+            const double sx = (v & 1) ? -hs : hs, sy = (v & 2) ? -hs : hs;
+            hx = fmax(hx, fabs(R00 * sx + R01 * sy + R02 * hl));
+            hy = fmax(hy, fabs(R10 * sx + R11 * sy + R12 * hl));
+        }
+    }
+    // B2: inclusive pixel range, padded by 2^-10 px, clamped to the frame
+    const double fj0 = ceil((cx - hx) / p - 0.5 - kBBoxPadPx), fj1 = floor((cx + hx) / p - 0.5 + kBBoxPadPx);
+    const double fi0 = ceil((cy - hy) / p - 0.5 - kBBoxPadPx), fi1 = floor((cy + hy) / p - 0.5 + kBBoxPadPx);
+    const double big = 1073741824.0;
+    if (!(fabs(fj0) <= 1.7976931348623157e308 && fabs(fj1) <= 1.7976931348623157e308 &&
+          fabs(fi0) <= 1.7976931348623157e308 && fabs(fi1) <= 1.7976931348623157e308)) {
+        a.tbox[n] = tb;                          // non-finite bound: not listed (the oracle does the same)
+        return;
+    }
+    const int j0 = max(0, min(a.W, (int)fmin(fmax(fj0, -big), big)));
+    const int j1 = max(-1, min(a.W - 1, (int)fmin(fmax(fj1, -big), big)));
+    const int i0 = max(0, min(a.H, (int)fmin(fmax(fi0, -big), big)));
+    const int i1 = max(-1, min(a.H - 1, (int)fmin(fmax(fi1, -big), big)));
+    if (j0 > j1 || i0 > i1) {
+        a.tbox[n] = tb;
+        return;
+    }
+    // B3: tile range + count
+    tb = make_int4(j0 / kTile, j1 / kTile, i0 / kTile, i1 / kTile);
+    a.tbox[n] = tb;
+    {
+        uint32_t* cnt = a.count + (size_t)b * a.ntx * a.nty;
+        for (int ty = tb.z; ty <= tb.w; ++ty)
+            for (int tx = tb.x; tx <= tb.y; ++tx) atomicAdd(&cnt[ty * a.ntx + tx], 1u);
+    }
+
+    // ---- H1: derived record, coordinates in pixels relative to pixel (jc, ic):  dx = p dj + ox -----------------
+    const double jc = fmin(fmax(floor(cx / p), -1.0e6), 1.0e6);
+    const double ic = fmin(fmax(floor(cy / p), -1.0e6), 1.0e6);
+    const double ox = (jc + 0.5) * p - cx, oy = (ic + 0.5) * p - cy;
+    const double dn = (double)fnp - a.n_medium;
+
+    float* r32 = a.rec32 + (size_t)n * kRecWords;
+    uint32_t* r32u = reinterpret_cast<uint32_t*>(r32);
+    r32[0] = (float)jc;
+    r32[1] = (float)ic;
+    r32u[2] = (uint32_t)j0 | ((uint32_t)j1 << 16);
+    r32u[3] = (uint32_t)i0 | ((uint32_t)i1 << 16);
+    r32u[7] = (uint32_t)n;                       // particle index: row of rec64 for the fp64 refinement
+
+    if (kind == 0u) {
+        // M = R diag(1/a^2, 1/b^2, 1/c^2) R^T; chord of {q^T M q <= 1} along z at (dx, dy):
+        // t = T0 sqrt(1 - d^T S d), S = Schur complement of M_zz, T0 = 2 / sqrt(M_zz)   (H5)
+        const double i0s = 1.0 / (e0 * e0), i1s = 1.0 / (e1 * e1), i2s = 1.0 / (e2 * e2);
+        const double Mxx = R00 * i0s * R00 + R01 * i1s * R01 + R02 * i2s * R02;
+        const double Mxy = R00 * i0s * R10 + R01 * i1s * R11 + R02 * i2s * R12;
+        const double Mxz = R00 * i0s * R20 + R01 * i1s * R21 + R02 * i2s * R22;
+        const double Myy = R10 * i0s * R10 + R11 * i1s * R11 + R12 * i2s * R12;
+        const double Myz = R10 * i0s * R20 + R11 * i1s * R21 + R12 * i2s * R22;
+        const double Mzz = R20 * i0s * R20 + R21 * i1s * R21 + R22 * i2s * R22;
+        const double Sxx = Mxx - Mxz * Mxz / Mzz, Sxy = Mxy - Mxz * Myz / Mzz, Syy = Myy - Myz * Myz / Mzz;
+        const double T0 = 2.0 / sqrt(Mzz);
+        double* c = reinterpret_cast<double*>(r32 + 8);
+        c[0] = Sxx * p * p;
+        c[1] = 2.0 * Sxy * p * p;
+        c[2] = Syy * p * p;
+        c[3] = 2.0 * p * (Sxx * ox + Sxy * oy);
+        c[4] = 2.0 * p * (Sxy * ox + Syy * oy);
+        c[5] = 1.0 - (Sxx * ox * ox + 2.0 * Sxy * ox * oy + Syy * oy * oy);
+        c[6] = jc;
+        c[7] = ic;
+        r32u[4] = 0u;
+        r32[5] = (float)(dn * T0);
+        r32[6] = 0.0f;
+#pragma unroll
+        for (int k = 24; k < 32; ++k) r32[k] = 0.0f;
+        return;
+    }
+
+    // ---- capped tetragonal prism: 12 half-spaces = 6 centrally symmetric slabs  |n_k . x| <= b_k  (Eq. 1) ----
+    const double s = e0, L = e1, hc = e2;
+    const double bn[6][3] = { {1.0, 0.0, 0.0}, {0.0, 1.0, 0.0}, {hc, 0.0, 0.5 * s}, {hc, 0.0, -0.5 * s},
+                              {0.0, hc, 0.5 * s}, {0.0, hc, -0.5 * s} };
+    const double bcap = hc * s * 0.5 + s * L * 0.25;
+    double nx[6], ny[6], nz[6], bb[6], G[6];
+    int ord[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        nx[k] = R00 * bn[k][0] + R01 * bn[k][1] + R02 * bn[k][2];
+        ny[k] = R10 * bn[k][0] + R11 * bn[k][1] + R12 * bn[k][2];
+        nz[k] = R20 * bn[k][0] + R21 * bn[k][1] + R22 * bn[k][2];
+        bb[k] = k < 2 ? 0.5 * s : bcap;
+        const double h = sqrt(nx[k] * nx[k] + ny[k] * ny[k]);
+        G[k] = nz[k] == 0.0 ? 1.0e300 : h / fabs(nz[k]);
+        ord[k] = k;
+    }
+    for (int u = 1; u < 6; ++u) {                // insertion sort, steepest first
+        const int v = ord[u];
+        int t = u - 1;
+        while (t >= 0 && G[ord[t]] < G[v]) { ord[t + 1] = ord[t]; --t; }
+        ord[t + 1] = v;
+    }
+    const double ext_px = fmax(hx, hy) / p + 1.0;
+    uint32_t flags = kFlagPrism;
+    int ns = 0;
+    double margin = 0.0;
+    double* r64 = a.rec64 + (size_t)n * kRec64Doubles;
+    for (int q = 0; q < 6; ++q) {
+        const int k = ord[q];
+        float U32, V32, X32, N32;
+        if (nz[k] == 0.0) {
+            // vertical face pair: no z bound; the line is inside the slab iff |n_x dx + n_y dy| <= b
+            r64[4 * q + 0] = nx[k] * p;
+            r64[4 * q + 1] = ny[k] * p;
+            r64[4 * q + 2] = nx[k] * ox + ny[k] * oy;
+            r64[4 * q + 3] = bb[k];
+            flags |= kFlagAllF64 | (1u << (16 + q));
+            U32 = 0.0f; V32 = 0.0f; X32 = 3.0e38f; N32 = -3.0e38f;
+            ++ns;
+        } else {
+            const double sg = nz[k] > 0.0 ? 1.0 : -1.0;
+            const double r = 1.0 / fabs(nz[k]);
+            const double U = sg * r * nx[k] * p, V = sg * r * ny[k] * p;
+            const double W0 = sg * r * (nx[k] * ox + ny[k] * oy), Cb = bb[k] * r;
+            const double Cx = Cb - W0, Cn = -Cb - W0;     // exit_k = Cx - U dj - V di ; enter_k = Cn - U dj - V di
+            r64[4 * q + 0] = U; r64[4 * q + 1] = V; r64[4 * q + 2] = Cx; r64[4 * q + 3] = Cn;
+            if (G[k] > kAllF64Slope) {
+                flags |= kFlagAllF64;
+                U32 = 0.0f; V32 = 0.0f; X32 = 3.0e38f; N32 = -3.0e38f;
+                ++ns;
+            } else {
+                U32 = (float)U; V32 = (float)V; X32 = (float)Cx; N32 = (float)Cn;
+                if (G[k] > (double)kSteepSlope) {
+                    ++ns;
+                    const double mag = fmax(fabs(Cx), fabs(Cn)) + (fabs(U) + fabs(V)) * ext_px;
+                    margin = fmax(margin, mag * 6.0e-7);
+                }
+            }
+        }
+        r32[8 + 4 * q + 0] = U32; r32[8 + 4 * q + 1] = V32; r32[8 + 4 * q + 2] = X32; r32[8 + 4 * q + 3] = N32;
+    }
+    flags |= (uint32_t)ns << 8;
+    r32u[4] = flags;
+    r32[5] = (float)dn;
+    r32[6] = (float)margin;
+}
+
+// H3: exclusive scan of count[0..n) -> offset[0..n], total -> status->pairs; count is reset to 0 (it becomes
+// the fill cursor).  One CTA: each thread scans a contiguous run, warp shuffles combine the runs.
+__global__ void __launch_bounds__(1024) k_scan(uint32_t* __restrict__ count, uint32_t* __restrict__ offset,
+                                               long long n, long long max_pairs, DeviceStatus* status)
+{
+    __shared__ unsigned long long warp_sum[32];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const long long per = (n + blockDim.x - 1) / blockDim.x;
+    const long long lo = min(n, per * tid), hi = min(n, lo + per);
+    unsigned long long s = 0;
+    for (long long k = lo; k < hi; ++k) s += count[k];
+    unsigned long long incl = s;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned long long v = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += v;
+    }
+    if (lane == 31) warp_sum[wid] = incl;
+    __syncthreads();
+    if (wid == 0) {
+        unsigned long long v = warp_sum[lane], t = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned long long u = __shfl_up_sync(0xffffffffu, t, d);
+            if (lane >= d) t += u;
+        }
+        warp_sum[lane] = t - v;                  // exclusive over warps
+        if (lane == 31) {
+            status->pairs = t;
+            if (t > (unsigned long long)max_pairs) atomicOr(&status->bits, OSOG_WOVERFLOW);
+            offset[n] = (uint32_t)min(t, 0xffffffffull);
+        }
+    }
+    __syncthreads();
+    unsigned long long run = warp_sum[wid] + (incl - s);
+    for (long long k = lo; k < hi; ++k) {
+        const uint32_t c = count[k];
+        offset[k] = (uint32_t)min(run, 0xffffffffull);
+        count[k] = 0u;
+        run += c;
+    }
+}
+
+// H4: every listed particle appends its index to each tile of its range.  Order inside a tile is whatever
+// the atomics give; the composition kernel sorts each segment ascending before use.
+__global__ void __launch_bounds__(128) k_fill(const int4* __restrict__ tbox, const int* __restrict__ pframe,
+                                              uint32_t* __restrict__ cursor, const uint32_t* __restrict__ offset,
+                                              uint32_t* __restrict__ list, long long N, int ntx, int nty,
+                                              const DeviceStatus* status)
+{
+    const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    if (status->bits & OSOG_WOVERFLOW) return;
+    const int4 tb = tbox[n];
+    if (tb.x > tb.y) return;
+    const size_t base = (size_t)pframe[n] * ntx * nty;
+    for (int ty = tb.z; ty <= tb.w; ++ty)
+        for (int tx = tb.x; tx <= tb.y; ++tx) {
+            const size_t t = base + (size_t)ty * ntx + tx;
+            const uint32_t pos = atomicAdd(&cursor[t], 1u);
+            list[offset[t] + pos] = (uint32_t)n;
+        }
+}
+
+__global__ void k_set_optics(FrameOptics* optics, const OpticsChunk oc)
+{
+    const int k = threadIdx.x;
+    if (k < oc.count) optics[oc.first + k] = oc.f[k];
+}
+
+static FrameOptics frame_optics(const osog_ctx* c, const osog_optics* o, int b)
+{
+    FrameOptics f;
+    const double lam = o->lambda_um[b];
+    f.inv_lambda = 1.0 / lam;
+    f.fx0_pitch = sin(o->tilt_x_rad) / lam * o->pitch_um;
+    f.fy0_pitch = sin(o->tilt_y_rad) / lam * o->pitch_um;
+    f.pupil_thresh = -1;
+    if (o->pupil_enabled && o->NA != nullptr) {
+        const double r = o->NA[b] * o->pitch_um / lam;
+        const double t = floor(r * r * ((double)c->H * c->H) * ((double)c->W * c->W));
+        f.pupil_thresh = t >= 9.0e18 ? -1 : (long long)t;     // a radius beyond every bin is all-pass
+    }
+    return f;
+}
+
+cudaError_t upload_optics(osog_ctx* c, const osog_optics* o, OpticsChunk* first)
+{
+    const int B = o->B;
+    for (int s = 0; s < B; s += kOpticsChunk) {
+        OpticsChunk oc;
+        oc.first = s;
+        oc.count = min(kOpticsChunk, B - s);
+        for (int k = 0; k < oc.count; ++k) oc.f[k] = frame_optics(c, o, s + k);
+        for (int k = oc.count; k < kOpticsChunk; ++k) oc.f[k] = oc.f[0];
+        if (s == 0 && first != nullptr) *first = oc;
+        if (s > 0 || first == nullptr) {
+            k_set_optics<<<1, kOpticsChunk, 0, c->stream>>>(c->optics, oc);
+            cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+        }
+    }
+    return cudaSuccess;
+}
+
+cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o)
+{
+    const int B = o->B;
+    const long long tiles = (long long)B * c->ntx * c->nty;
+    c->last_B = B;
+    c->last_tiles = tiles;
+    cudaError_t e;
+    if ((e = cudaMemsetAsync(c->count, 0, sizeof(uint32_t) * (size_t)tiles, c->stream)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(c->status, 0, sizeof(DeviceStatus), c->stream)) != cudaSuccess) return e;
+
+    PrepArgs a;
+    a.cx = p->cx; a.cy = p->cy; a.qw = p->qw; a.qx = p->qx; a.qy = p->qy; a.qz = p->qz;
+    a.d0 = p->d0; a.d1 = p->d1; a.d2 = p->d2; a.n_p = p->n_p; a.kind = p->kind;
+    a.frame_start = B > 1 ? p->frame_start : nullptr;
+    a.N = N; a.B = B; a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
+    a.pitch = o->pitch_um; a.n_medium = o->n_medium;
+    a.rec32 = c->rec32; a.rec64 = c->rec64; a.tbox = c->tbox; a.pframe = c->pframe; a.count = c->count;
+    a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.optics = c->optics; a.status = c->status;
+    a.has_ramp = (o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0) ? 1 : 0;
+    if ((e = upload_optics(c, o, &a.oc)) != cudaSuccess) return e;
+
+    long long items = N + (a.has_ramp ? (long long)B * (c->W + c->H) : 0);
+    if (items < B) items = B;
+    const int threads = 128;
+    const long long blocks = (items + threads - 1) / threads;
+    k_prepare<<<(unsigned)blocks, threads, 0, c->stream>>>(a);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    k_scan<<<1, 1024, 0, c->stream>>>(c->count, c->offset, tiles, c->max_pairs, c->status);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if (N > 0) {
+        k_fill<<<(unsigned)((N + threads - 1) / threads), threads, 0, c->stream>>>(
+            c->tbox, c->pframe, c->count, c->offset, c->list, N, c->ntx, c->nty, c->status);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+}  // namespace osog

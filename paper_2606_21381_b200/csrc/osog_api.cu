@@ -1,0 +1,300 @@
+// C ABI of libosog (include/osog.h): context management, argument checks, launch sequencing.
+#include <new>
+#include <cstring>
+#include "osog_internal.cuh"
+
+using namespace osog;
+
+namespace {
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+int cuda_fail(osog_ctx* c, cudaError_t e)
+{
+    if (c) c->last_cuda_error = (int)e;
+    return OSOG_ECUDA;
+}
+
+template <class T>
+cudaError_t dalloc(T** p, size_t n)
+{
+    *p = nullptr;
+    return cudaMalloc(reinterpret_cast<void**>(p), sizeof(T) * (n ? n : 1));
+}
+
+int check_call(const osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const void* out)
+{
+    if (!c || !p || !o || !out) return OSOG_EINVAL;
+    if (p->struct_size != sizeof(osog_particles) || o->struct_size != sizeof(osog_optics)) return OSOG_EINVAL;
+    if (N < 0 || N > c->max_particles) return OSOG_EINVAL;
+    if (o->B < 1 || o->B > c->max_frames) return OSOG_EINVAL;
+    if (!aligned16(out)) return OSOG_EINVAL;
+    if (!(o->pitch_um > 0.0) || !(o->pitch_um < 1.0e300) || !(fabs(o->n_medium) < 1.0e300)) return OSOG_EINVAL;
+    if (!o->lambda_um) return OSOG_EINVAL;
+    for (int b = 0; b < o->B; ++b)
+        if (!(o->lambda_um[b] > 0.0) || !(o->lambda_um[b] < 1.0e300)) return OSOG_EINVAL;
+    if (!(fabs(o->tilt_x_rad) < 1.0e300) || !(fabs(o->tilt_y_rad) < 1.0e300)) return OSOG_EINVAL;
+    if (N > 0) {
+        const void* cols[] = {p->cx, p->cy, p->qw, p->qx, p->qy, p->qz, p->d0, p->d1, p->d2, p->n_p, p->kind};
+        for (const void* q : cols)
+            if (!q) return OSOG_EINVAL;
+        const void* fcols[] = {p->cx, p->cy, p->qw, p->qx, p->qy, p->qz, p->d0, p->d1, p->d2, p->n_p};
+        for (const void* q : fcols)
+            if (reinterpret_cast<uintptr_t>(q) & 3u) return OSOG_EINVAL;
+    }
+    if (o->B > 1 && !p->frame_start) return OSOG_EINVAL;
+    return OSOG_OK;
+}
+
+int check_intensity(const osog_optics* o)
+{
+    if (!(o->read_noise_sigma >= 0.0) || !(o->read_noise_sigma < 1.0e300)) return OSOG_EINVAL;
+    if (o->pupil_enabled) {
+        if (!o->NA) return OSOG_EINVAL;
+        for (int b = 0; b < o->B; ++b)
+            if (!(o->NA[b] > 0.0) || !(o->NA[b] < 1.0e300)) return OSOG_EINVAL;
+    }
+    return OSOG_OK;
+}
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = false;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        ok = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+// forward FFT, pupil, inverse FFT of B frames held in `buf` (in place), then the sensor into d_intensity
+int optics_stage(osog_ctx* c, const osog_optics* o, float2* buf, float* d_intensity)
+{
+    const int B = o->B;
+    const size_t npx = (size_t)c->H * c->W;
+    for (int dir = 0; dir < 2; ++dir) {
+        const int sign = dir == 0 ? CUFFT_FORWARD : CUFFT_INVERSE;
+        if (B == c->max_frames && c->has_plan_batch) {
+            cufftResult r = cufftExecC2C(c->plan_batch, reinterpret_cast<cufftComplex*>(buf),
+                                         reinterpret_cast<cufftComplex*>(buf), sign);
+            if (r != CUFFT_SUCCESS) { c->last_cuda_error = 10000 + (int)r; return OSOG_ECUDA; }
+        } else {
+            for (int b = 0; b < B; ++b) {
+                cufftComplex* f = reinterpret_cast<cufftComplex*>(buf + (size_t)b * npx);
+                cufftResult r = cufftExecC2C(c->plan_one, f, f, sign);
+                if (r != CUFFT_SUCCESS) { c->last_cuda_error = 10000 + (int)r; return OSOG_ECUDA; }
+            }
+        }
+        if (dir == 0) {
+            cudaError_t e = launch_pupil(c, B, buf);
+            if (e != cudaSuccess) return cuda_fail(c, e);
+        }
+    }
+    cudaError_t e = launch_sensor(c, B, buf, d_intensity, o->read_noise_sigma, o->seed);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return OSOG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int osog_tile_size(void) { return kTile; }
+
+const char* osog_strerror(int code)
+{
+    switch (code) {
+        case OSOG_OK: return "ok";
+        case OSOG_EINVAL: return "invalid argument";
+        case OSOG_ECUDA: return "CUDA or cuFFT failure";
+        case OSOG_ECAPACITY: return "particle-tile pair list overflow";
+        case OSOG_ENOMEM: return "out of memory";
+        default: return "unknown error";
+    }
+}
+
+int osog_last_cuda_error(const osog_ctx* ctx) { return ctx ? ctx->last_cuda_error : 0; }
+
+int osog_destroy(osog_ctx* c)
+{
+    if (!c) return OSOG_EINVAL;
+    DeviceGuard g(c->device);
+    if (c->has_plan_one) cufftDestroy(c->plan_one);
+    if (c->has_plan_batch) cufftDestroy(c->plan_batch);
+    cudaFree(c->rec32); cudaFree(c->rec64); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
+    cudaFree(c->offset); cudaFree(c->list); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
+    cudaFree(c->status); cudaFree(c->field);
+    if (c->h_status) cudaFreeHost(c->h_status);
+    delete c;
+    return OSOG_OK;
+}
+
+int osog_create(osog_ctx** out, const osog_config* cfg)
+{
+    if (!out) return OSOG_EINVAL;
+    *out = nullptr;
+    if (!cfg || cfg->struct_size != sizeof(osog_config)) return OSOG_EINVAL;
+    if (cfg->H < 1 || cfg->W < 1 || cfg->H > 32768 || cfg->W > 32768) return OSOG_EINVAL;
+    if (cfg->max_frames < 1 || cfg->max_frames > 65535 || cfg->max_particles < 0 || cfg->max_pairs < 0) return OSOG_EINVAL;
+    if (cfg->max_particles > 0xfffffff0ll) return OSOG_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) return OSOG_ECUDA;
+
+    osog_ctx* c = new (std::nothrow) osog_ctx;
+    if (!c) return OSOG_ENOMEM;
+    std::memset(c, 0, sizeof(*c));
+    c->device = cfg->device;
+    c->stream = static_cast<cudaStream_t>(cfg->stream);
+    c->H = cfg->H; c->W = cfg->W; c->max_frames = cfg->max_frames;
+    c->max_particles = cfg->max_particles;
+    c->max_pairs = cfg->max_pairs > 0 ? cfg->max_pairs : 64 * cfg->max_particles + 1024;
+    if (c->max_pairs > 0xfffffff0ll) c->max_pairs = 0xfffffff0ll;
+    c->ntx = (c->W + kTile - 1) / kTile;
+    c->nty = (c->H + kTile - 1) / kTile;
+    c->max_tiles = (long long)c->max_frames * c->ntx * c->nty;
+    if (c->max_tiles > 0x7fffffffll) { delete c; return OSOG_EINVAL; }
+
+    DeviceGuard g(c->device);
+    if (!g.ok) { delete c; return OSOG_ECUDA; }
+    const size_t np = (size_t)c->max_particles, npx = (size_t)c->H * c->W;
+    cudaError_t e = cudaSuccess;
+    auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+    A(dalloc(&c->rec32, np * kRecWords));
+    A(dalloc(&c->rec64, np * kRec64Doubles));
+    A(dalloc(&c->tbox, np));
+    A(dalloc(&c->pframe, np));
+    A(dalloc(&c->count, (size_t)c->max_tiles));
+    A(dalloc(&c->offset, (size_t)c->max_tiles + 1));
+    A(dalloc(&c->list, (size_t)c->max_pairs));
+    A(dalloc(&c->ramp_x, (size_t)c->max_frames * c->W));
+    A(dalloc(&c->ramp_y, (size_t)c->max_frames * c->H));
+    A(dalloc(&c->optics, (size_t)c->max_frames));
+    A(dalloc(&c->status, 1));
+    A(dalloc(&c->field, (size_t)c->max_frames * npx));
+    if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&c->h_status), sizeof(DeviceStatus));
+    if (e == cudaSuccess) e = cudaMemset(c->status, 0, sizeof(DeviceStatus));
+    if (e == cudaSuccess) e = cudaMemset(c->offset, 0, sizeof(uint32_t) * ((size_t)c->max_tiles + 1));
+    if (e != cudaSuccess) {
+        const bool oom = e == cudaErrorMemoryAllocation;
+        cudaGetLastError();
+        osog_destroy(c);
+        return oom ? OSOG_ENOMEM : OSOG_ECUDA;
+    }
+    int dims[2] = {c->H, c->W};
+    if (cufftPlanMany(&c->plan_one, 2, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2C, 1) == CUFFT_SUCCESS) {
+        c->has_plan_one = true;
+        cufftSetStream(c->plan_one, c->stream);
+    }
+    if (c->max_frames > 1 &&
+        cufftPlanMany(&c->plan_batch, 2, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2C, c->max_frames) == CUFFT_SUCCESS) {
+        c->has_plan_batch = true;
+        cufftSetStream(c->plan_batch, c->stream);
+    }
+    if (!c->has_plan_one) { osog_destroy(c); return OSOG_ECUDA; }
+    *out = c;
+    return OSOG_OK;
+}
+
+static int render_common(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd,
+                         float2* d_field)
+{
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    cudaError_t e = launch_binning(c, p, N, o);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    const bool has_ramp = o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0;
+    e = launch_compose(c, N, o->B, has_ramp, d_opd, d_field);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return OSOG_OK;
+}
+
+int osog_render_opd(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd)
+{
+    const int r = check_call(c, p, N, o, d_opd);
+    if (r != OSOG_OK) return r;
+    return render_common(c, p, N, o, d_opd, nullptr);
+}
+
+int osog_render_field(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_field)
+{
+    const int r = check_call(c, p, N, o, d_field);
+    if (r != OSOG_OK) return r;
+    return render_common(c, p, N, o, nullptr, reinterpret_cast<float2*>(d_field));
+}
+
+int osog_render_intensity(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_intensity)
+{
+    int r = check_call(c, p, N, o, d_intensity);
+    if (r != OSOG_OK) return r;
+    if ((r = check_intensity(o)) != OSOG_OK) return r;
+    if ((r = render_common(c, p, N, o, nullptr, c->field)) != OSOG_OK) return r;
+    DeviceGuard g(c->device);
+    return optics_stage(c, o, c->field, d_intensity);
+}
+
+int osog_field_to_intensity(osog_ctx* c, const osog_optics* o, const float* d_field, float* d_intensity)
+{
+    if (!c || !o || !d_field || !d_intensity || o->struct_size != sizeof(osog_optics)) return OSOG_EINVAL;
+    if (o->B < 1 || o->B > c->max_frames || !o->lambda_um || !aligned16(d_field) || !aligned16(d_intensity)) return OSOG_EINVAL;
+    if (!(o->pitch_um > 0.0)) return OSOG_EINVAL;
+    for (int b = 0; b < o->B; ++b)
+        if (!(o->lambda_um[b] > 0.0)) return OSOG_EINVAL;
+    int r = check_intensity(o);
+    if (r != OSOG_OK) return r;
+    DeviceGuard g(c->device);
+    cudaError_t e = upload_optics(c, o, nullptr);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = cudaMemcpyAsync(c->field, d_field, sizeof(float2) * (size_t)o->B * c->H * c->W, cudaMemcpyDeviceToDevice, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return optics_stage(c, o, c->field, d_intensity);
+}
+
+int osog_render_opd_atomic(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd)
+{
+    const int r = check_call(c, p, N, o, d_opd);
+    if (r != OSOG_OK) return r;
+    DeviceGuard g(c->device);
+    cudaError_t e = launch_binning(c, p, N, o);      // records + bounding boxes (the tile lists are not used)
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = launch_compose_atomic(c, N, o->B, d_opd);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return OSOG_OK;
+}
+
+int osog_status(osog_ctx* c, uint32_t* status_bits, int64_t* pairs)
+{
+    if (!c) return OSOG_EINVAL;
+    DeviceGuard g(c->device);
+    cudaError_t e = cudaMemcpyAsync(c->h_status, c->status, sizeof(DeviceStatus), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    if (status_bits) *status_bits = c->h_status->bits;
+    if (pairs) *pairs = (int64_t)c->h_status->pairs;
+    return (c->h_status->bits & OSOG_WOVERFLOW) ? OSOG_ECAPACITY : OSOG_OK;
+}
+
+int osog_debug_bins(osog_ctx* c, uint32_t* h_offset, uint32_t* h_list, int64_t cap, int64_t* n_tiles, int64_t* n_pairs)
+{
+    if (!c || cap < 0) return OSOG_EINVAL;
+    uint32_t bits = 0;
+    int64_t pairs = 0;
+    const int r = osog_status(c, &bits, &pairs);
+    if (r == OSOG_ECUDA || r == OSOG_EINVAL) return r;
+    if (n_tiles) *n_tiles = c->last_tiles;
+    if (n_pairs) *n_pairs = pairs;
+    DeviceGuard g(c->device);
+    cudaError_t e = cudaSuccess;
+    if (h_offset && c->last_tiles > 0)
+        e = cudaMemcpy(h_offset, c->offset, sizeof(uint32_t) * ((size_t)c->last_tiles + 1), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    const int64_t ncopy = pairs < cap ? pairs : cap;
+    if (h_list && ncopy > 0 && r == OSOG_OK) e = cudaMemcpy(h_list, c->list, sizeof(uint32_t) * (size_t)ncopy, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return r;
+}
+
+}  // extern "C"

@@ -1,0 +1,90 @@
+// Internal declarations shared by the CUDA translation units of libosog (NOT part of the C ABI).
+// Nothing here is shared with oracle/ ("independence").
+#pragma once
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+#include "../../include/osog.h"
+
+namespace osog {
+
+// ---- build-time constants -----------------------------------------------------------------------------------
+constexpr int kTile = 32;              // binning tile edge T (pixels); one CTA composes one tile
+constexpr int kComposeThreads = 256;   // 8 warps; each warp owns a 16 x 8 pixel sub-tile, each lane 4 x 1 pixels
+constexpr int kChunk = 96;             // particle records staged in shared memory per pass
+constexpr int kSortCap = 2048;         // longest tile list sorted in shared memory (longer: sorted in global memory)
+constexpr int kRecWords = 32;          // 128-byte fp32 record per particle
+constexpr int kRec64Doubles = 24;      // fp64 plane coefficients per prism (refinement path)
+constexpr double kBBoxPadPx = 1.0 / 1024.0;   // delta of DESIGN.md B2
+constexpr float kSteepSlope = 8.0f;    // slabs steeper than this (|n_xy| / |n_z|) are refined in fp64 where active
+constexpr double kAllF64Slope = 1.0e4; // a slab steeper than this (or vertical) sends the whole particle to fp64
+
+// record header flags (word 4)
+constexpr uint32_t kFlagPrism = 1u;
+constexpr uint32_t kFlagAllF64 = 16u;
+// bits 8..10: number of steep slabs (they come first); bits 16..21: per-slab "vertical" (n_z == 0) mask
+
+// status word layout (device int32 [4]): [0] status bits, [1] unused, [2..3] pairs needed (uint64 split)
+struct DeviceStatus {
+    uint32_t bits;
+    uint32_t pad;
+    unsigned long long pairs;
+};
+
+struct FrameOptics {          // per frame, device
+    double inv_lambda;        // 1 / lambda  (turns per um of OPD)
+    double fx0_pitch;         // sin(tilt_x) / lambda * p : turns per pixel along x
+    double fy0_pitch;
+    long long pupil_thresh;   // floor((NA p / lambda)^2 H^2 W^2), or -1 = all-pass
+};
+
+constexpr int kOpticsChunk = 16;
+struct OpticsChunk {          // passed by value to k_set_optics
+    int first, count;
+    FrameOptics f[kOpticsChunk];
+};
+
+}  // namespace osog
+
+struct osog_ctx {
+    int device;
+    cudaStream_t stream;
+    int H, W, max_frames;
+    long long max_particles, max_pairs;
+    int ntx, nty;                   // tiles per row / column
+    long long max_tiles;            // max_frames * ntx * nty
+    int last_cuda_error;
+    // last call
+    int last_B;
+    long long last_tiles;
+    // scratch (device)
+    float* rec32;                   // [max_particles][32]
+    double* rec64;                  // [max_particles][24]
+    int4* tbox;                     // [max_particles] tile range tx0, tx1, ty0, ty1 (tx0 > tx1: not listed)
+    int* pframe;                    // [max_particles] frame of the particle
+    uint32_t* count;                // [max_tiles] per-tile count, reused as the fill cursor
+    uint32_t* offset;               // [max_tiles + 1]
+    uint32_t* list;                 // [max_pairs]
+    float2* ramp_x;                 // [max_frames][W]  exp(i 2 pi fx0 x_j)
+    float2* ramp_y;                 // [max_frames][H]
+    osog::FrameOptics* optics;      // [max_frames]
+    osog::DeviceStatus* status;     // [1]
+    float2* field;                  // [max_frames][H][W] (intensity path)
+    osog::DeviceStatus* h_status;   // pinned host mirror
+    cufftHandle plan_one, plan_batch;
+    bool has_plan_one, has_plan_batch;
+};
+
+namespace osog {
+
+// binning.cu
+cudaError_t upload_optics(osog_ctx* c, const osog_optics* o, OpticsChunk* first);
+cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o);
+// compose.cu
+cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float* d_opd, float2* d_field);
+cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd);
+// optics.cu
+cudaError_t launch_pupil(osog_ctx* c, int B, float2* spec);
+cudaError_t launch_sensor(osog_ctx* c, int B, const float2* img, float* d_intensity, double sigma, uint64_t seed);
+
+}  // namespace osog
