@@ -1,0 +1,298 @@
+#!/usr/bin/env python
+"""bench.py - headline benchmark of the OSOG forward-render hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (H1-H7: prepare, bounding box + count, scan, fill, ordered tile
+composition with the fused field write-out) over one seeded synthetic batch = one osog_render_field call.
+Default workload: BASELINE.json configs[3] (the paper-scale headline: 40,000 mixed particles, 2048 x 2048,
+NA 0.65, 10 degree oblique ramp).  Prints ONE JSON line (see DESIGN.md section 8 for every key).
+
+--impl reference times the float64 CPU oracle (oracle/) on the host cores, on a bounded sample of the same
+workload; it is a deliberately plain program, a reported baseline and not the target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "particles/s (hot path osog_render_field, 40k particles on 2048^2)"
+UNIT = "particles/s"
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks and throttle reasons while the timed region runs."""
+
+    FIELDS = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self._stop = threading.Event()
+        self._th = threading.Thread(target=self._run, daemon=True)
+
+    def _sample(self):
+        try:
+            out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
+                                  "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+            parts = [x.strip() for x in out.strip().split(",")]
+            if len(parts) >= 6:
+                self.rows.append(parts)
+        except Exception:
+            pass
+
+    def _run(self):
+        while not self._stop.is_set():
+            self._sample()
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self._th.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._th.join(timeout=6)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if r[1].replace(".", "").isdigit()]
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        reasons = sorted({n for r in self.rows for n, v in zip(names, r[2:6]) if v.lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+def _sample_rows(scene, rows):
+    """Oracle OPD of `rows` consecutive pixel rows from the middle of frame 0 (a bounded sample of the workload)."""
+    from oracle import oracle as o
+    fs = scene.frame_start
+    cols = {k: v[int(fs[0]):int(fs[1])] for k, v in scene.cols.items()}
+    # a strip is its own frame whose pixel rows are shifted: move the particles instead of the window
+    i0 = (scene.H - rows) // 2
+    shifted = dict(cols)
+    shifted["cy"] = (cols["cy"].astype(np.float64) - i0 * scene.pitch_um).astype(np.float32)
+    return o.render_opd_frame(shifted, 0, cols["kind"].shape[0], rows, scene.W, scene.pitch_um, scene.n_medium)
+
+
+def cpu_baseline(scene, budget_s=12.0):
+    """Time the oracle as it stands on the host cores on a strip of frame 0; scale particles/s by area."""
+    cores = len(os.sched_getaffinity(0))
+    os.environ.setdefault("OMP_NUM_THREADS", str(cores))
+    rows = min(scene.H, 64)
+    t0 = time.perf_counter()
+    _sample_rows(scene, rows)                       # warm-up (also builds / loads the oracle library)
+    dt = time.perf_counter() - t0
+    rows = int(min(scene.H, max(64, rows * budget_s / max(dt, 1e-3) * 0.5)))
+    t0 = time.perf_counter()
+    _sample_rows(scene, rows)
+    dt = time.perf_counter() - t0
+    n0 = int(scene.frame_start[1] - scene.frame_start[0])
+    frac = rows / scene.H                            # fraction of one frame's pixels (and of its particle work)
+    pps = n0 * frac / dt
+    return {"value": pps, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"OPD of {rows} of {scene.H} pixel rows of frame 0 ({n0} particles), float64, bcircle mode, "
+                      f"{dt:.2f} s; particles/s = particles x row fraction / time"}, dt
+
+
+def run_reference(args):
+    from workloads import make_config, CONFIG_NAMES
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    scene = make_config(args.config)
+    vals = []
+    for _ in range(args.warmup):
+        cpu_baseline(scene, budget_s=4.0)
+    last = None
+    for _ in range(args.steps):
+        last, _dt = cpu_baseline(scene, budget_s=4.0)
+        vals.append(last["value"])
+    v = float(np.mean(vals))
+    n0 = int(scene.frame_start[1] - scene.frame_start[0])
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": n0 / v * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": CONFIG_NAMES[args.config], "N": scene.N, "H": scene.H, "W": scene.W, "B": scene.B},
+            "cpu_baseline": dict(last, value=v),
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_21381_b200 as og
+    from workloads import make_config, CONFIG_NAMES
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py: no CUDA device (the hot path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    # replicas only: every rank renders its own seeded copy of the workload, no collective
+    scene = make_config(args.config)
+    H, W, B, N = scene.H, scene.W, scene.B, scene.N
+    ctx = og.Context(H, W, N, max_frames=B, device=dev)
+    P = og.Particles.from_scene(scene, device=dev)
+    opt = og.optics_from_scene(scene)
+    field = torch.empty((B, H, W, 2), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)       # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    stream = torch.cuda.current_stream(dev)
+    # ---- device-resident timing: K steps, each bracketed by CUDA events on the launching stream, L2 flushed between
+    for _ in range(args.warmup):
+        flush.zero_()
+        ctx.render_field(P, opt, out=field)
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    with ClockSampler(local) as clk:
+        t_wall0 = time.perf_counter()
+        for k in range(args.steps):
+            flush.zero_()
+            ev[k][0].record(stream)
+            ctx.render_field(P, opt, out=field)
+            ev[k][1].record(stream)
+        barrier()
+        t_wall = time.perf_counter() - t_wall0
+        # keep the GPU busy a little longer so that the sampler sees clocks under load
+        t_end = time.perf_counter() + 0.6
+        while time.perf_counter() < t_end:
+            ctx.render_field(P, opt, out=field)
+        torch.cuda.synchronize()
+    ms = np.array([a.elapsed_time(b) for a, b in ev])
+    t_steps = float(ms.sum()) * 1e-3
+    r, bits, pairs = ctx.status()
+    assert r == 0, f"osog_status {r}"
+
+    # ---- end-to-end: host (pinned) particle arrays -> device, render, device -> host read of the result
+    names = ("cx", "cy", "qw", "qx", "qy", "qz", "d0", "d1", "d2", "n_p")
+    host = {k: torch.from_numpy(scene.cols[k]).pin_memory() for k in names}
+    host["kind"] = torch.from_numpy(scene.cols["kind"]).pin_memory()
+    devbuf = {k: torch.empty_like(v, device=dev) for k, v in host.items()}
+    P2 = og.Particles(devbuf, scene.frame_start if B > 1 else None, device=dev)
+    host_out = torch.empty((B, H, W, 2), dtype=torch.float32).pin_memory()
+    h2d = sum(v.numel() * v.element_size() for v in host.values())
+    d2h = host_out.numel() * host_out.element_size()
+
+    def e2e_step():
+        for k, v in host.items():
+            P2.t[k].copy_(v, non_blocking=True)
+        ctx.render_field(P2, opt, out=field)
+        host_out.copy_(field, non_blocking=True)
+
+    for _ in range(max(1, args.warmup // 2)):
+        e2e_step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        e2e_step()
+    e1.record(stream)
+    barrier()
+    t_e2e = e0.elapsed_time(e1) * 1e-3
+
+    # ---- dominant kernel (k_compose_tile) timed alone for the roofline, + the separately timed library stage
+    lib = og.lib()
+    inten = torch.empty((B, H, W), dtype=torch.float32, device=dev)
+    ctx.render_intensity(P, opt, out=inten)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(5):
+        ctx.field_to_intensity(opt, torch.view_as_complex(field), out=inten)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_optics = e0.elapsed_time(e1) / 5
+    e0.record(stream)
+    for _ in range(5):
+        ctx.render_opd(P, opt, out=inten)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_opd = e0.elapsed_time(e1) / 5
+
+    t = torch.tensor([t_steps, t_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    t_steps, t_e2e = (float(x) for x in t.cpu())
+    peak, peak_src = _peaks()
+    alg_bytes = 48 * N + 8 * pairs + 8 * B * H * W      # SoA read + list write/read + complex64 write
+    ms_step = t_steps / args.steps * 1e3
+    achieved = alg_bytes / (ms_step * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": world * N * args.steps / t_steps, "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32+f64", "data": "synthetic",
+        "config": {"workload": CONFIG_NAMES[args.config], "N": N, "H": H, "W": W, "B": B, "tile": og.osog_tile_size(),
+                   "pairs": int(pairs), "l2": "flushed between timed steps (256 MB memset)", "parallelism": "replicas only"},
+        "frames_per_s": world * B * args.steps / t_steps,
+        "ms_per_step_median": float(np.median(ms)), "ms_per_step_std": float(ms.std()),
+        "e2e": {"value": world * N * args.steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h)},
+        "gpu_launches": 4 * args.steps,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": None, "peak_source": peak_src, "algorithmic_bytes": int(alg_bytes),
+                     "kernel": "whole hot path (k_prepare, k_scan, k_fill, k_compose_tile)",
+                     "frac_of_nominal_8TBs": achieved / 8000.0},
+        "library_stage_ms": ms_optics, "opd_only_ms": ms_opd,
+        "paper_context": "PAPER.md:195: 40,000 particles < 50 ms on one A100 at 1024^2 (whole pipeline); context only",
+        "clocks": clk.summary(),
+    }
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"], _ = cpu_baseline(scene)
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = min(args.steps, 3)
+        args.warmup = min(args.warmup, 1)
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

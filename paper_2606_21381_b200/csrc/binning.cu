@@ -13,8 +13,7 @@ struct PrepArgs {
     long long N;
     int B, H, W, ntx, nty;
     double pitch, n_medium;
-    float* rec32;
-    double* rec64;
+    float* rec;
     int4* tbox;
     int* pframe;
     uint32_t* count;
@@ -138,19 +137,26 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
             for (int tx = tb.x; tx <= tb.y; ++tx) atomicAdd(&cnt[ty * a.ntx + tx], 1u);
     }
 
-    // ---- H1: derived record, coordinates in pixels relative to pixel (jc, ic):  dx = p dj + ox -----------------
+    // ---- H1: derived record (kRecWords words).  Coordinates are pixel offsets from pixel (jc, ic): dx = p dj + ox ----
     const double jc = fmin(fmax(floor(cx / p), -1.0e6), 1.0e6);
     const double ic = fmin(fmax(floor(cy / p), -1.0e6), 1.0e6);
     const double ox = (jc + 0.5) * p - cx, oy = (ic + 0.5) * p - cy;
     const double dn = (double)fnp - a.n_medium;
 
-    float* r32 = a.rec32 + (size_t)n * kRecWords;
+    float* r32 = a.rec + (size_t)n * kRecWords;
     uint32_t* r32u = reinterpret_cast<uint32_t*>(r32);
-    r32[0] = (float)jc;
-    r32[1] = (float)ic;
-    r32u[2] = (uint32_t)j0 | ((uint32_t)j1 << 16);
-    r32u[3] = (uint32_t)i0 | ((uint32_t)i1 << 16);
-    r32u[7] = (uint32_t)n;                       // particle index: row of rec64 for the fp64 refinement
+    double* r64 = reinterpret_cast<double*>(r32 + 16);
+    // words 0..7: data of the sub-tile cull (centre in pixel-index coordinates, oriented box, pixel bounding box)
+    r32[0] = (float)(cx / p - 0.5);
+    r32[1] = (float)(cy / p - 0.5);
+    r32u[6] = (uint32_t)j0 | ((uint32_t)j1 << 16);
+    r32u[7] = (uint32_t)i0 | ((uint32_t)i1 << 16);
+    r32u[11] = (uint32_t)n;
+    reinterpret_cast<int*>(r32)[12] = (int)jc;
+    reinterpret_cast<int*>(r32)[13] = (int)ic;
+    r32[14] = 0.0f;
+    r32[15] = 0.0f;
+    const double cull_pad = 1.0 / 64.0;          // px; covers the fp32 rounding of the cull test
 
     if (kind == 0u) {
         // M = R diag(1/a^2, 1/b^2, 1/c^2) R^T; chord of {q^T M q <= 1} along z at (dx, dy):
@@ -164,20 +170,27 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
         const double Mzz = R20 * i0s * R20 + R21 * i1s * R21 + R22 * i2s * R22;
         const double Sxx = Mxx - Mxz * Mxz / Mzz, Sxy = Mxy - Mxz * Myz / Mzz, Syy = Myy - Myz * Myz / Mzz;
         const double T0 = 2.0 / sqrt(Mzz);
-        double* c = reinterpret_cast<double*>(r32 + 8);
-        c[0] = Sxx * p * p;
-        c[1] = 2.0 * Sxy * p * p;
-        c[2] = Syy * p * p;
-        c[3] = 2.0 * p * (Sxx * ox + Sxy * oy);
-        c[4] = 2.0 * p * (Sxy * ox + Syy * oy);
-        c[5] = 1.0 - (Sxx * ox * ox + 2.0 * Sxy * ox * oy + Syy * oy * oy);
-        c[6] = jc;
-        c[7] = ic;
-        r32u[4] = 0u;
-        r32[5] = (float)(dn * T0);
-        r32[6] = 0.0f;
-#pragma unroll
-        for (int k = 24; k < 32; ++k) r32[k] = 0.0f;
+        // w(dj, di) = F1 - (A dj^2 + B dj di + C di^2 + D dj + E di)
+        r64[0] = Sxx * p * p;
+        r64[1] = 2.0 * Sxy * p * p;
+        r64[2] = Syy * p * p;
+        r64[3] = 2.0 * p * (Sxx * ox + Sxy * oy);
+        r64[4] = 2.0 * p * (Sxy * ox + Syy * oy);
+        r64[5] = 1.0 - (Sxx * ox * ox + 2.0 * Sxy * ox * oy + Syy * oy * oy);
+        // oriented box of the silhouette ellipse {d^T S d <= 1}: principal axes of S
+        const double hd = 0.5 * (Sxx - Syy), rad = sqrt(hd * hd + Sxy * Sxy), mid = 0.5 * (Sxx + Syy);
+        const double lmin = fmax(mid - rad, 1.0e-300), lmax = mid + rad;
+        double vx = Sxy, vy = lmin - Sxx;        // eigenvector of the small eigenvalue = long axis
+        if (fabs(lmin - Syy) > fabs(vy)) { vx = lmin - Syy; vy = Sxy; }
+        double vn = sqrt(vx * vx + vy * vy);
+        if (!(vn > 1.0e-280)) { vx = 1.0; vy = 0.0; vn = 1.0; }
+        r32[2] = (float)(vx / vn);
+        r32[3] = (float)(vy / vn);
+        r32[4] = (float)((1.0 / sqrt(lmin)) / p * (1.0 + 1.0e-5) + cull_pad);
+        r32[5] = (float)((1.0 / sqrt(lmax)) / p * (1.0 + 1.0e-5) + cull_pad);
+        r32u[8] = 0u;
+        r32[9] = (float)(dn * T0);
+        r32[10] = 0.0f;
         return;
     }
 
@@ -204,14 +217,10 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
         while (t >= 0 && G[ord[t]] < G[v]) { ord[t + 1] = ord[t]; --t; }
         ord[t + 1] = v;
     }
-    const double ext_px = fmax(hx, hy) / p + 1.0;
     uint32_t flags = kFlagPrism;
     int ns = 0;
-    double margin = 0.0;
-    double* r64 = a.rec64 + (size_t)n * kRec64Doubles;
     for (int q = 0; q < 6; ++q) {
         const int k = ord[q];
-        float U32, V32, X32, N32;
         if (nz[k] == 0.0) {
             // vertical face pair: no z bound; the line is inside the slab iff |n_x dx + n_y dy| <= b
             r64[4 * q + 0] = nx[k] * p;
@@ -219,34 +228,41 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
             r64[4 * q + 2] = nx[k] * ox + ny[k] * oy;
             r64[4 * q + 3] = bb[k];
             flags |= kFlagAllF64 | (1u << (16 + q));
-            U32 = 0.0f; V32 = 0.0f; X32 = 3.0e38f; N32 = -3.0e38f;
             ++ns;
         } else {
             const double sg = nz[k] > 0.0 ? 1.0 : -1.0;
             const double r = 1.0 / fabs(nz[k]);
-            const double U = sg * r * nx[k] * p, V = sg * r * ny[k] * p;
             const double W0 = sg * r * (nx[k] * ox + ny[k] * oy), Cb = bb[k] * r;
-            const double Cx = Cb - W0, Cn = -Cb - W0;     // exit_k = Cx - U dj - V di ; enter_k = Cn - U dj - V di
-            r64[4 * q + 0] = U; r64[4 * q + 1] = V; r64[4 * q + 2] = Cx; r64[4 * q + 3] = Cn;
-            if (G[k] > kAllF64Slope) {
-                flags |= kFlagAllF64;
-                U32 = 0.0f; V32 = 0.0f; X32 = 3.0e38f; N32 = -3.0e38f;
-                ++ns;
-            } else {
-                U32 = (float)U; V32 = (float)V; X32 = (float)Cx; N32 = (float)Cn;
-                if (G[k] > (double)kSteepSlope) {
-                    ++ns;
-                    const double mag = fmax(fabs(Cx), fabs(Cn)) + (fabs(U) + fabs(V)) * ext_px;
-                    margin = fmax(margin, mag * 6.0e-7);
-                }
-            }
+            r64[4 * q + 0] = sg * r * nx[k] * p;          // U:  exit_k = Cx - U dj - V di
+            r64[4 * q + 1] = sg * r * ny[k] * p;          // V:  enter_k = Cn - U dj - V di
+            r64[4 * q + 2] = Cb - W0;                     // Cx
+            r64[4 * q + 3] = -Cb - W0;                    // Cn
+            if (G[k] > kAllF64Slope) flags |= kFlagAllF64;
+            if (G[k] > (double)kSteepSlope) ++ns;
         }
-        r32[8 + 4 * q + 0] = U32; r32[8 + 4 * q + 1] = V32; r32[8 + 4 * q + 2] = X32; r32[8 + 4 * q + 3] = N32;
     }
+    if (ns > 2) flags |= kFlagAllF64;            // more than two steep slabs: rare, every pixel goes to fp64
     flags |= (uint32_t)ns << 8;
-    r32u[4] = flags;
-    r32[5] = (float)dn;
-    r32[6] = (float)margin;
+    // oriented box of the silhouette: along the projected long axis (body z) and across it, over the 10 vertices
+    double ax = R02, ay = R12;
+    const double an = sqrt(ax * ax + ay * ay);
+    if (an > 1.0e-12) { ax /= an; ay /= an; } else { ax = 1.0; ay = 0.0; }
+    const double hs = 0.5 * s, hl = 0.5 * L, ap = 0.5 * L + hc;
+    double ha = fabs((R02 * ax + R12 * ay) * ap), hb = fabs((-R02 * ay + R12 * ax) * ap);
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+        const double sx = (v & 1) ? -hs : hs, sy = (v & 2) ? -hs : hs;
+        const double px = R00 * sx + R01 * sy + R02 * hl, py = R10 * sx + R11 * sy + R12 * hl;
+        ha = fmax(ha, fabs(px * ax + py * ay));
+        hb = fmax(hb, fabs(-px * ay + py * ax));
+    }
+    r32[2] = (float)ax;
+    r32[3] = (float)ay;
+    r32[4] = (float)(ha / p * (1.0 + 1.0e-5) + cull_pad);
+    r32[5] = (float)(hb / p * (1.0 + 1.0e-5) + cull_pad);
+    r32u[8] = flags;
+    r32[9] = (float)dn;
+    r32[10] = 0.0f;
 }
 
 // H3: exclusive scan of count[0..n) -> offset[0..n], total -> status->pairs; count is reset to 0 (it becomes
@@ -370,7 +386,7 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     a.frame_start = B > 1 ? p->frame_start : nullptr;
     a.N = N; a.B = B; a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
     a.pitch = o->pitch_um; a.n_medium = o->n_medium;
-    a.rec32 = c->rec32; a.rec64 = c->rec64; a.tbox = c->tbox; a.pframe = c->pframe; a.count = c->count;
+    a.rec = c->rec; a.tbox = c->tbox; a.pframe = c->pframe; a.count = c->count;
     a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.optics = c->optics; a.status = c->status;
     a.has_ramp = (o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0) ? 1 : 0;
     if ((e = upload_optics(c, o, &a.oc)) != cudaSuccess) return e;

@@ -1,15 +1,19 @@
-// H5-H7 of DESIGN.md: per-tile ordered composition.  One CTA per 32 x 32 pixel tile: sort the tile's
-// particle list ascending (deterministic summation order), stage the particle records in shared memory with
-// cp.async, let each warp cull the staged particles against its own 16 x 8 pixel sub-tile (ballot
-// compaction), evaluate the ray-convex thickness for 4 pixels per lane, accumulate OPD per pixel in fp64
-// registers, and write OPD and / or exp(i 2 pi OPD / lambda) * ramp straight from the registers.
+// H5-H7 of DESIGN.md: per-tile ordered composition.  One CTA per 32 x 32 pixel tile:
+//   1. sort the tile's particle list ascending (deterministic summation order) and write it back,
+//   2. stage the 256-byte particle records in shared memory with cp.async (chunks of kChunk),
+//   3. per warp (16 x 8 pixel sub-tile, 4 x 1 pixels per lane): one lane per staged particle tests the particle's
+//      pixel bounding box and oriented box against the sub-tile (ballot compaction keeps ascending order) and
+//      re-bases the survivor's fp64 coefficients to the sub-tile origin, rounding them to fp32 only there,
+//   4. all lanes walk the survivors: ray-convex thickness from the re-based coefficients (packed fp32 FMA and
+//      3-input min/max for the prism slabs, fp64 quadratic + fp32 sqrt for the ellipsoid), OPD accumulated per
+//      pixel in fp64 registers,
+//   5. write OPD and / or exp(i 2 pi OPD / lambda) * ramp straight from the registers.
 #include "osog_internal.cuh"
 
 namespace osog {
 
 struct ComposeArgs {
-    const float* rec32;
-    const double* rec64;
+    const float* rec;
     const uint32_t* offset;
     uint32_t* list;
     const FrameOptics* optics;
@@ -21,13 +25,45 @@ struct ComposeArgs {
     int ramp_y_on;
 };
 
+constexpr int kWarps = kComposeThreads / 32;
+constexpr int kRecStride4 = kRecWords / 4 + 1;     // staged record stride in float4 (padded: conflict-free lane-per-record reads)
+constexpr int kSlotStride4 = 9;                    // survivor slot stride in float4 (7 used, padded to an odd count)
+constexpr int kSmemRec = kChunk * kRecStride4 * 16;
+constexpr int kSmemIds = kSortCap * 4;
+constexpr int kSmemSlots = kWarps * 32 * kSlotStride4 * 16;
+constexpr int kSmemBytes = kSmemRec + kSmemIds + kSmemSlots;
+
+// ---- small PTX helpers ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float fast_sqrt(float x)
 {
     float r;
     asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
 }
-
+__device__ __forceinline__ float min3(float a, float b, float c)
+{
+    float r;
+    asm("min.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+    return r;
+}
+__device__ __forceinline__ float max3(float a, float b, float c)
+{
+    float r;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+    return r;
+}
+// packed fp32 FMA (Blackwell FFMA2): d = a * b + c on both halves
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c)
+{
+    unsigned long long ra, rb, rc, rd;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(b.x), "f"(b.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rc) : "f"(c.x), "f"(c.y));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd) : "l"(ra), "l"(rb), "l"(rc));
+    float2 d;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
+    return d;
+}
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
 {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -38,33 +74,9 @@ __device__ __forceinline__ void cp_async_wait_all()
     asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
 }
 
-// ---- thickness kernels -----------------------------------------------------------------------------------------
-// Ellipsoid (kind 0): w = 1 - d^T S d as a quadratic polynomial of the integer pixel offsets, evaluated in
-// fp64 (2 DFMA per pixel after the per-row terms), then t = T0 sqrt(max(w, 0)) in fp32.  acc += dn T0 sqrt(w).
-template <int NPX>
-__device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ rec, double jd, double id, double (&acc)[NPX])
-{
-    const float4 h1 = rec[1];
-    const double2 c01 = *reinterpret_cast<const double2*>(rec + 2);   // A, B
-    const double2 c23 = *reinterpret_cast<const double2*>(rec + 3);   // C, D
-    const double2 c45 = *reinterpret_cast<const double2*>(rec + 4);   // E, F1
-    const double2 c67 = *reinterpret_cast<const double2*>(rec + 5);   // jc, ic
-    const double K = (double)h1.y;
-    const double dj = jd - c67.x, di = id - c67.y;
-    const double b1 = fma(c01.y, di, c23.y);
-    const double c1 = fma(-fma(c23.x, di, c45.x), di, c45.y);
-#pragma unroll
-    for (int k = 0; k < NPX; ++k) {
-        const double djk = dj + (double)k;
-        const double g = fma(c01.x, djk, b1);
-        const float w = (float)fma(-djk, g, c1);
-        const float t = fast_sqrt(fmaxf(w, 0.0f));
-        acc[k] = fma((double)t, K, acc[k]);
-    }
-}
-
-// Prism, fp64, one pixel: the 6 slabs from the fp64 coefficients (exit_k = Cx - U dj - V di, enter_k = Cn - ...).
-__device__ __noinline__ double prism_t64(const double* __restrict__ r64, uint32_t vmask, double dj, double di)
+// ---- fp64 prism evaluation (refinement of flagged pixels, and the atomic variant) -------------------------------------
+// r64: 24 doubles (U, V, Cx, Cn per slab, relative to pixel (jc, ic)); dj, di: pixel offsets from (jc, ic).
+__device__ __noinline__ double prism_t64(const double* r64, uint32_t vmask, double dj, double di)
 {
     double ex = 1.0e300, en = -1.0e300;
     for (int q = 0; q < 6; ++q) {
@@ -83,76 +95,140 @@ __device__ __noinline__ double prism_t64(const double* __restrict__ r64, uint32_
     return t > 0.0 ? t : 0.0;
 }
 
-// Prism (kind 1): 6 slabs in fp32; the first ns slabs are the steep ones.  A pixel where a steep slab is (within
-// the margin) the active entry or exit face is re-evaluated in fp64 ("precision").
-template <int NPX>
-__device__ __forceinline__ void eval_prism(const float4* __restrict__ rec, const double* __restrict__ rec64,
-                                           float jf, float fi, double (&acc)[NPX])
+// ---- per-warp preparation of one survivor (executed by ONE lane per particle) -----------------------------------------
+// Re-base the particle's fp64 coefficients from its own reference pixel (jc, ic) to the warp's sub-tile origin
+// (wx0, wy0) and round to fp32 there: all later arithmetic uses pixel offsets 0..15 / 0..7.
+__device__ __forceinline__ void fill_slot(float4* __restrict__ slot, const float4* __restrict__ rec, int k, int wx0, int wy0)
 {
-    const float4 h0 = rec[0];
-    const float4 h1 = rec[1];
-    const uint32_t flags = __float_as_uint(h1.x);
+    const float4 h2 = rec[2];                                  // flags, dn | K, -, id
+    const int4 h3 = *reinterpret_cast<const int4*>(rec + 3);   // jc, ic
+    const uint32_t flags = __float_as_uint(h2.x);
+    const double oj = (double)(wx0 - h3.x), oi = (double)(wy0 - h3.y);
+    const double* c = reinterpret_cast<const double*>(rec + 4);
+    if (!(flags & kFlagPrism)) {
+        // w(dj, di) = F1 - (A dj^2 + B dj di + C di^2 + D dj + E di) with dj = oj + lx, di = oi + ly
+        const double A = c[0], B = c[1], C = c[2], D = c[3], E = c[4], F1 = c[5];
+        double2* s = reinterpret_cast<double2*>(slot);
+        s[0] = make_double2(-A, -B);                                              // c20, c11
+        s[1] = make_double2(-C, -fma(2.0 * A, oj, fma(B, oi, D)));                // c02, c10
+        s[2] = make_double2(-fma(B, oj, fma(2.0 * C, oi, E)),                     // c01
+                            F1 - fma(fma(A, oj, fma(B, oi, D)), oj, fma(C, oi, E) * oi));   // c00
+        slot[6] = make_float4(h2.x, h2.y, 0.0f, __int_as_float(k));
+        return;
+    }
     const int ns = (flags >> 8) & 7;
-    const float margin = h1.z;
-    const float dj = jf - h0.x, di = fi - h0.y;
-    float exs[NPX], ens[NPX], exr[NPX], enr[NPX];
+    float ex[6], en[6], u[6], v[6];
+    float margin = 0.0f;
 #pragma unroll
-    for (int k = 0; k < NPX; ++k) { exs[k] = 3.0e38f; ens[k] = -3.0e38f; exr[k] = 3.0e38f; enr[k] = -3.0e38f; }
-    int q = 0;
-#pragma unroll 1
-    for (; q < ns; ++q) {
-        const float4 s = rec[2 + q];                   // U, V, Cx, Cn
-        const float ek = fmaf(-s.y, di, s.z), nk = fmaf(-s.y, di, s.w);
-#pragma unroll
-        for (int k = 0; k < NPX; ++k) {
-            const float djk = dj + (float)k;
-            exs[k] = fminf(exs[k], fmaf(-s.x, djk, ek));
-            ens[k] = fmaxf(ens[k], fmaf(-s.x, djk, nk));
-        }
+    for (int q = 0; q < 6; ++q) {
+        const double2 uv = *reinterpret_cast<const double2*>(c + 4 * q);
+        const double2 xn = *reinterpret_cast<const double2*>(c + 4 * q + 2);
+        const double m = fma(uv.x, oj, uv.y * oi);
+        float fu = (float)uv.x, fv = (float)uv.y, fx = (float)(xn.x - m), fn = (float)(xn.y - m);
+        const bool inert = ((flags >> (16 + q)) & 1u) || !(fabsf(fu) < 1.0e30f) || !(fabsf(fv) < 1.0e30f) ||
+                           !(fabsf(fx) < 1.0e30f) || !(fabsf(fn) < 1.0e30f);
+        if (inert) { fu = 0.0f; fv = 0.0f; fx = 3.0e38f; fn = -3.0e38f; }
+        else if (q < ns) margin = fmaxf(margin, fabsf(fx) + fabsf(fn) + 15.0f * fabsf(fu) + 7.0f * fabsf(fv));
+        u[q] = fu; v[q] = fv; ex[q] = fx; en[q] = fn;
     }
-#pragma unroll 1
-    for (; q < 6; ++q) {
-        const float4 s = rec[2 + q];
-        const float ek = fmaf(-s.y, di, s.z), nk = fmaf(-s.y, di, s.w);
+    slot[0] = make_float4(ex[0], ex[1], ex[2], ex[3]);
+    slot[1] = make_float4(ex[4], ex[5], en[0], en[1]);
+    slot[2] = make_float4(en[2], en[3], en[4], en[5]);
+    slot[3] = make_float4(u[0], u[1], u[2], u[3]);
+    slot[4] = make_float4(u[4], u[5], v[0], v[1]);
+    slot[5] = make_float4(v[2], v[3], v[4], v[5]);
+    slot[6] = make_float4(h2.x, h2.y, margin * 4.0e-7f, __int_as_float(k));
+}
+
+// ---- thickness, 4 pixels of one row per lane --------------------------------------------------------------------------
+struct LaneGeom {
+    float2 nlx[4];     // (-lx_k, -lx_k), lx_k = 4 (lane & 3) + k : pixel column offset inside the warp sub-tile
+    float2 nly;        // (-ly, -ly),     ly = lane >> 2
+    double lxd[4], lyd;
+};
+
+__device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ slot, const LaneGeom& g, double (&acc)[4])
+{
+    const double2 c0 = *reinterpret_cast<const double2*>(slot + 0);   // c20, c11
+    const double2 c1 = *reinterpret_cast<const double2*>(slot + 1);   // c02, c10
+    const double2 c2 = *reinterpret_cast<const double2*>(slot + 2);   // c01, c00
+    const double K = (double)slot[6].y;
+    const double b1 = fma(c0.y, g.lyd, c1.y);
+    const double cc = fma(fma(c1.x, g.lyd, c2.x), g.lyd, c2.y);
 #pragma unroll
-        for (int k = 0; k < NPX; ++k) {
-            const float djk = dj + (float)k;
-            exr[k] = fminf(exr[k], fmaf(-s.x, djk, ek));
-            enr[k] = fmaxf(enr[k], fmaf(-s.x, djk, nk));
-        }
-    }
-    float t[NPX];
-    bool any = false;
-    unsigned fmask = 0u;
-#pragma unroll
-    for (int k = 0; k < NPX; ++k) {
-        t[k] = fminf(exs[k], exr[k]) - fmaxf(ens[k], enr[k]);
-        bool f = false;
-        if (ns > 0) {
-            f = (t[k] > -2.0f * margin) && (exs[k] < exr[k] + margin || ens[k] > enr[k] - margin);
-            f = f || (flags & kFlagAllF64);
-        }
-        if (f) fmask |= 1u << k;
-        any = any || f;
-        t[k] = fmaxf(t[k], 0.0f);
-    }
-    const double dn = (double)h1.y;
-    if (any) {
-        const uint32_t id = __float_as_uint(h1.w);
-        const double* r64 = rec64 + (size_t)id * kRec64Doubles;
-        const double djd = (double)dj, did = (double)di;
-#pragma unroll
-        for (int k = 0; k < NPX; ++k) {
-            if ((fmask >> k) & 1u) acc[k] = fma(prism_t64(r64, flags >> 16, djd + (double)k, did), dn, acc[k]);
-            else acc[k] = fma((double)t[k], dn, acc[k]);
-        }
-    } else {
-#pragma unroll
-        for (int k = 0; k < NPX; ++k) acc[k] = fma((double)t[k], dn, acc[k]);
+    for (int k = 0; k < 4; ++k) {
+        const double w = fma(fma(c0.x, g.lxd[k], b1), g.lxd[k], cc);      // 1 - d^T S d
+        const float t = fast_sqrt(fmaxf((float)w, 0.0f));
+        acc[k] = fma((double)t, K, acc[k]);
     }
 }
 
-// ---- list ordering ----------------------------------------------------------------------------------------------
+// NS = number of steep slabs (they come first); NS == 0: no pixel can need refinement.
+template <int NS>
+__device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, const float4* __restrict__ s_rec,
+                                           const LaneGeom& g, int wx0, int wy0, int lane, double (&acc)[4])
+{
+    const float4 a0 = slot[0], a1 = slot[1], a2 = slot[2], a3 = slot[3], a4 = slot[4], a5 = slot[5], a6 = slot[6];
+    const float2 v01 = make_float2(a4.z, a4.w), v23 = make_float2(a5.x, a5.y), v45 = make_float2(a5.z, a5.w);
+    const float2 u01 = make_float2(a3.x, a3.y), u23 = make_float2(a3.z, a3.w), u45 = make_float2(a4.x, a4.y);
+    // row terms: value of every plane at this lane's row, column offset 0
+    const float2 ek01 = ffma2(v01, g.nly, make_float2(a0.x, a0.y));
+    const float2 ek23 = ffma2(v23, g.nly, make_float2(a0.z, a0.w));
+    const float2 ek45 = ffma2(v45, g.nly, make_float2(a1.x, a1.y));
+    const float2 nk01 = ffma2(v01, g.nly, make_float2(a1.z, a1.w));
+    const float2 nk23 = ffma2(v23, g.nly, make_float2(a2.x, a2.y));
+    const float2 nk45 = ffma2(v45, g.nly, make_float2(a2.z, a2.w));
+    const double dn = (double)a6.y;
+    float t[4];
+    unsigned fmask = 0u;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float2 e01 = ffma2(u01, g.nlx[k], ek01), e23 = ffma2(u23, g.nlx[k], ek23), e45 = ffma2(u45, g.nlx[k], ek45);
+        const float2 n01 = ffma2(u01, g.nlx[k], nk01), n23 = ffma2(u23, g.nlx[k], nk23), n45 = ffma2(u45, g.nlx[k], nk45);
+        float tk;
+        if (NS == 0) {
+            const float ex = fminf(min3(e01.x, e01.y, e23.x), min3(e23.y, e45.x, e45.y));
+            const float en = fmaxf(max3(n01.x, n01.y, n23.x), max3(n23.y, n45.x, n45.y));
+            tk = ex - en;
+        } else {
+            const float margin = a6.z;
+            float exs, ens, exr, enr;
+            if (NS == 1) {
+                exs = e01.x; ens = n01.x;
+                exr = fminf(min3(e01.y, e23.x, e23.y), fminf(e45.x, e45.y));
+                enr = fmaxf(max3(n01.y, n23.x, n23.y), fmaxf(n45.x, n45.y));
+            } else {
+                exs = fminf(e01.x, e01.y); ens = fmaxf(n01.x, n01.y);
+                exr = fminf(fminf(e23.x, e23.y), fminf(e45.x, e45.y));
+                enr = fmaxf(fmaxf(n23.x, n23.y), fmaxf(n45.x, n45.y));
+            }
+            tk = fminf(exs, exr) - fmaxf(ens, enr);
+            // a steep slab is (within its fp32 error) the active entry or exit face and the pixel is not clearly outside
+            if ((tk > -2.0f * margin) && (exs < exr + margin || ens > enr - margin)) fmask |= 1u << k;
+        }
+        t[k] = fmaxf(tk, 0.0f);
+    }
+    if (NS != 0) {
+        const uint32_t flags = __float_as_uint(a6.x);
+        if (flags & kFlagAllF64) fmask = 0xfu;
+        if (fmask) {
+            const float4* rec = s_rec + __float_as_int(a6.w) * kRecStride4;
+            const int4 h3 = *reinterpret_cast<const int4*>(rec + 3);
+            const double* r64 = reinterpret_cast<const double*>(rec + 4);
+            const double dj = (double)(wx0 + 4 * (lane & 3) - h3.x), di = (double)(wy0 + (lane >> 2) - h3.y);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                if ((fmask >> k) & 1u) acc[k] = fma(prism_t64(r64, flags >> 16, dj + (double)k, di), dn, acc[k]);
+                else acc[k] = fma((double)t[k], dn, acc[k]);
+            }
+            return;
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) acc[k] = fma((double)t[k], dn, acc[k]);
+}
+
+// ---- list ordering ----------------------------------------------------------------------------------------------------
 // In-place ascending sort of list[0..L) in GLOBAL memory by one CTA (only for lists longer than kSortCap):
 // bitonic network in its "all comparators ascending" form, so that virtual +inf padding beyond L never moves.
 __device__ void sort_global(uint32_t* a, uint32_t L)
@@ -182,14 +258,13 @@ __device__ void sort_global(uint32_t* a, uint32_t L)
     }
 }
 
-constexpr int kWarps = kComposeThreads / 32;
-
 template <bool OPD, bool FIELD, bool RAMP>
 __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeArgs a)
 {
-    __shared__ __align__(16) float4 s_rec[kChunk * 8];          // staged 128-byte records
-    __shared__ uint32_t s_ids[kSortCap];                        // this tile's list, ascending
-    __shared__ uint8_t s_surv[kWarps][kChunk];                  // per-warp survivors of the sub-tile cull
+    extern __shared__ __align__(16) unsigned char smem[];
+    float4* s_rec = reinterpret_cast<float4*>(smem);                               // staged records (padded stride)
+    uint32_t* s_ids = reinterpret_cast<uint32_t*>(smem + kSmemRec);               // this tile's list, ascending
+    float4* s_slots = reinterpret_cast<float4*>(smem + kSmemRec + kSmemIds);      // per-warp survivor slots
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int tpf = a.ntx * a.nty;
@@ -202,10 +277,10 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeA
     const uint32_t L = overflow ? 0u : a.offset[tile + 1] - beg;
     uint32_t* glist = a.list + beg;
 
-    // ---- H4 (second half): canonical order ------------------------------------------------------------------
+    // ---- H4 (second half): canonical order ------------------------------------------------------------------------
     const bool in_smem = L <= (uint32_t)kSortCap;
     if (in_smem) {
-        uint32_t* s_in = reinterpret_cast<uint32_t*>(s_rec);    // kChunk * 32 words >= kSortCap
+        uint32_t* s_in = reinterpret_cast<uint32_t*>(s_slots);   // kSmemSlots >= kSmemIds
         for (uint32_t k = tid; k < L; k += kComposeThreads) s_in[k] = glist[k];
         __syncthreads();
         for (uint32_t k = tid; k < L; k += kComposeThreads) {
@@ -220,47 +295,71 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeA
         sort_global(glist, L);
     }
 
-    // ---- pixel ownership ----------------------------------------------------------------------------------------
+    // ---- pixel ownership ------------------------------------------------------------------------------------------------
     const int wx0 = tx * kTile + (wid & 1) * 16, wy0 = ty * kTile + (wid >> 1) * 8;   // warp sub-tile origin
-    const int j = wx0 + (lane & 3) * 4, i = wy0 + (lane >> 2);
-    const float jf = (float)j, fi = (float)i;
-    const double jd = (double)j, id = (double)i;
+    const int lx = (lane & 3) * 4, ly = lane >> 2;
+    const int j = wx0 + lx, i = wy0 + ly;
+    LaneGeom g;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        g.nlx[k] = make_float2(-(float)(lx + k), -(float)(lx + k));
+        g.lxd[k] = (double)(lx + k);
+    }
+    g.nly = make_float2(-(float)ly, -(float)ly);
+    g.lyd = (double)ly;
+    // sub-tile rectangle (pixel centres) for the cull: centre in pixel-index coordinates, half extents 7.5 x 3.5
+    const float rcx = (float)wx0 + 7.5f, rcy = (float)wy0 + 3.5f;
+    float4* my_slots = s_slots + wid * 32 * kSlotStride4;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
 
     for (uint32_t c0 = 0; c0 < L; c0 += kChunk) {
         const int nC = (int)min((uint32_t)kChunk, L - c0);
         if (c0 > 0) __syncthreads();                             // everyone is done with the previous chunk
-        for (int u = tid; u < nC * 8; u += kComposeThreads) {
-            const uint32_t pid = in_smem ? s_ids[c0 + (u >> 3)] : glist[c0 + (u >> 3)];
-            cp_async16(&s_rec[u], a.rec32 + (size_t)pid * kRecWords + (u & 7) * 4);
+        for (int u = tid; u < nC * 16; u += kComposeThreads) {
+            const uint32_t pid = in_smem ? s_ids[c0 + (u >> 4)] : glist[c0 + (u >> 4)];
+            cp_async16(&s_rec[(u >> 4) * kRecStride4 + (u & 15)], a.rec + (size_t)pid * kRecWords + (u & 15) * 4);
         }
         cp_async_wait_all();
         __syncthreads();
-        // warp-level cull: keep the staged particles whose pixel bounding box meets this warp's 16 x 8 sub-tile
-        int ns = 0;
+
         for (int base = 0; base < nC; base += 32) {
+            // ---- cull + re-base: lane <-> staged particle base + lane ------------------------------------------------
             const int k = base + lane;
             bool keep = false;
+            const float4* rec = s_rec + k * kRecStride4;
             if (k < nC) {
-                const float4 h0 = s_rec[k * 8];
-                const uint32_t bx = __float_as_uint(h0.z), by = __float_as_uint(h0.w);
+                const float4 h0 = rec[0], h1 = rec[1];           // cxp, cyp, ax, ay | ha, hb, bbx, bby
+                const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
                 const int pj0 = bx & 0xffff, pj1 = bx >> 16, pi0 = by & 0xffff, pi1 = by >> 16;
                 keep = pj0 <= wx0 + 15 && pj1 >= wx0 && pi0 <= wy0 + 7 && pi1 >= wy0;
+                // separating-axis test against the particle's oriented box (the silhouette lies inside it)
+                const float ddx = rcx - h0.x, ddy = rcy - h0.y;
+                const float pa = fabsf(ddx * h0.z + ddy * h0.w), pb = fabsf(ddy * h0.z - ddx * h0.w);
+                const float ra = 7.5f * fabsf(h0.z) + 3.5f * fabsf(h0.w), rb = 7.5f * fabsf(h0.w) + 3.5f * fabsf(h0.z);
+                keep = keep && pa <= h1.x + ra && pb <= h1.y + rb;
             }
             const unsigned m = __ballot_sync(0xffffffffu, keep);
-            if (keep) s_surv[wid][ns + __popc(m & ((1u << lane) - 1u))] = (uint8_t)k;
-            ns += __popc(m);
-        }
-        __syncwarp();
-        for (int s = 0; s < ns; ++s) {
-            const float4* rec = &s_rec[(int)s_surv[wid][s] * 8];
-            const uint32_t flags = __float_as_uint(rec[1].x);
-            if (flags & kFlagPrism) eval_prism<4>(rec, a.rec64, jf, fi, acc);
-            else eval_ellipsoid<4>(rec, jd, id, acc);
+            if (keep) fill_slot(my_slots + __popc(m & ((1u << lane) - 1u)) * kSlotStride4, rec, k, wx0, wy0);
+            __syncwarp();
+            // ---- all lanes walk the survivors in ascending order ------------------------------------------------------
+            const int nsv = __popc(m);
+            for (int s = 0; s < nsv; ++s) {
+                const float4* slot = my_slots + s * kSlotStride4;
+                const uint32_t flags = __float_as_uint(slot[6].x);
+                if (!(flags & kFlagPrism)) {
+                    eval_ellipsoid(slot, g, acc);
+                } else {
+                    const int ns = (flags >> 8) & 7;
+                    if (ns == 0) eval_prism<0>(slot, s_rec, g, wx0, wy0, lane, acc);
+                    else if (ns == 1) eval_prism<1>(slot, s_rec, g, wx0, wy0, lane, acc);
+                    else eval_prism<2>(slot, s_rec, g, wx0, wy0, lane, acc);
+                }
+            }
+            __syncwarp();
         }
     }
 
-    // ---- H6/H7: write-out straight from the registers --------------------------------------------------------------
+    // ---- H6/H7: write-out straight from the registers ----------------------------------------------------------------------
     if (i >= a.H || j >= a.W) return;
     const size_t row = ((size_t)b * a.H + i) * a.W;
     const bool vec = ((a.W & 3) == 0);                           // then j + 3 < W and the row base is 16-byte aligned
@@ -306,53 +405,68 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeA
     }
 }
 
+template <bool OPD, bool FIELD, bool RAMP>
+static cudaError_t launch_variant(const ComposeArgs& a, unsigned grid, cudaStream_t stream)
+{
+    // opt in to > 48 KB dynamic shared memory (cheap, idempotent; per device, so done on every launch)
+    cudaError_t e = cudaFuncSetAttribute(k_compose_tile<OPD, FIELD, RAMP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         kSmemBytes);
+    if (e != cudaSuccess) return e;
+    k_compose_tile<OPD, FIELD, RAMP><<<grid, kComposeThreads, kSmemBytes, stream>>>(a);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float* d_opd, float2* d_field)
 {
     (void)N;
     ComposeArgs a;
-    a.rec32 = c->rec32; a.rec64 = c->rec64; a.offset = c->offset; a.list = c->list; a.optics = c->optics;
+    a.rec = c->rec; a.offset = c->offset; a.list = c->list; a.optics = c->optics;
     a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.status = c->status;
     a.opd = d_opd; a.field = d_field;
     a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
     a.ramp_y_on = 1;
     const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
-    const dim3 blk(kComposeThreads);
-    if (d_opd != nullptr && d_field == nullptr) k_compose_tile<true, false, false><<<grid, blk, 0, c->stream>>>(a);
-    else if (d_opd == nullptr && !has_ramp) k_compose_tile<false, true, false><<<grid, blk, 0, c->stream>>>(a);
-    else if (d_opd == nullptr && has_ramp) k_compose_tile<false, true, true><<<grid, blk, 0, c->stream>>>(a);
-    else if (!has_ramp) k_compose_tile<true, true, false><<<grid, blk, 0, c->stream>>>(a);
-    else k_compose_tile<true, true, true><<<grid, blk, 0, c->stream>>>(a);
-    return cudaGetLastError();
+    if (d_opd != nullptr && d_field == nullptr) return launch_variant<true, false, false>(a, grid, c->stream);
+    if (d_opd == nullptr && !has_ramp) return launch_variant<false, true, false>(a, grid, c->stream);
+    if (d_opd == nullptr && has_ramp) return launch_variant<false, true, true>(a, grid, c->stream);
+    if (!has_ramp) return launch_variant<true, true, false>(a, grid, c->stream);
+    return launch_variant<true, true, true>(a, grid, c->stream);
 }
 
-// ---- measured alternative: paper-style scatter-add with global atomics ------------------------
-// One warp per particle walks the particle's pixel bounding box and atomicAdd's (n_p - n_m) t into the frame.
-// Summation order, hence the last bits, depend on scheduling: NOT deterministic.  The frame must be zeroed first.
-__global__ void __launch_bounds__(256) k_compose_atomic(const float* __restrict__ rec32, const double* __restrict__ rec64,
-                                                        const int4* __restrict__ tbox, const int* __restrict__ pframe,
-                                                        long long N, int H, int W, float* __restrict__ opd)
+// ---- measured alternative: paper-style scatter-add with global atomics ----------------------------
+// One warp per particle walks the particle's pixel bounding box and atomicAdd's (n_p - n_m) t into the frame (fp64
+// thickness per pixel, fp32 atomics).  Summation order, hence the last bits, depend on scheduling: NOT deterministic.
+// The frame must be zeroed first.
+__global__ void __launch_bounds__(256) k_compose_atomic(const float* __restrict__ recs, const int4* __restrict__ tbox,
+                                                        const int* __restrict__ pframe, long long N, int H, int W,
+                                                        float* __restrict__ opd)
 {
     const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (n >= N) return;
     if (tbox[n].x > tbox[n].y) return;
-    const float4* rec = reinterpret_cast<const float4*>(rec32 + (size_t)n * kRecWords);
-    const float4 h0 = rec[0];
-    const uint32_t bx = __float_as_uint(h0.z), by = __float_as_uint(h0.w);
+    const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)n * kRecWords);
+    const float4 h1 = rec[1], h2 = rec[2];
+    const int4 h3 = *reinterpret_cast<const int4*>(rec + 3);
+    const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
     const int j0 = bx & 0xffff, j1 = bx >> 16, i0 = by & 0xffff, i1 = by >> 16;
-    const uint32_t flags = __float_as_uint(rec[1].x);
+    const uint32_t flags = __float_as_uint(h2.x);
+    const double* c = reinterpret_cast<const double*>(rec + 4);
+    const double K = (double)h2.y;
     const int bw = j1 - j0 + 1, np = bw * (i1 - i0 + 1);
     float* frame = opd + (size_t)pframe[n] * H * W;
     for (int q = lane; q < np; q += 32) {
         const int i = i0 + q / bw, j = j0 + q % bw;
-        double acc[1] = {0.0};
+        const double dj = (double)(j - h3.x), di = (double)(i - h3.y);
+        double v;
         if (flags & kFlagPrism) {
-            eval_prism<1>(rec, rec64, (float)j, (float)i, acc);
+            v = K * prism_t64(c, flags >> 16, dj, di);
         } else {
-            eval_ellipsoid<1>(rec, (double)j, (double)i, acc);
+            const double w = c[5] - fma(fma(c[0], dj, fma(c[1], di, c[3])), dj, fma(c[2], di, c[4]) * di);
+            v = K * (double)fast_sqrt(fmaxf((float)w, 0.0f));
         }
-        const float v = (float)acc[0];
-        if (v != 0.0f) atomicAdd(&frame[(size_t)i * W + j], v);
+        const float f = (float)v;
+        if (f != 0.0f) atomicAdd(&frame[(size_t)i * W + j], f);
     }
 }
 
@@ -361,8 +475,8 @@ cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd)
     cudaError_t e = cudaMemsetAsync(d_opd, 0, sizeof(float) * (size_t)B * c->H * c->W, c->stream);
     if (e != cudaSuccess || N == 0) return e;
     const long long threads = N * 32;
-    k_compose_atomic<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(c->rec32, c->rec64, c->tbox, c->pframe, N,
-                                                                              c->H, c->W, d_opd);
+    k_compose_atomic<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(c->rec, c->tbox, c->pframe, N, c->H, c->W,
+                                                                              d_opd);
     return cudaGetLastError();
 }
 

@@ -125,7 +125,7 @@ int osog_destroy(osog_ctx* c)
     DeviceGuard g(c->device);
     if (c->has_plan_one) cufftDestroy(c->plan_one);
     if (c->has_plan_batch) cufftDestroy(c->plan_batch);
-    cudaFree(c->rec32); cudaFree(c->rec64); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
+    cudaFree(c->rec); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
     cudaFree(c->offset); cudaFree(c->list); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
     cudaFree(c->status); cudaFree(c->field);
     if (c->h_status) cudaFreeHost(c->h_status);
@@ -163,8 +163,7 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     const size_t np = (size_t)c->max_particles, npx = (size_t)c->H * c->W;
     cudaError_t e = cudaSuccess;
     auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
-    A(dalloc(&c->rec32, np * kRecWords));
-    A(dalloc(&c->rec64, np * kRec64Doubles));
+    A(dalloc(&c->rec, np * kRecWords));
     A(dalloc(&c->tbox, np));
     A(dalloc(&c->pframe, np));
     A(dalloc(&c->count, (size_t)c->max_tiles));

@@ -11,15 +11,14 @@ namespace osog {
 // ---- build-time constants -----------------------------------------------------------------------------------
 constexpr int kTile = 32;              // binning tile edge T (pixels); one CTA composes one tile
 constexpr int kComposeThreads = 256;   // 8 warps; each warp owns a 16 x 8 pixel sub-tile, each lane 4 x 1 pixels
-constexpr int kChunk = 96;             // particle records staged in shared memory per pass
+constexpr int kChunk = 64;             // particle records staged in shared memory per pass
 constexpr int kSortCap = 2048;         // longest tile list sorted in shared memory (longer: sorted in global memory)
-constexpr int kRecWords = 32;          // 128-byte fp32 record per particle
-constexpr int kRec64Doubles = 24;      // fp64 plane coefficients per prism (refinement path)
+constexpr int kRecWords = 64;          // 256-byte record per particle: 16 header words + up to 24 doubles
 constexpr double kBBoxPadPx = 1.0 / 1024.0;   // delta of DESIGN.md B2
-constexpr float kSteepSlope = 8.0f;    // slabs steeper than this (|n_xy| / |n_z|) are refined in fp64 where active
+constexpr float kSteepSlope = 16.0f;   // slabs steeper than this (|n_xy| / |n_z|) are refined in fp64 where active
 constexpr double kAllF64Slope = 1.0e4; // a slab steeper than this (or vertical) sends the whole particle to fp64
 
-// record header flags (word 4)
+// record header flags (word 8)
 constexpr uint32_t kFlagPrism = 1u;
 constexpr uint32_t kFlagAllF64 = 16u;
 // bits 8..10: number of steep slabs (they come first); bits 16..21: per-slab "vertical" (n_z == 0) mask
@@ -58,8 +57,7 @@ struct osog_ctx {
     int last_B;
     long long last_tiles;
     // scratch (device)
-    float* rec32;                   // [max_particles][32]
-    double* rec64;                  // [max_particles][24]
+    float* rec;                     // [max_particles][kRecWords]
     int4* tbox;                     // [max_particles] tile range tx0, tx1, ty0, ty1 (tx0 > tx1: not listed)
     int* pframe;                    // [max_particles] frame of the particle
     uint32_t* count;                // [max_tiles] per-tile count, reused as the fill cursor
