@@ -1,0 +1,135 @@
+"""GPU edge cases through the C ABI: empty input, ragged frames, off-frame and invalid particles, a tile list
+longer than the shared-memory sort capacity, pair-list overflow, vertical prism faces (fp64 path), batches with
+per-frame optics (more than one optics chunk), y tilt, all-pass pupil (Parseval), and argument errors."""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+from workloads import make_config, make_scene
+from test_gpu_parity import check_against_oracle, render_all, og, o  # noqa: F401  (fixtures)
+
+pytestmark = pytest.mark.gpu
+
+
+def _mixed(n, H, W, seed, spread=1.0, B=1):
+    rng = np.random.default_rng(seed)
+    q = rng.standard_normal((n, 4)); q /= np.linalg.norm(q, axis=1, keepdims=True)
+    kind = (rng.uniform(size=n) < 0.5).astype(np.uint8)
+    s = rng.uniform(0.4, 2.5, n)
+    d = np.where(kind[:, None] == 1, np.stack([s, s * rng.uniform(1, 3, n), 0.5 * s], 1), rng.uniform(0.3, 3.0, (n, 3)))
+    return dict(cx=rng.uniform(-1.0, W * 0.1 * spread + 1.0, n), cy=rng.uniform(-1.0, H * 0.1 * spread + 1.0, n),
+                qw=q[:, 0], qx=q[:, 1], qy=q[:, 2], qz=q[:, 3], d0=d[:, 0], d1=d[:, 1], d2=d[:, 2],
+                n_p=rng.uniform(1.36, 1.5, n), kind=kind)
+
+
+def test_zero_particles_uniform_field_and_intensity(og, o):
+    sc = make_scene("empty", 96, 128, dict(cx=[], cy=[], d0=[], d1=[], d2=[], n_p=[]))
+    g = render_all(og, sc)
+    assert np.all(g["opd"] == 0.0)
+    assert np.all(g["field"] == 1.0 + 0.0j)
+    assert np.abs(g["intensity"] - 1.0).max() <= 1e-6          # P9: N = 0, no ramp -> I == 1
+    assert g["bins"][2].size == 0 and g["status"] == (0, 0, 0)
+
+
+@pytest.mark.parametrize("H,W", [(70, 50), (33, 97), (1, 5), (130, 4)])
+def test_ragged_frames_and_off_frame_particles(og, o, H, W):
+    sc = make_scene("ragged", H, W, _mixed(40, H, W, seed=H * 1000 + W), tilt_x_rad=0.05, tilt_y_rad=-0.03)
+    check_against_oracle(og, o, sc)
+
+
+def test_invalid_particles_are_skipped_and_reported(og, o):
+    cols = _mixed(30, 64, 64, seed=5)
+    cols["d1"][3] = -1.0
+    cols["cx"][7] = np.nan
+    cols["qy"][11] = np.inf
+    cols["kind"][13] = 7
+    cols["d0"][17] = 0.0
+    sc = make_scene("bad", 64, 64, cols)
+    g, _ = check_against_oracle(og, o, sc)
+    assert g["status"][1] & og.OSOG_WBADPARTICLE
+
+
+def test_list_longer_than_shared_sort_capacity(og, o):
+    """2,600 small spheres inside one 32 x 32 tile: the tile's list is sorted in global memory and composed
+    in many chunks."""
+    rng = np.random.default_rng(11)
+    n = 2600
+    cols = dict(cx=rng.uniform(3.3, 6.2, n), cy=rng.uniform(3.3, 6.2, n), d0=np.full(n, 0.12), d1=np.full(n, 0.12),
+                d2=np.full(n, 0.12), n_p=rng.uniform(1.36, 1.5, n))
+    sc = make_scene("crowd", 96, 96, cols)
+    g, _ = check_against_oracle(og, o, sc)
+    assert g["bins"][0].max() > 2048
+
+
+def test_pair_list_overflow_is_reported_and_frames_zeroed(og):
+    sc = make_config(2, n_override=300)
+    ctx = og.Context(sc.H, sc.W, sc.N, max_pairs=50)
+    P = og.Particles.from_scene(sc)
+    opt = og.optics_from_scene(sc)
+    opd = ctx.render_opd(P, opt)
+    r, bits, pairs = ctx.status()
+    assert r == og.OSOG_ECAPACITY and (bits & og.OSOG_WOVERFLOW) and pairs > 50
+    assert float(opd.abs().max()) == 0.0
+    ctx.close()
+    ctx = og.Context(sc.H, sc.W, sc.N, max_pairs=pairs)      # the reported need is exactly enough
+    ctx.render_opd(P, opt)
+    assert ctx.status()[0] == 0
+    ctx.close()
+
+
+def test_prisms_with_vertical_faces_take_the_fp64_path(og, o):
+    """Identity and 90-degree rotations give face normals with n_z == 0 exactly (thickness is discontinuous at those
+    faces); centres are placed so that no pixel centre lies within 1e-3 um of a vertical face."""
+    r = np.sqrt(0.5)
+    cols = dict(cx=[3.213, 9.047, 6.131], cy=[3.377, 4.021, 9.563], qw=[1.0, r, r], qx=[0.0, r, 0.0], qy=[0.0, 0.0, r],
+                qz=[0.0, 0.0, 0.0], d0=[2.03, 1.57, 1.21], d1=[3.3, 4.1, 2.9], d2=[1.0, 0.8, 0.6], n_p=[1.45, 1.40, 1.42],
+                kind=np.ones(3, np.uint8))
+    check_against_oracle(og, o, make_scene("vertical", 128, 128, cols))
+
+
+def test_batch_with_per_frame_optics_across_optics_chunks(og, o):
+    B, n = 19, 60                                             # 19 frames > one 16-frame optics chunk
+    rng = np.random.default_rng(3)
+    parts = [_mixed(n, 64, 96, seed=100 + b) for b in range(B)]
+    cols = {k: np.concatenate([p[k] for p in parts]) for k in parts[0]}
+    sc = make_scene("batch", 64, 96, cols, lam=rng.uniform(0.45, 0.65, B), NA=rng.uniform(0.3, 0.8, B), seed=77,
+                    frame_start=np.arange(B + 1) * n, tilt_x_rad=0.1, read_noise_sigma=0.01)
+    check_against_oracle(og, o, sc)
+
+
+def test_partial_batch_uses_the_single_frame_plan(og, o):
+    sc = make_config(5, n_override=200)
+    import paper_2606_21381_b200 as m
+    ctx = m.Context(sc.H, sc.W, sc.N, max_frames=sc.B + 3)
+    P = m.Particles.from_scene(sc)
+    I = ctx.render_intensity(P, m.optics_from_scene(sc)).cpu().numpy().astype(np.float64)
+    Iref = o.render_intensity(sc)
+    assert np.abs(I - Iref).max() <= 1e-4 * Iref.mean()
+    ctx.close()
+
+
+def test_all_pass_pupil_conserves_energy(og, o):
+    sc = make_config(2, n_override=200)
+    g, _ = check_against_oracle(og, o, sc, pupil=False, what=("field", "intensity"))
+    assert abs(g["intensity"].sum() / (sc.H * sc.W) - 1.0) < 1e-5      # P11: sum |U|^2 = H W for |U| = 1
+
+
+def test_argument_errors(og):
+    sc = make_config(1)
+    ctx = og.Context(sc.H, sc.W, 10)                          # max_particles 10 < 64
+    P = og.Particles.from_scene(sc)
+    opt = og.optics_from_scene(sc)
+    with pytest.raises(og.OsogError) as e:
+        ctx.render_opd(P, opt)
+    assert e.value.code == og.OSOG_EINVAL
+    ctx.close()
+    ctx = og.Context(sc.H, sc.W, sc.N)
+    bad = og.make_optics(1, -0.1, 1.33, 0.55, 0.4)
+    with pytest.raises(og.OsogError):
+        ctx.render_opd(P, bad)
+    two = og.make_optics(2, 0.1, 1.33, 0.55, 0.4)             # B > max_frames
+    with pytest.raises(og.OsogError):
+        ctx.render_opd(P, two)
+    assert og.lib().osog_render_opd(ctx._ctx, C.byref(P.c), P.N, C.byref(opt), None) == og.OSOG_EINVAL
+    ctx.close()

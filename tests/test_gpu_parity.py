@@ -1,0 +1,96 @@
+"""GPU parity tests: libosog.so (through the C ABI binding) against the float64 CPU oracle on the same seeded
+inputs.  Bars (BASELINE.json north_star): bin offsets / lists bit-exact; OPD |g - o| <= 1e-5 um + 1e-5 |o|;
+complex field and intensity max abs error <= 1e-4 * mean(oracle intensity)."""
+import numpy as np
+import pytest
+
+from workloads import make_config, make_scene
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def og():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2606_21381_b200 as m
+    m.lib()                       # fails loudly if libosog.so is missing / cannot be built
+    return m
+
+
+@pytest.fixture(scope="module")
+def o():
+    from oracle import oracle
+    return oracle
+
+
+def render_all(og, sc, pupil=True, max_pairs=0):
+    import torch
+    ctx = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B, max_pairs=max_pairs)
+    P = og.Particles.from_scene(sc)
+    opt = og.optics_from_scene(sc, pupil_enabled=pupil)
+    out = {}
+    out["opd"] = ctx.render_opd(P, opt).cpu().numpy().astype(np.float64)
+    out["bins"] = ctx.debug_bins()
+    out["status"] = ctx.status()
+    out["field"] = ctx.render_field(P, opt).cpu().numpy().astype(np.complex128)
+    out["intensity"] = ctx.render_intensity(P, opt).cpu().numpy().astype(np.float64)
+    torch.cuda.synchronize()
+    ctx.close()
+    return out
+
+
+def check_against_oracle(og, o, sc, pupil=True, what=("bins", "opd", "field", "intensity")):
+    g = render_all(og, sc, pupil)
+    assert g["status"][0] == 0
+    ref = o.render_opd(sc)
+    if "bins" in what:
+        oc, oo, ol = o.binning(sc, og.osog_tile_size())
+        cnt, off, lst = g["bins"]
+        assert np.array_equal(off, oo), "tile offsets differ"
+        assert np.array_equal(cnt, oc), "tile counts differ"
+        assert np.array_equal(lst, ol), "tile lists differ"
+        assert g["status"][2] == ol.size
+    if "opd" in what:
+        err = np.abs(g["opd"] - ref)
+        tol = 1e-5 + 1e-5 * np.abs(ref)
+        assert np.all(err <= tol), f"OPD: {np.count_nonzero(err > tol)} pixels out, max {err.max():.3e}"
+    Uref = o.render_field(sc, opd=ref)
+    Iref = o.render_intensity(sc, U=Uref, pupil_enabled=pupil)
+    tol = 1e-4 * Iref.mean()
+    if "field" in what:
+        e = np.abs(g["field"] - Uref).max()
+        assert e <= tol, f"field max abs err {e:.3e} > {tol:.3e}"
+    if "intensity" in what:
+        e = np.abs(g["intensity"] - Iref).max()
+        assert e <= tol, f"intensity max abs err {e:.3e} > {tol:.3e}"
+    return g, ref
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_baseline_config_matches_oracle(og, o, k):
+    """BASELINE.json configs 1-5 at full size, in the launch configuration bench.py times."""
+    check_against_oracle(og, o, make_config(k))
+
+
+def test_run_to_run_bitwise_determinism(og):
+    import torch
+    sc = make_config(3, n_override=4000)
+    ctx = og.Context(sc.H, sc.W, sc.N)
+    P = og.Particles.from_scene(sc)
+    opt = og.optics_from_scene(sc)
+    a = ctx.render_field(P, opt).clone()
+    for _ in range(3):
+        b = ctx.render_field(P, opt)
+        assert torch.equal(torch.view_as_real(a), torch.view_as_real(b))
+    ctx.close()
+
+
+def test_atomic_alternative_within_tolerance(og, o):
+    sc = make_config(2)
+    ctx = og.Context(sc.H, sc.W, sc.N)
+    P = og.Particles.from_scene(sc)
+    g = ctx.render_opd_atomic(P, og.optics_from_scene(sc)).cpu().numpy().astype(np.float64)
+    ref = o.render_opd(sc)
+    assert np.all(np.abs(g - ref) <= 1e-5 + 1e-5 * np.abs(ref))
+    ctx.close()
