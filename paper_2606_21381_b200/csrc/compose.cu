@@ -1,6 +1,6 @@
 // H5-H7 of DESIGN.md: per-tile ordered composition.  One CTA per 32 x 32 pixel tile:
 //   1. sort the tile's particle list ascending (deterministic summation order) and write it back,
-//   2. stage the 256-byte particle records in shared memory with cp.async (chunks of kChunk),
+//   2. (from then on every warp is independent: no barrier) walk the list in batches of 32 particles,
 //   3. per warp (16 x 8 pixel sub-tile, 4 x 1 pixels per lane): one lane per staged particle tests the particle's
 //      pixel bounding box and oriented box against the sub-tile (ballot compaction keeps ascending order) and
 //      re-bases the survivor's fp64 coefficients to the sub-tile origin, rounding them to fp32 only there,
@@ -26,12 +26,10 @@ struct ComposeArgs {
 };
 
 constexpr int kWarps = kComposeThreads / 32;
-constexpr int kRecStride4 = kRecWords / 4 + 1;     // staged record stride in float4 (padded: conflict-free lane-per-record reads)
-constexpr int kSlotStride4 = 9;                    // survivor slot stride in float4 (7 used, padded to an odd count)
-constexpr int kSmemRec = kChunk * kRecStride4 * 16;
+constexpr int kSlotStride4 = 9;                    // survivor slot stride in float4 (8 used, odd stride: conflict-free lane-per-slot writes)
 constexpr int kSmemIds = kSortCap * 4;
 constexpr int kSmemSlots = kWarps * 32 * kSlotStride4 * 16;
-constexpr int kSmemBytes = kSmemRec + kSmemIds + kSmemSlots;
+constexpr int kSmemBytes = kSmemIds + kSmemSlots;
 
 // ---- small PTX helpers ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float fast_sqrt(float x)
@@ -95,49 +93,45 @@ __device__ __noinline__ double prism_t64(const double* r64, uint32_t vmask, doub
     return t > 0.0 ? t : 0.0;
 }
 
-// ---- per-warp preparation of one survivor (executed by ONE lane per particle) -----------------------------------------
+// ---- per-warp preparation of the survivors: work item = (survivor slot, slab q), one lane per item -------------------
 // Re-base the particle's fp64 coefficients from its own reference pixel (jc, ic) to the warp's sub-tile origin
 // (wx0, wy0) and round to fp32 there: all later arithmetic uses pixel offsets 0..15 / 0..7.
-__device__ __forceinline__ void fill_slot(float4* __restrict__ slot, const float4* __restrict__ rec, int k, int wx0, int wy0)
+// Slot layout (words): 0..5 Ex, 6..11 En, 12..17 U, 18..23 V, 24 flags, 25 dn, 26 -, 27 particle index, 28..29 margins.
+// Ellipsoid slot: doubles c20, c11, c02, c10, c01, c00 in words 0..11; 24 flags, 25 K, 27 particle index.
+__device__ __forceinline__ void rebase_item(float4* __restrict__ slot, const float* __restrict__ recs, int q, int wx0, int wy0)
 {
-    const float4 h2 = rec[2];                                  // flags, dn | K, -, id
-    const int4 h3 = *reinterpret_cast<const int4*>(rec + 3);   // jc, ic
+    float* sw = reinterpret_cast<float*>(slot);
+    const uint32_t pid = __float_as_uint(sw[27]);
+    const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)pid * kRecWords);
+    const float4 h2 = __ldg(rec + 2);                                  // flags, dn | K, -, id
+    const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));     // jc, ic
     const uint32_t flags = __float_as_uint(h2.x);
     const double oj = (double)(wx0 - h3.x), oi = (double)(wy0 - h3.y);
-    const double* c = reinterpret_cast<const double*>(rec + 4);
+    const double2* c = reinterpret_cast<const double2*>(rec + 4);
+    if (q == 0) { sw[24] = h2.x; sw[25] = h2.y; }
     if (!(flags & kFlagPrism)) {
+        if (q != 0) return;
         // w(dj, di) = F1 - (A dj^2 + B dj di + C di^2 + D dj + E di) with dj = oj + lx, di = oi + ly
-        const double A = c[0], B = c[1], C = c[2], D = c[3], E = c[4], F1 = c[5];
+        const double2 ab = __ldg(c), cd = __ldg(c + 1), ef = __ldg(c + 2);
+        const double A = ab.x, B = ab.y, C = cd.x, D = cd.y, E = ef.x, F1 = ef.y;
         double2* s = reinterpret_cast<double2*>(slot);
         s[0] = make_double2(-A, -B);                                              // c20, c11
         s[1] = make_double2(-C, -fma(2.0 * A, oj, fma(B, oi, D)));                // c02, c10
         s[2] = make_double2(-fma(B, oj, fma(2.0 * C, oi, E)),                     // c01
                             F1 - fma(fma(A, oj, fma(B, oi, D)), oj, fma(C, oi, E) * oi));   // c00
-        slot[6] = make_float4(h2.x, h2.y, 0.0f, __int_as_float(k));
         return;
     }
     const int ns = (flags >> 8) & 7;
-    float ex[6], en[6], u[6], v[6];
+    const double2 uv = __ldg(c + 2 * q), xn = __ldg(c + 2 * q + 1);
+    const double m = fma(uv.x, oj, uv.y * oi);
+    float fu = (float)uv.x, fv = (float)uv.y, fx = (float)(xn.x - m), fn = (float)(xn.y - m);
+    const bool inert = ((flags >> (16 + q)) & 1u) || !(fabsf(fu) < 1.0e30f) || !(fabsf(fv) < 1.0e30f) ||
+                       !(fabsf(fx) < 1.0e30f) || !(fabsf(fn) < 1.0e30f);
     float margin = 0.0f;
-#pragma unroll
-    for (int q = 0; q < 6; ++q) {
-        const double2 uv = *reinterpret_cast<const double2*>(c + 4 * q);
-        const double2 xn = *reinterpret_cast<const double2*>(c + 4 * q + 2);
-        const double m = fma(uv.x, oj, uv.y * oi);
-        float fu = (float)uv.x, fv = (float)uv.y, fx = (float)(xn.x - m), fn = (float)(xn.y - m);
-        const bool inert = ((flags >> (16 + q)) & 1u) || !(fabsf(fu) < 1.0e30f) || !(fabsf(fv) < 1.0e30f) ||
-                           !(fabsf(fx) < 1.0e30f) || !(fabsf(fn) < 1.0e30f);
-        if (inert) { fu = 0.0f; fv = 0.0f; fx = 3.0e38f; fn = -3.0e38f; }
-        else if (q < ns) margin = fmaxf(margin, fabsf(fx) + fabsf(fn) + 15.0f * fabsf(fu) + 7.0f * fabsf(fv));
-        u[q] = fu; v[q] = fv; ex[q] = fx; en[q] = fn;
-    }
-    slot[0] = make_float4(ex[0], ex[1], ex[2], ex[3]);
-    slot[1] = make_float4(ex[4], ex[5], en[0], en[1]);
-    slot[2] = make_float4(en[2], en[3], en[4], en[5]);
-    slot[3] = make_float4(u[0], u[1], u[2], u[3]);
-    slot[4] = make_float4(u[4], u[5], v[0], v[1]);
-    slot[5] = make_float4(v[2], v[3], v[4], v[5]);
-    slot[6] = make_float4(h2.x, h2.y, margin * 4.0e-7f, __int_as_float(k));
+    if (inert) { fu = 0.0f; fv = 0.0f; fx = 3.0e38f; fn = -3.0e38f; }
+    else if (q < ns) margin = 4.0e-7f * (fabsf(fx) + fabsf(fn) + 15.0f * fabsf(fu) + 7.0f * fabsf(fv));
+    sw[q] = fx; sw[6 + q] = fn; sw[12 + q] = fu; sw[18 + q] = fv;
+    if (q < 2) sw[28 + q] = margin;
 }
 
 // ---- thickness, 4 pixels of one row per lane --------------------------------------------------------------------------
@@ -165,7 +159,7 @@ __device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ slot, 
 
 // NS = number of steep slabs (they come first); NS == 0: no pixel can need refinement.
 template <int NS>
-__device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, const float4* __restrict__ s_rec,
+__device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, const float* __restrict__ recs,
                                            const LaneGeom& g, int wx0, int wy0, int lane, double (&acc)[4])
 {
     const float4 a0 = slot[0], a1 = slot[1], a2 = slot[2], a3 = slot[3], a4 = slot[4], a5 = slot[5], a6 = slot[6];
@@ -191,7 +185,7 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
             const float en = fmaxf(max3(n01.x, n01.y, n23.x), max3(n23.y, n45.x, n45.y));
             tk = ex - en;
         } else {
-            const float margin = a6.z;
+            const float margin = NS == 1 ? slot[7].x : fmaxf(slot[7].x, slot[7].y);
             float exs, ens, exr, enr;
             if (NS == 1) {
                 exs = e01.x; ens = n01.x;
@@ -212,8 +206,8 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
         const uint32_t flags = __float_as_uint(a6.x);
         if (flags & kFlagAllF64) fmask = 0xfu;
         if (fmask) {
-            const float4* rec = s_rec + __float_as_int(a6.w) * kRecStride4;
-            const int4 h3 = *reinterpret_cast<const int4*>(rec + 3);
+            const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)__float_as_uint(a6.w) * kRecWords);
+            const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));
             const double* r64 = reinterpret_cast<const double*>(rec + 4);
             const double dj = (double)(wx0 + 4 * (lane & 3) - h3.x), di = (double)(wy0 + (lane >> 2) - h3.y);
 #pragma unroll
@@ -262,9 +256,8 @@ template <bool OPD, bool FIELD, bool RAMP>
 __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
-    float4* s_rec = reinterpret_cast<float4*>(smem);                               // staged records (padded stride)
-    uint32_t* s_ids = reinterpret_cast<uint32_t*>(smem + kSmemRec);               // this tile's list, ascending
-    float4* s_slots = reinterpret_cast<float4*>(smem + kSmemRec + kSmemIds);      // per-warp survivor slots
+    uint32_t* s_ids = reinterpret_cast<uint32_t*>(smem);                          // this tile's list, ascending
+    float4* s_slots = reinterpret_cast<float4*>(smem + kSmemIds);                 // per-warp survivor slots
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int tpf = a.ntx * a.nty;
@@ -312,51 +305,51 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeA
     float4* my_slots = s_slots + wid * 32 * kSlotStride4;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
 
-    for (uint32_t c0 = 0; c0 < L; c0 += kChunk) {
-        const int nC = (int)min((uint32_t)kChunk, L - c0);
-        if (c0 > 0) __syncthreads();                             // everyone is done with the previous chunk
-        for (int u = tid; u < nC * 16; u += kComposeThreads) {
-            const uint32_t pid = in_smem ? s_ids[c0 + (u >> 4)] : glist[c0 + (u >> 4)];
-            cp_async16(&s_rec[(u >> 4) * kRecStride4 + (u & 15)], a.rec + (size_t)pid * kRecWords + (u & 15) * 4);
+    // From here on the warps of the CTA are independent (no barrier): each walks the whole list in batches of 32.
+    const float4* recs4 = reinterpret_cast<const float4*>(a.rec);
+    for (uint32_t base = 0; base < L; base += 32) {
+        // ---- cull: lane <-> particle base + lane; records are read through L1 / L2 (10 MB, L2 resident) -----------------
+        const uint32_t k = base + lane;
+        bool keep = false;
+        uint32_t pid = 0;
+        if (k < L) {
+            pid = in_smem ? s_ids[k] : glist[k];
+            const float4* rec = recs4 + (size_t)pid * (kRecWords / 4);
+            const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);   // cxp, cyp, ax, ay | ha, hb, bbx, bby
+            const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
+            const int pj0 = bx & 0xffff, pj1 = bx >> 16, pi0 = by & 0xffff, pi1 = by >> 16;
+            keep = pj0 <= wx0 + 15 && pj1 >= wx0 && pi0 <= wy0 + 7 && pi1 >= wy0;
+            // separating-axis test against the particle's oriented box (the silhouette lies inside it)
+            const float ddx = rcx - h0.x, ddy = rcy - h0.y;
+            const float pa = fabsf(ddx * h0.z + ddy * h0.w), pb = fabsf(ddy * h0.z - ddx * h0.w);
+            const float ra = 7.5f * fabsf(h0.z) + 3.5f * fabsf(h0.w), rb = 7.5f * fabsf(h0.w) + 3.5f * fabsf(h0.z);
+            keep = keep && pa <= h1.x + ra && pb <= h1.y + rb;
         }
-        cp_async_wait_all();
-        __syncthreads();
-
-        for (int base = 0; base < nC; base += 32) {
-            // ---- cull + re-base: lane <-> staged particle base + lane ------------------------------------------------
-            const int k = base + lane;
-            bool keep = false;
-            const float4* rec = s_rec + k * kRecStride4;
-            if (k < nC) {
-                const float4 h0 = rec[0], h1 = rec[1];           // cxp, cyp, ax, ay | ha, hb, bbx, bby
-                const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
-                const int pj0 = bx & 0xffff, pj1 = bx >> 16, pi0 = by & 0xffff, pi1 = by >> 16;
-                keep = pj0 <= wx0 + 15 && pj1 >= wx0 && pi0 <= wy0 + 7 && pi1 >= wy0;
-                // separating-axis test against the particle's oriented box (the silhouette lies inside it)
-                const float ddx = rcx - h0.x, ddy = rcy - h0.y;
-                const float pa = fabsf(ddx * h0.z + ddy * h0.w), pb = fabsf(ddy * h0.z - ddx * h0.w);
-                const float ra = 7.5f * fabsf(h0.z) + 3.5f * fabsf(h0.w), rb = 7.5f * fabsf(h0.w) + 3.5f * fabsf(h0.z);
-                keep = keep && pa <= h1.x + ra && pb <= h1.y + rb;
-            }
-            const unsigned m = __ballot_sync(0xffffffffu, keep);
-            if (keep) fill_slot(my_slots + __popc(m & ((1u << lane) - 1u)) * kSlotStride4, rec, k, wx0, wy0);
-            __syncwarp();
-            // ---- all lanes walk the survivors in ascending order ------------------------------------------------------
-            const int nsv = __popc(m);
-            for (int s = 0; s < nsv; ++s) {
-                const float4* slot = my_slots + s * kSlotStride4;
-                const uint32_t flags = __float_as_uint(slot[6].x);
-                if (!(flags & kFlagPrism)) {
-                    eval_ellipsoid(slot, g, acc);
-                } else {
-                    const int ns = (flags >> 8) & 7;
-                    if (ns == 0) eval_prism<0>(slot, s_rec, g, wx0, wy0, lane, acc);
-                    else if (ns == 1) eval_prism<1>(slot, s_rec, g, wx0, wy0, lane, acc);
-                    else eval_prism<2>(slot, s_rec, g, wx0, wy0, lane, acc);
-                }
-            }
-            __syncwarp();
+        const unsigned m = __ballot_sync(0xffffffffu, keep);
+        const int nsv = __popc(m);
+        if (keep)
+            reinterpret_cast<uint32_t*>(my_slots + __popc(m & ((1u << lane) - 1u)) * kSlotStride4)[27] = pid;
+        __syncwarp();
+        // ---- re-base: one lane per (survivor, slab) ------------------------------------------------------------------------
+        for (int it = lane; it < nsv * 6; it += 32) {
+            const int sidx = it / 6;
+            rebase_item(my_slots + sidx * kSlotStride4, a.rec, it - 6 * sidx, wx0, wy0);
         }
+        __syncwarp();
+        // ---- all lanes walk the survivors in ascending order ------------------------------------------------------------------
+        const float4* slot = my_slots;
+        for (int sv = 0; sv < nsv; ++sv, slot += kSlotStride4) {
+            const uint32_t flags = __float_as_uint(slot[6].x);
+            if (!(flags & kFlagPrism)) {
+                eval_ellipsoid(slot, g, acc);
+            } else {
+                const int ns = (flags >> 8) & 7;
+                if (ns == 0) eval_prism<0>(slot, a.rec, g, wx0, wy0, lane, acc);
+                else if (ns == 1) eval_prism<1>(slot, a.rec, g, wx0, wy0, lane, acc);
+                else eval_prism<2>(slot, a.rec, g, wx0, wy0, lane, acc);
+            }
+        }
+        __syncwarp();
     }
 
     // ---- H6/H7: write-out straight from the registers ----------------------------------------------------------------------
