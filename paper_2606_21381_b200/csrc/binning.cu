@@ -149,7 +149,7 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
     // words 0..7: data of the sub-tile cull (centre in pixel-index coordinates, oriented box, pixel bounding box)
     r32[0] = (float)(cx / p - 0.5);
     r32[1] = (float)(cy / p - 0.5);
-    r32u[6] = (uint32_t)j0 | ((uint32_t)j1 << 16);
+    r32u[6] = (uint32_t)j0 | ((uint32_t)j1 << 16) | (kind == 1u ? 0x80000000u : 0u);   // bit 31: prism
     r32u[7] = (uint32_t)i0 | ((uint32_t)i1 << 16);
     r32u[11] = (uint32_t)n;
     reinterpret_cast<int*>(r32)[12] = (int)jc;
@@ -177,6 +177,8 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
         r64[3] = 2.0 * p * (Sxx * ox + Sxy * oy);
         r64[4] = 2.0 * p * (Sxy * ox + Syy * oy);
         r64[5] = 1.0 - (Sxx * ox * ox + 2.0 * Sxy * ox * oy + Syy * oy * oy);
+        r64[6] = jc;
+        r64[7] = ic;
         // oriented box of the silhouette ellipse {d^T S d <= 1}: principal axes of S
         const double hd = 0.5 * (Sxx - Syy), rad = sqrt(hd * hd + Sxy * Sxy), mid = 0.5 * (Sxx + Syy);
         const double lmin = fmax(mid - rad, 1.0e-300), lmax = mid + rad;

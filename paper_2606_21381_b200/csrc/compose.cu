@@ -93,76 +93,76 @@ __device__ __noinline__ double prism_t64(const double* r64, uint32_t vmask, doub
     return t > 0.0 ? t : 0.0;
 }
 
-// ---- per-warp preparation of the survivors: work item = (survivor slot, slab q), one lane per item -------------------
-// Re-base the particle's fp64 coefficients from its own reference pixel (jc, ic) to the warp's sub-tile origin
-// (wx0, wy0) and round to fp32 there: all later arithmetic uses pixel offsets 0..15 / 0..7.
-// Slot layout (words): 0..5 Ex, 6..11 En, 12..17 U, 18..23 V, 24 flags, 25 dn, 26 -, 27 particle index, 28..29 margins.
-// Ellipsoid slot: doubles c20, c11, c02, c10, c01, c00 in words 0..11; 24 flags, 25 K, 27 particle index.
+// ---- per-warp preparation of the prism survivors: work item = (survivor slot, slab q), one lane per item -------------
+// Re-base the slab's fp64 coefficients from the particle's reference pixel (jc, ic) to the warp's sub-tile origin
+// (wx0, wy0) and round to fp32 there: all later fp32 arithmetic uses pixel offsets 0..15 / 0..7.
+// Slot layout (words): 0..5 Ex, 6..11 En, 12..17 U, 18..23 V, 24 flags, 25 dn, 27 particle index.
+// An ellipsoid survivor only has words 24 (flags = 0) and 27: it is evaluated from its record directly.
 __device__ __forceinline__ void rebase_item(float4* __restrict__ slot, const float* __restrict__ recs, int q, int wx0, int wy0)
 {
     float* sw = reinterpret_cast<float*>(slot);
     const uint32_t pid = __float_as_uint(sw[27]);
     const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)pid * kRecWords);
-    const float4 h2 = __ldg(rec + 2);                                  // flags, dn | K, -, id
     const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));     // jc, ic
-    const uint32_t flags = __float_as_uint(h2.x);
-    const double oj = (double)(wx0 - h3.x), oi = (double)(wy0 - h3.y);
     const double2* c = reinterpret_cast<const double2*>(rec + 4);
-    if (q == 0) { sw[24] = h2.x; sw[25] = h2.y; }
-    if (!(flags & kFlagPrism)) {
-        if (q != 0) return;
-        // w(dj, di) = F1 - (A dj^2 + B dj di + C di^2 + D dj + E di) with dj = oj + lx, di = oi + ly
-        const double2 ab = __ldg(c), cd = __ldg(c + 1), ef = __ldg(c + 2);
-        const double A = ab.x, B = ab.y, C = cd.x, D = cd.y, E = ef.x, F1 = ef.y;
-        double2* s = reinterpret_cast<double2*>(slot);
-        s[0] = make_double2(-A, -B);                                              // c20, c11
-        s[1] = make_double2(-C, -fma(2.0 * A, oj, fma(B, oi, D)));                // c02, c10
-        s[2] = make_double2(-fma(B, oj, fma(2.0 * C, oi, E)),                     // c01
-                            F1 - fma(fma(A, oj, fma(B, oi, D)), oj, fma(C, oi, E) * oi));   // c00
-        return;
+    const double2 uv = __ldg(c + 2 * q), xn = __ldg(c + 2 * q + 1);    // U, V | Cx, Cn
+    if (q == 0) {
+        const float4 h2 = __ldg(rec + 2);                              // flags, dn, -, id
+        sw[24] = h2.x; sw[25] = h2.y;
     }
-    const int ns = (flags >> 8) & 7;
-    const double2 uv = __ldg(c + 2 * q), xn = __ldg(c + 2 * q + 1);
+    const double oj = (double)(wx0 - h3.x), oi = (double)(wy0 - h3.y);
     const double m = fma(uv.x, oj, uv.y * oi);
-    float fu = (float)uv.x, fv = (float)uv.y, fx = (float)(xn.x - m), fn = (float)(xn.y - m);
-    const bool inert = ((flags >> (16 + q)) & 1u) || !(fabsf(fu) < 1.0e30f) || !(fabsf(fv) < 1.0e30f) ||
-                       !(fabsf(fx) < 1.0e30f) || !(fabsf(fn) < 1.0e30f);
-    float margin = 0.0f;
-    if (inert) { fu = 0.0f; fv = 0.0f; fx = 3.0e38f; fn = -3.0e38f; }
-    else if (q < ns) margin = 4.0e-7f * (fabsf(fx) + fabsf(fn) + 15.0f * fabsf(fu) + 7.0f * fabsf(fv));
-    sw[q] = fx; sw[6 + q] = fn; sw[12 + q] = fu; sw[18 + q] = fv;
-    if (q < 2) sw[28 + q] = margin;
+    sw[q] = (float)(xn.x - m); sw[6 + q] = (float)(xn.y - m); sw[12 + q] = (float)uv.x; sw[18 + q] = (float)uv.y;
 }
 
 // ---- thickness, 4 pixels of one row per lane --------------------------------------------------------------------------
 struct LaneGeom {
     float2 nlx[4];     // (-lx_k, -lx_k), lx_k = 4 (lane & 3) + k : pixel column offset inside the warp sub-tile
     float2 nly;        // (-ly, -ly),     ly = lane >> 2
-    double lxd[4], lyd;
+    double xd, yd;     // absolute pixel column of this lane's first pixel, and its row
 };
 
-__device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ slot, const LaneGeom& g, double (&acc)[4])
+// Ellipsoid (kind 0), straight from the particle record (L1 / L2 broadcast loads): w = 1 - d^T S d as a quadratic
+// polynomial of the pixel offsets from (jc, ic), all in fp64 (2 DFMA per pixel after the row terms), then
+// t = T0 sqrt(max(w, 0)) in fp32 and acc += (dn T0) sqrt(w) in fp64.
+__device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ rec, const LaneGeom& g, double (&acc)[4])
 {
-    const double2 c0 = *reinterpret_cast<const double2*>(slot + 0);   // c20, c11
-    const double2 c1 = *reinterpret_cast<const double2*>(slot + 1);   // c02, c10
-    const double2 c2 = *reinterpret_cast<const double2*>(slot + 2);   // c01, c00
-    const double K = (double)slot[6].y;
-    const double b1 = fma(c0.y, g.lyd, c1.y);
-    const double cc = fma(fma(c1.x, g.lyd, c2.x), g.lyd, c2.y);
+    const double2* c = reinterpret_cast<const double2*>(rec + 4);
+    const double2 ab = __ldg(c), cd = __ldg(c + 1), ef = __ldg(c + 2), jic = __ldg(c + 3);   // A,B | C,D | E,F1 | jc,ic
+    const double K = (double)__ldg(reinterpret_cast<const float*>(rec) + 9);
+    const double dj = g.xd - jic.x, di = g.yd - jic.y;
+    const double b1 = fma(ab.y, di, cd.y);                       // B di + D
+    const double cc = fma(-fma(cd.x, di, ef.x), di, ef.y);       // F1 - (C di + E) di
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        const double w = fma(fma(c0.x, g.lxd[k], b1), g.lxd[k], cc);      // 1 - d^T S d
+        const double djk = dj + (double)k;
+        const double w = fma(-fma(ab.x, djk, b1), djk, cc);      // 1 - d^T S d
         const float t = fast_sqrt(fmaxf((float)w, 0.0f));
         acc[k] = fma((double)t, K, acc[k]);
     }
 }
 
-// NS = number of steep slabs (they come first); NS == 0: no pixel can need refinement.
-template <int NS>
-__device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, const float* __restrict__ recs,
-                                           const LaneGeom& g, int wx0, int wy0, int lane, double (&acc)[4])
+// Prism whose every pixel goes to fp64 (a vertical face, a slab steeper than kAllF64Slope, or > 2 steep slabs): rare.
+__device__ __noinline__ void eval_prism_f64(const float4* __restrict__ rec, double xd, double yd, double (&acc)[4])
 {
-    const float4 a0 = slot[0], a1 = slot[1], a2 = slot[2], a3 = slot[3], a4 = slot[4], a5 = slot[5], a6 = slot[6];
+    const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));
+    const float4 h2 = __ldg(rec + 2);
+    const double dj = xd - (double)h3.x, di = yd - (double)h3.y, dn = (double)h2.y;
+    const double* r64 = reinterpret_cast<const double*>(rec + 4);
+#pragma unroll 1
+    for (int k = 0; k < 4; ++k) acc[k] = fma(prism_t64(r64, __float_as_uint(h2.x) >> 16, dj + (double)k, di), dn, acc[k]);
+}
+
+// Prism (kind 1): 6 slabs, exit_k = Ex_k - U_k lx - V_k ly, enter_k = En_k - U_k lx - V_k ly from the re-based fp32
+// coefficients (packed FFMA2, two slabs per instruction), t = max(0, min_k exit_k - max_k enter_k) with 3-input
+// min / max.  The first NS (<= 2) slabs are steep (slope > kSteepSlope): their fp32 values are replaced, for every
+// pixel, by fp64 evaluations from the record (2 DFMA + 2 conversions per pixel and slab), so no pixel needs a
+// per-lane decision.
+template <int NS>
+__device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, const float4* __restrict__ rec,
+                                           const LaneGeom& g, double (&acc)[4])
+{
+    const float4 a0 = slot[0], a1 = slot[1], a2 = slot[2], a3 = slot[3], a4 = slot[4], a5 = slot[5];
     const float2 v01 = make_float2(a4.z, a4.w), v23 = make_float2(a5.x, a5.y), v45 = make_float2(a5.z, a5.w);
     const float2 u01 = make_float2(a3.x, a3.y), u23 = make_float2(a3.z, a3.w), u45 = make_float2(a4.x, a4.y);
     // row terms: value of every plane at this lane's row, column offset 0
@@ -172,54 +172,40 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
     const float2 nk01 = ffma2(v01, g.nly, make_float2(a1.z, a1.w));
     const float2 nk23 = ffma2(v23, g.nly, make_float2(a2.x, a2.y));
     const float2 nk45 = ffma2(v45, g.nly, make_float2(a2.z, a2.w));
-    const double dn = (double)a6.y;
-    float t[4];
-    unsigned fmask = 0u;
+    const double dn = (double)slot[6].y;
+    // steep slabs in fp64, relative to the particle's reference pixel
+    double sU[NS > 0 ? NS : 1], sX[NS > 0 ? NS : 1], sN[NS > 0 ? NS : 1], dj = 0.0;
+    if (NS > 0) {
+        const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));
+        const double2* c = reinterpret_cast<const double2*>(rec + 4);
+        dj = g.xd - (double)h3.x;
+        const double di = g.yd - (double)h3.y;
+#pragma unroll
+        for (int q = 0; q < NS; ++q) {
+            const double2 uv = __ldg(c + 2 * q), xn = __ldg(c + 2 * q + 1);
+            sU[q] = uv.x;
+            sX[q] = fma(-uv.y, di, xn.x);
+            sN[q] = fma(-uv.y, di, xn.y);
+        }
+    }
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        const float2 e01 = ffma2(u01, g.nlx[k], ek01), e23 = ffma2(u23, g.nlx[k], ek23), e45 = ffma2(u45, g.nlx[k], ek45);
-        const float2 n01 = ffma2(u01, g.nlx[k], nk01), n23 = ffma2(u23, g.nlx[k], nk23), n45 = ffma2(u45, g.nlx[k], nk45);
-        float tk;
-        if (NS == 0) {
-            const float ex = fminf(min3(e01.x, e01.y, e23.x), min3(e23.y, e45.x, e45.y));
-            const float en = fmaxf(max3(n01.x, n01.y, n23.x), max3(n23.y, n45.x, n45.y));
-            tk = ex - en;
-        } else {
-            const float margin = NS == 1 ? slot[7].x : fmaxf(slot[7].x, slot[7].y);
-            float exs, ens, exr, enr;
-            if (NS == 1) {
-                exs = e01.x; ens = n01.x;
-                exr = fminf(min3(e01.y, e23.x, e23.y), fminf(e45.x, e45.y));
-                enr = fmaxf(max3(n01.y, n23.x, n23.y), fmaxf(n45.x, n45.y));
-            } else {
-                exs = fminf(e01.x, e01.y); ens = fmaxf(n01.x, n01.y);
-                exr = fminf(fminf(e23.x, e23.y), fminf(e45.x, e45.y));
-                enr = fmaxf(fmaxf(n23.x, n23.y), fmaxf(n45.x, n45.y));
+        float2 e01 = ffma2(u01, g.nlx[k], ek01), e23 = ffma2(u23, g.nlx[k], ek23), e45 = ffma2(u45, g.nlx[k], ek45);
+        float2 n01 = ffma2(u01, g.nlx[k], nk01), n23 = ffma2(u23, g.nlx[k], nk23), n45 = ffma2(u45, g.nlx[k], nk45);
+        if (NS > 0) {
+            const double djk = dj + (double)k;
+            e01.x = (float)fma(-sU[0], djk, sX[0]);
+            n01.x = (float)fma(-sU[0], djk, sN[0]);
+            if (NS > 1) {
+                e01.y = (float)fma(-sU[NS - 1], djk, sX[NS - 1]);
+                n01.y = (float)fma(-sU[NS - 1], djk, sN[NS - 1]);
             }
-            tk = fminf(exs, exr) - fmaxf(ens, enr);
-            // a steep slab is (within its fp32 error) the active entry or exit face and the pixel is not clearly outside
-            if ((tk > -2.0f * margin) && (exs < exr + margin || ens > enr - margin)) fmask |= 1u << k;
         }
-        t[k] = fmaxf(tk, 0.0f);
+        const float ex = fminf(min3(e01.x, e01.y, e23.x), min3(e23.y, e45.x, e45.y));
+        const float en = fmaxf(max3(n01.x, n01.y, n23.x), max3(n23.y, n45.x, n45.y));
+        const float t = fmaxf(ex - en, 0.0f);
+        acc[k] = fma((double)t, dn, acc[k]);
     }
-    if (NS != 0) {
-        const uint32_t flags = __float_as_uint(a6.x);
-        if (flags & kFlagAllF64) fmask = 0xfu;
-        if (fmask) {
-            const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)__float_as_uint(a6.w) * kRecWords);
-            const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));
-            const double* r64 = reinterpret_cast<const double*>(rec + 4);
-            const double dj = (double)(wx0 + 4 * (lane & 3) - h3.x), di = (double)(wy0 + (lane >> 2) - h3.y);
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                if ((fmask >> k) & 1u) acc[k] = fma(prism_t64(r64, flags >> 16, dj + (double)k, di), dn, acc[k]);
-                else acc[k] = fma((double)t[k], dn, acc[k]);
-            }
-            return;
-        }
-    }
-#pragma unroll
-    for (int k = 0; k < 4; ++k) acc[k] = fma((double)t[k], dn, acc[k]);
 }
 
 // ---- list ordering ----------------------------------------------------------------------------------------------------
@@ -296,10 +282,10 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeA
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         g.nlx[k] = make_float2(-(float)(lx + k), -(float)(lx + k));
-        g.lxd[k] = (double)(lx + k);
     }
     g.nly = make_float2(-(float)ly, -(float)ly);
-    g.lyd = (double)ly;
+    g.xd = (double)j;
+    g.yd = (double)i;
     // sub-tile rectangle (pixel centres) for the cull: centre in pixel-index coordinates, half extents 7.5 x 3.5
     const float rcx = (float)wx0 + 7.5f, rcy = (float)wy0 + 3.5f;
     float4* my_slots = s_slots + wid * 32 * kSlotStride4;
@@ -310,14 +296,15 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeA
     for (uint32_t base = 0; base < L; base += 32) {
         // ---- cull: lane <-> particle base + lane; records are read through L1 / L2 (10 MB, L2 resident) -----------------
         const uint32_t k = base + lane;
-        bool keep = false;
+        bool keep = false, is_prism = false;
         uint32_t pid = 0;
         if (k < L) {
             pid = in_smem ? s_ids[k] : glist[k];
             const float4* rec = recs4 + (size_t)pid * (kRecWords / 4);
             const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);   // cxp, cyp, ax, ay | ha, hb, bbx, bby
             const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
-            const int pj0 = bx & 0xffff, pj1 = bx >> 16, pi0 = by & 0xffff, pi1 = by >> 16;
+            const int pj0 = bx & 0x7fff, pj1 = (bx >> 16) & 0x7fff, pi0 = by & 0xffff, pi1 = by >> 16;
+            is_prism = (bx >> 31) != 0u;
             keep = pj0 <= wx0 + 15 && pj1 >= wx0 && pi0 <= wy0 + 7 && pi1 >= wy0;
             // separating-axis test against the particle's oriented box (the silhouette lies inside it)
             const float ddx = rcx - h0.x, ddy = rcy - h0.y;
@@ -326,27 +313,39 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeA
             keep = keep && pa <= h1.x + ra && pb <= h1.y + rb;
         }
         const unsigned m = __ballot_sync(0xffffffffu, keep);
-        const int nsv = __popc(m);
-        if (keep)
-            reinterpret_cast<uint32_t*>(my_slots + __popc(m & ((1u << lane) - 1u)) * kSlotStride4)[27] = pid;
+        const unsigned mp = __ballot_sync(0xffffffffu, keep && is_prism);
+        const int nsv = __popc(m), npr = __popc(mp);
+        if (keep) {
+            const unsigned lt = (1u << lane) - 1u;
+            const int pos = __popc(m & lt);
+            uint32_t* sw = reinterpret_cast<uint32_t*>(my_slots + pos * kSlotStride4);
+            sw[27] = pid;
+            if (is_prism) reinterpret_cast<uint32_t*>(my_slots + __popc(mp & lt) * kSlotStride4)[26] = (uint32_t)pos;
+            else sw[24] = 0u;                                    // flags of an ellipsoid
+        }
         __syncwarp();
-        // ---- re-base: one lane per (survivor, slab) ------------------------------------------------------------------------
-        for (int it = lane; it < nsv * 6; it += 32) {
-            const int sidx = it / 6;
-            rebase_item(my_slots + sidx * kSlotStride4, a.rec, it - 6 * sidx, wx0, wy0);
+        // ---- re-base the prisms: one lane per (prism survivor, slab) ----------------------------------------------------------
+        for (int it = lane; it < npr * 6; it += 32) {
+            const int r = it / 6;
+            const uint32_t pos = reinterpret_cast<const uint32_t*>(my_slots + r * kSlotStride4)[26];
+            rebase_item(my_slots + pos * kSlotStride4, a.rec, it - 6 * r, wx0, wy0);
         }
         __syncwarp();
         // ---- all lanes walk the survivors in ascending order ------------------------------------------------------------------
         const float4* slot = my_slots;
         for (int sv = 0; sv < nsv; ++sv, slot += kSlotStride4) {
-            const uint32_t flags = __float_as_uint(slot[6].x);
+            const float4 h = slot[6];                            // flags, dn, -, particle index
+            const uint32_t flags = __float_as_uint(h.x);
+            const float4* rec = recs4 + (size_t)__float_as_uint(h.w) * (kRecWords / 4);
             if (!(flags & kFlagPrism)) {
-                eval_ellipsoid(slot, g, acc);
+                eval_ellipsoid(rec, g, acc);
+            } else if (flags & kFlagAllF64) {
+                eval_prism_f64(rec, g.xd, g.yd, acc);
             } else {
                 const int ns = (flags >> 8) & 7;
-                if (ns == 0) eval_prism<0>(slot, a.rec, g, wx0, wy0, lane, acc);
-                else if (ns == 1) eval_prism<1>(slot, a.rec, g, wx0, wy0, lane, acc);
-                else eval_prism<2>(slot, a.rec, g, wx0, wy0, lane, acc);
+                if (ns == 0) eval_prism<0>(slot, rec, g, acc);
+                else if (ns == 1) eval_prism<1>(slot, rec, g, acc);
+                else eval_prism<2>(slot, rec, g, acc);
             }
         }
         __syncwarp();
@@ -442,7 +441,7 @@ __global__ void __launch_bounds__(256) k_compose_atomic(const float* __restrict_
     const float4 h1 = rec[1], h2 = rec[2];
     const int4 h3 = *reinterpret_cast<const int4*>(rec + 3);
     const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
-    const int j0 = bx & 0xffff, j1 = bx >> 16, i0 = by & 0xffff, i1 = by >> 16;
+    const int j0 = bx & 0x7fff, j1 = (bx >> 16) & 0x7fff, i0 = by & 0xffff, i1 = by >> 16;
     const uint32_t flags = __float_as_uint(h2.x);
     const double* c = reinterpret_cast<const double*>(rec + 4);
     const double K = (double)h2.y;
