@@ -96,8 +96,8 @@ __device__ __noinline__ double prism_t64(const double* r64, uint32_t vmask, doub
 // ---- per-warp preparation of the prism survivors: work item = (survivor slot, slab q), one lane per item -------------
 // Re-base the slab's fp64 coefficients from the particle's reference pixel (jc, ic) to the warp's sub-tile origin
 // (wx0, wy0) and round to fp32 there: all later fp32 arithmetic uses pixel offsets 0..15 / 0..7.
-// Slot layout (words): 0..5 Ex, 6..11 En, 12..17 U, 18..23 V, 24 flags, 25 dn, 27 particle index.
-// An ellipsoid survivor only has words 24 (flags = 0) and 27: it is evaluated from its record directly.
+// Slot layout (words): 0..5 Ex, 6..11 En, 12..17 U, 18..23 V, 24 flags, 25 dn, 27 particle index, 28..35 slab 0 in
+// fp64 (Ex, En, U, V).  An ellipsoid slot holds the record's 8 doubles (A..F1, jc, ic) in words 0..15, 24 = 0, 25 = K.
 __device__ __forceinline__ void rebase_item(float4* __restrict__ slot, const float* __restrict__ recs, int q, int wx0, int wy0)
 {
     float* sw = reinterpret_cast<float*>(slot);
@@ -112,25 +112,30 @@ __device__ __forceinline__ void rebase_item(float4* __restrict__ slot, const flo
     }
     const double oj = (double)(wx0 - h3.x), oi = (double)(wy0 - h3.y);
     const double m = fma(uv.x, oj, uv.y * oi);
-    sw[q] = (float)(xn.x - m); sw[6 + q] = (float)(xn.y - m); sw[12 + q] = (float)uv.x; sw[18 + q] = (float)uv.y;
+    const double ex = xn.x - m, en = xn.y - m;
+    sw[q] = (float)ex; sw[6 + q] = (float)en; sw[12 + q] = (float)uv.x; sw[18 + q] = (float)uv.y;
+    if (q == 0) {                                                      // slab 0 also in fp64 (used when it is steep)
+        reinterpret_cast<double2*>(slot)[7] = make_double2(ex, en);
+        reinterpret_cast<double2*>(slot)[8] = uv;
+    }
 }
 
 // ---- thickness, 4 pixels of one row per lane --------------------------------------------------------------------------
 struct LaneGeom {
     float2 nlx[4];     // (-lx_k, -lx_k), lx_k = 4 (lane & 3) + k : pixel column offset inside the warp sub-tile
     float2 nly;        // (-ly, -ly),     ly = lane >> 2
-    double xd, yd;     // absolute pixel column of this lane's first pixel, and its row
+    float xf, yf;      // absolute pixel column of this lane's first pixel, and its row (exact small integers)
 };
 
-// Ellipsoid (kind 0), straight from the particle record (L1 / L2 broadcast loads): w = 1 - d^T S d as a quadratic
-// polynomial of the pixel offsets from (jc, ic), all in fp64 (2 DFMA per pixel after the row terms), then
+// Ellipsoid (kind 0), from the record doubles copied into the slot: w = 1 - d^T S d as a quadratic polynomial of
+// the pixel offsets from (jc, ic), all in fp64 (2 DFMA per pixel after the row terms), then
 // t = T0 sqrt(max(w, 0)) in fp32 and acc += (dn T0) sqrt(w) in fp64.
-__device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ rec, const LaneGeom& g, double (&acc)[4])
+__device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ slot, float K, const LaneGeom& g, double (&acc)[4])
 {
-    const double2* c = reinterpret_cast<const double2*>(rec + 4);
-    const double2 ab = __ldg(c), cd = __ldg(c + 1), ef = __ldg(c + 2), jic = __ldg(c + 3);   // A,B | C,D | E,F1 | jc,ic
-    const double K = (double)__ldg(reinterpret_cast<const float*>(rec) + 9);
-    const double dj = g.xd - jic.x, di = g.yd - jic.y;
+    const double2* c = reinterpret_cast<const double2*>(slot);
+    const double2 ab = c[0], cd = c[1], ef = c[2], jic = c[3];   // A,B | C,D | E,F1 | jc,ic
+    const double Kd = (double)K;
+    const double dj = (double)g.xf - jic.x, di = (double)g.yf - jic.y;
     const double b1 = fma(ab.y, di, cd.y);                       // B di + D
     const double cc = fma(-fma(cd.x, di, ef.x), di, ef.y);       // F1 - (C di + E) di
 #pragma unroll
@@ -138,19 +143,18 @@ __device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ rec, c
         const double djk = dj + (double)k;
         const double w = fma(-fma(ab.x, djk, b1), djk, cc);      // 1 - d^T S d
         const float t = fast_sqrt(fmaxf((float)w, 0.0f));
-        acc[k] = fma((double)t, K, acc[k]);
+        acc[k] = fma((double)t, Kd, acc[k]);
     }
 }
 
 // Prism whose every pixel goes to fp64 (a vertical face, a slab steeper than kAllF64Slope, or > 2 steep slabs): rare.
-__device__ __noinline__ void eval_prism_f64(const float4* __restrict__ rec, double xd, double yd, double (&acc)[4])
+// One pixel per call; returns dn * t (by value, so that the accumulators stay in registers).
+__device__ __noinline__ double prism_f64_px(const float4* __restrict__ rec, double xd, double yd)
 {
     const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));
     const float4 h2 = __ldg(rec + 2);
-    const double dj = xd - (double)h3.x, di = yd - (double)h3.y, dn = (double)h2.y;
-    const double* r64 = reinterpret_cast<const double*>(rec + 4);
-#pragma unroll 1
-    for (int k = 0; k < 4; ++k) acc[k] = fma(prism_t64(r64, __float_as_uint(h2.x) >> 16, dj + (double)k, di), dn, acc[k]);
+    return (double)h2.y * prism_t64(reinterpret_cast<const double*>(rec + 4), __float_as_uint(h2.x) >> 16,
+                                    xd - (double)h3.x, yd - (double)h3.y);
 }
 
 // Prism (kind 1): 6 slabs, exit_k = Ex_k - U_k lx - V_k ly, enter_k = En_k - U_k lx - V_k ly from the re-based fp32
@@ -159,7 +163,7 @@ __device__ __noinline__ void eval_prism_f64(const float4* __restrict__ rec, doub
 // pixel, by fp64 evaluations from the record (2 DFMA + 2 conversions per pixel and slab), so no pixel needs a
 // per-lane decision.
 template <int NS>
-__device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, const float4* __restrict__ rec,
+__device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, const float4* __restrict__ rec, float dnf,
                                            const LaneGeom& g, double (&acc)[4])
 {
     const float4 a0 = slot[0], a1 = slot[1], a2 = slot[2], a3 = slot[3], a4 = slot[4], a5 = slot[5];
@@ -172,39 +176,43 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
     const float2 nk01 = ffma2(v01, g.nly, make_float2(a1.z, a1.w));
     const float2 nk23 = ffma2(v23, g.nly, make_float2(a2.x, a2.y));
     const float2 nk45 = ffma2(v45, g.nly, make_float2(a2.z, a2.w));
-    const double dn = (double)slot[6].y;
-    // steep slabs in fp64, relative to the particle's reference pixel
-    double sU[NS > 0 ? NS : 1], sX[NS > 0 ? NS : 1], sN[NS > 0 ? NS : 1], dj = 0.0;
+    // steep slabs in fp64: slab 0 from the slot (re-based to the sub-tile origin), slab 1 from the record
+    double u0 = 0.0, x0 = 0.0, n0 = 0.0, u1 = 0.0, x1 = 0.0, n1 = 0.0, dj = 0.0;
     if (NS > 0) {
+        const double2 xn = reinterpret_cast<const double2*>(slot)[7], uv = reinterpret_cast<const double2*>(slot)[8];
+        const double nly = (double)g.nly.x;
+        u0 = uv.x;
+        x0 = fma(uv.y, nly, xn.x);
+        n0 = fma(uv.y, nly, xn.y);
+    }
+    if (NS > 1) {
         const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));
         const double2* c = reinterpret_cast<const double2*>(rec + 4);
-        dj = g.xd - (double)h3.x;
-        const double di = g.yd - (double)h3.y;
-#pragma unroll
-        for (int q = 0; q < NS; ++q) {
-            const double2 uv = __ldg(c + 2 * q), xn = __ldg(c + 2 * q + 1);
-            sU[q] = uv.x;
-            sX[q] = fma(-uv.y, di, xn.x);
-            sN[q] = fma(-uv.y, di, xn.y);
-        }
+        const double2 uv = __ldg(c + 2), xn = __ldg(c + 3);
+        dj = (double)g.xf - (double)h3.x;
+        const double di = (double)g.yf - (double)h3.y;
+        u1 = uv.x;
+        x1 = fma(-uv.y, di, xn.x);
+        n1 = fma(-uv.y, di, xn.y);
     }
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         float2 e01 = ffma2(u01, g.nlx[k], ek01), e23 = ffma2(u23, g.nlx[k], ek23), e45 = ffma2(u45, g.nlx[k], ek45);
         float2 n01 = ffma2(u01, g.nlx[k], nk01), n23 = ffma2(u23, g.nlx[k], nk23), n45 = ffma2(u45, g.nlx[k], nk45);
         if (NS > 0) {
+            const double nlxk = (double)g.nlx[k].x;
+            e01.x = (float)fma(u0, nlxk, x0);
+            n01.x = (float)fma(u0, nlxk, n0);
+        }
+        if (NS > 1) {
             const double djk = dj + (double)k;
-            e01.x = (float)fma(-sU[0], djk, sX[0]);
-            n01.x = (float)fma(-sU[0], djk, sN[0]);
-            if (NS > 1) {
-                e01.y = (float)fma(-sU[NS - 1], djk, sX[NS - 1]);
-                n01.y = (float)fma(-sU[NS - 1], djk, sN[NS - 1]);
-            }
+            e01.y = (float)fma(-u1, djk, x1);
+            n01.y = (float)fma(-u1, djk, n1);
         }
         const float ex = fminf(min3(e01.x, e01.y, e23.x), min3(e23.y, e45.x, e45.y));
         const float en = fmaxf(max3(n01.x, n01.y, n23.x), max3(n23.y, n45.x, n45.y));
         const float t = fmaxf(ex - en, 0.0f);
-        acc[k] = fma((double)t, dn, acc[k]);
+        acc[k] = fma((double)t, (double)dnf, acc[k]);
     }
 }
 
@@ -284,8 +292,8 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeA
         g.nlx[k] = make_float2(-(float)(lx + k), -(float)(lx + k));
     }
     g.nly = make_float2(-(float)ly, -(float)ly);
-    g.xd = (double)j;
-    g.yd = (double)i;
+    g.xf = (float)j;
+    g.yf = (float)i;
     // sub-tile rectangle (pixel centres) for the cull: centre in pixel-index coordinates, half extents 7.5 x 3.5
     const float rcx = (float)wx0 + 7.5f, rcy = (float)wy0 + 3.5f;
     float4* my_slots = s_slots + wid * 32 * kSlotStride4;
@@ -321,7 +329,15 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeA
             uint32_t* sw = reinterpret_cast<uint32_t*>(my_slots + pos * kSlotStride4);
             sw[27] = pid;
             if (is_prism) reinterpret_cast<uint32_t*>(my_slots + __popc(mp & lt) * kSlotStride4)[26] = (uint32_t)pos;
-            else sw[24] = 0u;                                    // flags of an ellipsoid
+            else {                                               // ellipsoid: copy the record's doubles into the slot
+                const float4* rec = recs4 + (size_t)pid * (kRecWords / 4);
+                float4* sl = my_slots + pos * kSlotStride4;
+                const float4 c0 = __ldg(rec + 4), c1 = __ldg(rec + 5), c2 = __ldg(rec + 6), c3 = __ldg(rec + 7);
+                const float K = __ldg(reinterpret_cast<const float*>(rec) + 9);
+                sl[0] = c0; sl[1] = c1; sl[2] = c2; sl[3] = c3;
+                sw[24] = 0u;
+                reinterpret_cast<float*>(sw)[25] = K;
+            }
         }
         __syncwarp();
         // ---- re-base the prisms: one lane per (prism survivor, slab) ----------------------------------------------------------
@@ -338,14 +354,15 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeA
             const uint32_t flags = __float_as_uint(h.x);
             const float4* rec = recs4 + (size_t)__float_as_uint(h.w) * (kRecWords / 4);
             if (!(flags & kFlagPrism)) {
-                eval_ellipsoid(rec, g, acc);
+                eval_ellipsoid(slot, h.y, g, acc);
             } else if (flags & kFlagAllF64) {
-                eval_prism_f64(rec, g.xd, g.yd, acc);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) acc[k] += prism_f64_px(rec, (double)(g.xf + (float)k), (double)g.yf);
             } else {
                 const int ns = (flags >> 8) & 7;
-                if (ns == 0) eval_prism<0>(slot, rec, g, acc);
-                else if (ns == 1) eval_prism<1>(slot, rec, g, acc);
-                else eval_prism<2>(slot, rec, g, acc);
+                if (ns == 0) eval_prism<0>(slot, rec, h.y, g, acc);
+                else if (ns == 1) eval_prism<1>(slot, rec, h.y, g, acc);
+                else eval_prism<2>(slot, rec, h.y, g, acc);
             }
         }
         __syncwarp();
