@@ -310,25 +310,28 @@ __global__ void __launch_bounds__(1024) k_scan(uint32_t* __restrict__ count, uin
     }
 }
 
-// H4: every listed particle appends its index to each tile of its range.  Order inside a tile is whatever
-// the atomics give; the composition kernel sorts each segment ascending before use.
-__global__ void __launch_bounds__(128) k_fill(const int4* __restrict__ tbox, const int* __restrict__ pframe,
+// H4: every listed particle appends its index to each tile of its range: one warp per particle, one lane per tile
+// (the atomics return the cursor, so a single thread walking its tiles would pay one memory round trip per tile).
+// Order inside a tile is whatever the atomics give; the composition kernel sorts each segment ascending before use.
+__global__ void __launch_bounds__(256) k_fill(const int4* __restrict__ tbox, const int* __restrict__ pframe,
                                               uint32_t* __restrict__ cursor, const uint32_t* __restrict__ offset,
                                               uint32_t* __restrict__ list, long long N, int ntx, int nty,
                                               const DeviceStatus* status)
 {
-    const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
     if (n >= N) return;
     if (status->bits & OSOG_WOVERFLOW) return;
     const int4 tb = tbox[n];
     if (tb.x > tb.y) return;
     const size_t base = (size_t)pframe[n] * ntx * nty;
-    for (int ty = tb.z; ty <= tb.w; ++ty)
-        for (int tx = tb.x; tx <= tb.y; ++tx) {
-            const size_t t = base + (size_t)ty * ntx + tx;
-            const uint32_t pos = atomicAdd(&cursor[t], 1u);
-            list[offset[t] + pos] = (uint32_t)n;
-        }
+    const int tw = tb.y - tb.x + 1, nt = tw * (tb.w - tb.z + 1);
+    for (int q = lane; q < nt; q += 32) {
+        const int ty = tb.z + q / tw, tx = tb.x + q % tw;
+        const size_t t = base + (size_t)ty * ntx + tx;
+        const uint32_t pos = atomicAdd(&cursor[t], 1u);
+        list[offset[t] + pos] = (uint32_t)n;
+    }
 }
 
 __global__ void k_set_optics(FrameOptics* optics, const OpticsChunk oc)
@@ -402,7 +405,7 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     k_scan<<<1, 1024, 0, c->stream>>>(c->count, c->offset, tiles, c->max_pairs, c->status);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     if (N > 0) {
-        k_fill<<<(unsigned)((N + threads - 1) / threads), threads, 0, c->stream>>>(
+        k_fill<<<(unsigned)((N * 32 + 255) / 256), 256, 0, c->stream>>>(
             c->tbox, c->pframe, c->count, c->offset, c->list, N, c->ntx, c->nty, c->status);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }

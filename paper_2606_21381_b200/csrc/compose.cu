@@ -247,7 +247,7 @@ __device__ void sort_global(uint32_t* a, uint32_t L)
 }
 
 template <bool OPD, bool FIELD, bool RAMP>
-__global__ void __launch_bounds__(kComposeThreads) k_compose_tile(const ComposeArgs a)
+__global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const ComposeArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t* s_ids = reinterpret_cast<uint32_t*>(smem);                          // this tile's list, ascending
