@@ -6,7 +6,7 @@
 One "step" = one pass of the whole hot path (H1-H7: prepare, bounding box + count, scan, fill, ordered tile
 composition with the fused field write-out) over one seeded synthetic batch = one osog_render_field call.
 Default workload: BASELINE.json configs[3] (the paper-scale headline: 40,000 mixed particles, 2048 x 2048,
-NA 0.65, 10 degree oblique ramp).  Prints ONE JSON line (see DESIGN.md section 8 for every key).
+NA 0.65, 10 degree oblique ramp).  Prints ONE JSON line (see DESIGN.md section 10 for every key).
 
 --impl reference times the float64 CPU oracle (oracle/) on the host cores, on a bounded sample of the same
 workload; it is a deliberately plain program, a reported baseline and not the target.
@@ -103,7 +103,7 @@ def cpu_baseline(scene, budget_s=12.0):
     t0 = time.perf_counter()
     _sample_rows(scene, rows)                       # warm-up (also builds / loads the oracle library)
     dt = time.perf_counter() - t0
-    rows = int(min(scene.H, max(64, rows * budget_s / max(dt, 1e-3) * 0.5)))
+    rows = int(min(scene.H, max(16, rows * budget_s / max(dt, 1e-3) * 0.5)))
     t0 = time.perf_counter()
     _sample_rows(scene, rows)
     dt = time.perf_counter() - t0
@@ -122,11 +122,12 @@ def run_reference(args):
         return 0
     scene = make_config(args.config)
     vals = []
+    budget = min(4.0, 150.0 / max(1, args.steps + args.warmup))   # whole run stays within a few minutes
     for _ in range(args.warmup):
-        cpu_baseline(scene, budget_s=4.0)
+        cpu_baseline(scene, budget_s=budget)
     last = None
     for _ in range(args.steps):
-        last, _dt = cpu_baseline(scene, budget_s=4.0)
+        last, _dt = cpu_baseline(scene, budget_s=budget)
         vals.append(last["value"])
     v = float(np.mean(vals))
     n0 = int(scene.frame_start[1] - scene.frame_start[0])
@@ -288,8 +289,6 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
-        args.steps = min(args.steps, 3)
-        args.warmup = min(args.warmup, 1)
         return run_reference(args)
     return run_ours(args)
 
