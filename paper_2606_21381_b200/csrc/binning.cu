@@ -138,8 +138,9 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
     }
 
     // ---- H1: derived record (kRecWords words).  Coordinates are pixel offsets from pixel (jc, ic): dx = p dj + ox ----
-    const double jc = fmin(fmax(floor(cx / p), -1.0e6), 1.0e6);
-    const double ic = fmin(fmax(floor(cy / p), -1.0e6), 1.0e6);
+    const double ip = 1.0 / p;
+    const double jc = fmin(fmax(floor(cx * ip), -1.0e6), 1.0e6);      // reference pixel: any nearby pixel will do
+    const double ic = fmin(fmax(floor(cy * ip), -1.0e6), 1.0e6);
     const double ox = (jc + 0.5) * p - cx, oy = (ic + 0.5) * p - cy;
     const double dn = (double)fnp - a.n_medium;
 
@@ -147,8 +148,8 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
     uint32_t* r32u = reinterpret_cast<uint32_t*>(r32);
     double* r64 = reinterpret_cast<double*>(r32 + 16);
     // words 0..7: data of the sub-tile cull (centre in pixel-index coordinates, oriented box, pixel bounding box)
-    r32[0] = (float)(cx / p - 0.5);
-    r32[1] = (float)(cy / p - 0.5);
+    r32[0] = (float)(cx * ip - 0.5);
+    r32[1] = (float)(cy * ip - 0.5);
     r32u[6] = (uint32_t)j0 | ((uint32_t)j1 << 16) | (kind == 1u ? 0x80000000u : 0u);   // bit 31: prism
     r32u[7] = (uint32_t)i0 | ((uint32_t)i1 << 16);
     r32u[11] = (uint32_t)n;
@@ -168,8 +169,9 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
         const double Myy = R10 * i0s * R10 + R11 * i1s * R11 + R12 * i2s * R12;
         const double Myz = R10 * i0s * R20 + R11 * i1s * R21 + R12 * i2s * R22;
         const double Mzz = R20 * i0s * R20 + R21 * i1s * R21 + R22 * i2s * R22;
-        const double Sxx = Mxx - Mxz * Mxz / Mzz, Sxy = Mxy - Mxz * Myz / Mzz, Syy = Myy - Myz * Myz / Mzz;
-        const double T0 = 2.0 / sqrt(Mzz);
+        const double iMzz = 1.0 / Mzz;
+        const double Sxx = Mxx - Mxz * Mxz * iMzz, Sxy = Mxy - Mxz * Myz * iMzz, Syy = Myy - Myz * Myz * iMzz;
+        const double T0 = 2.0 * rsqrt(Mzz);
         // w(dj, di) = F1 - (A dj^2 + B dj di + C di^2 + D dj + E di)
         r64[0] = Sxx * p * p;
         r64[1] = 2.0 * Sxy * p * p;
@@ -184,12 +186,13 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
         const double lmin = fmax(mid - rad, 1.0e-300), lmax = mid + rad;
         double vx = Sxy, vy = lmin - Sxx;        // eigenvector of the small eigenvalue = long axis
         if (fabs(lmin - Syy) > fabs(vy)) { vx = lmin - Syy; vy = Sxy; }
-        double vn = sqrt(vx * vx + vy * vy);
-        if (!(vn > 1.0e-280)) { vx = 1.0; vy = 0.0; vn = 1.0; }
-        r32[2] = (float)(vx / vn);
-        r32[3] = (float)(vy / vn);
-        r32[4] = (float)((1.0 / sqrt(lmin)) / p * (1.0 + 1.0e-5) + cull_pad);
-        r32[5] = (float)((1.0 / sqrt(lmax)) / p * (1.0 + 1.0e-5) + cull_pad);
+        const double vn2 = vx * vx + vy * vy;
+        double ivn = rsqrt(vn2);
+        if (!(vn2 > 1.0e-280)) { vx = 1.0; vy = 0.0; ivn = 1.0; }
+        r32[2] = (float)(vx * ivn);
+        r32[3] = (float)(vy * ivn);
+        r32[4] = (float)(rsqrt(lmin) * ip * (1.0 + 1.0e-5) + cull_pad);
+        r32[5] = (float)(rsqrt(lmax) * ip * (1.0 + 1.0e-5) + cull_pad);
         r32u[8] = 0u;
         r32[9] = (float)(dn * T0);
         r32[10] = 0.0f;
@@ -197,50 +200,52 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
     }
 
     // ---- capped tetragonal prism: 12 half-spaces = 6 centrally symmetric slabs  |n_k . x| <= b_k  (Eq. 1) ----
+    // Everything below is fully unrolled with constant indices (registers, no local memory); slabs are written to the
+    // record in order of decreasing slope |n_xy| / |n_z| (rank by cross-multiplied comparisons, no division).
     const double s = e0, L = e1, hc = e2;
-    const double bn[6][3] = { {1.0, 0.0, 0.0}, {0.0, 1.0, 0.0}, {hc, 0.0, 0.5 * s}, {hc, 0.0, -0.5 * s},
-                              {0.0, hc, 0.5 * s}, {0.0, hc, -0.5 * s} };
+    const double hs2 = 0.5 * s;
     const double bcap = hc * s * 0.5 + s * L * 0.25;
-    double nx[6], ny[6], nz[6], bb[6], G[6];
-    int ord[6];
+    double nx[6], ny[6], nz[6], h2[6], z2[6];
+    // body normals (1,0,0), (0,1,0), (hc,0,s/2), (hc,0,-s/2), (0,hc,s/2), (0,hc,-s/2) rotated to the world frame
+    nx[0] = R00; ny[0] = R10; nz[0] = R20;
+    nx[1] = R01; ny[1] = R11; nz[1] = R21;
+    nx[2] = R00 * hc + R02 * hs2; ny[2] = R10 * hc + R12 * hs2; nz[2] = R20 * hc + R22 * hs2;
+    nx[3] = R00 * hc - R02 * hs2; ny[3] = R10 * hc - R12 * hs2; nz[3] = R20 * hc - R22 * hs2;
+    nx[4] = R01 * hc + R02 * hs2; ny[4] = R11 * hc + R12 * hs2; nz[4] = R21 * hc + R22 * hs2;
+    nx[5] = R01 * hc - R02 * hs2; ny[5] = R11 * hc - R12 * hs2; nz[5] = R21 * hc - R22 * hs2;
 #pragma unroll
-    for (int k = 0; k < 6; ++k) {
-        nx[k] = R00 * bn[k][0] + R01 * bn[k][1] + R02 * bn[k][2];
-        ny[k] = R10 * bn[k][0] + R11 * bn[k][1] + R12 * bn[k][2];
-        nz[k] = R20 * bn[k][0] + R21 * bn[k][1] + R22 * bn[k][2];
-        bb[k] = k < 2 ? 0.5 * s : bcap;
-        const double h = sqrt(nx[k] * nx[k] + ny[k] * ny[k]);
-        G[k] = nz[k] == 0.0 ? 1.0e300 : h / fabs(nz[k]);
-        ord[k] = k;
-    }
-    for (int u = 1; u < 6; ++u) {                // insertion sort, steepest first
-        const int v = ord[u];
-        int t = u - 1;
-        while (t >= 0 && G[ord[t]] < G[v]) { ord[t + 1] = ord[t]; --t; }
-        ord[t + 1] = v;
-    }
+    for (int k = 0; k < 6; ++k) { h2[k] = nx[k] * nx[k] + ny[k] * ny[k]; z2[k] = nz[k] * nz[k]; }
     uint32_t flags = kFlagPrism;
     int ns = 0;
-    for (int q = 0; q < 6; ++q) {
-        const int k = ord[q];
+    const double g0sq = (double)kSteepSlope * (double)kSteepSlope, gasq = kAllF64Slope * kAllF64Slope;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        int q = 0;                                   // rank of slab k: number of slabs steeper than it (ties: lower index first)
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+            if (j == k) continue;
+            const double lhs = h2[j] * z2[k], rhs = h2[k] * z2[j];      // slope_j > slope_k  <=>  lhs > rhs
+            q += (lhs > rhs || (lhs == rhs && j < k)) ? 1 : 0;
+        }
+        const double bk = k < 2 ? hs2 : bcap;
+        double* o4 = r64 + 4 * q;
         if (nz[k] == 0.0) {
             // vertical face pair: no z bound; the line is inside the slab iff |n_x dx + n_y dy| <= b
-            r64[4 * q + 0] = nx[k] * p;
-            r64[4 * q + 1] = ny[k] * p;
-            r64[4 * q + 2] = nx[k] * ox + ny[k] * oy;
-            r64[4 * q + 3] = bb[k];
+            o4[0] = nx[k] * p;
+            o4[1] = ny[k] * p;
+            o4[2] = nx[k] * ox + ny[k] * oy;
+            o4[3] = bk;
             flags |= kFlagAllF64 | (1u << (16 + q));
             ++ns;
         } else {
-            const double sg = nz[k] > 0.0 ? 1.0 : -1.0;
-            const double r = 1.0 / fabs(nz[k]);
-            const double W0 = sg * r * (nx[k] * ox + ny[k] * oy), Cb = bb[k] * r;
-            r64[4 * q + 0] = sg * r * nx[k] * p;          // U:  exit_k = Cx - U dj - V di
-            r64[4 * q + 1] = sg * r * ny[k] * p;          // V:  enter_k = Cn - U dj - V di
-            r64[4 * q + 2] = Cb - W0;                     // Cx
-            r64[4 * q + 3] = -Cb - W0;                    // Cn
-            if (G[k] > kAllF64Slope) flags |= kFlagAllF64;
-            if (G[k] > (double)kSteepSlope) ++ns;
+            const double r = (nz[k] > 0.0 ? 1.0 : -1.0) / fabs(nz[k]);  // sigma / |n_z|
+            const double W0 = r * (nx[k] * ox + ny[k] * oy), Cb = bk * fabs(r);
+            o4[0] = r * nx[k] * p;                    // U:  exit_k = Cx - U dj - V di
+            o4[1] = r * ny[k] * p;                    // V:  enter_k = Cn - U dj - V di
+            o4[2] = Cb - W0;                          // Cx
+            o4[3] = -Cb - W0;                         // Cn
+            if (h2[k] > gasq * z2[k]) flags |= kFlagAllF64;
+            if (h2[k] > g0sq * z2[k]) ++ns;
         }
     }
     if (ns > 2) flags |= kFlagAllF64;            // more than two steep slabs: rare, every pixel goes to fp64
@@ -249,7 +254,7 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
     double ax = R02, ay = R12;
     const double an = sqrt(ax * ax + ay * ay);
     if (an > 1.0e-12) { ax /= an; ay /= an; } else { ax = 1.0; ay = 0.0; }
-    const double hs = 0.5 * s, hl = 0.5 * L, ap = 0.5 * L + hc;
+    const double hs = hs2, hl = 0.5 * L, ap = 0.5 * L + hc;
     double ha = fabs((R02 * ax + R12 * ay) * ap), hb = fabs((-R02 * ay + R12 * ax) * ap);
 #pragma unroll
     for (int v = 0; v < 4; ++v) {
@@ -260,8 +265,8 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
     }
     r32[2] = (float)ax;
     r32[3] = (float)ay;
-    r32[4] = (float)(ha / p * (1.0 + 1.0e-5) + cull_pad);
-    r32[5] = (float)(hb / p * (1.0 + 1.0e-5) + cull_pad);
+    r32[4] = (float)(ha * ip * (1.0 + 1.0e-5) + cull_pad);
+    r32[5] = (float)(hb * ip * (1.0 + 1.0e-5) + cull_pad);
     r32u[8] = flags;
     r32[9] = (float)dn;
     r32[10] = 0.0f;
