@@ -108,7 +108,9 @@ __device__ __forceinline__ void rebase_item(float4* __restrict__ slot, const flo
     const double2 uv = __ldg(c + 2 * q), xn = __ldg(c + 2 * q + 1);    // U, V | Cx, Cn
     if (q == 0) {
         const float4 h2 = __ldg(rec + 2);                              // flags, dn, -, id
-        sw[24] = h2.x; sw[25] = h2.y;
+        const uint32_t flags = __float_as_uint(h2.x);                  // slot word 24 = evaluation code of the survivor:
+        const uint32_t code = (flags & kFlagAllF64) ? 4u : 1u + ((flags >> 8) & 7u);   // 0 ellipsoid, 1 + NS, 4 all-fp64
+        sw[24] = __uint_as_float(code); sw[25] = h2.y;
     }
     const double oj = (double)(wx0 - h3.x), oi = (double)(wy0 - h3.y);
     const double m = fma(uv.x, oj, uv.y * oi);
@@ -350,19 +352,22 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
         // ---- all lanes walk the survivors in ascending order ------------------------------------------------------------------
         const float4* slot = my_slots;
         for (int sv = 0; sv < nsv; ++sv, slot += kSlotStride4) {
-            const float4 h = slot[6];                            // flags, dn, -, particle index
-            const uint32_t flags = __float_as_uint(h.x);
-            const float4* rec = recs4 + (size_t)__float_as_uint(h.w) * (kRecWords / 4);
-            if (!(flags & kFlagPrism)) {
+            const float4 h = slot[6];                            // code, dn | K, -, particle index
+            const uint32_t code = __float_as_uint(h.x);
+            if (code == 1u) {
+                eval_prism<0>(slot, nullptr, h.y, g, acc);
+            } else if (code == 0u) {
                 eval_ellipsoid(slot, h.y, g, acc);
-            } else if (flags & kFlagAllF64) {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) acc[k] += prism_f64_px(rec, (double)(g.xf + (float)k), (double)g.yf);
+            } else if (code == 2u) {
+                eval_prism<1>(slot, nullptr, h.y, g, acc);
             } else {
-                const int ns = (flags >> 8) & 7;
-                if (ns == 0) eval_prism<0>(slot, rec, h.y, g, acc);
-                else if (ns == 1) eval_prism<1>(slot, rec, h.y, g, acc);
-                else eval_prism<2>(slot, rec, h.y, g, acc);
+                const float4* rec = recs4 + (size_t)__float_as_uint(h.w) * (kRecWords / 4);
+                if (code == 3u) {
+                    eval_prism<2>(slot, rec, h.y, g, acc);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) acc[k] += prism_f64_px(rec, (double)(g.xf + (float)k), (double)g.yf);
+                }
             }
         }
         __syncwarp();
