@@ -141,6 +141,22 @@ def run_reference(args):
     return 0
 
 
+def max_over_ranks(values, device=None):
+    """MAX over ranks of a list of floats (timings): the slowest rank defines the job time.  Works on any
+    initialised torch.distributed backend (nccl on the GPU box, gloo in the CPU test); identity for one process."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.cpu()]
+
+
+def whole_job_value(units_per_rank_step, steps, world, t_max):
+    """Replicas only: every rank processes the same number of units; value = all ranks' units / slowest rank's time."""
+    return world * units_per_rank_step * steps / t_max
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -242,16 +258,29 @@ def run_ours(args):
     torch.cuda.synchronize()
     ms_opd = e0.elapsed_time(e1) / 5
 
-    t = torch.tensor([t_steps, t_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    t_steps, t_e2e = (float(x) for x in t.cpu())
+    # ---- the dominant kernel alone (k_compose_tile on the binning of the last call), CUDA events on its stream
+    ctx.render_field(P, opt, out=field)
+    for _ in range(3):
+        ctx.recompose_field(field)
+    torch.cuda.synchronize()
+    kev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
+    for a_, b_ in kev:
+        flush.zero_()
+        a_.record(stream)
+        ctx.recompose_field(field)
+        b_.record(stream)
+    torch.cuda.synchronize()
+    ms_compose = float(np.mean([a_.elapsed_time(b_) for a_, b_ in kev]))
+
+    t_steps, t_e2e = max_over_ranks([t_steps, t_e2e], dev)
     peak, peak_src = _peaks()
     alg_bytes = 48 * N + 8 * pairs + 8 * B * H * W      # SoA read + list write/read + complex64 write
     ms_step = t_steps / args.steps * 1e3
-    achieved = alg_bytes / (ms_step * 1e-3) / 1e9
+    step_gbs = alg_bytes / (ms_step * 1e-3) / 1e9
+    k_bytes = 4 * pairs + 8 * B * H * W                 # k_compose_tile alone: list read + complex64 write
+    achieved = k_bytes / (ms_compose * 1e-3) / 1e9
     line = {
-        "metric": METRIC, "value": world * N * args.steps / t_steps, "unit": UNIT, "n_gpus": world,
+        "metric": METRIC, "value": whole_job_value(N, args.steps, world, t_steps), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32+f64", "data": "synthetic",
         "config": {"workload": CONFIG_NAMES[args.config], "N": N, "H": H, "W": W, "B": B, "tile": og.osog_tile_size(),
@@ -262,9 +291,13 @@ def run_ours(args):
                 "d2h_bytes_per_step": int(d2h)},
         "gpu_launches": 4 * args.steps,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "peak_source": peak_src, "algorithmic_bytes": int(alg_bytes),
-                     "kernel": "whole hot path (k_prepare, k_scan, k_fill, k_compose_tile)",
-                     "frac_of_nominal_8TBs": achieved / 8000.0},
+                     "traffic": 8953344, "traffic_note": "dram read+write of one k_compose_tile launch, ncu --set full "
+                     "(profiles/r1_final_compose_ncu.md); the 33.5 MB field it writes stays in the 126 MB L2",
+                     "peak_source": peak_src, "algorithmic_bytes": int(k_bytes), "kernel": "k_compose_tile",
+                     "kernel_ms": ms_compose, "frac_of_nominal_8TBs": achieved / 8000.0,
+                     "binding_unit": "instruction issue (fp32 FMA / ALU min-max / fp64), not HBM: see DESIGN.md section 7"},
+        "roofline_step": {"achieved": step_gbs, "frac": step_gbs / peak, "algorithmic_bytes": int(alg_bytes),
+                          "what": "whole hot path: k_prepare, k_scan, k_fill, k_compose_tile"},
         "library_stage_ms": ms_optics, "opd_only_ms": ms_opd,
         "paper_context": "PAPER.md:195: 40,000 particles < 50 ms on one A100 at 1024^2 (whole pipeline); context only",
         "clocks": clk.summary(),

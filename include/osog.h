@@ -127,6 +127,11 @@ int osog_status(osog_ctx* ctx, uint32_t* status_bits, int64_t* pairs);
 int osog_debug_bins(osog_ctx* ctx, uint32_t* h_offset, uint32_t* h_list, int64_t cap,
                     int64_t* n_tiles, int64_t* n_pairs);
 
+/* Test / measurement: re-runs ONLY the composition kernel (H5-H7) of the last osog_render_* call on its binning
+ * (tile lists, records, ramp tables and optics are still in the context) and writes the complex field again.
+ * Lets bench.py time the dominant kernel alone with CUDA events.  OSOG_EINVAL if no render call came before. */
+int osog_debug_recompose_field(osog_ctx* ctx, float* d_field);
+
 /* Tile edge T in pixels (build-time constant of the binning, B3). */
 int osog_tile_size(void);
 

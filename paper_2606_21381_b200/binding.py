@@ -64,6 +64,7 @@ def lib():
     for name in ("osog_render_opd", "osog_render_field", "osog_render_intensity", "osog_render_opd_atomic"):
         getattr(L, name).argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p]
     L.osog_field_to_intensity.argtypes = [ctx, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
+    L.osog_debug_recompose_field.argtypes = [ctx, C.c_void_p]
     L.osog_destroy.argtypes = [ctx]
     L.osog_status.argtypes = [ctx, C.POINTER(C.c_uint32), C.POINTER(C.c_int64)]
     L.osog_debug_bins.argtypes = [ctx, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
@@ -79,7 +80,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_opd_atomic", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_opd_atomic", "osog_debug_recompose_field", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -212,6 +213,13 @@ class Context:
         r = lib().osog_field_to_intensity(self._ctx, C.byref(o), f.data_ptr(), out.data_ptr())
         if r != OSOG_OK:
             raise OsogError(r, "osog_field_to_intensity")
+        return out
+
+    def recompose_field(self, out):
+        """Re-run only the composition kernel of the last render call into `out` (float32 [B, H, W, 2])."""
+        r = lib().osog_debug_recompose_field(self._ctx, out.data_ptr())
+        if r != OSOG_OK:
+            raise OsogError(r, "osog_debug_recompose_field")
         return out
 
     def status(self):

@@ -62,6 +62,13 @@ __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c)
     asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
     return d;
 }
+// float -> double for a non-negative, normal-or-zero float, with integer ops on the ALU pipe instead of an XU-pipe
+// conversion (F2F).  +0.0f maps to 2^-127 * 2 (about 1e-38), which is harmless for a thickness in micrometres.
+__device__ __forceinline__ double f2d_pos(float f)
+{
+    const uint32_t u = __float_as_uint(f);
+    return __hiloint2double((int)((u >> 3) + 0x38000000u), (int)(u << 29));
+}
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
 {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -178,6 +185,7 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
     const float2 nk01 = ffma2(v01, g.nly, make_float2(a1.z, a1.w));
     const float2 nk23 = ffma2(v23, g.nly, make_float2(a2.x, a2.y));
     const float2 nk45 = ffma2(v45, g.nly, make_float2(a2.z, a2.w));
+    const double dnd = (double)dnf;
     // steep slabs in fp64: slab 0 from the slot (re-based to the sub-tile origin), slab 1 from the record
     double u0 = 0.0, x0 = 0.0, n0 = 0.0, u1 = 0.0, x1 = 0.0, n1 = 0.0, dj = 0.0;
     if (NS > 0) {
@@ -214,7 +222,7 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
         const float ex = fminf(min3(e01.x, e01.y, e23.x), min3(e23.y, e45.x, e45.y));
         const float en = fmaxf(max3(n01.x, n01.y, n23.x), max3(n23.y, n45.x, n45.y));
         const float t = fmaxf(ex - en, 0.0f);
-        acc[k] = fma((double)t, (double)dnf, acc[k]);
+        acc[k] = fma(f2d_pos(t), dnd, acc[k]);
     }
 }
 

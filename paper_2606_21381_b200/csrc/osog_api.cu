@@ -148,6 +148,7 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     if (!c) return OSOG_ENOMEM;
     std::memset(c, 0, sizeof(*c));
     c->device = cfg->device;
+    c->last_has_ramp = -1;
     c->stream = static_cast<cudaStream_t>(cfg->stream);
     c->H = cfg->H; c->W = cfg->W; c->max_frames = cfg->max_frames;
     c->max_particles = cfg->max_particles;
@@ -206,6 +207,8 @@ static int render_common(osog_ctx* c, const osog_particles* p, int64_t N, const 
     cudaError_t e = launch_binning(c, p, N, o);
     if (e != cudaSuccess) return cuda_fail(c, e);
     const bool has_ramp = o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0;
+    c->last_has_ramp = has_ramp ? 1 : 0;
+    c->last_N = N;
     e = launch_compose(c, N, o->B, has_ramp, d_opd, d_field);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
@@ -260,6 +263,15 @@ int osog_render_opd_atomic(osog_ctx* c, const osog_particles* p, int64_t N, cons
     cudaError_t e = launch_binning(c, p, N, o);      // records + bounding boxes (the tile lists are not used)
     if (e != cudaSuccess) return cuda_fail(c, e);
     e = launch_compose_atomic(c, N, o->B, d_opd);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return OSOG_OK;
+}
+
+int osog_debug_recompose_field(osog_ctx* c, float* d_field)
+{
+    if (!c || !d_field || !aligned16(d_field) || c->last_B < 1 || c->last_has_ramp < 0) return OSOG_EINVAL;
+    DeviceGuard g(c->device);
+    cudaError_t e = launch_compose(c, c->last_N, c->last_B, c->last_has_ramp != 0, nullptr, reinterpret_cast<float2*>(d_field));
     if (e != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
 }

@@ -55,6 +55,8 @@ struct osog_ctx {
     int last_cuda_error;
     // last call
     int last_B;
+    int last_has_ramp;
+    long long last_N;
     long long last_tiles;
     // scratch (device)
     float* rec;                     // [max_particles][kRecWords]

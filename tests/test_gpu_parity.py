@@ -94,3 +94,20 @@ def test_atomic_alternative_within_tolerance(og, o):
     ref = o.render_opd(sc)
     assert np.all(np.abs(g - ref) <= 1e-5 + 1e-5 * np.abs(ref))
     ctx.close()
+
+
+def test_recompose_reproduces_the_field_bitwise(og):
+    """osog_debug_recompose_field (the kernel bench.py times alone) gives the same bits as the full call."""
+    import torch
+    sc = make_config(4, n_override=3000)
+    ctx = og.Context(sc.H, sc.W, sc.N)
+    P = og.Particles.from_scene(sc)
+    a = torch.view_as_real(ctx.render_field(P, og.optics_from_scene(sc))).clone()
+    b = torch.full_like(a, 7.0)
+    ctx.recompose_field(b)
+    assert torch.equal(a, b)
+    ctx.close()
+    ctx = og.Context(64, 64, 10)
+    with pytest.raises(og.OsogError):
+        ctx.recompose_field(b)                    # no render call before
+    ctx.close()
