@@ -150,7 +150,8 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
     // words 0..7: data of the sub-tile cull (centre in pixel-index coordinates, oriented box, pixel bounding box)
     r32[0] = (float)(cx * ip - 0.5);
     r32[1] = (float)(cy * ip - 0.5);
-    r32u[6] = (uint32_t)j0 | ((uint32_t)j1 << 16) | (kind == 1u ? 0x80000000u : 0u);   // bit 31: prism
+    // bits 15 of both words and bit 31 of the second carry the evaluation code (0 ellipsoid, 1 + steep slabs, 4 all-fp64)
+    r32u[6] = (uint32_t)j0 | ((uint32_t)j1 << 16);
     r32u[7] = (uint32_t)i0 | ((uint32_t)i1 << 16);
     r32u[11] = (uint32_t)n;
     reinterpret_cast<int*>(r32)[12] = (int)jc;
@@ -268,6 +269,11 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
     r32[4] = (float)(ha * ip * (1.0 + 1.0e-5) + cull_pad);
     r32[5] = (float)(hb * ip * (1.0 + 1.0e-5) + cull_pad);
     r32u[8] = flags;
+    {
+        const uint32_t code = (flags & kFlagAllF64) ? 4u : 1u + (uint32_t)ns;
+        r32u[6] |= (code & 1u) << 15;
+        r32u[7] |= ((code >> 1) & 1u) << 15 | ((code >> 2) & 1u) << 31;
+    }
     r32[9] = (float)dn;
     r32[10] = 0.0f;
 }

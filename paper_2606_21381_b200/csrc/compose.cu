@@ -4,7 +4,7 @@
 //   3. per warp (16 x 8 pixel sub-tile, 4 x 1 pixels per lane): one lane per staged particle tests the particle's
 //      pixel bounding box and oriented box against the sub-tile (ballot compaction keeps ascending order) and
 //      re-bases the survivor's fp64 coefficients to the sub-tile origin, rounding them to fp32 only there,
-//   4. all lanes walk the survivors: ray-convex thickness from the re-based coefficients (packed fp32 FMA and
+//   4. all lanes walk the survivors (grouped by evaluation class, one branch-free loop per class): ray-convex thickness from the re-based coefficients (packed fp32 FMA and
 //      3-input min/max for the prism slabs, fp64 quadratic + fp32 sqrt for the ellipsoid), OPD accumulated per
 //      pixel in fp64 registers,
 //   5. write OPD and / or exp(i 2 pi OPD / lambda) * ramp straight from the registers.
@@ -114,10 +114,7 @@ __device__ __forceinline__ void rebase_item(float4* __restrict__ slot, const flo
     const double2* c = reinterpret_cast<const double2*>(rec + 4);
     const double2 uv = __ldg(c + 2 * q), xn = __ldg(c + 2 * q + 1);    // U, V | Cx, Cn
     if (q == 0) {
-        const float4 h2 = __ldg(rec + 2);                              // flags, dn, -, id
-        const uint32_t flags = __float_as_uint(h2.x);                  // slot word 24 = evaluation code of the survivor:
-        const uint32_t code = (flags & kFlagAllF64) ? 4u : 1u + ((flags >> 8) & 7u);   // 0 ellipsoid, 1 + NS, 4 all-fp64
-        sw[24] = __uint_as_float(code); sw[25] = h2.y;
+        sw[25] = __ldg(reinterpret_cast<const float*>(rec) + 9);         // dn
     }
     const double oj = (double)(wx0 - h3.x), oi = (double)(wy0 - h3.y);
     const double m = fma(uv.x, oj, uv.y * oi);
@@ -314,15 +311,15 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
     for (uint32_t base = 0; base < L; base += 32) {
         // ---- cull: lane <-> particle base + lane; records are read through L1 / L2 (10 MB, L2 resident) -----------------
         const uint32_t k = base + lane;
-        bool keep = false, is_prism = false;
-        uint32_t pid = 0;
+        bool keep = false;
+        uint32_t pid = 0, code = 0;
         if (k < L) {
             pid = in_smem ? s_ids[k] : glist[k];
             const float4* rec = recs4 + (size_t)pid * (kRecWords / 4);
             const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);   // cxp, cyp, ax, ay | ha, hb, bbx, bby
             const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
-            const int pj0 = bx & 0x7fff, pj1 = (bx >> 16) & 0x7fff, pi0 = by & 0xffff, pi1 = by >> 16;
-            is_prism = (bx >> 31) != 0u;
+            const int pj0 = bx & 0x7fff, pj1 = (bx >> 16) & 0x7fff, pi0 = by & 0x7fff, pi1 = (by >> 16) & 0x7fff;
+            code = ((bx >> 15) & 1u) | (((by >> 15) & 1u) << 1) | ((by >> 31) << 2);
             keep = pj0 <= wx0 + 15 && pj1 >= wx0 && pi0 <= wy0 + 7 && pi1 >= wy0;
             // separating-axis test against the particle's oriented box (the silhouette lies inside it)
             const float ddx = rcx - h0.x, ddy = rcy - h0.y;
@@ -330,54 +327,58 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
             const float ra = 7.5f * fabsf(h0.z) + 3.5f * fabsf(h0.w), rb = 7.5f * fabsf(h0.w) + 3.5f * fabsf(h0.z);
             keep = keep && pa <= h1.x + ra && pb <= h1.y + rb;
         }
-        const unsigned m = __ballot_sync(0xffffffffu, keep);
-        const unsigned mp = __ballot_sync(0xffffffffu, keep && is_prism);
-        const int nsv = __popc(m), npr = __popc(mp);
+        // Survivors are grouped by evaluation class (fixed, data-dependent order: NS0 prisms, NS1, NS2, all-fp64,
+        // ellipsoids; ascending particle index inside a class), so each class runs in its own branch-free loop.
+        const unsigned m1 = __ballot_sync(0xffffffffu, keep && code == 1u);
+        const unsigned m2 = __ballot_sync(0xffffffffu, keep && code == 2u);
+        const unsigned m3 = __ballot_sync(0xffffffffu, keep && code == 3u);
+        const unsigned m4 = __ballot_sync(0xffffffffu, keep && code == 4u);
+        const unsigned m0 = __ballot_sync(0xffffffffu, keep && code == 0u);
+        const int n1 = __popc(m1), n2 = __popc(m2), n3 = __popc(m3), n4 = __popc(m4), n0 = __popc(m0);
         if (keep) {
             const unsigned lt = (1u << lane) - 1u;
-            const int pos = __popc(m & lt);
-            uint32_t* sw = reinterpret_cast<uint32_t*>(my_slots + pos * kSlotStride4);
-            sw[27] = pid;
-            if (is_prism) reinterpret_cast<uint32_t*>(my_slots + __popc(mp & lt) * kSlotStride4)[26] = (uint32_t)pos;
-            else {                                               // ellipsoid: copy the record's doubles into the slot
+            int pos;
+            if (code == 1u) pos = __popc(m1 & lt);
+            else if (code == 2u) pos = n1 + __popc(m2 & lt);
+            else if (code == 3u) pos = n1 + n2 + __popc(m3 & lt);
+            else if (code == 4u) pos = n1 + n2 + n3 + __popc(m4 & lt);
+            else pos = n1 + n2 + n3 + n4 + __popc(m0 & lt);
+            float4* sl = my_slots + pos * kSlotStride4;
+            reinterpret_cast<uint32_t*>(sl)[27] = pid;
+            if (code == 0u) {                                    // ellipsoid: copy the record's doubles into the slot
                 const float4* rec = recs4 + (size_t)pid * (kRecWords / 4);
-                float4* sl = my_slots + pos * kSlotStride4;
                 const float4 c0 = __ldg(rec + 4), c1 = __ldg(rec + 5), c2 = __ldg(rec + 6), c3 = __ldg(rec + 7);
                 const float K = __ldg(reinterpret_cast<const float*>(rec) + 9);
                 sl[0] = c0; sl[1] = c1; sl[2] = c2; sl[3] = c3;
-                sw[24] = 0u;
-                reinterpret_cast<float*>(sw)[25] = K;
+                reinterpret_cast<float*>(sl)[25] = K;
             }
         }
         __syncwarp();
-        // ---- re-base the prisms: one lane per (prism survivor, slab) ----------------------------------------------------------
+        // ---- re-base the prisms (classes 1..3 occupy slots 0 .. n1+n2+n3-1): one lane per (prism, slab) -----------------------
+        const int npr = n1 + n2 + n3;
         for (int it = lane; it < npr * 6; it += 32) {
             const int r = it / 6;
-            const uint32_t pos = reinterpret_cast<const uint32_t*>(my_slots + r * kSlotStride4)[26];
-            rebase_item(my_slots + pos * kSlotStride4, a.rec, it - 6 * r, wx0, wy0);
+            rebase_item(my_slots + r * kSlotStride4, a.rec, it - 6 * r, wx0, wy0);
         }
         __syncwarp();
-        // ---- all lanes walk the survivors in ascending order ------------------------------------------------------------------
+        // ---- all lanes walk the survivors, class by class ----------------------------------------------------------------------
         const float4* slot = my_slots;
-        for (int sv = 0; sv < nsv; ++sv, slot += kSlotStride4) {
-            const float4 h = slot[6];                            // code, dn | K, -, particle index
-            const uint32_t code = __float_as_uint(h.x);
-            if (code == 1u) {
-                eval_prism<0>(slot, nullptr, h.y, g, acc);
-            } else if (code == 0u) {
-                eval_ellipsoid(slot, h.y, g, acc);
-            } else if (code == 2u) {
-                eval_prism<1>(slot, nullptr, h.y, g, acc);
+#pragma unroll 1
+        for (int sv = 0; sv < n1; ++sv, slot += kSlotStride4) eval_prism<0>(slot, nullptr, slot[6].y, g, acc);
+#pragma unroll 1
+        for (int sv = 0; sv < n2; ++sv, slot += kSlotStride4) eval_prism<1>(slot, nullptr, slot[6].y, g, acc);
+#pragma unroll 1
+        for (int sv = 0; sv < n3 + n4; ++sv, slot += kSlotStride4) {
+            const float4* rec = recs4 + (size_t)__float_as_uint(slot[6].w) * (kRecWords / 4);
+            if (sv < n3) {
+                eval_prism<2>(slot, rec, slot[6].y, g, acc);
             } else {
-                const float4* rec = recs4 + (size_t)__float_as_uint(h.w) * (kRecWords / 4);
-                if (code == 3u) {
-                    eval_prism<2>(slot, rec, h.y, g, acc);
-                } else {
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) acc[k] += prism_f64_px(rec, (double)(g.xf + (float)k), (double)g.yf);
-                }
+                for (int k = 0; k < 4; ++k) acc[k] += prism_f64_px(rec, (double)(g.xf + (float)k), (double)g.yf);
             }
         }
+#pragma unroll 1
+        for (int sv = 0; sv < n0; ++sv, slot += kSlotStride4) eval_ellipsoid(slot, slot[6].y, g, acc);
         __syncwarp();
     }
 
@@ -471,7 +472,7 @@ __global__ void __launch_bounds__(256) k_compose_atomic(const float* __restrict_
     const float4 h1 = rec[1], h2 = rec[2];
     const int4 h3 = *reinterpret_cast<const int4*>(rec + 3);
     const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
-    const int j0 = bx & 0x7fff, j1 = (bx >> 16) & 0x7fff, i0 = by & 0xffff, i1 = by >> 16;
+    const int j0 = bx & 0x7fff, j1 = (bx >> 16) & 0x7fff, i0 = by & 0x7fff, i1 = (by >> 16) & 0x7fff;
     const uint32_t flags = __float_as_uint(h2.x);
     const double* c = reinterpret_cast<const double*>(rec + 4);
     const double K = (double)h2.y;
