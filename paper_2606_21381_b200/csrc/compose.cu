@@ -149,7 +149,7 @@ __device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ slot, 
         const double djk = dj + (double)k;
         const double w = fma(-fma(ab.x, djk, b1), djk, cc);      // 1 - d^T S d
         const float t = fast_sqrt(fmaxf((float)w, 0.0f));
-        acc[k] = fma((double)t, Kd, acc[k]);
+        acc[k] = fma(f2d_pos(t), Kd, acc[k]);
     }
 }
 
