@@ -41,10 +41,10 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
 
     if (gid < a.B && gid < kOpticsChunk) a.optics[gid] = a.oc.f[gid];
 
-    if (gid >= a.N) {
+    if (gid >= 2 * a.N) {
         // ---- phase-ramp tables exp(i 2 pi fx0 x_j), x_j = (j + 1/2) p  (oblique illumination)
         if (!a.has_ramp) return;
-        long long r = gid - a.N;
+        long long r = gid - 2 * a.N;
         const long long nx = (long long)a.B * a.W, ny = (long long)a.B * a.H;
         if (r < nx) {
             const int b = (int)(r / a.W), j = (int)(r % a.W);
@@ -59,8 +59,10 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
         return;
     }
 
-    // ---- H1/H2: one particle ---------------------------------------------------------------------------------
-    const long long n = gid;
+    // ---- H1/H2: one particle = two threads: role 0 does the binning (bounding box, tile range, counts), role 1 the
+    // derived record (the two halves are independent; splitting them halves the latency-bound critical path)
+    const long long n = gid >> 1;
+    const int role = (int)(gid & 1);
     const float fcx = a.cx[n], fcy = a.cy[n], fqw = a.qw[n], fqx = a.qx[n], fqy = a.qy[n], fqz = a.qz[n];
     const float fd0 = a.d0[n], fd1 = a.d1[n], fd2 = a.d2[n], fnp = a.n_p[n];
     const unsigned kind = a.kind[n];
@@ -77,12 +79,13 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
         }
         b = lo;
     }
-    a.pframe[n] = b;
-
     int4 tb = make_int4(1, 0, 1, 0);             // empty tile range
+    if (role == 0) a.pframe[n] = b;
     if (!valid) {
-        atomicOr(&a.status->bits, OSOG_WBADPARTICLE);
-        a.tbox[n] = tb;
+        if (role == 0) {
+            atomicOr(&a.status->bits, OSOG_WBADPARTICLE);
+            a.tbox[n] = tb;
+        }
         return;
     }
 
@@ -95,6 +98,10 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
     const double R20 = 2.0 * (x * z - w * y), R21 = 2.0 * (y * z + w * x), R22 = 1.0 - 2.0 * (x * x + y * y);
     const double e0 = fd0, e1 = fd1, e2 = fd2;
 
+    float* r32 = a.rec + (size_t)n * kRecWords;
+    uint32_t* r32u = reinterpret_cast<uint32_t*>(r32);
+    const double ip = 1.0 / p;
+    if (role == 0) {
     // B1: half extents of the projection
     double hx, hy;
     if (kind == 0u) {
@@ -137,27 +144,28 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
             for (int tx = tb.x; tx <= tb.y; ++tx) atomicAdd(&cnt[ty * a.ntx + tx], 1u);
     }
 
-    // ---- H1: derived record (kRecWords words).  Coordinates are pixel offsets from pixel (jc, ic): dx = p dj + ox ----
-    const double ip = 1.0 / p;
+    // words 0, 1, 6, 7 of the record: centre in pixel-index coordinates and the packed pixel bounding box
+    r32[0] = (float)(cx * ip - 0.5);
+    r32[1] = (float)(cy * ip - 0.5);
+    r32u[6] = (uint32_t)j0 | ((uint32_t)j1 << 16);
+    r32u[7] = (uint32_t)i0 | ((uint32_t)i1 << 16);
+    return;
+    }
+
+    // ---- H1 (role 1): derived record.  Coordinates are pixel offsets from pixel (jc, ic): dx = p dj + ox ----
     const double jc = fmin(fmax(floor(cx * ip), -1.0e6), 1.0e6);      // reference pixel: any nearby pixel will do
     const double ic = fmin(fmax(floor(cy * ip), -1.0e6), 1.0e6);
     const double ox = (jc + 0.5) * p - cx, oy = (ic + 0.5) * p - cy;
     const double dn = (double)fnp - a.n_medium;
-
-    float* r32 = a.rec + (size_t)n * kRecWords;
-    uint32_t* r32u = reinterpret_cast<uint32_t*>(r32);
     double* r64 = reinterpret_cast<double*>(r32 + 16);
-    // words 0..7: data of the sub-tile cull (centre in pixel-index coordinates, oriented box, pixel bounding box)
-    r32[0] = (float)(cx * ip - 0.5);
-    r32[1] = (float)(cy * ip - 0.5);
-    // bits 15 of both words and bit 31 of the second carry the evaluation code (0 ellipsoid, 1 + steep slabs, 4 all-fp64)
-    r32u[6] = (uint32_t)j0 | ((uint32_t)j1 << 16);
-    r32u[7] = (uint32_t)i0 | ((uint32_t)i1 << 16);
     r32u[11] = (uint32_t)n;
     reinterpret_cast<int*>(r32)[12] = (int)jc;
     reinterpret_cast<int*>(r32)[13] = (int)ic;
     r32[14] = 0.0f;
     r32[15] = 0.0f;
+    // Words 2..5: oriented box of the silhouette (unit axis with a_x >= 0, half lengths > 0); their sign bits carry the
+    // evaluation code of the particle (0 ellipsoid, 1 + number of steep slabs, 4 all-fp64): bit 0 in the sign of
+    // the first half length, bit 1 in the second, bit 2 in the sign of a_x.
     const double cull_pad = 1.0 / 64.0;          // px; covers the fp32 rounding of the cull test
 
     if (kind == 0u) {
@@ -190,7 +198,8 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
         const double vn2 = vx * vx + vy * vy;
         double ivn = rsqrt(vn2);
         if (!(vn2 > 1.0e-280)) { vx = 1.0; vy = 0.0; ivn = 1.0; }
-        r32[2] = (float)(vx * ivn);
+        if (vx < 0.0) { vx = -vx; vy = -vy; }
+        r32[2] = fabsf((float)(vx * ivn));
         r32[3] = (float)(vy * ivn);
         r32[4] = (float)(rsqrt(lmin) * ip * (1.0 + 1.0e-5) + cull_pad);
         r32[5] = (float)(rsqrt(lmax) * ip * (1.0 + 1.0e-5) + cull_pad);
@@ -264,16 +273,13 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
         ha = fmax(ha, fabs(px * ax + py * ay));
         hb = fmax(hb, fabs(-px * ay + py * ax));
     }
-    r32[2] = (float)ax;
+    if (ax < 0.0) { ax = -ax; ay = -ay; }
+    const uint32_t code = (flags & kFlagAllF64) ? 4u : 1u + (uint32_t)ns;
+    r32u[2] = (__float_as_uint((float)ax) & 0x7fffffffu) | ((code >> 2) << 31);
     r32[3] = (float)ay;
-    r32[4] = (float)(ha * ip * (1.0 + 1.0e-5) + cull_pad);
-    r32[5] = (float)(hb * ip * (1.0 + 1.0e-5) + cull_pad);
+    r32u[4] = __float_as_uint((float)(ha * ip * (1.0 + 1.0e-5) + cull_pad)) | ((code & 1u) << 31);
+    r32u[5] = __float_as_uint((float)(hb * ip * (1.0 + 1.0e-5) + cull_pad)) | (((code >> 1) & 1u) << 31);
     r32u[8] = flags;
-    {
-        const uint32_t code = (flags & kFlagAllF64) ? 4u : 1u + (uint32_t)ns;
-        r32u[6] |= (code & 1u) << 15;
-        r32u[7] |= ((code >> 1) & 1u) << 15 | ((code >> 2) & 1u) << 31;
-    }
     r32[9] = (float)dn;
     r32[10] = 0.0f;
 }
@@ -407,7 +413,7 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     a.has_ramp = (o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0) ? 1 : 0;
     if ((e = upload_optics(c, o, &a.oc)) != cudaSuccess) return e;
 
-    long long items = N + (a.has_ramp ? (long long)B * (c->W + c->H) : 0);
+    long long items = 2 * N + (a.has_ramp ? (long long)B * (c->W + c->H) : 0);
     if (items < B) items = B;
     const int threads = 128;
     const long long blocks = (items + threads - 1) / threads;

@@ -318,14 +318,16 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
             const float4* rec = recs4 + (size_t)pid * (kRecWords / 4);
             const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);   // cxp, cyp, ax, ay | ha, hb, bbx, bby
             const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
-            const int pj0 = bx & 0x7fff, pj1 = (bx >> 16) & 0x7fff, pi0 = by & 0x7fff, pi1 = (by >> 16) & 0x7fff;
-            code = ((bx >> 15) & 1u) | (((by >> 15) & 1u) << 1) | ((by >> 31) << 2);
+            const int pj0 = bx & 0xffff, pj1 = bx >> 16, pi0 = by & 0xffff, pi1 = by >> 16;
+            // evaluation code in the sign bits of the (positive) half lengths and of a_x (a_x >= 0 by construction)
+            code = (__float_as_uint(h1.x) >> 31) | ((__float_as_uint(h1.y) >> 31) << 1) | ((__float_as_uint(h0.z) >> 31) << 2);
             keep = pj0 <= wx0 + 15 && pj1 >= wx0 && pi0 <= wy0 + 7 && pi1 >= wy0;
             // separating-axis test against the particle's oriented box (the silhouette lies inside it)
+            const float axx = fabsf(h0.z), ayy = h0.w, ha = fabsf(h1.x), hb = fabsf(h1.y);
             const float ddx = rcx - h0.x, ddy = rcy - h0.y;
-            const float pa = fabsf(ddx * h0.z + ddy * h0.w), pb = fabsf(ddy * h0.z - ddx * h0.w);
-            const float ra = 7.5f * fabsf(h0.z) + 3.5f * fabsf(h0.w), rb = 7.5f * fabsf(h0.w) + 3.5f * fabsf(h0.z);
-            keep = keep && pa <= h1.x + ra && pb <= h1.y + rb;
+            const float pa = fabsf(ddx * axx + ddy * ayy), pb = fabsf(ddy * axx - ddx * ayy);
+            const float ra = 7.5f * axx + 3.5f * fabsf(ayy), rb = 7.5f * fabsf(ayy) + 3.5f * axx;
+            keep = keep && pa <= ha + ra && pb <= hb + rb;
         }
         // Survivors are grouped by evaluation class (fixed, data-dependent order: NS0 prisms, NS1, NS2, all-fp64,
         // ellipsoids; ascending particle index inside a class), so each class runs in its own branch-free loop.
@@ -472,7 +474,7 @@ __global__ void __launch_bounds__(256) k_compose_atomic(const float* __restrict_
     const float4 h1 = rec[1], h2 = rec[2];
     const int4 h3 = *reinterpret_cast<const int4*>(rec + 3);
     const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
-    const int j0 = bx & 0x7fff, j1 = (bx >> 16) & 0x7fff, i0 = by & 0x7fff, i1 = (by >> 16) & 0x7fff;
+    const int j0 = bx & 0xffff, j1 = bx >> 16, i0 = by & 0xffff, i1 = by >> 16;
     const uint32_t flags = __float_as_uint(h2.x);
     const double* c = reinterpret_cast<const double*>(rec + 4);
     const double K = (double)h2.y;
