@@ -258,6 +258,14 @@ def run_ours(args):
     torch.cuda.synchronize()
     ms_opd = e0.elapsed_time(e1) / 5
 
+    # ---- measured alternative (paper-style global atomicAdd scatter), OPD only, for the record
+    e0.record(stream)
+    for _ in range(3):
+        ctx.render_opd_atomic(P, opt, out=inten)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_atomic = e0.elapsed_time(e1) / 3
+
     # ---- the dominant kernel alone (k_compose_tile on the binning of the last call), CUDA events on its stream
     ctx.render_field(P, opt, out=field)
     for _ in range(3):
@@ -298,7 +306,7 @@ def run_ours(args):
                      "binding_unit": "instruction issue (fp32 FMA / ALU min-max / fp64), not HBM: see DESIGN.md section 7"},
         "roofline_step": {"achieved": step_gbs, "frac": step_gbs / peak, "algorithmic_bytes": int(alg_bytes),
                           "what": "whole hot path: k_prepare, k_scan, k_fill, k_compose_tile"},
-        "library_stage_ms": ms_optics, "opd_only_ms": ms_opd,
+        "library_stage_ms": ms_optics, "opd_only_ms": ms_opd, "atomic_alternative_opd_ms": ms_atomic,
         "paper_context": "PAPER.md:195: 40,000 particles < 50 ms on one A100 at 1024^2 (whole pipeline); context only",
         "clocks": clk.summary(),
     }

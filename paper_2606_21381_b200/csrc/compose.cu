@@ -277,12 +277,30 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
         uint32_t* s_in = reinterpret_cast<uint32_t*>(s_slots);   // kSmemSlots >= kSmemIds
         for (uint32_t k = tid; k < L; k += kComposeThreads) s_in[k] = glist[k];
         __syncthreads();
-        for (uint32_t k = tid; k < L; k += kComposeThreads) {
-            const uint32_t v = s_in[k];
+        if (L * 2u <= (uint32_t)kComposeThreads) {
+            // short list (the usual case): S = 2, 4 or 8 adjacent lanes share one element, each counts the smaller ids
+            // in its part of the list, a shuffle adds the parts (rank sort: ids are unique inside a tile)
+            const uint32_t S = L * 8u <= (uint32_t)kComposeThreads ? 8u : (L * 4u <= (uint32_t)kComposeThreads ? 4u : 2u);
+            const uint32_t e = (uint32_t)tid / S, h = (uint32_t)tid % S;
+            const uint32_t part = (L + S - 1u) / S, m0 = h * part, m1 = min(L, m0 + part);
+            const uint32_t v = e < L ? s_in[e] : 0u;
             uint32_t r = 0;
-            for (uint32_t m = 0; m < L; ++m) r += s_in[m] < v ? 1u : 0u;
-            s_ids[r] = v;
-            glist[r] = v;                                        // write the sorted segment back (osog_debug_bins)
+            for (uint32_t m = m0; m < m1; ++m) r += s_in[m] < v ? 1u : 0u;
+            r += __shfl_xor_sync(0xffffffffu, r, 1);
+            if (S > 2u) r += __shfl_xor_sync(0xffffffffu, r, 2);
+            if (S > 4u) r += __shfl_xor_sync(0xffffffffu, r, 4);
+            if (e < L && h == 0u) {
+                s_ids[r] = v;
+                glist[r] = v;                                    // write the sorted segment back (osog_debug_bins)
+            }
+        } else {
+            for (uint32_t k = tid; k < L; k += kComposeThreads) {
+                const uint32_t v = s_in[k];
+                uint32_t r = 0;
+                for (uint32_t m = 0; m < L; ++m) r += s_in[m] < v ? 1u : 0u;
+                s_ids[r] = v;
+                glist[r] = v;
+            }
         }
         __syncthreads();
     } else {
