@@ -287,8 +287,11 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
 // H3: exclusive scan of count[0..n) -> offset[0..n], total -> status->pairs; count is reset to 0 (it becomes
 // the fill cursor).  One CTA: each thread scans a contiguous run, warp shuffles combine the runs.
 __global__ void __launch_bounds__(1024) k_scan(uint32_t* __restrict__ count, uint32_t* __restrict__ offset,
-                                               long long n, long long max_pairs, DeviceStatus* status)
+                                               long long n, long long max_pairs, DeviceStatus* status,
+                                               DeviceStatus* status_next)
 {
+    if (threadIdx.x == 0) { status_next->bits = 0u; status_next->pad = 0u; status_next->pairs = 0ull; }   // for the next call
+
     __shared__ unsigned long long warp_sum[32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const long long per = (n + blockDim.x - 1) / blockDim.x;
@@ -399,8 +402,17 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     c->last_B = B;
     c->last_tiles = tiles;
     cudaError_t e;
-    if ((e = cudaMemsetAsync(c->count, 0, sizeof(uint32_t) * (size_t)tiles, c->stream)) != cudaSuccess) return e;
-    if ((e = cudaMemsetAsync(c->status, 0, sizeof(DeviceStatus), c->stream)) != cudaSuccess) return e;
+    // Invariant kept by the kernels themselves (no memset nodes in the steady state): count[] is all zero on entry
+    // (k_scan turns it into the fill cursor, k_compose_tile zeroes its own tile's entry again) and the status slot of
+    // this call was cleared by the previous call's k_scan.  After a failed or atomic-variant call: clear explicitly.
+    if (c->scratch_dirty) {
+        if ((e = cudaMemsetAsync(c->count, 0, sizeof(uint32_t) * (size_t)c->max_tiles, c->stream)) != cudaSuccess) return e;
+        if ((e = cudaMemsetAsync(c->status, 0, 2 * sizeof(DeviceStatus), c->stream)) != cudaSuccess) return e;
+    }
+    c->scratch_dirty = true;
+    c->status_idx ^= 1;
+    DeviceStatus* status = c->status + c->status_idx;
+    DeviceStatus* status_next = c->status + (c->status_idx ^ 1);
 
     PrepArgs a;
     a.cx = p->cx; a.cy = p->cy; a.qw = p->qw; a.qx = p->qx; a.qy = p->qy; a.qz = p->qz;
@@ -409,7 +421,7 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     a.N = N; a.B = B; a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
     a.pitch = o->pitch_um; a.n_medium = o->n_medium;
     a.rec = c->rec; a.tbox = c->tbox; a.pframe = c->pframe; a.count = c->count;
-    a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.optics = c->optics; a.status = c->status;
+    a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.optics = c->optics; a.status = status;
     a.has_ramp = (o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0) ? 1 : 0;
     if ((e = upload_optics(c, o, &a.oc)) != cudaSuccess) return e;
 
@@ -419,11 +431,11 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     const long long blocks = (items + threads - 1) / threads;
     k_prepare<<<(unsigned)blocks, threads, 0, c->stream>>>(a);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    k_scan<<<1, 1024, 0, c->stream>>>(c->count, c->offset, tiles, c->max_pairs, c->status);
+    k_scan<<<1, 1024, 0, c->stream>>>(c->count, c->offset, tiles, c->max_pairs, status, status_next);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     if (N > 0) {
         k_fill<<<(unsigned)((N * 32 + 255) / 256), 256, 0, c->stream>>>(
-            c->tbox, c->pframe, c->count, c->offset, c->list, N, c->ntx, c->nty, c->status);
+            c->tbox, c->pframe, c->count, c->offset, c->list, N, c->ntx, c->nty, status);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
     return cudaSuccess;

@@ -15,6 +15,7 @@ namespace osog {
 struct ComposeArgs {
     const float* rec;
     const uint32_t* offset;
+    uint32_t* count;
     uint32_t* list;
     const FrameOptics* optics;
     const float2 *ramp_x, *ramp_y;
@@ -270,6 +271,7 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
     const uint32_t beg = a.offset[tile];
     const uint32_t L = overflow ? 0u : a.offset[tile + 1] - beg;
     uint32_t* glist = a.list + beg;
+    if (tid == 0) a.count[tile] = 0u;                            // keep the "count is zero on entry" invariant (binning.cu)
 
     // ---- H4 (second half): canonical order ------------------------------------------------------------------------
     const bool in_smem = L <= (uint32_t)kSortCap;
@@ -463,8 +465,8 @@ cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float
 {
     (void)N;
     ComposeArgs a;
-    a.rec = c->rec; a.offset = c->offset; a.list = c->list; a.optics = c->optics;
-    a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.status = c->status;
+    a.rec = c->rec; a.offset = c->offset; a.count = c->count; a.list = c->list; a.optics = c->optics;
+    a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.status = c->status + c->status_idx;
     a.opd = d_opd; a.field = d_field;
     a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
     a.ramp_y_on = 1;

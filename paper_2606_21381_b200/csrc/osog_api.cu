@@ -173,10 +173,11 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     A(dalloc(&c->ramp_x, (size_t)c->max_frames * c->W));
     A(dalloc(&c->ramp_y, (size_t)c->max_frames * c->H));
     A(dalloc(&c->optics, (size_t)c->max_frames));
-    A(dalloc(&c->status, 1));
+    A(dalloc(&c->status, 2));
     A(dalloc(&c->field, (size_t)c->max_frames * npx));
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&c->h_status), sizeof(DeviceStatus));
-    if (e == cudaSuccess) e = cudaMemset(c->status, 0, sizeof(DeviceStatus));
+    if (e == cudaSuccess) e = cudaMemset(c->status, 0, 2 * sizeof(DeviceStatus));
+    if (e == cudaSuccess) e = cudaMemset(c->count, 0, sizeof(uint32_t) * (size_t)c->max_tiles);
     if (e == cudaSuccess) e = cudaMemset(c->offset, 0, sizeof(uint32_t) * ((size_t)c->max_tiles + 1));
     if (e != cudaSuccess) {
         const bool oom = e == cudaErrorMemoryAllocation;
@@ -211,6 +212,7 @@ static int render_common(osog_ctx* c, const osog_particles* p, int64_t N, const 
     c->last_N = N;
     e = launch_compose(c, N, o->B, has_ramp, d_opd, d_field);
     if (e != cudaSuccess) return cuda_fail(c, e);
+    c->scratch_dirty = false;                        // the compose kernel re-zeroes the tile counts it used
     return OSOG_OK;
 }
 
@@ -280,7 +282,7 @@ int osog_status(osog_ctx* c, uint32_t* status_bits, int64_t* pairs)
 {
     if (!c) return OSOG_EINVAL;
     DeviceGuard g(c->device);
-    cudaError_t e = cudaMemcpyAsync(c->h_status, c->status, sizeof(DeviceStatus), cudaMemcpyDeviceToHost, c->stream);
+    cudaError_t e = cudaMemcpyAsync(c->h_status, c->status + c->status_idx, sizeof(DeviceStatus), cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e);
     if (status_bits) *status_bits = c->h_status->bits;

@@ -68,7 +68,9 @@ struct osog_ctx {
     float2* ramp_x;                 // [max_frames][W]  exp(i 2 pi fx0 x_j)
     float2* ramp_y;                 // [max_frames][H]
     osog::FrameOptics* optics;      // [max_frames]
-    osog::DeviceStatus* status;     // [1]
+    osog::DeviceStatus* status;     // [2]: slot of the current call / slot being reset for the next call
+    int status_idx;                 // slot used by the last render call
+    bool scratch_dirty;             // a call failed midway: count / status must be cleared explicitly
     float2* field;                  // [max_frames][H][W] (intensity path)
     osog::DeviceStatus* h_status;   // pinned host mirror
     cufftHandle plan_one, plan_batch;

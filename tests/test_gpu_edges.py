@@ -133,3 +133,35 @@ def test_argument_errors(og):
         ctx.render_opd(P, two)
     assert og.lib().osog_render_opd(ctx._ctx, C.byref(P.c), P.N, C.byref(opt), None) == og.OSOG_EINVAL
     ctx.close()
+
+
+def test_context_reuse_keeps_scratch_invariants(og, o):
+    """The tile counters and the status slot are kept clean by the kernels themselves (no memset per call): a context
+    reused across different scenes, after the atomic variant and after an overflowing call, must give the same bits
+    as a fresh context."""
+    import torch
+    big = make_config(2, n_override=400)
+    small = make_scene("reuse", big.H, big.W, _mixed(50, big.H, big.W, seed=9))
+    fresh = og.Context(big.H, big.W, 400)
+    ref_small = fresh.render_opd(og.Particles.from_scene(small), og.optics_from_scene(small)).clone()
+    ref_big = fresh.render_opd(og.Particles.from_scene(big), og.optics_from_scene(big)).clone()
+    fresh.close()
+    ctx = og.Context(big.H, big.W, 400, max_pairs=3000)
+    Pb, Ps = og.Particles.from_scene(big), og.Particles.from_scene(small)
+    ob, os_ = og.optics_from_scene(big), og.optics_from_scene(small)
+    ctx.render_opd_atomic(Pb, ob)
+    assert torch.equal(ctx.render_opd(Ps, os_), ref_small)
+    assert ctx.status() == (0, 0, ctx.status()[2])
+    tiny = og.Context(big.H, big.W, 400, max_pairs=10)
+    tiny.render_opd(Pb, ob)
+    assert tiny.status()[0] == og.OSOG_ECAPACITY
+    out = tiny.render_opd(og.Particles.from_scene(make_scene("one", big.H, big.W, dict(cx=[5.0], cy=[5.0], d0=[1.0], d1=[1.0], d2=[1.0], n_p=[1.4]))),
+                          os_)
+    assert tiny.status()[0] == 0 and float(out.max()) > 0.0        # the overflow bit does not stick to the next call
+    tiny.close()
+    assert torch.equal(ctx.render_opd(Pb, ob), ref_big)
+    cnt, off, lst = ctx.debug_bins()
+    oc, oo, ol = o.binning(big, og.osog_tile_size())
+    assert np.array_equal(off, oo) and np.array_equal(lst, ol)
+    assert torch.equal(ctx.render_opd(Ps, os_), ref_small)
+    ctx.close()
