@@ -385,6 +385,10 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
         __syncwarp();
         // ---- all lanes walk the survivors, class by class ----------------------------------------------------------------------
         const float4* slot = my_slots;
+#ifdef OSOG_EXP_NOEVAL                                           // experiment: skeleton only
+        if (a.H < 0)
+#endif
+        {
 #pragma unroll 1
         for (int sv = 0; sv < n1; ++sv, slot += kSlotStride4) eval_prism<0>(slot, nullptr, slot[6].y, g, acc);
 #pragma unroll 1
@@ -401,6 +405,7 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
         }
 #pragma unroll 1
         for (int sv = 0; sv < n0; ++sv, slot += kSlotStride4) eval_ellipsoid(slot, slot[6].y, g, acc);
+        }
         __syncwarp();
     }
 
