@@ -29,8 +29,9 @@ struct ComposeArgs {
 constexpr int kWarps = kComposeThreads / 32;
 constexpr int kSlotStride4 = 9;                    // survivor slot stride in float4 (8 used, odd stride: conflict-free lane-per-slot writes)
 constexpr int kSmemIds = kSortCap * 4;
+constexpr int kSmemMeta = kSortCap * 2;              // per list entry: sub-tile mask (8 bits) | evaluation code << 8
 constexpr int kSmemSlots = kWarps * 32 * kSlotStride4 * 16;
-constexpr int kSmemBytes = kSmemIds + kSmemSlots;
+constexpr int kSmemBytes = kSmemIds + kSmemMeta + kSmemSlots;
 
 // ---- small PTX helpers ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float fast_sqrt(float x)
@@ -125,6 +126,26 @@ __device__ __forceinline__ void rebase_item(float4* __restrict__ slot, const flo
         reinterpret_cast<double2*>(slot)[7] = make_double2(ex, en);
         reinterpret_cast<double2*>(slot)[8] = uv;
     }
+}
+
+// ---- sub-tile cull ---------------------------------------------------------------------------------------------------------
+// Does the particle (header words 0..7: centre, oriented box, packed pixel bounding box) touch the 16 x 8 pixel
+// sub-tile with origin (sx0, sy0)?  Bounding-box overlap, then a separating-axis test against the oriented box of the
+// silhouette (which contains it by construction).
+__device__ __forceinline__ bool cull_subtile(const float4 h0, const float4 h1, int sx0, int sy0)
+{
+    const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
+    const int pj0 = bx & 0xffff, pj1 = bx >> 16, pi0 = by & 0xffff, pi1 = by >> 16;
+    const float axx = fabsf(h0.z), ayy = h0.w, ha = fabsf(h1.x), hb = fabsf(h1.y);
+    const float ddx = (float)sx0 + 7.5f - h0.x, ddy = (float)sy0 + 3.5f - h0.y;
+    const float pa = fabsf(ddx * axx + ddy * ayy), pb = fabsf(ddy * axx - ddx * ayy);
+    const float ra = 7.5f * axx + 3.5f * fabsf(ayy), rb = 7.5f * fabsf(ayy) + 3.5f * axx;
+    return pj0 <= sx0 + 15 && pj1 >= sx0 && pi0 <= sy0 + 7 && pi1 >= sy0 && pa <= ha + ra && pb <= hb + rb;
+}
+// evaluation code in the sign bits of the (positive) half lengths and of a_x (a_x >= 0 by construction)
+__device__ __forceinline__ uint32_t header_code(const float4 h0, const float4 h1)
+{
+    return (__float_as_uint(h1.x) >> 31) | ((__float_as_uint(h1.y) >> 31) << 1) | ((__float_as_uint(h0.z) >> 31) << 2);
 }
 
 // ---- thickness, 4 pixels of one row per lane --------------------------------------------------------------------------
@@ -259,7 +280,8 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
 {
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t* s_ids = reinterpret_cast<uint32_t*>(smem);                          // this tile's list, ascending
-    float4* s_slots = reinterpret_cast<float4*>(smem + kSmemIds);                 // per-warp survivor slots
+    uint16_t* s_meta = reinterpret_cast<uint16_t*>(smem + kSmemIds);              // per entry: sub-tile mask | code << 8
+    float4* s_slots = reinterpret_cast<float4*>(smem + kSmemIds + kSmemMeta);     // per-warp survivor slots
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int tpf = a.ntx * a.nty;
@@ -321,33 +343,43 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
     g.nly = make_float2(-(float)ly, -(float)ly);
     g.xf = (float)j;
     g.yf = (float)i;
-    // sub-tile rectangle (pixel centres) for the cull: centre in pixel-index coordinates, half extents 7.5 x 3.5
-    const float rcx = (float)wx0 + 7.5f, rcy = (float)wy0 + 3.5f;
     float4* my_slots = s_slots + wid * 32 * kSlotStride4;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
 
-    // From here on the warps of the CTA are independent (no barrier): each walks the whole list in batches of 32.
+    // ---- CTA-level cull: one thread per list entry tests the particle against all 8 sub-tiles of the tile (one header
+    // read per entry instead of one per warp) and leaves an 8-bit mask + the evaluation code in shared memory.
     const float4* recs4 = reinterpret_cast<const float4*>(a.rec);
+    if (in_smem) {
+        for (uint32_t k = tid; k < L; k += kComposeThreads) {
+            const float4* rec = recs4 + (size_t)s_ids[k] * (kRecWords / 4);
+            const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);   // cxp, cyp, ax, ay | ha, hb, bbx, bby
+            uint32_t mask = 0;
+#pragma unroll
+            for (int w = 0; w < kWarps; ++w)
+                mask |= cull_subtile(h0, h1, tx * kTile + (w & 1) * 16, ty * kTile + (w >> 1) * 8) ? (1u << w) : 0u;
+            const uint32_t code = header_code(h0, h1);
+            s_meta[k] = (uint16_t)(mask | (code << 8));
+            if (mask != 0u && code != 0u) asm volatile("prefetch.global.L1 [%0];" ::"l"(rec + 8));   // 2nd line: slabs 2..5
+        }
+        __syncthreads();
+    }
+    // From here on the warps of the CTA are independent (no barrier): each walks the whole list in batches of 32.
     for (uint32_t base = 0; base < L; base += 32) {
-        // ---- cull: lane <-> particle base + lane; records are read through L1 / L2 (10 MB, L2 resident) -----------------
+        // ---- lane <-> list entry base + lane: survivors of this warp's sub-tile -------------------------------------------
         const uint32_t k = base + lane;
         bool keep = false;
         uint32_t pid = 0, code = 0;
-        if (k < L) {
-            pid = in_smem ? s_ids[k] : glist[k];
+        if (in_smem) {
+            const uint32_t meta = k < L ? s_meta[k] : 0u;
+            keep = ((meta >> wid) & 1u) != 0u;
+            code = meta >> 8;
+            if (keep) pid = s_ids[k];
+        } else if (k < L) {                                      // very long list (sorted in global memory): per-warp cull
+            pid = glist[k];
             const float4* rec = recs4 + (size_t)pid * (kRecWords / 4);
-            const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);   // cxp, cyp, ax, ay | ha, hb, bbx, bby
-            const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
-            const int pj0 = bx & 0xffff, pj1 = bx >> 16, pi0 = by & 0xffff, pi1 = by >> 16;
-            // evaluation code in the sign bits of the (positive) half lengths and of a_x (a_x >= 0 by construction)
-            code = (__float_as_uint(h1.x) >> 31) | ((__float_as_uint(h1.y) >> 31) << 1) | ((__float_as_uint(h0.z) >> 31) << 2);
-            keep = pj0 <= wx0 + 15 && pj1 >= wx0 && pi0 <= wy0 + 7 && pi1 >= wy0;
-            // separating-axis test against the particle's oriented box (the silhouette lies inside it)
-            const float axx = fabsf(h0.z), ayy = h0.w, ha = fabsf(h1.x), hb = fabsf(h1.y);
-            const float ddx = rcx - h0.x, ddy = rcy - h0.y;
-            const float pa = fabsf(ddx * axx + ddy * ayy), pb = fabsf(ddy * axx - ddx * ayy);
-            const float ra = 7.5f * axx + 3.5f * fabsf(ayy), rb = 7.5f * fabsf(ayy) + 3.5f * axx;
-            keep = keep && pa <= ha + ra && pb <= hb + rb;
+            const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);
+            code = header_code(h0, h1);
+            keep = cull_subtile(h0, h1, wx0, wy0);
         }
         // Survivors are grouped by evaluation class (fixed, data-dependent order: NS0 prisms, NS1, NS2, all-fp64,
         // ellipsoids; ascending particle index inside a class), so each class runs in its own branch-free loop.
