@@ -299,7 +299,7 @@ def run_ours(args):
                 "d2h_bytes_per_step": int(d2h)},
         "gpu_launches": 4 * args.steps,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": 8942336, "traffic_note": "dram read+write of one k_compose_tile launch, ncu --set full "
+                     "traffic": 8953856, "traffic_note": "dram read+write of one k_compose_tile launch, ncu --set full "
                      "(profiles/r1_final_compose_ncu.md); the 33.5 MB field it writes stays in the 126 MB L2",
                      "peak_source": peak_src, "algorithmic_bytes": int(k_bytes), "kernel": "k_compose_tile",
                      "kernel_ms": ms_compose, "frac_of_nominal_8TBs": achieved / 8000.0,
