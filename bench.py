@@ -39,6 +39,35 @@ def _peaks():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+# ALU roofline: the composition is bound by instruction issue, not by HBM.
+ALU_INSTR_PER_ELLIPSOID_PAIR = 13      # ~12 fp32 instructions + 1 MUFU per true covered pair
+ALU_INSTR_PER_PRISM_PAIR = 40          # 12 plane values + min / max + accumulate per true covered pair
+ALU_INSTR_PER_PIXEL = 30               # sincospi + complex multiply + store per output pixel
+N_SM, SMSP_PER_SM, LANES = 148, 4, 32  # B200: one warp instruction per clock and SM sub-partition
+
+
+def _sm_clock_ghz():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["sm_max_mhz"]) * 1e-3, "MEASURED_PEAKS.json sm_max_mhz"
+    except Exception:
+        return 1.965, "fallback 1965 MHz"
+
+
+def _covered_pairs(name):
+    """True covered (particle, pixel) pairs of a workload, from tests/golden/covered_pairs.txt (written by the oracle
+    through tests/golden/make_covered_pairs.py; a stored workload statistic, no oracle code runs here)."""
+    try:
+        with open(os.path.join(ROOT, "tests", "golden", "covered_pairs.txt")) as f:
+            for ln in f:
+                p = ln.split()
+                if len(p) == 3 and p[0] == name:
+                    return int(p[1]), int(p[2])
+    except OSError:
+        pass
+    return None
+
+
 class ClockSampler:
     """Samples nvidia-smi SM clocks and throttle reasons while the timed region runs."""
 
@@ -287,6 +316,30 @@ def run_ours(args):
     step_gbs = alg_bytes / (ms_step * 1e-3) / 1e9
     k_bytes = 4 * pairs + 8 * B * H * W                 # k_compose_tile alone: list read + complex64 write
     achieved = k_bytes / (ms_compose * 1e-3) / 1e9
+    hbm = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+           "traffic": 8953856, "traffic_note": "dram read+write of one k_compose_tile launch, ncu --set full "
+           "(profiles/r1_final_compose_ncu.md); the 33.5 MB field it writes stays in the 126 MB L2",
+           "peak_source": peak_src, "algorithmic_bytes": int(k_bytes), "kernel": "k_compose_tile",
+           "kernel_ms": ms_compose, "frac_of_nominal_8TBs": achieved / 8000.0,
+           "note": "BASELINE.json's '% of B200 HBM roofline'; the kernel is bound by instruction issue, see roofline"}
+    cp = _covered_pairs(CONFIG_NAMES[args.config])
+    if cp is not None:
+        ghz, ghz_src = _sm_clock_ghz()
+        alu_peak = N_SM * SMSP_PER_SM * LANES * ghz * 1e-3                      # T lane-instructions / s
+        alg_instr = (ALU_INSTR_PER_ELLIPSOID_PAIR * cp[0] + ALU_INSTR_PER_PRISM_PAIR * cp[1]
+                     + ALU_INSTR_PER_PIXEL * B * H * W)
+        alu_ach = alg_instr / (ms_compose * 1e-3) / 1e12
+        roof = {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "T lane-instructions/s",
+                "frac": alu_ach / alu_peak, "traffic": hbm["traffic"], "kernel": "k_compose_tile",
+                "kernel_ms": ms_compose, "algorithmic_instructions": int(alg_instr),
+                "units": {"ellipsoid_pairs": cp[0], "prism_pairs": cp[1], "pixels": B * H * W,
+                          "instr_per_unit": [ALU_INSTR_PER_ELLIPSOID_PAIR, ALU_INSTR_PER_PRISM_PAIR,
+                                             ALU_INSTR_PER_PIXEL],
+                          "source": "tests/golden/covered_pairs.txt (oracle count of pairs with positive thickness)"},
+                "peak_source": f"{N_SM} SMs x {SMSP_PER_SM} sub-partitions x {LANES} lanes x {ghz:.3f} GHz "
+                               f"({ghz_src}): one warp instruction per clock and sub-partition (DESIGN.md section 7)"}
+    else:
+        roof = hbm
     line = {
         "metric": METRIC, "value": whole_job_value(N, args.steps, world, t_steps), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
@@ -298,12 +351,7 @@ def run_ours(args):
         "e2e": {"value": world * N * args.steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h)},
         "gpu_launches": 4 * args.steps,
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": 8953856, "traffic_note": "dram read+write of one k_compose_tile launch, ncu --set full "
-                     "(profiles/r1_final_compose_ncu.md); the 33.5 MB field it writes stays in the 126 MB L2",
-                     "peak_source": peak_src, "algorithmic_bytes": int(k_bytes), "kernel": "k_compose_tile",
-                     "kernel_ms": ms_compose, "frac_of_nominal_8TBs": achieved / 8000.0,
-                     "binding_unit": "instruction issue (fp32 FMA / ALU min-max / fp64), not HBM: see DESIGN.md section 7"},
+        "roofline": roof, "roofline_hbm": hbm,
         "roofline_step": {"achieved": step_gbs, "frac": step_gbs / peak, "algorithmic_bytes": int(alg_bytes),
                           "what": "whole hot path: k_prepare, k_scan, k_fill, k_compose_tile"},
         "library_stage_ms": ms_optics, "opd_only_ms": ms_opd, "atomic_alternative_opd_ms": ms_atomic,

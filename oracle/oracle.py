@@ -39,6 +39,9 @@ def _lib():
         lib.osog_oracle_render_opd.argtypes = [ctypes.c_int64] + [fp] * 10 + [u8p] + [
             ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, dp]
         lib.osog_oracle_render_opd.restype = None
+        lib.osog_oracle_count_covered.argtypes = [ctypes.c_int64] + [fp] * 10 + [u8p] + [
+            ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int64)]
+        lib.osog_oracle_count_covered.restype = None
         lib.osog_oracle_thickness.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double]
         lib.osog_oracle_thickness.restype = ctypes.c_double
         lib.osog_oracle_circumradius.argtypes = [ctypes.c_uint8] + [ctypes.c_float] * 3
@@ -109,6 +112,26 @@ def render_opd_frame(cols, lo, hi, H, W, pitch, n_medium, mode="bcircle") -> np.
         _ptr(kind, ctypes.c_uint8), H, W, float(pitch), float(n_medium),
         {"full": 0, "bcircle": 1}[mode], _ptr(out, ctypes.c_double))
     return out
+
+
+def count_covered(scene, mode="bcircle"):
+    """Workload statistic: (ellipsoid pairs, prism pairs) = number of (particle, pixel) pairs with positive
+    thickness, summed over the frames of a workloads.Scene (the "true covered pairs" of SURVEY.md 8(d))."""
+    fs = scene.frame_start
+    f = ctypes.c_float
+    tot = np.zeros(2, dtype=np.int64)
+    for b in range(scene.B):
+        lo, hi = int(fs[b]), int(fs[b + 1])
+        a = {k: np.ascontiguousarray(scene.cols[k][lo:hi], dtype=np.float32) for k in _COLS}
+        kind = np.ascontiguousarray(scene.cols["kind"][lo:hi], dtype=np.uint8)
+        out = np.zeros(2, dtype=np.int64)
+        _lib().osog_oracle_count_covered(
+            hi - lo, _ptr(a["cx"], f), _ptr(a["cy"], f), _ptr(a["qw"], f), _ptr(a["qx"], f), _ptr(a["qy"], f),
+            _ptr(a["qz"], f), _ptr(a["d0"], f), _ptr(a["d1"], f), _ptr(a["d2"], f), _ptr(a["n_p"], f),
+            _ptr(kind, ctypes.c_uint8), scene.H, scene.W, float(scene.pitch_um),
+            {"full": 0, "bcircle": 1}[mode], _ptr(out, ctypes.c_int64))
+        tot += out
+    return int(tot[0]), int(tot[1])
 
 
 def render_opd(scene, mode="bcircle") -> np.ndarray:

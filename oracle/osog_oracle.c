@@ -190,3 +190,48 @@ void osog_oracle_render_opd(int64_t N,
         }
     }
 }
+
+/* Workload statistic (not part of the rendered result): number of (particle, pixel) pairs of one frame
+ * whose thickness is positive, counted separately for ellipsoids (pairs[0]) and prisms (pairs[1]).
+ * These are the "true covered pairs" of SURVEY.md section 8(d): the units of arithmetic the method
+ * cannot avoid.  Same loops and the same thickness functions as osog_oracle_render_opd. */
+void osog_oracle_count_covered(int64_t N,
+                               const float *cx, const float *cy,
+                               const float *qw, const float *qx, const float *qy, const float *qz,
+                               const float *d0, const float *d1, const float *d2,
+                               const float *n_p, const uint8_t *kind,
+                               int H, int W, double pitch, int mode, int64_t pairs[2])
+{
+    int64_t ne = 0, np = 0;
+#pragma omp parallel for schedule(dynamic, 4) reduction(+ : ne, np)
+    for (int i = 0; i < H; ++i) {
+        const double y = (i + 0.5) * pitch;
+        for (int64_t n = 0; n < N; ++n) {
+            if (!osog_oracle_particle_valid(cx[n], cy[n], qw[n], qx[n], qy[n], qz[n],
+                                            d0[n], d1[n], d2[n], n_p[n], kind[n])) continue;
+            const double dy = y - (double)cy[n];
+            const double q[4] = { qw[n], qx[n], qy[n], qz[n] };
+            double R[9];
+            osog_oracle_rot_from_quat(q, R);
+            double Aw[OSOG_ORACLE_MAX_PLANES][3], b[OSOG_ORACLE_MAX_PLANES];
+            int M = 0;
+            if (kind[n] == 1) M = prism_world_planes(R, d0[n], d1[n], d2[n], Aw, b);
+            double r2 = INFINITY;
+            if (mode == 1) {
+                const double r = osog_oracle_circumradius(kind[n], d0[n], d1[n], d2[n]) * (1.0 + 1e-9);
+                r2 = r * r;
+                if (dy * dy > r2) continue;
+            }
+            for (int j = 0; j < W; ++j) {
+                const double dx = (j + 0.5) * pitch - (double)cx[n];
+                if (dx * dx + dy * dy > r2) continue;
+                const double t = kind[n] == 0
+                    ? osog_oracle_thickness_ellipsoid(R, d0[n], d1[n], d2[n], dx, dy)
+                    : osog_oracle_thickness_polyhedron(M, Aw, b, dx, dy);
+                if (t > 0.0) { if (kind[n] == 0) ++ne; else ++np; }
+            }
+        }
+    }
+    pairs[0] = ne;
+    pairs[1] = np;
+}

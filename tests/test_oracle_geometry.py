@@ -251,3 +251,39 @@ def test_P13_brute_force_ray_marching_inside_test_only(kind):
                 covered += t_march > 0
                 assert got[i, j] == pytest.approx(t_march, abs=2 * dz + 1e-6 * rmax)
         assert covered >= 12         # the test really exercises covered pixels and the silhouette
+
+
+# ---- workload statistic: covered (particle, pixel) pairs (bench.py's ALU roofline units) -------------------------------
+def test_count_covered_sphere_is_the_gauss_circle_count_and_golden_file_matches():
+    from workloads import make_scene, make_config, CONFIG_NAMES
+    import os
+    # two spheres + one prism with identity rotation: pixel centres strictly inside the disc r < R, or inside the square
+    # |dx|, |dy| < s/2 (pin P5: the identity prism's shadow is the square), counted directly with numpy
+    H = W = 96
+    p = 0.1
+    cols = dict(cx=[3.07, 6.51, 4.83], cy=[4.12, 2.93, 7.0], d0=[1.7, 0.93, 1.24], d1=[1.7, 0.93, 2.0], d2=[1.7, 0.93, 0.6],
+                n_p=[1.4, 1.4, 1.4], kind=np.array([0, 0, 1], np.uint8))
+    sc = make_scene("count", H, W, cols)
+    x = (np.arange(W) + 0.5) * p
+    X, Y = np.meshgrid(x, x)
+    f = lambda v: float(np.float32(v))
+    want_e = sum(int(np.count_nonzero((X - f(cx)) ** 2 + (Y - f(cy)) ** 2 < f(r) ** 2))
+                 for cx, cy, r in zip(cols["cx"][:2], cols["cy"][:2], cols["d0"][:2]))
+    want_p = int(np.count_nonzero((np.abs(X - f(4.83)) < f(1.24) / 2) & (np.abs(Y - f(7.0)) < f(1.24) / 2)))
+    for mode in ("full", "bcircle"):
+        assert o.count_covered(sc, mode) == (want_e, want_p)
+    # the stored counts are what the oracle gives today for the small workloads (config 1: also = non-zero thickness
+    # pixels summed over single-particle renders)
+    stored = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "covered_pairs.txt")) as fh:
+        for ln in fh:
+            q = ln.split()
+            if len(q) == 3 and not ln.startswith("#"):
+                stored[q[0]] = (int(q[1]), int(q[2]))
+    assert set(stored) == set(CONFIG_NAMES.values())
+    for cfg in (1, 2):
+        assert o.count_covered(make_config(cfg)) == stored[CONFIG_NAMES[cfg]]
+    sc1 = make_config(1)
+    from workloads import subset
+    tot = sum(int(np.count_nonzero(o.render_opd(subset(sc1, [n]))[0])) for n in range(sc1.N))
+    assert tot == stored[CONFIG_NAMES[1]][0]
