@@ -8,6 +8,9 @@ Pieces, each following the passage it cites (line numbers are /root/reference/PA
   field           U = exp(i 2 pi (OPD/lambda + fx0 x + fy0 y))                        Eq. 2 (A == 1), :113-115
   pupil_mask      circ(|k| / k_NA) on the FFT grid, integer comparison                Eq. 3 (delta z = 0)
   intensity       I = | IFFT2( FFT2(U) * P ) |^2                                      :90, :99
+  defocus_factor  exp(i dz sqrt(k0^2 - kx^2 - ky^2)) on the FFT grid                  Eq. 3 (delta z != 0), A20
+  pupil_function  P = circ(.) * defocus factor                                        Eq. 3
+  dic_image       | U(r+ds) e^{i theta} - U(r-ds) e^{-i theta} |^2 * |h_obj|^2         Eq. 5 (:101-104), A21, A22
   philox4x32_10   counter-based RNG, written from its published description
   read_noise      z ~ N(0,1) per (seed, frame, pixel) by Box-Muller                   :126 (Gaussian term)
   binning         bounding boxes -> tiles -> counts / offsets / ascending lists       DESIGN.md section 3 (B1-B4)
@@ -171,6 +174,58 @@ def pupil_mask(H, W, NA, pitch, lam) -> np.ndarray:
     return lhs <= pupil_threshold(H, W, NA, pitch, lam)
 
 
+def propagating_threshold(H, W, n_medium, pitch, lam) -> int:
+    """floor((n_medium p / lambda)^2 H^2 W^2): bin (my, mx) is a propagating wave (real k_z) iff
+    mx^2 H^2 + my^2 W^2 <= this - the same integer form as the pupil edge (A10), with NA replaced by n_medium."""
+    r = n_medium * pitch / lam
+    return int(math.floor(r * r * (float(H) * H) * (float(W) * W)))
+
+
+def defocus_factor(H, W, pitch, lam, n_medium, dz) -> np.ndarray:
+    """exp(i dz sqrt(k0^2 - kx^2 - ky^2)) of Eq. 3 on the FFT grid (reading A20): angular spatial
+    frequency k = 2 pi f with f = m / (W p) (m the signed FFT index, as for the pupil, A10) and k0 = 2 pi n_medium /
+    lambda, the wavenumber in the medium the particles sit in; so the phase in turns is dz sqrt((n_m/lambda)^2 - fx^2 -
+    fy^2).  Evanescent bins (negative radicand; always outside a physical pupil, NA <= n_m) carry no propagating
+    wave: they are set to 0 whenever dz != 0.  dz == 0 gives exactly 1 on every bin (Eq. 3 reduces to circ)."""
+    if dz == 0.0:
+        return np.ones((H, W), dtype=np.complex128)
+    mx = np.fft.fftfreq(W, d=1.0 / W).round().astype(np.int64)
+    my = np.fft.fftfreq(H, d=1.0 / H).round().astype(np.int64)
+    lhs = (mx * mx)[None, :] * (H * H) + (my * my)[:, None] * (W * W)
+    prop = lhs <= propagating_threshold(H, W, n_medium, pitch, lam)
+    fx = mx.astype(np.float64) / (W * pitch)
+    fy = my.astype(np.float64) / (H * pitch)
+    rad = (n_medium / lam) ** 2 - (fx * fx)[None, :] - (fy * fy)[:, None]
+    turns = dz * np.sqrt(np.maximum(rad, 0.0))
+    return np.where(prop, np.exp(2j * np.pi * turns), 0.0)
+
+
+def pupil_function(H, W, NA, pitch, lam, n_medium, dz=0.0, pupil_enabled=True) -> np.ndarray:
+    """P(kx, ky) of Eq. 3: circ(|k| / k_NA) times the defocus factor; complex128 [H, W]."""
+    P = defocus_factor(H, W, pitch, lam, n_medium, dz)
+    if pupil_enabled:
+        P = P * pupil_mask(H, W, NA, pitch, lam)
+    return P
+
+
+def dic_image(U, P, shear_px, theta) -> np.ndarray:
+    """Eq. 5:  I_DIC(r) = | U(r + ds) e^{i theta} - U(r - ds) e^{-i theta} |^2  *  |h_obj(r)|^2.
+    U: exit wave [H, W]; P: pupil function on the FFT grid (None = all-pass), h_obj = F^-1{P} (the same
+    normalised inverse FFT as coherent_image, so that U * h_obj = ifft2(fft2(U) P)); shear_px = (sx, sy): the half
+    shear ds in whole pixels along x (columns) and y (rows), the two copies are 2 ds apart (A21); theta: bias phase.
+    Both the shear and the convolution are circular, like the FFT stage of the coherent path (A11, A22).
+    |h_obj|^2 is used as Eq. 5 writes it, without renormalising it to unit sum (A22)."""
+    sx, sy = int(shear_px[0]), int(shear_px[1])
+    Up = np.roll(U, shift=(-sy, -sx), axis=(0, 1))          # Up[i, j] = U[i + sy, j + sx] = U(r + ds)
+    Um = np.roll(U, shift=(sy, sx), axis=(0, 1))            # U(r - ds)
+    d = Up * np.exp(1j * theta) - Um * np.exp(-1j * theta)
+    D = d.real * d.real + d.imag * d.imag
+    H, W = U.shape
+    h = np.fft.ifft2(np.ones((H, W), dtype=np.complex128) if P is None else P)
+    psf = h.real * h.real + h.imag * h.imag
+    return np.fft.ifft2(np.fft.fft2(D) * np.fft.fft2(psf)).real
+
+
 def coherent_image(U, mask=None) -> np.ndarray:
     """U * h_obj, h_obj = F^-1{P}: forward FFT, multiply by the pupil, inverse FFT
     (normalised so that an all-pass pupil returns U)."""
@@ -247,11 +302,32 @@ def render_intensity(scene, U=None, pupil_enabled=True, mode="bcircle") -> np.nd
     """float64 [B, H, W]: |coherent image|^2 + sigma * z."""
     if U is None:
         U = render_field(scene, mode=mode)
+    dz = float(getattr(scene, "defocus_um", 0.0))
     out = []
     for b in range(scene.B):
-        mask = pupil_mask(scene.H, scene.W, float(scene.NA[b]), scene.pitch_um, float(scene.lambda_um[b])) \
-            if pupil_enabled else None
+        if dz != 0.0:
+            mask = pupil_function(scene.H, scene.W, float(scene.NA[b]), scene.pitch_um, float(scene.lambda_um[b]),
+                                  scene.n_medium, dz, pupil_enabled)
+        else:
+            mask = pupil_mask(scene.H, scene.W, float(scene.NA[b]), scene.pitch_um, float(scene.lambda_um[b])) \
+                if pupil_enabled else None
         I = intensity(U[b], mask)
+        if scene.read_noise_sigma != 0.0:
+            I = I + scene.read_noise_sigma * read_noise(scene.seed, b, scene.H, scene.W)
+        out.append(I)
+    return np.stack(out)
+
+
+def render_dic(scene, shear_px, theta, U=None, pupil_enabled=True, mode="bcircle") -> np.ndarray:
+    """float64 [B, H, W]: Eq. 5 on the scene's exit wave, through the scene's pupil (with its defocus), + sigma * z."""
+    if U is None:
+        U = render_field(scene, mode=mode)
+    dz = float(getattr(scene, "defocus_um", 0.0))
+    out = []
+    for b in range(scene.B):
+        P = pupil_function(scene.H, scene.W, float(scene.NA[b]), scene.pitch_um, float(scene.lambda_um[b]),
+                           scene.n_medium, dz, pupil_enabled)
+        I = dic_image(U[b], P, shear_px, theta)
         if scene.read_noise_sigma != 0.0:
             I = I + scene.read_noise_sigma * read_noise(scene.seed, b, scene.H, scene.W)
         out.append(I)

@@ -44,6 +44,7 @@ class Scene:
     tilt_x_rad: float = 0.0
     tilt_y_rad: float = 0.0
     read_noise_sigma: float = 0.0
+    defocus_um: float = 0.0      # delta z of Eq. 3; 0 = in focus
     cols: dict = field(default_factory=dict)   # float32 [N] each + kind uint8 [N]
     frame_start: np.ndarray = None             # int32 [B+1]
 
