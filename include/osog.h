@@ -11,8 +11,11 @@
  *                  half-space intersection {x | A x <= b} of Eq. 1 for the capped tetragonal prism.
  *     U[b,i,j]   = exp(i 2 pi (OPD / lambda_b + fx0 x + fy0 y)),  fx0 = sin(tilt_x) / lambda_b   (Eq. 2 with A == 1,
  *                  oblique illumination as a phase ramp)
- *     I[b]       = | IFFT2( FFT2(U[b]) * circ(|k| / (NA_b / lambda_b)) ) |^2  (+ sigma * z[b,i,j])
- *                  (Eq. 3 with delta z = 0; I_BF; Gaussian read noise)
+ *     I[b]       = | IFFT2( FFT2(U[b]) * P_b ) |^2  (+ sigma * z[b,i,j]),
+ *                  P_b = circ(|k| / (NA_b / lambda_b)) * exp(i dz sqrt(k0^2 - kx^2 - ky^2)),  k0 = 2 pi n_medium / lambda_b
+ *                  (Eq. 3, readings A9, A10, A20; I_BF; Gaussian read noise)
+ *     I_DIC[b]   = | U(r + ds) e^{i theta} - U(r - ds) e^{-i theta} |^2  (*)  | IFFT2(P_b) |^2   (+ sigma * z)
+ *                  (Eq. 5; ds in whole pixels, shear and convolution circular, readings A21, A22)
  *
  * Conventions
  *   - One context per (device, stream).  Every render call ENQUEUES work on the context's stream and returns
@@ -36,7 +39,7 @@
 extern "C" {
 #endif
 
-#define OSOG_API_VERSION 1
+#define OSOG_API_VERSION 2   /* 2: osog_optics.defocus_um, osog_dic, osog_render_dic, osog_field_to_dic */
 
 enum {
     OSOG_OK = 0,
@@ -86,7 +89,18 @@ typedef struct {
     double   read_noise_sigma;        /* intensity only: I += sigma * z, z ~ N(0,1) Philox4x32-10 keyed (seed, frame, pixel); 0 = none */
     uint64_t seed;
     int32_t  pupil_enabled;           /* 0 = all-pass pupil (Parseval check), else circ(NA / lambda)          */
+    double   defocus_um;              /* delta z of Eq. 3 (intensity / DIC only): the pupil is multiplied by
+                                         exp(i 2 pi dz sqrt((n_medium/lambda)^2 - fx^2 - fy^2)); evanescent bins are
+                                         zeroed when dz != 0; 0 = in focus (exactly the circ-only pupil)            */
 } osog_optics;
+
+/* Differential interference contrast, Eq. 5.  struct_size = sizeof(osog_dic). */
+typedef struct {
+    uint32_t struct_size;
+    int32_t  shear_x_px, shear_y_px;  /* half shear ds in whole pixels along x (columns) / y (rows); the two copies
+                                         of the field are 2 ds apart; |shear| < W resp. H; wraps around the frame   */
+    double   bias_rad;                /* bias phase theta                                                         */
+} osog_dic;
 
 /* Create a context: allocates all scratch (records, bounding boxes, tile counts / offsets / lists, ramp
  * tables, one complex frame batch and the cuFFT plans).  *out is set to NULL on failure. */
@@ -103,12 +117,23 @@ int osog_render_field(osog_ctx* ctx, const osog_particles* p, int64_t N, const o
 /* Coherent intensity through the circular pupil: d_intensity is DEVICE float [B, H, W].  Runs the hot path
  * into the context's own complex frame, then the library stage: cuFFT forward, pupil mask (integer
  * comparison m_x^2 H^2 + m_y^2 W^2 <= floor((NA p / lambda)^2 H^2 W^2)) and 1/(HW), cuFFT inverse, |.|^2,
- * optional read noise. */
+ * optional read noise.  With o->defocus_um != 0 the pupil also carries the defocus phase of Eq. 3. */
 int osog_render_intensity(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_intensity);
 
 /* Library stage alone on a caller-supplied field (DEVICE complex64 [B, H, W], left untouched): used to time
  * the cuFFT stage separately from the hot path. */
 int osog_field_to_intensity(osog_ctx* ctx, const osog_optics* o, const float* d_field, float* d_intensity);
+
+/* DIC image (Eq. 5): d_dic is DEVICE float [B, H, W].  Runs the hot path into the context's own complex frame, then
+ * the library stage: D = |U(r+ds) e^{i theta} - U(r-ds) e^{-i theta}|^2, cuFFT forward of D; the pupil function P
+ * (circ and defocus of `o`) -> cuFFT inverse -> |h_obj|^2 -> cuFFT forward (the optical transfer function); product,
+ * cuFFT inverse, real part, optional read noise (same generator as the intensity).  The first DIC call of a context
+ * allocates one more complex frame batch (cudaMalloc, synchronous); later calls allocate nothing. */
+int osog_render_dic(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const osog_dic* dic,
+                    float* d_dic);
+
+/* Library stage of osog_render_dic alone on a caller-supplied field (DEVICE complex64 [B, H, W], left untouched). */
+int osog_field_to_dic(osog_ctx* ctx, const osog_optics* o, const osog_dic* dic, const float* d_field, float* d_dic);
 
 /* Measured alternative to the ordered tile composition (paper-style scatter-add): one warp
  * per particle, global atomicAdd into d_opd.  NOT deterministic in the last bits; kept for comparison only. */

@@ -34,7 +34,12 @@ class osog_optics(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("B", C.c_int32), ("pitch_um", C.c_double), ("n_medium", C.c_double),
                 ("lambda_um", C.POINTER(C.c_double)), ("NA", C.POINTER(C.c_double)),
                 ("tilt_x_rad", C.c_double), ("tilt_y_rad", C.c_double), ("read_noise_sigma", C.c_double),
-                ("seed", C.c_uint64), ("pupil_enabled", C.c_int32)]
+                ("seed", C.c_uint64), ("pupil_enabled", C.c_int32), ("defocus_um", C.c_double)]
+
+
+class osog_dic(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("shear_x_px", C.c_int32), ("shear_y_px", C.c_int32),
+                ("bias_rad", C.c_double)]
 
 
 class OsogError(RuntimeError):
@@ -64,6 +69,9 @@ def lib():
     for name in ("osog_render_opd", "osog_render_field", "osog_render_intensity", "osog_render_opd_atomic"):
         getattr(L, name).argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p]
     L.osog_field_to_intensity.argtypes = [ctx, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
+    L.osog_render_dic.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics),
+                                  C.POINTER(osog_dic), C.c_void_p]
+    L.osog_field_to_dic.argtypes = [ctx, C.POINTER(osog_optics), C.POINTER(osog_dic), C.c_void_p, C.c_void_p]
     L.osog_debug_recompose_field.argtypes = [ctx, C.c_void_p]
     L.osog_destroy.argtypes = [ctx]
     L.osog_status.argtypes = [ctx, C.POINTER(C.c_uint32), C.POINTER(C.c_int64)]
@@ -80,7 +88,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_opd_atomic", "osog_debug_recompose_field", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_debug_recompose_field", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -122,7 +130,7 @@ class Particles:
 
 
 def make_optics(B, pitch_um, n_medium, lambda_um, NA=None, tilt_x_rad=0.0, tilt_y_rad=0.0,
-                read_noise_sigma=0.0, seed=0, pupil_enabled=True):
+                read_noise_sigma=0.0, seed=0, pupil_enabled=True, defocus_um=0.0):
     """osog_optics plus the host arrays it points to (kept alive as attributes)."""
     o = osog_optics()
     o.struct_size = C.sizeof(osog_optics)
@@ -141,12 +149,21 @@ def make_optics(B, pitch_um, n_medium, lambda_um, NA=None, tilt_x_rad=0.0, tilt_
     o.read_noise_sigma = float(read_noise_sigma)
     o.seed = int(seed) & 0xFFFFFFFFFFFFFFFF
     o.pupil_enabled = 1 if pupil_enabled else 0
+    o.defocus_um = float(defocus_um)
     return o
+
+
+def make_dic(shear_x_px, shear_y_px, bias_rad):
+    d = osog_dic()
+    d.struct_size = C.sizeof(osog_dic)
+    d.shear_x_px, d.shear_y_px, d.bias_rad = int(shear_x_px), int(shear_y_px), float(bias_rad)
+    return d
 
 
 def optics_from_scene(scene, pupil_enabled=True):
     return make_optics(scene.B, scene.pitch_um, scene.n_medium, scene.lambda_um, scene.NA, scene.tilt_x_rad,
-                       scene.tilt_y_rad, scene.read_noise_sigma, scene.seed, pupil_enabled)
+                       scene.tilt_y_rad, scene.read_noise_sigma, scene.seed, pupil_enabled,
+                       getattr(scene, "defocus_um", 0.0))
 
 
 class Context:
@@ -213,6 +230,22 @@ class Context:
         r = lib().osog_field_to_intensity(self._ctx, C.byref(o), f.data_ptr(), out.data_ptr())
         if r != OSOG_OK:
             raise OsogError(r, "osog_field_to_intensity")
+        return out
+
+    def render_dic(self, p: Particles, o, dic, out=None):
+        """float32 [B, H, W] DIC image of Eq. 5 (osog_render_dic); `dic` from make_dic."""
+        out = self._out(o.B, out=out)
+        r = lib().osog_render_dic(self._ctx, C.byref(p.c), p.N, C.byref(o), C.byref(dic), out.data_ptr())
+        if r != OSOG_OK:
+            raise OsogError(r, "osog_render_dic")
+        return out
+
+    def field_to_dic(self, o, dic, field, out=None):
+        out = self._out(o.B, out=out)
+        f = self.torch.view_as_real(field) if field.is_complex() else field
+        r = lib().osog_field_to_dic(self._ctx, C.byref(o), C.byref(dic), f.data_ptr(), out.data_ptr())
+        if r != OSOG_OK:
+            raise OsogError(r, "osog_field_to_dic")
         return out
 
     def recompose_field(self, out):

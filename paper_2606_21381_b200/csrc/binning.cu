@@ -373,6 +373,13 @@ static FrameOptics frame_optics(const osog_ctx* c, const osog_optics* o, int b)
         const double t = floor(r * r * ((double)c->H * c->H) * ((double)c->W * c->W));
         f.pupil_thresh = t >= 9.0e18 ? -1 : (long long)t;     // a radius beyond every bin is all-pass
     }
+    f.defocus_um = o->defocus_um;
+    const double q = o->n_medium / lam;
+    f.nm_over_lambda_sq = q * q;
+    const double rp = o->n_medium * o->pitch_um / lam;
+    const double tp = floor(rp * rp * ((double)c->H * c->H) * ((double)c->W * c->W));
+    f.prop_thresh = tp >= 9.0e18 ? -1 : (long long)tp;
+    f.pad_ = 0.0;
     return f;
 }
 

@@ -1,5 +1,6 @@
 // Library stage around cuFFT (timed separately from the hot path, L1-L3):
-// pupil mask circ(|k| / (NA / lambda)) with the 1/(HW) normalisation (Eq. 3 with delta z = 0),
+// pupil function circ(|k| / (NA / lambda)) exp(i dz k_z) with the 1/(HW) normalisation (Eq. 3),
+// the DIC shear-and-interfere step and the element-wise helpers of its incoherent convolution (Eq. 5),
 // and the sensor: I = |.|^2 plus optional Gaussian read noise from Philox4x32-10.
 #include "osog_internal.cuh"
 
@@ -7,22 +8,85 @@ namespace osog {
 
 // Bin (ky, kx) of the unshifted FFT grid has signed index m = k for k <= (n-1)/2, else k - n.
 // It passes iff m_x^2 H^2 + m_y^2 W^2 <= floor((NA p / lambda)^2 H^2 W^2)  (64-bit integers, reading A10).
+// DEFOCUS: the passing bin is also multiplied by exp(i 2 pi dz sqrt((n_m / lambda)^2 - fx^2 - fy^2)), f = m / (W p)
+// (Eq. 3, reading A20): turns in fp64, reduced to [-1/2, 1/2], sincospi in fp32; evanescent bins
+// (m_x^2 H^2 + m_y^2 W^2 > floor((n_m p / lambda)^2 H^2 W^2)) are zeroed.
+// Returns the pupil value of the bin times `scale` (0 = blocked).
+template <bool DEFOCUS>
+__device__ __forceinline__ float2 pupil_value(const FrameOptics& fo, int kx, int ky, int H, int W, double inv_wp,
+                                              double inv_hp, float scale)
+{
+    const long long mx = kx <= (W - 1) / 2 ? kx : kx - W;
+    const long long my = ky <= (H - 1) / 2 ? ky : ky - H;
+    const long long lhs = mx * mx * ((long long)H * H) + my * my * ((long long)W * W);
+    bool pass = fo.pupil_thresh < 0 || lhs <= fo.pupil_thresh;
+    if (!DEFOCUS) return make_float2(pass ? scale : 0.0f, 0.0f);
+    pass = pass && (fo.prop_thresh < 0 || lhs <= fo.prop_thresh);
+    if (!pass) return make_float2(0.0f, 0.0f);
+    const double fx = (double)mx * inv_wp, fy = (double)my * inv_hp;
+    const double rad = fo.nm_over_lambda_sq - fx * fx - fy * fy;
+    double turns = fo.defocus_um * sqrt(fmax(rad, 0.0));
+    turns -= rint(turns);
+    float sn, cs;
+    sincospif(2.0f * (float)turns, &sn, &cs);
+    return make_float2(cs * scale, sn * scale);
+}
+
+// spec *= P * scale (in place), or with FILL: spec = P * scale
+template <bool DEFOCUS, bool FILL>
 __global__ void __launch_bounds__(256) k_pupil(float2* __restrict__ spec, const FrameOptics* __restrict__ optics,
-                                               int H, int W, float scale)
+                                               int H, int W, double inv_wp, double inv_hp, float scale)
 {
     const int kx = blockIdx.x * blockDim.x + threadIdx.x;
     const int ky = blockIdx.y, b = blockIdx.z;
     if (kx >= W) return;
-    const long long thr = optics[b].pupil_thresh;
-    const long long mx = kx <= (W - 1) / 2 ? kx : kx - W;
-    const long long my = ky <= (H - 1) / 2 ? ky : ky - H;
-    const long long lhs = mx * mx * ((long long)H * H) + my * my * ((long long)W * W);
+    const float2 pv = pupil_value<DEFOCUS>(optics[b], kx, ky, H, W, inv_wp, inv_hp, scale);
     const size_t idx = ((size_t)b * H + ky) * W + kx;
-    float2 v = spec[idx];
-    const float s = (thr < 0 || lhs <= thr) ? scale : 0.0f;
-    v.x *= s;
-    v.y *= s;
-    spec[idx] = v;
+    if (FILL) {
+        spec[idx] = pv;
+    } else {
+        const float2 v = spec[idx];
+        spec[idx] = DEFOCUS ? make_float2(v.x * pv.x - v.y * pv.y, v.x * pv.y + v.y * pv.x)
+                            : make_float2(v.x * pv.x, v.y * pv.x);
+    }
+}
+
+// DIC, Eq. 5: out = (|U(r + ds) e^{i theta} - U(r - ds) e^{-i theta}|^2, 0); ds = (sx, sy) whole
+// pixels, indices wrap around the frame (readings A21, A22).  e = (cos theta, sin theta).
+__global__ void __launch_bounds__(256) k_dic_shear(const float2* __restrict__ field, float2* __restrict__ out, int H,
+                                                   int W, int sx, int sy, float2 e)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = blockIdx.y, b = blockIdx.z;
+    if (j >= W) return;
+    int jp = j + sx, jm = j - sx, ip = i + sy, im = i - sy;         // |sx| < W, |sy| < H
+    jp += jp < 0 ? W : (jp >= W ? -W : 0);
+    jm += jm < 0 ? W : (jm >= W ? -W : 0);
+    ip += ip < 0 ? H : (ip >= H ? -H : 0);
+    im += im < 0 ? H : (im >= H ? -H : 0);
+    const float2* f = field + (size_t)b * H * W;
+    const float2 up = f[(size_t)ip * W + jp], um = f[(size_t)im * W + jm];
+    const float dr = (up.x * e.x - up.y * e.y) - (um.x * e.x + um.y * e.y);
+    const float di = (up.x * e.y + up.y * e.x) - (um.y * e.x - um.x * e.y);
+    out[((size_t)b * H + i) * W + j] = make_float2(dr * dr + di * di, 0.0f);
+}
+
+// buf = (|buf|^2 * scale, 0)
+__global__ void __launch_bounds__(256) k_abs2(float2* __restrict__ buf, size_t n, float scale)
+{
+    const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const float2 v = buf[k];
+    buf[k] = make_float2((v.x * v.x + v.y * v.y) * scale, 0.0f);
+}
+
+// a = a * b * scale (complex)
+__global__ void __launch_bounds__(256) k_cmul(float2* __restrict__ a, const float2* __restrict__ b, size_t n, float scale)
+{
+    const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const float2 x = a[k], y = b[k];
+    a[k] = make_float2((x.x * y.x - x.y * y.y) * scale, (x.x * y.y + x.y * y.x) * scale);
 }
 
 __device__ __forceinline__ void philox_round(uint32_t (&c)[4], uint32_t k0, uint32_t k1)
@@ -52,6 +116,8 @@ __device__ __forceinline__ float read_noise_z(uint64_t seed, uint32_t frame, uin
     return sqrtf(l) * cospif(2.0f * u2);
 }
 
+// REAL = false: I = |img|^2; REAL = true: I = Re img (the DIC image is a real convolution)
+template <bool REAL>
 __global__ void __launch_bounds__(256) k_sensor(const float2* __restrict__ img, float* __restrict__ out, int H, int W,
                                                 float sigma, uint64_t seed)
 {
@@ -60,15 +126,53 @@ __global__ void __launch_bounds__(256) k_sensor(const float2* __restrict__ img, 
     const int b = blockIdx.y;
     if (pix >= npx) return;
     const float2 v = img[(size_t)b * npx + pix];
-    float I = v.x * v.x + v.y * v.y;
+    float I = REAL ? v.x : v.x * v.x + v.y * v.y;
     if (sigma != 0.0f) I = fmaf(sigma, read_noise_z(seed, (uint32_t)b, (uint32_t)pix), I);
     out[(size_t)b * npx + pix] = I;
 }
 
-cudaError_t launch_pupil(osog_ctx* c, int B, float2* spec)
+static cudaError_t pupil_launch(osog_ctx* c, int B, float2* spec, double pitch, bool defocus, bool fill, float scale)
 {
     const dim3 grid((c->W + 255) / 256, c->H, B);
-    k_pupil<<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, (float)(1.0 / ((double)c->H * c->W)));
+    const double inv_wp = 1.0 / ((double)c->W * pitch), inv_hp = 1.0 / ((double)c->H * pitch);
+    if (fill) {
+        if (defocus) k_pupil<true, true><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale);
+        else k_pupil<false, true><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale);
+    } else {
+        if (defocus) k_pupil<true, false><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale);
+        else k_pupil<false, false><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pupil(osog_ctx* c, int B, float2* spec, double pitch, bool defocus)
+{
+    return pupil_launch(c, B, spec, pitch, defocus, false, (float)(1.0 / ((double)c->H * c->W)));
+}
+
+cudaError_t launch_pupil_fill(osog_ctx* c, int B, float2* spec, double pitch, bool defocus)
+{
+    return pupil_launch(c, B, spec, pitch, defocus, true, 1.0f);
+}
+
+cudaError_t launch_dic_shear(osog_ctx* c, int B, const float2* field, float2* out, int sx, int sy, double theta)
+{
+    const dim3 grid((c->W + 255) / 256, c->H, B);
+    k_dic_shear<<<grid, 256, 0, c->stream>>>(field, out, c->H, c->W, sx, sy, make_float2((float)cos(theta), (float)sin(theta)));
+    return cudaGetLastError();
+}
+
+cudaError_t launch_abs2(osog_ctx* c, int B, float2* buf, double scale)
+{
+    const size_t n = (size_t)B * c->H * c->W;
+    k_abs2<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(buf, n, (float)scale);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cmul(osog_ctx* c, int B, float2* a, const float2* b, double scale)
+{
+    const size_t n = (size_t)B * c->H * c->W;
+    k_cmul<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(a, b, n, (float)scale);
     return cudaGetLastError();
 }
 
@@ -76,7 +180,15 @@ cudaError_t launch_sensor(osog_ctx* c, int B, const float2* img, float* d_intens
 {
     const size_t npx = (size_t)c->H * c->W;
     const dim3 grid((unsigned)((npx + 255) / 256), B);
-    k_sensor<<<grid, 256, 0, c->stream>>>(img, d_intensity, c->H, c->W, (float)sigma, seed);
+    k_sensor<false><<<grid, 256, 0, c->stream>>>(img, d_intensity, c->H, c->W, (float)sigma, seed);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_out, double sigma, uint64_t seed)
+{
+    const size_t npx = (size_t)c->H * c->W;
+    const dim3 grid((unsigned)((npx + 255) / 256), B);
+    k_sensor<true><<<grid, 256, 0, c->stream>>>(img, d_out, c->H, c->W, (float)sigma, seed);
     return cudaGetLastError();
 }
 

@@ -49,6 +49,7 @@ int check_call(const osog_ctx* c, const osog_particles* p, int64_t N, const osog
 int check_intensity(const osog_optics* o)
 {
     if (!(o->read_noise_sigma >= 0.0) || !(o->read_noise_sigma < 1.0e300)) return OSOG_EINVAL;
+    if (!(fabs(o->defocus_um) < 1.0e300)) return OSOG_EINVAL;
     if (o->pupil_enabled) {
         if (!o->NA) return OSOG_EINVAL;
         for (int b = 0; b < o->B; ++b)
@@ -71,31 +72,70 @@ struct DeviceGuard {
     }
 };
 
-// forward FFT, pupil, inverse FFT of B frames held in `buf` (in place), then the sensor into d_intensity
+// one 2-D C2C transform of each of the B frames in `buf`, in place
+int fft_frames(osog_ctx* c, float2* buf, int B, int sign)
+{
+    const size_t npx = (size_t)c->H * c->W;
+    if (B == c->max_frames && c->has_plan_batch) {
+        cufftResult r = cufftExecC2C(c->plan_batch, reinterpret_cast<cufftComplex*>(buf),
+                                     reinterpret_cast<cufftComplex*>(buf), sign);
+        if (r != CUFFT_SUCCESS) { c->last_cuda_error = 10000 + (int)r; return OSOG_ECUDA; }
+        return OSOG_OK;
+    }
+    for (int b = 0; b < B; ++b) {
+        cufftComplex* f = reinterpret_cast<cufftComplex*>(buf + (size_t)b * npx);
+        cufftResult r = cufftExecC2C(c->plan_one, f, f, sign);
+        if (r != CUFFT_SUCCESS) { c->last_cuda_error = 10000 + (int)r; return OSOG_ECUDA; }
+    }
+    return OSOG_OK;
+}
+
+// forward FFT, pupil function, inverse FFT of B frames held in `buf` (in place), then the sensor into d_intensity
 int optics_stage(osog_ctx* c, const osog_optics* o, float2* buf, float* d_intensity)
 {
     const int B = o->B;
-    const size_t npx = (size_t)c->H * c->W;
-    for (int dir = 0; dir < 2; ++dir) {
-        const int sign = dir == 0 ? CUFFT_FORWARD : CUFFT_INVERSE;
-        if (B == c->max_frames && c->has_plan_batch) {
-            cufftResult r = cufftExecC2C(c->plan_batch, reinterpret_cast<cufftComplex*>(buf),
-                                         reinterpret_cast<cufftComplex*>(buf), sign);
-            if (r != CUFFT_SUCCESS) { c->last_cuda_error = 10000 + (int)r; return OSOG_ECUDA; }
-        } else {
-            for (int b = 0; b < B; ++b) {
-                cufftComplex* f = reinterpret_cast<cufftComplex*>(buf + (size_t)b * npx);
-                cufftResult r = cufftExecC2C(c->plan_one, f, f, sign);
-                if (r != CUFFT_SUCCESS) { c->last_cuda_error = 10000 + (int)r; return OSOG_ECUDA; }
-            }
-        }
-        if (dir == 0) {
-            cudaError_t e = launch_pupil(c, B, buf);
-            if (e != cudaSuccess) return cuda_fail(c, e);
-        }
-    }
-    cudaError_t e = launch_sensor(c, B, buf, d_intensity, o->read_noise_sigma, o->seed);
+    int r = fft_frames(c, buf, B, CUFFT_FORWARD);
+    if (r != OSOG_OK) return r;
+    cudaError_t e = launch_pupil(c, B, buf, o->pitch_um, o->defocus_um != 0.0);
     if (e != cudaSuccess) return cuda_fail(c, e);
+    if ((r = fft_frames(c, buf, B, CUFFT_INVERSE)) != OSOG_OK) return r;
+    e = launch_sensor(c, B, buf, d_intensity, o->read_noise_sigma, o->seed);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return OSOG_OK;
+}
+
+int check_dic(const osog_ctx* c, const osog_dic* d)
+{
+    if (!d || d->struct_size != sizeof(osog_dic)) return OSOG_EINVAL;
+    if (d->shear_x_px <= -c->W || d->shear_x_px >= c->W || d->shear_y_px <= -c->H || d->shear_y_px >= c->H) return OSOG_EINVAL;
+    if (!(fabs(d->bias_rad) < 1.0e300)) return OSOG_EINVAL;
+    return OSOG_OK;
+}
+
+// Eq. 5 on the B frames of U held in c->field (overwritten): see include/osog.h, osog_render_dic
+int dic_stage(osog_ctx* c, const osog_optics* o, const osog_dic* d, float* d_dic)
+{
+    const int B = o->B;
+    const double hw = (double)c->H * c->W;
+    if (!c->work) {                                  // first DIC call of this context: the second complex batch
+        cudaError_t ea = dalloc(&c->work, (size_t)c->max_frames * c->H * c->W);
+        if (ea != cudaSuccess) { cudaGetLastError(); c->work = nullptr; return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea); }
+    }
+    const bool defocus = o->defocus_um != 0.0;
+    cudaError_t e;
+    int r;
+    // D = |U(r+ds) e^{i theta} - U(r-ds) e^{-i theta}|^2 and its spectrum
+    if ((e = launch_dic_shear(c, B, c->field, c->work, d->shear_x_px, d->shear_y_px, d->bias_rad)) != cudaSuccess) return cuda_fail(c, e);
+    if ((r = fft_frames(c, c->work, B, CUFFT_FORWARD)) != OSOG_OK) return r;
+    // optical transfer function: P -> h_obj = F^-1{P} -> |h_obj|^2 -> F{.}   (U is no longer needed: reuse its buffer)
+    if ((e = launch_pupil_fill(c, B, c->field, o->pitch_um, defocus)) != cudaSuccess) return cuda_fail(c, e);
+    if ((r = fft_frames(c, c->field, B, CUFFT_INVERSE)) != OSOG_OK) return r;
+    if ((e = launch_abs2(c, B, c->field, 1.0 / (hw * hw))) != cudaSuccess) return cuda_fail(c, e);      // cuFFT's inverse is unnormalised
+    if ((r = fft_frames(c, c->field, B, CUFFT_FORWARD)) != OSOG_OK) return r;
+    // I = F^-1{ F{D} OTF }
+    if ((e = launch_cmul(c, B, c->work, c->field, 1.0 / hw)) != cudaSuccess) return cuda_fail(c, e);
+    if ((r = fft_frames(c, c->work, B, CUFFT_INVERSE)) != OSOG_OK) return r;
+    if ((e = launch_sensor_real(c, B, c->work, d_dic, o->read_noise_sigma, o->seed)) != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
 }
 
@@ -127,7 +167,7 @@ int osog_destroy(osog_ctx* c)
     if (c->has_plan_batch) cufftDestroy(c->plan_batch);
     cudaFree(c->rec); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
     cudaFree(c->offset); cudaFree(c->list); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
-    cudaFree(c->status); cudaFree(c->field);
+    cudaFree(c->status); cudaFree(c->field); cudaFree(c->work);
     if (c->h_status) cudaFreeHost(c->h_status);
     delete c;
     return OSOG_OK;
@@ -255,6 +295,35 @@ int osog_field_to_intensity(osog_ctx* c, const osog_optics* o, const float* d_fi
     e = cudaMemcpyAsync(c->field, d_field, sizeof(float2) * (size_t)o->B * c->H * c->W, cudaMemcpyDeviceToDevice, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return optics_stage(c, o, c->field, d_intensity);
+}
+
+int osog_render_dic(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const osog_dic* d, float* d_dic)
+{
+    int r = check_call(c, p, N, o, d_dic);
+    if (r != OSOG_OK) return r;
+    if ((r = check_intensity(o)) != OSOG_OK) return r;
+    if ((r = check_dic(c, d)) != OSOG_OK) return r;
+    if ((r = render_common(c, p, N, o, nullptr, c->field)) != OSOG_OK) return r;
+    DeviceGuard g(c->device);
+    return dic_stage(c, o, d, d_dic);
+}
+
+int osog_field_to_dic(osog_ctx* c, const osog_optics* o, const osog_dic* d, const float* d_field, float* d_dic)
+{
+    if (!c || !o || !d_field || !d_dic || o->struct_size != sizeof(osog_optics)) return OSOG_EINVAL;
+    if (o->B < 1 || o->B > c->max_frames || !o->lambda_um || !aligned16(d_field) || !aligned16(d_dic)) return OSOG_EINVAL;
+    if (!(o->pitch_um > 0.0)) return OSOG_EINVAL;
+    for (int b = 0; b < o->B; ++b)
+        if (!(o->lambda_um[b] > 0.0)) return OSOG_EINVAL;
+    int r = check_intensity(o);
+    if (r != OSOG_OK) return r;
+    if ((r = check_dic(c, d)) != OSOG_OK) return r;
+    DeviceGuard g(c->device);
+    cudaError_t e = upload_optics(c, o, nullptr);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = cudaMemcpyAsync(c->field, d_field, sizeof(float2) * (size_t)o->B * c->H * c->W, cudaMemcpyDeviceToDevice, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return dic_stage(c, o, d, d_dic);
 }
 
 int osog_render_opd_atomic(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd)

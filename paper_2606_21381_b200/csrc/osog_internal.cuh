@@ -35,6 +35,10 @@ struct FrameOptics {          // per frame, device
     double fx0_pitch;         // sin(tilt_x) / lambda * p : turns per pixel along x
     double fy0_pitch;
     long long pupil_thresh;   // floor((NA p / lambda)^2 H^2 W^2), or -1 = all-pass
+    long long prop_thresh;    // floor((n_m p / lambda)^2 H^2 W^2): propagating bins (defocus only), or -1 = all
+    double nm_over_lambda_sq; // (n_medium / lambda)^2, cycles^2 / um^2
+    double defocus_um;        // delta z of Eq. 3; 0 = none
+    double pad_;
 };
 
 constexpr int kOpticsChunk = 16;
@@ -72,6 +76,7 @@ struct osog_ctx {
     int status_idx;                 // slot used by the last render call
     bool scratch_dirty;             // a call failed midway: count / status must be cleared explicitly
     float2* field;                  // [max_frames][H][W] (intensity path)
+    float2* work;                   // [max_frames][H][W] second complex batch (DIC path; allocated by the first DIC call)
     osog::DeviceStatus* h_status;   // pinned host mirror
     cufftHandle plan_one, plan_batch;
     bool has_plan_one, has_plan_batch;
@@ -86,7 +91,12 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
 cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float* d_opd, float2* d_field);
 cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd);
 // optics.cu
-cudaError_t launch_pupil(osog_ctx* c, int B, float2* spec);
+cudaError_t launch_pupil(osog_ctx* c, int B, float2* spec, double pitch, bool defocus);
+cudaError_t launch_pupil_fill(osog_ctx* c, int B, float2* spec, double pitch, bool defocus);
+cudaError_t launch_dic_shear(osog_ctx* c, int B, const float2* field, float2* out, int sx, int sy, double theta);
+cudaError_t launch_abs2(osog_ctx* c, int B, float2* buf, double scale);
+cudaError_t launch_cmul(osog_ctx* c, int B, float2* a, const float2* b, double scale);
+cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_out, double sigma, uint64_t seed);
 cudaError_t launch_sensor(osog_ctx* c, int B, const float2* img, float* d_intensity, double sigma, uint64_t seed);
 
 }  // namespace osog

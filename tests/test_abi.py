@@ -31,7 +31,8 @@ def test_header_symbols_are_exported():
 def test_struct_layouts_follow_the_header():
     src = re.sub(r"/\*.*?\*/", "", open(HEADER).read(), flags=re.S)
     bodies = {m.group(2): m.group(1) for m in re.finditer(r"typedef struct \{([^}]*)\} (\w+);", src)}
-    for name, st in (("osog_config", og.osog_config), ("osog_particles", og.osog_particles), ("osog_optics", og.osog_optics)):
+    for name, st in (("osog_config", og.osog_config), ("osog_particles", og.osog_particles), ("osog_optics", og.osog_optics),
+                     ("osog_dic", og.osog_dic)):
         body = bodies[name]
         fields = []
         for decl in body.split(";"):
@@ -43,7 +44,8 @@ def test_struct_layouts_follow_the_header():
         assert fields == [f[0] for f in st._fields_], name
     assert C.sizeof(og.osog_config) == 48
     assert C.sizeof(og.osog_particles) == 8 + 13 * 8
-    assert C.sizeof(og.osog_optics) == 80
+    assert C.sizeof(og.osog_optics) == 88
+    assert C.sizeof(og.osog_dic) == 24
 
 
 def test_calls_that_need_no_device():
