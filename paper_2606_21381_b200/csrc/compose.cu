@@ -17,6 +17,7 @@ struct ComposeArgs {
     const uint32_t* offset;
     uint32_t* count;
     uint32_t* list;
+    uint16_t* meta;
     const FrameOptics* optics;
     const float2 *ramp_x, *ramp_y;
     const DeviceStatus* status;
@@ -28,16 +29,14 @@ struct ComposeArgs {
 
 constexpr int kWarps = kComposeThreads / 32;
 constexpr int kSlotStride4 = 9;                    // survivor slot stride in float4 (8 used, odd stride: conflict-free lane-per-slot writes)
-constexpr int kSmemIds = kSortCap * 4;
-constexpr int kSmemMeta = kSortCap * 2;              // per list entry: sub-tile mask (8 bits) | evaluation code << 8
 constexpr int kSmemSlots = kWarps * 32 * kSlotStride4 * 16;
-constexpr int kSmemBytes = kSmemIds + kSmemMeta + kSmemSlots;
+constexpr int kSmemBytes = kSmemSlots;             // k_compose_tile: per-warp survivor slots only
 
 // ---- small PTX helpers ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float fast_sqrt(float x)
 {
     float r;
-    asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));    // one MUFU.SQRT (no denormal fix-up: w < 1e-38 -> t = 0)
     return r;
 }
 __device__ __forceinline__ float min3(float a, float b, float c)
@@ -245,16 +244,32 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
     }
 }
 
-// ---- list ordering ----------------------------------------------------------------------------------------------------
-// In-place ascending sort of list[0..L) in GLOBAL memory by one CTA (only for lists longer than kSortCap):
-// bitonic network in its "all comparators ascending" form, so that virtual +inf padding beyond L never moves.
-__device__ void sort_global(uint32_t* a, uint32_t L)
+// ---- H4 (second half) + tile-level cull: one WARP per tile ------------------------------------------------------------
+// Sorts the tile's list ascending in place (the canonical, deterministic summation order) and writes one 16-bit word
+// per list entry: bits 0..7 = which of the tile's 8 warp sub-tiles (16 x 8 pixels) the particle can touch (bounding
+// box + oriented-box test), bits 8..10 = the evaluation code of the record.  k_compose_tile then needs no barrier.
+// Rank sort (ids are unique inside a tile): the list is staged in the warp's shared-memory slice, every lane counts
+// the ids smaller than its own with broadcast 128-bit reads; the record header loads of the cull are issued first so
+// that their latency hides behind the counting.  Lists longer than kWarpSortCap (pathological crowding) are sorted in
+// global memory by the same warp (bitonic network, slow but correct).
+constexpr int kWarpSortCap = 1024;                 // list entries a warp sorts in shared memory (4 KB per warp)
+
+__device__ __forceinline__ uint32_t tile_meta(const float4 h0, const float4 h1, int tx, int ty)
+{
+    uint32_t mask = 0;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w)
+        mask |= cull_subtile(h0, h1, tx * kTile + (w & 1) * 16, ty * kTile + (w >> 1) * 8) ? (1u << w) : 0u;
+    return mask | (header_code(h0, h1) << 8);
+}
+
+__device__ void sort_global_warp(uint32_t* a, uint32_t L, int lane)
 {
     uint32_t P = 1;
     while (P < L) P <<= 1;
     for (uint32_t k = 2; k <= P; k <<= 1) {
         for (uint32_t j = k >> 1; j > 0; j >>= 1) {
-            for (uint32_t t = threadIdx.x; t < (P >> 1); t += blockDim.x) {
+            for (uint32_t t = lane; t < (P >> 1); t += 32) {
                 uint32_t lo, hi;
                 if (j == (k >> 1)) {                       // first step of a merge: mirror inside the block of size k
                     const uint32_t blk = t / j, r = t % j;
@@ -264,24 +279,69 @@ __device__ void sort_global(uint32_t* a, uint32_t L)
                     lo = (t / j) * (2 * j) + (t % j);
                     hi = lo + j;
                 }
-                if (hi < L) {
+                if (hi < L) {                              // virtual +inf padding beyond L never moves
                     const uint32_t x = a[lo], y = a[hi];
                     if (x > y) { a[lo] = y; a[hi] = x; }
                 }
             }
             __threadfence_block();
-            __syncthreads();
+            __syncwarp();
         }
     }
 }
 
+__global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __restrict__ recs, const uint32_t* __restrict__ offset,
+                                                             uint32_t* __restrict__ count, uint32_t* __restrict__ list,
+                                                             uint16_t* __restrict__ meta, const DeviceStatus* __restrict__ status,
+                                                             int ntx, int nty, int n_tiles)
+{
+    __shared__ __align__(16) uint32_t s_all[kWarps * kWarpSortCap];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int tile = blockIdx.x * kWarps + wid;
+    if (tile >= n_tiles) return;
+    if (lane == 0) count[tile] = 0u;                             // keep the "count is zero on entry" invariant (binning.cu)
+    if ((status->bits & OSOG_WOVERFLOW) != 0u) return;
+    const uint32_t beg = offset[tile];
+    const uint32_t L = offset[tile + 1] - beg;
+    if (L == 0u) return;
+    uint32_t* glist = list + beg;
+    const int tpf = ntx * nty;
+    const int rt = tile % tpf;
+    const int ty = rt / ntx, tx = rt - ty * ntx;
+    const float4* recs4 = reinterpret_cast<const float4*>(recs);
+    if (L <= (uint32_t)kWarpSortCap) {
+        uint32_t* s = s_all + wid * kWarpSortCap;
+        const uint32_t L4 = (L + 3u) & ~3u;
+        for (uint32_t k = lane; k < L4; k += 32) s[k] = k < L ? glist[k] : 0xffffffffu;
+        __syncwarp();
+        for (uint32_t k = lane; k < L; k += 32) {
+            const uint32_t v = s[k];
+            const float4* rec = recs4 + (size_t)v * (kRecWords / 4);
+            const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);   // cxp, cyp, ax, ay | ha, hb, bbx, bby
+            uint32_t r = 0;
+            const uint4* s4 = reinterpret_cast<const uint4*>(s);
+            for (uint32_t m = 0; m < L4 / 4; ++m) {
+                const uint4 q = s4[m];
+                r += (q.x < v ? 1u : 0u) + (q.y < v ? 1u : 0u) + (q.z < v ? 1u : 0u) + (q.w < v ? 1u : 0u);
+            }
+            glist[r] = v;                                        // the sorted segment (also what osog_debug_bins returns)
+            meta[beg + r] = (uint16_t)tile_meta(h0, h1, tx, ty);
+        }
+    } else {
+        sort_global_warp(glist, L, lane);
+        for (uint32_t k = lane; k < L; k += 32) {
+            const float4* rec = recs4 + (size_t)glist[k] * (kRecWords / 4);
+            meta[beg + k] = (uint16_t)tile_meta(__ldg(rec), __ldg(rec + 1), tx, ty);
+        }
+    }
+}
+
+// ---- H5-H7: every warp is independent (no barrier, no shared list): it walks its tile's sorted list in batches of 32
 template <bool OPD, bool FIELD, bool RAMP>
 __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const ComposeArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
-    uint32_t* s_ids = reinterpret_cast<uint32_t*>(smem);                          // this tile's list, ascending
-    uint16_t* s_meta = reinterpret_cast<uint16_t*>(smem + kSmemIds);              // per entry: sub-tile mask | code << 8
-    float4* s_slots = reinterpret_cast<float4*>(smem + kSmemIds + kSmemMeta);     // per-warp survivor slots
+    float4* s_slots = reinterpret_cast<float4*>(smem);                            // per-warp survivor slots
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int tpf = a.ntx * a.nty;
@@ -292,44 +352,8 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
     const bool overflow = (a.status->bits & OSOG_WOVERFLOW) != 0u;
     const uint32_t beg = a.offset[tile];
     const uint32_t L = overflow ? 0u : a.offset[tile + 1] - beg;
-    uint32_t* glist = a.list + beg;
-    if (tid == 0) a.count[tile] = 0u;                            // keep the "count is zero on entry" invariant (binning.cu)
-
-    // ---- H4 (second half): canonical order ------------------------------------------------------------------------
-    const bool in_smem = L <= (uint32_t)kSortCap;
-    if (in_smem) {
-        uint32_t* s_in = reinterpret_cast<uint32_t*>(s_slots);   // kSmemSlots >= kSmemIds
-        for (uint32_t k = tid; k < L; k += kComposeThreads) s_in[k] = glist[k];
-        __syncthreads();
-        if (L * 2u <= (uint32_t)kComposeThreads) {
-            // short list (the usual case): S = 2, 4 or 8 adjacent lanes share one element, each counts the smaller ids
-            // in its part of the list, a shuffle adds the parts (rank sort: ids are unique inside a tile)
-            const uint32_t S = L * 8u <= (uint32_t)kComposeThreads ? 8u : (L * 4u <= (uint32_t)kComposeThreads ? 4u : 2u);
-            const uint32_t e = (uint32_t)tid / S, h = (uint32_t)tid % S;
-            const uint32_t part = (L + S - 1u) / S, m0 = h * part, m1 = min(L, m0 + part);
-            const uint32_t v = e < L ? s_in[e] : 0u;
-            uint32_t r = 0;
-            for (uint32_t m = m0; m < m1; ++m) r += s_in[m] < v ? 1u : 0u;
-            r += __shfl_xor_sync(0xffffffffu, r, 1);
-            if (S > 2u) r += __shfl_xor_sync(0xffffffffu, r, 2);
-            if (S > 4u) r += __shfl_xor_sync(0xffffffffu, r, 4);
-            if (e < L && h == 0u) {
-                s_ids[r] = v;
-                glist[r] = v;                                    // write the sorted segment back (osog_debug_bins)
-            }
-        } else {
-            for (uint32_t k = tid; k < L; k += kComposeThreads) {
-                const uint32_t v = s_in[k];
-                uint32_t r = 0;
-                for (uint32_t m = 0; m < L; ++m) r += s_in[m] < v ? 1u : 0u;
-                s_ids[r] = v;
-                glist[r] = v;
-            }
-        }
-        __syncthreads();
-    } else {
-        sort_global(glist, L);
-    }
+    const uint32_t* __restrict__ glist = a.list + beg;
+    const uint16_t* __restrict__ gmeta = a.meta + beg;
 
     // ---- pixel ownership ------------------------------------------------------------------------------------------------
     const int wx0 = tx * kTile + (wid & 1) * 16, wy0 = ty * kTile + (wid >> 1) * 8;   // warp sub-tile origin
@@ -346,41 +370,21 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
     float4* my_slots = s_slots + wid * 32 * kSlotStride4;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
 
-    // ---- CTA-level cull: one thread per list entry tests the particle against all 8 sub-tiles of the tile (one header
-    // read per entry instead of one per warp) and leaves an 8-bit mask + the evaluation code in shared memory.
     const float4* recs4 = reinterpret_cast<const float4*>(a.rec);
-    if (in_smem) {
-        for (uint32_t k = tid; k < L; k += kComposeThreads) {
-            const float4* rec = recs4 + (size_t)s_ids[k] * (kRecWords / 4);
-            const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);   // cxp, cyp, ax, ay | ha, hb, bbx, bby
-            uint32_t mask = 0;
-#pragma unroll
-            for (int w = 0; w < kWarps; ++w)
-                mask |= cull_subtile(h0, h1, tx * kTile + (w & 1) * 16, ty * kTile + (w >> 1) * 8) ? (1u << w) : 0u;
-            const uint32_t code = header_code(h0, h1);
-            s_meta[k] = (uint16_t)(mask | (code << 8));
-            if (mask != 0u && code != 0u) asm volatile("prefetch.global.L1 [%0];" ::"l"(rec + 8));   // 2nd line: slabs 2..5
-        }
-        __syncthreads();
-    }
-    // From here on the warps of the CTA are independent (no barrier): each walks the whole list in batches of 32.
+    // entry of the first batch (the loop below always holds the next batch's entry in registers: the list loads of
+    // batch n + 1 are in flight while batch n is evaluated)
+    uint32_t nmeta = lane < L ? gmeta[lane] : 0u;
+    uint32_t npid = lane < L ? glist[lane] : 0u;
     for (uint32_t base = 0; base < L; base += 32) {
         // ---- lane <-> list entry base + lane: survivors of this warp's sub-tile -------------------------------------------
-        const uint32_t k = base + lane;
-        bool keep = false;
-        uint32_t pid = 0, code = 0;
-        if (in_smem) {
-            const uint32_t meta = k < L ? s_meta[k] : 0u;
-            keep = ((meta >> wid) & 1u) != 0u;
-            code = meta >> 8;
-            if (keep) pid = s_ids[k];
-        } else if (k < L) {                                      // very long list (sorted in global memory): per-warp cull
-            pid = glist[k];
-            const float4* rec = recs4 + (size_t)pid * (kRecWords / 4);
-            const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);
-            code = header_code(h0, h1);
-            keep = cull_subtile(h0, h1, wx0, wy0);
+        const uint32_t meta = nmeta, pid = npid;
+        {
+            const uint32_t kn = base + 32 + lane;
+            nmeta = kn < L ? gmeta[kn] : 0u;
+            npid = kn < L ? glist[kn] : 0u;
         }
+        const bool keep = ((meta >> wid) & 1u) != 0u;
+        const uint32_t code = meta >> 8;
         // Survivors are grouped by evaluation class (fixed, data-dependent order: NS0 prisms, NS1, NS2, all-fp64,
         // ellipsoids; ascending particle index inside a class), so each class runs in its own branch-free loop.
         const unsigned m1 = __ballot_sync(0xffffffffu, keep && code == 1u);
@@ -498,16 +502,23 @@ static cudaError_t launch_variant(const ComposeArgs& a, unsigned grid, cudaStrea
     return cudaGetLastError();
 }
 
-cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float* d_opd, float2* d_field)
+// sort_first = false: the lists of the last call are already sorted and culled (osog_debug_recompose_field)
+cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float* d_opd, float2* d_field, bool sort_first)
 {
     (void)N;
     ComposeArgs a;
-    a.rec = c->rec; a.offset = c->offset; a.count = c->count; a.list = c->list; a.optics = c->optics;
+    a.rec = c->rec; a.offset = c->offset; a.count = c->count; a.list = c->list; a.meta = c->meta; a.optics = c->optics;
     a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.status = c->status + c->status_idx;
     a.opd = d_opd; a.field = d_field;
     a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
     a.ramp_y_on = 1;
     const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
+    if (sort_first) {
+        k_sort_cull<<<(grid + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(c->rec, c->offset, c->count, c->list, c->meta,
+                                                                                     a.status, c->ntx, c->nty, (int)grid);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
     if (d_opd != nullptr && d_field == nullptr) return launch_variant<true, false, false>(a, grid, c->stream);
     if (d_opd == nullptr && !has_ramp) return launch_variant<false, true, false>(a, grid, c->stream);
     if (d_opd == nullptr && has_ramp) return launch_variant<false, true, true>(a, grid, c->stream);

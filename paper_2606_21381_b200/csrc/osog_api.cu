@@ -166,7 +166,7 @@ int osog_destroy(osog_ctx* c)
     if (c->has_plan_one) cufftDestroy(c->plan_one);
     if (c->has_plan_batch) cufftDestroy(c->plan_batch);
     cudaFree(c->rec); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
-    cudaFree(c->offset); cudaFree(c->list); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
+    cudaFree(c->offset); cudaFree(c->list); cudaFree(c->meta); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
     cudaFree(c->status); cudaFree(c->field); cudaFree(c->work);
     if (c->h_status) cudaFreeHost(c->h_status);
     delete c;
@@ -210,6 +210,7 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     A(dalloc(&c->count, (size_t)c->max_tiles));
     A(dalloc(&c->offset, (size_t)c->max_tiles + 1));
     A(dalloc(&c->list, (size_t)c->max_pairs));
+    A(dalloc(&c->meta, (size_t)c->max_pairs));
     A(dalloc(&c->ramp_x, (size_t)c->max_frames * c->W));
     A(dalloc(&c->ramp_y, (size_t)c->max_frames * c->H));
     A(dalloc(&c->optics, (size_t)c->max_frames));
@@ -342,7 +343,7 @@ int osog_debug_recompose_field(osog_ctx* c, float* d_field)
 {
     if (!c || !d_field || !aligned16(d_field) || c->last_B < 1 || c->last_has_ramp < 0) return OSOG_EINVAL;
     DeviceGuard g(c->device);
-    cudaError_t e = launch_compose(c, c->last_N, c->last_B, c->last_has_ramp != 0, nullptr, reinterpret_cast<float2*>(d_field));
+    cudaError_t e = launch_compose(c, c->last_N, c->last_B, c->last_has_ramp != 0, nullptr, reinterpret_cast<float2*>(d_field), false);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
 }

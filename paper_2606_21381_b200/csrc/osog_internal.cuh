@@ -11,8 +11,6 @@ namespace osog {
 // ---- build-time constants -----------------------------------------------------------------------------------
 constexpr int kTile = 32;              // binning tile edge T (pixels); one CTA composes one tile
 constexpr int kComposeThreads = 256;   // 8 warps; each warp owns a 16 x 8 pixel sub-tile, each lane 4 x 1 pixels
-constexpr int kChunk = 64;             // particle records staged in shared memory per pass
-constexpr int kSortCap = 2048;         // longest tile list sorted in shared memory (longer: sorted in global memory)
 constexpr int kRecWords = 64;          // 256-byte record per particle: 16 header words + up to 24 doubles
 constexpr double kBBoxPadPx = 1.0 / 1024.0;   // delta of DESIGN.md B2
 constexpr float kSteepSlope = 16.0f;   // slabs steeper than this (|n_xy| / |n_z|) are refined in fp64 where active
@@ -69,6 +67,7 @@ struct osog_ctx {
     uint32_t* count;                // [max_tiles] per-tile count, reused as the fill cursor
     uint32_t* offset;               // [max_tiles + 1]
     uint32_t* list;                 // [max_pairs]
+    uint16_t* meta;                 // [max_pairs] per list entry: sub-tile mask | evaluation code << 8 (k_sort_cull)
     float2* ramp_x;                 // [max_frames][W]  exp(i 2 pi fx0 x_j)
     float2* ramp_y;                 // [max_frames][H]
     osog::FrameOptics* optics;      // [max_frames]
@@ -88,7 +87,7 @@ namespace osog {
 cudaError_t upload_optics(osog_ctx* c, const osog_optics* o, OpticsChunk* first);
 cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o);
 // compose.cu
-cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float* d_opd, float2* d_field);
+cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float* d_opd, float2* d_field, bool sort_first = true);
 cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd);
 // optics.cu
 cudaError_t launch_pupil(osog_ctx* c, int B, float2* spec, double pitch, bool defocus);
