@@ -70,6 +70,14 @@ __device__ __forceinline__ double f2d_pos(float f)
     const uint32_t u = __float_as_uint(f);
     return __hiloint2double((int)((u >> 3) + 0x38000000u), (int)(u << 29));
 }
+// double -> float of max(w, 0) by truncation, with integer ops on the ALU pipe instead of an XU-pipe F2F.F32.F64 + FMNMX:
+// a negative or tiny w (< 2^-126) gives +0 or a denormal below 1e-44, which sqrt.approx.ftz flushes to 0.
+// Relative error < 2^-23 (truncation of the mantissa), i.e. 2^-24 in the thickness sqrt(w).
+__device__ __forceinline__ float d2f_pos_trunc(double w)
+{
+    const int hi = max(__double2hiint(w) - 0x38000000, 0);
+    return __uint_as_float(__funnelshift_l((unsigned)__double2loint(w), (unsigned)hi, 3));
+}
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
 {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -169,7 +177,7 @@ __device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ slot, 
     for (int k = 0; k < 4; ++k) {
         const double djk = dj + (double)k;
         const double w = fma(-fma(ab.x, djk, b1), djk, cc);      // 1 - d^T S d
-        const float t = fast_sqrt(fmaxf((float)w, 0.0f));
+        const float t = fast_sqrt(d2f_pos_trunc(w));
         acc[k] = fma(f2d_pos(t), Kd, acc[k]);
     }
 }
