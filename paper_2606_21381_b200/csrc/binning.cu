@@ -35,16 +35,22 @@ __device__ __forceinline__ float2 cis_turns(double t)
     return make_float2((float)c, (float)s);
 }
 
-__global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
+constexpr int kPrepThreads = 128;
+
+// Grid layout (blocks of 128 threads): [0, nb) binning role, one particle per thread; [nb, 2 nb) record role, one
+// particle per thread, the block's 128 particles permuted so that prisms come first and ellipsoids last (warps are then
+// uniform in the code path they take, except one mixed warp per block); [2 nb, ...) ramp tables.  nb = ceil(N / 128).
+__global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
 {
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long nb = (a.N + kPrepThreads - 1) / kPrepThreads;
 
     if (gid < a.B && gid < kOpticsChunk) a.optics[gid] = a.oc.f[gid];
 
-    if (gid >= 2 * a.N) {
+    if ((long long)blockIdx.x >= 2 * nb) {
         // ---- phase-ramp tables exp(i 2 pi fx0 x_j), x_j = (j + 1/2) p  (oblique illumination)
         if (!a.has_ramp) return;
-        long long r = gid - 2 * a.N;
+        long long r = gid - 2 * nb * kPrepThreads;
         const long long nx = (long long)a.B * a.W, ny = (long long)a.B * a.H;
         if (r < nx) {
             const int b = (int)(r / a.W), j = (int)(r % a.W);
@@ -59,10 +65,32 @@ __global__ void __launch_bounds__(128) k_prepare(const PrepArgs a)
         return;
     }
 
-    // ---- H1/H2: one particle = two threads: role 0 does the binning (bounding box, tile range, counts), role 1 the
-    // derived record (the two halves are independent; splitting them halves the latency-bound critical path)
-    const long long n = gid >> 1;
-    const int role = (int)(gid & 1);
+    // ---- H1/H2: one particle = two threads in different blocks: role 0 does the binning (bounding box, tile range,
+    // counts), role 1 the derived record (the two halves are independent; splitting them halves the critical path)
+    const int role = (long long)blockIdx.x >= nb ? 1 : 0;
+    long long n = (long long)(blockIdx.x - (role ? nb : 0)) * kPrepThreads + threadIdx.x;
+    if (role == 1) {
+        __shared__ unsigned char s_perm[kPrepThreads];
+        __shared__ int s_np[kPrepThreads / 32];
+        const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+        const bool is_prism = n < a.N && a.kind[n] == 1u;
+        const unsigned mp = __ballot_sync(0xffffffffu, is_prism);
+        if (lane == 0) s_np[wid] = __popc(mp);
+        __syncthreads();
+        int before_p = 0, total_p = 0;
+#pragma unroll
+        for (int w = 0; w < kPrepThreads / 32; ++w) {
+            if (w < wid) before_p += s_np[w];
+            total_p += s_np[w];
+        }
+        const unsigned lt = (1u << lane) - 1u;
+        const int pos = is_prism ? before_p + __popc(mp & lt)
+                                 : total_p + (wid * 32 - before_p) + __popc(~mp & lt);
+        s_perm[pos] = (unsigned char)threadIdx.x;
+        __syncthreads();
+        n += (int)s_perm[threadIdx.x] - (int)threadIdx.x;
+    }
+    if (n >= a.N) return;
     const float fcx = a.cx[n], fcy = a.cy[n], fqw = a.qw[n], fqx = a.qx[n], fqy = a.qy[n], fqz = a.qz[n];
     const float fd0 = a.d0[n], fd1 = a.d1[n], fd2 = a.d2[n], fnp = a.n_p[n];
     const unsigned kind = a.kind[n];
@@ -432,10 +460,11 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     a.has_ramp = (o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0) ? 1 : 0;
     if ((e = upload_optics(c, o, &a.oc)) != cudaSuccess) return e;
 
-    long long items = 2 * N + (a.has_ramp ? (long long)B * (c->W + c->H) : 0);
-    if (items < B) items = B;
-    const int threads = 128;
-    const long long blocks = (items + threads - 1) / threads;
+    const int threads = kPrepThreads;
+    const long long nb = (N + threads - 1) / threads;
+    const long long ramp_items = a.has_ramp ? (long long)B * (c->W + c->H) : 0;
+    long long blocks = 2 * nb + (ramp_items + threads - 1) / threads;
+    if (blocks * threads < B) blocks = (B + threads - 1) / threads;     // the first threads also upload the optics
     k_prepare<<<(unsigned)blocks, threads, 0, c->stream>>>(a);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     k_scan<<<1, 1024, 0, c->stream>>>(c->count, c->offset, tiles, c->max_pairs, status, status_next);
