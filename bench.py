@@ -360,7 +360,7 @@ def run_ours(args):
         "ms_per_step_median": float(np.median(ms)), "ms_per_step_std": float(ms.std()),
         "e2e": {"value": world * N * args.steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h)},
-        "gpu_launches": 5 * args.steps,
+        "gpu_launches": 3 * args.steps,
         "roofline": roof, "roofline_hbm": hbm,
         "roofline_step": {"achieved": step_gbs, "frac": step_gbs / peak, "algorithmic_bytes": int(alg_bytes),
                           "what": "whole hot path: k_prepare, k_scan, k_fill, k_compose_tile"},

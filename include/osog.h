@@ -45,7 +45,7 @@ enum {
     OSOG_OK = 0,
     OSOG_EINVAL = -1,     /* null / misaligned pointer, bad size, N > max_particles, B > max_frames, bad optics */
     OSOG_ECUDA = -2,      /* CUDA runtime, launch or cuFFT failure (osog_last_cuda_error gives the code)       */
-    OSOG_ECAPACITY = -3,  /* (particle, tile) pair list overflow: the frames of that call are zero-filled       */
+    OSOG_ECAPACITY = -3,  /* some tile's particle list exceeded its capacity: the frames of that call are zero-filled */
     OSOG_ENOMEM = -4      /* allocation failure in osog_create                                                 */
 };
 /* status bits returned by osog_status (sticky until the next render call) */
@@ -62,7 +62,9 @@ typedef struct {
     int32_t  H, W;           /* frame height / width in pixels, 1 .. 32768; need not be tile multiples     */
     int32_t  max_frames;     /* largest batch B of one call, >= 1                                          */
     int64_t  max_particles;  /* largest N (total over the batch) of one call, >= 0                         */
-    int64_t  max_pairs;      /* capacity of the (particle, tile) pair list; 0 = 64 * max_particles + 1024  */
+    int64_t  max_pairs;      /* capacity of the (particle, tile) pair lists; 0 = 64 * max_particles + 1024.  It is
+                                divided evenly among the max_frames * ceil(H/T) * ceil(W/T) tiles of the context:
+                                one tile's list holds floor(max_pairs / tiles) entries (at least 1)               */
 } osog_config;
 
 /* Particle state, Structure of Arrays ("S in R^{N x D}"): one DEVICE array of length N per
@@ -102,12 +104,12 @@ typedef struct {
     double   bias_rad;                /* bias phase theta                                                         */
 } osog_dic;
 
-/* Create a context: allocates all scratch (records, bounding boxes, tile counts / offsets / lists, ramp
+/* Create a context: allocates all scratch (records, bounding boxes, per-tile counters and fixed-capacity lists, ramp
  * tables, one complex frame batch and the cuFFT plans).  *out is set to NULL on failure. */
 int osog_create(osog_ctx** out, const osog_config* cfg);
 
 /* OPD frame(s): d_opd is DEVICE float [B, H, W], row-major, micrometres.  Steps H1-H6 of DESIGN.md:
- * prepare + bounding box + tile count, scan, fill, per-tile ordered composition. */
+ * prepare + bounding box + append to the per-tile lists, per-tile sort + cull, per-tile ordered composition. */
 int osog_render_opd(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd);
 
 /* Complex exit wave: d_field is DEVICE float [B, H, W, 2] (interleaved re, im = complex64).  Same steps as
@@ -142,11 +144,13 @@ int osog_render_opd_atomic(osog_ctx* ctx, const osog_particles* p, int64_t N, co
 int osog_destroy(osog_ctx* ctx);
 
 /* Synchronises the stream.  *status_bits = OSOG_W* bits of the last render call, *pairs = number of
- * (particle, tile) pairs that call needed (compare with max_pairs).  Either pointer may be NULL.
+ * (particle, tile) pairs of that call; if it overflowed: the max_pairs that would have sufficed (longest tile
+ * list x tiles of the context).  Either pointer may be NULL.
  * Returns OSOG_ECAPACITY if the last call overflowed, OSOG_ECUDA on a sticky CUDA error, else OSOG_OK. */
 int osog_status(osog_ctx* ctx, uint32_t* status_bits, int64_t* pairs);
 
-/* Test / diagnostics: synchronises, then copies the binning of the last render call to HOST arrays:
+/* Test / diagnostics: synchronises, then writes the binning of the last render call to HOST arrays (the scan and
+ * the compaction of the tiles' fixed-capacity slices run on the host):
  * h_offset [n_tiles + 1] (exclusive scan of the per-tile counts), h_list [min(pairs, cap)] (each tile's
  * segment in ascending particle index).  Tile id = frame * tiles_per_frame + (i / T) * ceil(W / T) + (j / T).
  * Any pointer may be NULL.  *n_tiles and *n_pairs are always written. */

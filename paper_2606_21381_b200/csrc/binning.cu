@@ -1,7 +1,7 @@
-// H1-H4 of DESIGN.md: per-particle preparation (fp64), bounding box -> tile range -> per-tile count,
-// exclusive scan, fill of the per-tile particle lists.  Integer results must equal the oracle's binning
-// bit for bit (B1-B4); the canonical (ascending) order of each list is established by
-// the composition kernel, which sorts its own segment and writes it back (compose.cu).
+// H1-H4 of DESIGN.md: per-particle preparation (fp64), bounding box -> tile range -> append to the per-tile lists
+// (fixed capacity per tile, the atomic on the tile's counter gives the slot: no scan and no second fill pass).  Integer
+// results must equal the oracle's binning bit for bit (B1-B4); the canonical (ascending) order of
+// each list is established by k_sort_cull (compose.cu); osog_debug_bins builds the exclusive scan on the host.
 #include "osog_internal.cuh"
 
 namespace osog {
@@ -16,7 +16,9 @@ struct PrepArgs {
     float* rec;
     int4* tbox;
     int* pframe;
-    uint32_t* count;
+    uint32_t* count;              // this call's slot of the per-tile counters (all zero on entry)
+    uint32_t* list;               // [tiles][tile_cap]
+    int tile_cap;
     float2 *ramp_x, *ramp_y;
     FrameOptics* optics;
     DeviceStatus* status;
@@ -163,13 +165,25 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
         a.tbox[n] = tb;
         return;
     }
-    // B3: tile range + count
+    // B3 / H4: tile range; append the particle to every tile of the range.  The atomic on the tile's counter returns the
+    // slot; up to 4 atomics of a tile row are in flight before their slots are used (one memory round trip per row).
     tb = make_int4(j0 / kTile, j1 / kTile, i0 / kTile, i1 / kTile);
     a.tbox[n] = tb;
     {
-        uint32_t* cnt = a.count + (size_t)b * a.ntx * a.nty;
-        for (int ty = tb.z; ty <= tb.w; ++ty)
-            for (int tx = tb.x; tx <= tb.y; ++tx) atomicAdd(&cnt[ty * a.ntx + tx], 1u);
+        const size_t t0 = (size_t)b * a.ntx * a.nty;
+        const uint32_t cap = (uint32_t)a.tile_cap;
+        for (int ty = tb.z; ty <= tb.w; ++ty) {
+            for (int tx = tb.x; tx <= tb.y; tx += 4) {
+                const size_t t = t0 + (size_t)ty * a.ntx + tx;
+                uint32_t pos[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    if (tx + q <= tb.y) pos[q] = atomicAdd(&a.count[t + q], 1u);
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    if (tx + q <= tb.y && pos[q] < cap) a.list[(t + q) * cap + pos[q]] = (uint32_t)n;
+            }
+        }
     }
 
     // words 0, 1, 6, 7 of the record: centre in pixel-index coordinates and the packed pixel bounding box
@@ -312,76 +326,6 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
     r32[10] = 0.0f;
 }
 
-// H3: exclusive scan of count[0..n) -> offset[0..n], total -> status->pairs; count is reset to 0 (it becomes
-// the fill cursor).  One CTA: each thread scans a contiguous run, warp shuffles combine the runs.
-__global__ void __launch_bounds__(1024) k_scan(uint32_t* __restrict__ count, uint32_t* __restrict__ offset,
-                                               long long n, long long max_pairs, DeviceStatus* status,
-                                               DeviceStatus* status_next)
-{
-    if (threadIdx.x == 0) { status_next->bits = 0u; status_next->pad = 0u; status_next->pairs = 0ull; }   // for the next call
-
-    __shared__ unsigned long long warp_sum[32];
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const long long per = (n + blockDim.x - 1) / blockDim.x;
-    const long long lo = min(n, per * tid), hi = min(n, lo + per);
-    unsigned long long s = 0;
-    for (long long k = lo; k < hi; ++k) s += count[k];
-    unsigned long long incl = s;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const unsigned long long v = __shfl_up_sync(0xffffffffu, incl, d);
-        if (lane >= d) incl += v;
-    }
-    if (lane == 31) warp_sum[wid] = incl;
-    __syncthreads();
-    if (wid == 0) {
-        unsigned long long v = warp_sum[lane], t = v;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const unsigned long long u = __shfl_up_sync(0xffffffffu, t, d);
-            if (lane >= d) t += u;
-        }
-        warp_sum[lane] = t - v;                  // exclusive over warps
-        if (lane == 31) {
-            status->pairs = t;
-            if (t > (unsigned long long)max_pairs) atomicOr(&status->bits, OSOG_WOVERFLOW);
-            offset[n] = (uint32_t)min(t, 0xffffffffull);
-        }
-    }
-    __syncthreads();
-    unsigned long long run = warp_sum[wid] + (incl - s);
-    for (long long k = lo; k < hi; ++k) {
-        const uint32_t c = count[k];
-        offset[k] = (uint32_t)min(run, 0xffffffffull);
-        count[k] = 0u;
-        run += c;
-    }
-}
-
-// H4: every listed particle appends its index to each tile of its range: one warp per particle, one lane per tile
-// (the atomics return the cursor, so a single thread walking its tiles would pay one memory round trip per tile).
-// Order inside a tile is whatever the atomics give; the composition kernel sorts each segment ascending before use.
-__global__ void __launch_bounds__(256) k_fill(const int4* __restrict__ tbox, const int* __restrict__ pframe,
-                                              uint32_t* __restrict__ cursor, const uint32_t* __restrict__ offset,
-                                              uint32_t* __restrict__ list, long long N, int ntx, int nty,
-                                              const DeviceStatus* status)
-{
-    const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
-    if (n >= N) return;
-    if (status->bits & OSOG_WOVERFLOW) return;
-    const int4 tb = tbox[n];
-    if (tb.x > tb.y) return;
-    const size_t base = (size_t)pframe[n] * ntx * nty;
-    const int tw = tb.y - tb.x + 1, nt = tw * (tb.w - tb.z + 1);
-    for (int q = lane; q < nt; q += 32) {
-        const int ty = tb.z + q / tw, tx = tb.x + q % tw;
-        const size_t t = base + (size_t)ty * ntx + tx;
-        const uint32_t pos = atomicAdd(&cursor[t], 1u);
-        list[offset[t] + pos] = (uint32_t)n;
-    }
-}
-
 __global__ void k_set_optics(FrameOptics* optics, const OpticsChunk oc)
 {
     const int k = threadIdx.x;
@@ -437,17 +381,16 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     c->last_B = B;
     c->last_tiles = tiles;
     cudaError_t e;
-    // Invariant kept by the kernels themselves (no memset nodes in the steady state): count[] is all zero on entry
-    // (k_scan turns it into the fill cursor, k_compose_tile zeroes its own tile's entry again) and the status slot of
-    // this call was cleared by the previous call's k_scan.  After a failed or atomic-variant call: clear explicitly.
+    // Invariant kept by the kernels themselves (no memset nodes in the steady state): the counter slot and the status
+    // slot of this call are all zero on entry (cleared by the previous call's k_sort_cull, which works on the other
+    // slot).  After a failed or atomic-variant call: clear explicitly.
     if (c->scratch_dirty) {
-        if ((e = cudaMemsetAsync(c->count, 0, sizeof(uint32_t) * (size_t)c->max_tiles, c->stream)) != cudaSuccess) return e;
+        if ((e = cudaMemsetAsync(c->count, 0, sizeof(uint32_t) * 2 * (size_t)c->max_tiles, c->stream)) != cudaSuccess) return e;
         if ((e = cudaMemsetAsync(c->status, 0, 2 * sizeof(DeviceStatus), c->stream)) != cudaSuccess) return e;
     }
     c->scratch_dirty = true;
     c->status_idx ^= 1;
     DeviceStatus* status = c->status + c->status_idx;
-    DeviceStatus* status_next = c->status + (c->status_idx ^ 1);
 
     PrepArgs a;
     a.cx = p->cx; a.cy = p->cy; a.qw = p->qw; a.qx = p->qx; a.qy = p->qy; a.qz = p->qz;
@@ -455,7 +398,8 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     a.frame_start = B > 1 ? p->frame_start : nullptr;
     a.N = N; a.B = B; a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
     a.pitch = o->pitch_um; a.n_medium = o->n_medium;
-    a.rec = c->rec; a.tbox = c->tbox; a.pframe = c->pframe; a.count = c->count;
+    a.rec = c->rec; a.tbox = c->tbox; a.pframe = c->pframe;
+    a.count = c->count + (size_t)c->status_idx * c->max_tiles; a.list = c->list; a.tile_cap = c->tile_cap;
     a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.optics = c->optics; a.status = status;
     a.has_ramp = (o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0) ? 1 : 0;
     if ((e = upload_optics(c, o, &a.oc)) != cudaSuccess) return e;
@@ -467,13 +411,6 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     if (blocks * threads < B) blocks = (B + threads - 1) / threads;     // the first threads also upload the optics
     k_prepare<<<(unsigned)blocks, threads, 0, c->stream>>>(a);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    k_scan<<<1, 1024, 0, c->stream>>>(c->count, c->offset, tiles, c->max_pairs, status, status_next);
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    if (N > 0) {
-        k_fill<<<(unsigned)((N * 32 + 255) / 256), 256, 0, c->stream>>>(
-            c->tbox, c->pframe, c->count, c->offset, c->list, N, c->ntx, c->nty, status);
-        if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    }
     return cudaSuccess;
 }
 

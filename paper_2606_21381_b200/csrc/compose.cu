@@ -14,10 +14,10 @@ namespace osog {
 
 struct ComposeArgs {
     const float* rec;
-    const uint32_t* offset;
-    uint32_t* count;
-    uint32_t* list;
-    uint16_t* meta;
+    const uint32_t* count;       // this call's per-tile list lengths
+    const uint32_t* list;        // [tiles][tile_cap], sorted by k_sort_cull
+    const uint16_t* meta;        // [tiles][tile_cap]
+    int tile_cap;
     const FrameOptics* optics;
     const float2 *ramp_x, *ramp_y;
     const DeviceStatus* status;
@@ -298,20 +298,39 @@ __device__ void sort_global_warp(uint32_t* a, uint32_t L, int lane)
     }
 }
 
-__global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __restrict__ recs, const uint32_t* __restrict__ offset,
-                                                             uint32_t* __restrict__ count, uint32_t* __restrict__ list,
-                                                             uint16_t* __restrict__ meta, const DeviceStatus* __restrict__ status,
+__global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __restrict__ recs, const uint32_t* __restrict__ count,
+                                                             uint32_t* __restrict__ count_next, uint32_t* __restrict__ list,
+                                                             uint16_t* __restrict__ meta, DeviceStatus* __restrict__ status,
+                                                             DeviceStatus* __restrict__ status_next, int tile_cap,
                                                              int ntx, int nty, int n_tiles)
 {
     __shared__ __align__(16) uint32_t s_all[kWarps * kWarpSortCap];
+    __shared__ uint32_t s_len[kWarps];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int tile = blockIdx.x * kWarps + wid;
-    if (tile >= n_tiles) return;
-    if (lane == 0) count[tile] = 0u;                             // keep the "count is zero on entry" invariant (binning.cu)
-    if ((status->bits & OSOG_WOVERFLOW) != 0u) return;
-    const uint32_t beg = offset[tile];
-    const uint32_t L = offset[tile + 1] - beg;
-    if (L == 0u) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {                   // the other status slot belongs to the next call
+        status_next->bits = 0u; status_next->max_count = 0u; status_next->pairs = 0ull;
+    }
+    // list length of the tile; the other counter slot is cleared for the next call; the call's totals (number of pairs,
+    // longest list, overflow of the per-tile capacity) are reduced per CTA
+    const uint32_t Lraw = tile < n_tiles ? count[tile] : 0u;
+    if (tile < n_tiles && lane == 0) count_next[tile] = 0u;
+    if (lane == 0) s_len[wid] = Lraw;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t mx = 0;
+        unsigned long long sum = 0;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) { mx = max(mx, s_len[w]); sum += s_len[w]; }
+        if (sum != 0ull) {
+            atomicAdd(&status->pairs, sum);
+            atomicMax(&status->max_count, mx);
+            if (mx > (uint32_t)tile_cap) atomicOr(&status->bits, OSOG_WOVERFLOW);
+        }
+    }
+    const uint32_t L = Lraw;
+    if (L == 0u || L > (uint32_t)tile_cap) return;               // empty, or overflow (the frames are zero-filled)
+    const size_t beg = (size_t)tile * tile_cap;
     uint32_t* glist = list + beg;
     const int tpf = ntx * nty;
     const int rt = tile % tpf;
@@ -358,8 +377,8 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
     const int ty = rt / a.ntx, tx = rt - ty * a.ntx;
 
     const bool overflow = (a.status->bits & OSOG_WOVERFLOW) != 0u;
-    const uint32_t beg = a.offset[tile];
-    const uint32_t L = overflow ? 0u : a.offset[tile + 1] - beg;
+    const size_t beg = (size_t)tile * a.tile_cap;
+    const uint32_t L = overflow ? 0u : a.count[tile];
     const uint32_t* __restrict__ glist = a.list + beg;
     const uint16_t* __restrict__ gmeta = a.meta + beg;
 
@@ -515,15 +534,17 @@ cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float
 {
     (void)N;
     ComposeArgs a;
-    a.rec = c->rec; a.offset = c->offset; a.count = c->count; a.list = c->list; a.meta = c->meta; a.optics = c->optics;
+    a.rec = c->rec; a.count = c->count + (size_t)c->status_idx * c->max_tiles; a.list = c->list; a.meta = c->meta;
+    a.tile_cap = c->tile_cap; a.optics = c->optics;
     a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.status = c->status + c->status_idx;
     a.opd = d_opd; a.field = d_field;
     a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
     a.ramp_y_on = 1;
     const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
     if (sort_first) {
-        k_sort_cull<<<(grid + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(c->rec, c->offset, c->count, c->list, c->meta,
-                                                                                     a.status, c->ntx, c->nty, (int)grid);
+        k_sort_cull<<<(grid + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(
+            c->rec, a.count, c->count + (size_t)(c->status_idx ^ 1) * c->max_tiles, c->list, c->meta,
+            c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty, (int)grid);
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }

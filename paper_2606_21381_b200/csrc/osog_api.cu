@@ -1,6 +1,7 @@
 // C ABI of libosog (include/osog.h): context management, argument checks, launch sequencing.
 #include <new>
 #include <cstring>
+#include <vector>
 #include "osog_internal.cuh"
 
 using namespace osog;
@@ -166,7 +167,7 @@ int osog_destroy(osog_ctx* c)
     if (c->has_plan_one) cufftDestroy(c->plan_one);
     if (c->has_plan_batch) cufftDestroy(c->plan_batch);
     cudaFree(c->rec); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
-    cudaFree(c->offset); cudaFree(c->list); cudaFree(c->meta); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
+    cudaFree(c->list); cudaFree(c->meta); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
     cudaFree(c->status); cudaFree(c->field); cudaFree(c->work);
     if (c->h_status) cudaFreeHost(c->h_status);
     delete c;
@@ -198,6 +199,13 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     c->nty = (c->H + kTile - 1) / kTile;
     c->max_tiles = (long long)c->max_frames * c->ntx * c->nty;
     if (c->max_tiles > 0x7fffffffll) { delete c; return OSOG_EINVAL; }
+    // every tile owns a fixed slice of the pair list (no scan, no second fill pass): capacity per tile
+    {
+        long long cap = c->max_pairs / c->max_tiles;
+        if (cap < 1) cap = 1;
+        if (cap > 0x3fffffffll) cap = 0x3fffffffll;
+        c->tile_cap = (int)cap;
+    }
 
     DeviceGuard g(c->device);
     if (!g.ok) { delete c; return OSOG_ECUDA; }
@@ -207,10 +215,9 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     A(dalloc(&c->rec, np * kRecWords));
     A(dalloc(&c->tbox, np));
     A(dalloc(&c->pframe, np));
-    A(dalloc(&c->count, (size_t)c->max_tiles));
-    A(dalloc(&c->offset, (size_t)c->max_tiles + 1));
-    A(dalloc(&c->list, (size_t)c->max_pairs));
-    A(dalloc(&c->meta, (size_t)c->max_pairs));
+    A(dalloc(&c->count, 2 * (size_t)c->max_tiles));
+    A(dalloc(&c->list, (size_t)c->max_tiles * c->tile_cap));
+    A(dalloc(&c->meta, (size_t)c->max_tiles * c->tile_cap));
     A(dalloc(&c->ramp_x, (size_t)c->max_frames * c->W));
     A(dalloc(&c->ramp_y, (size_t)c->max_frames * c->H));
     A(dalloc(&c->optics, (size_t)c->max_frames));
@@ -218,8 +225,7 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     A(dalloc(&c->field, (size_t)c->max_frames * npx));
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&c->h_status), sizeof(DeviceStatus));
     if (e == cudaSuccess) e = cudaMemset(c->status, 0, 2 * sizeof(DeviceStatus));
-    if (e == cudaSuccess) e = cudaMemset(c->count, 0, sizeof(uint32_t) * (size_t)c->max_tiles);
-    if (e == cudaSuccess) e = cudaMemset(c->offset, 0, sizeof(uint32_t) * ((size_t)c->max_tiles + 1));
+    if (e == cudaSuccess) e = cudaMemset(c->count, 0, sizeof(uint32_t) * 2 * (size_t)c->max_tiles);
     if (e != cudaSuccess) {
         const bool oom = e == cudaErrorMemoryAllocation;
         cudaGetLastError();
@@ -253,7 +259,7 @@ static int render_common(osog_ctx* c, const osog_particles* p, int64_t N, const 
     c->last_N = N;
     e = launch_compose(c, N, o->B, has_ramp, d_opd, d_field);
     if (e != cudaSuccess) return cuda_fail(c, e);
-    c->scratch_dirty = false;                        // the compose kernel re-zeroes the tile counts it used
+    c->scratch_dirty = false;                        // k_sort_cull cleared the counter / status slots of the next call
     return OSOG_OK;
 }
 
@@ -355,9 +361,11 @@ int osog_status(osog_ctx* c, uint32_t* status_bits, int64_t* pairs)
     cudaError_t e = cudaMemcpyAsync(c->h_status, c->status + c->status_idx, sizeof(DeviceStatus), cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e);
+    const bool overflow = (c->h_status->bits & OSOG_WOVERFLOW) != 0u;
     if (status_bits) *status_bits = c->h_status->bits;
-    if (pairs) *pairs = (int64_t)c->h_status->pairs;
-    return (c->h_status->bits & OSOG_WOVERFLOW) ? OSOG_ECAPACITY : OSOG_OK;
+    // on overflow: the max_pairs that would have sufficed = longest tile list x tiles of the context
+    if (pairs) *pairs = overflow ? (int64_t)c->h_status->max_count * c->max_tiles : (int64_t)c->h_status->pairs;
+    return overflow ? OSOG_ECAPACITY : OSOG_OK;
 }
 
 int osog_debug_bins(osog_ctx* c, uint32_t* h_offset, uint32_t* h_list, int64_t cap, int64_t* n_tiles, int64_t* n_pairs)
@@ -369,14 +377,29 @@ int osog_debug_bins(osog_ctx* c, uint32_t* h_offset, uint32_t* h_list, int64_t c
     if (r == OSOG_ECUDA || r == OSOG_EINVAL) return r;
     if (n_tiles) *n_tiles = c->last_tiles;
     if (n_pairs) *n_pairs = pairs;
+    if (c->last_tiles <= 0 || (!h_offset && !h_list)) return r;
     DeviceGuard g(c->device);
-    cudaError_t e = cudaSuccess;
-    if (h_offset && c->last_tiles > 0)
-        e = cudaMemcpy(h_offset, c->offset, sizeof(uint32_t) * ((size_t)c->last_tiles + 1), cudaMemcpyDeviceToHost);
+    // host side: per-tile counts -> exclusive scan; the tiles' fixed-capacity slices -> one compact list
+    const size_t nt = (size_t)c->last_tiles;
+    std::vector<uint32_t> cnt(nt);
+    cudaError_t e = cudaMemcpy(cnt.data(), c->count + (size_t)c->status_idx * c->max_tiles, sizeof(uint32_t) * nt, cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return cuda_fail(c, e);
-    const int64_t ncopy = pairs < cap ? pairs : cap;
-    if (h_list && ncopy > 0 && r == OSOG_OK) e = cudaMemcpy(h_list, c->list, sizeof(uint32_t) * (size_t)ncopy, cudaMemcpyDeviceToHost);
-    if (e != cudaSuccess) return cuda_fail(c, e);
+    if (h_offset) {
+        unsigned long long run = 0;
+        for (size_t t = 0; t < nt; ++t) {
+            h_offset[t] = (uint32_t)(run < 0xffffffffull ? run : 0xffffffffull);
+            run += cnt[t];
+        }
+        h_offset[nt] = (uint32_t)(run < 0xffffffffull ? run : 0xffffffffull);
+    }
+    if (h_list && r == OSOG_OK && cap > 0) {
+        std::vector<uint32_t> all(nt * (size_t)c->tile_cap);
+        e = cudaMemcpy(all.data(), c->list, sizeof(uint32_t) * all.size(), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return cuda_fail(c, e);
+        int64_t k = 0;
+        for (size_t t = 0; t < nt && k < cap; ++t)
+            for (uint32_t q = 0; q < cnt[t] && k < cap; ++q) h_list[k++] = all[t * (size_t)c->tile_cap + q];
+    }
     return r;
 }
 

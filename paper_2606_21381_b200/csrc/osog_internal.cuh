@@ -21,10 +21,10 @@ constexpr uint32_t kFlagPrism = 1u;
 constexpr uint32_t kFlagAllF64 = 16u;
 // bits 8..10: number of steep slabs (they come first); bits 16..21: per-slab "vertical" (n_z == 0) mask
 
-// status word layout (device int32 [4]): [0] status bits, [1] unused, [2..3] pairs needed (uint64 split)
+// status of one render call (device): status bits, longest tile list, total number of (particle, tile) pairs
 struct DeviceStatus {
     uint32_t bits;
-    uint32_t pad;
+    uint32_t max_count;
     unsigned long long pairs;
 };
 
@@ -54,6 +54,7 @@ struct osog_ctx {
     long long max_particles, max_pairs;
     int ntx, nty;                   // tiles per row / column
     long long max_tiles;            // max_frames * ntx * nty
+    int tile_cap;                   // list entries one tile can hold: max(1, max_pairs / max_tiles)
     int last_cuda_error;
     // last call
     int last_B;
@@ -64,10 +65,10 @@ struct osog_ctx {
     float* rec;                     // [max_particles][kRecWords]
     int4* tbox;                     // [max_particles] tile range tx0, tx1, ty0, ty1 (tx0 > tx1: not listed)
     int* pframe;                    // [max_particles] frame of the particle
-    uint32_t* count;                // [max_tiles] per-tile count, reused as the fill cursor
-    uint32_t* offset;               // [max_tiles + 1]
-    uint32_t* list;                 // [max_pairs]
-    uint16_t* meta;                 // [max_pairs] per list entry: sub-tile mask | evaluation code << 8 (k_sort_cull)
+    uint32_t* count;                // [2][max_tiles] per-tile list length; slot status_idx belongs to the current call, the
+                                    // other slot is zeroed by that call's k_sort_cull for the next call
+    uint32_t* list;                 // [max_tiles][tile_cap] tile t's particle indices at list + t * tile_cap
+    uint16_t* meta;                 // [max_tiles][tile_cap] per list entry: sub-tile mask | evaluation code << 8 (k_sort_cull)
     float2* ramp_x;                 // [max_frames][W]  exp(i 2 pi fx0 x_j)
     float2* ramp_y;                 // [max_frames][H]
     osog::FrameOptics* optics;      // [max_frames]

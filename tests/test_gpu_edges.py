@@ -72,9 +72,17 @@ def test_pair_list_overflow_is_reported_and_frames_zeroed(og):
     assert r == og.OSOG_ECAPACITY and (bits & og.OSOG_WOVERFLOW) and pairs > 50
     assert float(opd.abs().max()) == 0.0
     ctx.close()
+    tiles = (sc.H // og.osog_tile_size()) * (sc.W // og.osog_tile_size())
+    assert pairs % tiles == 0                                # = longest tile list x tiles of the context
     ctx = og.Context(sc.H, sc.W, sc.N, max_pairs=pairs)      # the reported need is exactly enough
     ctx.render_opd(P, opt)
     assert ctx.status()[0] == 0
+    cnt = ctx.debug_bins()[0]
+    assert int(cnt.max()) * tiles == pairs and ctx.status()[2] == int(cnt.sum())
+    ctx.close()
+    ctx = og.Context(sc.H, sc.W, sc.N, max_pairs=pairs - tiles)   # one entry less per tile is not
+    ctx.render_opd(P, opt)
+    assert ctx.status()[0] == og.OSOG_ECAPACITY
     ctx.close()
 
 
@@ -146,7 +154,7 @@ def test_context_reuse_keeps_scratch_invariants(og, o):
     ref_small = fresh.render_opd(og.Particles.from_scene(small), og.optics_from_scene(small)).clone()
     ref_big = fresh.render_opd(og.Particles.from_scene(big), og.optics_from_scene(big)).clone()
     fresh.close()
-    ctx = og.Context(big.H, big.W, 400, max_pairs=3000)
+    ctx = og.Context(big.H, big.W, 400, max_pairs=40 * 1024)     # 40 entries per tile
     Pb, Ps = og.Particles.from_scene(big), og.Particles.from_scene(small)
     ob, os_ = og.optics_from_scene(big), og.optics_from_scene(small)
     ctx.render_opd_atomic(Pb, ob)
