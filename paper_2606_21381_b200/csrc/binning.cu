@@ -166,23 +166,27 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
         return;
     }
     // B3 / H4: tile range; append the particle to every tile of the range.  The atomic on the tile's counter returns the
-    // slot; up to 4 atomics of a tile row are in flight before their slots are used (one memory round trip per row).
+    // slot; up to 16 atomics are in flight before their slots are used (one memory round trip per 16 tiles).
     tb = make_int4(j0 / kTile, j1 / kTile, i0 / kTile, i1 / kTile);
     a.tbox[n] = tb;
     {
         const size_t t0 = (size_t)b * a.ntx * a.nty;
         const uint32_t cap = (uint32_t)a.tile_cap;
-        for (int ty = tb.z; ty <= tb.w; ++ty) {
-            for (int tx = tb.x; tx <= tb.y; tx += 4) {
-                const size_t t = t0 + (size_t)ty * a.ntx + tx;
-                uint32_t pos[4];
+        const int tw = tb.y - tb.x + 1, nt = tw * (tb.w - tb.z + 1);
+        int tx = tb.x, ty = tb.z;
+        uint32_t* cnt = a.count + t0;
+        uint32_t* lst = a.list + t0 * cap;
+        for (int q0 = 0; q0 < nt; q0 += 16) {
+            uint32_t t[16], pos[16];
 #pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    if (tx + q <= tb.y) pos[q] = atomicAdd(&a.count[t + q], 1u);
-#pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    if (tx + q <= tb.y && pos[q] < cap) a.list[(t + q) * cap + pos[q]] = (uint32_t)n;
+            for (int q = 0; q < 16; ++q) {
+                t[q] = (uint32_t)(ty * a.ntx + tx);
+                if (q0 + q < nt) pos[q] = atomicAdd(&cnt[t[q]], 1u);
+                if (++tx > tb.y) { tx = tb.x; ++ty; }
             }
+#pragma unroll
+            for (int q = 0; q < 16; ++q)
+                if (q0 + q < nt && pos[q] < cap) lst[(size_t)t[q] * cap + pos[q]] = (uint32_t)n;
         }
     }
 
