@@ -262,6 +262,12 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
 // global memory by the same warp (bitonic network, slow but correct).
 constexpr int kWarpSortCap = 1024;                 // list entries a warp sorts in shared memory (4 KB per warp)
 
+// r += (a < v): one compare and one predicated add
+__device__ __forceinline__ void count_less(uint32_t& r, uint32_t a, uint32_t v)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %1, %2;\n\t@p add.u32 %0, %0, 1;\n\t}" : "+r"(r) : "r"(a), "r"(v));
+}
+
 __device__ __forceinline__ uint32_t tile_meta(const float4 h0, const float4 h1, int tx, int ty)
 {
     uint32_t mask = 0;
@@ -345,12 +351,13 @@ __global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __re
             const uint32_t v = s[k];
             const float4* rec = recs4 + (size_t)v * (kRecWords / 4);
             const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);   // cxp, cyp, ax, ay | ha, hb, bbx, bby
-            uint32_t r = 0;
+            uint32_t r = 0, r1 = 0;                               // two chains of predicated adds
             const uint4* s4 = reinterpret_cast<const uint4*>(s);
             for (uint32_t m = 0; m < L4 / 4; ++m) {
                 const uint4 q = s4[m];
-                r += (q.x < v ? 1u : 0u) + (q.y < v ? 1u : 0u) + (q.z < v ? 1u : 0u) + (q.w < v ? 1u : 0u);
+                count_less(r, q.x, v); count_less(r1, q.y, v); count_less(r, q.z, v); count_less(r1, q.w, v);
             }
+            r += r1;
             glist[r] = v;                                        // the sorted segment (also what osog_debug_bins returns)
             meta[beg + r] = (uint16_t)tile_meta(h0, h1, tx, ty);
         }
