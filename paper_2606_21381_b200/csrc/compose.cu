@@ -29,7 +29,12 @@ struct ComposeArgs {
 
 constexpr int kWarps = kComposeThreads / 32;
 constexpr int kSlotStride4 = 9;                    // survivor slot stride in float4 (8 used, odd stride: conflict-free lane-per-slot writes)
-constexpr int kSmemSlots = kWarps * 32 * kSlotStride4 * 16;
+#ifndef OSOG_CTA_SPLIT
+#define OSOG_CTA_SPLIT 2
+#endif
+constexpr int kCtaSplit = OSOG_CTA_SPLIT;             // compose CTAs per tile (each takes kWarps / kCtaSplit sub-tiles)
+constexpr int kCtaWarps = kWarps / kCtaSplit;
+constexpr int kSmemSlots = kCtaWarps * 32 * kSlotStride4 * 16;
 constexpr int kSmemBytes = kSmemSlots;             // k_compose_tile: per-warp survivor slots only
 
 // ---- small PTX helpers ------------------------------------------------------------------------------------------------
@@ -372,14 +377,15 @@ __global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __re
 
 // ---- H5-H7: every warp is independent (no barrier, no shared list): it walks its tile's sorted list in batches of 32
 template <bool OPD, bool FIELD, bool RAMP>
-__global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const ComposeArgs a)
+__global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(const ComposeArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     float4* s_slots = reinterpret_cast<float4*>(smem);                            // per-warp survivor slots
 
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int wid = (tid >> 5) + kCtaWarps * (int)(blockIdx.x % kCtaSplit);     // sub-tile of the tile
     const int tpf = a.ntx * a.nty;
-    const int tile = blockIdx.x;
+    const int tile = blockIdx.x / kCtaSplit;
     const int b = tile / tpf, rt = tile - b * tpf;
     const int ty = rt / a.ntx, tx = rt - ty * a.ntx;
 
@@ -401,7 +407,7 @@ __global__ void __launch_bounds__(kComposeThreads, 4) k_compose_tile(const Compo
     g.nly = make_float2(-(float)ly, -(float)ly);
     g.xf = (float)j;
     g.yf = (float)i;
-    float4* my_slots = s_slots + wid * 32 * kSlotStride4;
+    float4* my_slots = s_slots + (tid >> 5) * 32 * kSlotStride4;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
 
     const float4* recs4 = reinterpret_cast<const float4*>(a.rec);
@@ -532,7 +538,7 @@ static cudaError_t launch_variant(const ComposeArgs& a, unsigned grid, cudaStrea
     cudaError_t e = cudaFuncSetAttribute(k_compose_tile<OPD, FIELD, RAMP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          kSmemBytes);
     if (e != cudaSuccess) return e;
-    k_compose_tile<OPD, FIELD, RAMP><<<grid, kComposeThreads, kSmemBytes, stream>>>(a);
+    k_compose_tile<OPD, FIELD, RAMP><<<grid * kCtaSplit, kCtaWarps * 32, kSmemBytes, stream>>>(a);
     return cudaGetLastError();
 }
 
