@@ -3,7 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
 
-One "step" = one pass of the whole hot path (H1-H7: prepare, bounding box + count, scan, fill, ordered tile
+One "step" = one pass of the whole hot path (H1-H7: prepare, bounding box + list append, per-tile sort + cull, ordered tile
 composition with the fused field write-out) over one seeded synthetic batch = one osog_render_field call.
 Default workload: BASELINE.json configs[3] (the paper-scale headline: 40,000 mixed particles, 2048 x 2048,
 NA 0.65, 10 degree oblique ramp).  Prints ONE JSON line (see DESIGN.md section 10 for every key).
@@ -327,8 +327,8 @@ def run_ours(args):
     k_bytes = 4 * pairs + 8 * B * H * W                 # k_compose_tile alone: list read + complex64 write
     achieved = k_bytes / (ms_compose * 1e-3) / 1e9
     hbm = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-           "traffic": 8953856, "traffic_note": "dram read+write of one k_compose_tile launch, ncu --set full "
-           "(profiles/r1_final_compose_ncu.md); the 33.5 MB field it writes stays in the 126 MB L2",
+           "traffic": 10553088, "traffic_note": "dram read+write of one k_compose_tile launch, ncu --set full "
+           "(profiles/r1_final3_compose_ncu.md); the 33.5 MB field it writes stays in the 126 MB L2",
            "peak_source": peak_src, "algorithmic_bytes": int(k_bytes), "kernel": "k_compose_tile",
            "kernel_ms": ms_compose, "frac_of_nominal_8TBs": achieved / 8000.0,
            "note": "BASELINE.json's '% of B200 HBM roofline'; the kernel is bound by instruction issue, see roofline"}
@@ -363,7 +363,7 @@ def run_ours(args):
         "gpu_launches": 3 * args.steps,
         "roofline": roof, "roofline_hbm": hbm,
         "roofline_step": {"achieved": step_gbs, "frac": step_gbs / peak, "algorithmic_bytes": int(alg_bytes),
-                          "what": "whole hot path: k_prepare, k_scan, k_fill, k_compose_tile"},
+                          "what": "whole hot path: k_prepare, k_sort_cull, k_compose_tile"},
         "library_stage_ms": ms_optics, "dic_stage_ms": ms_dic, "opd_only_ms": ms_opd, "atomic_alternative_opd_ms": ms_atomic,
         "paper_context": "PAPER.md:195: 40,000 particles < 50 ms on one A100 at 1024^2 (whole pipeline); context only",
         "clocks": clk.summary(),
