@@ -39,6 +39,126 @@ __device__ __forceinline__ float2 cis_turns(double t)
 
 constexpr int kPrepThreads = 128;
 
+// ---- binning role of k_prepare (H2 + H4): one particle per thread, list appends balanced over the warp -------------------
+// B1-B2 (fp64): half extents of the projection, inclusive pixel range padded by 2^-10 px, clamped to the frame; B3: tile
+// range.  H4: the (particle, tile) pairs of the warp's 32 particles are dealt out evenly to its lanes (prefix sum of the
+// tile counts + a binary search in shared memory), so that every lane has about the same number of list appends and
+// all of them are in flight at once: the atomic on the tile's counter returns the slot of the tile's slice.
+__device__ __forceinline__ void binning_role(const PrepArgs& a, long long n)
+{
+    __shared__ int s_pre[kPrepThreads / 32][33];
+    __shared__ int4 s_box[kPrepThreads / 32][32];      // tx0, tile columns, ty0, particle index
+    __shared__ uint32_t s_t0[kPrepThreads / 32][32];   // first tile of the particle's frame
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int4 tb = make_int4(1, 0, 1, 0);                 // empty tile range
+    int b = 0;
+    if (n < a.N) {
+        const float fcx = a.cx[n], fcy = a.cy[n], fqw = a.qw[n], fqx = a.qx[n], fqy = a.qy[n], fqz = a.qz[n];
+        const float fd0 = a.d0[n], fd1 = a.d1[n], fd2 = a.d2[n], fnp = a.n_p[n];
+        const unsigned kind = a.kind[n];
+        const bool valid = finite_f(fcx) && finite_f(fcy) && finite_f(fqw) && finite_f(fqx) && finite_f(fqy) && finite_f(fqz) &&
+                           finite_f(fd0) && finite_f(fd1) && finite_f(fd2) && finite_f(fnp) &&
+                           fd0 > 0.0f && fd1 > 0.0f && fd2 > 0.0f && kind <= 1u;
+        if (a.frame_start != nullptr) {              // largest b with frame_start[b] <= n
+            int lo = 0, hi = a.B;
+            while (hi - lo > 1) {
+                const int mid = (lo + hi) >> 1;
+                if ((long long)a.frame_start[mid] <= n) lo = mid; else hi = mid;
+            }
+            b = lo;
+        }
+        a.pframe[n] = b;
+        if (!valid) {
+            atomicOr(&a.status->bits, OSOG_WBADPARTICLE);
+        } else {
+            const double p = a.pitch;
+            const double cx = fcx, cy = fcy;
+            const double w = fqw, x = fqx, y = fqy, z = fqz;
+            // rows x and y of the Hamilton active rotation body -> world, no renormalisation (reading A4)
+            const double R00 = 1.0 - 2.0 * (y * y + z * z), R01 = 2.0 * (x * y - w * z), R02 = 2.0 * (x * z + w * y);
+            const double R10 = 2.0 * (x * y + w * z), R11 = 1.0 - 2.0 * (x * x + z * z), R12 = 2.0 * (y * z - w * x);
+            const double e0 = fd0, e1 = fd1, e2 = fd2;
+            // B1: half extents of the projection
+            double hx, hy;
+            if (kind == 0u) {
+                hx = sqrt(R00 * R00 * e0 * e0 + R01 * R01 * e1 * e1 + R02 * R02 * e2 * e2);
+                hy = sqrt(R10 * R10 * e0 * e0 + R11 * R11 * e1 * e1 + R12 * R12 * e2 * e2);
+            } else {
+                const double hs = 0.5 * e0, hl = 0.5 * e1, ap = 0.5 * e1 + e2;
+                hx = fabs(R02 * ap);
+                hy = fabs(R12 * ap);
+#pragma unroll
+                for (int v = 0; v < 4; ++v) {        // (+-s/2, +-s/2, +L/2); the -L/2 half mirrors it through the centre
+                    const double sx = (v & 1) ? -hs : hs, sy = (v & 2) ? -hs : hs;
+                    hx = fmax(hx, fabs(R00 * sx + R01 * sy + R02 * hl));
+                    hy = fmax(hy, fabs(R10 * sx + R11 * sy + R12 * hl));
+                }
+            }
+            // B2: inclusive pixel range, padded by 2^-10 px, clamped to the frame
+            const double fj0 = ceil((cx - hx) / p - 0.5 - kBBoxPadPx), fj1 = floor((cx + hx) / p - 0.5 + kBBoxPadPx);
+            const double fi0 = ceil((cy - hy) / p - 0.5 - kBBoxPadPx), fi1 = floor((cy + hy) / p - 0.5 + kBBoxPadPx);
+            const double big = 1073741824.0;
+            if (fabs(fj0) <= 1.7976931348623157e308 && fabs(fj1) <= 1.7976931348623157e308 &&
+                fabs(fi0) <= 1.7976931348623157e308 && fabs(fi1) <= 1.7976931348623157e308) {   // else: not listed (as the oracle)
+                const int j0 = max(0, min(a.W, (int)fmin(fmax(fj0, -big), big)));
+                const int j1 = max(-1, min(a.W - 1, (int)fmin(fmax(fj1, -big), big)));
+                const int i0 = max(0, min(a.H, (int)fmin(fmax(fi0, -big), big)));
+                const int i1 = max(-1, min(a.H - 1, (int)fmin(fmax(fi1, -big), big)));
+                if (j0 <= j1 && i0 <= i1) {
+                    tb = make_int4(j0 / kTile, j1 / kTile, i0 / kTile, i1 / kTile);      // B3
+                    // words 0, 1, 6, 7 of the record: centre in pixel-index coordinates and the packed pixel bounding box
+                    float* r32 = a.rec + (size_t)n * kRecWords;
+                    uint32_t* r32u = reinterpret_cast<uint32_t*>(r32);
+                    const double ip = 1.0 / p;
+                    r32[0] = (float)(cx * ip - 0.5);
+                    r32[1] = (float)(cy * ip - 0.5);
+                    r32u[6] = (uint32_t)j0 | ((uint32_t)j1 << 16);
+                    r32u[7] = (uint32_t)i0 | ((uint32_t)i1 << 16);
+                }
+            }
+        }
+        a.tbox[n] = tb;
+    }
+    // ---- H4: deal the warp's (particle, tile) pairs out to its lanes
+    const int tw = tb.y - tb.x + 1;
+    const int nt = tb.x > tb.y ? 0 : tw * (tb.w - tb.z + 1);
+    int incl = nt;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += v;
+    }
+    const int total = __shfl_sync(0xffffffffu, incl, 31);
+    s_pre[wid][lane] = incl - nt;
+    if (lane == 31) s_pre[wid][32] = total;
+    s_box[wid][lane] = make_int4(tb.x, tw, tb.z, (int)(uint32_t)n);
+    s_t0[wid][lane] = (uint32_t)((size_t)b * a.ntx * a.nty);
+    __syncwarp();
+    const uint32_t cap = (uint32_t)a.tile_cap;
+    for (int k0 = 0; k0 < total; k0 += 32 * 8) {
+        uint32_t t[8], pos[8], id[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int k = k0 + q * 32 + lane;
+            if (k < total) {
+                int s = 0;                                       // largest s with pre[s] <= k (lanes without tiles share the
+#pragma unroll                                                   // prefix of their successor and are never picked)
+                for (int step = 16; step > 0; step >>= 1)
+                    if (s_pre[wid][s + step] <= k) s += step;
+                const int4 bx = s_box[wid][s];
+                const int local = k - s_pre[wid][s];
+                const int dy = local / bx.y, dx = local - dy * bx.y;
+                t[q] = s_t0[wid][s] + (uint32_t)((bx.z + dy) * a.ntx + bx.x + dx);
+                id[q] = (uint32_t)bx.w;
+                pos[q] = atomicAdd(&a.count[t[q]], 1u);
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+            if (k0 + q * 32 + lane < total && pos[q] < cap) a.list[(size_t)t[q] * cap + pos[q]] = id[q];
+    }
+}
+
 // Grid layout (blocks of 128 threads): [0, nb) binning role, one particle per thread; [nb, 2 nb) record role, one
 // particle per thread, the block's 128 particles permuted so that prisms come first and ellipsoids last (warps are then
 // uniform in the code path they take, except one mixed warp per block); [2 nb, ...) ramp tables.  nb = ceil(N / 128).
@@ -92,32 +212,19 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
         __syncthreads();
         n += (int)s_perm[threadIdx.x] - (int)threadIdx.x;
     }
+    if (role == 0) {
+        binning_role(a, n);
+        return;
+    }
     if (n >= a.N) return;
     const float fcx = a.cx[n], fcy = a.cy[n], fqw = a.qw[n], fqx = a.qx[n], fqy = a.qy[n], fqz = a.qz[n];
     const float fd0 = a.d0[n], fd1 = a.d1[n], fd2 = a.d2[n], fnp = a.n_p[n];
     const unsigned kind = a.kind[n];
-    bool valid = finite_f(fcx) && finite_f(fcy) && finite_f(fqw) && finite_f(fqx) && finite_f(fqy) && finite_f(fqz) &&
+    const bool valid = finite_f(fcx) && finite_f(fcy) && finite_f(fqw) && finite_f(fqx) && finite_f(fqy) && finite_f(fqz) &&
                  finite_f(fd0) && finite_f(fd1) && finite_f(fd2) && finite_f(fnp) &&
                  fd0 > 0.0f && fd1 > 0.0f && fd2 > 0.0f && kind <= 1u;
 
-    int b = 0;
-    if (a.frame_start != nullptr) {              // largest b with frame_start[b] <= n
-        int lo = 0, hi = a.B;
-        while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if ((long long)a.frame_start[mid] <= n) lo = mid; else hi = mid;
-        }
-        b = lo;
-    }
-    int4 tb = make_int4(1, 0, 1, 0);             // empty tile range
-    if (role == 0) a.pframe[n] = b;
-    if (!valid) {
-        if (role == 0) {
-            atomicOr(&a.status->bits, OSOG_WBADPARTICLE);
-            a.tbox[n] = tb;
-        }
-        return;
-    }
+    if (!valid) return;                          // flagged by the binning role
 
     const double p = a.pitch;
     const double cx = fcx, cy = fcy;
@@ -131,73 +238,6 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
     float* r32 = a.rec + (size_t)n * kRecWords;
     uint32_t* r32u = reinterpret_cast<uint32_t*>(r32);
     const double ip = 1.0 / p;
-    if (role == 0) {
-    // B1: half extents of the projection
-    double hx, hy;
-    if (kind == 0u) {
-        hx = sqrt(R00 * R00 * e0 * e0 + R01 * R01 * e1 * e1 + R02 * R02 * e2 * e2);
-        hy = sqrt(R10 * R10 * e0 * e0 + R11 * R11 * e1 * e1 + R12 * R12 * e2 * e2);
-    } else {
-        const double hs = 0.5 * e0, hl = 0.5 * e1, ap = 0.5 * e1 + e2;
-        hx = fabs(R02 * ap);
-        hy = fabs(R12 * ap);
-#pragma unroll
-        for (int v = 0; v < 4; ++v) {            // (+-s/2, +-s/2, +L/2); the -L/2 half mirrors it through the centre
-            const double sx = (v & 1) ? -hs : hs, sy = (v & 2) ? -hs : hs;
-            hx = fmax(hx, fabs(R00 * sx + R01 * sy + R02 * hl));
-            hy = fmax(hy, fabs(R10 * sx + R11 * sy + R12 * hl));
-        }
-    }
-    // B2: inclusive pixel range, padded by 2^-10 px, clamped to the frame
-    const double fj0 = ceil((cx - hx) / p - 0.5 - kBBoxPadPx), fj1 = floor((cx + hx) / p - 0.5 + kBBoxPadPx);
-    const double fi0 = ceil((cy - hy) / p - 0.5 - kBBoxPadPx), fi1 = floor((cy + hy) / p - 0.5 + kBBoxPadPx);
-    const double big = 1073741824.0;
-    if (!(fabs(fj0) <= 1.7976931348623157e308 && fabs(fj1) <= 1.7976931348623157e308 &&
-          fabs(fi0) <= 1.7976931348623157e308 && fabs(fi1) <= 1.7976931348623157e308)) {
-        a.tbox[n] = tb;                          // non-finite bound: not listed (the oracle does the same)
-        return;
-    }
-    const int j0 = max(0, min(a.W, (int)fmin(fmax(fj0, -big), big)));
-    const int j1 = max(-1, min(a.W - 1, (int)fmin(fmax(fj1, -big), big)));
-    const int i0 = max(0, min(a.H, (int)fmin(fmax(fi0, -big), big)));
-    const int i1 = max(-1, min(a.H - 1, (int)fmin(fmax(fi1, -big), big)));
-    if (j0 > j1 || i0 > i1) {
-        a.tbox[n] = tb;
-        return;
-    }
-    // B3 / H4: tile range; append the particle to every tile of the range.  The atomic on the tile's counter returns the
-    // slot; up to 16 atomics are in flight before their slots are used (one memory round trip per 16 tiles).
-    tb = make_int4(j0 / kTile, j1 / kTile, i0 / kTile, i1 / kTile);
-    a.tbox[n] = tb;
-    {
-        const size_t t0 = (size_t)b * a.ntx * a.nty;
-        const uint32_t cap = (uint32_t)a.tile_cap;
-        const int tw = tb.y - tb.x + 1, nt = tw * (tb.w - tb.z + 1);
-        int tx = tb.x, ty = tb.z;
-        uint32_t* cnt = a.count + t0;
-        uint32_t* lst = a.list + t0 * cap;
-        for (int q0 = 0; q0 < nt; q0 += 16) {
-            uint32_t t[16], pos[16];
-#pragma unroll
-            for (int q = 0; q < 16; ++q) {
-                t[q] = (uint32_t)(ty * a.ntx + tx);
-                if (q0 + q < nt) pos[q] = atomicAdd(&cnt[t[q]], 1u);
-                if (++tx > tb.y) { tx = tb.x; ++ty; }
-            }
-#pragma unroll
-            for (int q = 0; q < 16; ++q)
-                if (q0 + q < nt && pos[q] < cap) lst[(size_t)t[q] * cap + pos[q]] = (uint32_t)n;
-        }
-    }
-
-    // words 0, 1, 6, 7 of the record: centre in pixel-index coordinates and the packed pixel bounding box
-    r32[0] = (float)(cx * ip - 0.5);
-    r32[1] = (float)(cy * ip - 0.5);
-    r32u[6] = (uint32_t)j0 | ((uint32_t)j1 << 16);
-    r32u[7] = (uint32_t)i0 | ((uint32_t)i1 << 16);
-    return;
-    }
-
     // ---- H1 (role 1): derived record.  Coordinates are pixel offsets from pixel (jc, ic): dx = p dj + ox ----
     const double jc = fmin(fmax(floor(cx * ip), -1.0e6), 1.0e6);      // reference pixel: any nearby pixel will do
     const double ic = fmin(fmax(floor(cy * ip), -1.0e6), 1.0e6);
