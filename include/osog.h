@@ -129,8 +129,10 @@ int osog_field_to_intensity(osog_ctx* ctx, const osog_optics* o, const float* d_
 /* DIC image (Eq. 5): d_dic is DEVICE float [B, H, W].  Runs the hot path into the context's own complex frame, then
  * the library stage: D = |U(r+ds) e^{i theta} - U(r-ds) e^{-i theta}|^2, cuFFT forward of D; the pupil function P
  * (circ and defocus of `o`) -> cuFFT inverse -> |h_obj|^2 -> cuFFT forward (the optical transfer function); product,
- * cuFFT inverse, real part, optional read noise (same generator as the intensity).  The first DIC call of a context
- * allocates one more complex frame batch (cudaMalloc, synchronous); later calls allocate nothing. */
+ * cuFFT inverse, real part, optional read noise (same generator as the intensity).  The transfer function depends on
+ * the optics alone: it is kept in the context and rebuilt only when B, pitch, n_medium, defocus, pupil_enabled, a
+ * wavelength or an NA differ from the previous DIC call.  The first DIC call of a context allocates two more complex
+ * frame batches (cudaMalloc, synchronous); later calls allocate nothing. */
 int osog_render_dic(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const osog_dic* dic,
                     float* d_dic);
 

@@ -118,23 +118,38 @@ int dic_stage(osog_ctx* c, const osog_optics* o, const osog_dic* d, float* d_dic
 {
     const int B = o->B;
     const double hw = (double)c->H * c->W;
-    if (!c->work) {                                  // first DIC call of this context: the second complex batch
-        cudaError_t ea = dalloc(&c->work, (size_t)c->max_frames * c->H * c->W);
-        if (ea != cudaSuccess) { cudaGetLastError(); c->work = nullptr; return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea); }
+    if (!c->work || !c->otf) {                       // first DIC call of this context: two more complex batches
+        for (float2** buf : {&c->work, &c->otf}) {
+            if (*buf) continue;
+            cudaError_t ea = dalloc(buf, (size_t)c->max_frames * c->H * c->W);
+            if (ea != cudaSuccess) { cudaGetLastError(); *buf = nullptr; return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea); }
+        }
     }
+    if (!c->otf_key) c->otf_key = new (std::nothrow) std::vector<double>();
+    if (!c->otf_key) return OSOG_ENOMEM;
     const bool defocus = o->defocus_um != 0.0;
     cudaError_t e;
     int r;
     // D = |U(r+ds) e^{i theta} - U(r-ds) e^{-i theta}|^2 and its spectrum
     if ((e = launch_dic_shear(c, B, c->field, c->work, d->shear_x_px, d->shear_y_px, d->bias_rad)) != cudaSuccess) return cuda_fail(c, e);
     if ((r = fft_frames(c, c->work, B, CUFFT_FORWARD)) != OSOG_OK) return r;
-    // optical transfer function: P -> h_obj = F^-1{P} -> |h_obj|^2 -> F{.}   (U is no longer needed: reuse its buffer)
-    if ((e = launch_pupil_fill(c, B, c->field, o->pitch_um, defocus)) != cudaSuccess) return cuda_fail(c, e);
-    if ((r = fft_frames(c, c->field, B, CUFFT_INVERSE)) != OSOG_OK) return r;
-    if ((e = launch_abs2(c, B, c->field, 1.0 / (hw * hw))) != cudaSuccess) return cuda_fail(c, e);      // cuFFT's inverse is unnormalised
-    if ((r = fft_frames(c, c->field, B, CUFFT_FORWARD)) != OSOG_OK) return r;
+    // optical transfer function: P -> h_obj = F^-1{P} -> |h_obj|^2 -> F{.}; it depends on the optics alone, so it is kept
+    // and rebuilt only when they change (the same stream orders the rebuild against earlier readers)
+    std::vector<double> key = {(double)B, o->pitch_um, o->n_medium, o->defocus_um, (double)(o->pupil_enabled != 0)};
+    for (int b = 0; b < B; ++b) {
+        key.push_back(o->lambda_um[b]);
+        key.push_back(o->pupil_enabled ? o->NA[b] : 0.0);
+    }
+    if (key != *c->otf_key) {
+        c->otf_key->clear();
+        if ((e = launch_pupil_fill(c, B, c->otf, o->pitch_um, defocus)) != cudaSuccess) return cuda_fail(c, e);
+        if ((r = fft_frames(c, c->otf, B, CUFFT_INVERSE)) != OSOG_OK) return r;
+        if ((e = launch_abs2(c, B, c->otf, 1.0 / (hw * hw))) != cudaSuccess) return cuda_fail(c, e);    // cuFFT's inverse is unnormalised
+        if ((r = fft_frames(c, c->otf, B, CUFFT_FORWARD)) != OSOG_OK) return r;
+        *c->otf_key = key;
+    }
     // I = F^-1{ F{D} OTF }
-    if ((e = launch_cmul(c, B, c->work, c->field, 1.0 / hw)) != cudaSuccess) return cuda_fail(c, e);
+    if ((e = launch_cmul(c, B, c->work, c->otf, 1.0 / hw)) != cudaSuccess) return cuda_fail(c, e);
     if ((r = fft_frames(c, c->work, B, CUFFT_INVERSE)) != OSOG_OK) return r;
     if ((e = launch_sensor_real(c, B, c->work, d_dic, o->read_noise_sigma, o->seed)) != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
@@ -168,7 +183,8 @@ int osog_destroy(osog_ctx* c)
     if (c->has_plan_batch) cufftDestroy(c->plan_batch);
     cudaFree(c->rec); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
     cudaFree(c->list); cudaFree(c->meta); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
-    cudaFree(c->status); cudaFree(c->field); cudaFree(c->work);
+    cudaFree(c->status); cudaFree(c->field); cudaFree(c->work); cudaFree(c->otf);
+    delete c->otf_key;
     if (c->h_status) cudaFreeHost(c->h_status);
     delete c;
     return OSOG_OK;

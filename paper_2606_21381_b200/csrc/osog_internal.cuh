@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <cufft.h>
 #include <stdint.h>
+#include <vector>
 #include "../../include/osog.h"
 
 namespace osog {
@@ -77,6 +78,8 @@ struct osog_ctx {
     bool scratch_dirty;             // a call failed midway: count / status must be cleared explicitly
     float2* field;                  // [max_frames][H][W] (intensity path)
     float2* work;                   // [max_frames][H][W] second complex batch (DIC path; allocated by the first DIC call)
+    float2* otf;                    // [max_frames][H][W] optical transfer function F{|F^-1{P}|^2} of the last DIC call
+    std::vector<double>* otf_key;   // optics the cached OTF was built for (B, pitch, n_medium, defocus, pupil, lambda[], NA[])
     osog::DeviceStatus* h_status;   // pinned host mirror
     cufftHandle plan_one, plan_batch;
     bool has_plan_one, has_plan_batch;

@@ -174,3 +174,25 @@ def test_dic_argument_errors(og):
     ctx.render_dic(P, opt, og.make_dic(63, -63, 0.1))             # the largest allowed shear is fine
     assert ctx.status()[0] == 0
     ctx.close()
+
+
+def test_cached_transfer_function_follows_the_optics(og, o, fields):
+    """The OTF is kept between DIC calls and rebuilt only when the optics change: same optics twice -> same bits; a new
+    NA, wavelength-independent defocus or pupil switch on the same context -> still the oracle's image."""
+    import torch
+    sc0, U = fields(1)
+    ctx = og.Context(sc0.H, sc0.W, sc0.N)
+    P = og.Particles.from_scene(sc0)
+    dic = og.make_dic(2, 1, 0.5)
+    first = ctx.render_dic(P, og.optics_from_scene(sc0), dic).clone()
+    assert torch.equal(ctx.render_dic(P, og.optics_from_scene(sc0), dic), first)
+    for change in (dict(NA=np.array([0.7])), dict(defocus_um=2.5), dict(lambda_um=np.array([0.48])), dict()):
+        sc = replace(sc0, **change)
+        Uc = o.render_field(sc) if "lambda_um" in change else U
+        ref = o.render_dic(sc, (2, 1), 0.5, U=Uc)
+        g = ctx.render_dic(P, og.optics_from_scene(sc), dic).cpu().numpy().astype(np.float64)
+        assert np.abs(g - ref).max() <= 1e-4 * ref.mean(), change
+    ref = o.render_dic(sc0, (2, 1), 0.5, U=U, pupil_enabled=False)
+    g = ctx.render_dic(P, og.optics_from_scene(sc0, pupil_enabled=False), dic).cpu().numpy().astype(np.float64)
+    assert np.abs(g - ref).max() <= 1e-4 * ref.mean()
+    ctx.close()
