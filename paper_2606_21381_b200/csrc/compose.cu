@@ -1,12 +1,15 @@
-// H5-H7 of DESIGN.md: per-tile ordered composition.  One CTA per 32 x 32 pixel tile:
-//   1. sort the tile's particle list ascending (deterministic summation order) and write it back,
-//   2. (from then on every warp is independent: no barrier) walk the list in batches of 32 particles,
-//   3. per warp (16 x 8 pixel sub-tile, 4 x 1 pixels per lane): one lane per staged particle tests the particle's
-//      pixel bounding box and oriented box against the sub-tile (ballot compaction keeps ascending order) and
-//      re-bases the survivor's fp64 coefficients to the sub-tile origin, rounding them to fp32 only there,
-//   4. all lanes walk the survivors (grouped by evaluation class, one branch-free loop per class): ray-convex thickness from the re-based coefficients (packed fp32 FMA and
-//      3-input min/max for the prism slabs, fp64 quadratic + fp32 sqrt for the ellipsoid), OPD accumulated per
-//      pixel in fp64 registers,
+// H4 (second half) - H7 of DESIGN.md: per-tile ordered composition, two kernels.
+// k_sort_cull, one warp per 32 x 32 pixel tile:
+//   1. sort the tile's particle list ascending (deterministic summation order), in place,
+//   2. per list entry, test the particle's pixel bounding box and oriented box against the tile's eight 16 x 8 pixel
+//      sub-tiles: 8-bit mask + evaluation code of the record -> meta.
+// k_compose_tile, two CTAs of four warps per tile, every warp independent (no barrier, no shared list):
+//   3. per warp (one sub-tile, 4 x 1 pixels per lane): walk the sorted list in batches of 32 entries, keep those whose
+//      mask bit is set (ballot compaction keeps ascending order inside an evaluation class), re-base the survivors'
+//      fp64 coefficients to the sub-tile origin, rounding them to fp32 only there,
+//   4. all lanes walk the survivors (grouped by evaluation class, one branch-free loop per class): ray-convex thickness
+//      from the re-based coefficients (packed fp32 FMA and 3-input min/max for the prism slabs, fp64 quadratic + fp32
+//      sqrt for the ellipsoid), OPD accumulated per pixel in fp64 registers,
 //   5. write OPD and / or exp(i 2 pi OPD / lambda) * ramp straight from the registers.
 #include "osog_internal.cuh"
 
