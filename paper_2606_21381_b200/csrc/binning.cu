@@ -431,9 +431,11 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     if (c->scratch_dirty) {
         if ((e = cudaMemsetAsync(c->count, 0, sizeof(uint32_t) * 2 * (size_t)c->max_tiles, c->stream)) != cudaSuccess) return e;
         if ((e = cudaMemsetAsync(c->status, 0, 2 * sizeof(DeviceStatus), c->stream)) != cudaSuccess) return e;
+        c->slot_tiles[0] = c->slot_tiles[1] = 0;
     }
     c->scratch_dirty = true;
     c->status_idx ^= 1;
+    c->slot_tiles[c->status_idx] = tiles;
     DeviceStatus* status = c->status + c->status_idx;
 
     PrepArgs a;

@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __re
                                                              uint32_t* __restrict__ count_next, uint32_t* __restrict__ list,
                                                              uint16_t* __restrict__ meta, DeviceStatus* __restrict__ status,
                                                              DeviceStatus* __restrict__ status_next, int tile_cap,
-                                                             int ntx, int nty, int n_tiles)
+                                                             int ntx, int nty, int n_tiles, int n_clear)
 {
     __shared__ __align__(16) uint32_t s_all[kWarps * kWarpSortCap];
     __shared__ uint32_t s_len[kWarps];
@@ -328,7 +328,7 @@ __global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __re
     // list length of the tile; the other counter slot is cleared for the next call; the call's totals (number of pairs,
     // longest list, overflow of the per-tile capacity) are reduced per CTA
     const uint32_t Lraw = tile < n_tiles ? count[tile] : 0u;
-    if (tile < n_tiles && lane == 0) count_next[tile] = 0u;
+    if (tile < n_clear && lane == 0) count_next[tile] = 0u;    // every counter the other slot's last user touched
     if (lane == 0) s_len[wid] = Lraw;
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -558,9 +558,12 @@ cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float
     a.ramp_y_on = 1;
     const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
     if (sort_first) {
-        k_sort_cull<<<(grid + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(
+        const long long n_clear = c->slot_tiles[c->status_idx ^ 1];
+        const unsigned cover = (unsigned)(n_clear > (long long)grid ? n_clear : (long long)grid);
+        k_sort_cull<<<(cover + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(
             c->rec, a.count, c->count + (size_t)(c->status_idx ^ 1) * c->max_tiles, c->list, c->meta,
-            c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty, (int)grid);
+            c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty, (int)grid, (int)n_clear);
+        c->slot_tiles[c->status_idx ^ 1] = 0;
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }

@@ -75,6 +75,7 @@ struct osog_ctx {
     osog::FrameOptics* optics;      // [max_frames]
     osog::DeviceStatus* status;     // [2]: slot of the current call / slot being reset for the next call
     int status_idx;                 // slot used by the last render call
+    long long slot_tiles[2];        // tiles whose counters a slot's last user may have left non-zero
     bool scratch_dirty;             // a call failed midway: count / status must be cleared explicitly
     float2* field;                  // [max_frames][H][W] (intensity path)
     float2* work;                   // [max_frames][H][W] second complex batch (DIC path; allocated by the first DIC call)

@@ -173,3 +173,21 @@ def test_context_reuse_keeps_scratch_invariants(og, o):
     assert np.array_equal(off, oo) and np.array_equal(lst, ol)
     assert torch.equal(ctx.render_opd(Ps, os_), ref_small)
     ctx.close()
+
+
+def test_context_reuse_with_changing_batch_size(og):
+    """The per-tile counters are double-buffered and each call clears the other slot for the next one: a small batch
+    between two large ones must not leave stale counts in the tiles it did not use (same bits as fresh contexts)."""
+    import torch
+    H = W = 160
+    scenes = [make_scene(f"b{B}", H, W, _mixed(30 * B, H, W, seed=100 + B), frame_start=[30 * k for k in range(B + 1)],
+                         lam=np.full(B, 0.55), NA=np.full(B, 0.5)) for B in (4, 1, 3, 4, 2, 4)]
+    ctx = og.Context(H, W, 120, max_frames=4)
+    for sc in scenes:
+        fresh = og.Context(H, W, 120, max_frames=4)
+        want = fresh.render_opd(og.Particles.from_scene(sc), og.optics_from_scene(sc)).clone()
+        fresh.close()
+        got = ctx.render_opd(og.Particles.from_scene(sc), og.optics_from_scene(sc))
+        assert ctx.status()[0] == 0
+        assert torch.equal(got, want), sc.name
+    ctx.close()
