@@ -304,6 +304,13 @@ def run_ours(args):
     e1.record(stream)
     torch.cuda.synchronize()
     ms_atomic = e0.elapsed_time(e1) / 3
+    ctx.render_opd_smem_atomic(P, opt, out=inten)
+    e0.record(stream)
+    for _ in range(3):
+        ctx.render_opd_smem_atomic(P, opt, out=inten)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_smem_atomic = e0.elapsed_time(e1) / 3
 
     # ---- the dominant kernel alone (k_compose_tile on the binning of the last call), CUDA events on its stream
     ctx.render_field(P, opt, out=field)
@@ -364,7 +371,7 @@ def run_ours(args):
         "roofline": roof, "roofline_hbm": hbm,
         "roofline_step": {"achieved": step_gbs, "frac": step_gbs / peak, "algorithmic_bytes": int(alg_bytes),
                           "what": "whole hot path: k_prepare, k_sort_cull, k_compose_tile"},
-        "library_stage_ms": ms_optics, "dic_stage_ms": ms_dic, "opd_only_ms": ms_opd, "atomic_alternative_opd_ms": ms_atomic,
+        "library_stage_ms": ms_optics, "dic_stage_ms": ms_dic, "opd_only_ms": ms_opd, "atomic_alternative_opd_ms": ms_atomic, "smem_atomic_alternative_opd_ms": ms_smem_atomic,
         "paper_context": "PAPER.md:195: 40,000 particles < 50 ms on one A100 at 1024^2 (whole pipeline); context only",
         "clocks": clk.summary(),
     }

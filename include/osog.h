@@ -143,6 +143,11 @@ int osog_field_to_dic(osog_ctx* ctx, const osog_optics* o, const osog_dic* dic, 
  * per particle, global atomicAdd into d_opd.  NOT deterministic in the last bits; kept for comparison only. */
 int osog_render_opd_atomic(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd);
 
+/* Second measured alternative: the same tile lists, but one CTA per tile accumulates the tile in SHARED memory with fp32
+ * atomics (one warp per listed particle) and writes it out once.  NOT deterministic in the last bits, fp32 sum; kept for
+ * comparison with the ordered register accumulation only. */
+int osog_render_opd_smem_atomic(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd);
+
 int osog_destroy(osog_ctx* ctx);
 
 /* Synchronises the stream.  *status_bits = OSOG_W* bits of the last render call, *pairs = number of

@@ -66,7 +66,8 @@ def lib():
     L = C.CDLL(path)
     ctx = C.c_void_p
     L.osog_create.argtypes = [C.POINTER(ctx), C.POINTER(osog_config)]
-    for name in ("osog_render_opd", "osog_render_field", "osog_render_intensity", "osog_render_opd_atomic"):
+    for name in ("osog_render_opd", "osog_render_field", "osog_render_intensity", "osog_render_opd_atomic",
+                 "osog_render_opd_smem_atomic"):
         getattr(L, name).argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p]
     L.osog_field_to_intensity.argtypes = [ctx, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_dic.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics),
@@ -88,7 +89,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_debug_recompose_field", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_debug_recompose_field", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -214,6 +215,9 @@ class Context:
 
     def render_opd_atomic(self, p: Particles, o, out=None):
         return self._call("osog_render_opd_atomic", p, o, self._out(o.B, out=out))
+
+    def render_opd_smem_atomic(self, p: Particles, o, out=None):
+        return self._call("osog_render_opd_smem_atomic", p, o, self._out(o.B, out=out))
 
     def render_field(self, p: Particles, o, out=None):
         """complex64 [B, H, W] exit wave (osog_render_field); `out` is a float32 [B, H, W, 2] buffer."""

@@ -611,6 +611,76 @@ __global__ void __launch_bounds__(256) k_compose_atomic(const float* __restrict_
     }
 }
 
+// ---- measured alternative: tile lists + shared-memory atomics (north_star's "accumulate in shared memory") -------------
+// One CTA per 32 x 32 tile keeps the tile's OPD in shared memory; one warp per listed particle walks the part of the
+// particle's pixel bounding box that lies in the tile and atomicAdd's (n_p - n_m) t into it (fp64 thickness per pixel, fp32
+// shared-memory atomics).  The order in which the warps reach a pixel depends on scheduling: NOT deterministic in the last
+// bits, and the sum is fp32.  Kept to be measured against the ordered register accumulation of k_compose_tile.
+__global__ void __launch_bounds__(kComposeThreads) k_compose_smem_atomic(const float* __restrict__ recs, const uint32_t* __restrict__ count,
+                                                                       const uint32_t* __restrict__ list, int tile_cap,
+                                                                       const DeviceStatus* __restrict__ status, int ntx, int nty,
+                                                                       int H, int W, float* __restrict__ opd)
+{
+    __shared__ float s_acc[kTile * kTile];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int tile = blockIdx.x, tpf = ntx * nty;
+    const int b = tile / tpf, rt = tile - b * tpf;
+    const int ty = rt / ntx, tx = rt - ty * ntx;
+    const int x0 = tx * kTile, y0 = ty * kTile;
+    for (int k = tid; k < kTile * kTile; k += kComposeThreads) s_acc[k] = 0.0f;
+    __syncthreads();
+    const uint32_t L = (status->bits & OSOG_WOVERFLOW) ? 0u : count[tile];
+    const uint32_t* glist = list + (size_t)tile * tile_cap;
+    for (uint32_t k = wid; k < L; k += kWarps) {
+        const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)glist[k] * kRecWords);
+        const float4 h1 = __ldg(rec + 1), h2 = __ldg(rec + 2);
+        const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));
+        const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
+        const int j0 = max((int)(bx & 0xffff), x0), j1 = min((int)(bx >> 16), x0 + kTile - 1);
+        const int i0 = max((int)(by & 0xffff), y0), i1 = min((int)(by >> 16), y0 + kTile - 1);
+        const uint32_t flags = __float_as_uint(h2.x);
+        const double* c = reinterpret_cast<const double*>(rec + 4);
+        const double K = (double)h2.y;
+        const int bw = j1 - j0 + 1, np = bw * (i1 - i0 + 1);
+        for (int q = lane; q < np; q += 32) {
+            const int i = i0 + q / bw, j = j0 + q % bw;
+            const double dj = (double)(j - h3.x), di = (double)(i - h3.y);
+            double v;
+            if (flags & kFlagPrism) {
+                v = K * prism_t64(c, flags >> 16, dj, di);
+            } else {
+                const double w = c[5] - fma(fma(c[0], dj, fma(c[1], di, c[3])), dj, fma(c[2], di, c[4]) * di);
+                v = K * (double)fast_sqrt(fmaxf((float)w, 0.0f));
+            }
+            const float f = (float)v;
+            if (f != 0.0f) atomicAdd(&s_acc[(i - y0) * kTile + (j - x0)], f);
+        }
+    }
+    __syncthreads();
+    for (int k = tid; k < kTile * kTile; k += kComposeThreads) {
+        const int i = y0 + k / kTile, j = x0 + k % kTile;
+        if (i < H && j < W) opd[((size_t)b * H + i) * W + j] = s_acc[k];
+    }
+}
+
+// runs k_sort_cull first (it keeps the counter / status invariants; the order it establishes is not used here)
+cudaError_t launch_compose_smem_atomic(osog_ctx* c, int B, float* d_opd)
+{
+    const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
+    const uint32_t* count = c->count + (size_t)c->status_idx * c->max_tiles;
+    const long long n_clear = c->slot_tiles[c->status_idx ^ 1];
+    const unsigned cover = (unsigned)(n_clear > (long long)grid ? n_clear : (long long)grid);
+    k_sort_cull<<<(cover + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(
+        c->rec, count, c->count + (size_t)(c->status_idx ^ 1) * c->max_tiles, c->list, c->meta,
+        c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty, (int)grid, (int)n_clear);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    c->slot_tiles[c->status_idx ^ 1] = 0;
+    k_compose_smem_atomic<<<grid, kComposeThreads, 0, c->stream>>>(c->rec, count, c->list, c->tile_cap, c->status + c->status_idx,
+                                                                  c->ntx, c->nty, c->H, c->W, d_opd);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd)
 {
     cudaError_t e = cudaMemsetAsync(d_opd, 0, sizeof(float) * (size_t)B * c->H * c->W, c->stream);

@@ -361,6 +361,20 @@ int osog_render_opd_atomic(osog_ctx* c, const osog_particles* p, int64_t N, cons
     return OSOG_OK;
 }
 
+int osog_render_opd_smem_atomic(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd)
+{
+    const int r = check_call(c, p, N, o, d_opd);
+    if (r != OSOG_OK) return r;
+    DeviceGuard g(c->device);
+    cudaError_t e = launch_binning(c, p, N, o);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->last_has_ramp = -1;                           // no field-capable composition ran: osog_debug_recompose_field refuses
+    e = launch_compose_smem_atomic(c, o->B, d_opd);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->scratch_dirty = false;
+    return OSOG_OK;
+}
+
 int osog_debug_recompose_field(osog_ctx* c, float* d_field)
 {
     if (!c || !d_field || !aligned16(d_field) || c->last_B < 1 || c->last_has_ramp < 0) return OSOG_EINVAL;

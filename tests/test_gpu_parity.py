@@ -96,6 +96,23 @@ def test_atomic_alternative_within_tolerance(og, o):
     ctx.close()
 
 
+def test_smem_atomic_alternative_within_tolerance(og, o):
+    """Shared-memory-atomic variant (fp32 sum, scheduling-dependent order): inside the OPD bar on configs 2 and 5, and
+    the context is clean afterwards (the ordered path gives the same bits as on a fresh context)."""
+    import torch
+    for k in (2, 5):
+        sc = make_config(k)
+        ctx = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B)
+        P, opt = og.Particles.from_scene(sc), og.optics_from_scene(sc)
+        want = ctx.render_opd(P, opt).clone()
+        g = ctx.render_opd_smem_atomic(P, opt).cpu().numpy().astype(np.float64)
+        assert ctx.status()[0] == 0
+        ref = o.render_opd(sc)
+        assert np.all(np.abs(g - ref) <= 1e-5 + 1e-5 * np.abs(ref))
+        assert torch.equal(ctx.render_opd(P, opt), want)
+        ctx.close()
+
+
 def test_recompose_reproduces_the_field_bitwise(og):
     """osog_debug_recompose_field (the kernel bench.py times alone) gives the same bits as the full call."""
     import torch
