@@ -164,6 +164,7 @@ __device__ __forceinline__ void binning_role(const PrepArgs& a, long long n)
 // uniform in the code path they take, except one mixed warp per block); [2 nb, ...) ramp tables.  nb = ceil(N / 128).
 __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
 {
+    pdl_trigger();                               // k_sort_cull's CTAs may become resident (they wait for this grid to finish)
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long nb = (a.N + kPrepThreads - 1) / kPrepThreads;
 

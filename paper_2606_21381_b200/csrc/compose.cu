@@ -320,6 +320,8 @@ __global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __re
 {
     __shared__ __align__(16) uint32_t s_all[kWarps * kWarpSortCap];
     __shared__ uint32_t s_len[kWarps];
+    pdl_trigger();                                               // k_compose_tile's CTAs may become resident
+    pdl_wait();                                                  // k_prepare has finished, its lists and records are visible
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int tile = blockIdx.x * kWarps + wid;
     if (blockIdx.x == 0 && threadIdx.x == 0) {                   // the other status slot belongs to the next call
@@ -391,6 +393,7 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
     const int tile = blockIdx.x / kCtaSplit;
     const int b = tile / tpf, rt = tile - b * tpf;
     const int ty = rt / a.ntx, tx = rt - ty * a.ntx;
+    pdl_wait();                                                  // k_sort_cull (and all before it) has finished
 
     const bool overflow = (a.status->bits & OSOG_WOVERFLOW) != 0u;
     const size_t beg = (size_t)tile * a.tile_cap;
@@ -541,8 +544,7 @@ static cudaError_t launch_variant(const ComposeArgs& a, unsigned grid, cudaStrea
     cudaError_t e = cudaFuncSetAttribute(k_compose_tile<OPD, FIELD, RAMP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          kSmemBytes);
     if (e != cudaSuccess) return e;
-    k_compose_tile<OPD, FIELD, RAMP><<<grid * kCtaSplit, kCtaWarps * 32, kSmemBytes, stream>>>(a);
-    return cudaGetLastError();
+    return launch_pdl(k_compose_tile<OPD, FIELD, RAMP>, dim3(grid * kCtaSplit), dim3(kCtaWarps * 32), (size_t)kSmemBytes, stream, a);
 }
 
 // sort_first = false: the lists of the last call are already sorted and culled (osog_debug_recompose_field)
@@ -560,11 +562,11 @@ cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float
     if (sort_first) {
         const long long n_clear = c->slot_tiles[c->status_idx ^ 1];
         const unsigned cover = (unsigned)(n_clear > (long long)grid ? n_clear : (long long)grid);
-        k_sort_cull<<<(cover + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(
-            c->rec, a.count, c->count + (size_t)(c->status_idx ^ 1) * c->max_tiles, c->list, c->meta,
-            c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty, (int)grid, (int)n_clear);
+        const cudaError_t e = launch_pdl(k_sort_cull, dim3((cover + kWarps - 1) / kWarps), dim3(kComposeThreads), 0, c->stream,
+                                         c->rec, a.count, c->count + (size_t)(c->status_idx ^ 1) * c->max_tiles, c->list, c->meta,
+                                         c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty,
+                                         (int)grid, (int)n_clear);
         c->slot_tiles[c->status_idx ^ 1] = 0;
-        const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
     if (d_opd != nullptr && d_field == nullptr) return launch_variant<true, false, false>(a, grid, c->stream);

@@ -88,6 +88,28 @@ struct osog_ctx {
 
 namespace osog {
 
+// ---- programmatic dependent launch (sm_90+): a kernel launched with launch_pdl may start while its predecessor in the
+// stream is still running; it must call pdl_wait() before it touches anything the predecessor reads or writes.  A kernel
+// calls pdl_trigger() once it no longer minds its successor's CTAs becoming resident (they then block in pdl_wait()).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <class... KArgs, class... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // binning.cu
 cudaError_t upload_optics(osog_ctx* c, const osog_optics* o, OpticsChunk* first);
 cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o);
