@@ -260,15 +260,19 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
     }
 }
 
-// ---- H4 (second half) + tile-level cull: one WARP per tile ------------------------------------------------------------
+// ---- H4 (second half) + tile-level cull: two WARPS per tile ------------------------------------------------------------
 // Sorts the tile's list ascending in place (the canonical, deterministic summation order) and writes one 16-bit word
 // per list entry: bits 0..7 = which of the tile's 8 warp sub-tiles (16 x 8 pixels) the particle can touch (bounding
 // box + oriented-box test), bits 8..10 = the evaluation code of the record.  k_compose_tile then needs no barrier.
-// Rank sort (ids are unique inside a tile): the list is staged in the warp's shared-memory slice, every lane counts
+// Rank sort (ids are unique inside a tile): the list is staged in the tile's shared-memory slice, every lane counts
 // the ids smaller than its own with broadcast 128-bit reads; the record header loads of the cull are issued first so
 // that their latency hides behind the counting.  Lists longer than kWarpSortCap (pathological crowding) are sorted in
 // global memory by the same warp (bitonic network, slow but correct).
-constexpr int kWarpSortCap = 1024;                 // list entries a warp sorts in shared memory (4 KB per warp)
+constexpr int kWarpSortCap = 1024;                 // list entries sorted in shared memory (4 KB per tile)
+#ifndef OSOG_SORT_WARPS
+#define OSOG_SORT_WARPS 2
+#endif
+constexpr int kSortWarps = OSOG_SORT_WARPS;        // warps that share one tile in k_sort_cull (power of two <= kWarps)
 
 // r += (a < v): one compare and one predicated add
 __device__ __forceinline__ void count_less(uint32_t& r, uint32_t a, uint32_t v)
@@ -318,20 +322,22 @@ __global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __re
                                                              DeviceStatus* __restrict__ status_next, int tile_cap,
                                                              int ntx, int nty, int n_tiles, int n_clear)
 {
-    __shared__ __align__(16) uint32_t s_all[kWarps * kWarpSortCap];
+    __shared__ __align__(16) uint32_t s_all[(kWarps / kSortWarps) * kWarpSortCap];
     __shared__ uint32_t s_len[kWarps];
     pdl_trigger();                                               // k_compose_tile's CTAs may become resident
     pdl_wait();                                                  // k_prepare has finished, its lists and records are visible
+    // kSortWarps warps per tile: they stage the list together in one shared slice, each ranks / culls every kSortWarps-th group of 32 entries
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int tile = blockIdx.x * kWarps + wid;
+    const int half = wid % kSortWarps;                           // this warp's part of the tile's work
+    const int tile = (blockIdx.x * kWarps + wid) / kSortWarps;
     if (blockIdx.x == 0 && threadIdx.x == 0) {                   // the other status slot belongs to the next call
         status_next->bits = 0u; status_next->max_count = 0u; status_next->pairs = 0ull;
     }
     // list length of the tile; the other counter slot is cleared for the next call; the call's totals (number of pairs,
     // longest list, overflow of the per-tile capacity) are reduced per CTA
     const uint32_t Lraw = tile < n_tiles ? count[tile] : 0u;
-    if (tile < n_clear && lane == 0) count_next[tile] = 0u;    // every counter the other slot's last user touched
-    if (lane == 0) s_len[wid] = Lraw;
+    if (tile < n_clear && lane == 0 && half == 0) count_next[tile] = 0u;    // every counter the other slot's last user touched
+    if (lane == 0) s_len[wid] = half == 0 ? Lraw : 0u;
     __syncthreads();
     if (threadIdx.x == 0) {
         uint32_t mx = 0;
@@ -353,11 +359,11 @@ __global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __re
     const int ty = rt / ntx, tx = rt - ty * ntx;
     const float4* recs4 = reinterpret_cast<const float4*>(recs);
     if (L <= (uint32_t)kWarpSortCap) {
-        uint32_t* s = s_all + wid * kWarpSortCap;
+        uint32_t* s = s_all + (wid / kSortWarps) * kWarpSortCap; // the tile's warps share one slice
         const uint32_t L4 = (L + 3u) & ~3u;
-        for (uint32_t k = lane; k < L4; k += 32) s[k] = k < L ? glist[k] : 0xffffffffu;
-        __syncwarp();
-        for (uint32_t k = lane; k < L; k += 32) {
+        for (uint32_t k = lane + 32 * half; k < L4; k += 32 * kSortWarps) s[k] = k < L ? glist[k] : 0xffffffffu;
+        asm volatile("bar.sync %0, %1;" ::"r"(1 + wid / kSortWarps), "n"(32 * kSortWarps) : "memory");   // tile barrier: the list is staged, glist may be overwritten
+        for (uint32_t k = lane + 32 * half; k < L; k += 32 * kSortWarps) {
             const uint32_t v = s[k];
             const float4* rec = recs4 + (size_t)v * (kRecWords / 4);
             const float4 h0 = __ldg(rec), h1 = __ldg(rec + 1);   // cxp, cyp, ax, ay | ha, hb, bbx, bby
@@ -371,7 +377,7 @@ __global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __re
             glist[r] = v;                                        // the sorted segment (also what osog_debug_bins returns)
             meta[beg + r] = (uint16_t)tile_meta(h0, h1, tx, ty);
         }
-    } else {
+    } else if (half == 0) {
         sort_global_warp(glist, L, lane);
         for (uint32_t k = lane; k < L; k += 32) {
             const float4* rec = recs4 + (size_t)glist[k] * (kRecWords / 4);
@@ -562,7 +568,7 @@ cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float
     if (sort_first) {
         const long long n_clear = c->slot_tiles[c->status_idx ^ 1];
         const unsigned cover = (unsigned)(n_clear > (long long)grid ? n_clear : (long long)grid);
-        const cudaError_t e = launch_pdl(k_sort_cull, dim3((cover + kWarps - 1) / kWarps), dim3(kComposeThreads), 0, c->stream,
+        const cudaError_t e = launch_pdl(k_sort_cull, dim3((kSortWarps * cover + kWarps - 1) / kWarps), dim3(kComposeThreads), 0, c->stream,
                                          c->rec, a.count, c->count + (size_t)(c->status_idx ^ 1) * c->max_tiles, c->list, c->meta,
                                          c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty,
                                          (int)grid, (int)n_clear);
@@ -672,7 +678,7 @@ cudaError_t launch_compose_smem_atomic(osog_ctx* c, int B, float* d_opd)
     const uint32_t* count = c->count + (size_t)c->status_idx * c->max_tiles;
     const long long n_clear = c->slot_tiles[c->status_idx ^ 1];
     const unsigned cover = (unsigned)(n_clear > (long long)grid ? n_clear : (long long)grid);
-    k_sort_cull<<<(cover + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(
+    k_sort_cull<<<(kSortWarps * cover + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(
         c->rec, count, c->count + (size_t)(c->status_idx ^ 1) * c->max_tiles, c->list, c->meta,
         c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty, (int)grid, (int)n_clear);
     cudaError_t e = cudaGetLastError();
