@@ -351,7 +351,7 @@ def run_ours(args):
     achieved = k_bytes / (ms_compose * 1e-3) / 1e9
     hbm = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
            "traffic": 10553088, "traffic_note": "dram read+write of one k_compose_tile launch, ncu --set full "
-           "(profiles/r1_final3_compose_ncu.md); the 33.5 MB field it writes stays in the 126 MB L2",
+           "(profiles/r1_final4_compose_ncu.md); the 33.5 MB field it writes stays in the 126 MB L2",
            "peak_source": peak_src, "algorithmic_bytes": int(k_bytes), "kernel": "k_compose_tile",
            "kernel_ms": ms_compose, "frac_of_nominal_8TBs": achieved / 8000.0,
            "note": "BASELINE.json's '% of B200 HBM roofline'; the kernel is bound by instruction issue, see roofline"}
