@@ -14,6 +14,7 @@ Pieces, each following the passage it cites (line numbers are /root/reference/PA
   philox4x32_10   counter-based RNG, written from its published description
   read_noise      z ~ N(0,1) per (seed, frame, pixel) by Box-Muller                   :126 (Gaussian term)
   binning         bounding boxes -> tiles -> counts / offsets / ascending lists       DESIGN.md section 3 (B1-B4)
+  particle_obbs   oriented bounding box of each silhouette (detector labels)          :76, :138-146, A23
 
 Every reading of the paper taken here (units, pixel centres, quaternion convention, pupil edge,
 FFT normalisation, noise model ...) is listed in DESIGN.md section 3.  Pins: tests/test_oracle_*.py.
@@ -381,6 +382,47 @@ def half_extents(cols):
     isp = (cols["kind"] == 1)[:, None]
     h = np.where(isp, hp, he)
     return h[:, 0], h[:, 1]
+
+
+def particle_obbs(scene) -> np.ndarray:
+    """Oriented bounding box of every particle's silhouette, the geometric label the paper's detector is trained on
+    ("YOLOv11 ... OBB"; instance geometry of the G-buffer): float64 [N, 6] =
+    (centre x, centre y, axis u_x, axis u_y, half length along u, half length across u), lengths and centre in pixel
+    units (pixel-index coordinates c / p - 1/2), u a unit vector with u_x >= 0.  Reading A23:
+      ellipsoid  the silhouette is the ellipse {d : d^T Q^-1 d <= 1}, Q = (R diag(a^2, b^2, c^2) R^T) restricted to x, y;
+                 the box is its principal-axis box: u = eigenvector of the larger eigenvalue, half lengths sqrt(eigenvalues)
+      prism      u = normalised projection of the body's long axis (R e_z)_{xy} ((1, 0) if that projection vanishes);
+                 half lengths = largest |(R v)_{xy} . u| and |(R v)_{xy} . u_perp| over the 10 vertices
+    Invalid particles give NaN."""
+    cols = scene.cols
+    R = _rot_all(cols)
+    n = R.shape[0]
+    p = scene.pitch_um
+    out = np.full((n, 6), np.nan)
+    ok = particle_valid(cols)
+    d = np.stack([cols[k].astype(np.float64) for k in ("d0", "d1", "d2")], axis=1)
+    for k in range(n):
+        if not ok[k]:
+            continue
+        if cols["kind"][k] == 0:
+            Q = (R[k] @ np.diag(d[k] ** 2) @ R[k].T)[:2, :2]
+            lam, V = np.linalg.eigh(Q)                       # ascending eigenvalues
+            u = V[:, 1]
+            ha, hb = math.sqrt(lam[1]), math.sqrt(max(lam[0], 0.0))
+        else:
+            s_, L, hc = d[k]
+            u = R[k][:2, 2].copy()
+            nu = math.hypot(u[0], u[1])
+            u = u / nu if nu > 1e-12 else np.array([1.0, 0.0])
+            verts = [(sx * s_ / 2, sy * s_ / 2, sz * L / 2) for sx in (1, -1) for sy in (1, -1) for sz in (1, -1)]
+            verts += [(0.0, 0.0, L / 2 + hc), (0.0, 0.0, -(L / 2 + hc))]
+            P2 = (R[k] @ np.asarray(verts).T)[:2].T          # projected vertices [10, 2]
+            ha = float(np.abs(P2 @ u).max())
+            hb = float(np.abs(P2 @ np.array([-u[1], u[0]])).max())
+        if u[0] < 0.0:
+            u = -u
+        out[k] = (float(cols["cx"][k]) / p - 0.5, float(cols["cy"][k]) / p - 0.5, u[0], u[1], ha / p, hb / p)
+    return out
 
 
 def bboxes(cols, H, W, pitch):
