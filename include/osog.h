@@ -143,6 +143,14 @@ int osog_field_to_dic(osog_ctx* ctx, const osog_optics* o, const osog_dic* dic, 
  * per particle, global atomicAdd into d_opd.  NOT deterministic in the last bits; kept for comparison only. */
 int osog_render_opd_atomic(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd);
 
+/* Instance labels (reading A23; the paper's detector is trained on oriented bounding boxes,
+ * PAPER.md:76, 138-146): d_obb is DEVICE float [N, 6] = (centre x, centre y, u_x, u_y, half length along u, half length
+ * across u) of every particle's silhouette, centre and lengths in pixels (pixel-index coordinates c / p - 1/2), u a unit
+ * vector with u_x >= 0.  Ellipsoid: principal-axis box of the silhouette ellipse; prism: box along the projected long
+ * axis over the 10 projected vertices.  From the geometry alone: no clipping to the frame, no visibility test.  Invalid
+ * particles give NaN.  Runs the per-particle preparation kernel only (fp64 arithmetic, results rounded to float). */
+int osog_particle_obbs(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_obb);
+
 /* Second measured alternative: the same tile lists, but one CTA per tile accumulates the tile in SHARED memory with fp32
  * atomics (one warp per listed particle) and writes it out once.  NOT deterministic in the last bits, fp32 sum; kept for
  * comparison with the ordered register accumulation only. */

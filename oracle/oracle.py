@@ -389,10 +389,13 @@ def particle_obbs(scene) -> np.ndarray:
     ("YOLOv11 ... OBB"; instance geometry of the G-buffer): float64 [N, 6] =
     (centre x, centre y, axis u_x, axis u_y, half length along u, half length across u), lengths and centre in pixel
     units (pixel-index coordinates c / p - 1/2), u a unit vector with u_x >= 0.  Reading A23:
-      ellipsoid  the silhouette is the ellipse {d : d^T Q^-1 d <= 1}, Q = (R diag(a^2, b^2, c^2) R^T) restricted to x, y;
-                 the box is its principal-axis box: u = eigenvector of the larger eigenvalue, half lengths sqrt(eigenvalues)
+      ellipsoid  the body is {q : q^T M q <= 1}, M = R diag(1/a^2, 1/b^2, 1/c^2) R^T exactly as in the thickness function
+                 (R is not renormalised, A4, so M^-1 is not quite R diag(a^2, b^2, c^2) R^T); its shadow is the ellipse
+                 {d : d^T Q^-1 d <= 1} with Q = (M^-1) restricted to x, y; the box is the principal-axis box of that
+                 ellipse: u = eigenvector of the larger eigenvalue of Q, half lengths sqrt(eigenvalues)
       prism      u = normalised projection of the body's long axis (R e_z)_{xy} ((1, 0) if that projection vanishes);
-                 half lengths = largest |(R v)_{xy} . u| and |(R v)_{xy} . u_perp| over the 10 vertices
+                 half lengths = largest |(R v)_{xy} . u| and |(R v)_{xy} . u_perp| over the 10 vertices (vertices R v
+                 as in the binning spec B1)
     Invalid particles give NaN."""
     cols = scene.cols
     R = _rot_all(cols)
@@ -405,7 +408,7 @@ def particle_obbs(scene) -> np.ndarray:
         if not ok[k]:
             continue
         if cols["kind"][k] == 0:
-            Q = (R[k] @ np.diag(d[k] ** 2) @ R[k].T)[:2, :2]
+            Q = np.linalg.inv(R[k] @ np.diag(1.0 / d[k] ** 2) @ R[k].T)[:2, :2]
             lam, V = np.linalg.eigh(Q)                       # ascending eigenvalues
             u = V[:, 1]
             ha, hb = math.sqrt(lam[1]), math.sqrt(max(lam[0], 0.0))

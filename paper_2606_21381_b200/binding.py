@@ -67,7 +67,7 @@ def lib():
     ctx = C.c_void_p
     L.osog_create.argtypes = [C.POINTER(ctx), C.POINTER(osog_config)]
     for name in ("osog_render_opd", "osog_render_field", "osog_render_intensity", "osog_render_opd_atomic",
-                 "osog_render_opd_smem_atomic"):
+                 "osog_render_opd_smem_atomic", "osog_particle_obbs"):
         getattr(L, name).argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p]
     L.osog_field_to_intensity.argtypes = [ctx, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_dic.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics),
@@ -89,7 +89,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_debug_recompose_field", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_debug_recompose_field", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -215,6 +215,15 @@ class Context:
 
     def render_opd_atomic(self, p: Particles, o, out=None):
         return self._call("osog_render_opd_atomic", p, o, self._out(o.B, out=out))
+
+    def particle_obbs(self, p: Particles, o, out=None):
+        """float32 [N, 6] oriented-bounding-box labels (osog_particle_obbs)."""
+        if out is None:
+            out = self.torch.empty((p.N, 6), dtype=self.torch.float32, device=self.device)
+        r = lib().osog_particle_obbs(self._ctx, C.byref(p.c), p.N, C.byref(o), out.data_ptr())
+        if r != OSOG_OK:
+            raise OsogError(r, "osog_particle_obbs")
+        return out
 
     def render_opd_smem_atomic(self, p: Particles, o, out=None):
         return self._call("osog_render_opd_smem_atomic", p, o, self._out(o.B, out=out))

@@ -19,6 +19,7 @@ struct PrepArgs {
     uint32_t* count;              // this call's slot of the per-tile counters (all zero on entry)
     uint32_t* list;               // [tiles][tile_cap]
     int tile_cap;
+    float* obb;                   // [N][6] oriented-bounding-box labels (osog_particle_obbs), or nullptr
     float2 *ramp_x, *ramp_y;
     FrameOptics* optics;
     DeviceStatus* status;
@@ -225,7 +226,11 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
                  finite_f(fd0) && finite_f(fd1) && finite_f(fd2) && finite_f(fnp) &&
                  fd0 > 0.0f && fd1 > 0.0f && fd2 > 0.0f && kind <= 1u;
 
-    if (!valid) return;                          // flagged by the binning role
+    if (!valid) {                                // flagged by the binning role
+        if (a.obb != nullptr)
+            for (int k = 0; k < 6; ++k) a.obb[(size_t)n * 6 + k] = __int_as_float(0x7fc00000);
+        return;
+    }
 
     const double p = a.pitch;
     const double cx = fcx, cy = fcy;
@@ -293,6 +298,12 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
         r32u[8] = 0u;
         r32[9] = (float)(dn * T0);
         r32[10] = 0.0f;
+        if (a.obb != nullptr) {                  // label (reading A23): principal-axis box of the silhouette ellipse, no padding
+            float* ob = a.obb + (size_t)n * 6;
+            ob[0] = (float)(cx * ip - 0.5); ob[1] = (float)(cy * ip - 0.5);
+            ob[2] = (float)(vx * ivn); ob[3] = (float)(vy * ivn);
+            ob[4] = (float)(rsqrt(lmin) * ip); ob[5] = (float)(rsqrt(lmax) * ip);
+        }
         return;
     }
 
@@ -369,6 +380,12 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
     r32u[8] = flags;
     r32[9] = (float)dn;
     r32[10] = 0.0f;
+    if (a.obb != nullptr) {                      // label (reading A23): box along the projected long axis, no padding
+        float* ob = a.obb + (size_t)n * 6;
+        ob[0] = (float)(cx * ip - 0.5); ob[1] = (float)(cy * ip - 0.5);
+        ob[2] = (float)ax; ob[3] = (float)ay;
+        ob[4] = (float)(ha * ip); ob[5] = (float)(hb * ip);
+    }
 }
 
 __global__ void k_set_optics(FrameOptics* optics, const OpticsChunk oc)
@@ -419,7 +436,7 @@ cudaError_t upload_optics(osog_ctx* c, const osog_optics* o, OpticsChunk* first)
     return cudaSuccess;
 }
 
-cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o)
+cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o, float* d_obb)
 {
     const int B = o->B;
     const long long tiles = (long long)B * c->ntx * c->nty;
@@ -447,6 +464,7 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     a.pitch = o->pitch_um; a.n_medium = o->n_medium;
     a.rec = c->rec; a.tbox = c->tbox; a.pframe = c->pframe;
     a.count = c->count + (size_t)c->status_idx * c->max_tiles; a.list = c->list; a.tile_cap = c->tile_cap;
+    a.obb = d_obb;
     a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.optics = c->optics; a.status = status;
     a.has_ramp = (o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0) ? 1 : 0;
     if ((e = upload_optics(c, o, &a.oc)) != cudaSuccess) return e;

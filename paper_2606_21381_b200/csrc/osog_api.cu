@@ -361,6 +361,18 @@ int osog_render_opd_atomic(osog_ctx* c, const osog_particles* p, int64_t N, cons
     return OSOG_OK;
 }
 
+int osog_particle_obbs(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_obb)
+{
+    if (N == 0) return (c && p && o) ? OSOG_OK : OSOG_EINVAL;
+    const int r = check_call(c, p, N, o, d_obb);
+    if (r != OSOG_OK) return r;
+    DeviceGuard g(c->device);
+    cudaError_t e = launch_binning(c, p, N, o, d_obb);   // k_prepare alone; the tile lists it leaves are not used
+    if (e != cudaSuccess) return cuda_fail(c, e);        // (scratch_dirty stays set: the next render call clears them)
+    c->last_has_ramp = -1;
+    return OSOG_OK;
+}
+
 int osog_render_opd_smem_atomic(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd)
 {
     const int r = check_call(c, p, N, o, d_opd);

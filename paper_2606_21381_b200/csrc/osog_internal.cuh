@@ -112,7 +112,7 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 
 // binning.cu
 cudaError_t upload_optics(osog_ctx* c, const osog_optics* o, OpticsChunk* first);
-cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o);
+cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o, float* d_obb = nullptr);
 // compose.cu
 cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float* d_opd, float2* d_field, bool sort_first = true);
 cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd);
