@@ -15,6 +15,7 @@ Pieces, each following the passage it cites (line numbers are /root/reference/PA
   read_noise      z ~ N(0,1) per (seed, frame, pixel) by Box-Muller                   :126 (Gaussian term)
   binning         bounding boxes -> tiles -> counts / offsets / ascending lists       DESIGN.md section 3 (B1-B4)
   particle_obbs   oriented bounding box of each silhouette (detector labels)          :76, :138-146, A23
+  render_gbuffer  depth map and instance-id map (top-most particle per pixel), in C   :76, A24
 
 Every reading of the paper taken here (units, pixel centres, quaternion convention, pupil edge,
 FFT normalisation, noise model ...) is listed in DESIGN.md section 3.  Pins: tests/test_oracle_*.py.
@@ -46,6 +47,11 @@ def _lib():
         lib.osog_oracle_count_covered.argtypes = [ctypes.c_int64] + [fp] * 10 + [u8p] + [
             ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int64)]
         lib.osog_oracle_count_covered.restype = None
+        lib.osog_oracle_render_gbuffer.argtypes = [ctypes.c_int64] + [fp] * 11 + [u8p] + [
+            ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int32), dp]
+        lib.osog_oracle_render_gbuffer.restype = None
+        lib.osog_oracle_chord.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double, dp, dp]
+        lib.osog_oracle_chord.restype = ctypes.c_int
         lib.osog_oracle_thickness.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double]
         lib.osog_oracle_thickness.restype = ctypes.c_double
         lib.osog_oracle_circumradius.argtypes = [ctypes.c_uint8] + [ctypes.c_float] * 3
@@ -116,6 +122,38 @@ def render_opd_frame(cols, lo, hi, H, W, pitch, n_medium, mode="bcircle") -> np.
         _ptr(kind, ctypes.c_uint8), H, W, float(pitch), float(n_medium),
         {"full": 0, "bcircle": 1}[mode], _ptr(out, ctypes.c_double))
     return out
+
+
+def chord(kind, q, dims, dx, dy):
+    """(z_enter, z_exit) of the vertical line through the body relative to its centre, or None (no positive chord)."""
+    R = np.ascontiguousarray(rot_from_quat(q), dtype=np.float64).reshape(9)
+    d = np.ascontiguousarray(dims, dtype=np.float64)
+    ze, zx = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    ok = _lib().osog_oracle_chord(int(kind), _ptr(R, ctypes.c_double), _ptr(d, ctypes.c_double), float(dx), float(dy),
+                                  ctypes.byref(ze), ctypes.byref(zx))
+    return (ze.value, zx.value) if ok else None
+
+
+def render_gbuffer(scene, mode="bcircle"):
+    """(top_id int32 [B, H, W], depth float64 [B, H, W]) of a workloads.Scene: index (within the frame's particles,
+    i.e. relative to frame_start[b]) and top-surface height of the top-most particle above every pixel (reading A24)."""
+    fs = scene.frame_start
+    f = ctypes.c_float
+    ids, deps = [], []
+    for b in range(scene.B):
+        lo, hi = int(fs[b]), int(fs[b + 1])
+        a = {k: np.ascontiguousarray(scene.cols[k][lo:hi], dtype=np.float32) for k in _COLS + ("cz",)}
+        kind = np.ascontiguousarray(scene.cols["kind"][lo:hi], dtype=np.uint8)
+        tid = np.empty((scene.H, scene.W), dtype=np.int32)
+        dep = np.empty((scene.H, scene.W), dtype=np.float64)
+        _lib().osog_oracle_render_gbuffer(
+            hi - lo, _ptr(a["cx"], f), _ptr(a["cy"], f), _ptr(a["cz"], f), _ptr(a["qw"], f), _ptr(a["qx"], f),
+            _ptr(a["qy"], f), _ptr(a["qz"], f), _ptr(a["d0"], f), _ptr(a["d1"], f), _ptr(a["d2"], f), _ptr(a["n_p"], f),
+            _ptr(kind, ctypes.c_uint8), scene.H, scene.W, float(scene.pitch_um),
+            {"full": 0, "bcircle": 1}[mode], _ptr(tid, ctypes.c_int32), _ptr(dep, ctypes.c_double))
+        ids.append(tid)
+        deps.append(dep)
+    return np.stack(ids), np.stack(deps)
 
 
 def count_covered(scene, mode="bcircle"):

@@ -235,3 +235,90 @@ void osog_oracle_count_covered(int64_t N,
     pairs[0] = ne;
     pairs[1] = np;
 }
+
+/* ---- G-buffer extras ("depth maps ... strict instance masks"; reading A24) ----------
+ * Chord of the vertical line (dx, dy, .) through the body: [*z_enter, *z_exit] relative to the centre; returns 1 when the
+ * chord has positive length (the same condition as thickness > 0), else 0.  Ellipsoid: roots of A z^2 + 2 Bq z + C = 0,
+ * z = (-Bq -+ sqrt(disc)) / A; polyhedron: enter / exit of the Eq. 1 plane loop. */
+int osog_oracle_chord(uint8_t kind, const double R[9], const double dims[3], double dx, double dy,
+                      double *z_enter, double *z_exit)
+{
+    if (kind == 0) {
+        const double a = dims[0], b = dims[1], c = dims[2];
+        const double D[3] = { 1.0 / (a * a), 1.0 / (b * b), 1.0 / (c * c) };
+        double M[9];
+        for (int r = 0; r < 3; ++r)
+            for (int s = 0; s < 3; ++s) {
+                double acc = 0.0;
+                for (int k = 0; k < 3; ++k) acc += R[3 * r + k] * D[k] * R[3 * s + k];
+                M[3 * r + s] = acc;
+            }
+        const double A  = M[8];
+        const double Bq = M[2] * dx + M[5] * dy;
+        const double C  = M[0] * dx * dx + 2.0 * M[1] * dx * dy + M[4] * dy * dy - 1.0;
+        const double disc = Bq * Bq - A * C;
+        if (!(disc > 0.0)) return 0;
+        const double sq = sqrt(disc);
+        *z_enter = (-Bq - sq) / A;
+        *z_exit  = (-Bq + sq) / A;
+        return 1;
+    }
+    double Aw[OSOG_ORACLE_MAX_PLANES][3], bb[OSOG_ORACLE_MAX_PLANES];
+    const int M = prism_world_planes(R, dims[0], dims[1], dims[2], Aw, bb);
+    double enter = -INFINITY, exit_ = INFINITY;
+    for (int k = 0; k < M; ++k) {
+        const double g = bb[k] - Aw[k][0] * dx - Aw[k][1] * dy;
+        const double nz = Aw[k][2];
+        if (nz > 0.0)      { const double z = g / nz; if (z < exit_) exit_ = z; }
+        else if (nz < 0.0) { const double z = g / nz; if (z > enter) enter = z; }
+        else if (g < 0.0)  return 0;
+    }
+    if (!(exit_ - enter > 0.0)) return 0;
+    *z_enter = enter;
+    *z_exit = exit_;
+    return 1;
+}
+
+/* Depth and instance-id maps of one frame (reading A24): for every pixel, among the particles whose chord there has
+ * positive length, the one whose top surface  cz[n] + z_exit  is highest (+z points at the objective); ties go to the
+ * smallest index.  top_id[i*W+j] = that particle's index (-1: no particle), depth[i*W+j] = the height of its top
+ * surface in um (0 where top_id is -1).  cz may be NULL (all zero).  mode as in osog_oracle_render_opd. */
+void osog_oracle_render_gbuffer(int64_t N,
+                                const float *cx, const float *cy, const float *cz,
+                                const float *qw, const float *qx, const float *qy, const float *qz,
+                                const float *d0, const float *d1, const float *d2,
+                                const float *n_p, const uint8_t *kind,
+                                int H, int W, double pitch, int mode, int32_t *top_id, double *depth)
+{
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int i = 0; i < H; ++i) {
+        const double y = (i + 0.5) * pitch;
+        for (int j = 0; j < W; ++j) { top_id[(size_t)i * W + j] = -1; depth[(size_t)i * W + j] = 0.0; }
+        for (int64_t n = 0; n < N; ++n) {
+            if (!osog_oracle_particle_valid(cx[n], cy[n], qw[n], qx[n], qy[n], qz[n],
+                                            d0[n], d1[n], d2[n], n_p[n], kind[n])) continue;
+            if (cz != NULL && !isfinite((double)cz[n])) continue;
+            const double dy = y - (double)cy[n];
+            const double q[4] = { qw[n], qx[n], qy[n], qz[n] };
+            const double dims[3] = { d0[n], d1[n], d2[n] };
+            double R[9];
+            osog_oracle_rot_from_quat(q, R);
+            double r2 = INFINITY;
+            if (mode == 1) {
+                const double r = osog_oracle_circumradius(kind[n], d0[n], d1[n], d2[n]) * (1.0 + 1e-9);
+                r2 = r * r;
+                if (dy * dy > r2) continue;
+            }
+            const double zc = cz != NULL ? (double)cz[n] : 0.0;
+            for (int j = 0; j < W; ++j) {
+                const double dx = (j + 0.5) * pitch - (double)cx[n];
+                if (dx * dx + dy * dy > r2) continue;
+                double ze, zx;
+                if (!osog_oracle_chord(kind[n], R, dims, dx, dy, &ze, &zx)) continue;
+                const double top = zc + zx;
+                const size_t px = (size_t)i * W + j;
+                if (top_id[px] < 0 || top > depth[px]) { top_id[px] = (int32_t)n; depth[px] = top; }
+            }
+        }
+    }
+}
