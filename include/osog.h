@@ -71,7 +71,7 @@ typedef struct {
  * column, const, caller-owned.  Frame b owns particles frame_start[b] .. frame_start[b+1]-1. */
 typedef struct {
     uint32_t struct_size;
-    const float *cx, *cy, *cz;        /* centre, um; cz is accepted and unused (projection along z); may be NULL */
+    const float *cx, *cy, *cz;        /* centre, um; cz is used by osog_render_gbuffer only (projection along z); may be NULL */
     const float *qw, *qx, *qy, *qz;   /* unit quaternion (w, x, y, z), Hamilton, active body -> world, not renormalised */
     const float *d0, *d1, *d2;        /* kind 0: semi-axes a, b, c;  kind 1: side s, length L, cap height hc (um) */
     const float *n_p;                 /* refractive index of the particle                                    */
@@ -150,6 +150,14 @@ int osog_render_opd_atomic(osog_ctx* ctx, const osog_particles* p, int64_t N, co
  * axis over the 10 projected vertices.  From the geometry alone: no clipping to the frame, no visibility test.  Invalid
  * particles give NaN.  Runs the per-particle preparation kernel only (fp64 arithmetic, results rounded to float). */
 int osog_particle_obbs(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_obb);
+
+/* G-buffer extras (reading A24; "depth maps ... strict instance masks"): for every pixel,
+ * among the frame's particles whose chord there has positive length, the one whose top surface cz + z_exit is highest
+ * (+z points at the objective; this is the one call that uses cz; a NULL cz means 0, a non-finite cz removes the particle
+ * from these maps).  d_top_id is DEVICE int32 [B, H, W]: that particle's index within its frame (relative to
+ * frame_start[b]; ties go to the smallest index; -1 = no particle); d_depth is DEVICE float [B, H, W]: the height of that
+ * top surface in um (0 where d_top_id is -1).  Runs the binning, then one fp64 evaluation per listed (particle, pixel). */
+int osog_render_gbuffer(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, int32_t* d_top_id, float* d_depth);
 
 /* Second measured alternative: the same tile lists, but one CTA per tile accumulates the tile in SHARED memory with fp32
  * atomics (one warp per listed particle) and writes it out once.  NOT deterministic in the last bits, fp32 sum; kept for

@@ -7,7 +7,7 @@
 namespace osog {
 
 struct PrepArgs {
-    const float *cx, *cy, *qw, *qx, *qy, *qz, *d0, *d1, *d2, *n_p;
+    const float *cx, *cy, *cz, *qw, *qx, *qy, *qz, *d0, *d1, *d2, *n_p;   // cz may be nullptr (all zero)
     const uint8_t* kind;
     const int32_t* frame_start;   // device [B+1] or nullptr
     long long N;
@@ -297,7 +297,12 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
         r32[5] = (float)(rsqrt(lmax) * ip * (1.0 + 1.0e-5) + cull_pad);
         r32u[8] = 0u;
         r32[9] = (float)(dn * T0);
-        r32[10] = 0.0f;
+        r32[10] = a.cz != nullptr ? a.cz[n] : 0.0f;          // centre height (G-buffer depth map only)
+        // chord midpoint z = -(M_xz dx + M_yz dy) / M_zz as Z0 + Zx dj + Zy di, and T0 (G-buffer only)
+        r64[8] = -(Mxz * ox + Myz * oy) * iMzz;
+        r64[9] = -Mxz * p * iMzz;
+        r64[10] = -Myz * p * iMzz;
+        r64[11] = T0;
         if (a.obb != nullptr) {                  // label (reading A23): principal-axis box of the silhouette ellipse, no padding
             float* ob = a.obb + (size_t)n * 6;
             ob[0] = (float)(cx * ip - 0.5); ob[1] = (float)(cy * ip - 0.5);
@@ -379,7 +384,7 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
     r32u[5] = __float_as_uint((float)(hb * ip * (1.0 + 1.0e-5) + cull_pad)) | (((code >> 1) & 1u) << 31);
     r32u[8] = flags;
     r32[9] = (float)dn;
-    r32[10] = 0.0f;
+    r32[10] = a.cz != nullptr ? a.cz[n] : 0.0f;              // centre height (G-buffer depth map only)
     if (a.obb != nullptr) {                      // label (reading A23): box along the projected long axis, no padding
         float* ob = a.obb + (size_t)n * 6;
         ob[0] = (float)(cx * ip - 0.5); ob[1] = (float)(cy * ip - 0.5);
@@ -457,7 +462,7 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     DeviceStatus* status = c->status + c->status_idx;
 
     PrepArgs a;
-    a.cx = p->cx; a.cy = p->cy; a.qw = p->qw; a.qx = p->qx; a.qy = p->qy; a.qz = p->qz;
+    a.cx = p->cx; a.cy = p->cy; a.cz = p->cz; a.qw = p->qw; a.qx = p->qx; a.qy = p->qy; a.qz = p->qz;
     a.d0 = p->d0; a.d1 = p->d1; a.d2 = p->d2; a.n_p = p->n_p; a.kind = p->kind;
     a.frame_start = B > 1 ? p->frame_start : nullptr;
     a.N = N; a.B = B; a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;

@@ -619,6 +619,104 @@ __global__ void __launch_bounds__(256) k_compose_atomic(const float* __restrict_
     }
 }
 
+// ---- G-buffer extras (reading A24): depth map and instance-id map -----------------------------------
+// Chord of the vertical line through a prism, all in fp64 from the record (same plane data as prism_t64): false when
+// the chord has no positive length, else *z_exit = z of the exit point relative to the centre.
+__device__ __forceinline__ bool prism_exit64(const double* r64, uint32_t vmask, double dj, double di, double* z_exit)
+{
+    double ex = 1.0e300, en = -1.0e300;
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+        const double2 uv = *reinterpret_cast<const double2*>(r64 + 4 * q);
+        const double2 xn = *reinterpret_cast<const double2*>(r64 + 4 * q + 2);
+        const double m = fma(uv.x, dj, uv.y * di);
+        if ((vmask >> q) & 1u) {
+            if (fabs(m + xn.x) > xn.y) return false;   // outside a vertical slab
+        } else {
+            const double e = xn.x - m, n = xn.y - m;
+            ex = e < ex ? e : ex;
+            en = n > en ? n : en;
+        }
+    }
+    *z_exit = ex;
+    return ex - en > 0.0;
+}
+
+// One CTA of 8 warps per tile, warp = 16 x 8 pixel sub-tile, lane = 4 x 1 pixels (the layout of the composition).  Every
+// warp walks the tile's sorted list, skips the entries whose sub-tile mask bit is clear, and for the others evaluates the
+// top of the chord in fp64 straight from the record: the decision "which particle is on top" is taken in the precision
+// the oracle takes it in.  Ascending list order and a strict comparison give ties to the smallest index.
+__global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* __restrict__ recs, const uint32_t* __restrict__ count,
+                                                                const uint32_t* __restrict__ list, const uint16_t* __restrict__ meta,
+                                                                int tile_cap, const DeviceStatus* __restrict__ status,
+                                                                const int32_t* __restrict__ frame_start, int ntx, int nty, int H,
+                                                                int W, int32_t* __restrict__ top_id, float* __restrict__ depth)
+{
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int tile = blockIdx.x, tpf = ntx * nty;
+    const int b = tile / tpf, rt = tile - b * tpf;
+    const int ty = rt / ntx, tx = rt - ty * ntx;
+    const int j = tx * kTile + (wid & 1) * 16 + (lane & 3) * 4, i = ty * kTile + (wid >> 1) * 8 + (lane >> 2);
+    const uint32_t L = (status->bits & OSOG_WOVERFLOW) ? 0u : count[tile];
+    const uint32_t* glist = list + (size_t)tile * tile_cap;
+    const uint16_t* gmeta = meta + (size_t)tile * tile_cap;
+    const uint32_t first = frame_start != nullptr ? (uint32_t)frame_start[b] : 0u;
+    double best[4] = {0.0, 0.0, 0.0, 0.0};
+    int32_t who[4] = {-1, -1, -1, -1};
+    for (uint32_t k = 0; k < L; ++k) {
+        if (((gmeta[k] >> wid) & 1u) == 0u) continue;           // warp-uniform
+        const uint32_t pid = glist[k];
+        const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)pid * kRecWords);
+        const float4 h2 = __ldg(rec + 2);
+        const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));
+        const float czf = h2.z;
+        if (!(fabsf(czf) <= 3.402823466e38f)) continue;          // non-finite height: no entry in the depth map
+        const uint32_t flags = __float_as_uint(h2.x);
+        const double* c = reinterpret_cast<const double*>(rec + 4);
+        const double di = (double)(i - h3.y);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const double dj = (double)(j + q - h3.x);
+            double zx;
+            bool hit;
+            if (flags & kFlagPrism) {
+                hit = prism_exit64(c, flags >> 16, dj, di, &zx);
+            } else {
+                const double w = c[5] - fma(fma(c[0], dj, fma(c[1], di, c[3])), dj, fma(c[2], di, c[4]) * di);
+                hit = w > 0.0;
+                zx = fma(c[9], dj, fma(c[10], di, c[8])) + 0.5 * c[11] * sqrt(fmax(w, 0.0));
+            }
+            const double top = (double)czf + zx;
+            if (hit && (who[q] < 0 || top > best[q])) { best[q] = top; who[q] = (int32_t)(pid - first); }
+        }
+    }
+    if (i >= H) return;
+    const size_t row = ((size_t)b * H + i) * W;
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+        if (j + q < W) {
+            top_id[row + j + q] = who[q];
+            depth[row + j + q] = who[q] < 0 ? 0.0f : (float)best[q];
+        }
+}
+
+cudaError_t launch_gbuffer(osog_ctx* c, int B, const int32_t* d_frame_start, int32_t* d_top_id, float* d_depth)
+{
+    const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
+    const uint32_t* count = c->count + (size_t)c->status_idx * c->max_tiles;
+    const long long n_clear = c->slot_tiles[c->status_idx ^ 1];
+    const unsigned cover = (unsigned)(n_clear > (long long)grid ? n_clear : (long long)grid);
+    k_sort_cull<<<(kSortWarps * cover + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(
+        c->rec, count, c->count + (size_t)(c->status_idx ^ 1) * c->max_tiles, c->list, c->meta,
+        c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty, (int)grid, (int)n_clear);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    c->slot_tiles[c->status_idx ^ 1] = 0;
+    k_gbuffer_tile<<<grid, kComposeThreads, 0, c->stream>>>(c->rec, count, c->list, c->meta, c->tile_cap, c->status + c->status_idx,
+                                                           d_frame_start, c->ntx, c->nty, c->H, c->W, d_top_id, d_depth);
+    return cudaGetLastError();
+}
+
 // ---- measured alternative: tile lists + shared-memory atomics (north_star's "accumulate in shared memory") -------------
 // One CTA per 32 x 32 tile keeps the tile's OPD in shared memory; one warp per listed particle walks the part of the
 // particle's pixel bounding box that lies in the tile and atomicAdd's (n_p - n_m) t into it (fp64 thickness per pixel, fp32

@@ -373,6 +373,22 @@ int osog_particle_obbs(osog_ctx* c, const osog_particles* p, int64_t N, const os
     return OSOG_OK;
 }
 
+int osog_render_gbuffer(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, int32_t* d_top_id, float* d_depth)
+{
+    if (!d_top_id || !aligned16(d_top_id)) return OSOG_EINVAL;
+    const int r = check_call(c, p, N, o, d_depth);
+    if (r != OSOG_OK) return r;
+    if (p->cz != nullptr && (reinterpret_cast<uintptr_t>(p->cz) & 3u)) return OSOG_EINVAL;
+    DeviceGuard g(c->device);
+    cudaError_t e = launch_binning(c, p, N, o);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->last_has_ramp = -1;                           // no field-capable composition ran: osog_debug_recompose_field refuses
+    e = launch_gbuffer(c, o->B, o->B > 1 ? p->frame_start : nullptr, d_top_id, d_depth);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->scratch_dirty = false;
+    return OSOG_OK;
+}
+
 int osog_render_opd_smem_atomic(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd)
 {
     const int r = check_call(c, p, N, o, d_opd);
