@@ -253,7 +253,19 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
     r32u[11] = (uint32_t)n;
     reinterpret_cast<int*>(r32)[12] = (int)jc;
     reinterpret_cast<int*>(r32)[13] = (int)ic;
-    r32[14] = 0.0f;
+    // word 14: upper bound of the chord's top relative to the centre (G-buffer: a particle whose cz + bound lies below
+    // every top already found in a sub-tile is skipped); padded for the not-quite-orthogonal R of reading A4
+    {
+        double zmax;
+        if (kind == 0u) {
+            zmax = sqrt(R20 * R20 * e0 * e0 + R21 * R21 * e1 * e1 + R22 * R22 * e2 * e2);
+        } else {
+            const double hs = 0.5 * e0, hl = 0.5 * e1;
+            zmax = fabs(R22) * (hl + e2);
+            zmax = fmax(zmax, fabs(R20) * hs + fabs(R21) * hs + fabs(R22) * hl);
+        }
+        r32[14] = __double2float_ru(zmax * (1.0 + 1.0e-5) + 1.0e-6);
+    }
     r32[15] = 0.0f;
     // Words 2..5: oriented box of the silhouette (unit axis with a_x >= 0, half lengths > 0); their sign bits carry the
     // evaluation code of the particle (0 ellipsoid, 1 + number of steep slabs, 4 all-fp64): bit 0 in the sign of

@@ -663,6 +663,7 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
     const uint32_t first = frame_start != nullptr ? (uint32_t)frame_start[b] : 0u;
     double best[4] = {0.0, 0.0, 0.0, 0.0};
     int32_t who[4] = {-1, -1, -1, -1};
+    float floor_all = __int_as_float(0xff800000);                // -inf: nothing can be skipped yet
     for (uint32_t k = 0; k < L; ++k) {
         if (((gmeta[k] >> wid) & 1u) == 0u) continue;           // warp-uniform
         const uint32_t pid = glist[k];
@@ -671,6 +672,8 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
         const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));
         const float czf = h2.z;
         if (!(fabsf(czf) <= 3.402823466e38f)) continue;          // non-finite height: no entry in the depth map
+        // no point of this particle lies above cz + zmax: skip it when every pixel of the sub-tile already has a higher top
+        if (czf + __int_as_float(h3.z) < floor_all) continue;
         const uint32_t flags = __float_as_uint(h2.x);
         const double* c = reinterpret_cast<const double*>(rec + 4);
         const double di = (double)(i - h3.y);
@@ -689,6 +692,13 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
             const double top = (double)czf + zx;
             if (hit && (who[q] < 0 || top > best[q])) { best[q] = top; who[q] = (int32_t)(pid - first); }
         }
+        // lowest top over the warp's 128 pixels, rounded down (-inf while some pixel has no owner)
+        float lo = __int_as_float(0x7f800000);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) lo = fminf(lo, who[q] < 0 ? __int_as_float(0xff800000) : __double2float_rd(best[q]));
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, d));
+        floor_all = lo - 1.0e-5f;                                // margin for the float sum cz + zmax
     }
     if (i >= H) return;
     const size_t row = ((size_t)b * H + i) * W;
