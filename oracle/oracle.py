@@ -16,6 +16,7 @@ Pieces, each following the passage it cites (line numbers are /root/reference/PA
   binning         bounding boxes -> tiles -> counts / offsets / ascending lists       DESIGN.md section 3 (B1-B4)
   particle_obbs   oriented bounding box of each silhouette (detector labels)          :76, :138-146, A23
   render_gbuffer  depth map and instance-id map (top-most particle per pixel), in C   :76, A24
+  render_height / height_gradient / height_laplacian   h, grad h, lap h of the G-buffer :76, :92, :96-99, A25
 
 Every reading of the paper taken here (units, pixel centres, quaternion convention, pupil edge,
 FFT normalisation, noise model ...) is listed in DESIGN.md section 3.  Pins: tests/test_oracle_*.py.
@@ -420,6 +421,46 @@ def half_extents(cols):
     isp = (cols["kind"] == 1)[:, None]
     h = np.where(isp, hp, he)
     return h[:, 0], h[:, 1]
+
+
+def render_height(scene, mode="bcircle") -> np.ndarray:
+    """Height (total thickness) map h [B, H, W] float64 of the G-buffer ("spatially varying thickness
+    h(x, y)"): the sum over the frame's particles of their thickness along z, i.e. the OPD loop with n_p - n_medium = 1
+    exactly (n_p = 1, n_medium = 0 are passed to the same C loop)."""
+    fs = scene.frame_start
+    ones = dict(scene.cols)
+    ones["n_p"] = np.ones_like(scene.cols["n_p"])
+    return np.stack([render_opd_frame(ones, int(fs[b]), int(fs[b + 1]), scene.H, scene.W, scene.pitch_um, 0.0, mode)
+                     for b in range(scene.B)])
+
+
+def height_gradient(h, pitch):
+    """Finite-difference gradient of a height map on the pixel grid (reading A25; the paper takes the normals
+    N = <-grad_x h, -grad_y h, 1> "from the G-buffer"): central differences (h[j+1] - h[j-1]) / (2 p) inside,
+    one-sided differences (h[1] - h[0]) / p and (h[W-1] - h[W-2]) / p on the frame border.  Returns (gx, gy), x = columns."""
+    H, W = h.shape
+    gx = np.empty_like(h)
+    gy = np.empty_like(h)
+    for j in range(W):
+        jm, jp = max(j - 1, 0), min(j + 1, W - 1)
+        gx[:, j] = (h[:, jp] - h[:, jm]) / ((jp - jm) * pitch) if jp > jm else 0.0
+    for i in range(H):
+        im, ip = max(i - 1, 0), min(i + 1, H - 1)
+        gy[i, :] = (h[ip, :] - h[im, :]) / ((ip - im) * pitch) if ip > im else 0.0
+    return gx, gy
+
+
+def height_laplacian(h, pitch):
+    """Five-point Laplacian of a height map (the curvature term of Eq. 4, "C(x, y) ~ -lap h"; reading A25):
+    (h[i, j+1] + h[i, j-1] + h[i+1, j] + h[i-1, j] - 4 h[i, j]) / p^2 with the border pixels replicated outwards."""
+    H, W = h.shape
+    out = np.empty_like(h)
+    for i in range(H):
+        im, ip = max(i - 1, 0), min(i + 1, H - 1)
+        for j in range(W):
+            jm, jp = max(j - 1, 0), min(j + 1, W - 1)
+            out[i, j] = (h[i, jp] + h[i, jm] + h[ip, j] + h[im, j] - 4.0 * h[i, j]) / (pitch * pitch)
+    return out
 
 
 def particle_obbs(scene) -> np.ndarray:
