@@ -151,6 +151,14 @@ int osog_render_opd_atomic(osog_ctx* ctx, const osog_particles* p, int64_t N, co
  * particles give NaN.  Runs the per-particle preparation kernel only (fp64 arithmetic, results rounded to float). */
 int osog_particle_obbs(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_obb);
 
+/* Height map of the G-buffer and its derivatives (reading A25): d_h is DEVICE
+ * float [B, H, W], the sum of the particles' thicknesses in um (the hot path of osog_render_opd with the index contrast
+ * n_p - n_medium replaced by 1); d_grad (DEVICE float [B, H, W, 2], may be NULL) = (dh/dx, dh/dy) by central differences
+ * on the pixel grid, one-sided on the frame border (the normal of PAPER.md:92 is (-g_x, -g_y, 1)); d_lap (DEVICE float
+ * [B, H, W], may be NULL) = 5-point Laplacian of h in 1/um with the border pixels replicated (curvature term of Eq. 4). */
+int osog_render_height(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_h, float* d_grad,
+                       float* d_lap);
+
 /* G-buffer extras (reading A24; "depth maps ... strict instance masks"): for every pixel,
  * among the frame's particles whose chord there has positive length, the one whose top surface cz + z_exit is highest
  * (+z points at the objective; this is the one call that uses cz; a NULL cz means 0, a non-finite cz removes the particle

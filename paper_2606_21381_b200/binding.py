@@ -74,6 +74,8 @@ def lib():
                                   C.POINTER(osog_dic), C.c_void_p]
     L.osog_field_to_dic.argtypes = [ctx, C.POINTER(osog_optics), C.POINTER(osog_dic), C.c_void_p, C.c_void_p]
     L.osog_render_gbuffer.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
+    L.osog_render_height.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p,
+                                     C.c_void_p]
     L.osog_debug_recompose_field.argtypes = [ctx, C.c_void_p]
     L.osog_destroy.argtypes = [ctx]
     L.osog_status.argtypes = [ctx, C.POINTER(C.c_uint32), C.POINTER(C.c_int64)]
@@ -90,7 +92,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_debug_recompose_field", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_debug_recompose_field", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -216,6 +218,17 @@ class Context:
 
     def render_opd_atomic(self, p: Particles, o, out=None):
         return self._call("osog_render_opd_atomic", p, o, self._out(o.B, out=out))
+
+    def render_height(self, p: Particles, o, grad=True, lap=True):
+        """(h float32 [B, H, W], grad float32 [B, H, W, 2] or None, lap float32 [B, H, W] or None) (osog_render_height)."""
+        h = self._out(o.B)
+        g = self._out(o.B, 2) if grad else None
+        l = self._out(o.B) if lap else None
+        r = lib().osog_render_height(self._ctx, C.byref(p.c), p.N, C.byref(o), h.data_ptr(),
+                                     g.data_ptr() if grad else None, l.data_ptr() if lap else None)
+        if r != OSOG_OK:
+            raise OsogError(r, "osog_render_height")
+        return h, g, l
 
     def render_gbuffer(self, p: Particles, o):
         """(int32 [B, H, W] instance id of the top-most particle, float32 [B, H, W] height of its top surface)."""

@@ -20,6 +20,7 @@ struct PrepArgs {
     uint32_t* list;               // [tiles][tile_cap]
     int tile_cap;
     float* obb;                   // [N][6] oriented-bounding-box labels (osog_particle_obbs), or nullptr
+    int unit_dn;                  // 1: index contrast n_p - n_medium replaced by 1 (height map of the G-buffer)
     float2 *ramp_x, *ramp_y;
     FrameOptics* optics;
     DeviceStatus* status;
@@ -248,7 +249,7 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
     const double jc = fmin(fmax(floor(cx * ip), -1.0e6), 1.0e6);      // reference pixel: any nearby pixel will do
     const double ic = fmin(fmax(floor(cy * ip), -1.0e6), 1.0e6);
     const double ox = (jc + 0.5) * p - cx, oy = (ic + 0.5) * p - cy;
-    const double dn = (double)fnp - a.n_medium;
+    const double dn = a.unit_dn ? 1.0 : (double)fnp - a.n_medium;
     double* r64 = reinterpret_cast<double*>(r32 + 16);
     r32u[11] = (uint32_t)n;
     reinterpret_cast<int*>(r32)[12] = (int)jc;
@@ -453,7 +454,7 @@ cudaError_t upload_optics(osog_ctx* c, const osog_optics* o, OpticsChunk* first)
     return cudaSuccess;
 }
 
-cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o, float* d_obb)
+cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o, float* d_obb, bool unit_dn)
 {
     const int B = o->B;
     const long long tiles = (long long)B * c->ntx * c->nty;
@@ -482,6 +483,7 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     a.rec = c->rec; a.tbox = c->tbox; a.pframe = c->pframe;
     a.count = c->count + (size_t)c->status_idx * c->max_tiles; a.list = c->list; a.tile_cap = c->tile_cap;
     a.obb = d_obb;
+    a.unit_dn = unit_dn ? 1 : 0;
     a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.optics = c->optics; a.status = status;
     a.has_ramp = (o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0) ? 1 : 0;
     if ((e = upload_optics(c, o, &a.oc)) != cudaSuccess) return e;

@@ -71,6 +71,28 @@ __global__ void __launch_bounds__(256) k_dic_shear(const float2* __restrict__ fi
     out[((size_t)b * H + i) * W + j] = make_float2(dr * dr + di * di, 0.0f);
 }
 
+// G-buffer (reading A25): finite differences of the height map h on the pixel grid.  grad = (g_x, g_y) interleaved:
+// central differences inside, one-sided on the frame border; lap = 5-point Laplacian with the border pixels replicated.
+__global__ void __launch_bounds__(256) k_height_stencil(const float* __restrict__ h, int H, int W, float inv_p,
+                                                        float2* __restrict__ grad, float* __restrict__ lap)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = blockIdx.y, b = blockIdx.z;
+    if (j >= W) return;
+    const float* f = h + (size_t)b * H * W;
+    const int jm = max(j - 1, 0), jp = min(j + 1, W - 1), im = max(i - 1, 0), ip = min(i + 1, H - 1);
+    const float c = f[(size_t)i * W + j];
+    const float xl = f[(size_t)i * W + jm], xr = f[(size_t)i * W + jp];
+    const float yu = f[(size_t)im * W + j], yd = f[(size_t)ip * W + j];
+    const size_t idx = ((size_t)b * H + i) * W + j;
+    if (grad != nullptr) {
+        const float gx = jp > jm ? (xr - xl) * (inv_p / (float)(jp - jm)) : 0.0f;
+        const float gy = ip > im ? (yd - yu) * (inv_p / (float)(ip - im)) : 0.0f;
+        grad[idx] = make_float2(gx, gy);
+    }
+    if (lap != nullptr) lap[idx] = ((xl + xr) + (yu + yd) - 4.0f * c) * (inv_p * inv_p);
+}
+
 // buf = (|buf|^2 * scale, 0)
 __global__ void __launch_bounds__(256) k_abs2(float2* __restrict__ buf, size_t n, float scale)
 {
@@ -159,6 +181,13 @@ cudaError_t launch_dic_shear(osog_ctx* c, int B, const float2* field, float2* ou
 {
     const dim3 grid((c->W + 255) / 256, c->H, B);
     k_dic_shear<<<grid, 256, 0, c->stream>>>(field, out, c->H, c->W, sx, sy, make_float2((float)cos(theta), (float)sin(theta)));
+    return cudaGetLastError();
+}
+
+cudaError_t launch_height_stencil(osog_ctx* c, int B, const float* d_h, double pitch, float* d_grad, float* d_lap)
+{
+    const dim3 grid((c->W + 255) / 256, c->H, B);
+    k_height_stencil<<<grid, 256, 0, c->stream>>>(d_h, c->H, c->W, (float)(1.0 / pitch), reinterpret_cast<float2*>(d_grad), d_lap);
     return cudaGetLastError();
 }
 

@@ -264,11 +264,11 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
 }
 
 static int render_common(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd,
-                         float2* d_field)
+                         float2* d_field, bool unit_dn = false)
 {
     DeviceGuard g(c->device);
     if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
-    cudaError_t e = launch_binning(c, p, N, o);
+    cudaError_t e = launch_binning(c, p, N, o, nullptr, unit_dn);
     if (e != cudaSuccess) return cuda_fail(c, e);
     const bool has_ramp = o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0;
     c->last_has_ramp = has_ramp ? 1 : 0;
@@ -370,6 +370,20 @@ int osog_particle_obbs(osog_ctx* c, const osog_particles* p, int64_t N, const os
     cudaError_t e = launch_binning(c, p, N, o, d_obb);   // k_prepare alone; the tile lists it leaves are not used
     if (e != cudaSuccess) return cuda_fail(c, e);        // (scratch_dirty stays set: the next render call clears them)
     c->last_has_ramp = -1;
+    return OSOG_OK;
+}
+
+int osog_render_height(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_h, float* d_grad,
+                       float* d_lap)
+{
+    int r = check_call(c, p, N, o, d_h);
+    if (r != OSOG_OK) return r;
+    if ((d_grad && !aligned16(d_grad)) || (d_lap && !aligned16(d_lap))) return OSOG_EINVAL;
+    if ((r = render_common(c, p, N, o, d_h, nullptr, true)) != OSOG_OK) return r;     // the hot path with unit index contrast
+    if (!d_grad && !d_lap) return OSOG_OK;
+    DeviceGuard g(c->device);
+    const cudaError_t e = launch_height_stencil(c, o->B, d_h, o->pitch_um, d_grad, d_lap);
+    if (e != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
 }
 

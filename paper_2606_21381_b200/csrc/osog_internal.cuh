@@ -112,7 +112,8 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 
 // binning.cu
 cudaError_t upload_optics(osog_ctx* c, const osog_optics* o, OpticsChunk* first);
-cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o, float* d_obb = nullptr);
+cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o, float* d_obb = nullptr,
+                           bool unit_dn = false);
 // compose.cu
 cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float* d_opd, float2* d_field, bool sort_first = true);
 cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd);
@@ -124,6 +125,7 @@ cudaError_t launch_pupil_fill(osog_ctx* c, int B, float2* spec, double pitch, bo
 cudaError_t launch_dic_shear(osog_ctx* c, int B, const float2* field, float2* out, int sx, int sy, double theta);
 cudaError_t launch_abs2(osog_ctx* c, int B, float2* buf, double scale);
 cudaError_t launch_cmul(osog_ctx* c, int B, float2* a, const float2* b, double scale);
+cudaError_t launch_height_stencil(osog_ctx* c, int B, const float* d_h, double pitch, float* d_grad, float* d_lap);
 cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_out, double sigma, uint64_t seed);
 cudaError_t launch_sensor(osog_ctx* c, int B, const float2* img, float* d_intensity, double sigma, uint64_t seed);
 
