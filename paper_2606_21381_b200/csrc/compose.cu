@@ -86,6 +86,28 @@ __device__ __forceinline__ float d2f_pos_trunc(double w)
     const int hi = max(__double2hiint(w) - 0x38000000, 0);
     return __uint_as_float(__funnelshift_l((unsigned)__double2loint(w), (unsigned)hi, 3));
 }
+// sin(pi x), cos(pi x) for |x| <= 1 (the reduced phase of the write-out, in half turns): k = nearest integer to 2 x,
+// r = x - k / 2 in [-1/4, 1/4], Taylor polynomials of sin(pi r) (through r^9) and cos(pi r) (through r^8): truncation
+// errors 2e-9 and 2.5e-8, far below the fp32 rounding of the result; then the quadrant rotation by k.
+__device__ __forceinline__ void sincospi_unit(float x, float* sn, float* cs)
+{
+    const float kf = rintf(x + x);
+    const int k = (int)kf;
+    const float r = fmaf(kf, -0.5f, x);
+    const float r2 = r * r;
+    float sp = fmaf(r2, 0.0821458866f, -0.599264529f);
+    sp = fmaf(r2, sp, 2.55016404f);
+    sp = fmaf(r2, sp, -5.16771278f);
+    sp = fmaf(r2, sp, 3.14159265f) * r;
+    float cp = fmaf(r2, 0.235330630f, -1.33526277f);
+    cp = fmaf(r2, cp, 4.05871213f);
+    cp = fmaf(r2, cp, -4.93480220f);
+    cp = fmaf(r2, cp, 1.0f);
+    if (k & 1) { const float t = sp; sp = cp; cp = -t; }
+    if (k & 2) { sp = -sp; cp = -cp; }
+    *sn = sp;
+    *cs = cp;
+}
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
 {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -522,7 +544,7 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
             double turns = acc[k] * inv_lambda;                  // Eq. 2: phase = 2 pi OPD / lambda, kept in turns
             turns -= rint(turns);
             float s, c;
-            sincospif(2.0f * (float)turns, &s, &c);
+            sincospi_unit(2.0f * (float)turns, &s, &c);
             if (RAMP && j + k < a.W) {
                 float2 r = a.ramp_x[(size_t)b * a.W + j + k];
                 if (a.ramp_y_on) r = make_float2(r.x * ry.x - r.y * ry.y, r.x * ry.y + r.y * ry.x);
