@@ -22,9 +22,11 @@
  *     without synchronising; outputs are valid once the caller has synchronised that stream.
  *   - All particle arrays and all output buffers are DEVICE pointers, caller-owned, 16-byte aligned.  The
  *     library reads the inputs, OVERWRITES the whole output (never accumulates into it) and owns only its own
- *     scratch, allocated in osog_create and freed in osog_destroy.  No allocation happens in a render call.
+ *     scratch, allocated in osog_create and freed in osog_destroy.  No allocation happens in a render call (one exception:
+ *     the first DIC call of a context, see osog_render_dic).
  *   - Results are bitwise reproducible from run to run: every pixel sums its particles in an order fixed by the
- *     data alone (sorted tile lists, walked in batches), never by thread scheduling.
+ *     data alone (sorted tile lists, walked in batches), never by thread scheduling (the two
+ *     *_atomic alternatives are the stated exceptions).
  *   - There is no CPU fallback and no backend dispatch: without a CUDA device osog_create fails.
  *   - Return value: 0 = OK, negative = error (see the enum).  Nothing is printed, nothing throws or aborts.
  *   - Particles with a non-finite parameter, a non-positive dimension or kind > 1 are skipped (they join no
