@@ -191,3 +191,32 @@ def test_context_reuse_with_changing_batch_size(og):
         assert ctx.status()[0] == 0
         assert torch.equal(got, want), sc.name
     ctx.close()
+
+
+def test_batch_with_unequal_and_empty_frames(og, o):
+    """Frames of 0, 57, 5 and 130 particles in one call: every frame equals the single-frame render of its own particles
+    (same bits), the empty frame is the particle-free frame, bins / OPD / field / intensity / depth maps match the oracle."""
+    import torch
+    from workloads import subset
+    H = W = 128
+    counts = [0, 57, 5, 130]
+    fs = np.concatenate([[0], np.cumsum(counts)])
+    cols = _mixed(int(fs[-1]), H, W, seed=77)
+    B = len(counts)
+    sc = make_scene("uneven", H, W, cols, frame_start=fs, lam=np.array([0.5, 0.55, 0.6, 0.45]), NA=np.array([0.4, 0.5, 0.6, 0.7]),
+                    tilt_x_rad=0.07)
+    g, _ = check_against_oracle(og, o, sc)
+    assert np.all(g["opd"][0] == 0.0) and np.allclose(np.abs(g["field"][0]), 1.0, atol=1e-6)
+    ctx = og.Context(H, W, sc.N, max_frames=B)
+    tid, dep = ctx.render_gbuffer(og.Particles.from_scene(sc), og.optics_from_scene(sc))
+    rid, rdep = o.render_gbuffer(sc)
+    assert (tid.cpu().numpy() != rid).mean() <= 1e-5 and np.all(tid.cpu().numpy()[0] == -1)
+    assert np.all(np.abs(dep.cpu().numpy() - rdep) <= 1e-6 + 2e-7 * np.abs(rdep))
+    batch = ctx.render_opd(og.Particles.from_scene(sc), og.optics_from_scene(sc)).clone()
+    ctx.close()
+    one = og.Context(H, W, sc.N)
+    for b in range(1, B):
+        sub = make_scene("one", H, W, {k: v[fs[b]:fs[b + 1]] for k, v in sc.cols.items()}, lam=sc.lambda_um[b], NA=sc.NA[b],
+                         tilt_x_rad=0.07)
+        assert torch.equal(one.render_opd(og.Particles.from_scene(sub), og.optics_from_scene(sub))[0], batch[b])
+    one.close()
