@@ -642,28 +642,6 @@ __global__ void __launch_bounds__(256) k_compose_atomic(const float* __restrict_
 }
 
 // ---- G-buffer extras (reading A24): depth map and instance-id map -----------------------------------
-// Chord of the vertical line through a prism, all in fp64 from the record (same plane data as prism_t64): false when
-// the chord has no positive length, else *z_exit = z of the exit point relative to the centre.
-__device__ __forceinline__ bool prism_exit64(const double* r64, uint32_t vmask, double dj, double di, double* z_exit)
-{
-    double ex = 1.0e300, en = -1.0e300;
-#pragma unroll
-    for (int q = 0; q < 6; ++q) {
-        const double2 uv = *reinterpret_cast<const double2*>(r64 + 4 * q);
-        const double2 xn = *reinterpret_cast<const double2*>(r64 + 4 * q + 2);
-        const double m = fma(uv.x, dj, uv.y * di);
-        if ((vmask >> q) & 1u) {
-            if (fabs(m + xn.x) > xn.y) return false;   // outside a vertical slab
-        } else {
-            const double e = xn.x - m, n = xn.y - m;
-            ex = e < ex ? e : ex;
-            en = n > en ? n : en;
-        }
-    }
-    *z_exit = ex;
-    return ex - en > 0.0;
-}
-
 // One CTA of 8 warps per tile, warp = 16 x 8 pixel sub-tile, lane = 4 x 1 pixels (the layout of the composition).  Every
 // warp walks the tile's sorted list, skips the entries whose sub-tile mask bit is clear, and for the others evaluates the
 // top of the chord in fp64 straight from the record: the decision "which particle is on top" is taken in the precision
@@ -698,21 +676,48 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
         if (czf + __int_as_float(h3.z) < floor_all) continue;
         const uint32_t flags = __float_as_uint(h2.x);
         const double* c = reinterpret_cast<const double*>(rec + 4);
-        const double di = (double)(i - h3.y);
+        const double di = (double)(i - h3.y), dj0 = (double)(j - h3.x);
+        double zx[4];
+        bool hit[4];
+        if (flags & kFlagPrism) {
+            // slab by slab for the lane's four pixels: coefficients loaded and the row term formed once per slab
+            const uint32_t vmask = flags >> 16;
+            double ex[4] = {1.0e300, 1.0e300, 1.0e300, 1.0e300}, en[4] = {-1.0e300, -1.0e300, -1.0e300, -1.0e300};
+            bool out[4] = {false, false, false, false};
+#pragma unroll
+            for (int sl = 0; sl < 6; ++sl) {
+                const double2 uv = *reinterpret_cast<const double2*>(c + 4 * sl);
+                const double2 xn = *reinterpret_cast<const double2*>(c + 4 * sl + 2);
+                const double r = uv.y * di;
+                if ((vmask >> sl) & 1u) {                        // vertical slab (warp-uniform branch)
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) out[q] = out[q] || fabs(fma(uv.x, dj0 + (double)q, r) + xn.x) > xn.y;
+                } else {
+                    const double cx = xn.x - r, cn = xn.y - r;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const double m = uv.x * (dj0 + (double)q);
+                        const double e = cx - m, n = cn - m;
+                        ex[q] = e < ex[q] ? e : ex[q];
+                        en[q] = n > en[q] ? n : en[q];
+                    }
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) { hit[q] = !out[q] && ex[q] - en[q] > 0.0; zx[q] = ex[q]; }
+        } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const double dj = dj0 + (double)q;
+                const double w = c[5] - fma(fma(c[0], dj, fma(c[1], di, c[3])), dj, fma(c[2], di, c[4]) * di);
+                hit[q] = w > 0.0;
+                zx[q] = fma(c[9], dj, fma(c[10], di, c[8])) + 0.5 * c[11] * sqrt(fmax(w, 0.0));
+            }
+        }
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            const double dj = (double)(j + q - h3.x);
-            double zx;
-            bool hit;
-            if (flags & kFlagPrism) {
-                hit = prism_exit64(c, flags >> 16, dj, di, &zx);
-            } else {
-                const double w = c[5] - fma(fma(c[0], dj, fma(c[1], di, c[3])), dj, fma(c[2], di, c[4]) * di);
-                hit = w > 0.0;
-                zx = fma(c[9], dj, fma(c[10], di, c[8])) + 0.5 * c[11] * sqrt(fmax(w, 0.0));
-            }
-            const double top = (double)czf + zx;
-            if (hit && (who[q] < 0 || top > best[q])) { best[q] = top; who[q] = (int32_t)(pid - first); }
+            const double top = (double)czf + zx[q];
+            if (hit[q] && (who[q] < 0 || top > best[q])) { best[q] = top; who[q] = (int32_t)(pid - first); }
         }
         // lowest top over the warp's 128 pixels, rounded down (-inf while some pixel has no owner)
         float lo = __int_as_float(0x7f800000);
