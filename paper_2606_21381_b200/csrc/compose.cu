@@ -165,20 +165,9 @@ __device__ __forceinline__ void rebase_item(float4* __restrict__ slot, const flo
     }
 }
 
-// ---- sub-tile cull ---------------------------------------------------------------------------------------------------------
-// Does the particle (header words 0..7: centre, oriented box, packed pixel bounding box) touch the 16 x 8 pixel
-// sub-tile with origin (sx0, sy0)?  Bounding-box overlap, then a separating-axis test against the oriented box of the
+// ---- sub-tile cull (tile_meta below): does the particle (header words 0..7: centre, oriented box, packed pixel bounding
+// box) touch a 16 x 8 pixel sub-tile?  Bounding-box overlap, then a separating-axis test against the oriented box of the
 // silhouette (which contains it by construction).
-__device__ __forceinline__ bool cull_subtile(const float4 h0, const float4 h1, int sx0, int sy0)
-{
-    const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
-    const int pj0 = bx & 0xffff, pj1 = bx >> 16, pi0 = by & 0xffff, pi1 = by >> 16;
-    const float axx = fabsf(h0.z), ayy = h0.w, ha = fabsf(h1.x), hb = fabsf(h1.y);
-    const float ddx = (float)sx0 + 7.5f - h0.x, ddy = (float)sy0 + 3.5f - h0.y;
-    const float pa = fabsf(ddx * axx + ddy * ayy), pb = fabsf(ddy * axx - ddx * ayy);
-    const float ra = 7.5f * axx + 3.5f * fabsf(ayy), rb = 7.5f * fabsf(ayy) + 3.5f * axx;
-    return pj0 <= sx0 + 15 && pj1 >= sx0 && pi0 <= sy0 + 7 && pi1 >= sy0 && pa <= ha + ra && pb <= hb + rb;
-}
 // evaluation code in the sign bits of the (positive) half lengths and of a_x (a_x >= 0 by construction)
 __device__ __forceinline__ uint32_t header_code(const float4 h0, const float4 h1)
 {
@@ -302,12 +291,30 @@ __device__ __forceinline__ void count_less(uint32_t& r, uint32_t a, uint32_t v)
     asm("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %1, %2;\n\t@p add.u32 %0, %0, 1;\n\t}" : "+r"(r) : "r"(a), "r"(v));
 }
 
+// All eight sub-tile tests of one list entry at once: sub-tile (wx, wy) has origin (x0 + 16 wx, y0 + 8 wy) and centre
+// offset (7.5, 3.5); it is kept iff its pixel range overlaps the particle's pixel bounding box and its centre's
+// projections on the two box axes are within half length + the sub-tile's own half extent along that axis.
 __device__ __forceinline__ uint32_t tile_meta(const float4 h0, const float4 h1, int tx, int ty)
 {
+    const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
+    const int pj0 = bx & 0xffff, pj1 = bx >> 16, pi0 = by & 0xffff, pi1 = by >> 16;
+    const int x0 = tx * kTile, y0 = ty * kTile;
+    const float axx = fabsf(h0.z), ayy = h0.w, ha = fabsf(h1.x), hb = fabsf(h1.y);
+    const float ta = ha + (7.5f * axx + 3.5f * fabsf(ayy)), tb = hb + (7.5f * fabsf(ayy) + 3.5f * axx);
+    const float ddx0 = (float)x0 + 7.5f - h0.x, ddy0 = (float)y0 + 3.5f - h0.y;
     uint32_t mask = 0;
 #pragma unroll
-    for (int w = 0; w < kWarps; ++w)
-        mask |= cull_subtile(h0, h1, tx * kTile + (w & 1) * 16, ty * kTile + (w >> 1) * 8) ? (1u << w) : 0u;
+    for (int wy = 0; wy < 4; ++wy) {
+        const bool row_ok = pi0 <= y0 + 8 * wy + 7 && pi1 >= y0 + 8 * wy;
+        const float ddy = ddy0 + (float)(8 * wy);
+#pragma unroll
+        for (int wx = 0; wx < 2; ++wx) {
+            const bool col_ok = pj0 <= x0 + 16 * wx + 15 && pj1 >= x0 + 16 * wx;
+            const float ddx = ddx0 + (float)(16 * wx);
+            const float pa = fabsf(ddx * axx + ddy * ayy), pb = fabsf(ddy * axx - ddx * ayy);
+            mask |= (row_ok && col_ok && pa <= ta && pb <= tb) ? (1u << (2 * wy + wx)) : 0u;
+        }
+    }
     return mask | (header_code(h0, h1) << 8);
 }
 
