@@ -16,6 +16,7 @@ Pieces, each following the passage it cites (line numbers are /root/reference/PA
   binning         bounding boxes -> tiles -> counts / offsets / ascending lists       DESIGN.md section 3 (B1-B4)
   particle_obbs   oriented bounding box of each silhouette (detector labels)          :76, :138-146, A23
   render_gbuffer  depth map and instance-id map (top-most particle per pixel), in C   :76, A24
+  backward_np     dL/dn_p = sum_px G t_n: adjoint of the OPD sum in the indices, in C   :124 (NEXT-3, first step)
   render_height / height_gradient / height_laplacian   h, grad h, lap h of the G-buffer :76, :92, :96-99, A25
 
 Every reading of the paper taken here (units, pixel centres, quaternion convention, pupil edge,
@@ -53,6 +54,9 @@ def _lib():
         lib.osog_oracle_render_gbuffer.restype = None
         lib.osog_oracle_chord.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double, dp, dp]
         lib.osog_oracle_chord.restype = ctypes.c_int
+        lib.osog_oracle_backward_np.argtypes = [ctypes.c_int64] + [fp] * 10 + [u8p] + [
+            ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int, fp, dp]
+        lib.osog_oracle_backward_np.restype = None
         lib.osog_oracle_thickness.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double]
         lib.osog_oracle_thickness.restype = ctypes.c_double
         lib.osog_oracle_circumradius.argtypes = [ctypes.c_uint8] + [ctypes.c_float] * 3
@@ -155,6 +159,30 @@ def render_gbuffer(scene, mode="bcircle"):
         ids.append(tid)
         deps.append(dep)
     return np.stack(ids), np.stack(deps)
+
+
+def backward_np(scene, G, mode="bcircle") -> np.ndarray:
+    """dL/dn_p [N] float64 for an upstream gradient G = dL/dOPD (float32 [B, H, W]): sum over the particle's frame of
+    G * thickness (the OPD sum is linear in n_p)."""
+    fs = scene.frame_start
+    f = ctypes.c_float
+    out = np.zeros(scene.N, dtype=np.float64)
+    G = np.ascontiguousarray(G, dtype=np.float32)
+    for b in range(scene.B):
+        lo, hi = int(fs[b]), int(fs[b + 1])
+        if hi == lo:
+            continue
+        a = {k: np.ascontiguousarray(scene.cols[k][lo:hi], dtype=np.float32) for k in _COLS}
+        kind = np.ascontiguousarray(scene.cols["kind"][lo:hi], dtype=np.uint8)
+        g = np.zeros(hi - lo, dtype=np.float64)
+        Gb = np.ascontiguousarray(G[b])
+        _lib().osog_oracle_backward_np(
+            hi - lo, _ptr(a["cx"], f), _ptr(a["cy"], f), _ptr(a["qw"], f), _ptr(a["qx"], f), _ptr(a["qy"], f),
+            _ptr(a["qz"], f), _ptr(a["d0"], f), _ptr(a["d1"], f), _ptr(a["d2"], f), _ptr(a["n_p"], f),
+            _ptr(kind, ctypes.c_uint8), scene.H, scene.W, float(scene.pitch_um),
+            {"full": 0, "bcircle": 1}[mode], _ptr(Gb, f), _ptr(g, ctypes.c_double))
+        out[lo:hi] = g
+    return out
 
 
 def count_covered(scene, mode="bcircle"):

@@ -322,3 +322,47 @@ void osog_oracle_render_gbuffer(int64_t N,
         }
     }
 }
+
+/* ---- first step of the backward pass ("the gradient of the final image with respect to
+ * the initial state tensor"): adjoint of the OPD sum with respect to the refractive indices.  OPD[px] = sum_n (n_p[n] -
+ * n_medium) t_n[px] is linear in n_p, so for an upstream gradient G = dL/dOPD (one frame, row-major [H*W]) the gradient
+ * is  dL/dn_p[n] = sum over pixels of G[px] * t_n[px]  (pixels in row-major order, fp64 sum).  Invalid particles get 0. */
+void osog_oracle_backward_np(int64_t N,
+                             const float *cx, const float *cy,
+                             const float *qw, const float *qx, const float *qy, const float *qz,
+                             const float *d0, const float *d1, const float *d2,
+                             const float *n_p, const uint8_t *kind,
+                             int H, int W, double pitch, int mode, const float *G, double *g_np)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t n = 0; n < N; ++n) {
+        g_np[n] = 0.0;
+        if (!osog_oracle_particle_valid(cx[n], cy[n], qw[n], qx[n], qy[n], qz[n],
+                                        d0[n], d1[n], d2[n], n_p[n], kind[n])) continue;
+        const double q[4] = { qw[n], qx[n], qy[n], qz[n] };
+        double R[9];
+        osog_oracle_rot_from_quat(q, R);
+        double Aw[OSOG_ORACLE_MAX_PLANES][3], b[OSOG_ORACLE_MAX_PLANES];
+        int M = 0;
+        if (kind[n] == 1) M = prism_world_planes(R, d0[n], d1[n], d2[n], Aw, b);
+        double r2 = INFINITY;
+        if (mode == 1) {
+            const double r = osog_oracle_circumradius(kind[n], d0[n], d1[n], d2[n]) * (1.0 + 1e-9);
+            r2 = r * r;
+        }
+        double acc = 0.0;
+        for (int i = 0; i < H; ++i) {
+            const double dy = (i + 0.5) * pitch - (double)cy[n];
+            if (dy * dy > r2) continue;
+            for (int j = 0; j < W; ++j) {
+                const double dx = (j + 0.5) * pitch - (double)cx[n];
+                if (dx * dx + dy * dy > r2) continue;
+                const double t = kind[n] == 0
+                    ? osog_oracle_thickness_ellipsoid(R, d0[n], d1[n], d2[n], dx, dy)
+                    : osog_oracle_thickness_polyhedron(M, Aw, b, dx, dy);
+                acc += (double)G[(size_t)i * W + j] * t;
+            }
+        }
+        g_np[n] = acc;
+    }
+}
