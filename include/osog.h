@@ -66,7 +66,8 @@ typedef struct {
     int64_t  max_particles;  /* largest N (total over the batch) of one call, >= 0                         */
     int64_t  max_pairs;      /* capacity of the (particle, tile) pair lists; 0 = 64 * max_particles + 1024.  It is
                                 divided evenly among the max_frames * ceil(H/T) * ceil(W/T) tiles of the context:
-                                one tile's list holds floor(max_pairs / tiles) entries (at least 1)               */
+                                one tile's list holds floor(max_pairs / tiles) entries (at least 1; with the default
+                                sizing max_pairs = 0 at least 64, so that few particles on a large frame still fit)    */
 } osog_config;
 
 /* Particle state, Structure of Arrays ("S in R^{N x D}"): one DEVICE array of length N per
@@ -168,6 +169,15 @@ int osog_render_height(osog_ctx* ctx, const osog_particles* p, int64_t N, const 
  * frame_start[b]; ties go to the smallest index; -1 = no particle); d_depth is DEVICE float [B, H, W]: the height of that
  * top surface in um (0 where d_top_id is -1).  Runs the binning, then one fp64 evaluation per listed (particle, pixel). */
 int osog_render_gbuffer(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, int32_t* d_top_id, float* d_depth);
+
+/* First step of the backward pass ("the gradient of the final image with respect to the initial state
+ * tensor"): the OPD frame is linear in the refractive indices, OPD = sum_n (n_p[n] - n_medium) t_n, so for an
+ * upstream gradient d_gopd = dL/dOPD (DEVICE float [B, H, W], read only) the gradient is
+ * d_gnp[n] = dL/dn_p[n] = sum over the pixels of the particle's frame of d_gopd * t_n  (DEVICE float [N], overwritten;
+ * 0 for invalid or off-canvas particles).  One warp per particle gathers over the particle's pixel bounding box in a fixed
+ * order (fp64 thickness and sum): reproducible bit for bit.  Gradients with respect to centre, rotation and dimensions are
+ * not implemented. */
+int osog_backward_np(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gnp);
 
 /* Second measured alternative: the same tile lists, but one CTA per tile accumulates the tile in SHARED memory with fp32
  * atomics (one warp per listed particle) and writes it out once.  NOT deterministic in the last bits, fp32 sum; kept for

@@ -73,6 +73,7 @@ def lib():
     L.osog_render_dic.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics),
                                   C.POINTER(osog_dic), C.c_void_p]
     L.osog_field_to_dic.argtypes = [ctx, C.POINTER(osog_optics), C.POINTER(osog_dic), C.c_void_p, C.c_void_p]
+    L.osog_backward_np.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_gbuffer.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_height.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p,
                                      C.c_void_p]
@@ -92,7 +93,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_debug_recompose_field", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_backward_np", "osog_debug_recompose_field", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -229,6 +230,14 @@ class Context:
         if r != OSOG_OK:
             raise OsogError(r, "osog_render_height")
         return h, g, l
+
+    def backward_np(self, p: Particles, o, gopd):
+        """float32 [N] dL/dn_p for an upstream gradient gopd = dL/dOPD (float32 [B, H, W]) (osog_backward_np)."""
+        out = self.torch.empty((p.N,), dtype=self.torch.float32, device=self.device)
+        r = lib().osog_backward_np(self._ctx, C.byref(p.c), p.N, C.byref(o), gopd.data_ptr(), out.data_ptr())
+        if r != OSOG_OK:
+            raise OsogError(r, "osog_backward_np")
+        return out
 
     def render_gbuffer(self, p: Particles, o):
         """(int32 [B, H, W] instance id of the top-most particle, float32 [B, H, W] height of its top surface)."""

@@ -831,6 +831,55 @@ cudaError_t launch_compose_smem_atomic(osog_ctx* c, int B, float* d_opd)
     return cudaGetLastError();
 }
 
+// ---- first step of the backward pass: dL/dn_p[n] = sum_px G[px] t_n[px] ----------------
+// The OPD sum is linear in n_p, so its adjoint in n_p is a gather: one warp per particle walks the particle's pixel
+// bounding box (thickness in fp64 from the record), lane q takes pixels q, q + 32, ... in row-major order of the box and
+// a shuffle tree adds the 32 partial sums: a fixed order, so the result is reproducible bit for bit.
+__global__ void __launch_bounds__(256) k_backward_np(const float* __restrict__ recs, const int4* __restrict__ tbox,
+                                                     const int* __restrict__ pframe, long long N, int H, int W,
+                                                     const float* __restrict__ gopd, float* __restrict__ gnp)
+{
+    const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (n >= N) return;
+    double acc = 0.0;
+    if (tbox[n].x <= tbox[n].y) {                                // listed: valid and on the canvas (else the gradient is 0)
+        const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)n * kRecWords);
+        const float4 h1 = rec[1], h2 = rec[2];
+        const int4 h3 = *reinterpret_cast<const int4*>(rec + 3);
+        const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
+        const int j0 = bx & 0xffff, j1 = bx >> 16, i0 = by & 0xffff, i1 = by >> 16;
+        const uint32_t flags = __float_as_uint(h2.x);
+        const double* c = reinterpret_cast<const double*>(rec + 4);
+        const int bw = j1 - j0 + 1, np = bw * (i1 - i0 + 1);
+        const float* g = gopd + (size_t)pframe[n] * H * W;
+        for (int q = lane; q < np; q += 32) {
+            const int i = i0 + q / bw, j = j0 + q % bw;
+            const double dj = (double)(j - h3.x), di = (double)(i - h3.y);
+            double t;
+            if (flags & kFlagPrism) {
+                t = prism_t64(c, flags >> 16, dj, di);
+            } else {
+                const double w = c[5] - fma(fma(c[0], dj, fma(c[1], di, c[3])), dj, fma(c[2], di, c[4]) * di);
+                t = c[11] * sqrt(fmax(w, 0.0));                  // T0 sqrt(w)
+            }
+            acc = fma((double)g[(size_t)i * W + j], t, acc);
+        }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+    if (lane == 0) gnp[n] = (float)acc;
+}
+
+cudaError_t launch_backward_np(osog_ctx* c, long long N, const float* d_gopd, float* d_gnp)
+{
+    if (N == 0) return cudaSuccess;
+    const long long threads = N * 32;
+    k_backward_np<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(c->rec, c->tbox, c->pframe, N, c->H, c->W, d_gopd,
+                                                                           d_gnp);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd)
 {
     cudaError_t e = cudaMemsetAsync(d_opd, 0, sizeof(float) * (size_t)B * c->H * c->W, c->stream);

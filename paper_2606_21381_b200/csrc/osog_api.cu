@@ -219,6 +219,7 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     {
         long long cap = c->max_pairs / c->max_tiles;
         if (cap < 1) cap = 1;
+        if (cfg->max_pairs == 0 && cap < 64) cap = 64;           // default sizing: never fewer than 64 entries per tile
         if (cap > 0x3fffffffll) cap = 0x3fffffffll;
         c->tile_cap = (int)cap;
     }
@@ -400,6 +401,21 @@ int osog_render_gbuffer(osog_ctx* c, const osog_particles* p, int64_t N, const o
     e = launch_gbuffer(c, o->B, o->B > 1 ? p->frame_start : nullptr, d_top_id, d_depth);
     if (e != cudaSuccess) return cuda_fail(c, e);
     c->scratch_dirty = false;
+    return OSOG_OK;
+}
+
+int osog_backward_np(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gnp)
+{
+    if (!d_gopd || !aligned16(d_gopd)) return OSOG_EINVAL;
+    if (N == 0) return (c && p && o) ? OSOG_OK : OSOG_EINVAL;
+    const int r = check_call(c, p, N, o, d_gnp);
+    if (r != OSOG_OK) return r;
+    DeviceGuard g(c->device);
+    cudaError_t e = launch_binning(c, p, N, o);      // records + bounding boxes (the tile lists are not used)
+    if (e != cudaSuccess) return cuda_fail(c, e);    // (scratch_dirty stays set: the next render call clears them)
+    c->last_has_ramp = -1;
+    e = launch_backward_np(c, N, d_gopd, d_gnp);
+    if (e != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
 }
 

@@ -1,0 +1,69 @@
+"""GPU parity of the first backward step (osog_backward_np: dL/dn_p) against the oracle, and against
+the GPU's own forward model differenced in n_p (the OPD sum is linear in it)."""
+import numpy as np
+import pytest
+
+from workloads import make_config
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def og():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2606_21381_b200 as m
+    m.lib()
+    return m
+
+
+@pytest.fixture(scope="module")
+def o():
+    from oracle import oracle
+    return oracle
+
+
+@pytest.mark.parametrize("k,n", [(1, None), (2, None), (3, 2000), (4, 4000), (5, 300)])
+def test_backward_np_matches_oracle(og, o, k, n):
+    import torch
+    sc = make_config(k, n_override=n)
+    rng = np.random.default_rng(k)
+    G = rng.standard_normal((sc.B, sc.H, sc.W)).astype(np.float32)
+    ctx = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B)
+    P, opt = og.Particles.from_scene(sc), og.optics_from_scene(sc)
+    Gd = torch.from_numpy(G).cuda()
+    g = ctx.backward_np(P, opt, Gd)
+    g2 = ctx.backward_np(P, opt, Gd)
+    assert torch.equal(g, g2)                                    # fixed summation order: same bits
+    g = g.cpu().numpy().astype(np.float64)
+    ref = o.backward_np(sc, G)
+    # float32 result of a float64 sum of up to ~1e4 terms of either sign: bar relative to the sum of magnitudes
+    scale = o.backward_np(sc, np.abs(G))
+    assert np.all(np.abs(g - ref) <= 2e-7 * scale + 1e-6), float(np.abs(g - ref).max())
+    # the context still renders the same bits afterwards
+    a = ctx.render_opd(P, opt).clone()
+    fresh = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B)
+    assert torch.equal(a, fresh.render_opd(P, opt))
+    fresh.close()
+    ctx.close()
+
+
+def test_backward_np_is_the_forward_model_differenced(og):
+    """L = sum G * OPD(n_p) rendered by the hot path (fp32 output): (L(n_p + d e_n) - L(n_p)) / d ~ dL/dn_p[n]."""
+    import torch
+    sc = make_config(4, n_override=200)
+    rng = np.random.default_rng(9)
+    G = torch.from_numpy(np.abs(rng.standard_normal((1, sc.H, sc.W))).astype(np.float32)).cuda()
+    ctx = og.Context(sc.H, sc.W, sc.N)
+    P, opt = og.Particles.from_scene(sc), og.optics_from_scene(sc)
+    g = ctx.backward_np(P, opt, G).cpu().numpy().astype(np.float64)
+    L0 = float((G.double() * ctx.render_opd(P, opt).double()).sum())
+    assert ctx.status()[0] == 0 and L0 > 0.0
+    for n in (3, 77, 150):
+        cols = dict(sc.cols)
+        npn = cols["n_p"].copy(); npn[n] += np.float32(0.5); cols["n_p"] = npn
+        P1 = og.Particles(cols, None)
+        L1 = float((G.double() * ctx.render_opd(P1, opt).double()).sum())
+        step = float(npn[n]) - float(sc.cols["n_p"][n])
+        assert abs((L1 - L0) / step - g[n]) <= 2e-4 * abs(g[n]) + 1e-3, (n, (L1 - L0) / step, g[n])
+    ctx.close()
