@@ -17,6 +17,7 @@ Pieces, each following the passage it cites (line numbers are /root/reference/PA
   particle_obbs   oriented bounding box of each silhouette (detector labels)          :76, :138-146, A23
   render_gbuffer  depth map and instance-id map (top-most particle per pixel), in C   :76, A24
   backward_np     dL/dn_p = sum_px G t_n: adjoint of the OPD sum in the indices, in C   :124 (NEXT-3, first step)
+  thickness_grad / backward_centre   grad t per pixel; dL/d(cx, cy) = -dn sum_px G grad t  :124 (NEXT-3, second step)
   render_height / height_gradient / height_laplacian   h, grad h, lap h of the G-buffer :76, :92, :96-99, A25
 
 Every reading of the paper taken here (units, pixel centres, quaternion convention, pupil edge,
@@ -57,6 +58,11 @@ def _lib():
         lib.osog_oracle_backward_np.argtypes = [ctypes.c_int64] + [fp] * 10 + [u8p] + [
             ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int, fp, dp]
         lib.osog_oracle_backward_np.restype = None
+        lib.osog_oracle_backward_centre.argtypes = [ctypes.c_int64] + [fp] * 10 + [u8p] + [
+            ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, fp, dp]
+        lib.osog_oracle_backward_centre.restype = None
+        lib.osog_oracle_thickness_grad.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double, dp]
+        lib.osog_oracle_thickness_grad.restype = None
         lib.osog_oracle_thickness.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double]
         lib.osog_oracle_thickness.restype = ctypes.c_double
         lib.osog_oracle_circumradius.argtypes = [ctypes.c_uint8] + [ctypes.c_float] * 3
@@ -180,6 +186,40 @@ def backward_np(scene, G, mode="bcircle") -> np.ndarray:
             hi - lo, _ptr(a["cx"], f), _ptr(a["cy"], f), _ptr(a["qw"], f), _ptr(a["qx"], f), _ptr(a["qy"], f),
             _ptr(a["qz"], f), _ptr(a["d0"], f), _ptr(a["d1"], f), _ptr(a["d2"], f), _ptr(a["n_p"], f),
             _ptr(kind, ctypes.c_uint8), scene.H, scene.W, float(scene.pitch_um),
+            {"full": 0, "bcircle": 1}[mode], _ptr(Gb, f), _ptr(g, ctypes.c_double))
+        out[lo:hi] = g
+    return out
+
+
+def thickness_grad(kind, q, dims, dx, dy):
+    """(dt/dx, dt/dy) of one particle's thickness at the offset (dx, dy) from its centre (0 where the chord is empty)."""
+    R = np.ascontiguousarray(rot_from_quat(q), dtype=np.float64).reshape(9)
+    d = np.ascontiguousarray(dims, dtype=np.float64)
+    g = np.zeros(2, dtype=np.float64)
+    _lib().osog_oracle_thickness_grad(int(kind), _ptr(R, ctypes.c_double), _ptr(d, ctypes.c_double), float(dx), float(dy),
+                                      _ptr(g, ctypes.c_double))
+    return float(g[0]), float(g[1])
+
+
+def backward_centre(scene, G, mode="bcircle") -> np.ndarray:
+    """dL/d(cx, cy) [N, 2] float64 for an upstream gradient G = dL/dOPD (float32 [B, H, W]):
+    -(n_p - n_medium) * sum over the particle's frame of G * grad t."""
+    fs = scene.frame_start
+    f = ctypes.c_float
+    out = np.zeros((scene.N, 2), dtype=np.float64)
+    G = np.ascontiguousarray(G, dtype=np.float32)
+    for b in range(scene.B):
+        lo, hi = int(fs[b]), int(fs[b + 1])
+        if hi == lo:
+            continue
+        a = {k: np.ascontiguousarray(scene.cols[k][lo:hi], dtype=np.float32) for k in _COLS}
+        kind = np.ascontiguousarray(scene.cols["kind"][lo:hi], dtype=np.uint8)
+        g = np.zeros((hi - lo, 2), dtype=np.float64)
+        Gb = np.ascontiguousarray(G[b])
+        _lib().osog_oracle_backward_centre(
+            hi - lo, _ptr(a["cx"], f), _ptr(a["cy"], f), _ptr(a["qw"], f), _ptr(a["qx"], f), _ptr(a["qy"], f),
+            _ptr(a["qz"], f), _ptr(a["d0"], f), _ptr(a["d1"], f), _ptr(a["d2"], f), _ptr(a["n_p"], f),
+            _ptr(kind, ctypes.c_uint8), scene.H, scene.W, float(scene.pitch_um), float(scene.n_medium),
             {"full": 0, "bcircle": 1}[mode], _ptr(Gb, f), _ptr(g, ctypes.c_double))
         out[lo:hi] = g
     return out

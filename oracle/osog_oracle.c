@@ -366,3 +366,89 @@ void osog_oracle_backward_np(int64_t N,
         g_np[n] = acc;
     }
 }
+
+/* Gradient of the thickness with respect to the ray's lateral position (dx, dy) (equivalently minus the gradient with
+ * respect to the particle's centre).  Ellipsoid: t = 2 sqrt(disc) / A with disc = Bq^2 - A C, so
+ *   dt/dx = (d disc / dx) / (A sqrt(disc)),  d disc / dx = 2 Bq M_xz - 2 A (M_xx dx + M_xy dy)   (likewise y);
+ * polyhedron: t = exit - enter with exit = g_e / n_ez on the active exit plane e (the arg min) and enter on the active
+ * entry plane f (the arg max), g = b - n_x dx - n_y dy, so dt/dx = -n_ex / n_ez + n_fx / n_fz  (likewise y).
+ * Where the chord is empty the gradient is 0.  (At the measure-zero set where two planes tie the first one is taken.) */
+void osog_oracle_thickness_grad(uint8_t kind, const double R[9], const double dims[3], double dx, double dy, double grad[2])
+{
+    grad[0] = grad[1] = 0.0;
+    if (kind == 0) {
+        const double D[3] = { 1.0 / (dims[0] * dims[0]), 1.0 / (dims[1] * dims[1]), 1.0 / (dims[2] * dims[2]) };
+        double M[9];
+        for (int r = 0; r < 3; ++r)
+            for (int s = 0; s < 3; ++s) {
+                double acc = 0.0;
+                for (int k = 0; k < 3; ++k) acc += R[3 * r + k] * D[k] * R[3 * s + k];
+                M[3 * r + s] = acc;
+            }
+        const double A  = M[8];
+        const double Bq = M[2] * dx + M[5] * dy;
+        const double C  = M[0] * dx * dx + 2.0 * M[1] * dx * dy + M[4] * dy * dy - 1.0;
+        const double disc = Bq * Bq - A * C;
+        if (!(disc > 0.0)) return;
+        const double sq = sqrt(disc);
+        grad[0] = (2.0 * Bq * M[2] - 2.0 * A * (M[0] * dx + M[1] * dy)) / (A * sq);
+        grad[1] = (2.0 * Bq * M[5] - 2.0 * A * (M[1] * dx + M[4] * dy)) / (A * sq);
+        return;
+    }
+    double Aw[OSOG_ORACLE_MAX_PLANES][3], b[OSOG_ORACLE_MAX_PLANES];
+    const int M = prism_world_planes(R, dims[0], dims[1], dims[2], Aw, b);
+    double enter = -INFINITY, exit_ = INFINITY;
+    int ke = -1, kf = -1;
+    for (int k = 0; k < M; ++k) {
+        const double g = b[k] - Aw[k][0] * dx - Aw[k][1] * dy;
+        const double nz = Aw[k][2];
+        if (nz > 0.0)      { const double z = g / nz; if (z < exit_) { exit_ = z; ke = k; } }
+        else if (nz < 0.0) { const double z = g / nz; if (z > enter) { enter = z; kf = k; } }
+        else if (g < 0.0)  return;
+    }
+    if (!(exit_ - enter > 0.0)) return;
+    grad[0] = -Aw[ke][0] / Aw[ke][2] + Aw[kf][0] / Aw[kf][2];
+    grad[1] = -Aw[ke][1] / Aw[ke][2] + Aw[kf][1] / Aw[kf][2];
+}
+
+/* Second step of the backward pass: dL/d(cx, cy)[n] = -(n_p[n] - n_medium) * sum over pixels of G[px] * grad t_n[px]
+ * (the thickness depends on the pixel position minus the centre).  g_c is [N][2]. */
+void osog_oracle_backward_centre(int64_t N,
+                                 const float *cx, const float *cy,
+                                 const float *qw, const float *qx, const float *qy, const float *qz,
+                                 const float *d0, const float *d1, const float *d2,
+                                 const float *n_p, const uint8_t *kind,
+                                 int H, int W, double pitch, double n_medium, int mode, const float *G, double *g_c)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t n = 0; n < N; ++n) {
+        g_c[2 * n] = g_c[2 * n + 1] = 0.0;
+        if (!osog_oracle_particle_valid(cx[n], cy[n], qw[n], qx[n], qy[n], qz[n],
+                                        d0[n], d1[n], d2[n], n_p[n], kind[n])) continue;
+        const double q[4] = { qw[n], qx[n], qy[n], qz[n] };
+        const double dims[3] = { d0[n], d1[n], d2[n] };
+        double R[9];
+        osog_oracle_rot_from_quat(q, R);
+        double r2 = INFINITY;
+        if (mode == 1) {
+            const double r = osog_oracle_circumradius(kind[n], d0[n], d1[n], d2[n]) * (1.0 + 1e-9);
+            r2 = r * r;
+        }
+        double ax = 0.0, ay = 0.0;
+        for (int i = 0; i < H; ++i) {
+            const double dy = (i + 0.5) * pitch - (double)cy[n];
+            if (dy * dy > r2) continue;
+            for (int j = 0; j < W; ++j) {
+                const double dx = (j + 0.5) * pitch - (double)cx[n];
+                if (dx * dx + dy * dy > r2) continue;
+                double gr[2];
+                osog_oracle_thickness_grad(kind[n], R, dims, dx, dy, gr);
+                ax += (double)G[(size_t)i * W + j] * gr[0];
+                ay += (double)G[(size_t)i * W + j] * gr[1];
+            }
+        }
+        const double dn = (double)n_p[n] - n_medium;
+        g_c[2 * n] = -dn * ax;
+        g_c[2 * n + 1] = -dn * ay;
+    }
+}

@@ -55,3 +55,77 @@ def test_B3_linear_in_the_upstream_gradient_and_per_frame():
     g3 = o.backward_np(sc, G3)
     fs = sc.frame_start
     assert np.all(g3[fs[1]:] == 0.0) and np.array_equal(g3[:fs[1]], a[:fs[1]])
+
+
+# ---- gradient of the thickness in the lateral position, and dL/d(centre) -----------------------------------------------------
+def _rq(rng):
+    q = rng.standard_normal(4)
+    q /= np.linalg.norm(q)
+    return q.astype(np.float32).astype(np.float64)
+
+
+def test_B4_thickness_gradient_closed_forms():
+    # sphere: t = 2 sqrt(R^2 - r^2)  =>  grad t = -2 d / sqrt(R^2 - r^2); outside: 0
+    R = 1.7
+    for dx, dy in ((0.0, 0.0), (0.4, -0.9), (-1.2, 0.7)):
+        gx, gy = o.thickness_grad(0, [1, 0, 0, 0], [R, R, R], dx, dy)
+        s = np.sqrt(R * R - dx * dx - dy * dy)
+        assert abs(gx + 2 * dx / s) < 1e-12 and abs(gy + 2 * dy / s) < 1e-12
+    assert o.thickness_grad(0, [1, 0, 0, 0], [R, R, R], 1.5, 1.0) == (0.0, 0.0)
+    # prism, identity rotation: t = L + 2 hc (1 - max(|dx|, |dy|) / (s/2))  =>  slope -+ 2 hc / (s/2) along the dominant axis
+    s, L, hc = 1.2, 3.0, 0.5
+    k = 2 * hc / (s / 2)
+    assert np.allclose(o.thickness_grad(1, [1, 0, 0, 0], [s, L, hc], 0.3, 0.1), (-k, 0.0), atol=1e-12)
+    assert np.allclose(o.thickness_grad(1, [1, 0, 0, 0], [s, L, hc], -0.3, 0.1), (k, 0.0), atol=1e-12)
+    assert np.allclose(o.thickness_grad(1, [1, 0, 0, 0], [s, L, hc], 0.1, -0.4), (0.0, k), atol=1e-12)
+    assert o.thickness_grad(1, [1, 0, 0, 0], [s, L, hc], 0.7, 0.0) == (0.0, 0.0)
+
+
+def test_B5_thickness_gradient_is_the_pinned_thickness_differenced():
+    """Central differences of the (pinned) thickness function, away from the silhouette and from face edges: the prism is
+    piecewise linear (exact up to rounding), the ellipsoid smooth (O(h^2))."""
+    rng = np.random.default_rng(12)
+    h = 1e-5
+    checked = 0
+    for kind in (0, 1):
+        for _ in range(300):
+            q, dims = _rq(rng), rng.uniform(0.6, 3.0, 3)
+            dx, dy = rng.uniform(-1.5, 1.5, 2)
+            t0 = o.thickness(kind, q, dims, dx, dy)
+            if t0 < 0.2:
+                continue
+            fx = (o.thickness(kind, q, dims, dx + h, dy) - o.thickness(kind, q, dims, dx - h, dy)) / (2 * h)
+            fy = (o.thickness(kind, q, dims, dx, dy + h) - o.thickness(kind, q, dims, dx, dy - h)) / (2 * h)
+            # skip points within h of a face edge of the prism (the slope jumps there): detected by a second difference
+            if kind == 1:
+                sx = o.thickness(kind, q, dims, dx + h, dy) + o.thickness(kind, q, dims, dx - h, dy) - 2 * t0
+                sy = o.thickness(kind, q, dims, dx, dy + h) + o.thickness(kind, q, dims, dx, dy - h) - 2 * t0
+                if abs(sx) > 1e-9 or abs(sy) > 1e-9:
+                    continue
+            gx, gy = o.thickness_grad(kind, q, dims, dx, dy)
+            assert abs(gx - fx) <= 1e-6 * max(1.0, abs(gx)) and abs(gy - fy) <= 1e-6 * max(1.0, abs(gy)), (kind, gx, fx, gy, fy)
+            checked += 1
+    assert checked > 300
+
+
+def test_B6_backward_centre_sums_the_pixel_gradients_and_matches_a_shifted_render():
+    rng = np.random.default_rng(3)
+    sc = make_config(4, n_override=12)
+    G = rng.standard_normal((1, sc.H, sc.W)).astype(np.float32)
+    gc = o.backward_centre(sc, G)
+    assert np.array_equal(gc, o.backward_centre(sc, G, mode="full"))
+    # one prism (piecewise linear thickness): L(cx + d) - L(cx - d) over 2 d with the oracle's own forward render; the
+    # silhouette and the face edges sweep over a few pixel centres during the shift, so the agreement is to ~1e-3 only
+    n = int(np.nonzero(sc.cols["kind"] == 1)[0][0])
+    one = subset(sc, [n])
+    g1 = o.backward_centre(one, G)[0]
+    assert np.allclose(g1, gc[n], rtol=1e-12, atol=1e-12)
+    d = 2.0 ** -12                                                # exactly representable shift of the float32 centre
+    for axis, key in ((0, "cx"), (1, "cy")):
+        Ls = []
+        for sgn in (+1, -1):
+            cols = dict(one.cols); c = cols[key].copy(); c[0] = np.float32(c[0] + sgn * d); cols[key] = c
+            Ls.append(float((G.astype(np.float64) * o.render_opd(replace(one, cols=cols))).sum()))
+        fd = (Ls[0] - Ls[1]) / (2 * d)
+        scale = float(np.abs(G).max()) * 50.0
+        assert abs(fd - g1[axis]) <= 2e-2 * max(abs(g1[axis]), scale), (fd, g1[axis])
