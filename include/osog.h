@@ -175,9 +175,16 @@ int osog_render_gbuffer(osog_ctx* ctx, const osog_particles* p, int64_t N, const
  * upstream gradient d_gopd = dL/dOPD (DEVICE float [B, H, W], read only) the gradient is
  * d_gnp[n] = dL/dn_p[n] = sum over the pixels of the particle's frame of d_gopd * t_n  (DEVICE float [N], overwritten;
  * 0 for invalid or off-canvas particles).  One warp per particle gathers over the particle's pixel bounding box in a fixed
- * order (fp64 thickness and sum): reproducible bit for bit.  Gradients with respect to centre, rotation and dimensions are
- * not implemented. */
+ * order (fp64 thickness and sum): reproducible bit for bit. */
 int osog_backward_np(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gnp);
+
+/* Second step of the backward pass: gradient in the particle centres.  The thickness depends on (pixel position - centre),
+ * so d_gc[n] = (dL/dcx[n], dL/dcy[n]) = -(n_p[n] - n_medium) * sum over the pixels of d_gopd * grad t_n, DEVICE float [N, 2]
+ * in 1/um, overwritten (0 for invalid or off-canvas particles).  grad t is analytic: the slopes of the active exit and
+ * entry faces of a prism, T0 grad w / (2 sqrt w) for an ellipsoid (it grows like 1 / sqrt(w) towards the ellipsoid's
+ * outline: the sum over pixel centres is finite but dominated by the outline pixels).  Same fixed-order fp64 gather as
+ * osog_backward_np.  Gradients with respect to rotation and dimensions are not implemented. */
+int osog_backward_centre(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gc);
 
 /* Second measured alternative: the same tile lists, but one CTA per tile accumulates the tile in SHARED memory with fp32
  * atomics (one warp per listed particle) and writes it out once.  NOT deterministic in the last bits, fp32 sum; kept for

@@ -871,6 +871,89 @@ __global__ void __launch_bounds__(256) k_backward_np(const float* __restrict__ r
     if (lane == 0) gnp[n] = (float)acc;
 }
 
+// Gradient of a prism's thickness in the pixel offsets (dj, di), fp64 from the record: t = exit - enter on the active
+// planes (arg min / arg max), exit_k = Cx_k - U_k dj - V_k di, so dt/ddj = -(U_e - U_f), dt/ddi = -(V_e - V_f); 0 where
+// the chord is empty.
+__device__ __forceinline__ void prism_grad64(const double* r64, uint32_t vmask, double dj, double di, double* gj, double* gi)
+{
+    double ex = 1.0e300, en = -1.0e300, ue = 0.0, ve = 0.0, uf = 0.0, vf = 0.0;
+    bool out = false;
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+        const double2 uv = *reinterpret_cast<const double2*>(r64 + 4 * q);
+        const double2 xn = *reinterpret_cast<const double2*>(r64 + 4 * q + 2);
+        const double m = fma(uv.x, dj, uv.y * di);
+        if ((vmask >> q) & 1u) {
+            out = out || fabs(m + xn.x) > xn.y;
+        } else {
+            const double e = xn.x - m, n = xn.y - m;
+            if (e < ex) { ex = e; ue = uv.x; ve = uv.y; }
+            if (n > en) { en = n; uf = uv.x; vf = uv.y; }
+        }
+    }
+    const bool hit = !out && ex - en > 0.0;
+    *gj = hit ? uf - ue : 0.0;
+    *gi = hit ? vf - ve : 0.0;
+}
+
+// Second step: dL/d(cx, cy)[n] = -(n_p - n_m) sum_px G[px] grad t_n[px].  Same gather as k_backward_np; the gradient in
+// um^-1 is the gradient in pixel offsets divided by the pitch.  Ellipsoid: t = T0 sqrt(w), w the record's quadratic,
+// grad t = T0 grad w / (2 sqrt(w)).  record word 9 holds dn (prism) or dn T0 (ellipsoid).
+__global__ void __launch_bounds__(256) k_backward_centre(const float* __restrict__ recs, const int4* __restrict__ tbox,
+                                                         const int* __restrict__ pframe, long long N, int H, int W,
+                                                         double inv_pitch, const float* __restrict__ gopd,
+                                                         float2* __restrict__ gc)
+{
+    const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (n >= N) return;
+    double ax = 0.0, ay = 0.0, scale = 0.0;
+    if (tbox[n].x <= tbox[n].y) {
+        const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)n * kRecWords);
+        const float4 h1 = rec[1], h2 = rec[2];
+        const int4 h3 = *reinterpret_cast<const int4*>(rec + 3);
+        const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
+        const int j0 = bx & 0xffff, j1 = bx >> 16, i0 = by & 0xffff, i1 = by >> 16;
+        const uint32_t flags = __float_as_uint(h2.x);
+        const double* c = reinterpret_cast<const double*>(rec + 4);
+        const int bw = j1 - j0 + 1, np = bw * (i1 - i0 + 1);
+        const float* g = gopd + (size_t)pframe[n] * H * W;
+        scale = -(double)h2.y * inv_pitch;                       // -dn / p  (ellipsoid: -dn T0 / p, T0 folded in below)
+        for (int q = lane; q < np; q += 32) {
+            const int i = i0 + q / bw, j = j0 + q % bw;
+            const double dj = (double)(j - h3.x), di = (double)(i - h3.y);
+            double gj, gi;
+            if (flags & kFlagPrism) {
+                prism_grad64(c, flags >> 16, dj, di, &gj, &gi);
+            } else {
+                const double w = c[5] - fma(fma(c[0], dj, fma(c[1], di, c[3])), dj, fma(c[2], di, c[4]) * di);
+                const double r = w > 0.0 ? 0.5 * rsqrt(w) : 0.0;  // (the record's K = dn T0 supplies T0)
+                gj = -(2.0 * c[0] * dj + c[1] * di + c[3]) * r;
+                gi = -(c[1] * dj + 2.0 * c[2] * di + c[4]) * r;
+            }
+            const double gv = (double)g[(size_t)i * W + j];
+            ax = fma(gv, gj, ax);
+            ay = fma(gv, gi, ay);
+        }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        ax += __shfl_xor_sync(0xffffffffu, ax, d);
+        ay += __shfl_xor_sync(0xffffffffu, ay, d);
+    }
+    if (lane == 0) gc[n] = make_float2((float)(scale * ax), (float)(scale * ay));
+}
+
+cudaError_t launch_backward_centre(osog_ctx* c, long long N, double pitch, const float* d_gopd, float* d_gc)
+{
+    if (N == 0) return cudaSuccess;
+    const long long threads = N * 32;
+    k_backward_centre<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(c->rec, c->tbox, c->pframe, N, c->H, c->W,
+                                                                               1.0 / pitch, d_gopd,
+                                                                               reinterpret_cast<float2*>(d_gc));
+    return cudaGetLastError();
+}
+
 cudaError_t launch_backward_np(osog_ctx* c, long long N, const float* d_gopd, float* d_gnp)
 {
     if (N == 0) return cudaSuccess;

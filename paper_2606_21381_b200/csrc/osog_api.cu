@@ -419,6 +419,21 @@ int osog_backward_np(osog_ctx* c, const osog_particles* p, int64_t N, const osog
     return OSOG_OK;
 }
 
+int osog_backward_centre(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gc)
+{
+    if (!d_gopd || !aligned16(d_gopd)) return OSOG_EINVAL;
+    if (N == 0) return (c && p && o) ? OSOG_OK : OSOG_EINVAL;
+    const int r = check_call(c, p, N, o, d_gc);
+    if (r != OSOG_OK) return r;
+    DeviceGuard g(c->device);
+    cudaError_t e = launch_binning(c, p, N, o);      // records + bounding boxes (the tile lists are not used)
+    if (e != cudaSuccess) return cuda_fail(c, e);    // (scratch_dirty stays set: the next render call clears them)
+    c->last_has_ramp = -1;
+    e = launch_backward_centre(c, N, o->pitch_um, d_gopd, d_gc);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return OSOG_OK;
+}
+
 int osog_render_opd_smem_atomic(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd)
 {
     const int r = check_call(c, p, N, o, d_opd);

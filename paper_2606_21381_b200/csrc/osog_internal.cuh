@@ -119,6 +119,7 @@ cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float
 cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd);
 cudaError_t launch_compose_smem_atomic(osog_ctx* c, int B, float* d_opd);
 cudaError_t launch_backward_np(osog_ctx* c, long long N, const float* d_gopd, float* d_gnp);
+cudaError_t launch_backward_centre(osog_ctx* c, long long N, double pitch, const float* d_gopd, float* d_gc);
 cudaError_t launch_gbuffer(osog_ctx* c, int B, const int32_t* d_frame_start, int32_t* d_top_id, float* d_depth);
 // optics.cu
 cudaError_t launch_pupil(osog_ctx* c, int B, float2* spec, double pitch, bool defocus);

@@ -67,3 +67,25 @@ def test_backward_np_is_the_forward_model_differenced(og):
         step = float(npn[n]) - float(sc.cols["n_p"][n])
         assert abs((L1 - L0) / step - g[n]) <= 2e-4 * abs(g[n]) + 1e-3, (n, (L1 - L0) / step, g[n])
     ctx.close()
+
+
+@pytest.mark.parametrize("k,n", [(1, None), (2, None), (3, 2000), (4, 4000), (5, 300)])
+def test_backward_centre_matches_oracle(og, o, k, n):
+    import torch
+    sc = make_config(k, n_override=n)
+    rng = np.random.default_rng(20 + k)
+    G = rng.standard_normal((sc.B, sc.H, sc.W)).astype(np.float32)
+    ctx = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B)
+    P, opt = og.Particles.from_scene(sc), og.optics_from_scene(sc)
+    Gd = torch.from_numpy(G).cuda()
+    g = ctx.backward_centre(P, opt, Gd)
+    assert torch.equal(g, ctx.backward_centre(P, opt, Gd))      # fixed summation order: same bits
+    g = g.cpu().numpy().astype(np.float64)
+    ref = o.backward_centre(sc, G)
+    # both sides sum in float64; what is left is the float32 rounding of the result (measured: 8e-8 of the scale below)
+    # and, near an ellipsoid's outline where grad t ~ 1 / sqrt(w), the ~1e-9 relative difference of the two formulas for w
+    scale = np.abs(o.backward_centre(sc, np.abs(G))) + np.abs(ref)
+    big = np.maximum(scale.max(axis=1, keepdims=True), 1.0)
+    err = np.abs(g - ref)
+    assert np.all(err <= 5e-7 * big), float((err / big).max())
+    ctx.close()
