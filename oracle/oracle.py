@@ -17,6 +17,7 @@ Pieces, each following the passage it cites (line numbers are /root/reference/PA
   particle_obbs   oriented bounding box of each silhouette (detector labels)          :76, :138-146, A23
   render_gbuffer  depth map and instance-id map (top-most particle per pixel), in C   :76, A24
   backward_np     dL/dn_p = sum_px G t_n: adjoint of the OPD sum in the indices, in C   :124 (NEXT-3, first step)
+  backward_intensity   dL/dOPD from dL/dI: adjoint of field + pupil + |.|^2                :124 (NEXT-3)
   thickness_grad / backward_centre   grad t per pixel; dL/d(cx, cy) = -dn sum_px G grad t  :124 (NEXT-3, second step)
   render_height / height_gradient / height_laplacian   h, grad h, lap h of the G-buffer :76, :92, :96-99, A25
 
@@ -189,6 +190,28 @@ def backward_np(scene, G, mode="bcircle") -> np.ndarray:
             {"full": 0, "bcircle": 1}[mode], _ptr(Gb, f), _ptr(g, ctypes.c_double))
         out[lo:hi] = g
     return out
+
+
+def backward_intensity(scene, G_I, U=None, pupil_enabled=True, mode="bcircle") -> np.ndarray:
+    """Adjoint of the optics stage: for an upstream gradient G_I = dL/dI (real,
+    [B, H, W]) of the coherent intensity I = |V|^2, V = U * h_obj = ifft2(fft2(U) P), U = exp(i 2 pi OPD / lambda) ramp,
+    returns dL/dOPD [B, H, W] float64:
+        g_V = G_I V                      (dL = 2 Re sum conj(g_V) dV)
+        g_U = ifft2(conj(P) fft2(g_V))   (adjoint of the linear map U -> V)
+        dL/dOPD = (4 pi / lambda) Im(g_U conj(U))      (dU = i (2 pi / lambda) U dOPD)
+    The additive read noise has no gradient."""
+    if U is None:
+        U = render_field(scene, mode=mode)
+    dz = float(getattr(scene, "defocus_um", 0.0))
+    out = []
+    for b in range(scene.B):
+        lam = float(scene.lambda_um[b])
+        P = pupil_function(scene.H, scene.W, float(scene.NA[b]), scene.pitch_um, lam, scene.n_medium, dz, pupil_enabled)
+        V = np.fft.ifft2(np.fft.fft2(U[b]) * P)
+        gV = np.asarray(G_I[b], dtype=np.float64) * V
+        gU = np.fft.ifft2(np.conj(P) * np.fft.fft2(gV))
+        out.append((4.0 * np.pi / lam) * np.imag(gU * np.conj(U[b])))
+    return np.stack(out)
 
 
 def thickness_grad(kind, q, dims, dx, dy):

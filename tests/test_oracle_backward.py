@@ -129,3 +129,32 @@ def test_B6_backward_centre_sums_the_pixel_gradients_and_matches_a_shifted_rende
         fd = (Ls[0] - Ls[1]) / (2 * d)
         scale = float(np.abs(G).max()) * 50.0
         assert abs(fd - g1[axis]) <= 2e-2 * max(abs(g1[axis]), scale), (fd, g1[axis])
+
+
+def test_B7_adjoint_of_the_optics_stage_is_the_forward_model_differenced():
+    """L = sum W I with random weights W: dL/dOPD[px] from backward_intensity equals (L(OPD + d e_px) - L(OPD - d e_px)) / 2d
+    computed with the oracle's own forward functions (field, pupil, intensity), with and without defocus and ramp."""
+    rng = np.random.default_rng(21)
+    H, W_ = 24, 32
+    lam, p = 0.55, 0.1
+    for dz, tilt, NA in ((0.0, 0.0, 1.2), (1.3, 0.08, 1.0)):
+        opd = rng.uniform(0.0, 0.8, (H, W_))
+        Wt = rng.standard_normal((H, W_))
+        P = o.pupil_function(H, W_, NA, p, lam, 1.33, dz)
+        assert 10 < (np.abs(P) > 0).sum() < H * W_
+
+        def L(opd_):
+            return float((Wt * o.intensity(o.field(opd_, lam, p, tilt, 0.0), P)).sum())
+
+        sc = make_scene("adj", H, W_, dict(cx=[], cy=[], d0=[], d1=[], d2=[], n_p=[]), lam=lam, NA=NA, tilt_x_rad=tilt,
+                        defocus_um=dz)
+        U = o.field(opd, lam, p, tilt, 0.0)[None]
+        g = o.backward_intensity(sc, Wt[None], U=U)[0]
+        d = 1e-6
+        for (i, j) in ((0, 0), (5, 7), (23, 31), (11, 16), (2, 30)):
+            e = np.zeros_like(opd); e[i, j] = d
+            fd = (L(opd + e) - L(opd - e)) / (2 * d)
+            assert abs(fd - g[i, j]) <= 1e-6 * max(1.0, abs(g[i, j])), (dz, i, j, fd, g[i, j])
+    # all-pass pupil: I == 1 whatever the OPD, so every gradient vanishes
+    sc0 = replace(sc, defocus_um=0.0)
+    assert np.abs(o.backward_intensity(sc0, Wt[None], U=U, pupil_enabled=False)).max() < 1e-12
