@@ -170,6 +170,13 @@ int osog_render_height(osog_ctx* ctx, const osog_particles* p, int64_t N, const 
  * top surface in um (0 where d_top_id is -1).  Runs the binning, then one fp64 evaluation per listed (particle, pixel). */
 int osog_render_gbuffer(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, int32_t* d_top_id, float* d_depth);
 
+/* Adjoint of the optics stage: d_gI = dL/dI (DEVICE float [B, H, W], read only) is an upstream
+ * gradient of the coherent intensity of osog_render_intensity (noise-free part); d_gopd (DEVICE float [B, H, W], overwritten)
+ * receives dL/dOPD = (4 pi / lambda) Im(g_U conj(U)), g_U = F^-1{conj(P) F{d_gI V}}, V = U * h_obj.  Runs the hot path for U,
+ * then 4 cuFFTs and 4 element-wise passes; the result feeds osog_backward_np / osog_backward_centre.  The first call
+ * allocates one more complex frame batch (shared with the DIC path). */
+int osog_backward_intensity(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gI, float* d_gopd);
+
 /* First step of the backward pass ("the gradient of the final image with respect to the initial state
  * tensor"): the OPD frame is linear in the refractive indices, OPD = sum_n (n_p[n] - n_medium) t_n, so for an
  * upstream gradient d_gopd = dL/dOPD (DEVICE float [B, H, W], read only) the gradient is
@@ -182,7 +189,8 @@ int osog_backward_np(osog_ctx* ctx, const osog_particles* p, int64_t N, const os
  * so d_gc[n] = (dL/dcx[n], dL/dcy[n]) = -(n_p[n] - n_medium) * sum over the pixels of d_gopd * grad t_n, DEVICE float [N, 2]
  * in 1/um, overwritten (0 for invalid or off-canvas particles).  grad t is analytic: the slopes of the active exit and
  * entry faces of a prism, T0 grad w / (2 sqrt w) for an ellipsoid (it grows like 1 / sqrt(w) towards the ellipsoid's
- * outline: the sum over pixel centres is finite but dominated by the outline pixels).  Same fixed-order fp64 gather as
+ * outline: the sum over pixel centres is finite but dominated by the outline pixels; it is the almost-everywhere derivative
+ * of the pixel-sampled loss, which for ellipsoids also jumps whenever the outline crosses a pixel centre).  Same fixed-order fp64 gather as
  * osog_backward_np.  Gradients with respect to rotation and dimensions are not implemented. */
 int osog_backward_centre(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gc);
 

@@ -74,6 +74,7 @@ def lib():
                                   C.POINTER(osog_dic), C.c_void_p]
     L.osog_field_to_dic.argtypes = [ctx, C.POINTER(osog_optics), C.POINTER(osog_dic), C.c_void_p, C.c_void_p]
     L.osog_backward_np.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
+    L.osog_backward_intensity.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_backward_centre.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_gbuffer.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_height.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p,
@@ -94,7 +95,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_debug_recompose_field", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_intensity", "osog_debug_recompose_field", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -238,6 +239,14 @@ class Context:
         r = lib().osog_backward_np(self._ctx, C.byref(p.c), p.N, C.byref(o), gopd.data_ptr(), out.data_ptr())
         if r != OSOG_OK:
             raise OsogError(r, "osog_backward_np")
+        return out
+
+    def backward_intensity(self, p: Particles, o, gI):
+        """float32 [B, H, W] dL/dOPD for an upstream gradient gI = dL/dI of the coherent intensity (osog_backward_intensity)."""
+        out = self._out(o.B)
+        r = lib().osog_backward_intensity(self._ctx, C.byref(p.c), p.N, C.byref(o), gI.data_ptr(), out.data_ptr())
+        if r != OSOG_OK:
+            raise OsogError(r, "osog_backward_intensity")
         return out
 
     def backward_centre(self, p: Particles, o, gopd):

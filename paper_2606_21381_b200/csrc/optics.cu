@@ -33,14 +33,16 @@ __device__ __forceinline__ float2 pupil_value(const FrameOptics& fo, int kx, int
 }
 
 // spec *= P * scale (in place), or with FILL: spec = P * scale
+// imag_sign = -1: multiply by conj(P) (adjoint of the optics stage); only the defocus phase has an imaginary part
 template <bool DEFOCUS, bool FILL>
 __global__ void __launch_bounds__(256) k_pupil(float2* __restrict__ spec, const FrameOptics* __restrict__ optics,
-                                               int H, int W, double inv_wp, double inv_hp, float scale)
+                                               int H, int W, double inv_wp, double inv_hp, float scale, float imag_sign)
 {
     const int kx = blockIdx.x * blockDim.x + threadIdx.x;
     const int ky = blockIdx.y, b = blockIdx.z;
     if (kx >= W) return;
-    const float2 pv = pupil_value<DEFOCUS>(optics[b], kx, ky, H, W, inv_wp, inv_hp, scale);
+    float2 pv = pupil_value<DEFOCUS>(optics[b], kx, ky, H, W, inv_wp, inv_hp, scale);
+    if (DEFOCUS) pv.y *= imag_sign;
     const size_t idx = ((size_t)b * H + ky) * W + kx;
     if (FILL) {
         spec[idx] = pv;
@@ -153,16 +155,17 @@ __global__ void __launch_bounds__(256) k_sensor(const float2* __restrict__ img, 
     out[(size_t)b * npx + pix] = I;
 }
 
-static cudaError_t pupil_launch(osog_ctx* c, int B, float2* spec, double pitch, bool defocus, bool fill, float scale)
+static cudaError_t pupil_launch(osog_ctx* c, int B, float2* spec, double pitch, bool defocus, bool fill, float scale,
+                                float imag_sign = 1.0f)
 {
     const dim3 grid((c->W + 255) / 256, c->H, B);
     const double inv_wp = 1.0 / ((double)c->W * pitch), inv_hp = 1.0 / ((double)c->H * pitch);
     if (fill) {
-        if (defocus) k_pupil<true, true><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale);
-        else k_pupil<false, true><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale);
+        if (defocus) k_pupil<true, true><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale, imag_sign);
+        else k_pupil<false, true><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale, imag_sign);
     } else {
-        if (defocus) k_pupil<true, false><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale);
-        else k_pupil<false, false><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale);
+        if (defocus) k_pupil<true, false><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale, imag_sign);
+        else k_pupil<false, false><<<grid, 256, 0, c->stream>>>(spec, c->optics, c->H, c->W, inv_wp, inv_hp, scale, imag_sign);
     }
     return cudaGetLastError();
 }
@@ -170,6 +173,48 @@ static cudaError_t pupil_launch(osog_ctx* c, int B, float2* spec, double pitch, 
 cudaError_t launch_pupil(osog_ctx* c, int B, float2* spec, double pitch, bool defocus)
 {
     return pupil_launch(c, B, spec, pitch, defocus, false, (float)(1.0 / ((double)c->H * c->W)));
+}
+
+cudaError_t launch_pupil_conj(osog_ctx* c, int B, float2* spec, double pitch, bool defocus)
+{
+    return pupil_launch(c, B, spec, pitch, defocus, false, (float)(1.0 / ((double)c->H * c->W)), -1.0f);
+}
+
+// Adjoint of the optics stage: v *= g (g real, per pixel): g_V = G_I V
+__global__ void __launch_bounds__(256) k_mul_real(float2* __restrict__ v, const float* __restrict__ g, size_t n)
+{
+    const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const float2 x = v[k];
+    const float s = g[k];
+    v[k] = make_float2(x.x * s, x.y * s);
+}
+
+// dL/dOPD = (4 pi / lambda) Im(g_U conj(U))
+__global__ void __launch_bounds__(256) k_gopd(const float2* __restrict__ gu, const float2* __restrict__ u,
+                                              const FrameOptics* __restrict__ optics, size_t npx, float* __restrict__ gopd)
+{
+    const size_t pix = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int b = blockIdx.y;
+    if (pix >= npx) return;
+    const float2 a = gu[(size_t)b * npx + pix], w = u[(size_t)b * npx + pix];
+    const float k = (float)(12.566370614359172 * optics[b].inv_lambda);
+    gopd[(size_t)b * npx + pix] = k * (a.y * w.x - a.x * w.y);
+}
+
+cudaError_t launch_mul_real(osog_ctx* c, int B, float2* v, const float* g)
+{
+    const size_t n = (size_t)B * c->H * c->W;
+    k_mul_real<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(v, g, n);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gopd(osog_ctx* c, int B, const float2* gu, const float2* u, float* d_gopd)
+{
+    const size_t npx = (size_t)c->H * c->W;
+    const dim3 grid((unsigned)((npx + 255) / 256), B);
+    k_gopd<<<grid, 256, 0, c->stream>>>(gu, u, c->optics, npx, d_gopd);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_pupil_fill(osog_ctx* c, int B, float2* spec, double pitch, bool defocus)

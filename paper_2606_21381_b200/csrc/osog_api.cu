@@ -404,6 +404,36 @@ int osog_render_gbuffer(osog_ctx* c, const osog_particles* p, int64_t N, const o
     return OSOG_OK;
 }
 
+int osog_backward_intensity(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gI, float* d_gopd)
+{
+    if (!d_gI || !aligned16(d_gI)) return OSOG_EINVAL;
+    int r = check_call(c, p, N, o, d_gopd);
+    if (r != OSOG_OK) return r;
+    if ((r = check_intensity(o)) != OSOG_OK) return r;
+    if ((r = render_common(c, p, N, o, nullptr, c->field)) != OSOG_OK) return r;      // U, the exit wave
+    DeviceGuard g(c->device);
+    if (!c->work) {                                  // first call of this kind: a second complex batch
+        const cudaError_t ea = dalloc(&c->work, (size_t)c->max_frames * c->H * c->W);
+        if (ea != cudaSuccess) { cudaGetLastError(); c->work = nullptr; return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea); }
+    }
+    const int B = o->B;
+    const bool defocus = o->defocus_um != 0.0;
+    cudaError_t e = cudaMemcpyAsync(c->work, c->field, sizeof(float2) * (size_t)B * c->H * c->W, cudaMemcpyDeviceToDevice, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    // V = U * h_obj
+    if ((r = fft_frames(c, c->work, B, CUFFT_FORWARD)) != OSOG_OK) return r;
+    if ((e = launch_pupil(c, B, c->work, o->pitch_um, defocus)) != cudaSuccess) return cuda_fail(c, e);
+    if ((r = fft_frames(c, c->work, B, CUFFT_INVERSE)) != OSOG_OK) return r;
+    // g_V = G_I V;  g_U = F^-1{ conj(P) F{g_V} }
+    if ((e = launch_mul_real(c, B, c->work, d_gI)) != cudaSuccess) return cuda_fail(c, e);
+    if ((r = fft_frames(c, c->work, B, CUFFT_FORWARD)) != OSOG_OK) return r;
+    if ((e = launch_pupil_conj(c, B, c->work, o->pitch_um, defocus)) != cudaSuccess) return cuda_fail(c, e);
+    if ((r = fft_frames(c, c->work, B, CUFFT_INVERSE)) != OSOG_OK) return r;
+    // dL/dOPD = (4 pi / lambda) Im(g_U conj(U))
+    if ((e = launch_gopd(c, B, c->work, c->field, d_gopd)) != cudaSuccess) return cuda_fail(c, e);
+    return OSOG_OK;
+}
+
 int osog_backward_np(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gnp)
 {
     if (!d_gopd || !aligned16(d_gopd)) return OSOG_EINVAL;

@@ -124,6 +124,9 @@ cudaError_t launch_gbuffer(osog_ctx* c, int B, const int32_t* d_frame_start, int
 // optics.cu
 cudaError_t launch_pupil(osog_ctx* c, int B, float2* spec, double pitch, bool defocus);
 cudaError_t launch_pupil_fill(osog_ctx* c, int B, float2* spec, double pitch, bool defocus);
+cudaError_t launch_pupil_conj(osog_ctx* c, int B, float2* spec, double pitch, bool defocus);
+cudaError_t launch_mul_real(osog_ctx* c, int B, float2* v, const float* g);
+cudaError_t launch_gopd(osog_ctx* c, int B, const float2* gu, const float2* u, float* d_gopd);
 cudaError_t launch_dic_shear(osog_ctx* c, int B, const float2* field, float2* out, int sx, int sy, double theta);
 cudaError_t launch_abs2(osog_ctx* c, int B, float2* buf, double scale);
 cudaError_t launch_cmul(osog_ctx* c, int B, float2* a, const float2* b, double scale);
