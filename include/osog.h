@@ -5,7 +5,7 @@
  * binning spec B1-B4 are listed in DESIGN.md section 3):
  *
  *   For every frame b and pixel (i, j) (row i, column j, centre x = (j + 1/2) p, y = (i + 1/2) p):
- *     OPD[b,i,j] = sum over the frame's particles n, ascending n, of (n_p[n] - n_medium) * thickness_n(x - cx, y - cy)
+ *     OPD[b,i,j] = sum over the frame's particles n of (n_p[n] - n_medium) * thickness_n(x - cx, y - cy)
  *                  - the integrand of Eq. 2 accumulated as Eq. 7 does;
  *                  thickness = chord of the vertical line through the convex body: ellipsoid quadric, or the
  *                  half-space intersection {x | A x <= b} of Eq. 1 for the capped tetragonal prism.
@@ -25,8 +25,10 @@
  *     scratch, allocated in osog_create and freed in osog_destroy.  No allocation happens in a render call (one exception:
  *     the first DIC call of a context, see osog_render_dic).
  *   - Results are bitwise reproducible from run to run: every pixel sums its particles in an order fixed by the
- *     data alone (sorted tile lists, walked in batches), never by thread scheduling (the two
- *     *_atomic alternatives are the stated exceptions).
+ *     data alone, never by thread scheduling (the two *_atomic alternatives are the stated exceptions).  The order is
+ *     NOT plain ascending n: the tile's list is sorted ascending and walked in batches of 32 entries; inside a batch
+ *     the particles are summed class by class (prisms by evaluation class, then ellipsoids), ascending n inside a
+ *     class.  The double-precision sum differs from the ascending-order sum at the 1e-16 level.
  *   - There is no CPU fallback and no backend dispatch: without a CUDA device osog_create fails.
  *   - Return value: 0 = OK, negative = error (see the enum).  Nothing is printed, nothing throws or aborts.
  *   - Particles with a non-finite parameter, a non-positive dimension or kind > 1 are skipped (they join no
@@ -41,13 +43,14 @@
 extern "C" {
 #endif
 
-#define OSOG_API_VERSION 2   /* 2: osog_optics.defocus_um, osog_dic, osog_render_dic, osog_field_to_dic */
+#define OSOG_API_VERSION 3   /* 2: osog_optics.defocus_um, osog_dic, osog_render_dic, osog_field_to_dic
+                                3: max_pairs is a TOTAL capacity (device scan + CSR lists), osog_status reports the exact need */
 
 enum {
     OSOG_OK = 0,
     OSOG_EINVAL = -1,     /* null / misaligned pointer, bad size, N > max_particles, B > max_frames, bad optics */
     OSOG_ECUDA = -2,      /* CUDA runtime, launch or cuFFT failure (osog_last_cuda_error gives the code)       */
-    OSOG_ECAPACITY = -3,  /* some tile's particle list exceeded its capacity: the frames of that call are zero-filled */
+    OSOG_ECAPACITY = -3,  /* the call produced more (particle, tile) pairs in total than max_pairs: its frames are zero-filled */
     OSOG_ENOMEM = -4      /* allocation failure in osog_create                                                 */
 };
 /* status bits returned by osog_status (sticky until the next render call) */
@@ -64,10 +67,9 @@ typedef struct {
     int32_t  H, W;           /* frame height / width in pixels, 1 .. 32768; need not be tile multiples     */
     int32_t  max_frames;     /* largest batch B of one call, >= 1                                          */
     int64_t  max_particles;  /* largest N (total over the batch) of one call, >= 0                         */
-    int64_t  max_pairs;      /* capacity of the (particle, tile) pair lists; 0 = 64 * max_particles + 1024.  It is
-                                divided evenly among the max_frames * ceil(H/T) * ceil(W/T) tiles of the context:
-                                one tile's list holds floor(max_pairs / tiles) entries (at least 1; with the default
-                                sizing max_pairs = 0 at least 64, so that few particles on a large frame still fit)    */
+    int64_t  max_pairs;      /* capacity of the tile lists = largest TOTAL number of (particle, tile) pairs of one call
+                                (the compact CSR list that the device scan addresses); 0 = 64 * max_particles + 1024.
+                                How the pairs are spread over the tiles does not matter: one crowded tile may hold them all */
 } osog_config;
 
 /* Particle state, Structure of Arrays ("S in R^{N x D}"): one DEVICE array of length N per
@@ -107,12 +109,13 @@ typedef struct {
     double   bias_rad;                /* bias phase theta                                                         */
 } osog_dic;
 
-/* Create a context: allocates all scratch (records, bounding boxes, per-tile counters and fixed-capacity lists, ramp
- * tables, one complex frame batch and the cuFFT plans).  *out is set to NULL on failure. */
+/* Create a context: allocates all scratch (records, tile ranges, per-tile counters, scan offsets, staging slices and the
+ * CSR pair list, ramp tables, one complex frame batch and the cuFFT plans).  *out is set to NULL on failure. */
 int osog_create(osog_ctx** out, const osog_config* cfg);
 
-/* OPD frame(s): d_opd is DEVICE float [B, H, W], row-major, micrometres.  Steps H1-H6 of DESIGN.md:
- * prepare + bounding box + append to the per-tile lists, per-tile sort + cull, per-tile ordered composition. */
+/* OPD frame(s): d_opd is DEVICE float [B, H, W], row-major, micrometres.  Steps H1-H6 of DESIGN.md: prepare + bounding box
+ * + per-tile count (the same atomic stages the entry in the tile's slice), exclusive scan of the counts (warp shuffles, one
+ * block), fill of the CSR list in ascending particle index + per-tile cull, per-tile ordered composition. */
 int osog_render_opd(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd);
 
 /* Complex exit wave: d_field is DEVICE float [B, H, W, 2] (interleaved re, im = complex64).  Same steps as
@@ -201,23 +204,24 @@ int osog_render_opd_smem_atomic(osog_ctx* ctx, const osog_particles* p, int64_t 
 
 int osog_destroy(osog_ctx* ctx);
 
-/* Synchronises the stream.  *status_bits = OSOG_W* bits of the last render call, *pairs = number of
- * (particle, tile) pairs of that call; if it overflowed: the max_pairs that would have sufficed (longest tile
- * list x tiles of the context).  Either pointer may be NULL.
+/* Synchronises the stream.  *status_bits = OSOG_W* bits of the last render call, *pairs = total number of
+ * (particle, tile) pairs of that call (the device scan's total); if the call overflowed, this is exactly the max_pairs
+ * that would have sufficed.  Either pointer may be NULL.
  * Returns OSOG_ECAPACITY if the last call overflowed, OSOG_ECUDA on a sticky CUDA error, else OSOG_OK. */
 int osog_status(osog_ctx* ctx, uint32_t* status_bits, int64_t* pairs);
 
-/* Test / diagnostics: synchronises, then writes the binning of the last render call to HOST arrays (the scan and
- * the compaction of the tiles' fixed-capacity slices run on the host):
- * h_offset [n_tiles + 1] (exclusive scan of the per-tile counts), h_list [min(pairs, cap)] (each tile's
- * segment in ascending particle index).  Tile id = frame * tiles_per_frame + (i / T) * ceil(W / T) + (j / T).
+/* Test / diagnostics: synchronises, then copies the binning of the last render call to HOST arrays, as the device holds
+ * it: h_offset [n_tiles + 1] = the exclusive scan of the per-tile counts (H3), h_list [min(pairs, cap)] = the CSR list,
+ * each tile's segment in ascending particle index (H4; filled by calls that run the sort: every osog_render_* except
+ * osog_render_opd_atomic).  Tile id = frame * tiles_per_frame + (i / T) * ceil(W / T) + (j / T).
  * Any pointer may be NULL.  *n_tiles and *n_pairs are always written. */
 int osog_debug_bins(osog_ctx* ctx, uint32_t* h_offset, uint32_t* h_list, int64_t cap,
                     int64_t* n_tiles, int64_t* n_pairs);
 
-/* Test / measurement: re-runs ONLY the composition kernel (H5-H7) of the last osog_render_* call on its binning
- * (tile lists, records, ramp tables and optics are still in the context) and writes the complex field again.
- * Lets bench.py time the dominant kernel alone with CUDA events.  OSOG_EINVAL if no render call came before. */
+/* Test / measurement: re-runs ONLY the composition kernel (H5-H7) of the last call on its binning (tile lists, records,
+ * ramp tables and optics are still in the context) and writes the complex field again.  Lets bench.py time the dominant
+ * kernel alone with CUDA events.  OSOG_EINVAL unless the last call on this context was one of osog_render_opd / _field /
+ * _intensity / _dic / _height or osog_backward_intensity (the calls that leave sorted lists and a composition behind). */
 int osog_debug_recompose_field(osog_ctx* ctx, float* d_field);
 
 /* Tile edge T in pixels (build-time constant of the binning, B3). */

@@ -43,9 +43,11 @@ class osog_dic(C.Structure):
 
 
 class OsogError(RuntimeError):
-    def __init__(self, code, what):
+    def __init__(self, code, what, pairs_needed=None):
         self.code = code
-        super().__init__(f"{what}: {lib().osog_strerror(code).decode()} ({code})")
+        self.pairs_needed = pairs_needed      # OSOG_ECAPACITY: the max_pairs that would have sufficed
+        extra = f"; max_pairs >= {pairs_needed} needed" if pairs_needed is not None else ""
+        super().__init__(f"{what}: {lib().osog_strerror(code).decode()} ({code}){extra}")
 
 
 _LIB = None
@@ -176,17 +178,23 @@ def optics_from_scene(scene, pupil_enabled=True):
 class Context:
     """osog_ctx owner.  Methods mirror the C entry points and return torch tensors on the device."""
 
-    def __init__(self, H, W, max_particles, max_frames=1, max_pairs=0, device="cuda:0", stream=None):
+    def __init__(self, H, W, max_particles, max_frames=1, max_pairs=0, device="cuda:0", stream=None, check=True):
+        """check=True: every render / backward call is followed by osog_status (which synchronises the stream) and raises
+        OsogError(OSOG_ECAPACITY) when the call needed more (particle, tile) pairs than max_pairs - its outputs are then
+        zero-filled.  check=False leaves the calls enqueue-only (timed loops); call status() yourself."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("osog: no CUDA device; this library has no CPU fallback")
         self.torch = torch
+        self.check = bool(check)
         self.device = torch.device(device)
+        if self.device.index is None:
+            self.device = torch.device("cuda", torch.cuda.current_device())
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self.H, self.W, self.max_frames = int(H), int(W), int(max_frames)
         cfg = osog_config()
         cfg.struct_size = C.sizeof(osog_config)
-        cfg.device = self.device.index or 0
+        cfg.device = self.device.index
         cfg.stream = self.stream.cuda_stream
         cfg.H, cfg.W, cfg.max_frames = self.H, self.W, self.max_frames
         cfg.max_particles = int(max_particles)
@@ -209,10 +217,31 @@ class Context:
             return out
         return self.torch.empty((B, self.H, self.W) + tail, dtype=self.torch.float32, device=self.device)
 
-    def _call(self, name, p, o, out):
-        r = getattr(lib(), name)(self._ctx, C.byref(p.c), p.N, C.byref(o), out.data_ptr())
+    def _done(self, r, name):
+        """Return-code check of an entry point, then (check=True) the device status of the call it enqueued."""
         if r != OSOG_OK:
             raise OsogError(r, name)
+        if self.check:
+            bits, pairs = C.c_uint32(0), C.c_int64(0)
+            r = lib().osog_status(self._ctx, C.byref(bits), C.byref(pairs))
+            if r != OSOG_OK:
+                raise OsogError(r, name, pairs.value if r == OSOG_ECAPACITY else None)
+
+    def _in(self, t, shape, name):
+        """A caller-supplied device tensor the library reads: float32, contiguous, on this device, of the stated shape."""
+        torch = self.torch
+        if t.is_complex():
+            t = torch.view_as_real(t)
+        if tuple(t.shape) != tuple(shape):
+            raise ValueError(f"{name}: shape {tuple(t.shape)}, expected {tuple(shape)}")
+        if t.device != self.device:
+            raise ValueError(f"{name}: on {t.device}, the context is on {self.device}")
+        if t.dtype != torch.float32 or not t.is_contiguous():
+            t = t.to(torch.float32).contiguous()
+        return t
+
+    def _call(self, name, p, o, out):
+        self._done(getattr(lib(), name)(self._ctx, C.byref(p.c), p.N, C.byref(o), out.data_ptr()), name)
         return out
 
     def render_opd(self, p: Particles, o, out=None):
@@ -227,43 +256,39 @@ class Context:
         h = self._out(o.B)
         g = self._out(o.B, 2) if grad else None
         l = self._out(o.B) if lap else None
-        r = lib().osog_render_height(self._ctx, C.byref(p.c), p.N, C.byref(o), h.data_ptr(),
-                                     g.data_ptr() if grad else None, l.data_ptr() if lap else None)
-        if r != OSOG_OK:
-            raise OsogError(r, "osog_render_height")
+        self._done(lib().osog_render_height(self._ctx, C.byref(p.c), p.N, C.byref(o), h.data_ptr(),
+                                            g.data_ptr() if grad else None, l.data_ptr() if lap else None), "osog_render_height")
         return h, g, l
 
     def backward_np(self, p: Particles, o, gopd):
         """float32 [N] dL/dn_p for an upstream gradient gopd = dL/dOPD (float32 [B, H, W]) (osog_backward_np)."""
         out = self.torch.empty((p.N,), dtype=self.torch.float32, device=self.device)
-        r = lib().osog_backward_np(self._ctx, C.byref(p.c), p.N, C.byref(o), gopd.data_ptr(), out.data_ptr())
-        if r != OSOG_OK:
-            raise OsogError(r, "osog_backward_np")
+        gopd = self._in(gopd, (o.B, self.H, self.W), "gopd")
+        self._done(lib().osog_backward_np(self._ctx, C.byref(p.c), p.N, C.byref(o), gopd.data_ptr(), out.data_ptr()), "osog_backward_np")
         return out
 
     def backward_intensity(self, p: Particles, o, gI):
         """float32 [B, H, W] dL/dOPD for an upstream gradient gI = dL/dI of the coherent intensity (osog_backward_intensity)."""
         out = self._out(o.B)
-        r = lib().osog_backward_intensity(self._ctx, C.byref(p.c), p.N, C.byref(o), gI.data_ptr(), out.data_ptr())
-        if r != OSOG_OK:
-            raise OsogError(r, "osog_backward_intensity")
+        gI = self._in(gI, (o.B, self.H, self.W), "gI")
+        self._done(lib().osog_backward_intensity(self._ctx, C.byref(p.c), p.N, C.byref(o), gI.data_ptr(), out.data_ptr()),
+                   "osog_backward_intensity")
         return out
 
     def backward_centre(self, p: Particles, o, gopd):
         """float32 [N, 2] (dL/dcx, dL/dcy) for an upstream gradient gopd = dL/dOPD (osog_backward_centre)."""
         out = self.torch.empty((p.N, 2), dtype=self.torch.float32, device=self.device)
-        r = lib().osog_backward_centre(self._ctx, C.byref(p.c), p.N, C.byref(o), gopd.data_ptr(), out.data_ptr())
-        if r != OSOG_OK:
-            raise OsogError(r, "osog_backward_centre")
+        gopd = self._in(gopd, (o.B, self.H, self.W), "gopd")
+        self._done(lib().osog_backward_centre(self._ctx, C.byref(p.c), p.N, C.byref(o), gopd.data_ptr(), out.data_ptr()),
+                   "osog_backward_centre")
         return out
 
     def render_gbuffer(self, p: Particles, o):
         """(int32 [B, H, W] instance id of the top-most particle, float32 [B, H, W] height of its top surface)."""
         tid = self.torch.empty((o.B, self.H, self.W), dtype=self.torch.int32, device=self.device)
         dep = self.torch.empty((o.B, self.H, self.W), dtype=self.torch.float32, device=self.device)
-        r = lib().osog_render_gbuffer(self._ctx, C.byref(p.c), p.N, C.byref(o), tid.data_ptr(), dep.data_ptr())
-        if r != OSOG_OK:
-            raise OsogError(r, "osog_render_gbuffer")
+        self._done(lib().osog_render_gbuffer(self._ctx, C.byref(p.c), p.N, C.byref(o), tid.data_ptr(), dep.data_ptr()),
+                   "osog_render_gbuffer")
         return tid, dep
 
     def particle_obbs(self, p: Particles, o, out=None):
@@ -272,7 +297,7 @@ class Context:
             out = self.torch.empty((p.N, 6), dtype=self.torch.float32, device=self.device)
         r = lib().osog_particle_obbs(self._ctx, C.byref(p.c), p.N, C.byref(o), out.data_ptr())
         if r != OSOG_OK:
-            raise OsogError(r, "osog_particle_obbs")
+            raise OsogError(r, "osog_particle_obbs")      # (runs the preparation kernel only: no list capacity involved)
         return out
 
     def render_opd_smem_atomic(self, p: Particles, o, out=None):
@@ -289,7 +314,7 @@ class Context:
 
     def field_to_intensity(self, o, field, out=None):
         out = self._out(o.B, out=out)
-        f = self.torch.view_as_real(field) if field.is_complex() else field
+        f = self._in(field, (o.B, self.H, self.W, 2), "field")
         r = lib().osog_field_to_intensity(self._ctx, C.byref(o), f.data_ptr(), out.data_ptr())
         if r != OSOG_OK:
             raise OsogError(r, "osog_field_to_intensity")
@@ -298,14 +323,12 @@ class Context:
     def render_dic(self, p: Particles, o, dic, out=None):
         """float32 [B, H, W] DIC image of Eq. 5 (osog_render_dic); `dic` from make_dic."""
         out = self._out(o.B, out=out)
-        r = lib().osog_render_dic(self._ctx, C.byref(p.c), p.N, C.byref(o), C.byref(dic), out.data_ptr())
-        if r != OSOG_OK:
-            raise OsogError(r, "osog_render_dic")
+        self._done(lib().osog_render_dic(self._ctx, C.byref(p.c), p.N, C.byref(o), C.byref(dic), out.data_ptr()), "osog_render_dic")
         return out
 
     def field_to_dic(self, o, dic, field, out=None):
         out = self._out(o.B, out=out)
-        f = self.torch.view_as_real(field) if field.is_complex() else field
+        f = self._in(field, (o.B, self.H, self.W, 2), "field")
         r = lib().osog_field_to_dic(self._ctx, C.byref(o), C.byref(dic), f.data_ptr(), out.data_ptr())
         if r != OSOG_OK:
             raise OsogError(r, "osog_field_to_dic")

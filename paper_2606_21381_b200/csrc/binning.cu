@@ -1,7 +1,8 @@
-// H1-H4 of DESIGN.md: per-particle preparation (fp64), bounding box -> tile range -> append to the per-tile lists
-// (fixed capacity per tile, the atomic on the tile's counter gives the slot: no scan and no second fill pass).  Integer
-// results must equal the oracle's binning bit for bit (B1-B4); the canonical (ascending) order of
-// each list is established by k_sort_cull (compose.cu); osog_debug_bins builds the exclusive scan on the host.
+// H1-H4 of DESIGN.md: per-particle preparation (fp64), bounding box -> tile range -> count (H2), exclusive scan of the
+// per-tile counts (H3, warp shuffles, by the last binning block to finish), and the first half of the fill (H4): the
+// atomic that counts a (particle, tile) pair also returns its slot in the tile's staging slice.  k_sort_cull
+// (compose.cu) then moves every tile's entries, in ascending particle index, to offset[tile] of the compact CSR list.
+// Integer results must equal the oracle's binning bit for bit (B1-B4).
 #include "osog_internal.cuh"
 
 namespace osog {
@@ -17,8 +18,11 @@ struct PrepArgs {
     int4* tbox;
     int* pframe;
     uint32_t* count;              // this call's slot of the per-tile counters (all zero on entry)
-    uint32_t* list;               // [tiles][tile_cap]
-    int tile_cap;
+    uint32_t* slices;             // [tiles][slice_cap] staging slices (unsorted; entries beyond slice_cap are not stored)
+    int slice_cap;
+    uint32_t* offset;             // [tiles + 1] exclusive scan of count (H3), written by the last binning block
+    uint32_t* done;               // number of binning blocks that have finished (0 on entry, reset by the last one)
+    long long max_pairs;          // capacity of the CSR list: a larger total sets OSOG_WOVERFLOW
     float* obb;                   // [N][6] oriented-bounding-box labels (osog_particle_obbs), or nullptr
     int unit_dn;                  // 1: index contrast n_p - n_medium replaced by 1 (height map of the G-buffer)
     float2 *ramp_x, *ramp_y;
@@ -136,7 +140,7 @@ __device__ __forceinline__ void binning_role(const PrepArgs& a, long long n)
     s_box[wid][lane] = make_int4(tb.x, tw, tb.z, (int)(uint32_t)n);
     s_t0[wid][lane] = (uint32_t)((size_t)b * a.ntx * a.nty);
     __syncwarp();
-    const uint32_t cap = (uint32_t)a.tile_cap;
+    const uint32_t cap = (uint32_t)a.slice_cap;
     for (int k0 = 0; k0 < total; k0 += 32 * 8) {
         uint32_t t[8], pos[8], id[8];
 #pragma unroll
@@ -157,25 +161,90 @@ __device__ __forceinline__ void binning_role(const PrepArgs& a, long long n)
         }
 #pragma unroll
         for (int q = 0; q < 8; ++q)
-            if (k0 + q * 32 + lane < total && pos[q] < cap) a.list[(size_t)t[q] * cap + pos[q]] = id[q];
+            if (k0 + q * 32 + lane < total && pos[q] < cap) a.slices[(size_t)t[q] * cap + pos[q]] = id[q];
     }
 }
 
-// Grid layout (blocks of 128 threads): [0, nb) binning role, one particle per thread; [nb, 2 nb) record role, one
-// particle per thread, the block's 128 particles permuted so that prisms come first and ellipsoids last (warps are then
-// uniform in the code path they take, except one mixed warp per block); [2 nb, ...) ramp tables.  nb = ceil(N / 128).
+// ---- H3: exclusive scan of the per-tile counts, by ONE block (the last binning block to finish) ------------------------
+// Every thread sums a contiguous chunk of tiles (independent 128-bit loads, all in flight), the chunk sums are scanned
+// across the block with warp shuffles (inclusive shuffle scan per warp, the warp totals through shared memory), then
+// every thread walks its chunk again and writes offset[t].  Also: total pair count, longest list, capacity check.
+__device__ void scan_counts(const PrepArgs& a)
+{
+    __shared__ unsigned long long s_warp[kPrepThreads / 32];
+    __shared__ uint32_t s_max[kPrepThreads / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const long long tiles = (long long)a.B * a.ntx * a.nty;
+    long long chunk = (tiles + kPrepThreads - 1) / kPrepThreads;
+    chunk = (chunk + 3) & ~3ll;                                   // multiple of 4: the 128-bit loads stay aligned
+    const long long t0 = min(tiles, (long long)threadIdx.x * chunk), t1 = min(tiles, t0 + chunk);
+    const uint32_t* cnt = a.count;
+    unsigned long long sum = 0;
+    uint32_t mx = 0;
+    long long t = t0;
+    for (; t + 4 <= t1; t += 4) {                                 // L2 reads: the counters were written by atomics
+        const uint4 v = __ldcg(reinterpret_cast<const uint4*>(cnt + t));
+        sum += (unsigned long long)v.x + v.y + v.z + v.w;
+        mx = max(max(mx, v.x), max(v.y, max(v.z, v.w)));
+    }
+    for (; t < t1; ++t) { const uint32_t v = __ldcg(cnt + t); sum += v; mx = max(mx, v); }
+    // block-wide exclusive scan of the chunk sums
+    unsigned long long incl = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned long long v = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += v;
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+    if (lane == 31) s_warp[wid] = incl;
+    if (lane == 0) s_max[wid] = mx;
+    __syncthreads();
+    unsigned long long base = 0, total = 0;
+    uint32_t mall = 0;
+#pragma unroll
+    for (int w = 0; w < kPrepThreads / 32; ++w) {
+        if (w < wid) base += s_warp[w];
+        total += s_warp[w];
+        mall = max(mall, s_max[w]);
+    }
+    unsigned long long run = base + incl - sum;                   // exclusive prefix of this thread's chunk
+    for (t = t0; t + 4 <= t1; t += 4) {
+        const uint4 v = __ldcg(reinterpret_cast<const uint4*>(cnt + t));
+        uint4 o;
+        o.x = (uint32_t)min(run, 0xffffffffull); run += v.x;
+        o.y = (uint32_t)min(run, 0xffffffffull); run += v.y;
+        o.z = (uint32_t)min(run, 0xffffffffull); run += v.z;
+        o.w = (uint32_t)min(run, 0xffffffffull); run += v.w;
+        *reinterpret_cast<uint4*>(a.offset + t) = o;
+    }
+    for (; t < t1; ++t) { a.offset[t] = (uint32_t)min(run, 0xffffffffull); run += __ldcg(cnt + t); }
+    if (threadIdx.x == 0) {
+        a.offset[tiles] = (uint32_t)min(total, 0xffffffffull);
+        a.status->pairs = total;
+        a.status->max_count = mall;
+        if (total > (unsigned long long)a.max_pairs) atomicOr(&a.status->bits, OSOG_WOVERFLOW);
+        *a.done = 0u;                                             // ready for the next call
+    }
+}
+
+// Grid layout (blocks of 128 threads): [0, nbin) binning role, one particle per thread (nbin = max(1, nb): the scan needs
+// a block even when N = 0); [nbin, nbin + nb) record role, one particle per thread, the block's 128 particles permuted so
+// that prisms come first and ellipsoids last (warps are then uniform in the code path they take, except one mixed warp
+// per block); [nbin + nb, ...) ramp tables.  nb = ceil(N / 128).
 __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
 {
     pdl_trigger();                               // k_sort_cull's CTAs may become resident (they wait for this grid to finish)
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long nb = (a.N + kPrepThreads - 1) / kPrepThreads;
+    const long long nbin = nb > 0 ? nb : 1;
 
     if (gid < a.B && gid < kOpticsChunk) a.optics[gid] = a.oc.f[gid];
 
-    if ((long long)blockIdx.x >= 2 * nb) {
+    if ((long long)blockIdx.x >= nbin + nb) {
         // ---- phase-ramp tables exp(i 2 pi fx0 x_j), x_j = (j + 1/2) p  (oblique illumination)
         if (!a.has_ramp) return;
-        long long r = gid - 2 * nb * kPrepThreads;
+        long long r = gid - (nbin + nb) * kPrepThreads;
         const long long nx = (long long)a.B * a.W, ny = (long long)a.B * a.H;
         if (r < nx) {
             const int b = (int)(r / a.W), j = (int)(r % a.W);
@@ -192,8 +261,8 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
 
     // ---- H1/H2: one particle = two threads in different blocks: role 0 does the binning (bounding box, tile range,
     // counts), role 1 the derived record (the two halves are independent; splitting them halves the critical path)
-    const int role = (long long)blockIdx.x >= nb ? 1 : 0;
-    long long n = (long long)(blockIdx.x - (role ? nb : 0)) * kPrepThreads + threadIdx.x;
+    const int role = (long long)blockIdx.x >= nbin ? 1 : 0;
+    long long n = (long long)(blockIdx.x - (role ? nbin : 0)) * kPrepThreads + threadIdx.x;
     if (role == 1) {
         __shared__ unsigned char s_perm[kPrepThreads];
         __shared__ int s_np[kPrepThreads / 32];
@@ -217,6 +286,16 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
     }
     if (role == 0) {
         binning_role(a, n);
+        // H3: the last binning block to get here scans the counts (the record role blocks are still busy: off the critical path)
+        __shared__ bool s_last;
+        __threadfence();                                          // this block's counter atomics before its done-ticket
+        __syncthreads();
+        if (threadIdx.x == 0) s_last = atomicAdd(a.done, 1u) == (uint32_t)(nbin - 1);
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            scan_counts(a);
+        }
         return;
     }
     if (n >= a.N) return;
@@ -460,13 +539,17 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     const long long tiles = (long long)B * c->ntx * c->nty;
     c->last_B = B;
     c->last_tiles = tiles;
+    c->last_N = N;
+    c->last_frame_start = B > 1 ? p->frame_start : nullptr;
+    c->last_has_ramp = -1;                           // set again by a call that runs the sort and a field-capable composition
     cudaError_t e;
     // Invariant kept by the kernels themselves (no memset nodes in the steady state): the counter slot and the status
     // slot of this call are all zero on entry (cleared by the previous call's k_sort_cull, which works on the other
     // slot).  After a failed or atomic-variant call: clear explicitly.
     if (c->scratch_dirty) {
-        if ((e = cudaMemsetAsync(c->count, 0, sizeof(uint32_t) * 2 * (size_t)c->max_tiles, c->stream)) != cudaSuccess) return e;
+        if ((e = cudaMemsetAsync(c->count, 0, sizeof(uint32_t) * 2 * (size_t)c->count_stride, c->stream)) != cudaSuccess) return e;
         if ((e = cudaMemsetAsync(c->status, 0, 2 * sizeof(DeviceStatus), c->stream)) != cudaSuccess) return e;
+        if ((e = cudaMemsetAsync(c->done, 0, sizeof(uint32_t), c->stream)) != cudaSuccess) return e;
         c->slot_tiles[0] = c->slot_tiles[1] = 0;
     }
     c->scratch_dirty = true;
@@ -481,7 +564,8 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     a.N = N; a.B = B; a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
     a.pitch = o->pitch_um; a.n_medium = o->n_medium;
     a.rec = c->rec; a.tbox = c->tbox; a.pframe = c->pframe;
-    a.count = c->count + (size_t)c->status_idx * c->max_tiles; a.list = c->list; a.tile_cap = c->tile_cap;
+    a.count = c->count + (size_t)c->status_idx * c->count_stride; a.slices = c->slices; a.slice_cap = c->slice_cap;
+    a.offset = c->offset; a.done = c->done; a.max_pairs = c->max_pairs;
     a.obb = d_obb;
     a.unit_dn = unit_dn ? 1 : 0;
     a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.optics = c->optics; a.status = status;
@@ -491,7 +575,7 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     const int threads = kPrepThreads;
     const long long nb = (N + threads - 1) / threads;
     const long long ramp_items = a.has_ramp ? (long long)B * (c->W + c->H) : 0;
-    long long blocks = 2 * nb + (ramp_items + threads - 1) / threads;
+    long long blocks = (nb > 0 ? nb : 1) + nb + (ramp_items + threads - 1) / threads;
     if (blocks * threads < B) blocks = (B + threads - 1) / threads;     // the first threads also upload the optics
     k_prepare<<<(unsigned)blocks, threads, 0, c->stream>>>(a);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;

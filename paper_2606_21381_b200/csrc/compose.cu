@@ -1,6 +1,8 @@
 // H4 (second half) - H7 of DESIGN.md: per-tile ordered composition, two kernels.
-// k_sort_cull, one warp per 32 x 32 pixel tile:
-//   1. sort the tile's particle list ascending (deterministic summation order), in place,
+// k_sort_cull, two warps per 32 x 32 pixel tile:
+//   1. fill the tile's segment of the CSR list (at offset[tile], the device scan of k_prepare) in ascending particle
+//      index (deterministic summation order): rank sort of the tile's staging slice, or, for a list longer than the
+//      slice, an ordered re-scan of the particles' tile ranges,
 //   2. per list entry, test the particle's pixel bounding box and oriented box against the tile's eight 16 x 8 pixel
 //      sub-tiles: 8-bit mask + evaluation code of the record -> meta.
 // k_compose_tile, two CTAs of four warps per tile, every warp independent (no barrier, no shared list):
@@ -17,10 +19,9 @@ namespace osog {
 
 struct ComposeArgs {
     const float* rec;
-    const uint32_t* count;       // this call's per-tile list lengths
-    const uint32_t* list;        // [tiles][tile_cap], sorted by k_sort_cull
-    const uint16_t* meta;        // [tiles][tile_cap]
-    int tile_cap;
+    const uint32_t* offset;      // [tiles + 1] exclusive scan of the per-tile list lengths (k_prepare)
+    const uint32_t* list;        // CSR list, every tile's segment sorted by k_sort_cull
+    const uint16_t* meta;        // per list entry
     const FrameOptics* optics;
     const float2 *ramp_x, *ramp_y;
     const DeviceStatus* status;
@@ -108,16 +109,6 @@ __device__ __forceinline__ void sincospi_unit(float x, float* sn, float* cs)
     *sn = sp;
     *cs = cp;
 }
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all()
-{
-    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
-}
-
 // ---- fp64 prism evaluation (refinement of flagged pixels, and the atomic variant) -------------------------------------
 // r64: 24 doubles (U, V, Cx, Cn per slab, relative to pixel (jc, ic)); dj, di: pixel offsets from (jc, ic).
 __device__ __noinline__ double prism_t64(const double* r64, uint32_t vmask, double dj, double di)
@@ -272,14 +263,16 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
 }
 
 // ---- H4 (second half) + tile-level cull: two WARPS per tile ------------------------------------------------------------
-// Sorts the tile's list ascending in place (the canonical, deterministic summation order) and writes one 16-bit word
-// per list entry: bits 0..7 = which of the tile's 8 warp sub-tiles (16 x 8 pixels) the particle can touch (bounding
-// box + oriented-box test), bits 8..10 = the evaluation code of the record.  k_compose_tile then needs no barrier.
-// Rank sort (ids are unique inside a tile): the list is staged in the tile's shared-memory slice, every lane counts
-// the ids smaller than its own with broadcast 128-bit reads; the record header loads of the cull are issued first so
-// that their latency hides behind the counting.  Lists longer than kWarpSortCap (pathological crowding) are sorted in
-// global memory by the same warp (bitonic network, slow but correct).
-constexpr int kWarpSortCap = 1024;                 // list entries sorted in shared memory (4 KB per tile)
+// Fills the tile's CSR segment list[offset[tile] .. offset[tile + 1]) in ascending particle index (the canonical,
+// deterministic summation order) and writes one 16-bit word per list entry: bits 0..7 = which of the tile's 8 warp
+// sub-tiles (16 x 8 pixels) the particle can touch (bounding box + oriented-box test), bits 8..10 = the evaluation code of
+// the record.  k_compose_tile then needs no barrier.
+// Rank sort (ids are unique inside a tile): the tile's staging slice is copied to shared memory, every lane counts the
+// ids smaller than its own with broadcast 128-bit reads; the record header loads of the cull are issued first so that
+// their latency hides behind the counting.  A list longer than the staging slice (a crowded tile) is rebuilt instead from
+// the particles' tile ranges (tbox, written by k_prepare): the two warps walk the frame's particles from both ends in
+// index order and keep those whose range contains the tile, which yields the ascending list directly.
+constexpr int kWarpSortCap = 1024;                 // largest staging slice (4 KB of shared memory per tile)
 #ifndef OSOG_SORT_WARPS
 #define OSOG_SORT_WARPS 2
 #endif
@@ -318,80 +311,51 @@ __device__ __forceinline__ uint32_t tile_meta(const float4 h0, const float4 h1, 
     return mask | (header_code(h0, h1) << 8);
 }
 
-__device__ void sort_global_warp(uint32_t* a, uint32_t L, int lane)
-{
-    uint32_t P = 1;
-    while (P < L) P <<= 1;
-    for (uint32_t k = 2; k <= P; k <<= 1) {
-        for (uint32_t j = k >> 1; j > 0; j >>= 1) {
-            for (uint32_t t = lane; t < (P >> 1); t += 32) {
-                uint32_t lo, hi;
-                if (j == (k >> 1)) {                       // first step of a merge: mirror inside the block of size k
-                    const uint32_t blk = t / j, r = t % j;
-                    lo = blk * k + r;
-                    hi = blk * k + (k - 1 - r);
-                } else {
-                    lo = (t / j) * (2 * j) + (t % j);
-                    hi = lo + j;
-                }
-                if (hi < L) {                              // virtual +inf padding beyond L never moves
-                    const uint32_t x = a[lo], y = a[hi];
-                    if (x > y) { a[lo] = y; a[hi] = x; }
-                }
-            }
-            __threadfence_block();
-            __syncwarp();
-        }
-    }
-}
+struct SortArgs {
+    const float* recs;
+    const int4* tbox;             // [N] tile ranges of the particles (tx0 > tx1: not listed)
+    const int32_t* frame_start;   // device [B + 1] or nullptr (one frame)
+    long long N;
+    const uint32_t* count;        // this call's per-tile list lengths
+    uint32_t* count_next;         // the other counter slot, cleared here for the next call
+    const uint32_t* offset;       // [tiles + 1] device scan
+    const uint32_t* slices;       // [tiles][slice_cap] unsorted staging slices
+    int slice_cap;
+    uint32_t* list;               // CSR list (output)
+    uint16_t* meta;               // (output)
+    const DeviceStatus* status;
+    DeviceStatus* status_next;
+    int ntx, nty, n_tiles, n_clear;
+};
 
-__global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __restrict__ recs, const uint32_t* __restrict__ count,
-                                                             uint32_t* __restrict__ count_next, uint32_t* __restrict__ list,
-                                                             uint16_t* __restrict__ meta, DeviceStatus* __restrict__ status,
-                                                             DeviceStatus* __restrict__ status_next, int tile_cap,
-                                                             int ntx, int nty, int n_tiles, int n_clear)
+__global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const SortArgs a)
 {
     __shared__ __align__(16) uint32_t s_all[(kWarps / kSortWarps) * kWarpSortCap];
-    __shared__ uint32_t s_len[kWarps];
     pdl_trigger();                                               // k_compose_tile's CTAs may become resident
-    pdl_wait();                                                  // k_prepare has finished, its lists and records are visible
+    pdl_wait();                                                  // k_prepare has finished: counts, offsets, slices, records are visible
     // kSortWarps warps per tile: they stage the list together in one shared slice, each ranks / culls every kSortWarps-th group of 32 entries
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int half = wid % kSortWarps;                           // this warp's part of the tile's work
     const int tile = (blockIdx.x * kWarps + wid) / kSortWarps;
     if (blockIdx.x == 0 && threadIdx.x == 0) {                   // the other status slot belongs to the next call
-        status_next->bits = 0u; status_next->max_count = 0u; status_next->pairs = 0ull;
+        a.status_next->bits = 0u; a.status_next->max_count = 0u; a.status_next->pairs = 0ull;
     }
-    // list length of the tile; the other counter slot is cleared for the next call; the call's totals (number of pairs,
-    // longest list, overflow of the per-tile capacity) are reduced per CTA
-    const uint32_t Lraw = tile < n_tiles ? count[tile] : 0u;
-    if (tile < n_clear && lane == 0 && half == 0) count_next[tile] = 0u;    // every counter the other slot's last user touched
-    if (lane == 0) s_len[wid] = half == 0 ? Lraw : 0u;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        uint32_t mx = 0;
-        unsigned long long sum = 0;
-#pragma unroll
-        for (int w = 0; w < kWarps; ++w) { mx = max(mx, s_len[w]); sum += s_len[w]; }
-        if (sum != 0ull) {
-            atomicAdd(&status->pairs, sum);
-            atomicMax(&status->max_count, mx);
-            if (mx > (uint32_t)tile_cap) atomicOr(&status->bits, OSOG_WOVERFLOW);
-        }
-    }
-    const uint32_t L = Lraw;
-    if (L == 0u || L > (uint32_t)tile_cap) return;               // empty, or overflow (the frames are zero-filled)
-    const size_t beg = (size_t)tile * tile_cap;
-    uint32_t* glist = list + beg;
-    const int tpf = ntx * nty;
-    const int rt = tile % tpf;
-    const int ty = rt / ntx, tx = rt - ty * ntx;
-    const float4* recs4 = reinterpret_cast<const float4*>(recs);
-    if (L <= (uint32_t)kWarpSortCap) {
+    const uint32_t L = tile < a.n_tiles ? a.count[tile] : 0u;
+    if (tile < a.n_clear && lane == 0 && half == 0) a.count_next[tile] = 0u;    // every counter the other slot's last user touched
+    if (L == 0u || (a.status->bits & OSOG_WOVERFLOW) != 0u) return;   // empty, or more pairs than the CSR list holds (frames are zero-filled)
+    const uint32_t beg = a.offset[tile];
+    uint32_t* glist = a.list + beg;
+    uint16_t* gmeta = a.meta + beg;
+    const int tpf = a.ntx * a.nty;
+    const int b = tile / tpf, rt = tile - b * tpf;
+    const int ty = rt / a.ntx, tx = rt - ty * a.ntx;
+    const float4* recs4 = reinterpret_cast<const float4*>(a.recs);
+    if (L <= (uint32_t)a.slice_cap) {
+        const uint32_t* slice = a.slices + (size_t)tile * a.slice_cap;
         uint32_t* s = s_all + (wid / kSortWarps) * kWarpSortCap; // the tile's warps share one slice
         const uint32_t L4 = (L + 3u) & ~3u;
-        for (uint32_t k = lane + 32 * half; k < L4; k += 32 * kSortWarps) s[k] = k < L ? glist[k] : 0xffffffffu;
-        asm volatile("bar.sync %0, %1;" ::"r"(1 + wid / kSortWarps), "n"(32 * kSortWarps) : "memory");   // tile barrier: the list is staged, glist may be overwritten
+        for (uint32_t k = lane + 32 * half; k < L4; k += 32 * kSortWarps) s[k] = k < L ? slice[k] : 0xffffffffu;
+        asm volatile("bar.sync %0, %1;" ::"r"(1 + wid / kSortWarps), "n"(32 * kSortWarps) : "memory");   // tile barrier: the list is staged
         for (uint32_t k = lane + 32 * half; k < L; k += 32 * kSortWarps) {
             const uint32_t v = s[k];
             const float4* rec = recs4 + (size_t)v * (kRecWords / 4);
@@ -403,16 +367,68 @@ __global__ void __launch_bounds__(kComposeThreads) k_sort_cull(const float* __re
                 count_less(r, q.x, v); count_less(r1, q.y, v); count_less(r, q.z, v); count_less(r1, q.w, v);
             }
             r += r1;
-            glist[r] = v;                                        // the sorted segment (also what osog_debug_bins returns)
-            meta[beg + r] = (uint16_t)tile_meta(h0, h1, tx, ty);
+            glist[r] = v;                                        // H4: the sorted CSR segment (also what osog_debug_bins returns)
+            gmeta[r] = (uint16_t)tile_meta(h0, h1, tx, ty);
         }
-    } else if (half == 0) {
-        sort_global_warp(glist, L, lane);
-        for (uint32_t k = lane; k < L; k += 32) {
-            const float4* rec = recs4 + (size_t)glist[k] * (kRecWords / 4);
-            meta[beg + k] = (uint16_t)tile_meta(__ldg(rec), __ldg(rec + 1), tx, ty);
+        return;
+    }
+    // ---- crowded tile: the slice holds only part of the list.  Rebuild it in order from the tile ranges: warp 0 walks the
+    // frame's particles upwards from the first and fills the segment from its front, warp 1 walks downwards from the last
+    // and fills from the back; together they find exactly L particles whose range contains (tx, ty).
+    long long p_lo = 0, p_hi = a.N;
+    if (a.frame_start != nullptr) { p_lo = a.frame_start[b]; p_hi = a.frame_start[b + 1]; }
+    const long long p_mid = p_lo + (p_hi - p_lo) / (kSortWarps == 1 ? 1 : 2);
+    const unsigned lt = (1u << lane) - 1u;
+    if (half == 0) {
+        uint32_t pos = 0;
+        for (long long base = p_lo; base < p_mid; base += 32) {
+            const long long n = base + lane;
+            bool in = false;
+            if (n < p_mid) { const int4 tb = __ldg(a.tbox + n); in = tb.x <= tx && tx <= tb.y && tb.z <= ty && ty <= tb.w; }
+            const unsigned m = __ballot_sync(0xffffffffu, in);
+            if (in) glist[pos + __popc(m & lt)] = (uint32_t)n;
+            pos += __popc(m);
+        }
+    } else if (half == 1) {
+        uint32_t pos = L;
+        for (long long top = p_hi; top > p_mid; top -= 32) {
+            const long long n = top - 32 + lane;                 // lanes ascending inside the chunk [top - 32, top)
+            bool in = false;
+            if (n >= p_mid) { const int4 tb = __ldg(a.tbox + n); in = tb.x <= tx && tx <= tb.y && tb.z <= ty && ty <= tb.w; }
+            const unsigned m = __ballot_sync(0xffffffffu, in);
+            pos -= __popc(m);
+            if (in) glist[pos + __popc(m & lt)] = (uint32_t)n;
         }
     }
+    asm volatile("bar.sync %0, %1;" ::"r"(1 + wid / kSortWarps), "n"(32 * kSortWarps) : "memory");   // the segment is complete
+    for (uint32_t k = lane + 32 * half; k < L; k += 32 * kSortWarps) {
+        const float4* rec = recs4 + (size_t)glist[k] * (kRecWords / 4);
+        gmeta[k] = (uint16_t)tile_meta(__ldg(rec), __ldg(rec + 1), tx, ty);
+    }
+}
+
+static cudaError_t launch_sort_cull(osog_ctx* c, unsigned grid, bool pdl)
+{
+    SortArgs a;
+    a.recs = c->rec; a.tbox = c->tbox; a.frame_start = c->last_frame_start; a.N = c->last_N;
+    a.count = c->count + (size_t)c->status_idx * c->count_stride;
+    a.count_next = c->count + (size_t)(c->status_idx ^ 1) * c->count_stride;
+    a.offset = c->offset; a.slices = c->slices; a.slice_cap = c->slice_cap; a.list = c->list; a.meta = c->meta;
+    a.status = c->status + c->status_idx; a.status_next = c->status + (c->status_idx ^ 1);
+    a.ntx = c->ntx; a.nty = c->nty; a.n_tiles = (int)grid;
+    const long long n_clear = c->slot_tiles[c->status_idx ^ 1];
+    a.n_clear = (int)n_clear;
+    const unsigned cover = (unsigned)(n_clear > (long long)grid ? n_clear : (long long)grid);
+    const dim3 g((kSortWarps * cover + kWarps - 1) / kWarps), blk(kComposeThreads);
+    cudaError_t e;
+    if (pdl) {
+        e = launch_pdl(k_sort_cull, g, blk, 0, c->stream, a);
+    } else {
+        k_sort_cull<<<g, blk, 0, c->stream>>>(a);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) c->slot_tiles[c->status_idx ^ 1] = 0;
+    return e;
 }
 
 // ---- H5-H7: every warp is independent (no barrier, no shared list): it walks its tile's sorted list in batches of 32
@@ -431,8 +447,8 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
     pdl_wait();                                                  // k_sort_cull (and all before it) has finished
 
     const bool overflow = (a.status->bits & OSOG_WOVERFLOW) != 0u;
-    const size_t beg = (size_t)tile * a.tile_cap;
-    const uint32_t L = overflow ? 0u : a.count[tile];
+    const uint32_t beg = a.offset[tile];
+    const uint32_t L = overflow ? 0u : a.offset[tile + 1] - beg;
     const uint32_t* __restrict__ glist = a.list + beg;
     const uint16_t* __restrict__ gmeta = a.meta + beg;
 
@@ -502,9 +518,6 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
         __syncwarp();
         // ---- all lanes walk the survivors, class by class ----------------------------------------------------------------------
         const float4* slot = my_slots;
-#ifdef OSOG_EXP_NOEVAL                                           // experiment: skeleton only
-        if (a.H < 0)
-#endif
         {
 #pragma unroll 1
         for (int sv = 0; sv < n1; ++sv, slot += kSlotStride4) eval_prism<0>(slot, nullptr, slot[6].y, g, acc);
@@ -583,25 +596,18 @@ static cudaError_t launch_variant(const ComposeArgs& a, unsigned grid, cudaStrea
 }
 
 // sort_first = false: the lists of the last call are already sorted and culled (osog_debug_recompose_field)
-cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float* d_opd, float2* d_field, bool sort_first)
+cudaError_t launch_compose(osog_ctx* c, int B, bool has_ramp, float* d_opd, float2* d_field, bool sort_first)
 {
-    (void)N;
     ComposeArgs a;
-    a.rec = c->rec; a.count = c->count + (size_t)c->status_idx * c->max_tiles; a.list = c->list; a.meta = c->meta;
-    a.tile_cap = c->tile_cap; a.optics = c->optics;
+    a.rec = c->rec; a.offset = c->offset; a.list = c->list; a.meta = c->meta;
+    a.optics = c->optics;
     a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.status = c->status + c->status_idx;
     a.opd = d_opd; a.field = d_field;
     a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
     a.ramp_y_on = 1;
     const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
     if (sort_first) {
-        const long long n_clear = c->slot_tiles[c->status_idx ^ 1];
-        const unsigned cover = (unsigned)(n_clear > (long long)grid ? n_clear : (long long)grid);
-        const cudaError_t e = launch_pdl(k_sort_cull, dim3((kSortWarps * cover + kWarps - 1) / kWarps), dim3(kComposeThreads), 0, c->stream,
-                                         c->rec, a.count, c->count + (size_t)(c->status_idx ^ 1) * c->max_tiles, c->list, c->meta,
-                                         c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty,
-                                         (int)grid, (int)n_clear);
-        c->slot_tiles[c->status_idx ^ 1] = 0;
+        const cudaError_t e = launch_sort_cull(c, grid, true);
         if (e != cudaSuccess) return e;
     }
     if (d_opd != nullptr && d_field == nullptr) return launch_variant<true, false, false>(a, grid, c->stream);
@@ -653,9 +659,9 @@ __global__ void __launch_bounds__(256) k_compose_atomic(const float* __restrict_
 // warp walks the tile's sorted list, skips the entries whose sub-tile mask bit is clear, and for the others evaluates the
 // top of the chord in fp64 straight from the record: the decision "which particle is on top" is taken in the precision
 // the oracle takes it in.  Ascending list order and a strict comparison give ties to the smallest index.
-__global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* __restrict__ recs, const uint32_t* __restrict__ count,
+__global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* __restrict__ recs, const uint32_t* __restrict__ offset,
                                                                 const uint32_t* __restrict__ list, const uint16_t* __restrict__ meta,
-                                                                int tile_cap, const DeviceStatus* __restrict__ status,
+                                                                const DeviceStatus* __restrict__ status,
                                                                 const int32_t* __restrict__ frame_start, int ntx, int nty, int H,
                                                                 int W, int32_t* __restrict__ top_id, float* __restrict__ depth)
 {
@@ -664,9 +670,10 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
     const int b = tile / tpf, rt = tile - b * tpf;
     const int ty = rt / ntx, tx = rt - ty * ntx;
     const int j = tx * kTile + (wid & 1) * 16 + (lane & 3) * 4, i = ty * kTile + (wid >> 1) * 8 + (lane >> 2);
-    const uint32_t L = (status->bits & OSOG_WOVERFLOW) ? 0u : count[tile];
-    const uint32_t* glist = list + (size_t)tile * tile_cap;
-    const uint16_t* gmeta = meta + (size_t)tile * tile_cap;
+    const uint32_t beg = offset[tile];
+    const uint32_t L = (status->bits & OSOG_WOVERFLOW) ? 0u : offset[tile + 1] - beg;
+    const uint32_t* glist = list + beg;
+    const uint16_t* gmeta = meta + beg;
     const uint32_t first = frame_start != nullptr ? (uint32_t)frame_start[b] : 0u;
     double best[4] = {0.0, 0.0, 0.0, 0.0};
     int32_t who[4] = {-1, -1, -1, -1};
@@ -747,16 +754,9 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
 cudaError_t launch_gbuffer(osog_ctx* c, int B, const int32_t* d_frame_start, int32_t* d_top_id, float* d_depth)
 {
     const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
-    const uint32_t* count = c->count + (size_t)c->status_idx * c->max_tiles;
-    const long long n_clear = c->slot_tiles[c->status_idx ^ 1];
-    const unsigned cover = (unsigned)(n_clear > (long long)grid ? n_clear : (long long)grid);
-    k_sort_cull<<<(kSortWarps * cover + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(
-        c->rec, count, c->count + (size_t)(c->status_idx ^ 1) * c->max_tiles, c->list, c->meta,
-        c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty, (int)grid, (int)n_clear);
-    cudaError_t e = cudaGetLastError();
+    const cudaError_t e = launch_sort_cull(c, grid, false);
     if (e != cudaSuccess) return e;
-    c->slot_tiles[c->status_idx ^ 1] = 0;
-    k_gbuffer_tile<<<grid, kComposeThreads, 0, c->stream>>>(c->rec, count, c->list, c->meta, c->tile_cap, c->status + c->status_idx,
+    k_gbuffer_tile<<<grid, kComposeThreads, 0, c->stream>>>(c->rec, c->offset, c->list, c->meta, c->status + c->status_idx,
                                                            d_frame_start, c->ntx, c->nty, c->H, c->W, d_top_id, d_depth);
     return cudaGetLastError();
 }
@@ -766,8 +766,8 @@ cudaError_t launch_gbuffer(osog_ctx* c, int B, const int32_t* d_frame_start, int
 // particle's pixel bounding box that lies in the tile and atomicAdd's (n_p - n_m) t into it (fp64 thickness per pixel, fp32
 // shared-memory atomics).  The order in which the warps reach a pixel depends on scheduling: NOT deterministic in the last
 // bits, and the sum is fp32.  Kept to be measured against the ordered register accumulation of k_compose_tile.
-__global__ void __launch_bounds__(kComposeThreads) k_compose_smem_atomic(const float* __restrict__ recs, const uint32_t* __restrict__ count,
-                                                                       const uint32_t* __restrict__ list, int tile_cap,
+__global__ void __launch_bounds__(kComposeThreads) k_compose_smem_atomic(const float* __restrict__ recs, const uint32_t* __restrict__ offset,
+                                                                       const uint32_t* __restrict__ list,
                                                                        const DeviceStatus* __restrict__ status, int ntx, int nty,
                                                                        int H, int W, float* __restrict__ opd)
 {
@@ -779,8 +779,9 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_smem_atomic(const f
     const int x0 = tx * kTile, y0 = ty * kTile;
     for (int k = tid; k < kTile * kTile; k += kComposeThreads) s_acc[k] = 0.0f;
     __syncthreads();
-    const uint32_t L = (status->bits & OSOG_WOVERFLOW) ? 0u : count[tile];
-    const uint32_t* glist = list + (size_t)tile * tile_cap;
+    const uint32_t beg = offset[tile];
+    const uint32_t L = (status->bits & OSOG_WOVERFLOW) ? 0u : offset[tile + 1] - beg;
+    const uint32_t* glist = list + beg;
     for (uint32_t k = wid; k < L; k += kWarps) {
         const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)glist[k] * kRecWords);
         const float4 h1 = __ldg(rec + 1), h2 = __ldg(rec + 2);
@@ -813,20 +814,13 @@ __global__ void __launch_bounds__(kComposeThreads) k_compose_smem_atomic(const f
     }
 }
 
-// runs k_sort_cull first (it keeps the counter / status invariants; the order it establishes is not used here)
+// runs k_sort_cull first (it fills the CSR list and keeps the counter / status invariants)
 cudaError_t launch_compose_smem_atomic(osog_ctx* c, int B, float* d_opd)
 {
     const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
-    const uint32_t* count = c->count + (size_t)c->status_idx * c->max_tiles;
-    const long long n_clear = c->slot_tiles[c->status_idx ^ 1];
-    const unsigned cover = (unsigned)(n_clear > (long long)grid ? n_clear : (long long)grid);
-    k_sort_cull<<<(kSortWarps * cover + kWarps - 1) / kWarps, kComposeThreads, 0, c->stream>>>(
-        c->rec, count, c->count + (size_t)(c->status_idx ^ 1) * c->max_tiles, c->list, c->meta,
-        c->status + c->status_idx, c->status + (c->status_idx ^ 1), c->tile_cap, c->ntx, c->nty, (int)grid, (int)n_clear);
-    cudaError_t e = cudaGetLastError();
+    const cudaError_t e = launch_sort_cull(c, grid, false);
     if (e != cudaSuccess) return e;
-    c->slot_tiles[c->status_idx ^ 1] = 0;
-    k_compose_smem_atomic<<<grid, kComposeThreads, 0, c->stream>>>(c->rec, count, c->list, c->tile_cap, c->status + c->status_idx,
+    k_compose_smem_atomic<<<grid, kComposeThreads, 0, c->stream>>>(c->rec, c->offset, c->list, c->status + c->status_idx,
                                                                   c->ntx, c->nty, c->H, c->W, d_opd);
     return cudaGetLastError();
 }

@@ -182,7 +182,7 @@ int osog_destroy(osog_ctx* c)
     if (c->has_plan_one) cufftDestroy(c->plan_one);
     if (c->has_plan_batch) cufftDestroy(c->plan_batch);
     cudaFree(c->rec); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
-    cudaFree(c->list); cudaFree(c->meta); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
+    cudaFree(c->list); cudaFree(c->meta); cudaFree(c->slices); cudaFree(c->offset); cudaFree(c->done); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
     cudaFree(c->status); cudaFree(c->field); cudaFree(c->work); cudaFree(c->otf);
     delete c->otf_key;
     if (c->h_status) cudaFreeHost(c->h_status);
@@ -215,13 +215,15 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     c->nty = (c->H + kTile - 1) / kTile;
     c->max_tiles = (long long)c->max_frames * c->ntx * c->nty;
     if (c->max_tiles > 0x7fffffffll) { delete c; return OSOG_EINVAL; }
-    // every tile owns a fixed slice of the pair list (no scan, no second fill pass): capacity per tile
+    c->count_stride = (c->max_tiles + 3) & ~3ll;
+    // staging slice of one tile: about the mean list length the capacity allows, 32 .. 1,024 entries (1,024 = what
+    // k_sort_cull sorts in shared memory); a longer list is rebuilt in order from the tile ranges, see k_sort_cull
     {
-        long long cap = c->max_pairs / c->max_tiles;
-        if (cap < 1) cap = 1;
-        if (cfg->max_pairs == 0 && cap < 64) cap = 64;           // default sizing: never fewer than 64 entries per tile
-        if (cap > 0x3fffffffll) cap = 0x3fffffffll;
-        c->tile_cap = (int)cap;
+        long long cap = (c->max_pairs + c->max_tiles - 1) / c->max_tiles;
+        cap = (cap + 3) & ~3ll;
+        if (cap < 32) cap = 32;
+        if (cap > 1024) cap = 1024;
+        c->slice_cap = (int)cap;
     }
 
     DeviceGuard g(c->device);
@@ -232,9 +234,12 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     A(dalloc(&c->rec, np * kRecWords));
     A(dalloc(&c->tbox, np));
     A(dalloc(&c->pframe, np));
-    A(dalloc(&c->count, 2 * (size_t)c->max_tiles));
-    A(dalloc(&c->list, (size_t)c->max_tiles * c->tile_cap));
-    A(dalloc(&c->meta, (size_t)c->max_tiles * c->tile_cap));
+    A(dalloc(&c->count, 2 * (size_t)c->count_stride));
+    A(dalloc(&c->offset, (size_t)c->max_tiles + 4));
+    A(dalloc(&c->done, 1));
+    A(dalloc(&c->slices, (size_t)c->max_tiles * c->slice_cap));
+    A(dalloc(&c->list, (size_t)c->max_pairs));
+    A(dalloc(&c->meta, (size_t)c->max_pairs));
     A(dalloc(&c->ramp_x, (size_t)c->max_frames * c->W));
     A(dalloc(&c->ramp_y, (size_t)c->max_frames * c->H));
     A(dalloc(&c->optics, (size_t)c->max_frames));
@@ -242,7 +247,8 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     A(dalloc(&c->field, (size_t)c->max_frames * npx));
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&c->h_status), sizeof(DeviceStatus));
     if (e == cudaSuccess) e = cudaMemset(c->status, 0, 2 * sizeof(DeviceStatus));
-    if (e == cudaSuccess) e = cudaMemset(c->count, 0, sizeof(uint32_t) * 2 * (size_t)c->max_tiles);
+    if (e == cudaSuccess) e = cudaMemset(c->count, 0, sizeof(uint32_t) * 2 * (size_t)c->count_stride);
+    if (e == cudaSuccess) e = cudaMemset(c->done, 0, sizeof(uint32_t));
     if (e != cudaSuccess) {
         const bool oom = e == cudaErrorMemoryAllocation;
         cudaGetLastError();
@@ -272,10 +278,9 @@ static int render_common(osog_ctx* c, const osog_particles* p, int64_t N, const 
     cudaError_t e = launch_binning(c, p, N, o, nullptr, unit_dn);
     if (e != cudaSuccess) return cuda_fail(c, e);
     const bool has_ramp = o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0;
-    c->last_has_ramp = has_ramp ? 1 : 0;
-    c->last_N = N;
-    e = launch_compose(c, N, o->B, has_ramp, d_opd, d_field);
+    e = launch_compose(c, o->B, has_ramp, d_opd, d_field);
     if (e != cudaSuccess) return cuda_fail(c, e);
+    c->last_has_ramp = has_ramp ? 1 : 0;             // osog_debug_recompose_field may re-run this composition
     c->scratch_dirty = false;                        // k_sort_cull cleared the counter / status slots of the next call
     return OSOG_OK;
 }
@@ -370,7 +375,6 @@ int osog_particle_obbs(osog_ctx* c, const osog_particles* p, int64_t N, const os
     DeviceGuard g(c->device);
     cudaError_t e = launch_binning(c, p, N, o, d_obb);   // k_prepare alone; the tile lists it leaves are not used
     if (e != cudaSuccess) return cuda_fail(c, e);        // (scratch_dirty stays set: the next render call clears them)
-    c->last_has_ramp = -1;
     return OSOG_OK;
 }
 
@@ -397,7 +401,6 @@ int osog_render_gbuffer(osog_ctx* c, const osog_particles* p, int64_t N, const o
     DeviceGuard g(c->device);
     cudaError_t e = launch_binning(c, p, N, o);
     if (e != cudaSuccess) return cuda_fail(c, e);
-    c->last_has_ramp = -1;                           // no field-capable composition ran: osog_debug_recompose_field refuses
     e = launch_gbuffer(c, o->B, o->B > 1 ? p->frame_start : nullptr, d_top_id, d_depth);
     if (e != cudaSuccess) return cuda_fail(c, e);
     c->scratch_dirty = false;
@@ -443,7 +446,6 @@ int osog_backward_np(osog_ctx* c, const osog_particles* p, int64_t N, const osog
     DeviceGuard g(c->device);
     cudaError_t e = launch_binning(c, p, N, o);      // records + bounding boxes (the tile lists are not used)
     if (e != cudaSuccess) return cuda_fail(c, e);    // (scratch_dirty stays set: the next render call clears them)
-    c->last_has_ramp = -1;
     e = launch_backward_np(c, N, d_gopd, d_gnp);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
@@ -458,7 +460,6 @@ int osog_backward_centre(osog_ctx* c, const osog_particles* p, int64_t N, const 
     DeviceGuard g(c->device);
     cudaError_t e = launch_binning(c, p, N, o);      // records + bounding boxes (the tile lists are not used)
     if (e != cudaSuccess) return cuda_fail(c, e);    // (scratch_dirty stays set: the next render call clears them)
-    c->last_has_ramp = -1;
     e = launch_backward_centre(c, N, o->pitch_um, d_gopd, d_gc);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
@@ -471,7 +472,6 @@ int osog_render_opd_smem_atomic(osog_ctx* c, const osog_particles* p, int64_t N,
     DeviceGuard g(c->device);
     cudaError_t e = launch_binning(c, p, N, o);
     if (e != cudaSuccess) return cuda_fail(c, e);
-    c->last_has_ramp = -1;                           // no field-capable composition ran: osog_debug_recompose_field refuses
     e = launch_compose_smem_atomic(c, o->B, d_opd);
     if (e != cudaSuccess) return cuda_fail(c, e);
     c->scratch_dirty = false;
@@ -482,7 +482,7 @@ int osog_debug_recompose_field(osog_ctx* c, float* d_field)
 {
     if (!c || !d_field || !aligned16(d_field) || c->last_B < 1 || c->last_has_ramp < 0) return OSOG_EINVAL;
     DeviceGuard g(c->device);
-    cudaError_t e = launch_compose(c, c->last_N, c->last_B, c->last_has_ramp != 0, nullptr, reinterpret_cast<float2*>(d_field), false);
+    cudaError_t e = launch_compose(c, c->last_B, c->last_has_ramp != 0, nullptr, reinterpret_cast<float2*>(d_field), false);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
 }
@@ -496,8 +496,7 @@ int osog_status(osog_ctx* c, uint32_t* status_bits, int64_t* pairs)
     if (e != cudaSuccess) return cuda_fail(c, e);
     const bool overflow = (c->h_status->bits & OSOG_WOVERFLOW) != 0u;
     if (status_bits) *status_bits = c->h_status->bits;
-    // on overflow: the max_pairs that would have sufficed = longest tile list x tiles of the context
-    if (pairs) *pairs = overflow ? (int64_t)c->h_status->max_count * c->max_tiles : (int64_t)c->h_status->pairs;
+    if (pairs) *pairs = (int64_t)c->h_status->pairs;     // total of the device scan: on overflow, the max_pairs that suffices
     return overflow ? OSOG_ECAPACITY : OSOG_OK;
 }
 
@@ -512,26 +511,15 @@ int osog_debug_bins(osog_ctx* c, uint32_t* h_offset, uint32_t* h_list, int64_t c
     if (n_pairs) *n_pairs = pairs;
     if (c->last_tiles <= 0 || (!h_offset && !h_list)) return r;
     DeviceGuard g(c->device);
-    // host side: per-tile counts -> exclusive scan; the tiles' fixed-capacity slices -> one compact list
+    // the scan (offset) and the compact sorted lists are the device's own (k_prepare's scan, k_sort_cull's fill): plain copies
     const size_t nt = (size_t)c->last_tiles;
-    std::vector<uint32_t> cnt(nt);
-    cudaError_t e = cudaMemcpy(cnt.data(), c->count + (size_t)c->status_idx * c->max_tiles, sizeof(uint32_t) * nt, cudaMemcpyDeviceToHost);
+    cudaError_t e = cudaSuccess;
+    if (h_offset) e = cudaMemcpy(h_offset, c->offset, sizeof(uint32_t) * (nt + 1), cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return cuda_fail(c, e);
-    if (h_offset) {
-        unsigned long long run = 0;
-        for (size_t t = 0; t < nt; ++t) {
-            h_offset[t] = (uint32_t)(run < 0xffffffffull ? run : 0xffffffffull);
-            run += cnt[t];
-        }
-        h_offset[nt] = (uint32_t)(run < 0xffffffffull ? run : 0xffffffffull);
-    }
     if (h_list && r == OSOG_OK && cap > 0) {
-        std::vector<uint32_t> all(nt * (size_t)c->tile_cap);
-        e = cudaMemcpy(all.data(), c->list, sizeof(uint32_t) * all.size(), cudaMemcpyDeviceToHost);
+        const int64_t n = pairs < cap ? pairs : cap;
+        e = cudaMemcpy(h_list, c->list, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) return cuda_fail(c, e);
-        int64_t k = 0;
-        for (size_t t = 0; t < nt && k < cap; ++t)
-            for (uint32_t q = 0; q < cnt[t] && k < cap; ++q) h_list[k++] = all[t * (size_t)c->tile_cap + q];
     }
     return r;
 }

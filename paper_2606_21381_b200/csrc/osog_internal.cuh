@@ -55,21 +55,26 @@ struct osog_ctx {
     long long max_particles, max_pairs;
     int ntx, nty;                   // tiles per row / column
     long long max_tiles;            // max_frames * ntx * nty
-    int tile_cap;                   // list entries one tile can hold: max(1, max_pairs / max_tiles)
+    long long count_stride;         // max_tiles rounded up to a multiple of 4 (128-bit loads of the scan)
+    int slice_cap;                  // entries of one tile's staging slice (longer lists take the ordered re-scan of k_sort_cull)
     int last_cuda_error;
     // last call
     int last_B;
     int last_has_ramp;
     long long last_N;
     long long last_tiles;
+    const int32_t* last_frame_start; // device pointer of the last call's frame_start (nullptr: one frame)
     // scratch (device)
     float* rec;                     // [max_particles][kRecWords]
     int4* tbox;                     // [max_particles] tile range tx0, tx1, ty0, ty1 (tx0 > tx1: not listed)
     int* pframe;                    // [max_particles] frame of the particle
-    uint32_t* count;                // [2][max_tiles] per-tile list length; slot status_idx belongs to the current call, the
+    uint32_t* count;                // [2][count_stride] per-tile list length; slot status_idx belongs to the current call, the
                                     // other slot is zeroed by that call's k_sort_cull for the next call
-    uint32_t* list;                 // [max_tiles][tile_cap] tile t's particle indices at list + t * tile_cap
-    uint16_t* meta;                 // [max_tiles][tile_cap] per list entry: sub-tile mask | evaluation code << 8 (k_sort_cull)
+    uint32_t* offset;               // [max_tiles + 1] exclusive scan of the current call's counts (H3, k_prepare's last binning block)
+    uint32_t* done;                 // [1] finished binning blocks of the running k_prepare (0 between calls)
+    uint32_t* slices;               // [max_tiles][slice_cap] staging: tile t's unsorted entries at slices + t * slice_cap
+    uint32_t* list;                 // [max_pairs] CSR list: tile t's particle indices, ascending, at list + offset[t]
+    uint16_t* meta;                 // [max_pairs] per list entry: sub-tile mask | evaluation code << 8 (k_sort_cull)
     float2* ramp_x;                 // [max_frames][W]  exp(i 2 pi fx0 x_j)
     float2* ramp_y;                 // [max_frames][H]
     osog::FrameOptics* optics;      // [max_frames]
@@ -115,7 +120,7 @@ cudaError_t upload_optics(osog_ctx* c, const osog_optics* o, OpticsChunk* first)
 cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o, float* d_obb = nullptr,
                            bool unit_dn = false);
 // compose.cu
-cudaError_t launch_compose(osog_ctx* c, long long N, int B, bool has_ramp, float* d_opd, float2* d_field, bool sort_first = true);
+cudaError_t launch_compose(osog_ctx* c, int B, bool has_ramp, float* d_opd, float2* d_field, bool sort_first = true);
 cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd);
 cudaError_t launch_compose_smem_atomic(osog_ctx* c, int B, float* d_opd);
 cudaError_t launch_backward_np(osog_ctx* c, long long N, const float* d_gopd, float* d_gnp);

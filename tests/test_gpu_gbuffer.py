@@ -1,7 +1,10 @@
 """GPU parity of the G-buffer extras (osog_render_gbuffer: depth map and instance-id map, reading A24)
 against the oracle.  Both sides decide "which particle is on top" in float64; the GPU rounds the depth to float32.
-Where two top surfaces cross, a 1e-12 difference between the two float64 evaluations may flip the owner of a pixel: such
-pixels must be (very) rare and their depth must still agree (several owners are then correct: compare what is unique)."""
+The instance-id map is index work: it must equal the oracle's bit for bit, except where several owners really are
+correct.  Every differing pixel is therefore checked on its own (ids_valid): both particles must have a positive chord
+there and their two top surfaces must agree to 1e-9 um (a genuine tie up to the rounding of two float64 evaluation
+orders); coverage may differ only where the chord in question is shorter than 1e-9 um or the pixel centre lies within
+1e-7 um of the particle's outline.  Nothing is accepted by a rate."""
 from dataclasses import replace
 
 import numpy as np
@@ -35,6 +38,53 @@ def with_heights(sc, seed, spread=6.0):
     return replace(sc, cols=cols)
 
 
+TIE_UM = 1e-9          # two tops this close are the same height up to float64 rounding of different evaluation orders
+OUTLINE_UM = 1e-7      # a pixel centre this close to an outline may or may not be covered
+
+
+def _chord_at(o, sc, b, i, j, pid):
+    """oracle.chord of particle `pid` (index within frame b) at pixel (i, j): (z_enter, z_exit) or None; and its cz."""
+    n = int(sc.frame_start[b]) + int(pid)
+    c = sc.cols
+    dx = (j + 0.5) * sc.pitch_um - float(c["cx"][n])
+    dy = (i + 0.5) * sc.pitch_um - float(c["cy"][n])
+    q = [float(c[k][n]) for k in ("qw", "qx", "qy", "qz")]
+    d = [float(c[k][n]) for k in ("d0", "d1", "d2")]
+    kind = int(c["kind"][n])
+    return o.chord(kind, q, d, dx, dy), float(c["cz"][n]), (kind, q, d, dx, dy)
+
+
+def _near_outline(o, geom):
+    """True if some point within OUTLINE_UM of the pixel centre has a positive chord (the centre itself has none)."""
+    kind, q, d, dx, dy = geom
+    for ax, ay in ((1, 0), (-1, 0), (0, 1), (0, -1), (1, 1), (1, -1), (-1, 1), (-1, -1)):
+        if o.chord(kind, q, d, dx + ax * OUTLINE_UM, dy + ay * OUTLINE_UM) is not None:
+            return True
+    return False
+
+
+def ids_valid(o, sc, tid, rid):
+    """Per-pixel validity of every pixel where the GPU's instance id differs from the oracle's.  Returns their number."""
+    bad = []
+    where = np.argwhere(tid != rid)
+    for b, i, j in where:
+        t, r = int(tid[b, i, j]), int(rid[b, i, j])
+        if t >= 0 and r >= 0:                        # two owners: both must be hit, tops equal to TIE_UM
+            (ct, zt, _), (cr, zr, _) = _chord_at(o, sc, b, i, j, t), _chord_at(o, sc, b, i, j, r)
+            ok = ct is not None and cr is not None and abs((zt + ct[1]) - (zr + cr[1])) <= TIE_UM
+        elif r >= 0:                                 # the GPU sees no particle: the oracle's chord must be vanishing
+            cr, _, _ = _chord_at(o, sc, b, i, j, r)
+            ok = cr is not None and cr[1] - cr[0] < TIE_UM
+        else:                                        # the oracle sees none: the pixel centre must sit on the GPU owner's outline
+            ct, _, geom = _chord_at(o, sc, b, i, j, t)
+            ok = (ct is not None and ct[1] - ct[0] < TIE_UM) or (ct is None and _near_outline(o, geom))
+        if not ok:
+            bad.append((int(b), int(i), int(j), t, r))
+    print(f"gbuffer ids: {len(where)} of {tid.size} pixels with another (equally valid) owner")
+    assert not bad, f"{len(bad)} pixels with a wrong instance id, first (b, i, j, gpu, oracle): {bad[:5]}"
+    return len(where)
+
+
 def check(og, o, sc):
     ctx = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B)
     P = og.Particles.from_scene(sc)
@@ -46,10 +96,27 @@ def check(og, o, sc):
     rid, rdep = o.render_gbuffer(sc)
     tol = 1e-6 + 2e-7 * np.abs(rdep)
     assert np.all(np.abs(dep - rdep) <= tol), float(np.abs(dep - rdep).max())
-    differ = tid != rid
-    assert differ.mean() <= 1e-5, f"{int(differ.sum())} pixels with another owner"
-    assert np.array_equal(tid < 0, rid < 0) or (differ & ((tid < 0) | (rid < 0))).sum() <= 2
+    ids_valid(o, sc, tid, rid)
     return tid, dep, rid, rdep
+
+
+def test_ids_valid_rejects_a_wrong_id(o):
+    """The validity check itself (no GPU needed to run it, but it lives with the GPU tests it serves): a shifted id, an
+    invented owner on an empty pixel and a dropped owner are all refused; the oracle's own map passes with 0 differences."""
+    sc = with_heights(make_config(1), seed=41)
+    rid, _ = o.render_gbuffer(sc)
+    assert ids_valid(o, sc, rid, rid) == 0
+    i, j = np.argwhere(rid[0] >= 0)[100]
+    for wrong in ((int(rid[0, i, j]) + 1) % sc.N, -1):
+        t = rid.copy()
+        t[0, i, j] = wrong
+        with pytest.raises(AssertionError):
+            ids_valid(o, sc, t, rid)
+    i, j = np.argwhere(rid[0] < 0)[0]
+    t = rid.copy()
+    t[0, i, j] = 0
+    with pytest.raises(AssertionError):
+        ids_valid(o, sc, t, rid)
 
 
 @pytest.mark.parametrize("k,n", [(1, None), (2, None), (3, None), (4, None), (5, None)])
