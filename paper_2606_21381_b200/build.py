@@ -36,8 +36,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
            "-Xcompiler", "-fPIC,-Wall,-Wno-unused-function", "-shared",
            "-Xlinker", "-rpath=/usr/local/cuda/lib64",
            "-o", LIB + ".tmp"] + [os.path.join(CSRC, s) for s in SOURCES] + ["-lcufft"]
-    if os.environ.get("OSOG_NVCC_FLAGS"):              # extra flags for experiments, e.g. -DOSOG_EXP_NOEVAL
-        cmd[1:1] = os.environ["OSOG_NVCC_FLAGS"].split()
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.run(cmd, check=True)

@@ -73,29 +73,31 @@ struct DeviceGuard {
     }
 };
 
-// one 2-D C2C transform of each of the B frames in `buf`, in place
-int fft_frames(osog_ctx* c, float2* buf, int B, int sign)
+// one 2-D C2C transform of each of the B frames in `src` into `buf` (src == buf: in place; src is never written otherwise)
+int fft_frames(osog_ctx* c, float2* buf, int B, int sign, const float2* src = nullptr)
 {
     const size_t npx = (size_t)c->H * c->W;
+    float2* in = src ? const_cast<float2*>(src) : buf;
     if (B == c->max_frames && c->has_plan_batch) {
-        cufftResult r = cufftExecC2C(c->plan_batch, reinterpret_cast<cufftComplex*>(buf),
+        cufftResult r = cufftExecC2C(c->plan_batch, reinterpret_cast<cufftComplex*>(in),
                                      reinterpret_cast<cufftComplex*>(buf), sign);
         if (r != CUFFT_SUCCESS) { c->last_cuda_error = 10000 + (int)r; return OSOG_ECUDA; }
         return OSOG_OK;
     }
     for (int b = 0; b < B; ++b) {
         cufftComplex* f = reinterpret_cast<cufftComplex*>(buf + (size_t)b * npx);
-        cufftResult r = cufftExecC2C(c->plan_one, f, f, sign);
+        cufftResult r = cufftExecC2C(c->plan_one, reinterpret_cast<cufftComplex*>(in + (size_t)b * npx), f, sign);
         if (r != CUFFT_SUCCESS) { c->last_cuda_error = 10000 + (int)r; return OSOG_ECUDA; }
     }
     return OSOG_OK;
 }
 
-// forward FFT, pupil function, inverse FFT of B frames held in `buf` (in place), then the sensor into d_intensity
-int optics_stage(osog_ctx* c, const osog_optics* o, float2* buf, float* d_intensity)
+// forward FFT of the B frames of `src` into `buf` (src == nullptr: `buf` in place), pupil function, inverse FFT, then the
+// sensor into d_intensity
+int optics_stage(osog_ctx* c, const osog_optics* o, float2* buf, float* d_intensity, const float2* src = nullptr)
 {
     const int B = o->B;
-    int r = fft_frames(c, buf, B, CUFFT_FORWARD);
+    int r = fft_frames(c, buf, B, CUFFT_FORWARD, src);
     if (r != OSOG_OK) return r;
     cudaError_t e = launch_pupil(c, B, buf, o->pitch_um, o->defocus_um != 0.0);
     if (e != cudaSuccess) return cuda_fail(c, e);
@@ -321,9 +323,8 @@ int osog_field_to_intensity(osog_ctx* c, const osog_optics* o, const float* d_fi
     DeviceGuard g(c->device);
     cudaError_t e = upload_optics(c, o, nullptr);
     if (e != cudaSuccess) return cuda_fail(c, e);
-    e = cudaMemcpyAsync(c->field, d_field, sizeof(float2) * (size_t)o->B * c->H * c->W, cudaMemcpyDeviceToDevice, c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e);
-    return optics_stage(c, o, c->field, d_intensity);
+    // the first transform reads the caller's field and writes the context's frame: no copy, the stage the product runs
+    return optics_stage(c, o, c->field, d_intensity, reinterpret_cast<const float2*>(d_field));
 }
 
 int osog_render_dic(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const osog_dic* d, float* d_dic)
