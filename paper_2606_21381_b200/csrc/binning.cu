@@ -345,8 +345,13 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
             zmax = fmax(zmax, fabs(R20) * hs + fabs(R21) * hs + fabs(R22) * hl);
         }
         r32[14] = __double2float_ru(zmax * (1.0 + 1.0e-5) + 1.0e-6);
+        // word 15: power of two s with s * chord <= 1/2 for every chord of the body (chord <= 2 zmax): the composition
+        // evaluates s * t with a saturating subtraction (clamp to [0, 1] for free) and folds 1 / s into the index contrast
+        int ex2 = 0;
+        frexp(2.0 * zmax * (1.0 + 1.0e-5) + 2.0e-6, &ex2);      // 2 zmax < 2^ex2
+        ex2 = min(max(ex2 + 1, -60), 60);
+        r32[15] = (float)ldexp(1.0, -ex2);
     }
-    r32[15] = 0.0f;
     // Words 2..5: oriented box of the silhouette (unit axis with a_x >= 0, half lengths > 0); their sign bits carry the
     // evaluation code of the particle (0 ellipsoid, 1 + number of steep slabs, 4 all-fp64): bit 0 in the sign of
     // the first half length, bit 1 in the second, bit 2 in the sign of a_x.
@@ -374,6 +379,29 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
         r64[5] = 1.0 - (Sxx * ox * ox + 2.0 * Sxy * ox * oy + Syy * oy * oy);
         r64[6] = jc;
         r64[7] = ic;
+        // Words 40..53: the same quadratic for the composition kernel as (hi, lo) float pairs on an exact grid: hi is a
+        // multiple of q = 2^(e - 23) where 2^e bounds every intermediate of the Horner evaluation over the pixels the
+        // kernel can ask for (|dj| <= Rj, |di| <= Ri), so the fp32 FMAs on the hi parts are exact (integers times q below
+        // 2^24 q); lo = the remainder, fp32.  Signs arranged for w = F + (E + Cn ndi) ndi + (D + Bn ndi + An ndj) ndj with
+        // ndj = -(j - jc), ndi = -(i - ic): An = -A, Bn = -B, Cn = -C.
+        {
+            const double det = Sxx * Syy - Sxy * Sxy;
+            const double Rj = sqrt(fmax(Syy / det, 0.0)) * ip + 20.0, Ri = sqrt(fmax(Sxx / det, 0.0)) * ip + 20.0;
+            double Mb = 1.0 + fabs(r64[5]) + (fabs(r64[2]) * Ri + fabs(r64[4])) * Ri + (fabs(r64[0]) * Rj + fabs(r64[1]) * Ri + fabs(r64[3])) * Rj;
+            if (!(Mb < 1.0e30)) Mb = 1.0e30;                   // degenerate shape: the grid is coarse, the result stays finite
+            int eb = 0;
+            frexp(Mb, &eb);
+            const double q = ldexp(1.0, eb - 22), iq = ldexp(1.0, 22 - eb);
+            const double v[6] = {-r64[0], -r64[1], -r64[2], r64[3], r64[4], r64[5]};
+#pragma unroll
+            for (int k = 0; k < 6; ++k) {
+                const double hi = rint(v[k] * iq) * q;
+                r32[40 + 2 * k] = (float)hi;
+                r32[41 + 2 * k] = (float)(v[k] - hi);
+            }
+            r32[52] = (float)jc;
+            r32[53] = (float)ic;
+        }
         // oriented box of the silhouette ellipse {d^T S d <= 1}: principal axes of S
         const double hd = 0.5 * (Sxx - Syy), rad = sqrt(hd * hd + Sxy * Sxy), mid = 0.5 * (Sxx + Syy);
         const double lmin = fmax(mid - rad, 1.0e-300), lmax = mid + rad;

@@ -60,7 +60,7 @@ __device__ __forceinline__ float max3(float a, float b, float c)
     asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
     return r;
 }
-// packed fp32 FMA (Blackwell FFMA2): d = a * b + c on both halves
+// packed fp32 FMA (Blackwell FFMA2): d = a * b + c on both halves, one issue slot for two FMAs
 __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c)
 {
     unsigned long long ra, rb, rc, rd;
@@ -72,20 +72,26 @@ __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c)
     asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
     return d;
 }
-// float -> double for a non-negative, normal-or-zero float, with integer ops on the ALU pipe instead of an XU-pipe
-// conversion (F2F).  +0.0f maps to 2^-127 * 2 (about 1e-38), which is harmless for a thickness in micrometres.
-__device__ __forceinline__ double f2d_pos(float f)
+// float -> double (exact widening) with integer ops on the ALU pipe instead of an XU-pipe conversion (F2F, 8 cycles per
+// warp).  f must be normal or zero; +-0.0f maps to +-2^-126 (about 1e-38), harmless for a sum in micrometres.
+__device__ __forceinline__ double f2d(float f)
 {
     const uint32_t u = __float_as_uint(f);
-    return __hiloint2double((int)((u >> 3) + 0x38000000u), (int)(u << 29));
+    const uint32_t hi = (((u & 0x7fffffffu) >> 3) + 0x38000000u) | (u & 0x80000000u);
+    return __hiloint2double((int)hi, (int)(u << 29));
 }
-// double -> float of max(w, 0) by truncation, with integer ops on the ALU pipe instead of an XU-pipe F2F.F32.F64 + FMNMX:
-// a negative or tiny w (< 2^-126) gives +0 or a denormal below 1e-44, which sqrt.approx.ftz flushes to 0.
-// Relative error < 2^-23 (truncation of the mantissa), i.e. 2^-24 in the thickness sqrt(w).
-__device__ __forceinline__ float d2f_pos_trunc(double w)
+// saturating fp32 add / subtract: the result is clamped to [0, 1] by the FMA pipe (NaN -> 0), no separate min / max
+__device__ __forceinline__ float sub_sat(float a, float b)
 {
-    const int hi = max(__double2hiint(w) - 0x38000000, 0);
-    return __uint_as_float(__funnelshift_l((unsigned)__double2loint(w), (unsigned)hi, 3));
+    float r;
+    asm("sub.sat.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ float add_sat(float a, float b)
+{
+    float r;
+    asm("add.sat.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
+    return r;
 }
 // sin(pi x), cos(pi x) for |x| <= 1 (the reduced phase of the write-out, in half turns): k = nearest integer to 2 x,
 // r = x - k / 2 in [-1/4, 1/4], Taylor polynomials of sin(pi r) (through r^9) and cos(pi r) (through r^8): truncation
@@ -132,27 +138,38 @@ __device__ __noinline__ double prism_t64(const double* r64, uint32_t vmask, doub
 
 // ---- per-warp preparation of the prism survivors: work item = (survivor slot, slab q), one lane per item -------------
 // Re-base the slab's fp64 coefficients from the particle's reference pixel (jc, ic) to the warp's sub-tile origin
-// (wx0, wy0) and round to fp32 there: all later fp32 arithmetic uses pixel offsets 0..15 / 0..7.
-// Slot layout (words): 0..5 Ex, 6..11 En, 12..17 U, 18..23 V, 24 flags, 25 dn, 27 particle index, 28..35 slab 0 in
-// fp64 (Ex, En, U, V).  An ellipsoid slot holds the record's 8 doubles (A..F1, jc, ic) in words 0..15, 24 = 0, 25 = K.
+// (wx0, wy0), scale them by the particle's chord scale s (record word 15: s t <= 1/2) and round to fp32 there: all later
+// fp32 arithmetic uses pixel offsets 0..15 / 0..7.
+// A steep slab (slope > kSteepSlope; the first NS slabs of the record) is stored as (hi, lo) float pairs on an exact
+// grid: hi = multiple of q = 2^(e - 23), 2^e > every intermediate of  C - U lx - V ly  over the sub-tile, so the fp32 FMAs
+// on the hi parts are exact and hi + lo carries the fp64 value to 2^-24 relative of the (small) result.
+// Slot layout (words): 0..5 Ex, 6..11 En, 12..17 U, 18..23 V (hi parts for steep slabs), 25 dn / s, 27 particle index,
+// 28..31 lo parts (Ex, En, U, V) of slab 0, 32..35 of slab 1.  An ellipsoid slot holds the record's words 40..53.
 __device__ __forceinline__ void rebase_item(float4* __restrict__ slot, const float* __restrict__ recs, int q, int wx0, int wy0)
 {
     float* sw = reinterpret_cast<float*>(slot);
     const uint32_t pid = __float_as_uint(sw[27]);
     const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)pid * kRecWords);
-    const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));     // jc, ic
+    const float4 h2 = __ldg(rec + 2);                                  // flags, dn, cz, index
+    const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));     // jc, ic, zmax, chord scale
     const double2* c = reinterpret_cast<const double2*>(rec + 4);
     const double2 uv = __ldg(c + 2 * q), xn = __ldg(c + 2 * q + 1);    // U, V | Cx, Cn
-    if (q == 0) {
-        sw[25] = __ldg(reinterpret_cast<const float*>(rec) + 9);         // dn
-    }
+    const float tsc = __int_as_float(h3.w);
+    if (q == 0) sw[25] = h2.y / tsc;                                   // dn / s (s is a power of two: exact)
+    const double sc = (double)tsc;
     const double oj = (double)(wx0 - h3.x), oi = (double)(wy0 - h3.y);
     const double m = fma(uv.x, oj, uv.y * oi);
-    const double ex = xn.x - m, en = xn.y - m;
-    sw[q] = (float)ex; sw[6 + q] = (float)en; sw[12 + q] = (float)uv.x; sw[18 + q] = (float)uv.y;
-    if (q == 0) {                                                      // slab 0 also in fp64 (used when it is steep)
-        reinterpret_cast<double2*>(slot)[7] = make_double2(ex, en);
-        reinterpret_cast<double2*>(slot)[8] = uv;
+    const double ex = (xn.x - m) * sc, en = (xn.y - m) * sc, u = uv.x * sc, v = uv.y * sc;
+    const int ns = (int)((__float_as_uint(h2.x) >> 8) & 7u);
+    if (q >= ns) {
+        sw[q] = (float)ex; sw[6 + q] = (float)en; sw[12 + q] = (float)u; sw[18 + q] = (float)v;
+    } else {                                                           // steep slab (q = 0 or 1): exact-grid (hi, lo) pairs
+        const double mb = fmax(fabs(ex), fabs(en)) + 15.0 * fabs(u) + 7.0 * fabs(v);
+        const int e = ((__double2hiint(mb) >> 20) & 0x7ff) - 1021;     // mb < 2^e (one spare bit)
+        const double cq = __hiloint2double((e - 23 + 52 + 1023) << 20 | 0x80000, 0);   // 1.5 * 2^52 * q, q = 2^(e - 23)
+        const double exh = (ex + cq) - cq, enh = (en + cq) - cq, uh = (u + cq) - cq, vh = (v + cq) - cq;
+        sw[q] = (float)exh; sw[6 + q] = (float)enh; sw[12 + q] = (float)uh; sw[18 + q] = (float)vh;
+        slot[7 + q] = make_float4((float)(ex - exh), (float)(en - enh), (float)(u - uh), (float)(v - vh));
     }
 }
 
@@ -172,23 +189,29 @@ struct LaneGeom {
     float xf, yf;      // absolute pixel column of this lane's first pixel, and its row (exact small integers)
 };
 
-// Ellipsoid (kind 0), from the record doubles copied into the slot: w = 1 - d^T S d as a quadratic polynomial of
-// the pixel offsets from (jc, ic), all in fp64 (2 DFMA per pixel after the row terms), then
-// t = T0 sqrt(max(w, 0)) in fp32 and acc += (dn T0) sqrt(w) in fp64.
-__device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ slot, float K, const LaneGeom& g, double (&acc)[4])
+// Ellipsoid (kind 0): w = 1 - d^T S d as a quadratic polynomial of the pixel offsets from (jc, ic), from the record's
+// (hi, lo) coefficient pairs (k_prepare): Horner in packed fp32, exact on the hi halves, so w = hi + lo is good to
+// ~2^-47 of the largest intermediate (the precision the outline needs: t ~ sqrt(w)) without any fp64 instruction;
+// the saturating add clamps w to [0, 1] (w <= 1 by construction); pend += (dn T0) sqrt(w).
+__device__ __forceinline__ void eval_ellipsoid(const float4* __restrict__ slot, const LaneGeom& g, float (&pend)[4])
 {
-    const double2* c = reinterpret_cast<const double2*>(slot);
-    const double2 ab = c[0], cd = c[1], ef = c[2], jic = c[3];   // A,B | C,D | E,F1 | jc,ic
-    const double Kd = (double)K;
-    const double dj = (double)g.xf - jic.x, di = (double)g.yf - jic.y;
-    const double b1 = fma(ab.y, di, cd.y);                       // B di + D
-    const double cc = fma(-fma(cd.x, di, ef.x), di, ef.y);       // F1 - (C di + E) di
+    const float4 c0 = slot[0], c1 = slot[1], c2 = slot[2];      // An, Bn | Cn, D | E, F  (each as hi, lo)
+    const float4 c3 = slot[3];                                   // jc, ic
+    const float K = slot[6].y;
+    const float ndi = c3.y - g.yf, ndj0 = c3.x - g.xf;           // -(i - ic), -(j - jc): exact small integers
+    const float2 ndi2 = make_float2(ndi, ndi);
+    const float2 t1 = ffma2(make_float2(c1.x, c1.y), ndi2, make_float2(c2.x, c2.y));    // E + C di
+    const float2 wr = ffma2(t1, ndi2, make_float2(c2.z, c2.w));                          // F - (E + C di) di
+    const float2 gr = ffma2(make_float2(c0.z, c0.w), ndi2, make_float2(c1.z, c1.w));    // D + B di
+    const float2 an = make_float2(c0.x, c0.y);
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        const double djk = dj + (double)k;
-        const double w = fma(-fma(ab.x, djk, b1), djk, cc);      // 1 - d^T S d
-        const float t = fast_sqrt(d2f_pos_trunc(w));
-        acc[k] = fma(f2d_pos(t), Kd, acc[k]);
+        const float ndj = ndj0 - (float)k;
+        const float2 ndj2 = make_float2(ndj, ndj);
+        const float2 sl = ffma2(an, ndj2, gr);                   // D + B di + A dj
+        const float2 w2 = ffma2(sl, ndj2, wr);                   // w = F - (E + C di) di - (D + B di + A dj) dj
+        const float t = fast_sqrt(add_sat(w2.x, w2.y));
+        pend[k] = fmaf(t, K, pend[k]);
     }
 }
 
@@ -202,16 +225,15 @@ __device__ __noinline__ double prism_f64_px(const float4* __restrict__ rec, doub
                                     xd - (double)h3.x, yd - (double)h3.y);
 }
 
-// Prism (kind 1): 6 slabs, exit_k = Ex_k - U_k lx - V_k ly, enter_k = En_k - U_k lx - V_k ly from the re-based fp32
-// coefficients (packed FFMA2, two slabs per instruction), t = max(0, min_k exit_k - max_k enter_k) with 3-input
-// min / max.  The first NS (<= 2) slabs are steep (slope > kSteepSlope): their fp32 values are replaced, for every
-// pixel, by fp64 evaluations from the record (2 DFMA + 2 conversions per pixel and slab), so no pixel needs a
-// per-lane decision.
+// Prism (kind 1): 6 slabs, exit_k = Ex_k - U_k lx - V_k ly, enter_k = En_k - U_k lx - V_k ly from the re-based, scaled
+// fp32 coefficients (packed FFMA2, two slabs per instruction), s t = sat(min_k exit_k - max_k enter_k) with 3-input
+// min / max and a saturating subtraction.  The first NS (<= 2) slabs are steep (slope > kSteepSlope): their values are
+// the exact hi-part FMAs plus a packed lo-part FMA (one FFMA2 + 2 FADD per pixel and steep slab), no fp64.
 template <int NS>
-__device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, const float4* __restrict__ rec, float dnf,
-                                           const LaneGeom& g, double (&acc)[4])
+__device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, const LaneGeom& g, float (&pend)[4])
 {
     const float4 a0 = slot[0], a1 = slot[1], a2 = slot[2], a3 = slot[3], a4 = slot[4], a5 = slot[5];
+    const float dn = slot[6].y;
     const float2 v01 = make_float2(a4.z, a4.w), v23 = make_float2(a5.x, a5.y), v45 = make_float2(a5.z, a5.w);
     const float2 u01 = make_float2(a3.x, a3.y), u23 = make_float2(a3.z, a3.w), u45 = make_float2(a4.x, a4.y);
     // row terms: value of every plane at this lane's row, column offset 0
@@ -221,44 +243,46 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
     const float2 nk01 = ffma2(v01, g.nly, make_float2(a1.z, a1.w));
     const float2 nk23 = ffma2(v23, g.nly, make_float2(a2.x, a2.y));
     const float2 nk45 = ffma2(v45, g.nly, make_float2(a2.z, a2.w));
-    const double dnd = (double)dnf;
-    // steep slabs in fp64: slab 0 from the slot (re-based to the sub-tile origin), slab 1 from the record
-    double u0 = 0.0, x0 = 0.0, n0 = 0.0, u1 = 0.0, x1 = 0.0, n1 = 0.0, dj = 0.0;
+    float2 r0 = make_float2(0.f, 0.f), ul0 = r0, r1 = r0, ul1 = r0;   // lo parts of the steep slabs: (exit, enter) row terms, U
     if (NS > 0) {
-        const double2 xn = reinterpret_cast<const double2*>(slot)[7], uv = reinterpret_cast<const double2*>(slot)[8];
-        const double nly = (double)g.nly.x;
-        u0 = uv.x;
-        x0 = fma(uv.y, nly, xn.x);
-        n0 = fma(uv.y, nly, xn.y);
+        const float4 l = slot[7];
+        r0 = ffma2(make_float2(l.w, l.w), g.nly, make_float2(l.x, l.y));
+        ul0 = make_float2(l.z, l.z);
     }
     if (NS > 1) {
-        const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));
-        const double2* c = reinterpret_cast<const double2*>(rec + 4);
-        const double2 uv = __ldg(c + 2), xn = __ldg(c + 3);
-        dj = (double)g.xf - (double)h3.x;
-        const double di = (double)g.yf - (double)h3.y;
-        u1 = uv.x;
-        x1 = fma(-uv.y, di, xn.x);
-        n1 = fma(-uv.y, di, xn.y);
+        const float4 l = slot[8];
+        r1 = ffma2(make_float2(l.w, l.w), g.nly, make_float2(l.x, l.y));
+        ul1 = make_float2(l.z, l.z);
     }
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         float2 e01 = ffma2(u01, g.nlx[k], ek01), e23 = ffma2(u23, g.nlx[k], ek23), e45 = ffma2(u45, g.nlx[k], ek45);
         float2 n01 = ffma2(u01, g.nlx[k], nk01), n23 = ffma2(u23, g.nlx[k], nk23), n45 = ffma2(u45, g.nlx[k], nk45);
         if (NS > 0) {
-            const double nlxk = (double)g.nlx[k].x;
-            e01.x = (float)fma(u0, nlxk, x0);
-            n01.x = (float)fma(u0, nlxk, n0);
+            const float2 lo = ffma2(ul0, g.nlx[k], r0);
+            e01.x += lo.x;
+            n01.x += lo.y;
         }
         if (NS > 1) {
-            const double djk = dj + (double)k;
-            e01.y = (float)fma(-u1, djk, x1);
-            n01.y = (float)fma(-u1, djk, n1);
+            const float2 lo = ffma2(ul1, g.nlx[k], r1);
+            e01.y += lo.x;
+            n01.y += lo.y;
         }
         const float ex = fminf(min3(e01.x, e01.y, e23.x), min3(e23.y, e45.x, e45.y));
         const float en = fmaxf(max3(n01.x, n01.y, n23.x), max3(n23.y, n45.x, n45.y));
-        const float t = fmaxf(ex - en, 0.0f);
-        acc[k] = fma(f2d_pos(t), dnd, acc[k]);
+        pend[k] = fmaf(sub_sat(ex, en), dn, pend[k]);
+    }
+}
+
+// The evaluation loops add into fp32 partial sums; every kFlush survivors (and at the end of a class) these are widened
+// and added to the fp64 per-pixel accumulators: one ALU-pipe widening + DADD per pixel and kFlush particles.
+constexpr int kFlush = 4;
+__device__ __forceinline__ void flush(float (&pend)[4], double (&acc)[4])
+{
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        acc[k] += f2d(pend[k]);
+        pend[k] = 0.0f;
     }
 }
 
@@ -466,6 +490,7 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
     g.yf = (float)i;
     float4* my_slots = s_slots + (tid >> 5) * 32 * kSlotStride4;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    float pend[4] = {0.0f, 0.0f, 0.0f, 0.0f};
 
     const float4* recs4 = reinterpret_cast<const float4*>(a.rec);
     // entry of the first batch (the loop below always holds the next batch's entry in registers: the list loads of
@@ -500,9 +525,9 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
             else pos = n1 + n2 + n3 + n4 + __popc(m0 & lt);
             float4* sl = my_slots + pos * kSlotStride4;
             reinterpret_cast<uint32_t*>(sl)[27] = pid;
-            if (code == 0u) {                                    // ellipsoid: copy the record's doubles into the slot
+            if (code == 0u) {                                    // ellipsoid: copy the record's fp32 (hi, lo) coefficients into the slot
                 const float4* rec = recs4 + (size_t)pid * (kRecWords / 4);
-                const float4 c0 = __ldg(rec + 4), c1 = __ldg(rec + 5), c2 = __ldg(rec + 6), c3 = __ldg(rec + 7);
+                const float4 c0 = __ldg(rec + 10), c1 = __ldg(rec + 11), c2 = __ldg(rec + 12), c3 = __ldg(rec + 13);
                 const float K = __ldg(reinterpret_cast<const float*>(rec) + 9);
                 sl[0] = c0; sl[1] = c1; sl[2] = c2; sl[3] = c3;
                 reinterpret_cast<float*>(sl)[25] = K;
@@ -516,25 +541,37 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
             rebase_item(my_slots + r * kSlotStride4, a.rec, it - 6 * r, wx0, wy0);
         }
         __syncwarp();
-        // ---- all lanes walk the survivors, class by class ----------------------------------------------------------------------
+        // ---- all lanes walk the survivors, class by class; fp32 partial sums, flushed to fp64 every kFlush survivors ----------
         const float4* slot = my_slots;
-        {
 #pragma unroll 1
-        for (int sv = 0; sv < n1; ++sv, slot += kSlotStride4) eval_prism<0>(slot, nullptr, slot[6].y, g, acc);
+        for (int left = n1; left > 0; left -= kFlush) {
 #pragma unroll 1
-        for (int sv = 0; sv < n2; ++sv, slot += kSlotStride4) eval_prism<1>(slot, nullptr, slot[6].y, g, acc);
-#pragma unroll 1
-        for (int sv = 0; sv < n3 + n4; ++sv, slot += kSlotStride4) {
-            const float4* rec = recs4 + (size_t)__float_as_uint(slot[6].w) * (kRecWords / 4);
-            if (sv < n3) {
-                eval_prism<2>(slot, rec, slot[6].y, g, acc);
-            } else {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) acc[k] += prism_f64_px(rec, (double)(g.xf + (float)k), (double)g.yf);
-            }
+            for (int q = min(left, kFlush); q > 0; --q, slot += kSlotStride4) eval_prism<0>(slot, g, pend);
+            flush(pend, acc);
         }
 #pragma unroll 1
-        for (int sv = 0; sv < n0; ++sv, slot += kSlotStride4) eval_ellipsoid(slot, slot[6].y, g, acc);
+        for (int left = n2; left > 0; left -= kFlush) {
+#pragma unroll 1
+            for (int q = min(left, kFlush); q > 0; --q, slot += kSlotStride4) eval_prism<1>(slot, g, pend);
+            flush(pend, acc);
+        }
+#pragma unroll 1
+        for (int left = n3; left > 0; left -= kFlush) {
+#pragma unroll 1
+            for (int q = min(left, kFlush); q > 0; --q, slot += kSlotStride4) eval_prism<2>(slot, g, pend);
+            flush(pend, acc);
+        }
+#pragma unroll 1
+        for (int sv = 0; sv < n4; ++sv, slot += kSlotStride4) {
+            const float4* rec = recs4 + (size_t)__float_as_uint(slot[6].w) * (kRecWords / 4);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) acc[k] += prism_f64_px(rec, (double)(g.xf + (float)k), (double)g.yf);
+        }
+#pragma unroll 1
+        for (int left = n0; left > 0; left -= kFlush) {
+#pragma unroll 1
+            for (int q = min(left, kFlush); q > 0; --q, slot += kSlotStride4) eval_ellipsoid(slot, g, pend);
+            flush(pend, acc);
         }
         __syncwarp();
     }
