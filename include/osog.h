@@ -66,7 +66,7 @@ typedef struct {
     void*    stream;         /* cudaStream_t the context enqueues on (0 = legacy default stream)           */
     int32_t  H, W;           /* frame height / width in pixels, 1 .. 32768; need not be tile multiples     */
     int32_t  max_frames;     /* largest batch B of one call, >= 1                                          */
-    int64_t  max_particles;  /* largest N (total over the batch) of one call, >= 0                         */
+    int64_t  max_particles;  /* largest N (total over the batch) of one call, 0 .. 2^29 - 1                */
     int64_t  max_pairs;      /* capacity of the tile lists = largest TOTAL number of (particle, tile) pairs of one call
                                 (the compact CSR list that the device scan addresses); 0 = 64 * max_particles + 1024.
                                 How the pairs are spread over the tiles does not matter: one crowded tile may hold them all */

@@ -6,12 +6,13 @@
 //   2. per list entry, test the particle's pixel bounding box and oriented box against the tile's eight 16 x 8 pixel
 //      sub-tiles: 8-bit mask + evaluation code of the record -> meta.
 // k_compose_tile, two CTAs of four warps per tile, every warp independent (no barrier, no shared list):
-//   3. per warp (one sub-tile, 4 x 1 pixels per lane): walk the sorted list in batches of 32 entries, keep those whose
-//      mask bit is set (ballot compaction keeps ascending order inside an evaluation class), re-base the survivors'
-//      fp64 coefficients to the sub-tile origin, rounding them to fp32 only there,
-//   4. all lanes walk the survivors (grouped by evaluation class, one branch-free loop per class): ray-convex thickness
-//      from the re-based coefficients (packed fp32 FMA and 3-input min/max for the prism slabs, fp64 quadratic + fp32
-//      sqrt for the ellipsoid), OPD accumulated per pixel in fp64 registers,
+//   3. per warp (one sub-tile, 4 x 1 pixels per lane): walk the sorted list in batches of 32 entries and queue those whose
+//      mask bit is set; whenever 32 survivors are queued (or the list ends) every lane prepares ONE survivor: it re-bases
+//      a prism's fp64 slab coefficients to the sub-tile origin (rounding to fp32 only there), finds by an interval test
+//      which exit / entry planes can be active anywhere in the sub-tile, and picks the evaluation class,
+//   4. all lanes walk the prepared survivors class by class (one branch-free loop per class): ray-convex thickness from
+//      the re-based coefficients (packed fp32 FMA and 3-input min/max for the prism slabs, two-float fp32 quadratic + fp32
+//      sqrt for the ellipsoid), OPD accumulated per pixel in fp32 partial sums that are flushed to fp64 registers,
 //   5. write OPD and / or exp(i 2 pi OPD / lambda) * ramp straight from the registers.
 #include "osog_internal.cuh"
 
@@ -32,14 +33,15 @@ struct ComposeArgs {
 };
 
 constexpr int kWarps = kComposeThreads / 32;
-constexpr int kSlotStride4 = 9;                    // survivor slot stride in float4 (8 used, odd stride: conflict-free lane-per-slot writes)
+constexpr int kSlotStride4 = 11;                   // survivor slot stride in float4 (10 used, odd stride: conflict-free lane-per-slot writes)
+constexpr int kQueue = 64;                         // survivor queue entries per warp (32 being processed + up to 31 waiting)
 #ifndef OSOG_CTA_SPLIT
 #define OSOG_CTA_SPLIT 2
 #endif
 constexpr int kCtaSplit = OSOG_CTA_SPLIT;             // compose CTAs per tile (each takes kWarps / kCtaSplit sub-tiles)
 constexpr int kCtaWarps = kWarps / kCtaSplit;
 constexpr int kSmemSlots = kCtaWarps * 32 * kSlotStride4 * 16;
-constexpr int kSmemBytes = kSmemSlots;             // k_compose_tile: per-warp survivor slots only
+constexpr int kSmemBytes = kSmemSlots + kCtaWarps * kQueue * 4;   // k_compose_tile: per-warp survivor slots + survivor queues
 
 // ---- small PTX helpers ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float fast_sqrt(float x)
@@ -136,41 +138,80 @@ __device__ __noinline__ double prism_t64(const double* r64, uint32_t vmask, doub
     return t > 0.0 ? t : 0.0;
 }
 
-// ---- per-warp preparation of the prism survivors: work item = (survivor slot, slab q), one lane per item -------------
-// Re-base the slab's fp64 coefficients from the particle's reference pixel (jc, ic) to the warp's sub-tile origin
-// (wx0, wy0), scale them by the particle's chord scale s (record word 15: s t <= 1/2) and round to fp32 there: all later
-// fp32 arithmetic uses pixel offsets 0..15 / 0..7.
+// ---- preparation of one prism survivor by ONE lane (32 survivors are prepared at once, one per lane) --------------------
+// Evaluation classes of a prepared survivor:
+constexpr uint32_t kClsEllipsoid = 0u, kClsFull = 1u /* 1 + steep slabs: 1, 2, 3 */, kClsF64 = 4u, kClsPair = 5u, kClsNone = 7u;
+// For each of the 6 slabs: re-base its fp64 coefficients from the particle's reference pixel (jc, ic) to the warp's
+// sub-tile origin (wx0, wy0), scale them by the particle's chord scale s (record word 15: s t <= 1/2) and round to fp32
+// there: all later fp32 arithmetic uses pixel offsets 0..15 / 0..7.  Then an interval test over the
+// sub-tile: exit plane k takes values in [emin_k, emax_k]; it can be the lowest exit plane somewhere only if
+// emin_k <= min_q emax_q (likewise for the entry planes with max / min).  If the lowest possible exit lies below the
+// highest possible entry everywhere, the prism does not touch the sub-tile at all (kClsNone).  If at most two exit and two
+// entry planes remain, they are copied into a compact block (kClsPair: 2 + 2 planes instead of 6 + 6 per pixel).
 // A steep slab (slope > kSteepSlope; the first NS slabs of the record) is stored as (hi, lo) float pairs on an exact
 // grid: hi = multiple of q = 2^(e - 23), 2^e > every intermediate of  C - U lx - V ly  over the sub-tile, so the fp32 FMAs
-// on the hi parts are exact and hi + lo carries the fp64 value to 2^-24 relative of the (small) result.
+// on the hi parts are exact and hi + lo carries the fp64 value to 2^-24 relative of the (small) result; the class with the
+// lo-part FMAs (1 + NS) is only taken when a steep plane survives the interval test.
 // Slot layout (words): 0..5 Ex, 6..11 En, 12..17 U, 18..23 V (hi parts for steep slabs), 25 dn / s, 27 particle index,
-// 28..31 lo parts (Ex, En, U, V) of slab 0, 32..35 of slab 1.  An ellipsoid slot holds the record's words 40..53.
-__device__ __forceinline__ void rebase_item(float4* __restrict__ slot, const float* __restrict__ recs, int q, int wx0, int wy0)
+// 28..31 lo parts (Ex, En, U, V) of slab 0, 32..35 of slab 1; or, class kClsPair, words 28..39: Cx_a Cx_b Ux_a Ux_b |
+// Vx_a Vx_b Cn_c Cn_d | Un_c Un_d Vn_c Vn_d (exit planes a, b; entry planes c, d).  An ellipsoid slot holds the record's
+// words 40..53 in words 0..15.
+__device__ __forceinline__ uint32_t prep_prism(float4* __restrict__ slot, const float4* __restrict__ rec, int wx0, int wy0)
 {
     float* sw = reinterpret_cast<float*>(slot);
-    const uint32_t pid = __float_as_uint(sw[27]);
-    const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)pid * kRecWords);
     const float4 h2 = __ldg(rec + 2);                                  // flags, dn, cz, index
     const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));     // jc, ic, zmax, chord scale
     const double2* c = reinterpret_cast<const double2*>(rec + 4);
-    const double2 uv = __ldg(c + 2 * q), xn = __ldg(c + 2 * q + 1);    // U, V | Cx, Cn
     const float tsc = __int_as_float(h3.w);
-    if (q == 0) sw[25] = h2.y / tsc;                                   // dn / s (s is a power of two: exact)
+    sw[25] = h2.y / tsc;                                               // dn / s (s is a power of two: exact)
     const double sc = (double)tsc;
     const double oj = (double)(wx0 - h3.x), oi = (double)(wy0 - h3.y);
-    const double m = fma(uv.x, oj, uv.y * oi);
-    const double ex = (xn.x - m) * sc, en = (xn.y - m) * sc, u = uv.x * sc, v = uv.y * sc;
     const int ns = (int)((__float_as_uint(h2.x) >> 8) & 7u);
-    if (q >= ns) {
-        sw[q] = (float)ex; sw[6 + q] = (float)en; sw[12 + q] = (float)u; sw[18 + q] = (float)v;
-    } else {                                                           // steep slab (q = 0 or 1): exact-grid (hi, lo) pairs
-        const double mb = fmax(fabs(ex), fabs(en)) + 15.0 * fabs(u) + 7.0 * fabs(v);
-        const int e = ((__double2hiint(mb) >> 20) & 0x7ff) - 1021;     // mb < 2^e (one spare bit)
-        const double cq = __hiloint2double((e - 23 + 52 + 1023) << 20 | 0x80000, 0);   // 1.5 * 2^52 * q, q = 2^(e - 23)
-        const double exh = (ex + cq) - cq, enh = (en + cq) - cq, uh = (u + cq) - cq, vh = (v + cq) - cq;
-        sw[q] = (float)exh; sw[6 + q] = (float)enh; sw[12 + q] = (float)uh; sw[18 + q] = (float)vh;
-        slot[7 + q] = make_float4((float)(ex - exh), (float)(en - enh), (float)(u - uh), (float)(v - vh));
+    float emin[6], nmax[6];
+    float xlow = __int_as_float(0x7f800000), nhigh = __int_as_float(0xff800000);   // min_q emax_q, max_q nmin_q
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+        const double2 uv = __ldg(c + 2 * q), xn = __ldg(c + 2 * q + 1);    // U, V | Cx, Cn
+        const double m = fma(uv.x, oj, uv.y * oi);
+        const double ex = (xn.x - m) * sc, en = (xn.y - m) * sc, u = uv.x * sc, v = uv.y * sc;
+        float exf, enf, uf, vf;
+        if (q < 2 && q < ns) {                                         // steep slab: exact-grid (hi, lo) pairs
+            const double mb = fmax(fabs(ex), fabs(en)) + 15.0 * fabs(u) + 7.0 * fabs(v);
+            const int e = ((__double2hiint(mb) >> 20) & 0x7ff) - 1021; // mb < 2^e (one spare bit)
+            const double cq = __hiloint2double((e - 23 + 52 + 1023) << 20 | 0x80000, 0);   // 1.5 * 2^52 * q, q = 2^(e - 23)
+            const double exh = (ex + cq) - cq, enh = (en + cq) - cq, uh = (u + cq) - cq, vh = (v + cq) - cq;
+            exf = (float)exh; enf = (float)enh; uf = (float)uh; vf = (float)vh;
+            slot[7 + q] = make_float4((float)(ex - exh), (float)(en - enh), (float)(u - uh), (float)(v - vh));
+        } else {
+            exf = (float)ex; enf = (float)en; uf = (float)u; vf = (float)v;
+        }
+        sw[q] = exf; sw[6 + q] = enf; sw[12 + q] = uf; sw[18 + q] = vf;
+        // value range of  C - U lx - V ly  over lx in [0, 15], ly in [0, 7], padded for the fp32 roundings
+        const float au = 15.0f * uf, av = 7.0f * vf;
+        const float hi = -(fminf(au, 0.0f) + fminf(av, 0.0f)), lo = -(fmaxf(au, 0.0f) + fmaxf(av, 0.0f));
+        const float pad = 4.8e-7f * (fmaxf(fabsf(exf), fabsf(enf)) + fabsf(au) + fabsf(av));
+        emin[q] = exf + lo - pad;
+        nmax[q] = enf + hi + pad;
+        xlow = fminf(xlow, exf + hi + pad);
+        nhigh = fmaxf(nhigh, enf + lo - pad);
     }
+    if (!(xlow > nhigh)) return kClsNone;                              // empty chord everywhere in the sub-tile
+    uint32_t mx = 0u, mn = 0u;                                         // planes that can be active somewhere
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+        mx |= emin[q] <= xlow ? (1u << q) : 0u;
+        mn |= nmax[q] >= nhigh ? (1u << q) : 0u;
+    }
+    if ((mx | mn) & ((1u << ns) - 1u)) return kClsFull + (uint32_t)ns; // a steep plane matters here: lo-part classes
+    if (__popc(mx) > 2 || __popc(mn) > 2) return kClsFull;
+    const int a0 = __ffs(mx) - 1, c0 = __ffs(mn) - 1;
+    const uint32_t mx1 = mx & (mx - 1u), mn1 = mn & (mn - 1u);
+    const int a1 = mx1 ? __ffs(mx1) - 1 : a0, c1 = mn1 ? __ffs(mn1) - 1 : c0;      // a single plane is simply used twice
+    const float4 p0 = make_float4(sw[a0], sw[a1], sw[12 + a0], sw[12 + a1]);
+    const float4 p1 = make_float4(sw[18 + a0], sw[18 + a1], sw[6 + c0], sw[6 + c1]);
+    const float4 p2 = make_float4(sw[12 + c0], sw[12 + c1], sw[18 + c0], sw[18 + c1]);
+    slot[7] = p0; slot[8] = p1; slot[9] = p2;
+    return kClsPair;
 }
 
 // ---- sub-tile cull (tile_meta below): does the particle (header words 0..7: centre, oriented box, packed pixel bounding
@@ -274,15 +315,47 @@ __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, cons
     }
 }
 
+// Prism of which at most two exit and two entry planes can be active in this sub-tile (prep_prism): 2 + 2 plane values,
+// one min, one max per pixel.  Same fp32 coefficients as the full evaluation, so the result is the same number.
+__device__ __forceinline__ void eval_prism_pair(const float4* __restrict__ slot, const LaneGeom& g, float (&pend)[4])
+{
+    const float4 a = slot[7], b = slot[8], c = slot[9];
+    const float dn = slot[6].y;
+    const float2 xr = ffma2(make_float2(b.x, b.y), g.nly, make_float2(a.x, a.y));
+    const float2 nr = ffma2(make_float2(c.z, c.w), g.nly, make_float2(b.z, b.w));
+    const float2 xu = make_float2(a.z, a.w), nu = make_float2(c.x, c.y);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float2 e = ffma2(xu, g.nlx[k], xr), n = ffma2(nu, g.nlx[k], nr);
+        pend[k] = fmaf(sub_sat(fminf(e.x, e.y), fmaxf(n.x, n.y)), dn, pend[k]);
+    }
+}
+
 // The evaluation loops add into fp32 partial sums; every kFlush survivors (and at the end of a class) these are widened
-// and added to the fp64 per-pixel accumulators: one ALU-pipe widening + DADD per pixel and kFlush particles.
+// and added to the fp64 per-pixel accumulators: one widening conversion + DADD per pixel and kFlush particles.
 constexpr int kFlush = 4;
 __device__ __forceinline__ void flush(float (&pend)[4], double (&acc)[4])
 {
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        acc[k] += f2d(pend[k]);
+        acc[k] += (double)pend[k];
         pend[k] = 0.0f;
+    }
+}
+
+// all lanes evaluate the survivors whose bit is set in `m` (slot = survivor index), ascending, flushing every kFlush
+template <class Eval>
+__device__ __forceinline__ void run_class(unsigned m, const float4* __restrict__ my_slots, float (&pend)[4], double (&acc)[4], Eval eval)
+{
+#pragma unroll 1
+    while (m) {
+#pragma unroll 1
+        for (int q = 0; q < kFlush && m; ++q) {
+            const int r = __ffs(m) - 1;
+            m &= m - 1u;
+            eval(my_slots + r * kSlotStride4);
+        }
+        flush(pend, acc);
     }
 }
 
@@ -489,16 +562,19 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
     g.xf = (float)j;
     g.yf = (float)i;
     float4* my_slots = s_slots + (tid >> 5) * 32 * kSlotStride4;
+    uint32_t* my_queue = reinterpret_cast<uint32_t*>(smem + kSmemSlots) + (tid >> 5) * kQueue;   // particle index | class code << 29
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
     float pend[4] = {0.0f, 0.0f, 0.0f, 0.0f};
 
     const float4* recs4 = reinterpret_cast<const float4*>(a.rec);
+    const unsigned lt = (1u << lane) - 1u;
+    int nq = 0;                                                  // queued survivors (warp-uniform)
     // entry of the first batch (the loop below always holds the next batch's entry in registers: the list loads of
-    // batch n + 1 are in flight while batch n is evaluated)
+    // batch n + 1 are in flight while batch n is processed)
     uint32_t nmeta = lane < L ? gmeta[lane] : 0u;
     uint32_t npid = lane < L ? glist[lane] : 0u;
     for (uint32_t base = 0; base < L; base += 32) {
-        // ---- lane <-> list entry base + lane: survivors of this warp's sub-tile -------------------------------------------
+        // ---- lane <-> list entry base + lane: survivors of this warp's sub-tile join the queue, in list order ----------------
         const uint32_t meta = nmeta, pid = npid;
         {
             const uint32_t kn = base + 32 + lane;
@@ -506,74 +582,59 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
             npid = kn < L ? glist[kn] : 0u;
         }
         const bool keep = ((meta >> wid) & 1u) != 0u;
-        const uint32_t code = meta >> 8;
-        // Survivors are grouped by evaluation class (fixed, data-dependent order: NS0 prisms, NS1, NS2, all-fp64,
-        // ellipsoids; ascending particle index inside a class), so each class runs in its own branch-free loop.
-        const unsigned m1 = __ballot_sync(0xffffffffu, keep && code == 1u);
-        const unsigned m2 = __ballot_sync(0xffffffffu, keep && code == 2u);
-        const unsigned m3 = __ballot_sync(0xffffffffu, keep && code == 3u);
-        const unsigned m4 = __ballot_sync(0xffffffffu, keep && code == 4u);
-        const unsigned m0 = __ballot_sync(0xffffffffu, keep && code == 0u);
-        const int n1 = __popc(m1), n2 = __popc(m2), n3 = __popc(m3), n4 = __popc(m4), n0 = __popc(m0);
-        if (keep) {
-            const unsigned lt = (1u << lane) - 1u;
-            int pos;
-            if (code == 1u) pos = __popc(m1 & lt);
-            else if (code == 2u) pos = n1 + __popc(m2 & lt);
-            else if (code == 3u) pos = n1 + n2 + __popc(m3 & lt);
-            else if (code == 4u) pos = n1 + n2 + n3 + __popc(m4 & lt);
-            else pos = n1 + n2 + n3 + n4 + __popc(m0 & lt);
-            float4* sl = my_slots + pos * kSlotStride4;
-            reinterpret_cast<uint32_t*>(sl)[27] = pid;
-            if (code == 0u) {                                    // ellipsoid: copy the record's fp32 (hi, lo) coefficients into the slot
-                const float4* rec = recs4 + (size_t)pid * (kRecWords / 4);
-                const float4 c0 = __ldg(rec + 10), c1 = __ldg(rec + 11), c2 = __ldg(rec + 12), c3 = __ldg(rec + 13);
-                const float K = __ldg(reinterpret_cast<const float*>(rec) + 9);
-                sl[0] = c0; sl[1] = c1; sl[2] = c2; sl[3] = c3;
-                reinterpret_cast<float*>(sl)[25] = K;
+        const unsigned mk = __ballot_sync(0xffffffffu, keep);
+        if (keep) my_queue[nq + __popc(mk & lt)] = (pid & 0x1fffffffu) | ((meta >> 8) << 29);
+        nq += __popc(mk);
+        __syncwarp();
+        // ---- 32 survivors queued (or the list has ended): one lane prepares one survivor, then all lanes evaluate them ------------
+        const bool last = base + 32 >= L;
+        while (nq >= 32 || (last && nq > 0)) {
+            const int n = min(nq, 32);
+            uint32_t cls = kClsNone;
+            if (lane < n) {
+                const uint32_t ent = my_queue[lane];
+                const uint32_t spid = ent & 0x1fffffffu;
+                cls = ent >> 29;                                     // record code: 0 ellipsoid, 1..3 prism, 4 all-fp64 prism
+                const float4* rec = recs4 + (size_t)spid * (kRecWords / 4);
+                float4* sl = my_slots + lane * kSlotStride4;
+                reinterpret_cast<uint32_t*>(sl)[27] = spid;
+                if (cls == kClsEllipsoid) {                          // copy the record's fp32 (hi, lo) coefficients into the slot
+                    const float4 c0 = __ldg(rec + 10), c1 = __ldg(rec + 11), c2 = __ldg(rec + 12), c3 = __ldg(rec + 13);
+                    const float K = __ldg(reinterpret_cast<const float*>(rec) + 9);
+                    sl[0] = c0; sl[1] = c1; sl[2] = c2; sl[3] = c3;
+                    reinterpret_cast<float*>(sl)[25] = K;
+                } else if (cls != kClsF64) {
+                    cls = prep_prism(sl, rec, wx0, wy0);
+                }
             }
-        }
-        __syncwarp();
-        // ---- re-base the prisms (classes 1..3 occupy slots 0 .. n1+n2+n3-1): one lane per (prism, slab) -----------------------
-        const int npr = n1 + n2 + n3;
-        for (int it = lane; it < npr * 6; it += 32) {
-            const int r = it / 6;
-            rebase_item(my_slots + r * kSlotStride4, a.rec, it - 6 * r, wx0, wy0);
-        }
-        __syncwarp();
-        // ---- all lanes walk the survivors, class by class; fp32 partial sums, flushed to fp64 every kFlush survivors ----------
-        const float4* slot = my_slots;
+            const unsigned mp = __ballot_sync(0xffffffffu, cls == kClsPair);
+            const unsigned m1 = __ballot_sync(0xffffffffu, cls == kClsFull);
+            const unsigned m2 = __ballot_sync(0xffffffffu, cls == kClsFull + 1u);
+            const unsigned m3 = __ballot_sync(0xffffffffu, cls == kClsFull + 2u);
+            const unsigned m4 = __ballot_sync(0xffffffffu, cls == kClsF64);
+            const unsigned m0 = __ballot_sync(0xffffffffu, cls == kClsEllipsoid);
+            // the next 32 queue entries move to the front while the slots are being read
+            uint32_t moved = 0u;
+            if (32 + lane < nq) moved = my_queue[32 + lane];
+            __syncwarp();
+            if (32 + lane < nq) my_queue[lane] = moved;
+            nq -= n;
+            // Fixed, data-defined summation order: class by class (2 + 2 plane prisms, full prisms, one / two steep slabs,
+            // all-fp64 prisms, ellipsoids), ascending list position inside a class.
+            run_class(mp, my_slots, pend, acc, [&](const float4* slot) { eval_prism_pair(slot, g, pend); });
+            run_class(m1, my_slots, pend, acc, [&](const float4* slot) { eval_prism<0>(slot, g, pend); });
+            run_class(m2, my_slots, pend, acc, [&](const float4* slot) { eval_prism<1>(slot, g, pend); });
+            run_class(m3, my_slots, pend, acc, [&](const float4* slot) { eval_prism<2>(slot, g, pend); });
 #pragma unroll 1
-        for (int left = n1; left > 0; left -= kFlush) {
-#pragma unroll 1
-            for (int q = min(left, kFlush); q > 0; --q, slot += kSlotStride4) eval_prism<0>(slot, g, pend);
-            flush(pend, acc);
-        }
-#pragma unroll 1
-        for (int left = n2; left > 0; left -= kFlush) {
-#pragma unroll 1
-            for (int q = min(left, kFlush); q > 0; --q, slot += kSlotStride4) eval_prism<1>(slot, g, pend);
-            flush(pend, acc);
-        }
-#pragma unroll 1
-        for (int left = n3; left > 0; left -= kFlush) {
-#pragma unroll 1
-            for (int q = min(left, kFlush); q > 0; --q, slot += kSlotStride4) eval_prism<2>(slot, g, pend);
-            flush(pend, acc);
-        }
-#pragma unroll 1
-        for (int sv = 0; sv < n4; ++sv, slot += kSlotStride4) {
-            const float4* rec = recs4 + (size_t)__float_as_uint(slot[6].w) * (kRecWords / 4);
+            for (unsigned m = m4; m; m &= m - 1u) {
+                const float4* slot = my_slots + (__ffs(m) - 1) * kSlotStride4;
+                const float4* rec = recs4 + (size_t)__float_as_uint(slot[6].w) * (kRecWords / 4);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) acc[k] += prism_f64_px(rec, (double)(g.xf + (float)k), (double)g.yf);
+                for (int k = 0; k < 4; ++k) acc[k] += prism_f64_px(rec, (double)(g.xf + (float)k), (double)g.yf);
+            }
+            run_class(m0, my_slots, pend, acc, [&](const float4* slot) { eval_ellipsoid(slot, g, pend); });
+            __syncwarp();
         }
-#pragma unroll 1
-        for (int left = n0; left > 0; left -= kFlush) {
-#pragma unroll 1
-            for (int q = min(left, kFlush); q > 0; --q, slot += kSlotStride4) eval_ellipsoid(slot, g, pend);
-            flush(pend, acc);
-        }
-        __syncwarp();
     }
 
     // ---- H6/H7: write-out straight from the registers ----------------------------------------------------------------------

@@ -199,7 +199,7 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     if (!cfg || cfg->struct_size != sizeof(osog_config)) return OSOG_EINVAL;
     if (cfg->H < 1 || cfg->W < 1 || cfg->H > 32768 || cfg->W > 32768) return OSOG_EINVAL;
     if (cfg->max_frames < 1 || cfg->max_frames > 65535 || cfg->max_particles < 0 || cfg->max_pairs < 0) return OSOG_EINVAL;
-    if (cfg->max_particles > 0xfffffff0ll) return OSOG_EINVAL;
+    if (cfg->max_particles > 0x1fffffffll) return OSOG_EINVAL;       // 29-bit particle index in the survivor queues
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) return OSOG_ECUDA;
 
