@@ -15,6 +15,7 @@ struct PrepArgs {
     int B, H, W, ntx, nty;
     double pitch, n_medium;
     float* rec;
+    float* rec2;
     int4* tbox;
     int* pframe;
     uint32_t* count;              // this call's slot of the per-tile counters (all zero on entry)
@@ -228,76 +229,14 @@ __device__ void scan_counts(const PrepArgs& a)
     }
 }
 
-// Grid layout (blocks of 128 threads): [0, nbin) binning role, one particle per thread (nbin = max(1, nb): the scan needs
-// a block even when N = 0); [nbin, nbin + nb) record role, one particle per thread, the block's 128 particles permuted so
-// that prisms come first and ellipsoids last (warps are then uniform in the code path they take, except one mixed warp
-// per block); [nbin + nb, ...) ramp tables.  nb = ceil(N / 128).
-__global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
+// ---- record role of k_prepare (H1): EIGHT lanes per particle ------------------------------------------------------------
+// The derived record of a prism is a long fp64 dependency chain (rotation, 6 slab normals, slope ranking, a division and
+// an exact-grid split per slab, the oriented box): one thread per particle made k_prepare the latency-bound head of the
+// whole step.  Here the 8 lanes of a group all form the short common part (rotation, normals, slopes) and then split the
+// rest: lanes 0..5 one slab each (rank, coefficients, (hi, lo) pairs), lane 6 the oriented box and the header, lane 7 the
+// reference pixel / height bound / chord scale.  An ellipsoid uses lanes 0 (quadratic), 1 (oriented box), 7.
+__device__ __forceinline__ void record_role(const PrepArgs& a, long long n, int l8, unsigned gmask)
 {
-    pdl_trigger();                               // k_sort_cull's CTAs may become resident (they wait for this grid to finish)
-    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long nb = (a.N + kPrepThreads - 1) / kPrepThreads;
-    const long long nbin = nb > 0 ? nb : 1;
-
-    if (gid < a.B && gid < kOpticsChunk) a.optics[gid] = a.oc.f[gid];
-
-    if ((long long)blockIdx.x >= nbin + nb) {
-        // ---- phase-ramp tables exp(i 2 pi fx0 x_j), x_j = (j + 1/2) p  (oblique illumination, PAPER.md:113-115)
-        if (!a.has_ramp) return;
-        long long r = gid - (nbin + nb) * kPrepThreads;
-        const long long nx = (long long)a.B * a.W, ny = (long long)a.B * a.H;
-        if (r < nx) {
-            const int b = (int)(r / a.W), j = (int)(r % a.W);
-            const double f = b < kOpticsChunk ? a.oc.f[b].fx0_pitch : a.optics[b].fx0_pitch;
-            a.ramp_x[r] = cis_turns(f * (j + 0.5));
-        } else if (r - nx < ny) {
-            r -= nx;
-            const int b = (int)(r / a.H), i = (int)(r % a.H);
-            const double f = b < kOpticsChunk ? a.oc.f[b].fy0_pitch : a.optics[b].fy0_pitch;
-            a.ramp_y[r] = cis_turns(f * (i + 0.5));
-        }
-        return;
-    }
-
-    // ---- H1/H2: one particle = two threads in different blocks: role 0 does the binning (bounding box, tile range,
-    // counts), role 1 the derived record (the two halves are independent; splitting them halves the critical path)
-    const int role = (long long)blockIdx.x >= nbin ? 1 : 0;
-    long long n = (long long)(blockIdx.x - (role ? nbin : 0)) * kPrepThreads + threadIdx.x;
-    if (role == 1) {
-        __shared__ unsigned char s_perm[kPrepThreads];
-        __shared__ int s_np[kPrepThreads / 32];
-        const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-        const bool is_prism = n < a.N && a.kind[n] == 1u;
-        const unsigned mp = __ballot_sync(0xffffffffu, is_prism);
-        if (lane == 0) s_np[wid] = __popc(mp);
-        __syncthreads();
-        int before_p = 0, total_p = 0;
-#pragma unroll
-        for (int w = 0; w < kPrepThreads / 32; ++w) {
-            if (w < wid) before_p += s_np[w];
-            total_p += s_np[w];
-        }
-        const unsigned lt = (1u << lane) - 1u;
-        const int pos = is_prism ? before_p + __popc(mp & lt)
-                                 : total_p + (wid * 32 - before_p) + __popc(~mp & lt);
-        s_perm[pos] = (unsigned char)threadIdx.x;
-        __syncthreads();
-        n += (int)s_perm[threadIdx.x] - (int)threadIdx.x;
-    }
-    if (role == 0) {
-        binning_role(a, n);
-        // H3: the last binning block to get here scans the counts (the record role blocks are still busy: off the critical path)
-        __shared__ bool s_last;
-        __threadfence();                                          // this block's counter atomics before its done-ticket
-        __syncthreads();
-        if (threadIdx.x == 0) s_last = atomicAdd(a.done, 1u) == (uint32_t)(nbin - 1);
-        __syncthreads();
-        if (s_last) {
-            __threadfence();
-            scan_counts(a);
-        }
-        return;
-    }
     if (n >= a.N) return;
     const float fcx = a.cx[n], fcy = a.cy[n], fqw = a.qw[n], fqx = a.qx[n], fqy = a.qy[n], fqz = a.qz[n];
     const float fd0 = a.d0[n], fd1 = a.d1[n], fd2 = a.d2[n], fnp = a.n_p[n];
@@ -305,13 +244,10 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
     const bool valid = finite_f(fcx) && finite_f(fcy) && finite_f(fqw) && finite_f(fqx) && finite_f(fqy) && finite_f(fqz) &&
                  finite_f(fd0) && finite_f(fd1) && finite_f(fd2) && finite_f(fnp) &&
                  fd0 > 0.0f && fd1 > 0.0f && fd2 > 0.0f && kind <= 1u;
-
     if (!valid) {                                // flagged by the binning role
-        if (a.obb != nullptr)
-            for (int k = 0; k < 6; ++k) a.obb[(size_t)n * 6 + k] = __int_as_float(0x7fc00000);
+        if (a.obb != nullptr && l8 < 6) a.obb[(size_t)n * 6 + l8] = __int_as_float(0x7fc00000);
         return;
     }
-
     const double p = a.pitch;
     const double cx = fcx, cy = fcy;
     const double w = fqw, x = fqx, y = fqy, z = fqz;
@@ -324,33 +260,33 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
     float* r32 = a.rec + (size_t)n * kRecWords;
     uint32_t* r32u = reinterpret_cast<uint32_t*>(r32);
     const double ip = 1.0 / p;
-    // ---- H1 (role 1): derived record.  Coordinates are pixel offsets from pixel (jc, ic): dx = p dj + ox ----
+    // Coordinates are pixel offsets from pixel (jc, ic): dx = p dj + ox
     const double jc = fmin(fmax(floor(cx * ip), -1.0e6), 1.0e6);      // reference pixel: any nearby pixel will do
     const double ic = fmin(fmax(floor(cy * ip), -1.0e6), 1.0e6);
     const double ox = (jc + 0.5) * p - cx, oy = (ic + 0.5) * p - cy;
     const double dn = a.unit_dn ? 1.0 : (double)fnp - a.n_medium;
     double* r64 = reinterpret_cast<double*>(r32 + 16);
-    r32u[11] = (uint32_t)n;
-    reinterpret_cast<int*>(r32)[12] = (int)jc;
-    reinterpret_cast<int*>(r32)[13] = (int)ic;
-    // word 14: upper bound of the chord's top relative to the centre (G-buffer: a particle whose cz + bound lies below
-    // every top already found in a sub-tile is skipped); padded for the not-quite-orthogonal R of reading A4
-    {
-        double zmax;
-        if (kind == 0u) {
-            zmax = sqrt(R20 * R20 * e0 * e0 + R21 * R21 * e1 * e1 + R22 * R22 * e2 * e2);
-        } else {
-            const double hs = 0.5 * e0, hl = 0.5 * e1;
-            zmax = fabs(R22) * (hl + e2);
-            zmax = fmax(zmax, fabs(R20) * hs + fabs(R21) * hs + fabs(R22) * hl);
-        }
+    // upper bound of the chord's top relative to the centre (word 14; G-buffer: a particle whose cz + bound lies below every
+    // top already found in a sub-tile is skipped; padded for the not-quite-orthogonal R of reading A4), and the chord scale
+    // (word 15): the power of two s with s * chord <= 1/2 for every chord of the body (chord <= 2 zmax): the composition
+    // evaluates s * t with a saturating subtraction (clamp to [0, 1] for free) and folds 1 / s into the index contrast
+    double zmax;
+    if (kind == 0u) {
+        zmax = sqrt(R20 * R20 * e0 * e0 + R21 * R21 * e1 * e1 + R22 * R22 * e2 * e2);
+    } else {
+        const double hs = 0.5 * e0, hl = 0.5 * e1;
+        zmax = fabs(R22) * (hl + e2);
+        zmax = fmax(zmax, fabs(R20) * hs + fabs(R21) * hs + fabs(R22) * hl);
+    }
+    int ex2 = ((__double2hiint(2.0 * zmax * (1.0 + 1.0e-5) + 2.0e-6) >> 20) & 0x7ff) - 1022;     // 2 zmax < 2^ex2
+    ex2 = min(max(ex2 + 1, -60), 60);
+    const float tscf = __int_as_float((127 - ex2) << 23);
+    if (l8 == 7) {
+        r32u[11] = (uint32_t)n;
+        reinterpret_cast<int*>(r32)[12] = (int)jc;
+        reinterpret_cast<int*>(r32)[13] = (int)ic;
         r32[14] = __double2float_ru(zmax * (1.0 + 1.0e-5) + 1.0e-6);
-        // word 15: power of two s with s * chord <= 1/2 for every chord of the body (chord <= 2 zmax): the composition
-        // evaluates s * t with a saturating subtraction (clamp to [0, 1] for free) and folds 1 / s into the index contrast
-        int ex2 = 0;
-        frexp(2.0 * zmax * (1.0 + 1.0e-5) + 2.0e-6, &ex2);      // 2 zmax < 2^ex2
-        ex2 = min(max(ex2 + 1, -60), 60);
-        r32[15] = (float)ldexp(1.0, -ex2);
+        r32[15] = tscf;
     }
     // Words 2..5: oriented box of the silhouette (unit axis with a_x >= 0, half lengths > 0); their sign bits carry the
     // evaluation code of the particle (0 ellipsoid, 1 + number of steep slabs, 4 all-fp64): bit 0 in the sign of
@@ -358,6 +294,7 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
     const double cull_pad = 1.0 / 64.0;          // px; covers the fp32 rounding of the cull test
 
     if (kind == 0u) {
+        if (l8 > 1) return;
         // M = R diag(1/a^2, 1/b^2, 1/c^2) R^T; chord of {q^T M q <= 1} along z at (dx, dy):
         // t = T0 sqrt(1 - d^T S d), S = Schur complement of M_zz, T0 = 2 / sqrt(M_zz)   (H5)
         const double i0s = 1.0 / (e0 * e0), i1s = 1.0 / (e1 * e1), i2s = 1.0 / (e2 * e2);
@@ -369,40 +306,45 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
         const double Mzz = R20 * i0s * R20 + R21 * i1s * R21 + R22 * i2s * R22;
         const double iMzz = 1.0 / Mzz;
         const double Sxx = Mxx - Mxz * Mxz * iMzz, Sxy = Mxy - Mxz * Myz * iMzz, Syy = Myy - Myz * Myz * iMzz;
-        const double T0 = 2.0 * rsqrt(Mzz);
-        // w(dj, di) = F1 - (A dj^2 + B dj di + C di^2 + D dj + E di)
-        r64[0] = Sxx * p * p;
-        r64[1] = 2.0 * Sxy * p * p;
-        r64[2] = Syy * p * p;
-        r64[3] = 2.0 * p * (Sxx * ox + Sxy * oy);
-        r64[4] = 2.0 * p * (Sxy * ox + Syy * oy);
-        r64[5] = 1.0 - (Sxx * ox * ox + 2.0 * Sxy * ox * oy + Syy * oy * oy);
-        r64[6] = jc;
-        r64[7] = ic;
-        // Words 40..53: the same quadratic for the composition kernel as (hi, lo) float pairs on an exact grid: hi is a
-        // multiple of q = 2^(e - 23) where 2^e bounds every intermediate of the Horner evaluation over the pixels the
-        // kernel can ask for (|dj| <= Rj, |di| <= Ri), so the fp32 FMAs on the hi parts are exact (integers times q below
-        // 2^24 q); lo = the remainder, fp32.  Signs arranged for w = F + (E + Cn ndi) ndi + (D + Bn ndi + An ndj) ndj with
-        // ndj = -(j - jc), ndi = -(i - ic): An = -A, Bn = -B, Cn = -C.
-        {
+        if (l8 == 0) {
+            const double T0 = 2.0 * rsqrt(Mzz);
+            // w(dj, di) = F1 - (A dj^2 + B dj di + C di^2 + D dj + E di)
+            const double cA = Sxx * p * p, cB = 2.0 * Sxy * p * p, cC = Syy * p * p;
+            const double cD = 2.0 * p * (Sxx * ox + Sxy * oy), cE = 2.0 * p * (Sxy * ox + Syy * oy);
+            const double cF = 1.0 - (Sxx * ox * ox + 2.0 * Sxy * ox * oy + Syy * oy * oy);
+            r64[0] = cA; r64[1] = cB; r64[2] = cC; r64[3] = cD; r64[4] = cE; r64[5] = cF;
+            r64[6] = jc;
+            r64[7] = ic;
+            // Words 40..53: the same quadratic for the composition kernel as (hi, lo) float pairs on an exact grid: hi is a
+            // multiple of q = 2^(e - 22) where 2^e bounds every intermediate of the Horner evaluation over the pixels the
+            // kernel can ask for (|dj| <= Rj, |di| <= Ri), so the fp32 FMAs on the hi parts are exact (integers times q below
+            // 2^24 q); lo = the remainder, fp32.  Signs arranged for w = F + (E + Cn ndi) ndi + (D + Bn ndi + An ndj) ndj with
+            // ndj = -(j - jc), ndi = -(i - ic): An = -A, Bn = -B, Cn = -C.
             const double det = Sxx * Syy - Sxy * Sxy;
             const double Rj = sqrt(fmax(Syy / det, 0.0)) * ip + 20.0, Ri = sqrt(fmax(Sxx / det, 0.0)) * ip + 20.0;
-            double Mb = 1.0 + fabs(r64[5]) + (fabs(r64[2]) * Ri + fabs(r64[4])) * Ri + (fabs(r64[0]) * Rj + fabs(r64[1]) * Ri + fabs(r64[3])) * Rj;
+            double Mb = 1.0 + fabs(cF) + (fabs(cC) * Ri + fabs(cE)) * Ri + (fabs(cA) * Rj + fabs(cB) * Ri + fabs(cD)) * Rj;
             if (!(Mb < 1.0e30)) Mb = 1.0e30;                   // degenerate shape: the grid is coarse, the result stays finite
-            int eb = 0;
-            frexp(Mb, &eb);
-            const double q = ldexp(1.0, eb - 22), iq = ldexp(1.0, 22 - eb);
-            const double v[6] = {-r64[0], -r64[1], -r64[2], r64[3], r64[4], r64[5]};
+            const int eb = ((__double2hiint(Mb) >> 20) & 0x7ff) - 1022;                     // Mb < 2^eb
+            const double cq = __hiloint2double(((eb - 22 + 52 + 1023) << 20) | 0x80000, 0);  // 1.5 * 2^52 * q, q = 2^(eb - 22)
+            const double v[6] = {-cA, -cB, -cC, cD, cE, cF};
 #pragma unroll
             for (int k = 0; k < 6; ++k) {
-                const double hi = rint(v[k] * iq) * q;
+                const double hi = (v[k] + cq) - cq;
                 r32[40 + 2 * k] = (float)hi;
                 r32[41 + 2 * k] = (float)(v[k] - hi);
             }
             r32[52] = (float)jc;
             r32[53] = (float)ic;
+            r32u[8] = 0u;
+            r32[9] = (float)(dn * T0);
+            // chord midpoint z = -(M_xz dx + M_yz dy) / M_zz as Z0 + Zx dj + Zy di, and T0 (G-buffer only)
+            r64[8] = -(Mxz * ox + Myz * oy) * iMzz;
+            r64[9] = -Mxz * p * iMzz;
+            r64[10] = -Myz * p * iMzz;
+            r64[11] = T0;
+            return;
         }
-        // oriented box of the silhouette ellipse {d^T S d <= 1}: principal axes of S
+        // lane 1: oriented box of the silhouette ellipse {d^T S d <= 1}: principal axes of S
         const double hd = 0.5 * (Sxx - Syy), rad = sqrt(hd * hd + Sxy * Sxy), mid = 0.5 * (Sxx + Syy);
         const double lmin = fmax(mid - rad, 1.0e-300), lmax = mid + rad;
         double vx = Sxy, vy = lmin - Sxx;        // eigenvector of the small eigenvalue = long axis
@@ -415,14 +357,7 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
         r32[3] = (float)(vy * ivn);
         r32[4] = (float)(rsqrt(lmin) * ip * (1.0 + 1.0e-5) + cull_pad);
         r32[5] = (float)(rsqrt(lmax) * ip * (1.0 + 1.0e-5) + cull_pad);
-        r32u[8] = 0u;
-        r32[9] = (float)(dn * T0);
         r32[10] = a.cz != nullptr ? a.cz[n] : 0.0f;          // centre height (G-buffer depth map only)
-        // chord midpoint z = -(M_xz dx + M_yz dy) / M_zz as Z0 + Zx dj + Zy di, and T0 (G-buffer only)
-        r64[8] = -(Mxz * ox + Myz * oy) * iMzz;
-        r64[9] = -Mxz * p * iMzz;
-        r64[10] = -Myz * p * iMzz;
-        r64[11] = T0;
         if (a.obb != nullptr) {                  // label (reading A23): principal-axis box of the silhouette ellipse, no padding
             float* ob = a.obb + (size_t)n * 6;
             ob[0] = (float)(cx * ip - 0.5); ob[1] = (float)(cy * ip - 0.5);
@@ -446,43 +381,68 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
     nx[3] = R00 * hc - R02 * hs2; ny[3] = R10 * hc - R12 * hs2; nz[3] = R20 * hc - R22 * hs2;
     nx[4] = R01 * hc + R02 * hs2; ny[4] = R11 * hc + R12 * hs2; nz[4] = R21 * hc + R22 * hs2;
     nx[5] = R01 * hc - R02 * hs2; ny[5] = R11 * hc - R12 * hs2; nz[5] = R21 * hc - R22 * hs2;
-#pragma unroll
-    for (int k = 0; k < 6; ++k) { h2[k] = nx[k] * nx[k] + ny[k] * ny[k]; z2[k] = nz[k] * nz[k]; }
-    uint32_t flags = kFlagPrism;
-    int ns = 0;
     const double g0sq = (double)kSteepSlope * (double)kSteepSlope, gasq = kAllF64Slope * kAllF64Slope;
+    int ns = 0;
+    bool allf64 = false;
 #pragma unroll
     for (int k = 0; k < 6; ++k) {
-        int q = 0;                                   // rank of slab k: number of slabs steeper than it (ties: lower index first)
+        h2[k] = nx[k] * nx[k] + ny[k] * ny[k];
+        z2[k] = nz[k] * nz[k];
+        ns += (nz[k] == 0.0 || h2[k] > g0sq * z2[k]) ? 1 : 0;
+        allf64 = allf64 || nz[k] == 0.0 || h2[k] > gasq * z2[k];
+    }
+    if (ns > 2) allf64 = true;                   // more than two steep slabs: rare, every pixel goes to fp64
+    uint32_t vbit = 0u;
+    if (l8 < 6) {
+        // this lane's slab k = l8 (selected with constant indices: the arrays stay in registers)
+        double nxk = nx[0], nyk = ny[0], nzk = nz[0], h2k = h2[0], z2k = z2[0];
+#pragma unroll
+        for (int k = 1; k < 6; ++k)
+            if (k == l8) { nxk = nx[k]; nyk = ny[k]; nzk = nz[k]; h2k = h2[k]; z2k = z2[k]; }
+        int q = 0;                                   // rank of the slab: number of slabs steeper than it (ties: lower index first)
 #pragma unroll
         for (int j = 0; j < 6; ++j) {
-            if (j == k) continue;
-            const double lhs = h2[j] * z2[k], rhs = h2[k] * z2[j];      // slope_j > slope_k  <=>  lhs > rhs
-            q += (lhs > rhs || (lhs == rhs && j < k)) ? 1 : 0;
+            const double lhs = h2[j] * z2k, rhs = h2k * z2[j];      // slope_j > slope_k  <=>  lhs > rhs
+            q += (j != l8 && (lhs > rhs || (lhs == rhs && j < l8))) ? 1 : 0;
         }
-        const double bk = k < 2 ? hs2 : bcap;
-        double* o4 = r64 + 4 * q;
-        if (nz[k] == 0.0) {
+        const double bk = l8 < 2 ? hs2 : bcap;
+        double o0, o1, o2, o3;
+        if (nzk == 0.0) {
             // vertical face pair: no z bound; the line is inside the slab iff |n_x dx + n_y dy| <= b
-            o4[0] = nx[k] * p;
-            o4[1] = ny[k] * p;
-            o4[2] = nx[k] * ox + ny[k] * oy;
-            o4[3] = bk;
-            flags |= kFlagAllF64 | (1u << (16 + q));
-            ++ns;
+            o0 = nxk * p; o1 = nyk * p; o2 = nxk * ox + nyk * oy; o3 = bk;
+            vbit = 1u << (16 + q);
         } else {
-            const double r = (nz[k] > 0.0 ? 1.0 : -1.0) / fabs(nz[k]);  // sigma / |n_z|
-            const double W0 = r * (nx[k] * ox + ny[k] * oy), Cb = bk * fabs(r);
-            o4[0] = r * nx[k] * p;                    // U:  exit_k = Cx - U dj - V di
-            o4[1] = r * ny[k] * p;                    // V:  enter_k = Cn - U dj - V di
-            o4[2] = Cb - W0;                          // Cx
-            o4[3] = -Cb - W0;                         // Cn
-            if (h2[k] > gasq * z2[k]) flags |= kFlagAllF64;
-            if (h2[k] > g0sq * z2[k]) ++ns;
+            const double r = (nzk > 0.0 ? 1.0 : -1.0) / fabs(nzk);  // sigma / |n_z|
+            const double W0 = r * (nxk * ox + nyk * oy), Cb = bk * fabs(r);
+            o0 = r * nxk * p;                         // U:  exit_k = Cx - U dj - V di
+            o1 = r * nyk * p;                         // V:  enter_k = Cn - U dj - V di
+            o2 = Cb - W0;                             // Cx
+            o3 = -Cb - W0;                            // Cn
         }
+        double2* o4 = reinterpret_cast<double2*>(r64 + 4 * q);
+        o4[0] = make_double2(o0, o1);
+        o4[1] = make_double2(o2, o3);
+        // The slab once more for the composition kernel, scaled by the chord scale s (word 15) and split into (hi, lo)
+        // float pairs on an exact grid: hi = multiple of q_k = 2^(e_k - 22) with 2^e_k above every intermediate of
+        // C - U oj - V oi for all sub-tile origins (oj, oi) the kernel can ask for (|oj| + |oi| <= the body's diameter in
+        // pixels + 64), so the kernel's fp32 FMAs on the hi parts are exact and hi + lo reproduces the fp64 re-basing to
+        // ~2^-47 of that bound.  Layout per slab: (U_h, V_h, Cx_h, Cn_h), (U_l, V_l, Cx_l, Cn_l).
+        const double reach = (1.5 * s + L + 2.0 * hc) * ip + 64.0;
+        double mb = fmax(fabs(o2), fabs(o3)) + reach * (fabs(o0) + fabs(o1));
+        if (!(mb < 1.0e30)) mb = 1.0e30;
+        const int eb = ((__double2hiint(mb) >> 20) & 0x7ff) - 1022;                      // mb < 2^eb
+        const double cq = __hiloint2double(((eb - 22 + 52 + 1023) << 20) | 0x80000, 0);   // 1.5 * 2^52 * q, q = 2^(eb - 22)
+        const double h0 = (o0 + cq) - cq, h1 = (o1 + cq) - cq, h2s = (o2 + cq) - cq, h3s = (o3 + cq) - cq;
+        float4* pw = reinterpret_cast<float4*>(a.rec2 + (size_t)n * kPairWords) + 2 * q;
+        pw[0] = make_float4((float)h0 * tscf, (float)h1 * tscf, (float)h2s * tscf, (float)h3s * tscf);
+        pw[1] = make_float4((float)(o0 - h0) * tscf, (float)(o1 - h1) * tscf, (float)(o2 - h2s) * tscf, (float)(o3 - h3s) * tscf);
     }
-    if (ns > 2) flags |= kFlagAllF64;            // more than two steep slabs: rare, every pixel goes to fp64
-    flags |= (uint32_t)ns << 8;
+    // which ranks hold a vertical slab: OR over the group's lanes
+#pragma unroll
+    for (int d = 1; d < 8; d <<= 1) vbit |= __shfl_xor_sync(gmask, vbit, d);
+    if (l8 != 6) return;
+    uint32_t flags = kFlagPrism | vbit | ((uint32_t)ns << 8);
+    if (allf64) flags |= kFlagAllF64;
     // oriented box of the silhouette: along the projected long axis (body z) and across it, over the 10 vertices
     double ax = R02, ay = R12;
     const double an = sqrt(ax * ax + ay * ay);
@@ -497,7 +457,7 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
         hb = fmax(hb, fabs(-px * ay + py * ax));
     }
     if (ax < 0.0) { ax = -ax; ay = -ay; }
-    const uint32_t code = (flags & kFlagAllF64) ? 4u : 1u + (uint32_t)ns;
+    const uint32_t code = allf64 ? 4u : 1u + (uint32_t)ns;
     r32u[2] = (__float_as_uint((float)ax) & 0x7fffffffu) | ((code >> 2) << 31);
     r32[3] = (float)ay;
     r32u[4] = __float_as_uint((float)(ha * ip * (1.0 + 1.0e-5) + cull_pad)) | ((code & 1u) << 31);
@@ -511,6 +471,67 @@ __global__ void __launch_bounds__(kPrepThreads, 5) k_prepare(const PrepArgs a)
         ob[2] = (float)ax; ob[3] = (float)ay;
         ob[4] = (float)(ha * ip); ob[5] = (float)(hb * ip);
     }
+}
+
+constexpr int kRecPerBlock = kPrepThreads / 8;     // particles per record-role block
+
+// Grid layout (blocks of 128 threads): [0, nbin) binning role, one particle per thread (nbin = max(1, ceil(N / 128)): the
+// scan needs a block even when N = 0); [nbin, nbin + nrec) record role, 16 particles per block, 8 lanes each, the block's
+// particles permuted so that prisms come first (its warps are then uniform in the code path they take, except one mixed
+// warp per block); [nbin + nrec, ...) ramp tables.  nrec = ceil(N / 16).
+__global__ void __launch_bounds__(kPrepThreads, 6) k_prepare(const PrepArgs a)
+{
+    pdl_trigger();                               // k_sort_cull's CTAs may become resident (they wait for this grid to finish)
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long nb = (a.N + kPrepThreads - 1) / kPrepThreads;
+    const long long nbin = nb > 0 ? nb : 1;
+    const long long nrec = (a.N + kRecPerBlock - 1) / kRecPerBlock;
+
+    if (gid < a.B && gid < kOpticsChunk) a.optics[gid] = a.oc.f[gid];
+
+    if ((long long)blockIdx.x >= nbin + nrec) {
+        // ---- phase-ramp tables exp(i 2 pi fx0 x_j), x_j = (j + 1/2) p  (oblique illumination, PAPER.md:113-115)
+        if (!a.has_ramp) return;
+        long long r = gid - (nbin + nrec) * kPrepThreads;
+        const long long nx = (long long)a.B * a.W, ny = (long long)a.B * a.H;
+        if (r < nx) {
+            const int b = (int)(r / a.W), j = (int)(r % a.W);
+            const double f = b < kOpticsChunk ? a.oc.f[b].fx0_pitch : a.optics[b].fx0_pitch;
+            a.ramp_x[r] = cis_turns(f * (j + 0.5));
+        } else if (r - nx < ny) {
+            r -= nx;
+            const int b = (int)(r / a.H), i = (int)(r % a.H);
+            const double f = b < kOpticsChunk ? a.oc.f[b].fy0_pitch : a.optics[b].fy0_pitch;
+            a.ramp_y[r] = cis_turns(f * (i + 0.5));
+        }
+        return;
+    }
+
+    if ((long long)blockIdx.x < nbin) {
+        // ---- H2 + first half of H4: binning role, one particle per thread
+        binning_role(a, (long long)blockIdx.x * kPrepThreads + threadIdx.x);
+        // H3: the last binning block to get here scans the counts (the record role blocks are still busy: off the critical path)
+        __shared__ bool s_last;
+        __threadfence();                                          // this block's counter atomics before its done-ticket
+        __syncthreads();
+        if (threadIdx.x == 0) s_last = atomicAdd(a.done, 1u) == (uint32_t)(nbin - 1);
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            scan_counts(a);
+        }
+        return;
+    }
+
+    // ---- H1: record role, 8 lanes per particle; group g of the block takes the g-th particle in "prisms first" order
+    const int lane = threadIdx.x & 31;
+    const long long n0 = (long long)(blockIdx.x - nbin) * kRecPerBlock;
+    const long long np_ = n0 + (lane & (kRecPerBlock - 1));
+    const bool is_prism = np_ < a.N && a.kind[np_] == 1u;
+    const unsigned mp = __ballot_sync(0xffffffffu, is_prism) & ((1u << kRecPerBlock) - 1u);
+    const int g = threadIdx.x >> 3, npr = __popc(mp);
+    const int slot = g < npr ? (int)__fns(mp, 0, g + 1) : (int)__fns(~mp & ((1u << kRecPerBlock) - 1u), 0, g - npr + 1);
+    record_role(a, n0 + slot, threadIdx.x & 7, 0xffu << (lane & 24));
 }
 
 __global__ void k_set_optics(FrameOptics* optics, const OpticsChunk oc)
@@ -591,7 +612,7 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     a.frame_start = B > 1 ? p->frame_start : nullptr;
     a.N = N; a.B = B; a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
     a.pitch = o->pitch_um; a.n_medium = o->n_medium;
-    a.rec = c->rec; a.tbox = c->tbox; a.pframe = c->pframe;
+    a.rec = c->rec; a.rec2 = c->rec2; a.tbox = c->tbox; a.pframe = c->pframe;
     a.count = c->count + (size_t)c->status_idx * c->count_stride; a.slices = c->slices; a.slice_cap = c->slice_cap;
     a.offset = c->offset; a.done = c->done; a.max_pairs = c->max_pairs;
     a.obb = d_obb;
@@ -602,8 +623,9 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
 
     const int threads = kPrepThreads;
     const long long nb = (N + threads - 1) / threads;
+    const long long nrec = (N + kRecPerBlock - 1) / kRecPerBlock;
     const long long ramp_items = a.has_ramp ? (long long)B * (c->W + c->H) : 0;
-    long long blocks = (nb > 0 ? nb : 1) + nb + (ramp_items + threads - 1) / threads;
+    long long blocks = (nb > 0 ? nb : 1) + nrec + (ramp_items + threads - 1) / threads;
     if (blocks * threads < B) blocks = (B + threads - 1) / threads;     // the first threads also upload the optics
     k_prepare<<<(unsigned)blocks, threads, 0, c->stream>>>(a);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;

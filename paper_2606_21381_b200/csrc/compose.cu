@@ -20,6 +20,7 @@ namespace osog {
 
 struct ComposeArgs {
     const float* rec;
+    const float* rec2;           // prism slab coefficients as (hi, lo) float pairs (k_prepare)
     const uint32_t* offset;      // [tiles + 1] exclusive scan of the per-tile list lengths (k_prepare)
     const uint32_t* list;        // CSR list, every tile's segment sorted by k_sort_cull
     const uint16_t* meta;        // per list entry
@@ -141,59 +142,58 @@ __device__ __noinline__ double prism_t64(const double* r64, uint32_t vmask, doub
 // ---- preparation of one prism survivor by ONE lane (32 survivors are prepared at once, one per lane) --------------------
 // Evaluation classes of a prepared survivor:
 constexpr uint32_t kClsEllipsoid = 0u, kClsFull = 1u /* 1 + steep slabs: 1, 2, 3 */, kClsF64 = 4u, kClsPair = 5u, kClsNone = 7u;
-// For each of the 6 slabs: re-base its fp64 coefficients from the particle's reference pixel (jc, ic) to the warp's
-// sub-tile origin (wx0, wy0), scale them by the particle's chord scale s (record word 15: s t <= 1/2) and round to fp32
-// there: all later fp32 arithmetic uses pixel offsets 0..15 / 0..7.  Then an interval test over the
-// sub-tile: exit plane k takes values in [emin_k, emax_k]; it can be the lowest exit plane somewhere only if
-// emin_k <= min_q emax_q (likewise for the entry planes with max / min).  If the lowest possible exit lies below the
-// highest possible entry everywhere, the prism does not touch the sub-tile at all (kClsNone).  If at most two exit and two
-// entry planes remain, they are copied into a compact block (kClsPair: 2 + 2 planes instead of 6 + 6 per pixel).
-// A steep slab (slope > kSteepSlope; the first NS slabs of the record) is stored as (hi, lo) float pairs on an exact
-// grid: hi = multiple of q = 2^(e - 23), 2^e > every intermediate of  C - U lx - V ly  over the sub-tile, so the fp32 FMAs
-// on the hi parts are exact and hi + lo carries the fp64 value to 2^-24 relative of the (small) result; the class with the
-// lo-part FMAs (1 + NS) is only taken when a steep plane survives the interval test.
+// For each of the 6 slabs: re-base its coefficients from the particle's reference pixel (jc, ic) to the warp's sub-tile
+// origin (wx0, wy0) and round to fp32 there: all later fp32 arithmetic uses pixel offsets 0..15 / 0..7 (DESIGN.md section
+// 6).  The re-basing itself runs in fp32 on the record's exact-grid (hi, lo) pairs (k_prepare; already scaled by the
+// particle's chord scale s, s t <= 1/2): the FMAs on the hi parts are exact, so hi + lo carries the fp64 result.  Then an
+// interval test over the sub-tile: exit plane k takes values in [emin_k, emax_k]; it can be the lowest exit plane somewhere
+// only if emin_k <= min_q emax_q (likewise for the entry planes with max / min).  If the lowest possible exit lies below
+// the highest possible entry everywhere, the prism does not touch the sub-tile at all (kClsNone).  If at most two exit and
+// two entry planes remain, they are copied into a compact block (kClsPair: 2 + 2 planes instead of 6 + 6 per pixel).
+// A steep slab (slope > kSteepSlope; the first NS slabs of the record) is stored again as (hi, lo) pairs, now on the
+// finer grid of the sub-tile: hi = multiple of q = 2^(e - 21), 2^e > every intermediate of  C - U lx - V ly  over the
+// sub-tile, so the evaluation's fp32 FMAs on the hi parts are exact and hi + lo is good to 2^-24 relative of the (small)
+// result; the class with the lo-part FMAs (1 + NS) is only taken when a steep plane survives the interval test.
 // Slot layout (words): 0..5 Ex, 6..11 En, 12..17 U, 18..23 V (hi parts for steep slabs), 25 dn / s, 27 particle index,
 // 28..31 lo parts (Ex, En, U, V) of slab 0, 32..35 of slab 1; or, class kClsPair, words 28..39: Cx_a Cx_b Ux_a Ux_b |
 // Vx_a Vx_b Cn_c Cn_d | Un_c Un_d Vn_c Vn_d (exit planes a, b; entry planes c, d).  An ellipsoid slot holds the record's
 // words 40..53 in words 0..15.
-__device__ __forceinline__ uint32_t prep_prism(float4* __restrict__ slot, const float4* __restrict__ rec, int wx0, int wy0)
+__device__ __forceinline__ uint32_t prep_prism(float4* __restrict__ slot, const float4* __restrict__ rec, const float4* __restrict__ pairs,
+                                               int wx0, int wy0)
 {
     float* sw = reinterpret_cast<float*>(slot);
     const float4 h2 = __ldg(rec + 2);                                  // flags, dn, cz, index
     const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));     // jc, ic, zmax, chord scale
-    const double2* c = reinterpret_cast<const double2*>(rec + 4);
-    const float tsc = __int_as_float(h3.w);
-    sw[25] = h2.y / tsc;                                               // dn / s (s is a power of two: exact)
-    const double sc = (double)tsc;
-    const double oj = (double)(wx0 - h3.x), oi = (double)(wy0 - h3.y);
+    sw[25] = h2.y * __int_as_float(0x7f000000 - h3.w);                 // dn / s: s is a power of two, so 1 / s is an exponent flip (exact)
+    const float oj = (float)(wx0 - h3.x), oi = (float)(wy0 - h3.y);    // exact small integers
     const int ns = (int)((__float_as_uint(h2.x) >> 8) & 7u);
     float emin[6], nmax[6];
     float xlow = __int_as_float(0x7f800000), nhigh = __int_as_float(0xff800000);   // min_q emax_q, max_q nmin_q
 #pragma unroll
     for (int q = 0; q < 6; ++q) {
-        const double2 uv = __ldg(c + 2 * q), xn = __ldg(c + 2 * q + 1);    // U, V | Cx, Cn
-        const double m = fma(uv.x, oj, uv.y * oi);
-        const double ex = (xn.x - m) * sc, en = (xn.y - m) * sc, u = uv.x * sc, v = uv.y * sc;
-        float exf, enf, uf, vf;
-        if (q < 2 && q < ns) {                                         // steep slab: exact-grid (hi, lo) pairs
-            const double mb = fmax(fabs(ex), fabs(en)) + 15.0 * fabs(u) + 7.0 * fabs(v);
-            const int e = ((__double2hiint(mb) >> 20) & 0x7ff) - 1021; // mb < 2^e (one spare bit)
-            const double cq = __hiloint2double((e - 23 + 52 + 1023) << 20 | 0x80000, 0);   // 1.5 * 2^52 * q, q = 2^(e - 23)
-            const double exh = (ex + cq) - cq, enh = (en + cq) - cq, uh = (u + cq) - cq, vh = (v + cq) - cq;
-            exf = (float)exh; enf = (float)enh; uf = (float)uh; vf = (float)vh;
-            slot[7 + q] = make_float4((float)(ex - exh), (float)(en - enh), (float)(u - uh), (float)(v - vh));
-        } else {
-            exf = (float)ex; enf = (float)en; uf = (float)u; vf = (float)v;
+        const float4 h = __ldg(pairs + 2 * q), l = __ldg(pairs + 2 * q + 1);       // U, V, Cx, Cn: hi parts | lo parts
+        const float mh = fmaf(h.x, oj, h.y * oi);                      // exact (grid multiples below 2^24 q)
+        const float ml = fmaf(l.x, oj, l.y * oi);
+        const float xh = h.z - mh, nh = h.w - mh;                      // exact
+        const float xl = l.z - ml, nl = l.w - ml;
+        float exf = xh + xl, enf = nh + nl, uf = h.x + l.x, vf = h.y + l.y;   // one rounding each: the fp64 value in fp32
+        if (q < 2 && q < ns) {                                         // steep slab: (hi, lo) once more, on the sub-tile's grid
+            const float mb = fmaxf(fabsf(exf), fabsf(enf)) + 15.0f * fabsf(uf) + 7.0f * fabsf(vf);
+            const int e = (int)(__float_as_uint(mb) >> 23) - 126;      // mb < 2^e
+            const float cq = __int_as_float(((e + 129) << 23) | 0x400000);   // 1.5 * 2^23 * q, q = 2^(e - 21)
+            const float exh = (exf + cq) - cq, enh = (enf + cq) - cq, uh = (uf + cq) - cq, vh = (vf + cq) - cq;
+            slot[7 + q] = make_float4((xh - exh) + xl, (nh - enh) + nl, (h.x - uh) + l.x, (h.y - vh) + l.y);
+            exf = exh; enf = enh; uf = uh; vf = vh;
         }
         sw[q] = exf; sw[6 + q] = enf; sw[12 + q] = uf; sw[18 + q] = vf;
         // value range of  C - U lx - V ly  over lx in [0, 15], ly in [0, 7], padded for the fp32 roundings
         const float au = 15.0f * uf, av = 7.0f * vf;
-        const float hi = -(fminf(au, 0.0f) + fminf(av, 0.0f)), lo = -(fmaxf(au, 0.0f) + fmaxf(av, 0.0f));
         const float pad = 4.8e-7f * (fmaxf(fabsf(exf), fabsf(enf)) + fabsf(au) + fabsf(av));
-        emin[q] = exf + lo - pad;
-        nmax[q] = enf + hi + pad;
-        xlow = fminf(xlow, exf + hi + pad);
-        nhigh = fmaxf(nhigh, enf + lo - pad);
+        const float hi = pad - (fminf(au, 0.0f) + fminf(av, 0.0f)), lo = -pad - (fmaxf(au, 0.0f) + fmaxf(av, 0.0f));
+        emin[q] = exf + lo;
+        nmax[q] = enf + hi;
+        xlow = fminf(xlow, exf + hi);
+        nhigh = fmaxf(nhigh, enf + lo);
     }
     if (!(xlow > nhigh)) return kClsNone;                              // empty chord everywhere in the sub-tile
     uint32_t mx = 0u, mn = 0u;                                         // planes that can be active somewhere
@@ -583,7 +583,9 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
         }
         const bool keep = ((meta >> wid) & 1u) != 0u;
         const unsigned mk = __ballot_sync(0xffffffffu, keep);
-        if (keep) my_queue[nq + __popc(mk & lt)] = (pid & 0x1fffffffu) | ((meta >> 8) << 29);
+        if (keep) {
+            my_queue[nq + __popc(mk & lt)] = (pid & 0x1fffffffu) | ((meta >> 8) << 29);
+        }
         nq += __popc(mk);
         __syncwarp();
         // ---- 32 survivors queued (or the list has ended): one lane prepares one survivor, then all lanes evaluate them ------------
@@ -604,7 +606,7 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
                     sl[0] = c0; sl[1] = c1; sl[2] = c2; sl[3] = c3;
                     reinterpret_cast<float*>(sl)[25] = K;
                 } else if (cls != kClsF64) {
-                    cls = prep_prism(sl, rec, wx0, wy0);
+                    cls = prep_prism(sl, rec, reinterpret_cast<const float4*>(a.rec2 + (size_t)spid * kPairWords), wx0, wy0);
                 }
             }
             const unsigned mp = __ballot_sync(0xffffffffu, cls == kClsPair);
@@ -697,7 +699,7 @@ static cudaError_t launch_variant(const ComposeArgs& a, unsigned grid, cudaStrea
 cudaError_t launch_compose(osog_ctx* c, int B, bool has_ramp, float* d_opd, float2* d_field, bool sort_first)
 {
     ComposeArgs a;
-    a.rec = c->rec; a.offset = c->offset; a.list = c->list; a.meta = c->meta;
+    a.rec = c->rec; a.rec2 = c->rec2; a.offset = c->offset; a.list = c->list; a.meta = c->meta;
     a.optics = c->optics;
     a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.status = c->status + c->status_idx;
     a.opd = d_opd; a.field = d_field;

@@ -183,7 +183,7 @@ int osog_destroy(osog_ctx* c)
     DeviceGuard g(c->device);
     if (c->has_plan_one) cufftDestroy(c->plan_one);
     if (c->has_plan_batch) cufftDestroy(c->plan_batch);
-    cudaFree(c->rec); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
+    cudaFree(c->rec); cudaFree(c->rec2); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
     cudaFree(c->list); cudaFree(c->meta); cudaFree(c->slices); cudaFree(c->offset); cudaFree(c->done); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
     cudaFree(c->status); cudaFree(c->field); cudaFree(c->work); cudaFree(c->otf);
     delete c->otf_key;
@@ -234,6 +234,7 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     cudaError_t e = cudaSuccess;
     auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
     A(dalloc(&c->rec, np * kRecWords));
+    A(dalloc(&c->rec2, np * kPairWords));
     A(dalloc(&c->tbox, np));
     A(dalloc(&c->pframe, np));
     A(dalloc(&c->count, 2 * (size_t)c->count_stride));

@@ -13,6 +13,7 @@ namespace osog {
 constexpr int kTile = 32;              // binning tile edge T (pixels); one CTA composes one tile
 constexpr int kComposeThreads = 256;   // 8 warps; each warp owns a 16 x 8 pixel sub-tile, each lane 4 x 1 pixels
 constexpr int kRecWords = 64;          // 256-byte record per particle: 16 header words + up to 24 doubles
+constexpr int kPairWords = 48;         // prisms: 6 slabs x (U, V, Cx, Cn) as (hi, lo) float pairs for the composition kernel
 constexpr double kBBoxPadPx = 1.0 / 1024.0;   // delta of DESIGN.md B2
 constexpr float kSteepSlope = 16.0f;   // slabs steeper than this (|n_xy| / |n_z|) are refined in fp64 where active
 constexpr double kAllF64Slope = 1.0e4; // a slab steeper than this (or vertical) sends the whole particle to fp64
@@ -66,6 +67,7 @@ struct osog_ctx {
     const int32_t* last_frame_start; // device pointer of the last call's frame_start (nullptr: one frame)
     // scratch (device)
     float* rec;                     // [max_particles][kRecWords]
+    float* rec2;                    // [max_particles][kPairWords] prism slab coefficients as exact-grid (hi, lo) float pairs
     int4* tbox;                     // [max_particles] tile range tx0, tx1, ty0, ty1 (tx0 > tx1: not listed)
     int* pframe;                    // [max_particles] frame of the particle
     uint32_t* count;                // [2][count_stride] per-tile list length; slot status_idx belongs to the current call, the
