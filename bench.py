@@ -3,7 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
 
-One "step" = one pass of the whole hot path (H1-H7: prepare, bounding box + list append, per-tile sort + cull, ordered tile
+One "step" = one pass of the whole hot path (H1-H7: prepare, bounding box + count, scan, CSR fill + per-tile cull, ordered tile
 composition with the fused field write-out) over one seeded synthetic batch = one osog_render_field call.
 Default workload: BASELINE.json configs[3] (the paper-scale headline: 40,000 mixed particles, 2048 x 2048,
 NA 0.65, 10 degree oblique ramp).  Prints ONE JSON line (see DESIGN.md section 10 for every key).
@@ -27,6 +27,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "particles/s (hot path osog_render_field, 40k particles on 2048^2)"
+# identical in both arms' `config` (the driver compares them): how cache state is handled between timed steps
+TIMING_NOTE = "GPU arm: L2 flushed between timed steps (256 MB memset); CPU arm: every step recomputes its whole sample"
 UNIT = "particles/s"
 
 
@@ -43,7 +45,18 @@ def _peaks():
 ALU_INSTR_PER_ELLIPSOID_PAIR = 13      # ~12 fp32 instructions + 1 MUFU per true covered pair
 ALU_INSTR_PER_PRISM_PAIR = 40          # 12 plane values + min / max + accumulate per true covered pair
 ALU_INSTR_PER_PIXEL = 30               # sincospi + complex multiply + store per output pixel
-N_SM, SMSP_PER_SM, LANES = 148, 4, 32  # B200: one warp instruction per clock and SM sub-partition
+N_SM, SMSP_PER_SM, LANES = 148, 4, 32  # B200: one warp instruction per clock and SM sub-partition (nominal issue rate)
+
+
+def _roofline_inputs():
+    """Tracked measurement inputs of the roofline (profiles/r2_roofline_inputs.json): the FFMA issue rate measured by
+    paper_2606_21381_b200/issue_rates on this pool's B200 (profiles/r2_issue_rates.md) and the DRAM traffic of the
+    dominant kernel from its last ncu --set full capture (profiles/r2_compose_ncu.md), each with command, date and commit."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_roofline_inputs.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
 
 
 def _sm_clock_ghz():
@@ -163,7 +176,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": n0 / v * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": CONFIG_NAMES[args.config], "N": scene.N, "H": scene.H, "W": scene.W, "B": scene.B},
+            "config": {"workload": CONFIG_NAMES[args.config], "N": scene.N, "H": scene.H, "W": scene.W, "B": scene.B,
+                       "l2": TIMING_NOTE},
             "cpu_baseline": dict(last, value=v),
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -393,16 +407,22 @@ def run_ours(args):
     step_gbs = alg_bytes / (ms_step * 1e-3) / 1e9
     k_bytes = 4 * pairs + 8 * B * H * W                 # k_compose_tile alone: list read + complex64 write
     achieved = k_bytes / (ms_compose * 1e-3) / 1e9
+    rin = _roofline_inputs()
+    cap = rin.get("k_compose_tile_dram", {})
+    traffic = cap.get("bytes") if cap.get("workload") == CONFIG_NAMES[args.config] else None
     hbm = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-           "traffic": 10553088, "traffic_note": "dram read+write of one k_compose_tile launch, ncu --set full "
-           "(profiles/r1_final4_compose_ncu.md); the 33.5 MB field it writes stays in the 126 MB L2",
+           "traffic": traffic, "traffic_note": ("dram read+write of one k_compose_tile launch, ncu --set full, captured "
+           f"{cap.get('captured')} at commit {cap.get('commit')} ({cap.get('source')}); the field it writes mostly stays in "
+           "the 126 MB L2 during the launch") if traffic is not None else "no tracked ncu capture for this workload",
            "peak_source": peak_src, "algorithmic_bytes": int(k_bytes), "kernel": "k_compose_tile",
            "kernel_ms": ms_compose, "frac_of_nominal_8TBs": achieved / 8000.0,
            "note": "BASELINE.json's '% of B200 HBM roofline'; the kernel is bound by instruction issue, see roofline"}
     cp = _covered_pairs(CONFIG_NAMES[args.config])
     if cp is not None:
         ghz, ghz_src = _sm_clock_ghz()
-        alu_peak = N_SM * SMSP_PER_SM * LANES * ghz * 1e-3                      # T lane-instructions / s
+        ffma = rin.get("ffma_lanes_per_clk_per_sm", {})
+        lanes_per_clk = float(ffma.get("value", SMSP_PER_SM * LANES))           # measured FFMA issue rate, else the nominal 128
+        alu_peak = N_SM * lanes_per_clk * ghz * 1e-3                            # T lane-instructions / s
         alg_instr = (ALU_INSTR_PER_ELLIPSOID_PAIR * cp[0] + ALU_INSTR_PER_PRISM_PAIR * cp[1]
                      + ALU_INSTR_PER_PIXEL * B * H * W)
         alu_ach = alg_instr / (ms_compose * 1e-3) / 1e12
@@ -413,16 +433,20 @@ def run_ours(args):
                           "instr_per_unit": [ALU_INSTR_PER_ELLIPSOID_PAIR, ALU_INSTR_PER_PRISM_PAIR,
                                              ALU_INSTR_PER_PIXEL],
                           "source": "tests/golden/covered_pairs.txt (oracle count of pairs with positive thickness)"},
-                "peak_source": f"{N_SM} SMs x {SMSP_PER_SM} sub-partitions x {LANES} lanes x {ghz:.3f} GHz "
-                               f"({ghz_src}): one warp instruction per clock and sub-partition (DESIGN.md section 7)"}
+                "peak_source": (f"{N_SM} SMs x {lanes_per_clk:.1f} lane-instructions/clk/SM x {ghz:.3f} GHz ({ghz_src}); "
+                                + (f"the rate is the MEASURED FFMA issue rate ({ffma.get('source')}, {ffma.get('captured')}), "
+                                   f"{lanes_per_clk / (SMSP_PER_SM * LANES):.3f} of the nominal 128 = 4 sub-partitions x 32 lanes"
+                                   if ffma else "NOMINAL 4 sub-partitions x 32 lanes (no tracked measurement found)")
+                                + "; one warp instruction per clock and sub-partition is the ceiling of every pipe mix "
+                                  "(DESIGN.md section 7)")}
     else:
         roof = hbm
     line = {
         "metric": METRIC, "value": whole_job_value(N, args.steps, world, t_steps), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32+f64", "data": "synthetic",
-        "config": {"workload": CONFIG_NAMES[args.config], "N": N, "H": H, "W": W, "B": B, "tile": og.osog_tile_size(),
-                   "pairs": int(pairs), "l2": "flushed between timed steps (256 MB memset)", "parallelism": "replicas only"},
+        "config": {"workload": CONFIG_NAMES[args.config], "N": N, "H": H, "W": W, "B": B, "l2": TIMING_NOTE},
+        "extra": {"tile": og.osog_tile_size(), "pairs": int(pairs), "parallelism": "replicas only"},
         "frames_per_s": world * B * args.steps / t_steps,
         "ms_per_step_median": float(np.median(ms)), "ms_per_step_std": float(ms.std()),
         "e2e": {"value": world * N * args.steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d),

@@ -11,7 +11,7 @@
  *                  half-space intersection {x | A x <= b} of Eq. 1 for the capped tetragonal prism.
  *     U[b,i,j]   = exp(i 2 pi (OPD / lambda_b + fx0 x + fy0 y)),  fx0 = sin(tilt_x) / lambda_b   (Eq. 2 with A == 1,
  *                  oblique illumination as a phase ramp)
- *     I[b]       = | IFFT2( FFT2(U[b]) * P_b ) |^2  (+ sigma * z[b,i,j]),
+ *     I[b]       = | IFFT2( FFT2(U[b]) * P_b ) |^2  (-> Poisson(S I) / S)  (+ sigma * z[b,i,j]),
  *                  P_b = circ(|k| / (NA_b / lambda_b)) * exp(i dz sqrt(k0^2 - kx^2 - ky^2)),  k0 = 2 pi n_medium / lambda_b
  *                  (Eq. 3, readings A9, A10, A20; I_BF; Gaussian read noise)
  *     I_DIC[b]   = | U(r + ds) e^{i theta} - U(r - ds) e^{-i theta} |^2  (*)  | IFFT2(P_b) |^2   (+ sigma * z)
@@ -43,8 +43,9 @@
 extern "C" {
 #endif
 
-#define OSOG_API_VERSION 3   /* 2: osog_optics.defocus_um, osog_dic, osog_render_dic, osog_field_to_dic
-                                3: max_pairs is a TOTAL capacity (device scan + CSR lists), osog_status reports the exact need */
+#define OSOG_API_VERSION 4   /* 2: osog_optics.defocus_um, osog_dic, osog_render_dic, osog_field_to_dic
+                                3: max_pairs is a TOTAL capacity (device scan + CSR lists), osog_status reports the exact need
+                                4: osog_optics.shot_noise_photons (Poisson shot noise), osog_debug_poisson, osog_debug_check_guards */
 
 enum {
     OSOG_OK = 0,
@@ -99,6 +100,10 @@ typedef struct {
     double   defocus_um;              /* delta z of Eq. 3 (intensity / DIC only): the pupil is multiplied by
                                          exp(i 2 pi dz sqrt((n_medium/lambda)^2 - fx^2 - fy^2)); evanescent bins are
                                          zeroed when dz != 0; 0 = in focus (exactly the circ-only pupil)            */
+    double   shot_noise_photons;      /* intensity / DIC only: expected photon count S at unit intensity; the image becomes
+                                         Poisson(S max(I, 0)) / S (before the read noise), one draw per (seed, frame, pixel)
+                                         from the Philox stream with counter (pixel, frame, 1, block): inversion below
+                                         lambda = 10, transformed rejection (PTRS) above (reading A26); 0 = no shot noise  */
 } osog_optics;
 
 /* Differential interference contrast, Eq. 5.  struct_size = sizeof(osog_dic). */
@@ -223,6 +228,17 @@ int osog_debug_bins(osog_ctx* ctx, uint32_t* h_offset, uint32_t* h_list, int64_t
  * kernel alone with CUDA events.  OSOG_EINVAL unless the last call on this context was one of osog_render_opd / _field /
  * _intensity / _dic / _height or osog_backward_intensity (the calls that leave sorted lists and a composition behind). */
 int osog_debug_recompose_field(osog_ctx* ctx, float* d_field);
+
+/* Test hook of the shot noise (reading A26): d_counts[k] = the Poisson((double)d_lambda[k]) draw of
+ * pixel k of frame `frame` under `seed` (DEVICE float [n] in, DEVICE int32 [n] out), exactly the draw the sensor stage
+ * takes; lets the tests compare the integer draw with the oracle's bit for bit on given rates. */
+int osog_debug_poisson(osog_ctx* ctx, const float* d_lambda, int64_t n, uint64_t seed, uint32_t frame, int32_t* d_counts);
+
+/* Test / diagnostics: every scratch array of the context (records, tile ranges, counters, offsets, staging slices, CSR
+ * list, meta words, ramp tables, optics, status, complex frames) is followed by a 256-byte guard band written once in
+ * osog_create.  Synchronises and returns the number of guard bands that no longer hold their pattern (0 = no kernel wrote
+ * past the end of its scratch), or a negative error code.  (compute-sanitizer is not available on every pool.) */
+int osog_debug_check_guards(osog_ctx* ctx);
 
 /* Tile edge T in pixels (build-time constant of the binning, B3). */
 int osog_tile_size(void);

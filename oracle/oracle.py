@@ -419,6 +419,98 @@ def read_noise(seed, frame, H, W) -> np.ndarray:
 
 
 # --------------------------------------------------------------------------------------------
+# Poisson shot noise ("P(lambda) + G(0, sigma^2)"; reading A26)
+# --------------------------------------------------------------------------------------------
+POISSON_SMALL = 10.0       # below: inversion by sequential search; from here on: transformed rejection (PTRS)
+
+
+def shot_uniforms(seed, frame, pixels, block) -> np.ndarray:
+    """Two uniforms in [0, 1) with 53 random bits each for every pixel, from Philox block `block` of the shot-noise
+    stream: key = (seed low 32, seed high 32), counter = (pixel, frame, 1, block) (the read noise uses (pixel, frame, 0, 0));
+    u_a = ((r0 >> 5) 2^26 + (r1 >> 6)) 2^-53, u_b likewise from (r2, r3).  Returns float64 [n, 2]."""
+    pixels = np.asarray(pixels, dtype=np.uint64)
+    ctr = np.zeros((pixels.size, 4), dtype=np.uint64)
+    ctr[:, 0] = pixels
+    ctr[:, 1] = np.uint64(frame)
+    ctr[:, 2] = np.uint64(1)
+    ctr[:, 3] = np.uint64(block)
+    r = philox4x32_10(ctr, (seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF)).astype(np.uint64)
+    ua = ((r[:, 0] >> np.uint64(5)) * np.uint64(1 << 26) + (r[:, 1] >> np.uint64(6))).astype(np.float64) * 2.0 ** -53
+    ub = ((r[:, 2] >> np.uint64(5)) * np.uint64(1 << 26) + (r[:, 3] >> np.uint64(6))).astype(np.float64) * 2.0 ** -53
+    return np.stack([ua, ub], axis=1)
+
+
+def poisson_counts(lam, seed, frame, pixels=None) -> np.ndarray:
+    """One Poisson(lam[k]) draw per pixel (int64), a pure function of (seed, frame, pixel, lam) (reading A26).
+    lam < 10: inversion by sequential search with the first uniform of block 0: the smallest k with
+    sum_{j <= k} e^-lam lam^j / j! >= u (terms by the recurrence p_j = p_{j-1} lam / j, float64).
+    lam >= 10: Hoermann's transformed rejection with squeeze (PTRS, 1993), round j using the two uniforms of block j:
+    U = u_a - 1/2, V = u_b, us = 1/2 - |U|, k = floor((2 a / us + b) U + lam + 0.43); accept if us >= 0.07 and V <= v_r;
+    reject if k < 0 or (us < 0.013 and V > us); else accept iff
+    ln V + ln(1/alpha) - ln(a / us^2 + b) <= -lam + k ln lam - ln k!,
+    with b = 0.931 + 2.53 sqrt(lam), a = -0.059 + 0.02483 b, 1/alpha = 1.1239 + 1.1328 / (b - 3.4),
+    v_r = 0.9277 - 3.6224 / (b - 2)."""
+    from scipy.special import gammaln
+    lam = np.asarray(lam, dtype=np.float64).ravel()
+    n = lam.size
+    pixels = np.arange(n, dtype=np.uint64) if pixels is None else np.asarray(pixels, dtype=np.uint64).ravel()
+    out = np.zeros(n, dtype=np.int64)
+    small = (lam > 0.0) & (lam < POISSON_SMALL)
+    if small.any():
+        idx = np.flatnonzero(small)
+        l = lam[idx]
+        u = shot_uniforms(seed, frame, pixels[idx], 0)[:, 0]
+        p = np.exp(-l)
+        F = p.copy()
+        k = np.zeros(idx.size, dtype=np.int64)
+        for _ in range(200):                       # P(k > 200 | lam < 10) is far below 2^-53
+            more = u > F
+            if not more.any():
+                break
+            k = np.where(more, k + 1, k)
+            p = np.where(more, p * l / np.maximum(k, 1), p)
+            F = np.where(more, F + p, F)
+        out[idx] = k
+    large = lam >= POISSON_SMALL
+    todo = np.flatnonzero(large)
+    block = 0
+    while todo.size:
+        l = lam[todo]
+        uv = shot_uniforms(seed, frame, pixels[todo], block)
+        slam = np.sqrt(l)
+        b = 0.931 + 2.53 * slam
+        a = -0.059 + 0.02483 * b
+        inv_alpha = 1.1239 + 1.1328 / (b - 3.4)
+        vr = 0.9277 - 3.6224 / (b - 2.0)
+        U = uv[:, 0] - 0.5
+        V = uv[:, 1]
+        us = 0.5 - np.abs(U)
+        k = np.floor((2.0 * a / us + b) * U + l + 0.43)
+        fast = (us >= 0.07) & (V <= vr)
+        rej = (k < 0.0) | ((us < 0.013) & (V > us))
+        with np.errstate(divide="ignore", invalid="ignore"):
+            lhs = np.log(V) + np.log(inv_alpha) - np.log(a / (us * us) + b)
+            rhs = -l + k * np.log(l) - gammaln(k + 1.0)
+        acc = fast | (~rej & (lhs <= rhs))
+        out[todo[acc]] = k[acc].astype(np.int64)
+        todo = todo[~acc]
+        block += 1
+        if block > 1000:
+            raise RuntimeError("PTRS did not terminate")
+    return out
+
+
+def shot_noise(I, photons, seed, frame) -> np.ndarray:
+    """Photon-counted intensity of one frame: Poisson(photons * max(I, 0)) / photons (same units as I); photons = expected
+    photon count at I = 1; photons = 0 leaves I unchanged (reading A26)."""
+    if photons == 0.0:
+        return np.asarray(I, dtype=np.float64)
+    I = np.asarray(I, dtype=np.float64)
+    lam = photons * np.maximum(I.ravel(), 0.0)
+    return (poisson_counts(lam, seed, frame).astype(np.float64) / photons).reshape(I.shape)
+
+
+# --------------------------------------------------------------------------------------------
 # whole path for a Scene
 # --------------------------------------------------------------------------------------------
 def render_field(scene, opd=None, mode="bcircle") -> np.ndarray:
@@ -443,6 +535,7 @@ def render_intensity(scene, U=None, pupil_enabled=True, mode="bcircle") -> np.nd
             mask = pupil_mask(scene.H, scene.W, float(scene.NA[b]), scene.pitch_um, float(scene.lambda_um[b])) \
                 if pupil_enabled else None
         I = intensity(U[b], mask)
+        I = shot_noise(I, float(getattr(scene, "shot_noise_photons", 0.0)), scene.seed, b)
         if scene.read_noise_sigma != 0.0:
             I = I + scene.read_noise_sigma * read_noise(scene.seed, b, scene.H, scene.W)
         out.append(I)
@@ -459,6 +552,7 @@ def render_dic(scene, shear_px, theta, U=None, pupil_enabled=True, mode="bcircle
         P = pupil_function(scene.H, scene.W, float(scene.NA[b]), scene.pitch_um, float(scene.lambda_um[b]),
                            scene.n_medium, dz, pupil_enabled)
         I = dic_image(U[b], P, shear_px, theta)
+        I = shot_noise(I, float(getattr(scene, "shot_noise_photons", 0.0)), scene.seed, b)
         if scene.read_noise_sigma != 0.0:
             I = I + scene.read_noise_sigma * read_noise(scene.seed, b, scene.H, scene.W)
         out.append(I)

@@ -34,7 +34,8 @@ class osog_optics(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("B", C.c_int32), ("pitch_um", C.c_double), ("n_medium", C.c_double),
                 ("lambda_um", C.POINTER(C.c_double)), ("NA", C.POINTER(C.c_double)),
                 ("tilt_x_rad", C.c_double), ("tilt_y_rad", C.c_double), ("read_noise_sigma", C.c_double),
-                ("seed", C.c_uint64), ("pupil_enabled", C.c_int32), ("defocus_um", C.c_double)]
+                ("seed", C.c_uint64), ("pupil_enabled", C.c_int32), ("defocus_um", C.c_double),
+                ("shot_noise_photons", C.c_double)]
 
 
 class osog_dic(C.Structure):
@@ -82,6 +83,8 @@ def lib():
     L.osog_render_height.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p,
                                      C.c_void_p]
     L.osog_debug_recompose_field.argtypes = [ctx, C.c_void_p]
+    L.osog_debug_check_guards.argtypes = [ctx]
+    L.osog_debug_poisson.argtypes = [ctx, C.c_void_p, C.c_int64, C.c_uint64, C.c_uint32, C.c_void_p]
     L.osog_destroy.argtypes = [ctx]
     L.osog_status.argtypes = [ctx, C.POINTER(C.c_uint32), C.POINTER(C.c_int64)]
     L.osog_debug_bins.argtypes = [ctx, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
@@ -97,7 +100,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_intensity", "osog_debug_recompose_field", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_intensity", "osog_debug_recompose_field", "osog_debug_check_guards", "osog_debug_poisson", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -139,7 +142,7 @@ class Particles:
 
 
 def make_optics(B, pitch_um, n_medium, lambda_um, NA=None, tilt_x_rad=0.0, tilt_y_rad=0.0,
-                read_noise_sigma=0.0, seed=0, pupil_enabled=True, defocus_um=0.0):
+                read_noise_sigma=0.0, seed=0, pupil_enabled=True, defocus_um=0.0, shot_noise_photons=0.0):
     """osog_optics plus the host arrays it points to (kept alive as attributes)."""
     o = osog_optics()
     o.struct_size = C.sizeof(osog_optics)
@@ -159,6 +162,7 @@ def make_optics(B, pitch_um, n_medium, lambda_um, NA=None, tilt_x_rad=0.0, tilt_
     o.seed = int(seed) & 0xFFFFFFFFFFFFFFFF
     o.pupil_enabled = 1 if pupil_enabled else 0
     o.defocus_um = float(defocus_um)
+    o.shot_noise_photons = float(shot_noise_photons)
     return o
 
 
@@ -172,7 +176,7 @@ def make_dic(shear_x_px, shear_y_px, bias_rad):
 def optics_from_scene(scene, pupil_enabled=True):
     return make_optics(scene.B, scene.pitch_um, scene.n_medium, scene.lambda_um, scene.NA, scene.tilt_x_rad,
                        scene.tilt_y_rad, scene.read_noise_sigma, scene.seed, pupil_enabled,
-                       getattr(scene, "defocus_um", 0.0))
+                       getattr(scene, "defocus_um", 0.0), getattr(scene, "shot_noise_photons", 0.0))
 
 
 class Context:
@@ -340,6 +344,22 @@ class Context:
         if r != OSOG_OK:
             raise OsogError(r, "osog_debug_recompose_field")
         return out
+
+    def poisson(self, lam, seed, frame):
+        """int32 [n] Poisson draws of the sensor's shot-noise stream for the rates `lam` (float32 [n]) (osog_debug_poisson)."""
+        lam = lam.to(device=self.device, dtype=self.torch.float32).contiguous().view(-1)
+        out = self.torch.empty(lam.numel(), dtype=self.torch.int32, device=self.device)
+        r = lib().osog_debug_poisson(self._ctx, lam.data_ptr(), lam.numel(), int(seed) & 0xFFFFFFFFFFFFFFFF, int(frame), out.data_ptr())
+        if r != OSOG_OK:
+            raise OsogError(r, "osog_debug_poisson")
+        return out
+
+    def check_guards(self):
+        """Number of scratch guard bands a kernel has written into (0 = none); synchronises (osog_debug_check_guards)."""
+        r = lib().osog_debug_check_guards(self._ctx)
+        if r < 0:
+            raise OsogError(r, "osog_debug_check_guards")
+        return r
 
     def status(self):
         """(status bits, pairs needed) of the last render call; synchronises the stream."""

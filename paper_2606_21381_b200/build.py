@@ -43,5 +43,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_issue_rates() -> str:
+    """The instruction-rate microbenchmark behind the ALU roofline (csrc/issue_rates.cu), a standalone executable."""
+    out = os.path.join(HERE, "issue_rates")
+    subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-w", "-o", out,
+                    os.path.join(CSRC, "issue_rates.cu")], check=True)
+    return out
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--issue-rates" in sys.argv:
+        print(build_issue_rates())
+    else:
+        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

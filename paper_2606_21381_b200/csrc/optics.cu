@@ -140,10 +140,60 @@ __device__ __forceinline__ float read_noise_z(uint64_t seed, uint32_t frame, uin
     return sqrtf(l) * cospif(2.0f * u2);
 }
 
-// REAL = false: I = |img|^2; REAL = true: I = Re img (the DIC image is a real convolution)
-template <bool REAL>
+// ---- Poisson shot noise ("P(lambda) + G(0, sigma^2)"; reading A26) ---------------------
+// Two uniforms in [0, 1) with 53 random bits each from block `block` of the shot-noise stream of (seed, frame, pixel):
+// Philox4x32-10, key = (seed low, seed high), counter = (pixel, frame, 1, block); u_a = ((r0 >> 5) 2^26 + (r1 >> 6)) 2^-53.
+__device__ __forceinline__ void shot_uniforms(uint64_t seed, uint32_t frame, uint32_t pixel, uint32_t block, double* ua, double* ub)
+{
+    uint32_t c[4] = {pixel, frame, 1u, block};
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        philox_round(c, k0, k1);
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    *ua = ((double)(c[0] >> 5) * 67108864.0 + (double)(c[1] >> 6)) * 1.1102230246251565e-16;
+    *ub = ((double)(c[2] >> 5) * 67108864.0 + (double)(c[3] >> 6)) * 1.1102230246251565e-16;
+}
+
+// One Poisson(lam) draw, a pure function of (seed, frame, pixel, lam), all decisions in fp64.  lam < 10: inversion by
+// sequential search with the first uniform of block 0 (smallest k with CDF(k) >= u, terms by p_j = p_{j-1} lam / j).
+// lam >= 10: Hoermann's transformed rejection with squeeze (PTRS, 1993), round j using the two uniforms of block j.
+__device__ double poisson_draw(double lam, uint64_t seed, uint32_t frame, uint32_t pixel)
+{
+    if (!(lam > 0.0)) return 0.0;
+    double ua, ub;
+    if (lam < 10.0) {
+        shot_uniforms(seed, frame, pixel, 0u, &ua, &ub);
+        double p = exp(-lam), F = p;
+        int k = 0;
+        while (ua > F && k < 200) {
+            ++k;
+            p = p * lam / (double)k;
+            F += p;
+        }
+        return (double)k;
+    }
+    const double slam = sqrt(lam), b = 0.931 + 2.53 * slam, a = -0.059 + 0.02483 * b;
+    const double inv_alpha = 1.1239 + 1.1328 / (b - 3.4), vr = 0.9277 - 3.6224 / (b - 2.0);
+    const double llam = log(lam);
+    for (uint32_t block = 0; block <= 1000u; ++block) {
+        shot_uniforms(seed, frame, pixel, block, &ua, &ub);
+        const double U = ua - 0.5, V = ub, us = 0.5 - fabs(U);
+        const double k = floor((2.0 * a / us + b) * U + lam + 0.43);
+        if (us >= 0.07 && V <= vr) return k;
+        if (k < 0.0 || (us < 0.013 && V > us)) continue;
+        if (log(V) + log(inv_alpha) - log(a / (us * us) + b) <= -lam + k * llam - lgamma(k + 1.0)) return k;
+    }
+    return floor(lam);                                           // (never reached: the acceptance rate is > 0.85)
+}
+
+// REAL = false: I = |img|^2; REAL = true: I = Re img (the DIC image is a real convolution).  Then the
+// sensor: photon counting I <- Poisson(photons max(I, 0)) / photons (photons = 0: off), read noise + sigma z.
+template <bool REAL, bool SHOT>
 __global__ void __launch_bounds__(256) k_sensor(const float2* __restrict__ img, float* __restrict__ out, int H, int W,
-                                                float sigma, uint64_t seed)
+                                                float sigma, double photons, uint64_t seed)
 {
     const size_t npx = (size_t)H * W;
     const size_t pix = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -151,8 +201,24 @@ __global__ void __launch_bounds__(256) k_sensor(const float2* __restrict__ img, 
     if (pix >= npx) return;
     const float2 v = img[(size_t)b * npx + pix];
     float I = REAL ? v.x : v.x * v.x + v.y * v.y;
+    if (SHOT) I = (float)(poisson_draw(photons * fmax((double)I, 0.0), seed, (uint32_t)b, (uint32_t)pix) / photons);
     if (sigma != 0.0f) I = fmaf(sigma, read_noise_z(seed, (uint32_t)b, (uint32_t)pix), I);
     out[(size_t)b * npx + pix] = I;
+}
+
+// test hook: counts[k] = Poisson((double)lam[k]) for pixel k of `frame`
+__global__ void __launch_bounds__(256) k_poisson(const float* __restrict__ lam, size_t n, uint64_t seed, uint32_t frame,
+                                                 int32_t* __restrict__ counts)
+{
+    const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) counts[k] = (int32_t)poisson_draw((double)lam[k], seed, frame, (uint32_t)k);
+}
+
+cudaError_t launch_poisson(osog_ctx* c, const float* d_lam, size_t n, uint64_t seed, uint32_t frame, int32_t* d_counts)
+{
+    if (n == 0) return cudaSuccess;
+    k_poisson<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(d_lam, n, seed, frame, d_counts);
+    return cudaGetLastError();
 }
 
 static cudaError_t pupil_launch(osog_ctx* c, int B, float2* spec, double pitch, bool defocus, bool fill, float scale,
@@ -250,19 +316,21 @@ cudaError_t launch_cmul(osog_ctx* c, int B, float2* a, const float2* b, double s
     return cudaGetLastError();
 }
 
-cudaError_t launch_sensor(osog_ctx* c, int B, const float2* img, float* d_intensity, double sigma, uint64_t seed)
+cudaError_t launch_sensor(osog_ctx* c, int B, const float2* img, float* d_intensity, double sigma, double photons, uint64_t seed)
 {
     const size_t npx = (size_t)c->H * c->W;
     const dim3 grid((unsigned)((npx + 255) / 256), B);
-    k_sensor<false><<<grid, 256, 0, c->stream>>>(img, d_intensity, c->H, c->W, (float)sigma, seed);
+    if (photons != 0.0) k_sensor<false, true><<<grid, 256, 0, c->stream>>>(img, d_intensity, c->H, c->W, (float)sigma, photons, seed);
+    else k_sensor<false, false><<<grid, 256, 0, c->stream>>>(img, d_intensity, c->H, c->W, (float)sigma, photons, seed);
     return cudaGetLastError();
 }
 
-cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_out, double sigma, uint64_t seed)
+cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_out, double sigma, double photons, uint64_t seed)
 {
     const size_t npx = (size_t)c->H * c->W;
     const dim3 grid((unsigned)((npx + 255) / 256), B);
-    k_sensor<true><<<grid, 256, 0, c->stream>>>(img, d_out, c->H, c->W, (float)sigma, seed);
+    if (photons != 0.0) k_sensor<true, true><<<grid, 256, 0, c->stream>>>(img, d_out, c->H, c->W, (float)sigma, photons, seed);
+    else k_sensor<true, false><<<grid, 256, 0, c->stream>>>(img, d_out, c->H, c->W, (float)sigma, photons, seed);
     return cudaGetLastError();
 }
 

@@ -16,11 +16,21 @@ int cuda_fail(osog_ctx* c, cudaError_t e)
     return OSOG_ECUDA;
 }
 
+constexpr size_t kGuardBytes = 256;             // guard band behind every scratch array (osog_debug_check_guards)
+constexpr unsigned char kGuardByte = 0xA5;
+
+// scratch array of n elements followed by a guard band that no kernel may touch
 template <class T>
-cudaError_t dalloc(T** p, size_t n)
+cudaError_t dalloc(T** p, size_t n, osog_ctx* c = nullptr)
 {
     *p = nullptr;
-    return cudaMalloc(reinterpret_cast<void**>(p), sizeof(T) * (n ? n : 1));
+    const size_t bytes = sizeof(T) * (n ? n : 1);
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(p), bytes + kGuardBytes);
+    if (e != cudaSuccess) return e;
+    unsigned char* g = reinterpret_cast<unsigned char*>(*p) + bytes;
+    if ((e = cudaMemset(g, kGuardByte, kGuardBytes)) != cudaSuccess) return e;
+    if (c && c->guards) c->guards->emplace_back(g, kGuardBytes);
+    return cudaSuccess;
 }
 
 int check_call(const osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const void* out)
@@ -51,6 +61,7 @@ int check_intensity(const osog_optics* o)
 {
     if (!(o->read_noise_sigma >= 0.0) || !(o->read_noise_sigma < 1.0e300)) return OSOG_EINVAL;
     if (!(fabs(o->defocus_um) < 1.0e300)) return OSOG_EINVAL;
+    if (!(o->shot_noise_photons >= 0.0) || !(o->shot_noise_photons < 1.0e300)) return OSOG_EINVAL;
     if (o->pupil_enabled) {
         if (!o->NA) return OSOG_EINVAL;
         for (int b = 0; b < o->B; ++b)
@@ -102,7 +113,7 @@ int optics_stage(osog_ctx* c, const osog_optics* o, float2* buf, float* d_intens
     cudaError_t e = launch_pupil(c, B, buf, o->pitch_um, o->defocus_um != 0.0);
     if (e != cudaSuccess) return cuda_fail(c, e);
     if ((r = fft_frames(c, buf, B, CUFFT_INVERSE)) != OSOG_OK) return r;
-    e = launch_sensor(c, B, buf, d_intensity, o->read_noise_sigma, o->seed);
+    e = launch_sensor(c, B, buf, d_intensity, o->read_noise_sigma, o->shot_noise_photons, o->seed);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
 }
@@ -123,7 +134,7 @@ int dic_stage(osog_ctx* c, const osog_optics* o, const osog_dic* d, float* d_dic
     if (!c->work || !c->otf) {                       // first DIC call of this context: two more complex batches
         for (float2** buf : {&c->work, &c->otf}) {
             if (*buf) continue;
-            cudaError_t ea = dalloc(buf, (size_t)c->max_frames * c->H * c->W);
+            cudaError_t ea = dalloc(buf, (size_t)c->max_frames * c->H * c->W, c);
             if (ea != cudaSuccess) { cudaGetLastError(); *buf = nullptr; return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea); }
         }
     }
@@ -153,7 +164,7 @@ int dic_stage(osog_ctx* c, const osog_optics* o, const osog_dic* d, float* d_dic
     // I = F^-1{ F{D} OTF }
     if ((e = launch_cmul(c, B, c->work, c->otf, 1.0 / hw)) != cudaSuccess) return cuda_fail(c, e);
     if ((r = fft_frames(c, c->work, B, CUFFT_INVERSE)) != OSOG_OK) return r;
-    if ((e = launch_sensor_real(c, B, c->work, d_dic, o->read_noise_sigma, o->seed)) != cudaSuccess) return cuda_fail(c, e);
+    if ((e = launch_sensor_real(c, B, c->work, d_dic, o->read_noise_sigma, o->shot_noise_photons, o->seed)) != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
 }
 
@@ -187,6 +198,7 @@ int osog_destroy(osog_ctx* c)
     cudaFree(c->list); cudaFree(c->meta); cudaFree(c->slices); cudaFree(c->offset); cudaFree(c->done); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
     cudaFree(c->status); cudaFree(c->field); cudaFree(c->work); cudaFree(c->otf);
     delete c->otf_key;
+    delete c->guards;
     if (c->h_status) cudaFreeHost(c->h_status);
     delete c;
     return OSOG_OK;
@@ -230,24 +242,25 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
 
     DeviceGuard g(c->device);
     if (!g.ok) { delete c; return OSOG_ECUDA; }
+    c->guards = new (std::nothrow) std::vector<std::pair<unsigned char*, size_t>>();
     const size_t np = (size_t)c->max_particles, npx = (size_t)c->H * c->W;
     cudaError_t e = cudaSuccess;
     auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
-    A(dalloc(&c->rec, np * kRecWords));
-    A(dalloc(&c->rec2, np * kPairWords));
-    A(dalloc(&c->tbox, np));
-    A(dalloc(&c->pframe, np));
-    A(dalloc(&c->count, 2 * (size_t)c->count_stride));
-    A(dalloc(&c->offset, (size_t)c->max_tiles + 4));
-    A(dalloc(&c->done, 1));
-    A(dalloc(&c->slices, (size_t)c->max_tiles * c->slice_cap));
-    A(dalloc(&c->list, (size_t)c->max_pairs));
-    A(dalloc(&c->meta, (size_t)c->max_pairs));
-    A(dalloc(&c->ramp_x, (size_t)c->max_frames * c->W));
-    A(dalloc(&c->ramp_y, (size_t)c->max_frames * c->H));
-    A(dalloc(&c->optics, (size_t)c->max_frames));
-    A(dalloc(&c->status, 2));
-    A(dalloc(&c->field, (size_t)c->max_frames * npx));
+    A(dalloc(&c->rec, np * kRecWords, c));
+    A(dalloc(&c->rec2, np * kPairWords, c));
+    A(dalloc(&c->tbox, np, c));
+    A(dalloc(&c->pframe, np, c));
+    A(dalloc(&c->count, 2 * (size_t)c->count_stride, c));
+    A(dalloc(&c->offset, (size_t)c->max_tiles + 4, c));
+    A(dalloc(&c->done, 1, c));
+    A(dalloc(&c->slices, (size_t)c->max_tiles * c->slice_cap, c));
+    A(dalloc(&c->list, (size_t)c->max_pairs, c));
+    A(dalloc(&c->meta, (size_t)c->max_pairs, c));
+    A(dalloc(&c->ramp_x, (size_t)c->max_frames * c->W, c));
+    A(dalloc(&c->ramp_y, (size_t)c->max_frames * c->H, c));
+    A(dalloc(&c->optics, (size_t)c->max_frames, c));
+    A(dalloc(&c->status, 2, c));
+    A(dalloc(&c->field, (size_t)c->max_frames * npx, c));
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&c->h_status), sizeof(DeviceStatus));
     if (e == cudaSuccess) e = cudaMemset(c->status, 0, 2 * sizeof(DeviceStatus));
     if (e == cudaSuccess) e = cudaMemset(c->count, 0, sizeof(uint32_t) * 2 * (size_t)c->count_stride);
@@ -418,7 +431,7 @@ int osog_backward_intensity(osog_ctx* c, const osog_particles* p, int64_t N, con
     if ((r = render_common(c, p, N, o, nullptr, c->field)) != OSOG_OK) return r;      // U, the exit wave
     DeviceGuard g(c->device);
     if (!c->work) {                                  // first call of this kind: a second complex batch
-        const cudaError_t ea = dalloc(&c->work, (size_t)c->max_frames * c->H * c->W);
+        const cudaError_t ea = dalloc(&c->work, (size_t)c->max_frames * c->H * c->W, c);
         if (ea != cudaSuccess) { cudaGetLastError(); c->work = nullptr; return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea); }
     }
     const int B = o->B;
@@ -500,6 +513,31 @@ int osog_status(osog_ctx* c, uint32_t* status_bits, int64_t* pairs)
     if (status_bits) *status_bits = c->h_status->bits;
     if (pairs) *pairs = (int64_t)c->h_status->pairs;     // total of the device scan: on overflow, the max_pairs that suffices
     return overflow ? OSOG_ECAPACITY : OSOG_OK;
+}
+
+int osog_debug_poisson(osog_ctx* c, const float* d_lambda, int64_t n, uint64_t seed, uint32_t frame, int32_t* d_counts)
+{
+    if (!c || n < 0 || (n > 0 && (!d_lambda || !d_counts))) return OSOG_EINVAL;
+    DeviceGuard g(c->device);
+    const cudaError_t e = launch_poisson(c, d_lambda, (size_t)n, seed, frame, d_counts);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return OSOG_OK;
+}
+
+int osog_debug_check_guards(osog_ctx* c)
+{
+    if (!c || !c->guards) return OSOG_EINVAL;
+    DeviceGuard g(c->device);
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    int bad = 0;
+    std::vector<unsigned char> h(kGuardBytes);
+    for (const auto& gb : *c->guards) {
+        if ((e = cudaMemcpy(h.data(), gb.first, gb.second, cudaMemcpyDeviceToHost)) != cudaSuccess) return cuda_fail(c, e);
+        for (size_t k = 0; k < gb.second; ++k)
+            if (h[k] != kGuardByte) { ++bad; break; }
+    }
+    return bad;
 }
 
 int osog_debug_bins(osog_ctx* c, uint32_t* h_offset, uint32_t* h_list, int64_t cap, int64_t* n_tiles, int64_t* n_pairs)

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <cufft.h>
 #include <stdint.h>
+#include <utility>
 #include <vector>
 #include "../../include/osog.h"
 
@@ -89,6 +90,7 @@ struct osog_ctx {
     float2* otf;                    // [max_frames][H][W] optical transfer function F{|F^-1{P}|^2} of the last DIC call
     std::vector<double>* otf_key;   // optics the cached OTF was built for (B, pitch, n_medium, defocus, pupil, lambda[], NA[])
     osog::DeviceStatus* h_status;   // pinned host mirror
+    std::vector<std::pair<unsigned char*, size_t>>* guards;   // (start of the guard band, bytes) behind every scratch array
     cufftHandle plan_one, plan_batch;
     bool has_plan_one, has_plan_batch;
 };
@@ -138,7 +140,8 @@ cudaError_t launch_dic_shear(osog_ctx* c, int B, const float2* field, float2* ou
 cudaError_t launch_abs2(osog_ctx* c, int B, float2* buf, double scale);
 cudaError_t launch_cmul(osog_ctx* c, int B, float2* a, const float2* b, double scale);
 cudaError_t launch_height_stencil(osog_ctx* c, int B, const float* d_h, double pitch, float* d_grad, float* d_lap);
-cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_out, double sigma, uint64_t seed);
-cudaError_t launch_sensor(osog_ctx* c, int B, const float2* img, float* d_intensity, double sigma, uint64_t seed);
+cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_out, double sigma, double photons, uint64_t seed);
+cudaError_t launch_sensor(osog_ctx* c, int B, const float2* img, float* d_intensity, double sigma, double photons, uint64_t seed);
+cudaError_t launch_poisson(osog_ctx* c, const float* d_lam, size_t n, uint64_t seed, uint32_t frame, int32_t* d_counts);
 
 }  // namespace osog

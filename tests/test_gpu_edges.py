@@ -83,6 +83,7 @@ def test_pair_list_overflow_is_reported_and_frames_zeroed(og):
     ctx = og.Context(sc.H, sc.W, sc.N, max_pairs=pairs - 1, check=False)   # one entry less is not
     ctx.render_opd(P, opt)
     assert ctx.status()[0] == og.OSOG_ECAPACITY
+    assert ctx.check_guards() == 0                           # an overflowing call writes nothing past its (too small) list
     ctx.close()
 
 
@@ -128,7 +129,8 @@ def test_crowded_tiles_in_a_batch_take_the_ordered_rescan(og, o):
                           d1=np.full(per, 0.15), d2=np.full(per, 0.12), n_p=rng.uniform(1.36, 1.5, per)))
     cols = {k: np.concatenate([p[k] for p in parts]) for k in parts[0]}
     sc = make_scene("crowd_batch", H, W, cols, frame_start=np.arange(B + 1) * per, lam=np.full(B, 0.55), NA=np.full(B, 0.5))
-    g = render_all(og, sc, max_pairs=3 * 4500)                # staging slices of 500 entries per tile, the fullest lists are longer
+    g = render_all(og, sc, max_pairs=3 * 4500)
+    assert g["guards"] == 0                # staging slices of 500 entries per tile, the fullest lists are longer
     assert g["status"][0] == 0
     oc, oo, ol = o.binning(sc, og.osog_tile_size())
     cnt, off, lst = g["bins"]
@@ -242,6 +244,7 @@ def test_context_reuse_keeps_scratch_invariants(og, o):
     oc, oo, ol = o.binning(big, og.osog_tile_size())
     assert np.array_equal(off, oo) and np.array_equal(lst, ol)
     assert torch.equal(ctx.render_opd(Ps, os_), ref_small)
+    assert ctx.check_guards() == 0
     ctx.close()
 
 
@@ -260,6 +263,7 @@ def test_context_reuse_with_changing_batch_size(og):
         got = ctx.render_opd(og.Particles.from_scene(sc), og.optics_from_scene(sc))
         assert ctx.status()[0] == 0
         assert torch.equal(got, want), sc.name
+    assert ctx.check_guards() == 0
     ctx.close()
 
 

@@ -35,6 +35,7 @@ def render_all(og, sc, pupil=True, max_pairs=0):
     out["status"] = ctx.status()
     out["field"] = ctx.render_field(P, opt).cpu().numpy().astype(np.complex128)
     out["intensity"] = ctx.render_intensity(P, opt).cpu().numpy().astype(np.float64)
+    out["guards"] = ctx.check_guards()            # scratch guard bands: no kernel wrote past the end of its arrays
     torch.cuda.synchronize()
     ctx.close()
     return out
@@ -42,7 +43,7 @@ def render_all(og, sc, pupil=True, max_pairs=0):
 
 def check_against_oracle(og, o, sc, pupil=True, what=("bins", "opd", "field", "intensity")):
     g = render_all(og, sc, pupil)
-    assert g["status"][0] == 0
+    assert g["status"][0] == 0 and g["guards"] == 0
     ref = o.render_opd(sc)
     if "bins" in what:
         oc, oo, ol = o.binning(sc, og.osog_tile_size())

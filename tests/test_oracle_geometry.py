@@ -272,8 +272,8 @@ def test_count_covered_sphere_is_the_gauss_circle_count_and_golden_file_matches(
     want_p = int(np.count_nonzero((np.abs(X - f(4.83)) < f(1.24) / 2) & (np.abs(Y - f(7.0)) < f(1.24) / 2)))
     for mode in ("full", "bcircle"):
         assert o.count_covered(sc, mode) == (want_e, want_p)
-    # the stored counts are what the oracle gives today for the small workloads (config 1: also = non-zero thickness
-    # pixels summed over single-particle renders)
+    # the stored counts are what the oracle gives today for ALL five workloads (config 4's pair is the numerator of
+    # bench.py's headline ALU roofline fraction; config 1: also = non-zero thickness pixels summed over single-particle renders)
     stored = {}
     with open(os.path.join(os.path.dirname(__file__), "golden", "covered_pairs.txt")) as fh:
         for ln in fh:
@@ -281,7 +281,7 @@ def test_count_covered_sphere_is_the_gauss_circle_count_and_golden_file_matches(
             if len(q) == 3 and not ln.startswith("#"):
                 stored[q[0]] = (int(q[1]), int(q[2]))
     assert set(stored) == set(CONFIG_NAMES.values())
-    for cfg in (1, 2):
+    for cfg in (1, 2, 3, 4, 5):
         assert o.count_covered(make_config(cfg)) == stored[CONFIG_NAMES[cfg]]
     sc1 = make_config(1)
     from workloads import subset

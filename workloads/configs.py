@@ -45,6 +45,7 @@ class Scene:
     tilt_y_rad: float = 0.0
     read_noise_sigma: float = 0.0
     defocus_um: float = 0.0      # delta z of Eq. 3; 0 = in focus
+    shot_noise_photons: float = 0.0   # photons at unit intensity for the Poisson term of PAPER.md:126; 0 = off
     cols: dict = field(default_factory=dict)   # float32 [N] each + kind uint8 [N]
     frame_start: np.ndarray = None             # int32 [B+1]
 
