@@ -114,6 +114,15 @@ typedef struct {
     double   bias_rad;                /* bias phase theta                                                         */
 } osog_dic;
 
+/* Brightfield amplitude, Eq. 4 (reading A27).  struct_size = sizeof(osog_brightfield). */
+typedef struct {
+    uint32_t struct_size;
+    double   n_particle;              /* refractive index of the particle material for the Fresnel term (one value per call;
+                                         the medium side is osog_optics.n_medium)                                          */
+    double   delta_mu_per_um;         /* mu_p - mu_s of the Beer-Lambert term, 1/um                                         */
+    double   caustic_gain_um;         /* C = -caustic_gain * laplacian(h); the paper gives only the proportionality         */
+} osog_brightfield;
+
 /* Create a context: allocates all scratch (records, tile ranges, per-tile counters, scan offsets, staging slices and the
  * CSR pair list, ramp tables, one complex frame batch and the cuFFT plans).  *out is set to NULL on failure. */
 int osog_create(osog_ctx** out, const osog_config* cfg);
@@ -146,6 +155,15 @@ int osog_field_to_intensity(osog_ctx* ctx, const osog_optics* o, const float* d_
  * frame batches (cudaMalloc, synchronous); later calls allocate nothing. */
 int osog_render_dic(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const osog_dic* dic,
                     float* d_dic);
+
+/* Brightfield image with the amplitude of Eq. 4: d_intensity is DEVICE float [B, H, W],
+ * I_BF = |(A U_exit) * h_obj|^2 (+ shot / read noise), A = T_F(theta_i) exp(-h (mu_p - mu_s)) - gain * laplacian(h),
+ * T_F = unpolarised Fresnel transmittance from n_medium into n_particle at cos theta_i = 1 / sqrt(1 + |grad h|^2)
+ * (normal <-h_x, -h_y, 1> of PAPER.md:92, light along +z), h / grad h / laplacian h as osog_render_height gives them.
+ * Runs the hot path twice (height map with unit index contrast, then the exit wave), one element-wise pass that multiplies
+ * A into the wave, and the library stage of osog_render_intensity.  The first call allocates one real frame batch. */
+int osog_render_brightfield(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const osog_brightfield* bf,
+                            float* d_intensity);
 
 /* Library stage of osog_render_dic alone on a caller-supplied field (DEVICE complex64 [B, H, W], left untouched). */
 int osog_field_to_dic(osog_ctx* ctx, const osog_optics* o, const osog_dic* dic, const float* d_field, float* d_dic);

@@ -20,6 +20,8 @@ Pieces, each following the passage it cites (line numbers are /root/reference/PA
   backward_intensity   dL/dOPD from dL/dI: adjoint of field + pupil + |.|^2                :124 (NEXT-3)
   thickness_grad / backward_centre   grad t per pixel; dL/d(cx, cy) = -dn sum_px G grad t  :124 (NEXT-3, second step)
   render_height / height_gradient / height_laplacian   h, grad h, lap h of the G-buffer :76, :92, :96-99, A25
+  fresnel_transmittance / brightfield_amplitude / render_brightfield   Eq. 4       :94-99, A27
+  shot_uniforms / poisson_counts / shot_noise          Poisson shot noise          :126, A26
 
 Every reading of the paper taken here (units, pixel centres, quaternion convention, pupil edge,
 FFT normalisation, noise model ...) is listed in DESIGN.md section 3.  Pins: tests/test_oracle_*.py.
@@ -540,6 +542,53 @@ def render_intensity(scene, U=None, pupil_enabled=True, mode="bcircle") -> np.nd
             I = I + scene.read_noise_sigma * read_noise(scene.seed, b, scene.H, scene.W)
         out.append(I)
     return np.stack(out)
+
+
+# --------------------------------------------------------------------------------------------
+# brightfield amplitude, Eq. 4 (reading A27)
+# --------------------------------------------------------------------------------------------
+def fresnel_transmittance(cos_i, n1, n2) -> np.ndarray:
+    """Unpolarised Fresnel power transmittance T_F = 1 - (R_s + R_p) / 2 of a plane interface from index n1 into n2 at
+    incidence angle theta_i (cos_i = cos theta_i): Snell sin theta_t = (n1 / n2) sin theta_i,
+    R_s = ((n1 cos_i - n2 cos_t) / (n1 cos_i + n2 cos_t))^2, R_p = ((n1 cos_t - n2 cos_i) / (n1 cos_t + n2 cos_i))^2;
+    total internal reflection (sin theta_t > 1) gives 0."""
+    ci = np.clip(np.asarray(cos_i, dtype=np.float64), 0.0, 1.0)
+    if n1 == n2:                                   # no interface
+        return np.ones_like(ci)
+    si2 = 1.0 - ci * ci
+    st2 = (n1 / n2) ** 2 * si2
+    tir = st2 > 1.0
+    ct = np.sqrt(np.where(tir, 0.0, 1.0 - st2))
+    with np.errstate(divide="ignore", invalid="ignore"):
+        rs = ((n1 * ci - n2 * ct) / (n1 * ci + n2 * ct)) ** 2
+        rp = ((n1 * ct - n2 * ci) / (n1 * ct + n2 * ci)) ** 2
+    graze = ci == 0.0                              # theta_i = 90 degrees: everything is reflected
+    rs = np.where(graze, 1.0, rs)
+    rp = np.where(graze, 1.0, rp)
+    return np.where(tir, 0.0, 1.0 - 0.5 * (rs + rp))
+
+
+def brightfield_amplitude(h, pitch, n_medium, n_particle, delta_mu, caustic_gain) -> np.ndarray:
+    """A(x, y) of Eq. 4 for one frame: T_F(theta_i) exp(-h (mu_p - mu_s)) + C, with (reading A27) the normal
+    N = <-dh/dx, -dh/dy, 1> of PAPER.md:92 from the G-buffer's height gradient (A25), illumination along L = +z so that
+    cos theta_i = N.L / |N| = 1 / sqrt(1 + |grad h|^2), T_F the unpolarised Fresnel transmittance from the medium
+    (n_medium) into the particle material (n_particle, one value per call), delta_mu = mu_p - mu_s in 1/um, and the caustic
+    term C = -caustic_gain * laplacian(h) (gain in um, the paper only gives the proportionality)."""
+    h = np.asarray(h, dtype=np.float64)
+    gx, gy = height_gradient(h, pitch)
+    lap = height_laplacian(h, pitch)
+    cos_i = 1.0 / np.sqrt(1.0 + gx ** 2 + gy ** 2)
+    return fresnel_transmittance(cos_i, n_medium, n_particle) * np.exp(-h * delta_mu) - caustic_gain * lap
+
+
+def render_brightfield(scene, n_particle, delta_mu, caustic_gain, pupil_enabled=True, mode="bcircle") -> np.ndarray:
+    """float64 [B, H, W]: I_BF = |(A U_exit) * h_obj|^2 with A of Eq. 4 multiplying the exit wave of Eq. 2
+    (which the hot path renders with A = 1), then the sensor (shot noise, read noise)."""
+    U = render_field(scene, mode=mode)
+    h = render_height(scene, mode)
+    A = np.stack([brightfield_amplitude(h[b], scene.pitch_um, scene.n_medium, n_particle, delta_mu, caustic_gain)
+                  for b in range(scene.B)])
+    return render_intensity(scene, U=A * U, pupil_enabled=pupil_enabled, mode=mode)
 
 
 def render_dic(scene, shear_px, theta, U=None, pupil_enabled=True, mode="bcircle") -> np.ndarray:

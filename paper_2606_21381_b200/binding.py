@@ -43,6 +43,11 @@ class osog_dic(C.Structure):
                 ("bias_rad", C.c_double)]
 
 
+class osog_brightfield(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("n_particle", C.c_double), ("delta_mu_per_um", C.c_double),
+                ("caustic_gain_um", C.c_double)]
+
+
 class OsogError(RuntimeError):
     def __init__(self, code, what, pairs_needed=None):
         self.code = code
@@ -75,6 +80,8 @@ def lib():
     L.osog_field_to_intensity.argtypes = [ctx, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_dic.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics),
                                   C.POINTER(osog_dic), C.c_void_p]
+    L.osog_render_brightfield.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics),
+                                          C.POINTER(osog_brightfield), C.c_void_p]
     L.osog_field_to_dic.argtypes = [ctx, C.POINTER(osog_optics), C.POINTER(osog_dic), C.c_void_p, C.c_void_p]
     L.osog_backward_np.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_backward_intensity.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
@@ -100,7 +107,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_intensity", "osog_debug_recompose_field", "osog_debug_check_guards", "osog_debug_poisson", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_brightfield", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_intensity", "osog_debug_recompose_field", "osog_debug_check_guards", "osog_debug_poisson", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -171,6 +178,13 @@ def make_dic(shear_x_px, shear_y_px, bias_rad):
     d.struct_size = C.sizeof(osog_dic)
     d.shear_x_px, d.shear_y_px, d.bias_rad = int(shear_x_px), int(shear_y_px), float(bias_rad)
     return d
+
+
+def make_brightfield(n_particle, delta_mu_per_um=0.0, caustic_gain_um=0.0):
+    b = osog_brightfield()
+    b.struct_size = C.sizeof(osog_brightfield)
+    b.n_particle, b.delta_mu_per_um, b.caustic_gain_um = float(n_particle), float(delta_mu_per_um), float(caustic_gain_um)
+    return b
 
 
 def optics_from_scene(scene, pupil_enabled=True):
@@ -328,6 +342,13 @@ class Context:
         """float32 [B, H, W] DIC image of Eq. 5 (osog_render_dic); `dic` from make_dic."""
         out = self._out(o.B, out=out)
         self._done(lib().osog_render_dic(self._ctx, C.byref(p.c), p.N, C.byref(o), C.byref(dic), out.data_ptr()), "osog_render_dic")
+        return out
+
+    def render_brightfield(self, p: Particles, o, bf, out=None):
+        """float32 [B, H, W] brightfield image with the amplitude of Eq. 4 (osog_render_brightfield); `bf` from make_brightfield."""
+        out = self._out(o.B, out=out)
+        self._done(lib().osog_render_brightfield(self._ctx, C.byref(p.c), p.N, C.byref(o), C.byref(bf), out.data_ptr()),
+                   "osog_render_brightfield")
         return out
 
     def field_to_dic(self, o, dic, field, out=None):

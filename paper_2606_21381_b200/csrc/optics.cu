@@ -95,6 +95,56 @@ __global__ void __launch_bounds__(256) k_height_stencil(const float* __restrict_
     if (lap != nullptr) lap[idx] = ((xl + xr) + (yu + yd) - 4.0f * c) * (inv_p * inv_p);
 }
 
+cudaError_t launch_brightfield(osog_ctx* c, int B, float2* field, const float* d_h, double pitch, double n1, double n2,
+                               double dmu, double gain);
+// Brightfield amplitude, Eq. 4 (reading A27), multiplied into the exit wave in place:
+// A = T_F(theta_i) exp(-h dmu) + C, cos theta_i = 1 / sqrt(1 + |grad h|^2) (normal <-h_x, -h_y, 1>, light along +z), T_F the
+// unpolarised Fresnel transmittance from index n1 into n2, C = -gain lap h; grad h and lap h are the finite differences of
+// reading A25 (k_height_stencil's formulas), taken here straight from the height map.
+__global__ void __launch_bounds__(256) k_brightfield(float2* __restrict__ field, const float* __restrict__ h, int H, int W,
+                                                     float inv_p, float n1, float n2, float dmu, float gain)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = blockIdx.y, b = blockIdx.z;
+    if (j >= W) return;
+    const float* f = h + (size_t)b * H * W;
+    const int jm = max(j - 1, 0), jp = min(j + 1, W - 1), im = max(i - 1, 0), ip = min(i + 1, H - 1);
+    const float c = f[(size_t)i * W + j];
+    const float xl = f[(size_t)i * W + jm], xr = f[(size_t)i * W + jp];
+    const float yu = f[(size_t)im * W + j], yd = f[(size_t)ip * W + j];
+    const float gx = jp > jm ? (xr - xl) * (inv_p / (float)(jp - jm)) : 0.0f;
+    const float gy = ip > im ? (yd - yu) * (inv_p / (float)(ip - im)) : 0.0f;
+    const float lap = ((xl + xr) + (yu + yd) - 4.0f * c) * (inv_p * inv_p);
+    const float g2 = gx * gx + gy * gy;
+    float T = 1.0f;
+    if (n1 != n2) {
+        const float ci = rsqrtf(1.0f + g2);                      // cos theta_i
+        const float si2 = g2 / (1.0f + g2);                      // sin^2 theta_i (no cancellation near normal incidence)
+        const float r = n1 / n2, st2 = r * r * si2;
+        if (st2 > 1.0f) {
+            T = 0.0f;                                            // total internal reflection
+        } else {
+            const float ct = sqrtf(1.0f - st2);
+            const float as = n1 * ci, bs = n2 * ct, ap = n1 * ct, bp = n2 * ci;
+            const float rs = (as - bs) / (as + bs), rp = (ap - bp) / (ap + bp);
+            T = 1.0f - 0.5f * (rs * rs + rp * rp);
+        }
+    }
+    const float A = T * expf(-c * dmu) - gain * lap;
+    const size_t idx = ((size_t)b * H + i) * W + j;
+    const float2 u = field[idx];
+    field[idx] = make_float2(u.x * A, u.y * A);
+}
+
+cudaError_t launch_brightfield(osog_ctx* c, int B, float2* field, const float* d_h, double pitch, double n1, double n2,
+                               double dmu, double gain)
+{
+    const dim3 grid((c->W + 255) / 256, c->H, B);
+    k_brightfield<<<grid, 256, 0, c->stream>>>(field, d_h, c->H, c->W, (float)(1.0 / pitch), (float)n1, (float)n2, (float)dmu,
+                                              (float)gain);
+    return cudaGetLastError();
+}
+
 // buf = (|buf|^2 * scale, 0)
 __global__ void __launch_bounds__(256) k_abs2(float2* __restrict__ buf, size_t n, float scale)
 {

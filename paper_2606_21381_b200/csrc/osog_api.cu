@@ -196,7 +196,7 @@ int osog_destroy(osog_ctx* c)
     if (c->has_plan_batch) cufftDestroy(c->plan_batch);
     cudaFree(c->rec); cudaFree(c->rec2); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
     cudaFree(c->list); cudaFree(c->meta); cudaFree(c->slices); cudaFree(c->offset); cudaFree(c->done); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
-    cudaFree(c->status); cudaFree(c->field); cudaFree(c->work); cudaFree(c->otf);
+    cudaFree(c->status); cudaFree(c->field); cudaFree(c->work); cudaFree(c->otf); cudaFree(c->bf_h);
     delete c->otf_key;
     delete c->guards;
     if (c->h_status) cudaFreeHost(c->h_status);
@@ -350,6 +350,30 @@ int osog_render_dic(osog_ctx* c, const osog_particles* p, int64_t N, const osog_
     if ((r = render_common(c, p, N, o, nullptr, c->field)) != OSOG_OK) return r;
     DeviceGuard g(c->device);
     return dic_stage(c, o, d, d_dic);
+}
+
+int osog_render_brightfield(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const osog_brightfield* bf,
+                            float* d_intensity)
+{
+    int r = check_call(c, p, N, o, d_intensity);
+    if (r != OSOG_OK) return r;
+    if ((r = check_intensity(o)) != OSOG_OK) return r;
+    if (!bf || bf->struct_size != sizeof(osog_brightfield)) return OSOG_EINVAL;
+    if (!(bf->n_particle > 0.0) || !(bf->n_particle < 1.0e300) || !(o->n_medium > 0.0) || !(fabs(bf->delta_mu_per_um) < 1.0e300) ||
+        !(fabs(bf->caustic_gain_um) < 1.0e300))
+        return OSOG_EINVAL;
+    DeviceGuard g(c->device);
+    if (!c->bf_h) {                                  // first brightfield call of this context: one real frame batch
+        const cudaError_t ea = dalloc(&c->bf_h, (size_t)c->max_frames * c->H * c->W, c);
+        if (ea != cudaSuccess) { cudaGetLastError(); c->bf_h = nullptr; return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea); }
+    }
+    // height map (the hot path with unit index contrast), then the exit wave (the hot path proper); A multiplies U in place
+    if ((r = render_common(c, p, N, o, c->bf_h, nullptr, true)) != OSOG_OK) return r;
+    if ((r = render_common(c, p, N, o, nullptr, c->field)) != OSOG_OK) return r;
+    const cudaError_t e = launch_brightfield(c, o->B, c->field, c->bf_h, o->pitch_um, o->n_medium, bf->n_particle,
+                                             bf->delta_mu_per_um, bf->caustic_gain_um);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return optics_stage(c, o, c->field, d_intensity);
 }
 
 int osog_field_to_dic(osog_ctx* c, const osog_optics* o, const osog_dic* d, const float* d_field, float* d_dic)

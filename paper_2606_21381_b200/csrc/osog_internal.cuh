@@ -87,6 +87,7 @@ struct osog_ctx {
     bool scratch_dirty;             // a call failed midway: count / status must be cleared explicitly
     float2* field;                  // [max_frames][H][W] (intensity path)
     float2* work;                   // [max_frames][H][W] second complex batch (DIC path; allocated by the first DIC call)
+    float* bf_h;                    // [max_frames][H][W] height map of the brightfield path (allocated by its first call)
     float2* otf;                    // [max_frames][H][W] optical transfer function F{|F^-1{P}|^2} of the last DIC call
     std::vector<double>* otf_key;   // optics the cached OTF was built for (B, pitch, n_medium, defocus, pupil, lambda[], NA[])
     osog::DeviceStatus* h_status;   // pinned host mirror
@@ -139,6 +140,8 @@ cudaError_t launch_gopd(osog_ctx* c, int B, const float2* gu, const float2* u, f
 cudaError_t launch_dic_shear(osog_ctx* c, int B, const float2* field, float2* out, int sx, int sy, double theta);
 cudaError_t launch_abs2(osog_ctx* c, int B, float2* buf, double scale);
 cudaError_t launch_cmul(osog_ctx* c, int B, float2* a, const float2* b, double scale);
+cudaError_t launch_brightfield(osog_ctx* c, int B, float2* field, const float* d_h, double pitch, double n1, double n2,
+                               double dmu, double gain);
 cudaError_t launch_height_stencil(osog_ctx* c, int B, const float* d_h, double pitch, float* d_grad, float* d_lap);
 cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_out, double sigma, double photons, uint64_t seed);
 cudaError_t launch_sensor(osog_ctx* c, int B, const float2* img, float* d_intensity, double sigma, double photons, uint64_t seed);
