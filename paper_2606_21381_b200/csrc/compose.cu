@@ -186,14 +186,17 @@ __device__ __forceinline__ uint32_t prep_prism(float4* __restrict__ slot, const 
             exf = exh; enf = enh; uf = uh; vf = vh;
         }
         sw[q] = exf; sw[6 + q] = enf; sw[12 + q] = uf; sw[18 + q] = vf;
-        // value range of  C - U lx - V ly  over lx in [0, 15], ly in [0, 7], padded for the fp32 roundings
-        const float au = 15.0f * uf, av = 7.0f * vf;
-        const float pad = 4.8e-7f * (fmaxf(fabsf(exf), fabsf(enf)) + fabsf(au) + fabsf(av));
-        const float hi = pad - (fminf(au, 0.0f) + fminf(av, 0.0f)), lo = -pad - (fmaxf(au, 0.0f) + fmaxf(av, 0.0f));
-        emin[q] = exf + lo;
-        nmax[q] = enf + hi;
-        xlow = fminf(xlow, exf + hi);
-        nhigh = fmaxf(nhigh, enf + lo);
+        // value range of  C - U lx - V ly  over lx in [0, 15], ly in [0, 7]: centre value -+ half range, padded for the
+        // fp32 roundings of this block and of the evaluation (a few ulp of the largest magnitude involved)
+        const float ec = fmaf(-3.5f, vf, fmaf(-7.5f, uf, exf));
+        const float hr = fmaf(3.5f, fabsf(vf), 7.5f * fabsf(uf));
+        const float d = enf - exf;
+        const float hrp = fmaf(1.0e-6f, (fabsf(exf) + fabsf(enf)) + hr, hr);
+        const float lo_x = ec - hrp, hi_x = ec + hrp;
+        emin[q] = lo_x;
+        nmax[q] = hi_x + d;
+        xlow = fminf(xlow, hi_x);
+        nhigh = fmaxf(nhigh, lo_x + d);
     }
     if (!(xlow > nhigh)) return kClsNone;                              // empty chord everywhere in the sub-tile
     uint32_t mx = 0u, mn = 0u;                                         // planes that can be active somewhere
@@ -537,10 +540,8 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int wid = (tid >> 5) + kCtaWarps * (int)(blockIdx.x % kCtaSplit);     // sub-tile of the tile
-    const int tpf = a.ntx * a.nty;
-    const int tile = blockIdx.x / kCtaSplit;
-    const int b = tile / tpf, rt = tile - b * tpf;
-    const int ty = rt / a.ntx, tx = rt - ty * a.ntx;
+    const int tx = (int)blockIdx.x / kCtaSplit, ty = (int)blockIdx.y, b = (int)blockIdx.z;   // grid = (ntx * split, nty, B)
+    const int tile = (b * a.nty + ty) * a.ntx + tx;
     pdl_wait();                                                  // k_sort_cull (and all before it) has finished
 
     const bool overflow = (a.status->bits & OSOG_WOVERFLOW) != 0u;
@@ -686,13 +687,13 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
 }
 
 template <bool OPD, bool FIELD, bool RAMP>
-static cudaError_t launch_variant(const ComposeArgs& a, unsigned grid, cudaStream_t stream)
+static cudaError_t launch_variant(const ComposeArgs& a, int B, cudaStream_t stream)
 {
     // opt in to > 48 KB dynamic shared memory (cheap, idempotent; per device, so done on every launch)
     cudaError_t e = cudaFuncSetAttribute(k_compose_tile<OPD, FIELD, RAMP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          kSmemBytes);
     if (e != cudaSuccess) return e;
-    return launch_pdl(k_compose_tile<OPD, FIELD, RAMP>, dim3(grid * kCtaSplit), dim3(kCtaWarps * 32), (size_t)kSmemBytes, stream, a);
+    return launch_pdl(k_compose_tile<OPD, FIELD, RAMP>, dim3(a.ntx * kCtaSplit, a.nty, B), dim3(kCtaWarps * 32), (size_t)kSmemBytes, stream, a);
 }
 
 // sort_first = false: the lists of the last call are already sorted and culled (osog_debug_recompose_field)
@@ -710,11 +711,11 @@ cudaError_t launch_compose(osog_ctx* c, int B, bool has_ramp, float* d_opd, floa
         const cudaError_t e = launch_sort_cull(c, grid, true);
         if (e != cudaSuccess) return e;
     }
-    if (d_opd != nullptr && d_field == nullptr) return launch_variant<true, false, false>(a, grid, c->stream);
-    if (d_opd == nullptr && !has_ramp) return launch_variant<false, true, false>(a, grid, c->stream);
-    if (d_opd == nullptr && has_ramp) return launch_variant<false, true, true>(a, grid, c->stream);
-    if (!has_ramp) return launch_variant<true, true, false>(a, grid, c->stream);
-    return launch_variant<true, true, true>(a, grid, c->stream);
+    if (d_opd != nullptr && d_field == nullptr) return launch_variant<true, false, false>(a, B, c->stream);
+    if (d_opd == nullptr && !has_ramp) return launch_variant<false, true, false>(a, B, c->stream);
+    if (d_opd == nullptr && has_ramp) return launch_variant<false, true, true>(a, B, c->stream);
+    if (!has_ramp) return launch_variant<true, true, false>(a, B, c->stream);
+    return launch_variant<true, true, true>(a, B, c->stream);
 }
 
 // ---- measured alternative: paper-style scatter-add with global atomics ----------------------------
