@@ -217,8 +217,27 @@ int osog_backward_np(osog_ctx* ctx, const osog_particles* p, int64_t N, const os
  * entry faces of a prism, T0 grad w / (2 sqrt w) for an ellipsoid (it grows like 1 / sqrt(w) towards the ellipsoid's
  * outline: the sum over pixel centres is finite but dominated by the outline pixels; it is the almost-everywhere derivative
  * of the pixel-sampled loss, which for ellipsoids also jumps whenever the outline crosses a pixel centre).  Same fixed-order fp64 gather as
- * osog_backward_np.  Gradients with respect to rotation and dimensions are not implemented. */
+ * osog_backward_np.  (Rotation and dimensions: osog_backward_params.) */
 int osog_backward_centre(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gc);
+
+/* Third step of the backward pass: gradient in the shape parameters.  d_gpar[n] = (dL/dd0, dL/dd1, dL/dd2, dL/dqw, dL/dqx,
+ * dL/dqy, dL/dqz)[n] = (n_p[n] - n_medium) * sum over the pixels of d_gopd * dt_n/dtheta, DEVICE float [N, 7], overwritten
+ * (0 for invalid or off-canvas particles).  d0..d2 are the semi-axes (ellipsoid) or side, length, cap height (prism), in
+ * 1/um; the four quaternion components are independent variables of the rotation formula (the library never renormalises the
+ * quaternion, reading A4: project the gradient onto the tangent space of the unit sphere if the caller keeps |q| = 1).
+ * dt/dtheta is analytic (chain rule through R(q), the quadric M = R D R^T or the 12 planes; the active exit and entry planes
+ * of a prism) and shares the caveat of osog_backward_centre for ellipsoids (it grows like 1 / sqrt(w) at the outline).
+ * Works from the particle columns in fp64, same fixed-order gather as osog_backward_np. */
+int osog_backward_params(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gpar);
+
+/* Spectral loss of Eq. 8 (reading A28) and its gradient in the image: for every frame b,
+ * d_loss[b] = sum over all FFT bins of (log(|F(I_b)| + eps) - log(|F(T_b)| + eps))^2 (DEVICE double [B]), F the unnormalised
+ * 2-D DFT, natural logarithm, eps > 0; d_gI (DEVICE float [B, H, W], may be NULL) receives dL/dI = Re DFT2(W),
+ * W = 2 (a - b) / (|F| + eps) * conj(F) / |F|.  d_I, d_I_target: DEVICE float [B, H, W], read only.  3 cuFFTs (2 without the
+ * gradient) + 3 element-wise passes; the block sums of the loss are added in a fixed order (reproducible bits).  The result
+ * feeds osog_backward_intensity -> osog_backward_np / _centre / _params.  Overwrites the context's complex frames; the first
+ * call allocates one more complex frame batch (shared with the DIC path) and the block-sum scratch. */
+int osog_spectral_loss(osog_ctx* ctx, int32_t B, const float* d_I, const float* d_I_target, double eps, double* d_loss, float* d_gI);
 
 /* Second measured alternative: the same tile lists, but one CTA per tile accumulates the tile in SHARED memory with fp32
  * atomics (one warp per listed particle) and writes it out once.  NOT deterministic in the last bits, fp32 sum; kept for

@@ -19,6 +19,8 @@ Pieces, each following the passage it cites (line numbers are /root/reference/PA
   backward_np     dL/dn_p = sum_px G t_n: adjoint of the OPD sum in the indices, in C   :124 (NEXT-3, first step)
   backward_intensity   dL/dOPD from dL/dI: adjoint of field + pupil + |.|^2                :124 (NEXT-3)
   thickness_grad / backward_centre   grad t per pixel; dL/d(cx, cy) = -dn sum_px G grad t  :124 (NEXT-3, second step)
+  thickness_param_grad / backward_params   dt/d(dims, quaternion); dL/d(dims, q) = dn sum_px G dt/dtheta   :124 (NEXT-3, third step)
+  spectral_loss / spectral_loss_grad   Eq. 8 and its gradient in the image                   :168, A28
   render_height / height_gradient / height_laplacian   h, grad h, lap h of the G-buffer :76, :92, :96-99, A25
   fresnel_transmittance / brightfield_amplitude / render_brightfield   Eq. 4       :94-99, A27
   shot_uniforms / poisson_counts / shot_noise          Poisson shot noise          :126, A26
@@ -66,6 +68,11 @@ def _lib():
         lib.osog_oracle_backward_centre.restype = None
         lib.osog_oracle_thickness_grad.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double, dp]
         lib.osog_oracle_thickness_grad.restype = None
+        lib.osog_oracle_thickness_param_grad.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double, dp]
+        lib.osog_oracle_thickness_param_grad.restype = None
+        lib.osog_oracle_backward_params.argtypes = [ctypes.c_int64] + [fp] * 10 + [u8p] + [
+            ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, fp, dp]
+        lib.osog_oracle_backward_params.restype = None
         lib.osog_oracle_thickness.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double]
         lib.osog_oracle_thickness.restype = ctypes.c_double
         lib.osog_oracle_circumradius.argtypes = [ctypes.c_uint8] + [ctypes.c_float] * 3
@@ -248,6 +255,62 @@ def backward_centre(scene, G, mode="bcircle") -> np.ndarray:
             {"full": 0, "bcircle": 1}[mode], _ptr(Gb, f), _ptr(g, ctypes.c_double))
         out[lo:hi] = g
     return out
+
+
+def thickness_param_grad(kind, q, dims, dx, dy) -> np.ndarray:
+    """float64 [7]: dt/d(d0, d1, d2, qw, qx, qy, qz) of one particle's thickness at the offset (dx, dy) from its centre
+    (0 where the chord is empty); the quaternion components are independent variables of the un-normalised rotation formula."""
+    qq = np.ascontiguousarray(q, dtype=np.float64)
+    d = np.ascontiguousarray(dims, dtype=np.float64)
+    g = np.zeros(7, dtype=np.float64)
+    _lib().osog_oracle_thickness_param_grad(int(kind), _ptr(qq, ctypes.c_double), _ptr(d, ctypes.c_double), float(dx), float(dy),
+                                            _ptr(g, ctypes.c_double))
+    return g
+
+
+def backward_params(scene, G, mode="bcircle") -> np.ndarray:
+    """dL/d(d0, d1, d2, qw, qx, qy, qz) [N, 7] float64 for an upstream gradient G = dL/dOPD (float32 [B, H, W]):
+    (n_p - n_medium) * sum over the particle's frame of G * dt/dtheta."""
+    fs = scene.frame_start
+    f = ctypes.c_float
+    out = np.zeros((scene.N, 7), dtype=np.float64)
+    G = np.ascontiguousarray(G, dtype=np.float32)
+    for b in range(scene.B):
+        lo, hi = int(fs[b]), int(fs[b + 1])
+        if hi == lo:
+            continue
+        a = {k: np.ascontiguousarray(scene.cols[k][lo:hi], dtype=np.float32) for k in _COLS}
+        kind = np.ascontiguousarray(scene.cols["kind"][lo:hi], dtype=np.uint8)
+        g = np.zeros((hi - lo, 7), dtype=np.float64)
+        Gb = np.ascontiguousarray(G[b])
+        _lib().osog_oracle_backward_params(
+            hi - lo, _ptr(a["cx"], f), _ptr(a["cy"], f), _ptr(a["qw"], f), _ptr(a["qx"], f), _ptr(a["qy"], f),
+            _ptr(a["qz"], f), _ptr(a["d0"], f), _ptr(a["d1"], f), _ptr(a["d2"], f), _ptr(a["n_p"], f),
+            _ptr(kind, ctypes.c_uint8), scene.H, scene.W, float(scene.pitch_um), float(scene.n_medium),
+            {"full": 0, "bcircle": 1}[mode], _ptr(Gb, f), _ptr(g, ctypes.c_double))
+        out[lo:hi] = g
+    return out
+
+
+def spectral_loss(I, I_target, eps) -> float:
+    """Eq. 8 for one frame: || log(|F(I)| + eps) - log(|F(I_target)| + eps) ||^2 summed over all FFT bins,
+    F = the unnormalised 2-D DFT (reading A28: eps > 0 keeps the logarithm finite at empty bins; natural logarithm)."""
+    a = np.log(np.abs(np.fft.fft2(np.asarray(I, dtype=np.float64))) + eps)
+    b = np.log(np.abs(np.fft.fft2(np.asarray(I_target, dtype=np.float64))) + eps)
+    return float(((a - b) ** 2).sum())
+
+
+def spectral_loss_grad(I, I_target, eps) -> np.ndarray:
+    """dL_spectral / dI [H, W] float64.  With F_k = sum_x I_x e^{-i theta_kx}: d|F_k|/dI_x = Re(conj(F_k) e^{-i theta_kx}) / |F_k|,
+    so dL/dI_x = Re sum_k W_k e^{-i theta_kx} = Re(DFT2(W))_x with W_k = 2 (a_k - b_k) / (|F_k| + eps) * conj(F_k) / |F_k|
+    (W_k = 0 where F_k = 0)."""
+    F = np.fft.fft2(np.asarray(I, dtype=np.float64))
+    absF = np.abs(F)
+    a = np.log(absF + eps)
+    b = np.log(np.abs(np.fft.fft2(np.asarray(I_target, dtype=np.float64))) + eps)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        Wk = np.where(absF > 0.0, 2.0 * (a - b) / (absF + eps) * np.conj(F) / absF, 0.0)
+    return np.real(np.fft.fft2(Wk))
 
 
 def count_covered(scene, mode="bcircle"):

@@ -452,3 +452,159 @@ void osog_oracle_backward_centre(int64_t N,
         g_c[2 * n + 1] = -dn * ay;
     }
 }
+
+
+/* ---- third step of the backward pass: gradient of the thickness with respect to the
+ * particle's SHAPE parameters: grad[0..2] = dt/d(d0, d1, d2) (semi-axes a, b, c or side s, length L, cap height hc),
+ * grad[3..6] = dt/d(qw, qx, qy, qz) (the four quaternion components as independent variables of the rotation formula of
+ * osog_oracle_rot_from_quat, which does not renormalise: reading A4).  Chain rule written out:
+ *   ellipsoid: M = R D R^T, D = diag(1/a^2, 1/b^2, 1/c^2);  dM = dR D R^T + R dD R^T + R D dR^T;
+ *              A = M_zz, Bq = M_xz dx + M_yz dy, C = M_xx dx^2 + 2 M_xy dx dy + M_yy dy^2 - 1, disc = Bq^2 - A C,
+ *              t = 2 sqrt(disc) / A  =>  dt = d(disc) / (A sqrt(disc)) - 2 sqrt(disc) dA / A^2,
+ *              d(disc) = 2 Bq dBq - C dA - A dC;
+ *   prism:     plane k: world normal n = R n_hat, offset b; z_k = (b - n_x dx - n_y dy) / n_z;
+ *              dz_k = (db - dn_x dx - dn_y dy - z_k dn_z) / n_z, dn = dR n_hat + R dn_hat;
+ *              t = z_e - z_f on the active exit plane e (arg min) and entry plane f (arg max)  =>  dt = dz_e - dz_f.
+ * Where the chord is empty the gradient is 0. */
+static void rot_derivatives(const double q[4], double dR[4][9])
+{
+    const double w = q[0], x = q[1], y = q[2], z = q[3];
+    const double dw[9] = { 0.0, -2.0 * z, 2.0 * y,   2.0 * z, 0.0, -2.0 * x,   -2.0 * y, 2.0 * x, 0.0 };
+    const double dx[9] = { 0.0, 2.0 * y, 2.0 * z,    2.0 * y, -4.0 * x, -2.0 * w,   2.0 * z, 2.0 * w, -4.0 * x };
+    const double dy[9] = { -4.0 * y, 2.0 * x, 2.0 * w,   2.0 * x, 0.0, 2.0 * z,   -2.0 * w, 2.0 * z, -4.0 * y };
+    const double dz[9] = { -4.0 * z, -2.0 * w, 2.0 * x,   2.0 * w, -4.0 * z, 2.0 * y,   2.0 * x, 2.0 * y, 0.0 };
+    for (int k = 0; k < 9; ++k) { dR[0][k] = dw[k]; dR[1][k] = dx[k]; dR[2][k] = dy[k]; dR[3][k] = dz[k]; }
+}
+
+void osog_oracle_thickness_param_grad(uint8_t kind, const double q[4], const double dims[3], double dx, double dy,
+                                      double grad[7])
+{
+    for (int p = 0; p < 7; ++p) grad[p] = 0.0;
+    double R[9], dR[4][9];
+    osog_oracle_rot_from_quat(q, R);
+    rot_derivatives(q, dR);
+    if (kind == 0) {
+        const double D[3] = { 1.0 / (dims[0] * dims[0]), 1.0 / (dims[1] * dims[1]), 1.0 / (dims[2] * dims[2]) };
+        double M[9];
+        for (int r = 0; r < 3; ++r)
+            for (int s = 0; s < 3; ++s) {
+                double acc = 0.0;
+                for (int k = 0; k < 3; ++k) acc += R[3 * r + k] * D[k] * R[3 * s + k];
+                M[3 * r + s] = acc;
+            }
+        const double A  = M[8];
+        const double Bq = M[2] * dx + M[5] * dy;
+        const double C  = M[0] * dx * dx + 2.0 * M[1] * dx * dy + M[4] * dy * dy - 1.0;
+        const double disc = Bq * Bq - A * C;
+        if (!(disc > 0.0)) return;
+        const double sq = sqrt(disc);
+        for (int p = 0; p < 7; ++p) {
+            double dM[9];
+            for (int r = 0; r < 3; ++r)
+                for (int s = 0; s < 3; ++s) {
+                    double acc = 0.0;
+                    if (p < 3) {                       /* dD: only entry p of the diagonal, d(1/a^2)/da = -2/a^3 */
+                        const double dDp = -2.0 / (dims[p] * dims[p] * dims[p]);
+                        acc = R[3 * r + p] * dDp * R[3 * s + p];
+                    } else {
+                        const double *dRq = dR[p - 3];
+                        for (int k = 0; k < 3; ++k) acc += dRq[3 * r + k] * D[k] * R[3 * s + k] + R[3 * r + k] * D[k] * dRq[3 * s + k];
+                    }
+                    dM[3 * r + s] = acc;
+                }
+            const double dA  = dM[8];
+            const double dBq = dM[2] * dx + dM[5] * dy;
+            const double dC  = dM[0] * dx * dx + 2.0 * dM[1] * dx * dy + dM[4] * dy * dy;
+            const double ddisc = 2.0 * Bq * dBq - C * dA - A * dC;
+            grad[p] = ddisc / (A * sq) - 2.0 * sq * dA / (A * A);
+        }
+        return;
+    }
+    /* prism: body planes and their derivatives in (s, L, hc), in the construction order of osog_oracle_prism_planes */
+    const double s_ = dims[0], L_ = dims[1], hc = dims[2];
+    double Ab[OSOG_ORACLE_MAX_PLANES][3], b[OSOG_ORACLE_MAX_PLANES];
+    const int M = osog_oracle_prism_planes(s_, L_, hc, Ab, b);
+    double dAb[OSOG_ORACLE_MAX_PLANES][3][3], db[OSOG_ORACLE_MAX_PLANES][3];   /* [plane][parameter][component] */
+    for (int k = 0; k < M; ++k)
+        for (int p = 0; p < 3; ++p) { db[k][p] = 0.0; for (int c = 0; c < 3; ++c) dAb[k][p][c] = 0.0; }
+    for (int k = 0; k < 4; ++k) db[k][0] = 0.5;                                  /* side planes: b = s/2 */
+    for (int k = 4; k < 12; ++k) {
+        /* cap planes: normal (+-hc, 0, +-s/2) or (0, +-hc, +-s/2), b = hc s/2 + s L/4 */
+        db[k][0] = 0.5 * hc + 0.25 * L_;  db[k][1] = 0.25 * s_;  db[k][2] = 0.5 * s_;
+        const int lateral = k < 8 ? 0 : 1;                                       /* which lateral component carries +-hc */
+        dAb[k][2][lateral] = Ab[k][lateral] > 0.0 ? 1.0 : -1.0;                  /* d(+-hc)/dhc */
+        dAb[k][0][2] = Ab[k][2] > 0.0 ? 0.5 : -0.5;                              /* d(+-s/2)/ds */
+    }
+    double Aw[OSOG_ORACLE_MAX_PLANES][3];
+    for (int k = 0; k < M; ++k)
+        for (int r = 0; r < 3; ++r)
+            Aw[k][r] = R[3 * r + 0] * Ab[k][0] + R[3 * r + 1] * Ab[k][1] + R[3 * r + 2] * Ab[k][2];
+    double enter = -INFINITY, exit_ = INFINITY;
+    int ke = -1, kf = -1;
+    for (int k = 0; k < M; ++k) {
+        const double g = b[k] - Aw[k][0] * dx - Aw[k][1] * dy;
+        const double nz = Aw[k][2];
+        if (nz > 0.0)      { const double z = g / nz; if (z < exit_) { exit_ = z; ke = k; } }
+        else if (nz < 0.0) { const double z = g / nz; if (z > enter) { enter = z; kf = k; } }
+        else if (g < 0.0)  return;
+    }
+    if (!(exit_ - enter > 0.0)) return;
+    const int act[2] = { ke, kf };
+    const double zact[2] = { exit_, enter };
+    for (int p = 0; p < 7; ++p) {
+        double dz[2];
+        for (int a = 0; a < 2; ++a) {
+            const int k = act[a];
+            double dn[3], dbk;
+            if (p < 3) {
+                dbk = db[k][p];
+                for (int r = 0; r < 3; ++r)
+                    dn[r] = R[3 * r + 0] * dAb[k][p][0] + R[3 * r + 1] * dAb[k][p][1] + R[3 * r + 2] * dAb[k][p][2];
+            } else {
+                dbk = 0.0;
+                const double *dRq = dR[p - 3];
+                for (int r = 0; r < 3; ++r)
+                    dn[r] = dRq[3 * r + 0] * Ab[k][0] + dRq[3 * r + 1] * Ab[k][1] + dRq[3 * r + 2] * Ab[k][2];
+            }
+            dz[a] = (dbk - dn[0] * dx - dn[1] * dy - zact[a] * dn[2]) / Aw[k][2];
+        }
+        grad[p] = dz[0] - dz[1];
+    }
+}
+
+/* dL/d(d0, d1, d2, qw, qx, qy, qz)[n] = (n_p[n] - n_medium) * sum over pixels of G[px] * dt_n/dtheta[px];  g_p is [N][7]. */
+void osog_oracle_backward_params(int64_t N,
+                                 const float *cx, const float *cy,
+                                 const float *qw, const float *qx, const float *qy, const float *qz,
+                                 const float *d0, const float *d1, const float *d2,
+                                 const float *n_p, const uint8_t *kind,
+                                 int H, int W, double pitch, double n_medium, int mode, const float *G, double *g_p)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t n = 0; n < N; ++n) {
+        for (int p = 0; p < 7; ++p) g_p[7 * n + p] = 0.0;
+        if (!osog_oracle_particle_valid(cx[n], cy[n], qw[n], qx[n], qy[n], qz[n],
+                                        d0[n], d1[n], d2[n], n_p[n], kind[n])) continue;
+        const double q[4] = { qw[n], qx[n], qy[n], qz[n] };
+        const double dims[3] = { d0[n], d1[n], d2[n] };
+        double r2 = INFINITY;
+        if (mode == 1) {
+            const double r = osog_oracle_circumradius(kind[n], d0[n], d1[n], d2[n]) * (1.0 + 1e-9);
+            r2 = r * r;
+        }
+        double acc[7] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
+        for (int i = 0; i < H; ++i) {
+            const double dy = (i + 0.5) * pitch - (double)cy[n];
+            if (dy * dy > r2) continue;
+            for (int j = 0; j < W; ++j) {
+                const double dx = (j + 0.5) * pitch - (double)cx[n];
+                if (dx * dx + dy * dy > r2) continue;
+                double gr[7];
+                osog_oracle_thickness_param_grad(kind[n], q, dims, dx, dy, gr);
+                for (int p = 0; p < 7; ++p) acc[p] += (double)G[(size_t)i * W + j] * gr[p];
+            }
+        }
+        const double dn = (double)n_p[n] - n_medium;
+        for (int p = 0; p < 7; ++p) g_p[7 * n + p] = dn * acc[p];
+    }
+}

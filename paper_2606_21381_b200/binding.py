@@ -85,6 +85,8 @@ def lib():
     L.osog_field_to_dic.argtypes = [ctx, C.POINTER(osog_optics), C.POINTER(osog_dic), C.c_void_p, C.c_void_p]
     L.osog_backward_np.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_backward_intensity.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
+    L.osog_spectral_loss.argtypes = [ctx, C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
+    L.osog_backward_params.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_backward_centre.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_gbuffer.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_height.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p,
@@ -107,7 +109,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_brightfield", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_intensity", "osog_debug_recompose_field", "osog_debug_check_guards", "osog_debug_poisson", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_brightfield", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_params", "osog_spectral_loss", "osog_backward_intensity", "osog_debug_recompose_field", "osog_debug_check_guards", "osog_debug_poisson", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -300,6 +302,26 @@ class Context:
         self._done(lib().osog_backward_centre(self._ctx, C.byref(p.c), p.N, C.byref(o), gopd.data_ptr(), out.data_ptr()),
                    "osog_backward_centre")
         return out
+
+    def backward_params(self, p: Particles, o, gopd):
+        """float32 [N, 7] dL/d(d0, d1, d2, qw, qx, qy, qz) for an upstream gradient gopd = dL/dOPD (osog_backward_params)."""
+        out = self.torch.empty((p.N, 7), dtype=self.torch.float32, device=self.device)
+        gopd = self._in(gopd, (o.B, self.H, self.W), "gopd")
+        self._done(lib().osog_backward_params(self._ctx, C.byref(p.c), p.N, C.byref(o), gopd.data_ptr(), out.data_ptr()),
+                   "osog_backward_params")
+        return out
+
+    def spectral_loss(self, I, I_target, eps, grad=True):
+        """(float64 [B] loss of Eq. 8, float32 [B, H, W] dL/dI or None) for images I, I_target (float32 [B, H, W]) (osog_spectral_loss)."""
+        B = int(I.shape[0])
+        I = self._in(I, (B, self.H, self.W), "I")
+        T = self._in(I_target, (B, self.H, self.W), "I_target")
+        loss = self.torch.empty((B,), dtype=self.torch.float64, device=self.device)
+        g = self._out(B) if grad else None
+        r = lib().osog_spectral_loss(self._ctx, B, I.data_ptr(), T.data_ptr(), float(eps), loss.data_ptr(), g.data_ptr() if grad else None)
+        if r != OSOG_OK:
+            raise OsogError(r, "osog_spectral_loss")
+        return loss, g
 
     def render_gbuffer(self, p: Particles, o):
         """(int32 [B, H, W] instance id of the top-most particle, float32 [B, H, W] height of its top surface)."""

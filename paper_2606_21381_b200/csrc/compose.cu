@@ -1039,6 +1039,183 @@ __global__ void __launch_bounds__(256) k_backward_centre(const float* __restrict
     if (lane == 0) gc[n] = make_float2((float)(scale * ax), (float)(scale * ay));
 }
 
+// ---- third step of the backward pass: dL/d(d0, d1, d2, qw, qx, qy, qz)[n] =
+// (n_p - n_m) sum_px G[px] dt_n/dtheta[px].  The shape parameters enter through the rotation and the body's planes / quadric,
+// which the derived record no longer shows, so this kernel works from the particle columns themselves, all in fp64:
+//   ellipsoid: M = R D R^T; per parameter dM = dR D R^T + R dD R^T + R D dR^T (once per particle); per pixel
+//              disc = Bq^2 - A C, t = 2 sqrt(disc) / A, dt = d(disc) / (A sqrt(disc)) - 2 sqrt(disc) dA / A^2;
+//   prism:     per pixel the active exit / entry planes e, f of the 12 world planes (arg min / arg max of
+//              z_k = (b_k - n_x dx - n_y dy) / n_z); dz_k = (db_k - dn_x dx - dn_y dy - z_k dn_z) / n_z with
+//              dn = dR n_hat (rotation) or R dn_hat (dimensions); dt = dz_e - dz_f.
+// Same gather as k_backward_np: one warp per particle over its pixel bounding box, fixed order (reproducible bits).
+struct ParamGradArgs {
+    const float *cx, *cy, *qw, *qx, *qy, *qz, *d0, *d1, *d2, *n_p;
+    const uint8_t* kind;
+    const float* recs;
+    const int4* tbox;
+    const int* pframe;
+    long long N;
+    int H, W;
+    double pitch, n_medium;
+    const float* gopd;
+    float* gpar;                  // [N][7]
+};
+
+// body-frame plane k of the capped prism (0, 1: +-x; 2, 3: +-y; 4..7: (+-hc, 0, +-s/2); 8..11: (0, +-hc, +-s/2)) and its
+// derivatives in (s, L, hc)
+__device__ __forceinline__ void prism_plane(int k, double s, double L, double hc, double nb[3], double* b, double dnb[3][3], double db[3])
+{
+#pragma unroll
+    for (int p = 0; p < 3; ++p) { db[p] = 0.0; dnb[p][0] = dnb[p][1] = dnb[p][2] = 0.0; }
+    nb[0] = nb[1] = nb[2] = 0.0;
+    if (k < 4) {
+        nb[k >> 1] = (k & 1) ? -1.0 : 1.0;
+        *b = 0.5 * s;
+        db[0] = 0.5;
+        return;
+    }
+    const int lat = k < 8 ? 0 : 1;                 // lateral component that carries +-hc
+    const int kk = (k - 4) & 3;
+    const double sl = (kk & 1) ? -1.0 : 1.0, sz = (kk & 2) ? -1.0 : 1.0;
+    nb[lat] = sl * hc;
+    nb[2] = sz * 0.5 * s;
+    *b = hc * s * 0.5 + s * L * 0.25;
+    db[0] = 0.5 * hc + 0.25 * L; db[1] = 0.25 * s; db[2] = 0.5 * s;
+    dnb[2][lat] = sl;                              // d / dhc
+    dnb[0][2] = sz * 0.5;                          // d / ds
+}
+
+__global__ void __launch_bounds__(256) k_backward_params(const ParamGradArgs a)
+{
+    const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (n >= a.N) return;
+    double acc[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    double dn_idx = 0.0;
+    if (a.tbox[n].x <= a.tbox[n].y) {              // listed: valid and on the canvas (else the gradient is 0)
+        const float4* rec = reinterpret_cast<const float4*>(a.recs + (size_t)n * kRecWords);
+        const float4 h1 = rec[1];
+        const uint32_t bx = __float_as_uint(h1.z), by = __float_as_uint(h1.w);
+        const int j0 = bx & 0xffff, j1 = bx >> 16, i0 = by & 0xffff, i1 = by >> 16;
+        const int bw = j1 - j0 + 1, np = bw * (i1 - i0 + 1);
+        const float* g = a.gopd + (size_t)a.pframe[n] * a.H * a.W;
+        const double cx = a.cx[n], cy = a.cy[n], w = a.qw[n], x = a.qx[n], y = a.qy[n], z = a.qz[n];
+        const double e[3] = {(double)a.d0[n], (double)a.d1[n], (double)a.d2[n]};
+        dn_idx = (double)a.n_p[n] - a.n_medium;
+        const double R[9] = {1.0 - 2.0 * (y * y + z * z), 2.0 * (x * y - w * z), 2.0 * (x * z + w * y),
+                             2.0 * (x * y + w * z), 1.0 - 2.0 * (x * x + z * z), 2.0 * (y * z - w * x),
+                             2.0 * (x * z - w * y), 2.0 * (y * z + w * x), 1.0 - 2.0 * (x * x + y * y)};
+        const double dR[4][9] = {{0.0, -2.0 * z, 2.0 * y, 2.0 * z, 0.0, -2.0 * x, -2.0 * y, 2.0 * x, 0.0},
+                                 {0.0, 2.0 * y, 2.0 * z, 2.0 * y, -4.0 * x, -2.0 * w, 2.0 * z, 2.0 * w, -4.0 * x},
+                                 {-4.0 * y, 2.0 * x, 2.0 * w, 2.0 * x, 0.0, 2.0 * z, -2.0 * w, 2.0 * z, -4.0 * y},
+                                 {-4.0 * z, -2.0 * w, 2.0 * x, 2.0 * w, -4.0 * z, 2.0 * y, 2.0 * x, 2.0 * y, 0.0}};
+        if (a.kind[n] == 0u) {
+            const double D[3] = {1.0 / (e[0] * e[0]), 1.0 / (e[1] * e[1]), 1.0 / (e[2] * e[2])};
+            // symmetric 3 x 3 as (xx, xy, yy, xz, yz, zz)
+            const int ra[6] = {0, 0, 1, 0, 1, 2}, rb[6] = {0, 1, 1, 2, 2, 2};
+            double M[6], dM[7][6];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) {
+                M[c] = 0.0;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) M[c] += R[3 * ra[c] + k] * D[k] * R[3 * rb[c] + k];
+#pragma unroll
+                for (int p = 0; p < 3; ++p) dM[p][c] = R[3 * ra[c] + p] * (-2.0 * D[p] / e[p]) * R[3 * rb[c] + p];
+#pragma unroll
+                for (int p = 0; p < 4; ++p) {
+                    double v = 0.0;
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) v += (dR[p][3 * ra[c] + k] * R[3 * rb[c] + k] + R[3 * ra[c] + k] * dR[p][3 * rb[c] + k]) * D[k];
+                    dM[3 + p][c] = v;
+                }
+            }
+            for (int q = lane; q < np; q += 32) {
+                const int i = i0 + q / bw, j = j0 + q % bw;
+                const double dx = (j + 0.5) * a.pitch - cx, dy = (i + 0.5) * a.pitch - cy;
+                const double A = M[5], Bq = M[3] * dx + M[4] * dy, C = M[0] * dx * dx + 2.0 * M[1] * dx * dy + M[2] * dy * dy - 1.0;
+                const double disc = Bq * Bq - A * C;
+                if (!(disc > 0.0)) continue;
+                const double sq = sqrt(disc), gv = (double)g[(size_t)i * a.W + j];
+                const double c1 = 1.0 / (A * sq), c2 = 2.0 * sq / (A * A);
+#pragma unroll
+                for (int p = 0; p < 7; ++p) {
+                    const double dA = dM[p][5], dBq = dM[p][3] * dx + dM[p][4] * dy;
+                    const double dC = dM[p][0] * dx * dx + 2.0 * dM[p][1] * dx * dy + dM[p][2] * dy * dy;
+                    acc[p] = fma(gv, (2.0 * Bq * dBq - C * dA - A * dC) * c1 - c2 * dA, acc[p]);
+                }
+            }
+        } else {
+            double nw[12][3], bb[12];
+#pragma unroll 1
+            for (int k = 0; k < 12; ++k) {
+                double nb[3], dnb[3][3], db[3];
+                prism_plane(k, e[0], e[1], e[2], nb, &bb[k], dnb, db);
+                for (int r = 0; r < 3; ++r) nw[k][r] = R[3 * r] * nb[0] + R[3 * r + 1] * nb[1] + R[3 * r + 2] * nb[2];
+            }
+            for (int q = lane; q < np; q += 32) {
+                const int i = i0 + q / bw, j = j0 + q % bw;
+                const double dx = (j + 0.5) * a.pitch - cx, dy = (i + 0.5) * a.pitch - cy;
+                double ex = 1.0e300, en = -1.0e300;
+                int ke = 0, kf = 0;
+                bool out = false;
+#pragma unroll 1
+                for (int k = 0; k < 12; ++k) {
+                    const double gk = bb[k] - nw[k][0] * dx - nw[k][1] * dy, nz = nw[k][2];
+                    if (nz > 0.0) { const double zk = gk / nz; if (zk < ex) { ex = zk; ke = k; } }
+                    else if (nz < 0.0) { const double zk = gk / nz; if (zk > en) { en = zk; kf = k; } }
+                    else if (gk < 0.0) out = true;
+                }
+                if (out || !(ex - en > 0.0)) continue;
+                const double gv = (double)g[(size_t)i * a.W + j];
+#pragma unroll 1
+                for (int side = 0; side < 2; ++side) {
+                    const int k = side ? kf : ke;
+                    const double zk = side ? en : ex, sgn = side ? -1.0 : 1.0, inz = 1.0 / nw[k][2];
+                    double nb[3], bk, dnb[3][3], db[3];
+                    prism_plane(k, e[0], e[1], e[2], nb, &bk, dnb, db);
+#pragma unroll
+                    for (int p = 0; p < 7; ++p) {
+                        double dnx, dny, dnz, dbk;
+                        if (p < 3) {
+                            dbk = db[p];
+                            dnx = R[0] * dnb[p][0] + R[1] * dnb[p][1] + R[2] * dnb[p][2];
+                            dny = R[3] * dnb[p][0] + R[4] * dnb[p][1] + R[5] * dnb[p][2];
+                            dnz = R[6] * dnb[p][0] + R[7] * dnb[p][1] + R[8] * dnb[p][2];
+                        } else {
+                            dbk = 0.0;
+                            const double* d = dR[p - 3];
+                            dnx = d[0] * nb[0] + d[1] * nb[1] + d[2] * nb[2];
+                            dny = d[3] * nb[0] + d[4] * nb[1] + d[5] * nb[2];
+                            dnz = d[6] * nb[0] + d[7] * nb[1] + d[8] * nb[2];
+                        }
+                        acc[p] = fma(gv * sgn, (dbk - dnx * dx - dny * dy - zk * dnz) * inz, acc[p]);
+                    }
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int p = 0; p < 7; ++p) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) acc[p] += __shfl_xor_sync(0xffffffffu, acc[p], d);
+        if (lane == 0) a.gpar[(size_t)n * 7 + p] = (float)(dn_idx * acc[p]);
+    }
+}
+
+cudaError_t launch_backward_params(osog_ctx* c, const osog_particles* p, long long N, double pitch, double n_medium,
+                                   const float* d_gopd, float* d_gpar)
+{
+    if (N == 0) return cudaSuccess;
+    ParamGradArgs a;
+    a.cx = p->cx; a.cy = p->cy; a.qw = p->qw; a.qx = p->qx; a.qy = p->qy; a.qz = p->qz;
+    a.d0 = p->d0; a.d1 = p->d1; a.d2 = p->d2; a.n_p = p->n_p; a.kind = p->kind;
+    a.recs = c->rec; a.tbox = c->tbox; a.pframe = c->pframe; a.N = N; a.H = c->H; a.W = c->W;
+    a.pitch = pitch; a.n_medium = n_medium; a.gopd = d_gopd; a.gpar = d_gpar;
+    const long long threads = N * 32;
+    k_backward_params<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(a);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_backward_centre(osog_ctx* c, long long N, double pitch, const float* d_gopd, float* d_gc)
 {
     if (N == 0) return cudaSuccess;

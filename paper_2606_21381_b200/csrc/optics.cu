@@ -145,6 +145,97 @@ cudaError_t launch_brightfield(osog_ctx* c, int B, float2* field, const float* d
     return cudaGetLastError();
 }
 
+// ---- spectral loss of Eq. 8 (reading A28) and its gradient in the image -----------------
+__global__ void __launch_bounds__(256) k_real_to_complex(const float* __restrict__ a, const float* __restrict__ b,
+                                                         float2* __restrict__ ca, float2* __restrict__ cb, size_t n)
+{
+    const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    ca[k] = make_float2(a[k], 0.0f);
+    cb[k] = make_float2(b[k], 0.0f);
+}
+
+// per bin: d = log(|F| + eps) - log(|T| + eps); partial[b][block] = sum of d^2 over the block's bins (fixed order);
+// F <- W = 2 d / (|F| + eps) * conj(F) / |F|  (0 where F = 0): the forward DFT of W has dL/dI as its real part
+__global__ void __launch_bounds__(256) k_spectral_terms(float2* __restrict__ F, const float2* __restrict__ T, size_t npx, double eps,
+                                                        double* __restrict__ partial, int want_grad)
+{
+    __shared__ double s_sum[8];
+    const size_t pix = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int b = blockIdx.y;
+    double d2 = 0.0;
+    if (pix < npx) {
+        const float2 f = F[(size_t)b * npx + pix], t = T[(size_t)b * npx + pix];
+        const double af = sqrt((double)f.x * f.x + (double)f.y * f.y), at = sqrt((double)t.x * t.x + (double)t.y * t.y);
+        const double d = log(af + eps) - log(at + eps);
+        d2 = d * d;
+        if (want_grad) {
+            const double w = af > 0.0 ? 2.0 * d / ((af + eps) * af) : 0.0;
+            F[(size_t)b * npx + pix] = make_float2((float)(w * f.x), (float)(-w * f.y));
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) d2 += __shfl_xor_sync(0xffffffffu, d2, o);
+    if ((threadIdx.x & 31) == 0) s_sum[threadIdx.x >> 5] = d2;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) v += s_sum[w];
+        partial[(size_t)b * gridDim.x + blockIdx.x] = v;
+    }
+}
+
+// loss[b] = sum of the frame's block partials, in a fixed order (one block per frame)
+__global__ void __launch_bounds__(256) k_sum_partials(const double* __restrict__ partial, int nblk, double* __restrict__ loss)
+{
+    __shared__ double s_sum[8];
+    const int b = blockIdx.x;
+    double v = 0.0;
+    for (int k = threadIdx.x; k < nblk; k += 256) v += partial[(size_t)b * nblk + k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) s_sum[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) t += s_sum[w];
+        loss[b] = t;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_real_part(const float2* __restrict__ c, float* __restrict__ out, size_t n)
+{
+    const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) out[k] = c[k].x;
+}
+
+cudaError_t launch_real_to_complex(osog_ctx* c, int B, const float* a, const float* b, float2* ca, float2* cb)
+{
+    const size_t n = (size_t)B * c->H * c->W;
+    k_real_to_complex<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(a, b, ca, cb, n);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_spectral_terms(osog_ctx* c, int B, float2* F, const float2* T, double eps, double* partial, double* d_loss, bool want_grad)
+{
+    const size_t npx = (size_t)c->H * c->W;
+    const unsigned nblk = (unsigned)((npx + 255) / 256);
+    k_spectral_terms<<<dim3(nblk, B), 256, 0, c->stream>>>(F, T, npx, eps, partial, want_grad ? 1 : 0);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    k_sum_partials<<<B, 256, 0, c->stream>>>(partial, (int)nblk, d_loss);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_real_part(osog_ctx* c, int B, const float2* in, float* out)
+{
+    const size_t n = (size_t)B * c->H * c->W;
+    k_real_part<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(in, out, n);
+    return cudaGetLastError();
+}
+
 // buf = (|buf|^2 * scale, 0)
 __global__ void __launch_bounds__(256) k_abs2(float2* __restrict__ buf, size_t n, float scale)
 {

@@ -196,7 +196,7 @@ int osog_destroy(osog_ctx* c)
     if (c->has_plan_batch) cufftDestroy(c->plan_batch);
     cudaFree(c->rec); cudaFree(c->rec2); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
     cudaFree(c->list); cudaFree(c->meta); cudaFree(c->slices); cudaFree(c->offset); cudaFree(c->done); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
-    cudaFree(c->status); cudaFree(c->field); cudaFree(c->work); cudaFree(c->otf); cudaFree(c->bf_h);
+    cudaFree(c->status); cudaFree(c->field); cudaFree(c->work); cudaFree(c->otf); cudaFree(c->bf_h); cudaFree(c->spec_partial);
     delete c->otf_key;
     delete c->guards;
     if (c->h_status) cudaFreeHost(c->h_status);
@@ -500,6 +500,47 @@ int osog_backward_centre(osog_ctx* c, const osog_particles* p, int64_t N, const 
     cudaError_t e = launch_binning(c, p, N, o);      // records + bounding boxes (the tile lists are not used)
     if (e != cudaSuccess) return cuda_fail(c, e);    // (scratch_dirty stays set: the next render call clears them)
     e = launch_backward_centre(c, N, o->pitch_um, d_gopd, d_gc);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return OSOG_OK;
+}
+
+int osog_spectral_loss(osog_ctx* c, int32_t B, const float* d_I, const float* d_I_target, double eps, double* d_loss, float* d_gI)
+{
+    if (!c || !d_I || !d_I_target || !d_loss || B < 1 || B > c->max_frames || !(eps > 0.0) || !(eps < 1.0e300)) return OSOG_EINVAL;
+    if (!aligned16(d_I) || !aligned16(d_I_target) || (d_gI && !aligned16(d_gI))) return OSOG_EINVAL;
+    DeviceGuard g(c->device);
+    if (!c->work) {
+        const cudaError_t ea = dalloc(&c->work, (size_t)c->max_frames * c->H * c->W, c);
+        if (ea != cudaSuccess) { cudaGetLastError(); c->work = nullptr; return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea); }
+    }
+    const size_t nblk = ((size_t)c->H * c->W + 255) / 256;
+    if (!c->spec_partial) {
+        const cudaError_t ea = dalloc(&c->spec_partial, (size_t)c->max_frames * nblk, c);
+        if (ea != cudaSuccess) { cudaGetLastError(); c->spec_partial = nullptr; return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea); }
+    }
+    c->last_has_ramp = -1;                           // the context's complex frame is overwritten
+    cudaError_t e = launch_real_to_complex(c, B, d_I, d_I_target, c->field, c->work);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    int r;
+    if ((r = fft_frames(c, c->field, B, CUFFT_FORWARD)) != OSOG_OK) return r;
+    if ((r = fft_frames(c, c->work, B, CUFFT_FORWARD)) != OSOG_OK) return r;
+    if ((e = launch_spectral_terms(c, B, c->field, c->work, eps, c->spec_partial, d_loss, d_gI != nullptr)) != cudaSuccess) return cuda_fail(c, e);
+    if (!d_gI) return OSOG_OK;
+    if ((r = fft_frames(c, c->field, B, CUFFT_FORWARD)) != OSOG_OK) return r;
+    if ((e = launch_real_part(c, B, c->field, d_gI)) != cudaSuccess) return cuda_fail(c, e);
+    return OSOG_OK;
+}
+
+int osog_backward_params(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gpar)
+{
+    if (!d_gopd || !aligned16(d_gopd)) return OSOG_EINVAL;
+    if (N == 0) return (c && p && o) ? OSOG_OK : OSOG_EINVAL;
+    const int r = check_call(c, p, N, o, d_gpar);
+    if (r != OSOG_OK) return r;
+    DeviceGuard g(c->device);
+    cudaError_t e = launch_binning(c, p, N, o);      // tile ranges, frames and pixel bounding boxes (the tile lists are not used)
+    if (e != cudaSuccess) return cuda_fail(c, e);    // (scratch_dirty stays set: the next render call clears them)
+    e = launch_backward_params(c, p, N, o->pitch_um, o->n_medium, d_gopd, d_gpar);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return OSOG_OK;
 }

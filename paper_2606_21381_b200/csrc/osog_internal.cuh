@@ -87,6 +87,7 @@ struct osog_ctx {
     bool scratch_dirty;             // a call failed midway: count / status must be cleared explicitly
     float2* field;                  // [max_frames][H][W] (intensity path)
     float2* work;                   // [max_frames][H][W] second complex batch (DIC path; allocated by the first DIC call)
+    double* spec_partial;           // [max_frames][ceil(H W / 256)] block sums of the spectral loss (allocated by its first call)
     float* bf_h;                    // [max_frames][H][W] height map of the brightfield path (allocated by its first call)
     float2* otf;                    // [max_frames][H][W] optical transfer function F{|F^-1{P}|^2} of the last DIC call
     std::vector<double>* otf_key;   // optics the cached OTF was built for (B, pitch, n_medium, defocus, pupil, lambda[], NA[])
@@ -130,6 +131,8 @@ cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd)
 cudaError_t launch_compose_smem_atomic(osog_ctx* c, int B, float* d_opd);
 cudaError_t launch_backward_np(osog_ctx* c, long long N, const float* d_gopd, float* d_gnp);
 cudaError_t launch_backward_centre(osog_ctx* c, long long N, double pitch, const float* d_gopd, float* d_gc);
+cudaError_t launch_backward_params(osog_ctx* c, const osog_particles* p, long long N, double pitch, double n_medium,
+                                   const float* d_gopd, float* d_gpar);
 cudaError_t launch_gbuffer(osog_ctx* c, int B, const int32_t* d_frame_start, int32_t* d_top_id, float* d_depth);
 // optics.cu
 cudaError_t launch_pupil(osog_ctx* c, int B, float2* spec, double pitch, bool defocus);
@@ -142,6 +145,9 @@ cudaError_t launch_abs2(osog_ctx* c, int B, float2* buf, double scale);
 cudaError_t launch_cmul(osog_ctx* c, int B, float2* a, const float2* b, double scale);
 cudaError_t launch_brightfield(osog_ctx* c, int B, float2* field, const float* d_h, double pitch, double n1, double n2,
                                double dmu, double gain);
+cudaError_t launch_real_to_complex(osog_ctx* c, int B, const float* a, const float* b, float2* ca, float2* cb);
+cudaError_t launch_spectral_terms(osog_ctx* c, int B, float2* F, const float2* T, double eps, double* partial, double* d_loss, bool want_grad);
+cudaError_t launch_real_part(osog_ctx* c, int B, const float2* in, float* out);
 cudaError_t launch_height_stencil(osog_ctx* c, int B, const float* d_h, double pitch, float* d_grad, float* d_lap);
 cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_out, double sigma, double photons, uint64_t seed);
 cudaError_t launch_sensor(osog_ctx* c, int B, const float2* img, float* d_intensity, double sigma, double photons, uint64_t seed);

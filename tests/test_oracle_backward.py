@@ -158,3 +158,142 @@ def test_B7_adjoint_of_the_optics_stage_is_the_forward_model_differenced():
     # all-pass pupil: I == 1 whatever the OPD, so every gradient vanishes
     sc0 = replace(sc, defocus_um=0.0)
     assert np.abs(o.backward_intensity(sc0, Wt[None], U=U, pupil_enabled=False)).max() < 1e-12
+
+
+# ---- third step: shape parameters (dimensions, rotation) and the spectral loss of Eq. 8 -------------------------------------
+def _interior_points(kind, q, dims, rng, n):
+    """Offsets with a comfortably positive chord (not within a few 1e-3 of an outline or of a face change)."""
+    pts = []
+    r = o.circumradius(kind, dims)
+    while len(pts) < n:
+        dx, dy = rng.uniform(-r, r, 2)
+        if o.thickness(kind, q, dims, dx, dy) > 0.05 * r:
+            pts.append((dx, dy))
+    return pts
+
+
+def test_B8_shape_gradient_equals_the_differenced_thickness():
+    """dt/d(d0, d1, d2, qw, qx, qy, qz) against central differences of the pinned thickness (P1-P7, P13) at interior points,
+    both kinds, random rotations (the quaternion is NOT re-normalised after the step: the components are independent)."""
+    rng = np.random.default_rng(8)
+    h = 1e-6
+    checked = 0
+    for trial in range(60):
+        kind = trial % 2
+        q = rng.standard_normal(4); q /= np.linalg.norm(q)
+        dims = rng.uniform(0.8, 3.0, 3) if kind == 0 else np.array([rng.uniform(1, 3), rng.uniform(2, 6), rng.uniform(0.5, 1.5)])
+        for dx, dy in _interior_points(kind, q, dims, rng, 5):
+            g = o.thickness_param_grad(kind, q, dims, dx, dy)
+            par = np.concatenate([dims, q])
+            fd = np.zeros(7)
+            kink = False
+            for p in range(7):
+                up, dn_ = par.copy(), par.copy()
+                up[p] += h; dn_[p] -= h
+                tp, tm = o.thickness(kind, up[3:], up[:3], dx, dy), o.thickness(kind, dn_[3:], dn_[:3], dx, dy)
+                t0 = o.thickness(kind, q, dims, dx, dy)
+                fd[p] = (tp - tm) / (2 * h)
+                kink = kink or abs(tp - 2 * t0 + tm) > 1e-9              # a face change inside the stencil: skip the point
+            if kink:
+                continue
+            assert np.allclose(g, fd, rtol=2e-6, atol=2e-7), (kind, g, fd)
+            checked += 1
+    assert checked > 200
+
+
+def test_B9_shape_gradient_closed_forms():
+    # sphere a = b = c = R: t = 2 sqrt(R^2 - r^2); growing all three semi-axes together gives dt/dR = 2 R / sqrt(R^2 - r^2)
+    R, dx, dy = 2.0, 0.7, -0.4
+    g = o.thickness_param_grad(0, [1, 0, 0, 0], [R, R, R], dx, dy)
+    assert abs(g[:3].sum() - 2 * R / np.sqrt(R * R - dx * dx - dy * dy)) < 1e-12
+    # axis-aligned ellipsoid t = 2 c sqrt(1 - (dx/a)^2 - (dy/b)^2)
+    a, b, c = 2.0, 1.5, 0.8
+    w = 1 - (dx / a) ** 2 - (dy / b) ** 2
+    g = o.thickness_param_grad(0, [1, 0, 0, 0], [a, b, c], dx, dy)
+    assert np.allclose(g[:3], [2 * c * dx * dx / a ** 3 / np.sqrt(w), 2 * c * dy * dy / b ** 3 / np.sqrt(w), 2 * np.sqrt(w)], atol=1e-12)
+    # a sphere does not care about its rotation
+    q = np.array([0.3, -0.5, 0.4, 0.7]); q /= np.linalg.norm(q)
+    g = o.thickness_param_grad(0, q, [R, R, R], dx, dy)
+    tangent = g[3:] - (g[3:] @ q) * q                               # (the radial component rescales R(q): not a rotation)
+    assert np.abs(tangent).max() < 1e-12
+    # prism, identity rotation (P5): t = L + 2 hc (1 - m / (s/2)), m = max(|dx|, |dy|)
+    s, L, hc = 2.0, 3.0, 0.9
+    m = 0.61
+    g = o.thickness_param_grad(1, [1, 0, 0, 0], [s, L, hc], m, 0.2)
+    assert np.allclose(g[:3], [4 * hc * m / s ** 2, 1.0, 2 * (1 - m / (s / 2))], atol=1e-12)
+
+
+def test_B10_backward_params_sums_the_pixel_gradients_and_matches_the_differenced_forward_model():
+    sc = make_config(4, n_override=24)
+    for k in ("cx", "cy"):
+        sc.cols[k][:] = (sc.cols[k] / 16.0).astype(np.float32)
+    sc = replace(sc, H=128, W=128)
+    rng = np.random.default_rng(5)
+    G = rng.standard_normal((1, 128, 128)).astype(np.float32)
+    g = o.backward_params(sc, G)
+    assert np.array_equal(g, o.backward_params(sc, G, mode="full"))
+    # (a) the sum itself: dn * sum_px G * dt/dtheta with the pinned per-pixel gradient (B8, B9), written as a plain loop
+    for n in (2, 7):
+        c = sc.cols
+        q = [float(c[k][n]) for k in ("qw", "qx", "qy", "qz")]; d = [float(c[k][n]) for k in ("d0", "d1", "d2")]
+        acc = np.zeros(7)
+        for i in range(128):
+            for j in range(128):
+                dx, dy = (j + 0.5) * sc.pitch_um - float(c["cx"][n]), (i + 0.5) * sc.pitch_um - float(c["cy"][n])
+                if dx * dx + dy * dy < 200.0:
+                    acc += float(G[0, i, j]) * o.thickness_param_grad(int(c["kind"][n]), q, d, dx, dy)
+        assert np.allclose(g[n], (float(c["n_p"][n]) - sc.n_medium) * acc, rtol=1e-10, atol=1e-12)
+    # (b) against the forward model differenced in the parameter, for the PRISMS (piecewise linear thickness) with a smooth
+    # upstream gradient.  (For ellipsoids dt/dtheta grows like 1 / sqrt(w) towards the outline, the sum
+    # over pixel centres is dominated by the outline pixels and the pixel-sampled loss has sqrt-type kinks: its difference
+    # quotient scatters by up to 20 % around the almost-everywhere derivative; B8, B9 and (a) pin that case.)
+    jj, ii = np.meshgrid(np.arange(128), np.arange(128))
+    Gs = (np.cos(0.05 * jj + 0.3) * np.sin(0.04 * ii + 1.0)).astype(np.float32)[None]
+    gs = o.backward_params(sc, Gs)
+    names = ("d0", "d1", "d2", "qw", "qx", "qy", "qz")
+    h = 2.0 ** -11                                                  # exactly representable steps on the float32 scene
+    dev = []
+    for n in np.flatnonzero(sc.cols["kind"] == 1):
+        for p, name in enumerate(names):
+            vals = []
+            for sgn in (+1, -1):
+                cols = {k: v.copy() for k, v in sc.cols.items()}
+                cols[name][n] = np.float32(cols[name][n] + sgn * h)
+                step = float(cols[name][n]) - float(sc.cols[name][n])
+                vals.append((float((Gs[0].astype(np.float64) * o.render_opd(replace(sc, cols=cols))[0]).sum()), step))
+            fd = (vals[0][0] - vals[1][0]) / (vals[0][1] - vals[1][1])
+            dev.append(abs(gs[n, p] - fd) / max(abs(fd), np.abs(gs[n]).max()))
+    dev = np.array(dev)
+    # most of the 84 (prism, parameter) pairs agree to 1e-4; where a steep face sweeps over pixel centres within the step the
+    # difference quotient itself is off by up to a few per cent
+    assert len(dev) >= 70 and np.median(dev) < 1e-3 and np.percentile(dev, 90) < 1e-2 and dev.max() < 5e-2, \
+        (np.median(dev), np.percentile(dev, 90), dev.max())
+
+
+def test_B11_spectral_loss_and_its_gradient():
+    rng = np.random.default_rng(3)
+    I = 1.0 + 0.2 * rng.standard_normal((12, 10))
+    T = 1.0 + 0.2 * rng.standard_normal((12, 10))
+    eps = 1e-3
+    assert o.spectral_loss(T, T, eps) == 0.0
+    assert abs(o.spectral_loss(I, np.roll(T, (3, -2), (0, 1)), eps) - o.spectral_loss(I, T, eps)) < 1e-9   # |F| ignores circular shifts
+    # eps -> 0: scaling the image shifts every log|F| by log c: loss = n_bins log(c)^2 against itself
+    assert abs(o.spectral_loss(3.0 * T, T, 1e-300) - T.size * np.log(3.0) ** 2) < 1e-9
+    # brute-force DFT instead of the library FFT
+    ky, kx = np.meshgrid(np.arange(12), np.arange(10), indexing="ij")
+    def dft(A):
+        out = np.zeros((12, 10), complex)
+        for y in range(12):
+            for x in range(10):
+                out += A[y, x] * np.exp(-2j * np.pi * (ky * y / 12 + kx * x / 10))
+        return out
+    brute = ((np.log(np.abs(dft(I)) + eps) - np.log(np.abs(dft(T)) + eps)) ** 2).sum()
+    assert abs(brute - o.spectral_loss(I, T, eps)) < 1e-9
+    # gradient against central differences of the loss, pixel by pixel
+    g = o.spectral_loss_grad(I, T, eps)
+    h = 1e-6
+    for (y, x) in ((0, 0), (3, 7), (11, 9), (6, 2)):
+        up, dn_ = I.copy(), I.copy()
+        up[y, x] += h; dn_[y, x] -= h
+        fd = (o.spectral_loss(up, T, eps) - o.spectral_loss(dn_, T, eps)) / (2 * h)
+        assert abs(g[y, x] - fd) < 1e-5 * max(1.0, abs(fd))
