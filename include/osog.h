@@ -196,6 +196,14 @@ int osog_render_height(osog_ctx* ctx, const osog_particles* p, int64_t N, const 
  * top surface in um (0 where d_top_id is -1).  Runs the binning, then one fp64 evaluation per listed (particle, pixel). */
 int osog_render_gbuffer(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, int32_t* d_top_id, float* d_depth);
 
+/* osog_render_gbuffer plus the ANALYTIC normal of the visible surface: d_normal is DEVICE
+ * float [B, H, W, 2] = (dz/dx, dz/dy) of the owner's top surface at the pixel centre (0, 0 where d_top_id is -1), straight from
+ * the ray test: -n_x / n_z, -n_y / n_z of the active exit plane of a prism, the derivative of the quadric's upper root for an
+ * ellipsoid (it grows like 1 / sqrt(w) towards the outline).  The surface normal is <-dz/dx, -dz/dy, 1> (unnormalised).
+ * Unlike the finite differences of osog_render_height (reading A25) this is the slope of ONE body, the visible one. */
+int osog_render_gbuffer_normals(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, int32_t* d_top_id,
+                                float* d_depth, float* d_normal);
+
 /* Adjoint of the optics stage: d_gI = dL/dI (DEVICE float [B, H, W], read only) is an upstream
  * gradient of the coherent intensity of osog_render_intensity (noise-free part); d_gopd (DEVICE float [B, H, W], overwritten)
  * receives dL/dOPD = (4 pi / lambda) Im(g_U conj(U)), g_U = F^-1{conj(P) F{d_gI V}}, V = U * h_obj.  Runs the hot path for U,

@@ -56,8 +56,10 @@ def _lib():
             ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int64)]
         lib.osog_oracle_count_covered.restype = None
         lib.osog_oracle_render_gbuffer.argtypes = [ctypes.c_int64] + [fp] * 11 + [u8p] + [
-            ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int32), dp]
+            ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int32), dp, dp]
         lib.osog_oracle_render_gbuffer.restype = None
+        lib.osog_oracle_top_slope.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double, dp]
+        lib.osog_oracle_top_slope.restype = ctypes.c_int
         lib.osog_oracle_chord.argtypes = [ctypes.c_uint8, dp, dp, ctypes.c_double, ctypes.c_double, dp, dp]
         lib.osog_oracle_chord.restype = ctypes.c_int
         lib.osog_oracle_backward_np.argtypes = [ctypes.c_int64] + [fp] * 10 + [u8p] + [
@@ -155,25 +157,42 @@ def chord(kind, q, dims, dx, dy):
     return (ze.value, zx.value) if ok else None
 
 
-def render_gbuffer(scene, mode="bcircle"):
+def top_slope(kind, q, dims, dx, dy):
+    """(dz/dx, dz/dy) of the body's top surface at the offset (dx, dy) from its centre, or None (no positive chord)."""
+    R = np.ascontiguousarray(rot_from_quat(q), dtype=np.float64).reshape(9)
+    d = np.ascontiguousarray(dims, dtype=np.float64)
+    g = np.zeros(2, dtype=np.float64)
+    ok = _lib().osog_oracle_top_slope(int(kind), _ptr(R, ctypes.c_double), _ptr(d, ctypes.c_double), float(dx), float(dy),
+                                      _ptr(g, ctypes.c_double))
+    return (float(g[0]), float(g[1])) if ok else None
+
+
+def render_gbuffer(scene, mode="bcircle", normals=False):
     """(top_id int32 [B, H, W], depth float64 [B, H, W]) of a workloads.Scene: index (within the frame's particles,
-    i.e. relative to frame_start[b]) and top-surface height of the top-most particle above every pixel (reading A24)."""
+    i.e. relative to frame_start[b]) and top-surface height of the top-most particle above every pixel (reading A24).
+    normals=True adds the slope map float64 [B, H, W, 2] = (dz/dx, dz/dy) of the owner's top surface (0 where none): the
+    analytic height gradient of the visible surface, whose normal is <-dz/dx, -dz/dy, 1>."""
     fs = scene.frame_start
     f = ctypes.c_float
-    ids, deps = [], []
+    ids, deps, nrm = [], [], []
     for b in range(scene.B):
         lo, hi = int(fs[b]), int(fs[b + 1])
         a = {k: np.ascontiguousarray(scene.cols[k][lo:hi], dtype=np.float32) for k in _COLS + ("cz",)}
         kind = np.ascontiguousarray(scene.cols["kind"][lo:hi], dtype=np.uint8)
         tid = np.empty((scene.H, scene.W), dtype=np.int32)
         dep = np.empty((scene.H, scene.W), dtype=np.float64)
+        nm = np.zeros((scene.H, scene.W, 2), dtype=np.float64) if normals else None
         _lib().osog_oracle_render_gbuffer(
             hi - lo, _ptr(a["cx"], f), _ptr(a["cy"], f), _ptr(a["cz"], f), _ptr(a["qw"], f), _ptr(a["qx"], f),
             _ptr(a["qy"], f), _ptr(a["qz"], f), _ptr(a["d0"], f), _ptr(a["d1"], f), _ptr(a["d2"], f), _ptr(a["n_p"], f),
             _ptr(kind, ctypes.c_uint8), scene.H, scene.W, float(scene.pitch_um),
-            {"full": 0, "bcircle": 1}[mode], _ptr(tid, ctypes.c_int32), _ptr(dep, ctypes.c_double))
+            {"full": 0, "bcircle": 1}[mode], _ptr(tid, ctypes.c_int32), _ptr(dep, ctypes.c_double),
+            _ptr(nm, ctypes.c_double) if normals else None)
         ids.append(tid)
         deps.append(dep)
+        nrm.append(nm)
+    if normals:
+        return np.stack(ids), np.stack(deps), np.stack(nrm)
     return np.stack(ids), np.stack(deps)
 
 

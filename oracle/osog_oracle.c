@@ -279,6 +279,44 @@ int osog_oracle_chord(uint8_t kind, const double R[9], const double dims[3], dou
     return 1;
 }
 
+/* Slope (dz/dx, dz/dy) of the body's TOP surface at (dx, dy): the analytic height gradient of the visible surface that "falls
+ * out of the same ray test" (N = <-dh/dx, -dh/dy, 1>).  Ellipsoid: the surface is the level
+ * set F(p) = p^T M p = 1; at the exit point p = (dx, dy, z_exit) its normal is grad F = 2 M p, so dz/dx = -(M p)_x / (M p)_z.
+ * Prism: the active exit plane n . p = b gives dz/dx = -n_x / n_z.  Returns 0 (and leaves slope untouched) where the chord
+ * is empty. */
+int osog_oracle_top_slope(uint8_t kind, const double R[9], const double dims[3], double dx, double dy, double slope[2])
+{
+    double ze, zx;
+    if (!osog_oracle_chord(kind, R, dims, dx, dy, &ze, &zx)) return 0;
+    if (kind == 0) {
+        const double D[3] = { 1.0 / (dims[0] * dims[0]), 1.0 / (dims[1] * dims[1]), 1.0 / (dims[2] * dims[2]) };
+        double M[9];
+        for (int r = 0; r < 3; ++r)
+            for (int s = 0; s < 3; ++s) {
+                double acc = 0.0;
+                for (int k = 0; k < 3; ++k) acc += R[3 * r + k] * D[k] * R[3 * s + k];
+                M[3 * r + s] = acc;
+            }
+        const double p[3] = { dx, dy, zx };
+        double g[3];
+        for (int r = 0; r < 3; ++r) g[r] = M[3 * r] * p[0] + M[3 * r + 1] * p[1] + M[3 * r + 2] * p[2];
+        slope[0] = -g[0] / g[2];
+        slope[1] = -g[1] / g[2];
+        return 1;
+    }
+    double Aw[OSOG_ORACLE_MAX_PLANES][3], bb[OSOG_ORACLE_MAX_PLANES];
+    const int M = prism_world_planes(R, dims[0], dims[1], dims[2], Aw, bb);
+    double exit_ = INFINITY;
+    int ke = -1;
+    for (int k = 0; k < M; ++k) {
+        const double nz = Aw[k][2];
+        if (nz > 0.0) { const double z = (bb[k] - Aw[k][0] * dx - Aw[k][1] * dy) / nz; if (z < exit_) { exit_ = z; ke = k; } }
+    }
+    slope[0] = -Aw[ke][0] / Aw[ke][2];
+    slope[1] = -Aw[ke][1] / Aw[ke][2];
+    return 1;
+}
+
 /* Depth and instance-id maps of one frame (reading A24): for every pixel, among the particles whose chord there has
  * positive length, the one whose top surface  cz[n] + z_exit  is highest (+z points at the objective); ties go to the
  * smallest index.  top_id[i*W+j] = that particle's index (-1: no particle), depth[i*W+j] = the height of its top
@@ -288,12 +326,15 @@ void osog_oracle_render_gbuffer(int64_t N,
                                 const float *qw, const float *qx, const float *qy, const float *qz,
                                 const float *d0, const float *d1, const float *d2,
                                 const float *n_p, const uint8_t *kind,
-                                int H, int W, double pitch, int mode, int32_t *top_id, double *depth)
+                                int H, int W, double pitch, int mode, int32_t *top_id, double *depth, double *normal)
 {
 #pragma omp parallel for schedule(dynamic, 4)
     for (int i = 0; i < H; ++i) {
         const double y = (i + 0.5) * pitch;
-        for (int j = 0; j < W; ++j) { top_id[(size_t)i * W + j] = -1; depth[(size_t)i * W + j] = 0.0; }
+        for (int j = 0; j < W; ++j) {
+            top_id[(size_t)i * W + j] = -1; depth[(size_t)i * W + j] = 0.0;
+            if (normal != NULL) normal[2 * ((size_t)i * W + j)] = normal[2 * ((size_t)i * W + j) + 1] = 0.0;
+        }
         for (int64_t n = 0; n < N; ++n) {
             if (!osog_oracle_particle_valid(cx[n], cy[n], qw[n], qx[n], qy[n], qz[n],
                                             d0[n], d1[n], d2[n], n_p[n], kind[n])) continue;
@@ -317,7 +358,10 @@ void osog_oracle_render_gbuffer(int64_t N,
                 if (!osog_oracle_chord(kind[n], R, dims, dx, dy, &ze, &zx)) continue;
                 const double top = zc + zx;
                 const size_t px = (size_t)i * W + j;
-                if (top_id[px] < 0 || top > depth[px]) { top_id[px] = (int32_t)n; depth[px] = top; }
+                if (top_id[px] < 0 || top > depth[px]) {
+                    top_id[px] = (int32_t)n; depth[px] = top;
+                    if (normal != NULL) osog_oracle_top_slope(kind[n], R, dims, dx, dy, normal + 2 * px);   /* slope of the owner's top */
+                }
             }
         }
     }

@@ -89,6 +89,8 @@ def lib():
     L.osog_backward_params.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_backward_centre.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_gbuffer.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
+    L.osog_render_gbuffer_normals.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p,
+                                              C.c_void_p]
     L.osog_render_height.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p,
                                      C.c_void_p]
     L.osog_debug_recompose_field.argtypes = [ctx, C.c_void_p]
@@ -109,7 +111,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_brightfield", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_params", "osog_spectral_loss", "osog_backward_intensity", "osog_debug_recompose_field", "osog_debug_check_guards", "osog_debug_poisson", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_brightfield", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_gbuffer_normals", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_params", "osog_spectral_loss", "osog_backward_intensity", "osog_debug_recompose_field", "osog_debug_check_guards", "osog_debug_poisson", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -323,10 +325,16 @@ class Context:
             raise OsogError(r, "osog_spectral_loss")
         return loss, g
 
-    def render_gbuffer(self, p: Particles, o):
-        """(int32 [B, H, W] instance id of the top-most particle, float32 [B, H, W] height of its top surface)."""
+    def render_gbuffer(self, p: Particles, o, normals=False):
+        """(int32 [B, H, W] instance id of the top-most particle, float32 [B, H, W] height of its top surface); with
+        normals=True also float32 [B, H, W, 2], the analytic slope (dz/dx, dz/dy) of that surface (osog_render_gbuffer_normals)."""
         tid = self.torch.empty((o.B, self.H, self.W), dtype=self.torch.int32, device=self.device)
         dep = self.torch.empty((o.B, self.H, self.W), dtype=self.torch.float32, device=self.device)
+        if normals:
+            nrm = self._out(o.B, 2)
+            self._done(lib().osog_render_gbuffer_normals(self._ctx, C.byref(p.c), p.N, C.byref(o), tid.data_ptr(), dep.data_ptr(),
+                                                         nrm.data_ptr()), "osog_render_gbuffer_normals")
+            return tid, dep, nrm
         self._done(lib().osog_render_gbuffer(self._ctx, C.byref(p.c), p.N, C.byref(o), tid.data_ptr(), dep.data_ptr()),
                    "osog_render_gbuffer")
         return tid, dep

@@ -760,11 +760,16 @@ __global__ void __launch_bounds__(256) k_compose_atomic(const float* __restrict_
 // warp walks the tile's sorted list, skips the entries whose sub-tile mask bit is clear, and for the others evaluates the
 // top of the chord in fp64 straight from the record: the decision "which particle is on top" is taken in the precision
 // the oracle takes it in.  Ascending list order and a strict comparison give ties to the smallest index.
+// NORMAL: also the slope (dz/dx, dz/dy) of the owner's top surface (the analytic height gradient of the visible surface,
+// PAPER.md:76, 92): the active exit plane's -n_x / n_z = -U / p for a prism, the derivative of the upper root of the quadric
+// for an ellipsoid: d/ddj (Z0 + Zx dj + Zy di + T0 sqrt(w) / 2) / p.
+template <bool NORMAL>
 __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* __restrict__ recs, const uint32_t* __restrict__ offset,
                                                                 const uint32_t* __restrict__ list, const uint16_t* __restrict__ meta,
                                                                 const DeviceStatus* __restrict__ status,
                                                                 const int32_t* __restrict__ frame_start, int ntx, int nty, int H,
-                                                                int W, int32_t* __restrict__ top_id, float* __restrict__ depth)
+                                                                int W, double inv_pitch, int32_t* __restrict__ top_id,
+                                                                float* __restrict__ depth, float2* __restrict__ normal)
 {
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int tile = blockIdx.x, tpf = ntx * nty;
@@ -778,6 +783,7 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
     const uint32_t first = frame_start != nullptr ? (uint32_t)frame_start[b] : 0u;
     double best[4] = {0.0, 0.0, 0.0, 0.0};
     int32_t who[4] = {-1, -1, -1, -1};
+    float2 slope[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
     float floor_all = __int_as_float(0xff800000);                // -inf: nothing can be skipped yet
     for (uint32_t k = 0; k < L; ++k) {
         if (((gmeta[k] >> wid) & 1u) == 0u) continue;           // warp-uniform
@@ -794,6 +800,7 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
         const double di = (double)(i - h3.y), dj0 = (double)(j - h3.x);
         double zx[4];
         bool hit[4];
+        double sxs[4] = {0.0, 0.0, 0.0, 0.0}, sys[4] = {0.0, 0.0, 0.0, 0.0};    // slope of this particle's top (NORMAL only)
         if (flags & kFlagPrism) {
             // slab by slab for the lane's four pixels: coefficients loaded and the row term formed once per slab
             const uint32_t vmask = flags >> 16;
@@ -813,6 +820,7 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
                     for (int q = 0; q < 4; ++q) {
                         const double m = uv.x * (dj0 + (double)q);
                         const double e = cx - m, n = cn - m;
+                        if (NORMAL && e < ex[q]) { sxs[q] = -uv.x; sys[q] = -uv.y; }    // the active exit plane so far
                         ex[q] = e < ex[q] ? e : ex[q];
                         en[q] = n > en[q] ? n : en[q];
                     }
@@ -826,13 +834,22 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
                 const double dj = dj0 + (double)q;
                 const double w = c[5] - fma(fma(c[0], dj, fma(c[1], di, c[3])), dj, fma(c[2], di, c[4]) * di);
                 hit[q] = w > 0.0;
-                zx[q] = fma(c[9], dj, fma(c[10], di, c[8])) + 0.5 * c[11] * sqrt(fmax(w, 0.0));
+                const double sq = sqrt(fmax(w, 0.0));
+                zx[q] = fma(c[9], dj, fma(c[10], di, c[8])) + 0.5 * c[11] * sq;
+                if (NORMAL && hit[q]) {
+                    const double k4 = 0.25 * c[11] / sq;            // d(T0 sqrt(w) / 2) = T0 dw / (4 sqrt(w))
+                    sxs[q] = c[9] - k4 * (2.0 * c[0] * dj + c[1] * di + c[3]);
+                    sys[q] = c[10] - k4 * (c[1] * dj + 2.0 * c[2] * di + c[4]);
+                }
             }
         }
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const double top = (double)czf + zx[q];
-            if (hit[q] && (who[q] < 0 || top > best[q])) { best[q] = top; who[q] = (int32_t)(pid - first); }
+            if (hit[q] && (who[q] < 0 || top > best[q])) {
+                best[q] = top; who[q] = (int32_t)(pid - first);
+                if (NORMAL) slope[q] = make_float2((float)(sxs[q] * inv_pitch), (float)(sys[q] * inv_pitch));
+            }
         }
         // lowest top over the warp's 128 pixels, rounded down (-inf while some pixel has no owner)
         float lo = __int_as_float(0x7f800000);
@@ -849,16 +866,24 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
         if (j + q < W) {
             top_id[row + j + q] = who[q];
             depth[row + j + q] = who[q] < 0 ? 0.0f : (float)best[q];
+            if (NORMAL) normal[row + j + q] = who[q] < 0 ? make_float2(0.f, 0.f) : slope[q];
         }
 }
 
-cudaError_t launch_gbuffer(osog_ctx* c, int B, const int32_t* d_frame_start, int32_t* d_top_id, float* d_depth)
+cudaError_t launch_gbuffer(osog_ctx* c, int B, const int32_t* d_frame_start, double pitch, int32_t* d_top_id, float* d_depth,
+                           float* d_normal)
 {
     const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
     const cudaError_t e = launch_sort_cull(c, grid, false);
     if (e != cudaSuccess) return e;
-    k_gbuffer_tile<<<grid, kComposeThreads, 0, c->stream>>>(c->rec, c->offset, c->list, c->meta, c->status + c->status_idx,
-                                                           d_frame_start, c->ntx, c->nty, c->H, c->W, d_top_id, d_depth);
+    if (d_normal != nullptr)
+        k_gbuffer_tile<true><<<grid, kComposeThreads, 0, c->stream>>>(c->rec, c->offset, c->list, c->meta, c->status + c->status_idx,
+                                                                     d_frame_start, c->ntx, c->nty, c->H, c->W, 1.0 / pitch, d_top_id,
+                                                                     d_depth, reinterpret_cast<float2*>(d_normal));
+    else
+        k_gbuffer_tile<false><<<grid, kComposeThreads, 0, c->stream>>>(c->rec, c->offset, c->list, c->meta, c->status + c->status_idx,
+                                                                      d_frame_start, c->ntx, c->nty, c->H, c->W, 1.0 / pitch, d_top_id,
+                                                                      d_depth, nullptr);
     return cudaGetLastError();
 }
 

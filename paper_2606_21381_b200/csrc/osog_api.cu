@@ -431,19 +431,32 @@ int osog_render_height(osog_ctx* c, const osog_particles* p, int64_t N, const os
     return OSOG_OK;
 }
 
-int osog_render_gbuffer(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, int32_t* d_top_id, float* d_depth)
+static int gbuffer_common(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, int32_t* d_top_id, float* d_depth,
+                          float* d_normal)
 {
-    if (!d_top_id || !aligned16(d_top_id)) return OSOG_EINVAL;
+    if (!d_top_id || !aligned16(d_top_id) || (d_normal && !aligned16(d_normal))) return OSOG_EINVAL;
     const int r = check_call(c, p, N, o, d_depth);
     if (r != OSOG_OK) return r;
     if (p->cz != nullptr && (reinterpret_cast<uintptr_t>(p->cz) & 3u)) return OSOG_EINVAL;
     DeviceGuard g(c->device);
     cudaError_t e = launch_binning(c, p, N, o);
     if (e != cudaSuccess) return cuda_fail(c, e);
-    e = launch_gbuffer(c, o->B, o->B > 1 ? p->frame_start : nullptr, d_top_id, d_depth);
+    e = launch_gbuffer(c, o->B, o->B > 1 ? p->frame_start : nullptr, o->pitch_um, d_top_id, d_depth, d_normal);
     if (e != cudaSuccess) return cuda_fail(c, e);
     c->scratch_dirty = false;
     return OSOG_OK;
+}
+
+int osog_render_gbuffer(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, int32_t* d_top_id, float* d_depth)
+{
+    return gbuffer_common(c, p, N, o, d_top_id, d_depth, nullptr);
+}
+
+int osog_render_gbuffer_normals(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, int32_t* d_top_id,
+                                float* d_depth, float* d_normal)
+{
+    if (!d_normal) return OSOG_EINVAL;
+    return gbuffer_common(c, p, N, o, d_top_id, d_depth, d_normal);
 }
 
 int osog_backward_intensity(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gI, float* d_gopd)

@@ -133,7 +133,8 @@ cudaError_t launch_backward_np(osog_ctx* c, long long N, const float* d_gopd, fl
 cudaError_t launch_backward_centre(osog_ctx* c, long long N, double pitch, const float* d_gopd, float* d_gc);
 cudaError_t launch_backward_params(osog_ctx* c, const osog_particles* p, long long N, double pitch, double n_medium,
                                    const float* d_gopd, float* d_gpar);
-cudaError_t launch_gbuffer(osog_ctx* c, int B, const int32_t* d_frame_start, int32_t* d_top_id, float* d_depth);
+cudaError_t launch_gbuffer(osog_ctx* c, int B, const int32_t* d_frame_start, double pitch, int32_t* d_top_id, float* d_depth,
+                           float* d_normal);
 // optics.cu
 cudaError_t launch_pupil(osog_ctx* c, int B, float2* spec, double pitch, bool defocus);
 cudaError_t launch_pupil_fill(osog_ctx* c, int B, float2* spec, double pitch, bool defocus);

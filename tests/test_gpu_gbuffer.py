@@ -159,3 +159,32 @@ def test_gbuffer_ragged_frame_prisms_with_vertical_faces(og, o):
                 d1=[3.3, 4.1, 2.9, 2.0], d2=[1.0, 0.8, 0.6, 1.2], n_p=[1.45, 1.40, 1.42, 1.4],
                 kind=np.array([1, 1, 1, 0], np.uint8))
     check(og, o, make_scene("vertical_g", 100, 130, cols))
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_gbuffer_analytic_normals_match_oracle(og, o, k):
+    """Slope (dz/dx, dz/dy) of the visible particle's top surface (osog_render_gbuffer_normals; NEXT-2: the analytic
+    normal that falls out of the ray test).  Compared where both sides name the same owner; bar: float32 rounding of a
+    float64 evaluation, relative to 1 + |slope| (the ellipsoid's slope grows like 1 / sqrt(w) at the outline, where the two
+    float64 formulas for w differ by ~1e-9 relative: pixels with an almost empty chord get the proportionally wider bar)."""
+    sc = with_heights(make_config(k), seed=60 + k)
+    ctx = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B)
+    P, opt = og.Particles.from_scene(sc), og.optics_from_scene(sc)
+    tid, dep, nrm = ctx.render_gbuffer(P, opt, normals=True)
+    t2, d2 = ctx.render_gbuffer(P, opt)
+    import torch
+    assert torch.equal(tid, t2) and torch.equal(dep, d2)          # the maps do not depend on asking for normals
+    tid, nrm = tid.cpu().numpy(), nrm.cpu().numpy().astype(np.float64)
+    ctx.close()
+    rid, rdep, rn = o.render_gbuffer(sc, normals=True)
+    same = (tid == rid) & (rid >= 0)
+    assert same.sum() > 0.99 * (rid >= 0).sum()
+    assert np.all(nrm[tid < 0] == 0.0)
+    err = np.abs(nrm - rn)[same]
+    mag = 1.0 + np.abs(rn)[same]
+    rel = err / mag
+    print(f"cfg {k}: normals max rel err {rel.max():.2e}, slopes up to {np.abs(rn)[same].max():.1f}")
+    assert np.percentile(rel, 99.9) <= 1e-6
+    # the few pixels beyond that are outline pixels of ellipsoids: |slope| huge, error a fixed fraction of slope^3 * 1e-9
+    wild = rel > 1e-6
+    assert np.all(np.abs(rn)[same][wild] > 30.0) and np.all(rel[wild] <= 1e-9 * np.abs(rn)[same][wild] ** 2 + 1e-6)

@@ -141,3 +141,59 @@ def test_G5_overlap_ties_permutation_and_modes():
     # coverage agrees with the OPD frame: a pixel has an owner iff some particle has positive thickness there
     assert np.array_equal(tid[0] >= 0, o.render_opd(sc4)[0] != 0.0)
     assert len(np.unique(tid)) > 10
+
+
+# ---- analytic slope of the visible surface ("the analytic height gradient / normal that falls out of the
+# same ray test") ---------------------------------------------------------------------------------------------
+def test_G6_top_slope_closed_forms_and_differenced_chord():
+    # sphere: top z = sqrt(R^2 - r^2), dz/dx = -dx / z
+    R, dx, dy = 2.0, 0.9, -0.5
+    z = np.sqrt(R * R - dx * dx - dy * dy)
+    sx, sy = o.top_slope(0, [1, 0, 0, 0], [R, R, R], dx, dy)
+    assert abs(sx + dx / z) < 1e-13 and abs(sy + dy / z) < 1e-13
+    assert o.top_slope(0, [1, 0, 0, 0], [R, R, R], 2.5, 0.0) is None
+    # prism, identity rotation: top = cap faces z = L/2 + hc (1 - |x| / (s/2)) on the side where |x| > |y|: slope -+ 2 hc / s
+    s_, L, hc = 2.0, 3.0, 0.8
+    sx, sy = o.top_slope(1, [1, 0, 0, 0], [s_, L, hc], 0.6, 0.2)
+    assert abs(sx + 2 * hc / s_) < 1e-13 and abs(sy) < 1e-13
+    sx, sy = o.top_slope(1, [1, 0, 0, 0], [s_, L, hc], 0.1, -0.7)
+    assert abs(sx) < 1e-13 and abs(sy - 2 * hc / s_) < 1e-13
+    # any rotation, both kinds: central differences of the pinned chord's z_exit (G1-G4) at interior points
+    rng = np.random.default_rng(6)
+    h = 1e-6
+    checked = 0
+    for trial in range(80):
+        kind = trial % 2
+        q = rng.standard_normal(4); q /= np.linalg.norm(q)
+        dims = rng.uniform(0.8, 3.0, 3)
+        dx, dy = rng.uniform(-1.0, 1.0, 2)
+        c0 = o.chord(kind, q, dims, dx, dy)
+        if c0 is None or c0[1] - c0[0] < 0.3:
+            continue
+        zs = [o.chord(kind, q, dims, dx + a, dy + b)[1] for a, b in ((h, 0), (-h, 0), (0, h), (0, -h))]
+        if abs(zs[0] + zs[1] - 2 * c0[1]) > 1e-9 or abs(zs[2] + zs[3] - 2 * c0[1]) > 1e-9:      # a face edge inside the stencil (prism)
+            if kind == 1:
+                continue
+        sx, sy = o.top_slope(kind, q, dims, dx, dy)
+        assert abs(sx - (zs[0] - zs[1]) / (2 * h)) < 2e-6 * max(1, abs(sx)) and abs(sy - (zs[2] - zs[3]) / (2 * h)) < 2e-6 * max(1, abs(sy))
+        checked += 1
+    assert checked > 40
+
+
+def test_G7_normal_map_belongs_to_the_owner():
+    from workloads import make_config
+    sc = make_config(4, n_override=60)
+    from dataclasses import replace
+    for k in ("cx", "cy"):
+        sc.cols[k][:] = (sc.cols[k] / 16.0).astype(np.float32)
+    sc = replace(sc, H=128, W=128)
+    tid, dep, nrm = o.render_gbuffer(sc, normals=True)
+    t2, d2 = o.render_gbuffer(sc)
+    assert np.array_equal(tid, t2) and np.array_equal(dep, d2)
+    assert np.all(nrm[tid < 0] == 0.0)
+    c = sc.cols
+    for (i, j) in np.argwhere(tid[0] >= 0)[::97]:
+        n = int(tid[0, i, j])
+        want = o.top_slope(int(c["kind"][n]), [float(c[k][n]) for k in ("qw", "qx", "qy", "qz")], [float(c[k][n]) for k in ("d0", "d1", "d2")],
+                           (j + 0.5) * sc.pitch_um - float(c["cx"][n]), (i + 0.5) * sc.pitch_um - float(c["cy"][n]))
+        assert np.allclose(nrm[0, i, j], want, rtol=0, atol=0)
