@@ -43,9 +43,10 @@
 extern "C" {
 #endif
 
-#define OSOG_API_VERSION 4   /* 2: osog_optics.defocus_um, osog_dic, osog_render_dic, osog_field_to_dic
+#define OSOG_API_VERSION 5   /* 2: osog_optics.defocus_um, osog_dic, osog_render_dic, osog_field_to_dic
                                 3: max_pairs is a TOTAL capacity (device scan + CSR lists), osog_status reports the exact need
-                                4: osog_optics.shot_noise_photons (Poisson shot noise), osog_debug_poisson, osog_debug_check_guards */
+                                4: osog_optics.shot_noise_photons (Poisson shot noise), osog_debug_poisson, osog_debug_check_guards
+                                5: osog_optics.topography_amplitude (micro-topography), brightfield, backward_params, spectral loss */
 
 enum {
     OSOG_OK = 0,
@@ -104,6 +105,10 @@ typedef struct {
                                          Poisson(S max(I, 0)) / S (before the read noise), one draw per (seed, frame, pixel)
                                          from the Philox stream with counter (pixel, frame, 1, block): inversion below
                                          lambda = 10, transformed rejection (PTRS) above (reading A26); 0 = no shot noise  */
+    double   topography_amplitude;    /* procedural micro-topography (reading A29), every render call: each
+                                         particle's thickness at pixel (i, j) is multiplied by 1 + a * eta[b, i, j], eta ~ N(0, 1)
+                                         white per pixel from the Philox stream with counter (pixel, frame, 2, 0) of `seed`, so
+                                         OPD -> OPD (1 + a eta) before the phase is formed; 0 = smooth bodies                 */
 } osog_optics;
 
 /* Differential interference contrast, Eq. 5.  struct_size = sizeof(osog_dic). */

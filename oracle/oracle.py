@@ -24,6 +24,7 @@ Pieces, each following the passage it cites (line numbers are /root/reference/PA
   render_height / height_gradient / height_laplacian   h, grad h, lap h of the G-buffer :76, :92, :96-99, A25
   fresnel_transmittance / brightfield_amplitude / render_brightfield   Eq. 4       :94-99, A27
   shot_uniforms / poisson_counts / shot_noise          Poisson shot noise          :126, A26
+  topography_factor                                    micro-topography of the height map :74, A29
 
 Every reading of the paper taken here (units, pixel centres, quaternion convention, pupil edge,
 FFT normalisation, noise model ...) is listed in DESIGN.md section 3.  Pins: tests/test_oracle_*.py.
@@ -352,11 +353,21 @@ def count_covered(scene, mode="bcircle"):
     return int(tot[0]), int(tot[1])
 
 
+def topography_factor(scene, b) -> np.ndarray:
+    """Micro-topography of PAPER.md:74 (reading A29): the factor 1 + a eta[i, j] that multiplies every particle's thickness at
+    pixel (i, j) of frame b; eta ~ N(0, 1) white per pixel, Box-Muller on the Philox stream with counter (pixel, frame, 2, 0)
+    (the read noise uses word 2 = 0, the shot noise 1); a = scene.topography_amplitude (0: smooth bodies, factor 1)."""
+    a = float(getattr(scene, "topography_amplitude", 0.0))
+    if a == 0.0:
+        return np.ones((scene.H, scene.W), dtype=np.float64)
+    return 1.0 + a * _stream_normal(scene.seed, b, scene.H, scene.W, 2)
+
+
 def render_opd(scene, mode="bcircle") -> np.ndarray:
-    """OPD [B, H, W] float64 for a workloads.Scene."""
+    """OPD [B, H, W] float64 for a workloads.Scene (with the micro-topography factor of the scene, if any)."""
     fs = scene.frame_start
     return np.stack([render_opd_frame(scene.cols, int(fs[b]), int(fs[b + 1]), scene.H, scene.W,
-                                      scene.pitch_um, scene.n_medium, mode) for b in range(scene.B)])
+                                      scene.pitch_um, scene.n_medium, mode) * topography_factor(scene, b) for b in range(scene.B)])
 
 
 # --------------------------------------------------------------------------------------------
@@ -491,10 +502,16 @@ def read_noise(seed, frame, H, W) -> np.ndarray:
     """Standard normal z[i, j] for one frame (reading A13): Philox key = (seed low 32, seed high 32),
     counter = (pixel = i W + j, frame, 0, 0); u1 = (r0 + 1) 2^-32 in (0, 1], u2 = r1 2^-32 in [0, 1);
     z = sqrt(-2 ln u1) cos(2 pi u2) (Box-Muller)."""
+    return _stream_normal(seed, frame, H, W, 0)
+
+
+def _stream_normal(seed, frame, H, W, stream) -> np.ndarray:
+    """Box-Muller normals of the Philox stream with counter (pixel, frame, stream, 0)."""
     pix = np.arange(H * W, dtype=np.uint64)
     ctr = np.zeros((H * W, 4), dtype=np.uint64)
     ctr[:, 0] = pix
     ctr[:, 1] = np.uint64(frame)
+    ctr[:, 2] = np.uint64(stream)
     r = philox4x32_10(ctr, (seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF))
     u1 = (r[:, 0].astype(np.float64) + 1.0) * 2.0 ** -32
     u2 = r[:, 1].astype(np.float64) * 2.0 ** -32
@@ -747,7 +764,7 @@ def render_height(scene, mode="bcircle") -> np.ndarray:
     ones = dict(scene.cols)
     ones["n_p"] = np.ones_like(scene.cols["n_p"])
     return np.stack([render_opd_frame(ones, int(fs[b]), int(fs[b + 1]), scene.H, scene.W, scene.pitch_um, 0.0, mode)
-                     for b in range(scene.B)])
+                     * topography_factor(scene, b) for b in range(scene.B)])
 
 
 def height_gradient(h, pitch):

@@ -35,7 +35,7 @@ class osog_optics(C.Structure):
                 ("lambda_um", C.POINTER(C.c_double)), ("NA", C.POINTER(C.c_double)),
                 ("tilt_x_rad", C.c_double), ("tilt_y_rad", C.c_double), ("read_noise_sigma", C.c_double),
                 ("seed", C.c_uint64), ("pupil_enabled", C.c_int32), ("defocus_um", C.c_double),
-                ("shot_noise_photons", C.c_double)]
+                ("shot_noise_photons", C.c_double), ("topography_amplitude", C.c_double)]
 
 
 class osog_dic(C.Structure):
@@ -153,7 +153,8 @@ class Particles:
 
 
 def make_optics(B, pitch_um, n_medium, lambda_um, NA=None, tilt_x_rad=0.0, tilt_y_rad=0.0,
-                read_noise_sigma=0.0, seed=0, pupil_enabled=True, defocus_um=0.0, shot_noise_photons=0.0):
+                read_noise_sigma=0.0, seed=0, pupil_enabled=True, defocus_um=0.0, shot_noise_photons=0.0,
+                topography_amplitude=0.0):
     """osog_optics plus the host arrays it points to (kept alive as attributes)."""
     o = osog_optics()
     o.struct_size = C.sizeof(osog_optics)
@@ -174,6 +175,7 @@ def make_optics(B, pitch_um, n_medium, lambda_um, NA=None, tilt_x_rad=0.0, tilt_
     o.pupil_enabled = 1 if pupil_enabled else 0
     o.defocus_um = float(defocus_um)
     o.shot_noise_photons = float(shot_noise_photons)
+    o.topography_amplitude = float(topography_amplitude)
     return o
 
 
@@ -194,7 +196,8 @@ def make_brightfield(n_particle, delta_mu_per_um=0.0, caustic_gain_um=0.0):
 def optics_from_scene(scene, pupil_enabled=True):
     return make_optics(scene.B, scene.pitch_um, scene.n_medium, scene.lambda_um, scene.NA, scene.tilt_x_rad,
                        scene.tilt_y_rad, scene.read_noise_sigma, scene.seed, pupil_enabled,
-                       getattr(scene, "defocus_um", 0.0), getattr(scene, "shot_noise_photons", 0.0))
+                       getattr(scene, "defocus_um", 0.0), getattr(scene, "shot_noise_photons", 0.0),
+                       getattr(scene, "topography_amplitude", 0.0))
 
 
 class Context:

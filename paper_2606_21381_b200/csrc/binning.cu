@@ -591,6 +591,8 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     c->last_N = N;
     c->last_frame_start = B > 1 ? p->frame_start : nullptr;
     c->last_has_ramp = -1;                           // set again by a call that runs the sort and a field-capable composition
+    c->last_topo = o->topography_amplitude;
+    c->last_seed = o->seed;
     cudaError_t e;
     // Invariant kept by the kernels themselves (no memset nodes in the steady state): the counter slot and the status
     // slot of this call are all zero on entry (cleared by the previous call's k_sort_cull, which works on the other

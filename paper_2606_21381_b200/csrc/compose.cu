@@ -31,6 +31,8 @@ struct ComposeArgs {
     float2* field;
     int H, W, ntx, nty;
     int ramp_y_on;
+    float topo_amp;              // micro-topography (reading A29): the height map is multiplied by 1 + topo_amp * eta(pixel); 0 = off
+    unsigned long long seed;
 };
 
 constexpr int kWarps = kComposeThreads / 32;
@@ -531,6 +533,13 @@ static cudaError_t launch_sort_cull(osog_ctx* c, unsigned grid, bool pdl)
     return e;
 }
 
+// Micro-topography (reading A29): every thickness at a pixel is multiplied by 1 + amp * eta, eta ~ N(0, 1) white per
+// pixel (Philox stream 2 of (seed, frame, pixel)), hence so is the OPD sum.  Out of line: it runs once per pixel, rarely.
+__device__ __noinline__ double topo_factor(unsigned long long seed, uint32_t frame, uint32_t pixel, float amp)
+{
+    return 1.0 + (double)(amp * philox_normal(seed, frame, pixel, 2u));
+}
+
 // ---- H5-H7: every warp is independent (no barrier, no shared list): it walks its tile's sorted list in batches of 32
 template <bool OPD, bool FIELD, bool RAMP>
 __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(const ComposeArgs a)
@@ -642,6 +651,11 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
 
     // ---- H6/H7: write-out straight from the registers ----------------------------------------------------------------------
     if (i >= a.H || j >= a.W) return;
+    if (a.topo_amp != 0.0f) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (j + k < a.W) acc[k] *= topo_factor(a.seed, (uint32_t)b, (uint32_t)(i * a.W + j + k), a.topo_amp);
+    }
     const size_t row = ((size_t)b * a.H + i) * a.W;
     const bool vec = ((a.W & 3) == 0);                           // then j + 3 < W and the row base is 16-byte aligned
     if (OPD) {
@@ -706,6 +720,7 @@ cudaError_t launch_compose(osog_ctx* c, int B, bool has_ramp, float* d_opd, floa
     a.opd = d_opd; a.field = d_field;
     a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
     a.ramp_y_on = 1;
+    a.topo_amp = (float)c->last_topo; a.seed = c->last_seed;
     const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
     if (sort_first) {
         const cudaError_t e = launch_sort_cull(c, grid, true);
@@ -1170,12 +1185,16 @@ __global__ void __launch_bounds__(256) k_backward_params(const ParamGradArgs a)
                 }
             }
         } else {
-            double nw[12][3], bb[12];
-#pragma unroll 1
+            // per plane: z_k(dx, dy) = zc - za dx - zb dy (planes with n_z != 0), sign of n_z; vertical planes: g = zc - za dx - zb dy >= 0
+            double zc[12], za[12], zb[12], nzk[12];
+#pragma unroll
             for (int k = 0; k < 12; ++k) {
-                double nb[3], dnb[3][3], db[3];
-                prism_plane(k, e[0], e[1], e[2], nb, &bb[k], dnb, db);
-                for (int r = 0; r < 3; ++r) nw[k][r] = R[3 * r] * nb[0] + R[3 * r + 1] * nb[1] + R[3 * r + 2] * nb[2];
+                double nb[3], bk, dnb[3][3], db[3];
+                prism_plane(k, e[0], e[1], e[2], nb, &bk, dnb, db);
+                const double nx = R[0] * nb[0] + R[1] * nb[1] + R[2] * nb[2], ny = R[3] * nb[0] + R[4] * nb[1] + R[5] * nb[2];
+                nzk[k] = R[6] * nb[0] + R[7] * nb[1] + R[8] * nb[2];
+                const double inz = nzk[k] != 0.0 ? 1.0 / nzk[k] : 1.0;
+                zc[k] = bk * inz; za[k] = nx * inz; zb[k] = ny * inz;
             }
             for (int q = lane; q < np; q += 32) {
                 const int i = i0 + q / bw, j = j0 + q % bw;
@@ -1183,19 +1202,22 @@ __global__ void __launch_bounds__(256) k_backward_params(const ParamGradArgs a)
                 double ex = 1.0e300, en = -1.0e300;
                 int ke = 0, kf = 0;
                 bool out = false;
-#pragma unroll 1
+#pragma unroll
                 for (int k = 0; k < 12; ++k) {
-                    const double gk = bb[k] - nw[k][0] * dx - nw[k][1] * dy, nz = nw[k][2];
-                    if (nz > 0.0) { const double zk = gk / nz; if (zk < ex) { ex = zk; ke = k; } }
-                    else if (nz < 0.0) { const double zk = gk / nz; if (zk > en) { en = zk; kf = k; } }
-                    else if (gk < 0.0) out = true;
+                    const double zk = zc[k] - za[k] * dx - zb[k] * dy;
+                    if (nzk[k] > 0.0) { if (zk < ex) { ex = zk; ke = k; } }
+                    else if (nzk[k] < 0.0) { if (zk > en) { en = zk; kf = k; } }
+                    else if (zk < 0.0) out = true;
                 }
                 if (out || !(ex - en > 0.0)) continue;
                 const double gv = (double)g[(size_t)i * a.W + j];
 #pragma unroll 1
                 for (int side = 0; side < 2; ++side) {
                     const int k = side ? kf : ke;
-                    const double zk = side ? en : ex, sgn = side ? -1.0 : 1.0, inz = 1.0 / nw[k][2];
+                    double nzv = nzk[0];
+#pragma unroll
+                    for (int kk = 1; kk < 12; ++kk) nzv = kk == k ? nzk[kk] : nzv;
+                    const double zk = side ? en : ex, sgn = side ? -1.0 : 1.0, inz = 1.0 / nzv;
                     double nb[3], bk, dnb[3][3], db[3];
                     prism_plane(k, e[0], e[1], e[2], nb, &bk, dnb, db);
 #pragma unroll

@@ -254,31 +254,10 @@ __global__ void __launch_bounds__(256) k_cmul(float2* __restrict__ a, const floa
     a[k] = make_float2((x.x * y.x - x.y * y.y) * scale, (x.x * y.y + x.y * y.x) * scale);
 }
 
-__device__ __forceinline__ void philox_round(uint32_t (&c)[4], uint32_t k0, uint32_t k1)
-{
-    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
-    const uint32_t hi0 = __umulhi(M0, c[0]), lo0 = M0 * c[0];
-    const uint32_t hi1 = __umulhi(M1, c[2]), lo1 = M1 * c[2];
-    const uint32_t n0 = hi1 ^ c[1] ^ k0, n2 = hi0 ^ c[3] ^ k1;
-    c[0] = n0; c[1] = lo1; c[2] = n2; c[3] = lo0;
-}
-
-// Standard normal for (seed, frame, pixel): Philox4x32-10, key = (seed low, seed high), counter = (pixel, frame, 0, 0);
-// u1 = (r0 + 1) 2^-32, u2 = r1 2^-32, z = sqrt(-2 ln u1) cos(2 pi u2)   (reading A13)
+// Standard normal of the read noise (reading A13): stream 0 of the shared Philox generator (osog_internal.cuh)
 __device__ __forceinline__ float read_noise_z(uint64_t seed, uint32_t frame, uint32_t pixel)
 {
-    uint32_t c[4] = {pixel, frame, 0u, 0u};
-    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
-#pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        philox_round(c, k0, k1);
-        k0 += 0x9E3779B9u;
-        k1 += 0xBB67AE85u;
-    }
-    const double u1 = ((double)c[0] + 1.0) * 2.3283064365386963e-10;
-    const float l = -2.0f * (float)log(u1);
-    const float u2 = (float)c[1] * 2.3283064365386963e-10f;
-    return sqrtf(l) * cospif(2.0f * u2);
+    return philox_normal(seed, frame, pixel, 0u);
 }
 
 // ---- Poisson shot noise ("P(lambda) + G(0, sigma^2)"; reading A26) ---------------------

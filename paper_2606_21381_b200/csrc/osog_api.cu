@@ -45,6 +45,7 @@ int check_call(const osog_ctx* c, const osog_particles* p, int64_t N, const osog
     for (int b = 0; b < o->B; ++b)
         if (!(o->lambda_um[b] > 0.0) || !(o->lambda_um[b] < 1.0e300)) return OSOG_EINVAL;
     if (!(fabs(o->tilt_x_rad) < 1.0e300) || !(fabs(o->tilt_y_rad) < 1.0e300)) return OSOG_EINVAL;
+    if (!(fabs(o->topography_amplitude) < 1.0e30)) return OSOG_EINVAL;
     if (N > 0) {
         const void* cols[] = {p->cx, p->cy, p->qw, p->qx, p->qy, p->qz, p->d0, p->d1, p->d2, p->n_p, p->kind};
         for (const void* q : cols)

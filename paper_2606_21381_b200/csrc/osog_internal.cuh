@@ -65,6 +65,8 @@ struct osog_ctx {
     int last_has_ramp;
     long long last_N;
     long long last_tiles;
+    double last_topo;               // micro-topography amplitude and seed of the last render call (reading A29)
+    unsigned long long last_seed;
     const int32_t* last_frame_start; // device pointer of the last call's frame_start (nullptr: one frame)
     // scratch (device)
     float* rec;                     // [max_particles][kRecWords]
@@ -121,12 +123,41 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
+// ---- counter-based random numbers (Philox4x32-10), shared by the sensor stage and the micro-topography of the write-out ----
+__device__ __forceinline__ void philox_round(uint32_t (&c)[4], uint32_t k0, uint32_t k1)
+{
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+    const uint32_t hi0 = __umulhi(M0, c[0]), lo0 = M0 * c[0];
+    const uint32_t hi1 = __umulhi(M1, c[2]), lo1 = M1 * c[2];
+    const uint32_t n0 = hi1 ^ c[1] ^ k0, n2 = hi0 ^ c[3] ^ k1;
+    c[0] = n0; c[1] = lo1; c[2] = n2; c[3] = lo0;
+}
+
+// Standard normal for (seed, frame, pixel) of stream `stream`: key = (seed low, seed high), counter = (pixel, frame, stream, 0);
+// u1 = (r0 + 1) 2^-32, u2 = r1 2^-32, z = sqrt(-2 ln u1) cos(2 pi u2)   (readings A13: stream 0 = read noise; A29: stream 2 =
+// micro-topography; stream 1 is the shot noise's)
+__device__ __forceinline__ float philox_normal(uint64_t seed, uint32_t frame, uint32_t pixel, uint32_t stream)
+{
+    uint32_t c[4] = {pixel, frame, stream, 0u};
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        philox_round(c, k0, k1);
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    const double u1 = ((double)c[0] + 1.0) * 2.3283064365386963e-10;
+    const float l = -2.0f * (float)log(u1);
+    const float u2 = (float)c[1] * 2.3283064365386963e-10f;
+    return sqrtf(l) * cospif(2.0f * u2);
+}
+
 // binning.cu
 cudaError_t upload_optics(osog_ctx* c, const osog_optics* o, OpticsChunk* first);
 cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, const osog_optics* o, float* d_obb = nullptr,
                            bool unit_dn = false);
 // compose.cu
-cudaError_t launch_compose(osog_ctx* c, int B, bool has_ramp, float* d_opd, float2* d_field, bool sort_first = true);
+cudaError_t launch_compose(osog_ctx* c, int B, bool has_ramp, float* d_opd, float2* d_field, bool sort_first = true);   // uses c->last_topo / c->last_seed
 cudaError_t launch_compose_atomic(osog_ctx* c, long long N, int B, float* d_opd);
 cudaError_t launch_compose_smem_atomic(osog_ctx* c, int B, float* d_opd);
 cudaError_t launch_backward_np(osog_ctx* c, long long N, const float* d_gopd, float* d_gnp);

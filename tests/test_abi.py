@@ -44,7 +44,7 @@ def test_struct_layouts_follow_the_header():
         assert fields == [f[0] for f in st._fields_], name
     assert C.sizeof(og.osog_config) == 48
     assert C.sizeof(og.osog_particles) == 8 + 13 * 8
-    assert C.sizeof(og.osog_optics) == 96
+    assert C.sizeof(og.osog_optics) == 104
     assert C.sizeof(og.osog_dic) == 24
 
 

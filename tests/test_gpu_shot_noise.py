@@ -81,3 +81,32 @@ def test_dic_with_shot_noise_and_argument_check(og, o):
         ctx.render_intensity(P, bad)
     assert e.value.code == og.OSOG_EINVAL
     ctx.close()
+
+
+@pytest.mark.parametrize("k,amp", [(2, 0.05), (4, 0.02), (5, 0.03)])
+def test_micro_topography_matches_oracle(og, o, k, amp):
+    """Micro-topography of the height map (reading A29): OPD, field, intensity and height with
+    topography_amplitude > 0 against the oracle.  Bars: the hot path's own (OPD 1e-5 + 1e-5 |o|, field / intensity 1e-4 mean I),
+    widened by what the float32 Box-Muller normal of the kernel allows: |d eta| <= 2e-6, so OPD gets + amp * 2e-6 * |o| and
+    the field + 2 pi / lambda times that."""
+    sc = replace(make_config(k), topography_amplitude=amp)
+    ctx = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B)
+    P, opt = og.Particles.from_scene(sc), og.optics_from_scene(sc)
+    opd = ctx.render_opd(P, opt).cpu().numpy().astype(np.float64)
+    U = ctx.render_field(P, opt).cpu().numpy().astype(np.complex128)
+    I = ctx.render_intensity(P, opt).cpu().numpy().astype(np.float64)
+    h = ctx.render_height(P, opt, grad=False, lap=False)[0].cpu().numpy().astype(np.float64)
+    smooth = ctx.render_opd(P, og.optics_from_scene(replace(sc, topography_amplitude=0.0))).cpu().numpy()
+    assert ctx.status()[0] == 0 and ctx.check_guards() == 0
+    ctx.close()
+    ref = o.render_opd(sc)
+    assert np.all(np.abs(opd - ref) <= 1e-5 + (1e-5 + 2e-6 * amp) * np.abs(ref)), float(np.abs(opd - ref).max())
+    assert not np.allclose(opd, smooth, atol=1e-4)                  # it really is a different surface
+    href = o.render_height(sc)
+    assert np.all(np.abs(h - href) <= 1e-5 + (1e-5 + 2e-6 * amp) * np.abs(href))
+    Uref = o.render_field(sc, opd=ref)
+    Iref = o.render_intensity(sc, U=Uref)
+    lam_min = float(np.min(sc.lambda_um))
+    tol = 1e-4 * Iref.mean() + 2 * np.pi / lam_min * 2e-6 * amp * float(np.abs(ref).max())
+    assert np.abs(U - Uref).max() <= tol, (np.abs(U - Uref).max(), tol)
+    assert np.abs(I - Iref).max() <= 2 * tol, (np.abs(I - Iref).max(), tol)

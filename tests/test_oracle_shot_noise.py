@@ -72,3 +72,32 @@ def test_S5_shot_noise_of_an_image():
     assert abs(((J - I) ** 2).mean() - I.mean() / 500.0) < 0.1 * I.mean() / 500.0      # variance = I / photons
     neg = o.shot_noise(np.full((4, 4), -0.2), 100.0, 1, 0)
     assert np.all(neg == 0.0)                                                          # max(I, 0)
+
+
+# ---- micro-topography of the height map (reading A29) ------------------------------------------------------------
+def test_T1_topography_factor_statistics_keying_and_effect():
+    from dataclasses import replace
+    from workloads import make_config
+    sc = make_config(2, n_override=60)
+    sc.cols["cx"][:] = sc.cols["cx"] / 4; sc.cols["cy"][:] = sc.cols["cy"] / 4
+    sc = replace(sc, H=256, W=256)
+    smooth = o.render_opd(sc)
+    assert np.all(o.topography_factor(sc, 0) == 1.0)                                   # amplitude 0: off
+    a = 0.03
+    rough = replace(sc, topography_amplitude=a)
+    f = o.topography_factor(rough, 0)
+    eta = (f - 1.0) / a
+    n = eta.size
+    assert abs(eta.mean()) < 5 / np.sqrt(n) and abs(eta.var() - 1.0) < 5 * np.sqrt(2.0 / n)      # N(0, 1)
+    assert abs(stats.kstest(eta.ravel(), "norm").statistic) < 0.01
+    # white: neighbouring pixels uncorrelated; its own stream: uncorrelated with the read noise of the same key
+    assert abs(np.corrcoef(eta[:, :-1].ravel(), eta[:, 1:].ravel())[0, 1]) < 0.02
+    assert abs(np.corrcoef(eta[:-1].ravel(), eta[1:].ravel())[0, 1]) < 0.02
+    assert abs(np.corrcoef(eta.ravel(), o.read_noise(sc.seed, 0, 256, 256).ravel())[0, 1]) < 0.02
+    assert not np.array_equal(f, o.topography_factor(replace(rough, seed=sc.seed + 1), 0))
+    # every thickness at a pixel is scaled by the same factor: OPD and height scale with it, empty pixels stay empty
+    assert np.array_equal(o.render_opd(rough)[0], smooth[0] * f)
+    assert np.array_equal(o.render_height(rough)[0], o.render_height(sc)[0] * f)
+    assert np.all(o.render_opd(rough)[smooth == 0.0] == 0.0)
+    # and the images change accordingly: rougher bodies scatter more light out of the pupil
+    assert not np.allclose(o.render_intensity(rough), o.render_intensity(sc), atol=1e-6)

@@ -46,6 +46,7 @@ class Scene:
     read_noise_sigma: float = 0.0
     defocus_um: float = 0.0      # delta z of Eq. 3; 0 = in focus
     shot_noise_photons: float = 0.0   # photons at unit intensity for the Poisson term of PAPER.md:126; 0 = off
+    topography_amplitude: float = 0.0   # relative amplitude of the micro-topography of PAPER.md:74; 0 = smooth bodies
     cols: dict = field(default_factory=dict)   # float32 [N] each + kind uint8 [N]
     frame_start: np.ndarray = None             # int32 [B+1]
 
