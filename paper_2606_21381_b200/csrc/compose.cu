@@ -44,7 +44,7 @@ constexpr int kQueue = 64;                         // survivor queue entries per
 constexpr int kCtaSplit = OSOG_CTA_SPLIT;             // compose CTAs per tile (each takes kWarps / kCtaSplit sub-tiles)
 constexpr int kCtaWarps = kWarps / kCtaSplit;
 constexpr int kSmemSlots = kCtaWarps * 32 * kSlotStride4 * 16;
-constexpr int kSmemBytes = kSmemSlots + kCtaWarps * kQueue * 4;   // k_compose_tile: per-warp survivor slots + survivor queues
+constexpr int kSmemBytes = kSmemSlots + kCtaWarps * 2 * kQueue * 4;   // k_compose_tile: per-warp survivor slots + two survivor queues
 
 // ---- small PTX helpers ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float fast_sqrt(float x)
@@ -143,7 +143,7 @@ __device__ __noinline__ double prism_t64(const double* r64, uint32_t vmask, doub
 
 // ---- preparation of one prism survivor by ONE lane (32 survivors are prepared at once, one per lane) --------------------
 // Evaluation classes of a prepared survivor:
-constexpr uint32_t kClsEllipsoid = 0u, kClsFull = 1u /* 1 + steep slabs: 1, 2, 3 */, kClsF64 = 4u, kClsPair = 5u, kClsNone = 7u;
+constexpr uint32_t kClsFull = 1u /* 1 + steep slabs: 1, 2, 3 */, kClsF64 = 4u, kClsPair = 5u, kClsNone = 7u;
 // For each of the 6 slabs: re-base its coefficients from the particle's reference pixel (jc, ic) to the warp's sub-tile
 // origin (wx0, wy0) and round to fp32 there: all later fp32 arithmetic uses pixel offsets 0..15 / 0..7 (DESIGN.md section
 // 6).  The re-basing itself runs in fp32 on the record's exact-grid (hi, lo) pairs (k_prepare; already scaled by the
@@ -572,19 +572,21 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
     g.xf = (float)j;
     g.yf = (float)i;
     float4* my_slots = s_slots + (tid >> 5) * 32 * kSlotStride4;
-    uint32_t* my_queue = reinterpret_cast<uint32_t*>(smem + kSmemSlots) + (tid >> 5) * kQueue;   // particle index | class code << 29
+    // two survivor queues per warp: prisms (particle index | record code << 29) and ellipsoids (particle index)
+    uint32_t* queue_p = reinterpret_cast<uint32_t*>(smem + kSmemSlots) + (tid >> 5) * (2 * kQueue);
+    uint32_t* queue_e = queue_p + kQueue;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
     float pend[4] = {0.0f, 0.0f, 0.0f, 0.0f};
 
     const float4* recs4 = reinterpret_cast<const float4*>(a.rec);
     const unsigned lt = (1u << lane) - 1u;
-    int nq = 0;                                                  // queued survivors (warp-uniform)
+    int nqp = 0, nqe = 0;                                        // queued prisms / ellipsoids (warp-uniform)
     // entry of the first batch (the loop below always holds the next batch's entry in registers: the list loads of
     // batch n + 1 are in flight while batch n is processed)
     uint32_t nmeta = lane < L ? gmeta[lane] : 0u;
     uint32_t npid = lane < L ? glist[lane] : 0u;
     for (uint32_t base = 0; base < L; base += 32) {
-        // ---- lane <-> list entry base + lane: survivors of this warp's sub-tile join the queue, in list order ----------------
+        // ---- lane <-> list entry base + lane: survivors of this warp's sub-tile join their kind's queue, in list order ---------
         const uint32_t meta = nmeta, pid = npid;
         {
             const uint32_t kn = base + 32 + lane;
@@ -592,47 +594,42 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
             npid = kn < L ? glist[kn] : 0u;
         }
         const bool keep = ((meta >> wid) & 1u) != 0u;
-        const unsigned mk = __ballot_sync(0xffffffffu, keep);
+        const uint32_t code = meta >> 8;
+        const unsigned mkp = __ballot_sync(0xffffffffu, keep && code != 0u), mke = __ballot_sync(0xffffffffu, keep && code == 0u);
         if (keep) {
-            my_queue[nq + __popc(mk & lt)] = (pid & 0x1fffffffu) | ((meta >> 8) << 29);
+            if (code != 0u) queue_p[nqp + __popc(mkp & lt)] = (pid & 0x1fffffffu) | (code << 29);
+            else queue_e[nqe + __popc(mke & lt)] = pid;
         }
-        nq += __popc(mk);
+        nqp += __popc(mkp);
+        nqe += __popc(mke);
         __syncwarp();
-        // ---- 32 survivors queued (or the list has ended): one lane prepares one survivor, then all lanes evaluate them ------------
         const bool last = base + 32 >= L;
-        while (nq >= 32 || (last && nq > 0)) {
-            const int n = min(nq, 32);
+        // ---- 32 prisms queued (or the list has ended): one lane prepares one prism, then all lanes evaluate them class by class;
+        // fixed, data-defined summation order: 2 + 2 plane prisms, full prisms, one / two steep slabs, all-fp64 prisms, each class
+        // in ascending list position
+        while (nqp >= 32 || (last && nqp > 0)) {
+            const int n = min(nqp, 32);
             uint32_t cls = kClsNone;
             if (lane < n) {
-                const uint32_t ent = my_queue[lane];
+                const uint32_t ent = queue_p[lane];
                 const uint32_t spid = ent & 0x1fffffffu;
-                cls = ent >> 29;                                     // record code: 0 ellipsoid, 1..3 prism, 4 all-fp64 prism
-                const float4* rec = recs4 + (size_t)spid * (kRecWords / 4);
+                cls = ent >> 29;                                     // record code: 1..3 prism, 4 all-fp64 prism
                 float4* sl = my_slots + lane * kSlotStride4;
                 reinterpret_cast<uint32_t*>(sl)[27] = spid;
-                if (cls == kClsEllipsoid) {                          // copy the record's fp32 (hi, lo) coefficients into the slot
-                    const float4 c0 = __ldg(rec + 10), c1 = __ldg(rec + 11), c2 = __ldg(rec + 12), c3 = __ldg(rec + 13);
-                    const float K = __ldg(reinterpret_cast<const float*>(rec) + 9);
-                    sl[0] = c0; sl[1] = c1; sl[2] = c2; sl[3] = c3;
-                    reinterpret_cast<float*>(sl)[25] = K;
-                } else if (cls != kClsF64) {
-                    cls = prep_prism(sl, rec, reinterpret_cast<const float4*>(a.rec2 + (size_t)spid * kPairWords), wx0, wy0);
-                }
+                if (cls != kClsF64)
+                    cls = prep_prism(sl, recs4 + (size_t)spid * (kRecWords / 4),
+                                     reinterpret_cast<const float4*>(a.rec2 + (size_t)spid * kPairWords), wx0, wy0);
             }
             const unsigned mp = __ballot_sync(0xffffffffu, cls == kClsPair);
             const unsigned m1 = __ballot_sync(0xffffffffu, cls == kClsFull);
             const unsigned m2 = __ballot_sync(0xffffffffu, cls == kClsFull + 1u);
             const unsigned m3 = __ballot_sync(0xffffffffu, cls == kClsFull + 2u);
             const unsigned m4 = __ballot_sync(0xffffffffu, cls == kClsF64);
-            const unsigned m0 = __ballot_sync(0xffffffffu, cls == kClsEllipsoid);
-            // the next 32 queue entries move to the front while the slots are being read
-            uint32_t moved = 0u;
-            if (32 + lane < nq) moved = my_queue[32 + lane];
+            uint32_t moved = 0u;                                     // the next queue entries move to the front
+            if (32 + lane < nqp) moved = queue_p[32 + lane];
             __syncwarp();
-            if (32 + lane < nq) my_queue[lane] = moved;
-            nq -= n;
-            // Fixed, data-defined summation order: class by class (2 + 2 plane prisms, full prisms, one / two steep slabs,
-            // all-fp64 prisms, ellipsoids), ascending list position inside a class.
+            if (32 + lane < nqp) queue_p[lane] = moved;
+            nqp -= n;
             run_class(mp, my_slots, pend, acc, [&](const float4* slot) { eval_prism_pair(slot, g, pend); });
             run_class(m1, my_slots, pend, acc, [&](const float4* slot) { eval_prism<0>(slot, g, pend); });
             run_class(m2, my_slots, pend, acc, [&](const float4* slot) { eval_prism<1>(slot, g, pend); });
@@ -644,7 +641,32 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
 #pragma unroll
                 for (int k = 0; k < 4; ++k) acc[k] += prism_f64_px(rec, (double)(g.xf + (float)k), (double)g.yf);
             }
-            run_class(m0, my_slots, pend, acc, [&](const float4* slot) { eval_ellipsoid(slot, g, pend); });
+            __syncwarp();
+        }
+        // ---- 32 ellipsoids queued (or the list has ended): every lane copies one record's fp32 (hi, lo) coefficients into its
+        // slot, then all lanes evaluate slots 0 .. n-1 in order
+        while (nqe >= 32 || (last && nqe > 0)) {
+            const int n = min(nqe, 32);
+            if (lane < n) {
+                const float4* rec = recs4 + (size_t)queue_e[lane] * (kRecWords / 4);
+                float4* sl = my_slots + lane * kSlotStride4;
+                const float4 c0 = __ldg(rec + 10), c1 = __ldg(rec + 11), c2 = __ldg(rec + 12), c3 = __ldg(rec + 13);
+                const float K = __ldg(reinterpret_cast<const float*>(rec) + 9);
+                sl[0] = c0; sl[1] = c1; sl[2] = c2; sl[3] = c3;
+                reinterpret_cast<float*>(sl)[25] = K;
+            }
+            uint32_t moved = 0u;
+            if (32 + lane < nqe) moved = queue_e[32 + lane];
+            __syncwarp();
+            if (32 + lane < nqe) queue_e[lane] = moved;
+            nqe -= n;
+            const float4* slot = my_slots;
+#pragma unroll 1
+            for (int left = n; left > 0; left -= kFlush) {
+#pragma unroll 1
+                for (int q = min(left, kFlush); q > 0; --q, slot += kSlotStride4) eval_ellipsoid(slot, g, pend);
+                flush(pend, acc);
+            }
             __syncwarp();
         }
     }
