@@ -156,10 +156,10 @@ constexpr uint32_t kClsFull = 1u /* 1 + steep slabs: 1, 2, 3 */, kClsF64 = 4u, k
 // finer grid of the sub-tile: hi = multiple of q = 2^(e - 21), 2^e > every intermediate of  C - U lx - V ly  over the
 // sub-tile, so the evaluation's fp32 FMAs on the hi parts are exact and hi + lo is good to 2^-24 relative of the (small)
 // result; the class with the lo-part FMAs (1 + NS) is only taken when a steep plane survives the interval test.
-// Slot layout (words): 0..5 Ex, 6..11 En, 12..17 U, 18..23 V (hi parts for steep slabs), 25 dn / s, 27 particle index,
-// 28..31 lo parts (Ex, En, U, V) of slab 0, 32..35 of slab 1; or, class kClsPair, words 28..39: Cx_a Cx_b Ux_a Ux_b |
-// Vx_a Vx_b Cn_c Cn_d | Un_c Un_d Vn_c Vn_d (exit planes a, b; entry planes c, d).  An ellipsoid slot holds the record's
-// words 40..53 in words 0..15.
+// Slot layout (float4 units; one 128-bit store per slab, conflict-free across the lanes' slots): 0..5 = (Ex, En, U, V) of slab
+// 0..5 (hi parts for steep slabs), 6 = (-, dn / s, -, particle index), 7 and 8 = lo parts (Ex, En, U, V) of slab 0 and 1; or,
+// class kClsPair, 7..9 = Cx_a Cx_b Ux_a Ux_b | Vx_a Vx_b Cn_c Cn_d | Un_c Un_d Vn_c Vn_d (exit planes a, b; entry planes c, d).
+// An ellipsoid slot holds the record's words 40..53 in float4 0..3.
 __device__ __forceinline__ uint32_t prep_prism(float4* __restrict__ slot, const float4* __restrict__ rec, const float4* __restrict__ pairs,
                                                int wx0, int wy0)
 {
@@ -187,7 +187,7 @@ __device__ __forceinline__ uint32_t prep_prism(float4* __restrict__ slot, const 
             slot[7 + q] = make_float4((xh - exh) + xl, (nh - enh) + nl, (h.x - uh) + l.x, (h.y - vh) + l.y);
             exf = exh; enf = enh; uf = uh; vf = vh;
         }
-        sw[q] = exf; sw[6 + q] = enf; sw[12 + q] = uf; sw[18 + q] = vf;
+        slot[q] = make_float4(exf, enf, uf, vf);
         // value range of  C - U lx - V ly  over lx in [0, 15], ly in [0, 7]: centre value -+ half range, padded for the
         // fp32 roundings of this block and of the evaluation (a few ulp of the largest magnitude involved)
         const float ec = fmaf(-3.5f, vf, fmaf(-7.5f, uf, exf));
@@ -212,10 +212,10 @@ __device__ __forceinline__ uint32_t prep_prism(float4* __restrict__ slot, const 
     const int a0 = __ffs(mx) - 1, c0 = __ffs(mn) - 1;
     const uint32_t mx1 = mx & (mx - 1u), mn1 = mn & (mn - 1u);
     const int a1 = mx1 ? __ffs(mx1) - 1 : a0, c1 = mn1 ? __ffs(mn1) - 1 : c0;      // a single plane is simply used twice
-    const float4 p0 = make_float4(sw[a0], sw[a1], sw[12 + a0], sw[12 + a1]);
-    const float4 p1 = make_float4(sw[18 + a0], sw[18 + a1], sw[6 + c0], sw[6 + c1]);
-    const float4 p2 = make_float4(sw[12 + c0], sw[12 + c1], sw[18 + c0], sw[18 + c1]);
-    slot[7] = p0; slot[8] = p1; slot[9] = p2;
+    const float4 sa = slot[a0], sb = slot[a1], sc = slot[c0], sd = slot[c1];
+    slot[7] = make_float4(sa.x, sb.x, sa.z, sb.z);
+    slot[8] = make_float4(sa.w, sb.w, sc.y, sd.y);
+    slot[9] = make_float4(sc.z, sd.z, sc.w, sd.w);
     return kClsPair;
 }
 
@@ -272,50 +272,50 @@ __device__ __noinline__ double prism_f64_px(const float4* __restrict__ rec, doub
 }
 
 // Prism (kind 1): 6 slabs, exit_k = Ex_k - U_k lx - V_k ly, enter_k = En_k - U_k lx - V_k ly from the re-based, scaled
-// fp32 coefficients (packed FFMA2, two slabs per instruction), s t = sat(min_k exit_k - max_k enter_k) with 3-input
+// fp32 coefficients (packed FFMA2: the exit and the entry plane of one slab per instruction, they share U and V),
+// s t = sat(min_k exit_k - max_k enter_k) with 3-input
 // min / max and a saturating subtraction.  The first NS (<= 2) slabs are steep (slope > kSteepSlope): their values are
 // the exact hi-part FMAs plus a packed lo-part FMA (one FFMA2 + 2 FADD per pixel and steep slab), no fp64.
 template <int NS>
 __device__ __forceinline__ void eval_prism(const float4* __restrict__ slot, const LaneGeom& g, float (&pend)[4])
 {
-    const float4 a0 = slot[0], a1 = slot[1], a2 = slot[2], a3 = slot[3], a4 = slot[4], a5 = slot[5];
+    const float4 s0 = slot[0], s1 = slot[1], s2 = slot[2], s3 = slot[3], s4 = slot[4], s5 = slot[5];   // (Ex, En, U, V) per slab
     const float dn = slot[6].y;
-    const float2 v01 = make_float2(a4.z, a4.w), v23 = make_float2(a5.x, a5.y), v45 = make_float2(a5.z, a5.w);
-    const float2 u01 = make_float2(a3.x, a3.y), u23 = make_float2(a3.z, a3.w), u45 = make_float2(a4.x, a4.y);
-    // row terms: value of every plane at this lane's row, column offset 0
-    const float2 ek01 = ffma2(v01, g.nly, make_float2(a0.x, a0.y));
-    const float2 ek23 = ffma2(v23, g.nly, make_float2(a0.z, a0.w));
-    const float2 ek45 = ffma2(v45, g.nly, make_float2(a1.x, a1.y));
-    const float2 nk01 = ffma2(v01, g.nly, make_float2(a1.z, a1.w));
-    const float2 nk23 = ffma2(v23, g.nly, make_float2(a2.x, a2.y));
-    const float2 nk45 = ffma2(v45, g.nly, make_float2(a2.z, a2.w));
-    float2 r0 = make_float2(0.f, 0.f), ul0 = r0, r1 = r0, ul1 = r0;   // lo parts of the steep slabs: (exit, enter) row terms, U
+    // row terms: (exit, entry) value of every slab at this lane's row, column offset 0
+    const float2 r0 = ffma2(make_float2(s0.w, s0.w), g.nly, make_float2(s0.x, s0.y));
+    const float2 r1 = ffma2(make_float2(s1.w, s1.w), g.nly, make_float2(s1.x, s1.y));
+    const float2 r2 = ffma2(make_float2(s2.w, s2.w), g.nly, make_float2(s2.x, s2.y));
+    const float2 r3 = ffma2(make_float2(s3.w, s3.w), g.nly, make_float2(s3.x, s3.y));
+    const float2 r4 = ffma2(make_float2(s4.w, s4.w), g.nly, make_float2(s4.x, s4.y));
+    const float2 r5 = ffma2(make_float2(s5.w, s5.w), g.nly, make_float2(s5.x, s5.y));
+    float2 l0 = make_float2(0.f, 0.f), ul0 = l0, l1 = l0, ul1 = l0;   // lo parts of the steep slabs: (exit, entry) row terms, U
     if (NS > 0) {
         const float4 l = slot[7];
-        r0 = ffma2(make_float2(l.w, l.w), g.nly, make_float2(l.x, l.y));
+        l0 = ffma2(make_float2(l.w, l.w), g.nly, make_float2(l.x, l.y));
         ul0 = make_float2(l.z, l.z);
     }
     if (NS > 1) {
         const float4 l = slot[8];
-        r1 = ffma2(make_float2(l.w, l.w), g.nly, make_float2(l.x, l.y));
+        l1 = ffma2(make_float2(l.w, l.w), g.nly, make_float2(l.x, l.y));
         ul1 = make_float2(l.z, l.z);
     }
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        float2 e01 = ffma2(u01, g.nlx[k], ek01), e23 = ffma2(u23, g.nlx[k], ek23), e45 = ffma2(u45, g.nlx[k], ek45);
-        float2 n01 = ffma2(u01, g.nlx[k], nk01), n23 = ffma2(u23, g.nlx[k], nk23), n45 = ffma2(u45, g.nlx[k], nk45);
+        float2 p0 = ffma2(make_float2(s0.z, s0.z), g.nlx[k], r0), p1 = ffma2(make_float2(s1.z, s1.z), g.nlx[k], r1);
+        const float2 p2 = ffma2(make_float2(s2.z, s2.z), g.nlx[k], r2), p3 = ffma2(make_float2(s3.z, s3.z), g.nlx[k], r3);
+        const float2 p4 = ffma2(make_float2(s4.z, s4.z), g.nlx[k], r4), p5 = ffma2(make_float2(s5.z, s5.z), g.nlx[k], r5);
         if (NS > 0) {
-            const float2 lo = ffma2(ul0, g.nlx[k], r0);
-            e01.x += lo.x;
-            n01.x += lo.y;
+            const float2 lo = ffma2(ul0, g.nlx[k], l0);
+            p0.x += lo.x;
+            p0.y += lo.y;
         }
         if (NS > 1) {
-            const float2 lo = ffma2(ul1, g.nlx[k], r1);
-            e01.y += lo.x;
-            n01.y += lo.y;
+            const float2 lo = ffma2(ul1, g.nlx[k], l1);
+            p1.x += lo.x;
+            p1.y += lo.y;
         }
-        const float ex = fminf(min3(e01.x, e01.y, e23.x), min3(e23.y, e45.x, e45.y));
-        const float en = fmaxf(max3(n01.x, n01.y, n23.x), max3(n23.y, n45.x, n45.y));
+        const float ex = fminf(min3(p0.x, p1.x, p2.x), min3(p3.x, p4.x, p5.x));
+        const float en = fmaxf(max3(p0.y, p1.y, p2.y), max3(p3.y, p4.y, p5.y));
         pend[k] = fmaf(sub_sat(ex, en), dn, pend[k]);
     }
 }
