@@ -581,18 +581,13 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
     const float4* recs4 = reinterpret_cast<const float4*>(a.rec);
     const unsigned lt = (1u << lane) - 1u;
     int nqp = 0, nqe = 0;                                        // queued prisms / ellipsoids (warp-uniform)
-    // entry of the first batch (the loop below always holds the next batch's entry in registers: the list loads of
-    // batch n + 1 are in flight while batch n is processed)
-    uint32_t nmeta = lane < L ? gmeta[lane] : 0u;
-    uint32_t npid = lane < L ? glist[lane] : 0u;
+    // The list is read one entry per lane at the top of each batch.  Measured alternatives (profiles/r2_compose_ncu.md): a register
+    // prefetch of the next batch (its two registers spill at 64 registers and the spill store waits for the load: no gain) and
+    // cp.async staging of the next batch's particle indices and meta words in shared memory (137.2 against 133.9 us: not kept).
     for (uint32_t base = 0; base < L; base += 32) {
         // ---- lane <-> list entry base + lane: survivors of this warp's sub-tile join their kind's queue, in list order ---------
-        const uint32_t meta = nmeta, pid = npid;
-        {
-            const uint32_t kn = base + 32 + lane;
-            nmeta = kn < L ? gmeta[kn] : 0u;
-            npid = kn < L ? glist[kn] : 0u;
-        }
+        const uint32_t kq = base + lane;
+        const uint32_t meta = kq < L ? gmeta[kq] : 0u, pid = kq < L ? glist[kq] : 0u;
         const bool keep = ((meta >> wid) & 1u) != 0u;
         const uint32_t code = meta >> 8;
         const unsigned mkp = __ballot_sync(0xffffffffu, keep && code != 0u), mke = __ballot_sync(0xffffffffu, keep && code == 0u);
