@@ -216,7 +216,11 @@ int osog_render_gbuffer_normals(osog_ctx* ctx, const osog_particles* p, int64_t 
  * allocates one more complex frame batch (shared with the DIC path). */
 int osog_backward_intensity(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gI, float* d_gopd);
 
-/* First step of the backward pass ("the gradient of the final image with respect to the initial state
+/* The three gathers below (osog_backward_np / _centre / _params) differentiate the SMOOTH bodies: they return OSOG_EINVAL when
+ * o->topography_amplitude != 0 (with micro-topography the OPD is OPD (1 + a eta), so the caller would have to multiply the
+ * upstream gradient by the same per-pixel factor, which only the library can draw).
+ *
+ * First step of the backward pass ("the gradient of the final image with respect to the initial state
  * tensor"): the OPD frame is linear in the refractive indices, OPD = sum_n (n_p[n] - n_medium) t_n, so for an
  * upstream gradient d_gopd = dL/dOPD (DEVICE float [B, H, W], read only) the gradient is
  * d_gnp[n] = dL/dn_p[n] = sum over the pixels of the particle's frame of d_gopd * t_n  (DEVICE float [N], overwritten;

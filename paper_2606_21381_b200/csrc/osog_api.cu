@@ -496,6 +496,7 @@ int osog_backward_np(osog_ctx* c, const osog_particles* p, int64_t N, const osog
     if (N == 0) return (c && p && o) ? OSOG_OK : OSOG_EINVAL;
     const int r = check_call(c, p, N, o, d_gnp);
     if (r != OSOG_OK) return r;
+    if (o->topography_amplitude != 0.0) return OSOG_EINVAL;   // the gathers differentiate the smooth bodies (see osog.h)
     DeviceGuard g(c->device);
     cudaError_t e = launch_binning(c, p, N, o);      // records + bounding boxes (the tile lists are not used)
     if (e != cudaSuccess) return cuda_fail(c, e);    // (scratch_dirty stays set: the next render call clears them)
@@ -510,6 +511,7 @@ int osog_backward_centre(osog_ctx* c, const osog_particles* p, int64_t N, const 
     if (N == 0) return (c && p && o) ? OSOG_OK : OSOG_EINVAL;
     const int r = check_call(c, p, N, o, d_gc);
     if (r != OSOG_OK) return r;
+    if (o->topography_amplitude != 0.0) return OSOG_EINVAL;   // the gathers differentiate the smooth bodies (see osog.h)
     DeviceGuard g(c->device);
     cudaError_t e = launch_binning(c, p, N, o);      // records + bounding boxes (the tile lists are not used)
     if (e != cudaSuccess) return cuda_fail(c, e);    // (scratch_dirty stays set: the next render call clears them)
@@ -551,6 +553,7 @@ int osog_backward_params(osog_ctx* c, const osog_particles* p, int64_t N, const 
     if (N == 0) return (c && p && o) ? OSOG_OK : OSOG_EINVAL;
     const int r = check_call(c, p, N, o, d_gpar);
     if (r != OSOG_OK) return r;
+    if (o->topography_amplitude != 0.0) return OSOG_EINVAL;   // the gathers differentiate the smooth bodies (see osog.h)
     DeviceGuard g(c->device);
     cudaError_t e = launch_binning(c, p, N, o);      // tile ranges, frames and pixel bounding boxes (the tile lists are not used)
     if (e != cudaSuccess) return cuda_fail(c, e);    // (scratch_dirty stays set: the next render call clears them)

@@ -130,3 +130,17 @@ def test_end_to_end_fit_with_the_spectral_loss(og, o):
     assert losses[-1] < 0.5 * losses[0]
     assert err1[0] < err0[0] and err1[1] < err0[1]
     ctx.close()
+
+
+def test_gathers_refuse_micro_topography(og):
+    """The gradient gathers differentiate the smooth bodies: with topography_amplitude != 0 they return OSOG_EINVAL."""
+    import torch
+    sc = replace(make_config(2, n_override=50), topography_amplitude=0.02)
+    ctx = og.Context(sc.H, sc.W, sc.N)
+    P, opt = og.Particles.from_scene(sc), og.optics_from_scene(sc)
+    G = torch.ones((1, sc.H, sc.W), dtype=torch.float32, device="cuda")
+    for call in (ctx.backward_np, ctx.backward_centre, ctx.backward_params):
+        with pytest.raises(og.OsogError) as e:
+            call(P, opt, G)
+        assert e.value.code == og.OSOG_EINVAL
+    ctx.close()
