@@ -129,7 +129,7 @@ typedef struct {
 } osog_brightfield;
 
 /* Create a context: allocates all scratch (records, tile ranges, per-tile counters, scan offsets, staging slices and the
- * CSR pair list, ramp tables, one complex frame batch and the cuFFT plans).  *out is set to NULL on failure. */
+ * CSR pair list, one complex frame batch and the cuFFT plans).  *out is set to NULL on failure. */
 int osog_create(osog_ctx** out, const osog_config* cfg);
 
 /* OPD frame(s): d_opd is DEVICE float [B, H, W], row-major, micrometres.  Steps H1-H6 of DESIGN.md: prepare + bounding box
@@ -278,7 +278,7 @@ int osog_debug_bins(osog_ctx* ctx, uint32_t* h_offset, uint32_t* h_list, int64_t
                     int64_t* n_tiles, int64_t* n_pairs);
 
 /* Test / measurement: re-runs ONLY the composition kernel (H5-H7) of the last call on its binning (tile lists, records,
- * ramp tables and optics are still in the context) and writes the complex field again.  Lets bench.py time the dominant
+ * optics are still in the context) and writes the complex field again.  Lets bench.py time the dominant
  * kernel alone with CUDA events.  OSOG_EINVAL unless the last call on this context was one of osog_render_opd / _field /
  * _intensity / _dic / _height or osog_backward_intensity (the calls that leave sorted lists and a composition behind). */
 int osog_debug_recompose_field(osog_ctx* ctx, float* d_field);
@@ -289,7 +289,7 @@ int osog_debug_recompose_field(osog_ctx* ctx, float* d_field);
 int osog_debug_poisson(osog_ctx* ctx, const float* d_lambda, int64_t n, uint64_t seed, uint32_t frame, int32_t* d_counts);
 
 /* Test / diagnostics: every scratch array of the context (records, tile ranges, counters, offsets, staging slices, CSR
- * list, meta words, ramp tables, optics, status, complex frames) is followed by a 256-byte guard band written once in
+ * list, meta words, optics, status, complex frames) is followed by a 256-byte guard band written once in
  * osog_create.  Synchronises and returns the number of guard bands that no longer hold their pattern (0 = no kernel wrote
  * past the end of its scratch), or a negative error code.  (compute-sanitizer is not available on every pool.) */
 int osog_debug_check_guards(osog_ctx* ctx);

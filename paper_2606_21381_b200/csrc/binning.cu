@@ -26,23 +26,12 @@ struct PrepArgs {
     long long max_pairs;          // capacity of the CSR list: a larger total sets OSOG_WOVERFLOW
     float* obb;                   // [N][6] oriented-bounding-box labels (osog_particle_obbs), or nullptr
     int unit_dn;                  // 1: index contrast n_p - n_medium replaced by 1 (height map of the G-buffer)
-    float2 *ramp_x, *ramp_y;
     FrameOptics* optics;
     DeviceStatus* status;
-    int has_ramp;
     OpticsChunk oc;               // frames 0 .. min(B, kOpticsChunk)-1 by value
 };
 
 __device__ __forceinline__ bool finite_f(float v) { return fabsf(v) <= 3.402823466e38f; }   // false for NaN / inf
-
-// exp(i 2 pi t) for a double turn count, as float2
-__device__ __forceinline__ float2 cis_turns(double t)
-{
-    t -= rint(t);
-    double s, c;
-    sincospi(2.0 * t, &s, &c);
-    return make_float2((float)c, (float)s);
-}
 
 constexpr int kPrepThreads = 128;
 
@@ -478,7 +467,7 @@ constexpr int kRecPerBlock = kPrepThreads / 8;     // particles per record-role 
 // Grid layout (blocks of 128 threads): [0, nbin) binning role, one particle per thread (nbin = max(1, ceil(N / 128)): the
 // scan needs a block even when N = 0); [nbin, nbin + nrec) record role, 16 particles per block, 8 lanes each, the block's
 // particles permuted so that prisms come first (its warps are then uniform in the code path they take, except one mixed
-// warp per block); [nbin + nrec, ...) ramp tables.  nrec = ceil(N / 16).
+// warp per block).  nrec = ceil(N / 16).
 __global__ void __launch_bounds__(kPrepThreads, 6) k_prepare(const PrepArgs a)
 {
     pdl_trigger();                               // k_sort_cull's CTAs may become resident (they wait for this grid to finish)
@@ -489,23 +478,7 @@ __global__ void __launch_bounds__(kPrepThreads, 6) k_prepare(const PrepArgs a)
 
     if (gid < a.B && gid < kOpticsChunk) a.optics[gid] = a.oc.f[gid];
 
-    if ((long long)blockIdx.x >= nbin + nrec) {
-        // ---- phase-ramp tables exp(i 2 pi fx0 x_j), x_j = (j + 1/2) p  (oblique illumination)
-        if (!a.has_ramp) return;
-        long long r = gid - (nbin + nrec) * kPrepThreads;
-        const long long nx = (long long)a.B * a.W, ny = (long long)a.B * a.H;
-        if (r < nx) {
-            const int b = (int)(r / a.W), j = (int)(r % a.W);
-            const double f = b < kOpticsChunk ? a.oc.f[b].fx0_pitch : a.optics[b].fx0_pitch;
-            a.ramp_x[r] = cis_turns(f * (j + 0.5));
-        } else if (r - nx < ny) {
-            r -= nx;
-            const int b = (int)(r / a.H), i = (int)(r % a.H);
-            const double f = b < kOpticsChunk ? a.oc.f[b].fy0_pitch : a.optics[b].fy0_pitch;
-            a.ramp_y[r] = cis_turns(f * (i + 0.5));
-        }
-        return;
-    }
+    if ((long long)blockIdx.x >= nbin + nrec) return;          // blocks that only upload optics (B > blocks * threads)
 
     if ((long long)blockIdx.x < nbin) {
         // ---- H2 + first half of H4: binning role, one particle per thread
@@ -619,15 +592,13 @@ cudaError_t launch_binning(osog_ctx* c, const osog_particles* p, long long N, co
     a.offset = c->offset; a.done = c->done; a.max_pairs = c->max_pairs;
     a.obb = d_obb;
     a.unit_dn = unit_dn ? 1 : 0;
-    a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.optics = c->optics; a.status = status;
-    a.has_ramp = (o->tilt_x_rad != 0.0 || o->tilt_y_rad != 0.0) ? 1 : 0;
+    a.optics = c->optics; a.status = status;
     if ((e = upload_optics(c, o, &a.oc)) != cudaSuccess) return e;
 
     const int threads = kPrepThreads;
     const long long nb = (N + threads - 1) / threads;
     const long long nrec = (N + kRecPerBlock - 1) / kRecPerBlock;
-    const long long ramp_items = a.has_ramp ? (long long)B * (c->W + c->H) : 0;
-    long long blocks = (nb > 0 ? nb : 1) + nrec + (ramp_items + threads - 1) / threads;
+    long long blocks = (nb > 0 ? nb : 1) + nrec;
     if (blocks * threads < B) blocks = (B + threads - 1) / threads;     // the first threads also upload the optics
     k_prepare<<<(unsigned)blocks, threads, 0, c->stream>>>(a);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;

@@ -25,12 +25,10 @@ struct ComposeArgs {
     const uint32_t* list;        // CSR list, every tile's segment sorted by k_sort_cull
     const uint16_t* meta;        // per list entry
     const FrameOptics* optics;
-    const float2 *ramp_x, *ramp_y;
     const DeviceStatus* status;
     float* opd;
     float2* field;
     int H, W, ntx, nty;
-    int ramp_y_on;
     float topo_amp;              // micro-topography (reading A29): the height map is multiplied by 1 + topo_amp * eta(pixel); 0 = off
     unsigned long long seed;
 };
@@ -338,7 +336,7 @@ __device__ __forceinline__ void eval_prism_pair(const float4* __restrict__ slot,
 
 // The evaluation loops add into fp32 partial sums; every kFlush survivors (and at the end of a class) these are widened
 // and added to the fp64 per-pixel accumulators: one widening conversion + DADD per pixel and kFlush particles.
-constexpr int kFlush = 4;
+constexpr int kFlush = 8;
 __device__ __forceinline__ void flush(float (&pend)[4], double (&acc)[4])
 {
 #pragma unroll
@@ -687,25 +685,52 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
         }
     }
     if (FIELD) {
-        const double inv_lambda = a.optics[b].inv_lambda;
+        float2* out = a.field + row + j;
+        if (overflow) {                                              // warp-uniform: the frame is zero-filled
+            if (vec) {
+                reinterpret_cast<float4*>(out)[0] = make_float4(0.f, 0.f, 0.f, 0.f);
+                reinterpret_cast<float4*>(out)[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+            } else {
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (j + k < a.W) out[k] = make_float2(0.f, 0.f);
+            }
+            return;
+        }
+        // Eq. 2 with the oblique-illumination ramp: U = exp(i 2 pi (OPD / lambda + fx0 x_j + fy0 y_i)).  The
+        // three terms are added in turns, in fp64, and reduced to [-1/2, 1/2] before the one fp32 sincos per pixel (no ramp
+        // tables, no complex multiplications).
+        const FrameOptics* fo = a.optics + b;
+        const double inv_lambda = fo->inv_lambda;
+        double ramp0 = 0.0, ramp_dx = 0.0;
+        if (RAMP) {
+            ramp_dx = fo->fx0_pitch;
+            ramp0 = fma(ramp_dx, (double)j + 0.5, fo->fy0_pitch * ((double)i + 0.5));
+        }
+        // packed Horner coefficients of sin(pi r) / r and cos(pi r), |r| <= 1/4
+        const float2 c3 = make_float2(0.0821458866f, 0.235330630f), c2 = make_float2(-0.599264529f, -1.33526277f);
+        const float2 c1 = make_float2(2.55016404f, 4.05871213f), c0 = make_float2(-5.16771278f, -4.93480220f);
+        const float2 cc = make_float2(3.14159265f, 1.0f);
         float2 u[4];
-        float2 ry = make_float2(1.0f, 0.0f);
-        if (RAMP && a.ramp_y_on) ry = a.ramp_y[(size_t)b * a.H + i];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-            double turns = acc[k] * inv_lambda;                  // Eq. 2: phase = 2 pi OPD / lambda, kept in turns
+            double turns = fma(acc[k], inv_lambda, RAMP ? fma(ramp_dx, (double)k, ramp0) : 0.0);
             turns -= rint(turns);
-            float s, c;
-            sincospi_unit(2.0f * (float)turns, &s, &c);
-            if (RAMP && j + k < a.W) {
-                float2 r = a.ramp_x[(size_t)b * a.W + j + k];
-                if (a.ramp_y_on) r = make_float2(r.x * ry.x - r.y * ry.y, r.x * ry.y + r.y * ry.x);
-                const float c2 = c * r.x - s * r.y, s2 = c * r.y + s * r.x;
-                c = c2; s = s2;
-            }
-            u[k] = overflow ? make_float2(0.f, 0.f) : make_float2(c, s);
+            const float x = 2.0f * (float)turns;                     // angle / pi, in [-1, 1]
+            const float kf = rintf(x + x);
+            const int q = (int)kf;
+            const float r = fmaf(kf, -0.5f, x);
+            const float r2 = r * r;
+            const float2 rr = make_float2(r2, r2);
+            float2 pq = ffma2(rr, c3, c2);
+            pq = ffma2(rr, pq, c1);
+            pq = ffma2(rr, pq, c0);
+            pq = ffma2(rr, pq, cc);
+            float sp = pq.x * r, cp = pq.y;
+            if (q & 1) { const float t = sp; sp = cp; cp = -t; }
+            if (q & 2) { sp = -sp; cp = -cp; }
+            u[k] = make_float2(cp, sp);
         }
-        float2* out = a.field + row + j;
         if (vec) {
             reinterpret_cast<float4*>(out)[0] = make_float4(u[0].x, u[0].y, u[1].x, u[1].y);
             reinterpret_cast<float4*>(out)[1] = make_float4(u[2].x, u[2].y, u[3].x, u[3].y);
@@ -733,10 +758,9 @@ cudaError_t launch_compose(osog_ctx* c, int B, bool has_ramp, float* d_opd, floa
     ComposeArgs a;
     a.rec = c->rec; a.rec2 = c->rec2; a.offset = c->offset; a.list = c->list; a.meta = c->meta;
     a.optics = c->optics;
-    a.ramp_x = c->ramp_x; a.ramp_y = c->ramp_y; a.status = c->status + c->status_idx;
+    a.status = c->status + c->status_idx;
     a.opd = d_opd; a.field = d_field;
     a.H = c->H; a.W = c->W; a.ntx = c->ntx; a.nty = c->nty;
-    a.ramp_y_on = 1;
     a.topo_amp = (float)c->last_topo; a.seed = c->last_seed;
     const unsigned grid = (unsigned)((long long)B * c->ntx * c->nty);
     if (sort_first) {

@@ -196,7 +196,7 @@ int osog_destroy(osog_ctx* c)
     if (c->has_plan_one) cufftDestroy(c->plan_one);
     if (c->has_plan_batch) cufftDestroy(c->plan_batch);
     cudaFree(c->rec); cudaFree(c->rec2); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
-    cudaFree(c->list); cudaFree(c->meta); cudaFree(c->slices); cudaFree(c->offset); cudaFree(c->done); cudaFree(c->ramp_x); cudaFree(c->ramp_y); cudaFree(c->optics);
+    cudaFree(c->list); cudaFree(c->meta); cudaFree(c->slices); cudaFree(c->offset); cudaFree(c->done); cudaFree(c->optics);
     cudaFree(c->status); cudaFree(c->field); cudaFree(c->work); cudaFree(c->otf); cudaFree(c->bf_h); cudaFree(c->spec_partial);
     delete c->otf_key;
     delete c->guards;
@@ -257,8 +257,6 @@ int osog_create(osog_ctx** out, const osog_config* cfg)
     A(dalloc(&c->slices, (size_t)c->max_tiles * c->slice_cap, c));
     A(dalloc(&c->list, (size_t)c->max_pairs, c));
     A(dalloc(&c->meta, (size_t)c->max_pairs, c));
-    A(dalloc(&c->ramp_x, (size_t)c->max_frames * c->W, c));
-    A(dalloc(&c->ramp_y, (size_t)c->max_frames * c->H, c));
     A(dalloc(&c->optics, (size_t)c->max_frames, c));
     A(dalloc(&c->status, 2, c));
     A(dalloc(&c->field, (size_t)c->max_frames * npx, c));

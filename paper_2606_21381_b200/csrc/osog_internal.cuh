@@ -80,8 +80,6 @@ struct osog_ctx {
     uint32_t* slices;               // [max_tiles][slice_cap] staging: tile t's unsorted entries at slices + t * slice_cap
     uint32_t* list;                 // [max_pairs] CSR list: tile t's particle indices, ascending, at list + offset[t]
     uint16_t* meta;                 // [max_pairs] per list entry: sub-tile mask | evaluation code << 8 (k_sort_cull)
-    float2* ramp_x;                 // [max_frames][W]  exp(i 2 pi fx0 x_j)
-    float2* ramp_y;                 // [max_frames][H]
     osog::FrameOptics* optics;      // [max_frames]
     osog::DeviceStatus* status;     // [2]: slot of the current call / slot being reset for the next call
     int status_idx;                 // slot used by the last render call
