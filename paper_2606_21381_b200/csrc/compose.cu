@@ -1166,10 +1166,20 @@ __device__ __forceinline__ void prism_plane(int k, double s, double L, double hc
     dnb[0][2] = sz * 0.5;                          // d / ds
 }
 
-__global__ void __launch_bounds__(256) k_backward_params(const ParamGradArgs a)
+// The per-pixel derivative is LINEAR in a few per-pixel quantities, so the pixel loop only accumulates moments and the
+// seven parameters are formed once per particle:
+//   prism, pixel with active exit plane e and entry plane f:  dz_k/dtheta = (db_k - dn_x dx - dn_y dy - z_k dn_z) / n_z, so
+//     sum_px G dt/dtheta = sum_k sgn_k (db_k S0_k - dn_x Sx_k - dn_y Sy_k - dn_z Sz_k) / n_z,k  with the moments
+//     (S0, Sx, Sy)_k = sum over the pixels where plane k is active of G (1, dx, dy), Sz_k = zc_k S0_k - za_k Sx_k - zb_k Sy_k,
+//     sgn = +1 for exit planes (n_z > 0), -1 for entry planes.  36 moments per lane, in shared memory (lane-private columns).
+//   ellipsoid, w = G / sqrt(disc):  sum_px G dt/dtheta = (2 <Bq dBq> - dA <C> - A <dC>) / A - 2 dA sum(G sqrt(disc)) / A^2,
+//     <.> = sum_px w (.), every bracket a quadratic form in (dx, dy): moments sum w (1, dx^2, dx dy, dy^2) and sum G sqrt(disc).
+constexpr int kPgThreads = 128;
+__global__ void __launch_bounds__(kPgThreads, 4) k_backward_params(const ParamGradArgs a)
 {
+    __shared__ double s_mom[kPgThreads / 32][36][32];            // prism moments: [plane * 3 + (0, x, y)][lane]
     const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     if (n >= a.N) return;
     double acc[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     double dn_idx = 0.0;
@@ -1194,99 +1204,150 @@ __global__ void __launch_bounds__(256) k_backward_params(const ParamGradArgs a)
             const double D[3] = {1.0 / (e[0] * e[0]), 1.0 / (e[1] * e[1]), 1.0 / (e[2] * e[2])};
             // symmetric 3 x 3 as (xx, xy, yy, xz, yz, zz)
             const int ra[6] = {0, 0, 1, 0, 1, 2}, rb[6] = {0, 1, 1, 2, 2, 2};
-            double M[6], dM[7][6];
+            double M[6];
 #pragma unroll
             for (int c = 0; c < 6; ++c) {
                 M[c] = 0.0;
 #pragma unroll
                 for (int k = 0; k < 3; ++k) M[c] += R[3 * ra[c] + k] * D[k] * R[3 * rb[c] + k];
-#pragma unroll
-                for (int p = 0; p < 3; ++p) dM[p][c] = R[3 * ra[c] + p] * (-2.0 * D[p] / e[p]) * R[3 * rb[c] + p];
-#pragma unroll
-                for (int p = 0; p < 4; ++p) {
-                    double v = 0.0;
-#pragma unroll
-                    for (int k = 0; k < 3; ++k) v += (dR[p][3 * ra[c] + k] * R[3 * rb[c] + k] + R[3 * ra[c] + k] * dR[p][3 * rb[c] + k]) * D[k];
-                    dM[3 + p][c] = v;
-                }
             }
+            double m0 = 0.0, mxx = 0.0, mxy = 0.0, myy = 0.0, ms = 0.0;
+            int i = i0 + lane / bw, j = j0 + lane % bw;
             for (int q = lane; q < np; q += 32) {
-                const int i = i0 + q / bw, j = j0 + q % bw;
                 const double dx = (j + 0.5) * a.pitch - cx, dy = (i + 0.5) * a.pitch - cy;
+                const double gv = (double)g[(size_t)i * a.W + j];
+                j += 32;
+                while (j > j1) { j -= bw; ++i; }
                 const double A = M[5], Bq = M[3] * dx + M[4] * dy, C = M[0] * dx * dx + 2.0 * M[1] * dx * dy + M[2] * dy * dy - 1.0;
                 const double disc = Bq * Bq - A * C;
                 if (!(disc > 0.0)) continue;
-                const double sq = sqrt(disc), gv = (double)g[(size_t)i * a.W + j];
-                const double c1 = 1.0 / (A * sq), c2 = 2.0 * sq / (A * A);
+                const double sq = sqrt(disc);
+                const double wq = gv / sq;
+                m0 += wq;
+                mxx = fma(wq, dx * dx, mxx);
+                mxy = fma(wq, dx * dy, mxy);
+                myy = fma(wq, dy * dy, myy);
+                ms = fma(gv, sq, ms);
+            }
 #pragma unroll
-                for (int p = 0; p < 7; ++p) {
-                    const double dA = dM[p][5], dBq = dM[p][3] * dx + dM[p][4] * dy;
-                    const double dC = dM[p][0] * dx * dx + 2.0 * dM[p][1] * dx * dy + dM[p][2] * dy * dy;
-                    acc[p] = fma(gv, (2.0 * Bq * dBq - C * dA - A * dC) * c1 - c2 * dA, acc[p]);
+            for (int d = 16; d > 0; d >>= 1) {
+                m0 += __shfl_xor_sync(0xffffffffu, m0, d);
+                mxx += __shfl_xor_sync(0xffffffffu, mxx, d);
+                mxy += __shfl_xor_sync(0xffffffffu, mxy, d);
+                myy += __shfl_xor_sync(0xffffffffu, myy, d);
+                ms += __shfl_xor_sync(0xffffffffu, ms, d);
+            }
+            const double A = M[5], iA = 1.0 / A;
+            const double qC = M[0] * mxx + 2.0 * M[1] * mxy + M[2] * myy - m0;                       // <C>
+#pragma unroll
+            for (int p = 0; p < 7; ++p) {
+                double dM[6];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) {
+                    if (p < 3) {
+                        dM[c] = R[3 * ra[c] + p] * (-2.0 * D[p] / e[p]) * R[3 * rb[c] + p];
+                    } else {
+                        double v = 0.0;
+#pragma unroll
+                        for (int k = 0; k < 3; ++k)
+                            v += (dR[p - 3][3 * ra[c] + k] * R[3 * rb[c] + k] + R[3 * ra[c] + k] * dR[p - 3][3 * rb[c] + k]) * D[k];
+                        dM[c] = v;
+                    }
                 }
+                const double qBdB = M[3] * dM[3] * mxx + (M[3] * dM[4] + M[4] * dM[3]) * mxy + M[4] * dM[4] * myy;   // <Bq dBq>
+                const double qdC = dM[0] * mxx + 2.0 * dM[1] * mxy + dM[2] * myy;                                      // <dC>
+                acc[p] = (2.0 * qBdB - dM[5] * qC - A * qdC) * iA - 2.0 * dM[5] * ms * iA * iA;
             }
         } else {
-            // per plane: z_k(dx, dy) = zc - za dx - zb dy (planes with n_z != 0), sign of n_z; vertical planes: g = zc - za dx - zb dy >= 0
-            double zc[12], za[12], zb[12], nzk[12];
+            // The 12 planes are 6 centrally symmetric slabs (A, B = -A): with u = n_x / n_z, v = n_y / n_z, c = b / |n_z| of plane A,
+            // the slab's exit plane is z = c - u dx - v dy and its entry plane z = -c - u dx - v dy (exit = A iff n_z > 0).
+            // Vertical slab (n_z = 0): inside iff |n_x dx + n_y dy| <= b.
+            const int slabA[6] = {0, 2, 4, 5, 8, 9};
+            double su[6], sv[6], sc[6];
+            uint32_t vmask = 0u;
 #pragma unroll
-            for (int k = 0; k < 12; ++k) {
+            for (int sl = 0; sl < 6; ++sl) {
                 double nb[3], bk, dnb[3][3], db[3];
-                prism_plane(k, e[0], e[1], e[2], nb, &bk, dnb, db);
+                prism_plane(slabA[sl], e[0], e[1], e[2], nb, &bk, dnb, db);
                 const double nx = R[0] * nb[0] + R[1] * nb[1] + R[2] * nb[2], ny = R[3] * nb[0] + R[4] * nb[1] + R[5] * nb[2];
-                nzk[k] = R[6] * nb[0] + R[7] * nb[1] + R[8] * nb[2];
-                const double inz = nzk[k] != 0.0 ? 1.0 / nzk[k] : 1.0;
-                zc[k] = bk * inz; za[k] = nx * inz; zb[k] = ny * inz;
+                const double nz = R[6] * nb[0] + R[7] * nb[1] + R[8] * nb[2];
+                if (nz == 0.0) { vmask |= 1u << sl; su[sl] = nx; sv[sl] = ny; sc[sl] = bk; }
+                else { const double inz = 1.0 / nz; su[sl] = nx * inz; sv[sl] = ny * inz; sc[sl] = bk * fabs(inz); }
             }
+            double (*mom)[32] = s_mom[wid];                       // [(slab * 2 + (exit, entry)) * 3 + (0, x, y)][lane]
+#pragma unroll
+            for (int m = 0; m < 36; ++m) mom[m][lane] = 0.0;
+            int i = i0 + lane / bw, j = j0 + lane % bw;
             for (int q = lane; q < np; q += 32) {
-                const int i = i0 + q / bw, j = j0 + q % bw;
                 const double dx = (j + 0.5) * a.pitch - cx, dy = (i + 0.5) * a.pitch - cy;
+                const double gv = (double)g[(size_t)i * a.W + j];
+                j += 32;
+                while (j > j1) { j -= bw; ++i; }
                 double ex = 1.0e300, en = -1.0e300;
                 int ke = 0, kf = 0;
                 bool out = false;
 #pragma unroll
-                for (int k = 0; k < 12; ++k) {
-                    const double zk = zc[k] - za[k] * dx - zb[k] * dy;
-                    if (nzk[k] > 0.0) { if (zk < ex) { ex = zk; ke = k; } }
-                    else if (nzk[k] < 0.0) { if (zk > en) { en = zk; kf = k; } }
-                    else if (zk < 0.0) out = true;
+                for (int sl = 0; sl < 6; ++sl) {
+                    const double m = fma(su[sl], dx, sv[sl] * dy);
+                    if ((vmask >> sl) & 1u) {
+                        out = out || fabs(m) > sc[sl];
+                    } else {
+                        const double ze = sc[sl] - m, zn = -sc[sl] - m;
+                        if (ze < ex) { ex = ze; ke = sl; }
+                        if (zn > en) { en = zn; kf = sl; }
+                    }
                 }
                 if (out || !(ex - en > 0.0)) continue;
-                const double gv = (double)g[(size_t)i * a.W + j];
-#pragma unroll 1
-                for (int side = 0; side < 2; ++side) {
-                    const int k = side ? kf : ke;
-                    double nzv = nzk[0];
+                const double gx = gv * dx, gy = gv * dy;
+                double* me = &mom[6 * ke][lane];
+                double* mf = &mom[6 * kf + 3][lane];
+                me[0] += gv; me[32] += gx; me[64] += gy;
+                mf[0] += gv; mf[32] += gx; mf[64] += gy;
+            }
+            __syncwarp();
+            // the 36 moments summed over the lanes (shuffle tree: a fixed order), then the parameters, slab by slab
 #pragma unroll
-                    for (int kk = 1; kk < 12; ++kk) nzv = kk == k ? nzk[kk] : nzv;
-                    const double zk = side ? en : ex, sgn = side ? -1.0 : 1.0, inz = 1.0 / nzv;
-                    double nb[3], bk, dnb[3][3], db[3];
-                    prism_plane(k, e[0], e[1], e[2], nb, &bk, dnb, db);
+            for (int sl = 0; sl < 6; ++sl) {
+                double S[6];
 #pragma unroll
-                    for (int p = 0; p < 7; ++p) {
-                        double dnx, dny, dnz, dbk;
-                        if (p < 3) {
-                            dbk = db[p];
-                            dnx = R[0] * dnb[p][0] + R[1] * dnb[p][1] + R[2] * dnb[p][2];
-                            dny = R[3] * dnb[p][0] + R[4] * dnb[p][1] + R[5] * dnb[p][2];
-                            dnz = R[6] * dnb[p][0] + R[7] * dnb[p][1] + R[8] * dnb[p][2];
-                        } else {
-                            dbk = 0.0;
-                            const double* d = dR[p - 3];
-                            dnx = d[0] * nb[0] + d[1] * nb[1] + d[2] * nb[2];
-                            dny = d[3] * nb[0] + d[4] * nb[1] + d[5] * nb[2];
-                            dnz = d[6] * nb[0] + d[7] * nb[1] + d[8] * nb[2];
-                        }
-                        acc[p] = fma(gv * sgn, (dbk - dnx * dx - dny * dy - zk * dnz) * inz, acc[p]);
+                for (int m = 0; m < 6; ++m) {
+                    S[m] = mom[6 * sl + m][lane];
+#pragma unroll
+                    for (int d = 16; d > 0; d >>= 1) S[m] += __shfl_xor_sync(0xffffffffu, S[m], d);
+                }
+                if ((vmask >> sl) & 1u) continue;                // vertical slabs bound the silhouette only
+                double nb[3], bk, dnb[3][3], db[3];
+                prism_plane(slabA[sl], e[0], e[1], e[2], nb, &bk, dnb, db);
+                const double nz = R[6] * nb[0] + R[7] * nb[1] + R[8] * nb[2];
+                const double sg = nz > 0.0 ? 1.0 : -1.0, ianz = 1.0 / fabs(nz);
+                const double Sze = sc[sl] * S[0] - su[sl] * S[1] - sv[sl] * S[2];      // sum G z over the exit set
+                const double Szf = -sc[sl] * S[3] - su[sl] * S[4] - sv[sl] * S[5];     // ... over the entry set
+#pragma unroll
+                for (int p = 0; p < 7; ++p) {
+                    double dnx, dny, dnz, dbk;                   // derivatives of plane A's normal and offset
+                    if (p < 3) {
+                        dbk = db[p];
+                        dnx = R[0] * dnb[p][0] + R[1] * dnb[p][1] + R[2] * dnb[p][2];
+                        dny = R[3] * dnb[p][0] + R[4] * dnb[p][1] + R[5] * dnb[p][2];
+                        dnz = R[6] * dnb[p][0] + R[7] * dnb[p][1] + R[8] * dnb[p][2];
+                    } else {
+                        dbk = 0.0;
+                        const double* d = dR[p - 3];
+                        dnx = d[0] * nb[0] + d[1] * nb[1] + d[2] * nb[2];
+                        dny = d[3] * nb[0] + d[4] * nb[1] + d[5] * nb[2];
+                        dnz = d[6] * nb[0] + d[7] * nb[1] + d[8] * nb[2];
                     }
+                    // exit plane E = sg A (n_E,z = |n_z|):  sum G dz_E = (db S0 - sg Xe) / |n_z|;  entry plane F = -sg A (n_F,z = -|n_z|):
+                    // -sum G dz_F = (db S0' + sg Xf) / |n_z|
+                    const double Xe = dnx * S[1] + dny * S[2] + dnz * Sze, Xf = dnx * S[4] + dny * S[5] + dnz * Szf;
+                    acc[p] = fma(dbk * (S[0] + S[3]) + sg * (Xf - Xe), ianz, acc[p]);
                 }
             }
         }
     }
+    if (lane == 0) {
 #pragma unroll
-    for (int p = 0; p < 7; ++p) {
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) acc[p] += __shfl_xor_sync(0xffffffffu, acc[p], d);
-        if (lane == 0) a.gpar[(size_t)n * 7 + p] = (float)(dn_idx * acc[p]);
+        for (int p = 0; p < 7; ++p) a.gpar[(size_t)n * 7 + p] = (float)(dn_idx * acc[p]);
     }
 }
 
@@ -1300,7 +1361,7 @@ cudaError_t launch_backward_params(osog_ctx* c, const osog_particles* p, long lo
     a.recs = c->rec; a.tbox = c->tbox; a.pframe = c->pframe; a.N = N; a.H = c->H; a.W = c->W;
     a.pitch = pitch; a.n_medium = n_medium; a.gopd = d_gopd; a.gpar = d_gpar;
     const long long threads = N * 32;
-    k_backward_params<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(a);
+    k_backward_params<<<(unsigned)((threads + kPgThreads - 1) / kPgThreads), kPgThreads, 0, c->stream>>>(a);
     return cudaGetLastError();
 }
 
