@@ -14,6 +14,8 @@
 //      the re-based coefficients (packed fp32 FMA and 3-input min/max for the prism slabs, two-float fp32 quadratic + fp32
 //      sqrt for the ellipsoid), OPD accumulated per pixel in fp32 partial sums that are flushed to fp64 registers,
 //   5. write OPD and / or exp(i 2 pi OPD / lambda) * ramp straight from the registers.
+#include <type_traits>
+
 #include "osog_internal.cuh"
 
 namespace osog {
@@ -1029,47 +1031,54 @@ __global__ void __launch_bounds__(256) k_backward_np(const float* __restrict__ r
         const double* c = reinterpret_cast<const double*>(rec + 4);
         const int bw = j1 - j0 + 1, np = bw * (i1 - i0 + 1);
         const float* g = gopd + (size_t)pframe[n] * H * W;
-        for (int q = lane; q < np; q += 32) {
-            const int i = i0 + q / bw, j = j0 + q % bw;
-            const double dj = (double)(j - h3.x), di = (double)(i - h3.y);
-            double t;
-            if (flags & kFlagPrism) {
-                t = prism_t64(c, flags >> 16, dj, di);
-            } else {
-                const double w = c[5] - fma(fma(c[0], dj, fma(c[1], di, c[3])), dj, fma(c[2], di, c[4]) * di);
-                t = c[11] * sqrt(fmax(w, 0.0));                  // T0 sqrt(w)
+        int i = i0 + lane / bw, j = j0 + lane % bw;
+        if (flags & kFlagPrism) {
+            double2 uv[6], xn[6];                                // the record's slabs in registers for the whole walk
+#pragma unroll
+            for (int q = 0; q < 6; ++q) {
+                uv[q] = *reinterpret_cast<const double2*>(c + 4 * q);
+                xn[q] = *reinterpret_cast<const double2*>(c + 4 * q + 2);
             }
-            acc = fma((double)g[(size_t)i * W + j], t, acc);
+            const uint32_t vmask = flags >> 16;
+            auto walk = [&](auto vert) {                         // vert: the prism has a vertical slab (rare; its tests leave the common loop)
+            for (int q = lane; q < np; q += 32) {
+                const double dj = (double)(j - h3.x), di = (double)(i - h3.y);
+                const double gv = (double)g[(size_t)i * W + j];
+                j += 32;
+                while (j > j1) { j -= bw; ++i; }
+                double ex = 1.0e300, en = -1.0e300;
+                bool out = false;
+#pragma unroll
+                for (int s = 0; s < 6; ++s) {
+                    const double m = fma(uv[s].x, dj, uv[s].y * di);
+                    if (decltype(vert)::value && ((vmask >> s) & 1u)) {
+                        out = out || fabs(m + xn[s].x) > xn[s].y;
+                    } else {
+                        const double e = xn[s].x - m, f = xn[s].y - m;
+                        ex = e < ex ? e : ex;
+                        en = f > en ? f : en;
+                    }
+                }
+                const double t = ex - en;
+                if (!out && t > 0.0) acc = fma(gv, t, acc);
+            }
+            };
+            if (vmask) walk(std::true_type{}); else walk(std::false_type{});
+        } else {
+            const double c0 = c[0], c1 = c[1], c2 = c[2], c3 = c[3], c4 = c[4], c5 = c[5], T0 = c[11];
+            for (int q = lane; q < np; q += 32) {
+                const double dj = (double)(j - h3.x), di = (double)(i - h3.y);
+                const double gv = (double)g[(size_t)i * W + j];
+                j += 32;
+                while (j > j1) { j -= bw; ++i; }
+                const double w = c5 - fma(fma(c0, dj, fma(c1, di, c3)), dj, fma(c2, di, c4) * di);
+                acc = fma(gv, T0 * sqrt(fmax(w, 0.0)), acc);     // T0 sqrt(w)
+            }
         }
     }
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
     if (lane == 0) gnp[n] = (float)acc;
-}
-
-// Gradient of a prism's thickness in the pixel offsets (dj, di), fp64 from the record: t = exit - enter on the active
-// planes (arg min / arg max), exit_k = Cx_k - U_k dj - V_k di, so dt/ddj = -(U_e - U_f), dt/ddi = -(V_e - V_f); 0 where
-// the chord is empty.
-__device__ __forceinline__ void prism_grad64(const double* r64, uint32_t vmask, double dj, double di, double* gj, double* gi)
-{
-    double ex = 1.0e300, en = -1.0e300, ue = 0.0, ve = 0.0, uf = 0.0, vf = 0.0;
-    bool out = false;
-#pragma unroll
-    for (int q = 0; q < 6; ++q) {
-        const double2 uv = *reinterpret_cast<const double2*>(r64 + 4 * q);
-        const double2 xn = *reinterpret_cast<const double2*>(r64 + 4 * q + 2);
-        const double m = fma(uv.x, dj, uv.y * di);
-        if ((vmask >> q) & 1u) {
-            out = out || fabs(m + xn.x) > xn.y;
-        } else {
-            const double e = xn.x - m, n = xn.y - m;
-            if (e < ex) { ex = e; ue = uv.x; ve = uv.y; }
-            if (n > en) { en = n; uf = uv.x; vf = uv.y; }
-        }
-    }
-    const bool hit = !out && ex - en > 0.0;
-    *gj = hit ? uf - ue : 0.0;
-    *gi = hit ? vf - ve : 0.0;
 }
 
 // Second step: dL/d(cx, cy)[n] = -(n_p - n_m) sum_px G[px] grad t_n[px].  Same gather as k_backward_np; the gradient in
@@ -1080,8 +1089,9 @@ __global__ void __launch_bounds__(256) k_backward_centre(const float* __restrict
                                                          double inv_pitch, const float* __restrict__ gopd,
                                                          float2* __restrict__ gc)
 {
+    __shared__ double2 s_uv[256 / 32][6];                        // per warp: (U, V) of the prism's slabs, looked up by active-slab index
     const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     if (n >= N) return;
     double ax = 0.0, ay = 0.0, scale = 0.0;
     if (tbox[n].x <= tbox[n].y) {
@@ -1095,21 +1105,59 @@ __global__ void __launch_bounds__(256) k_backward_centre(const float* __restrict
         const int bw = j1 - j0 + 1, np = bw * (i1 - i0 + 1);
         const float* g = gopd + (size_t)pframe[n] * H * W;
         scale = -(double)h2.y * inv_pitch;                       // -dn / p  (ellipsoid: -dn T0 / p, T0 folded in below)
-        for (int q = lane; q < np; q += 32) {
-            const int i = i0 + q / bw, j = j0 + q % bw;
-            const double dj = (double)(j - h3.x), di = (double)(i - h3.y);
-            double gj, gi;
-            if (flags & kFlagPrism) {
-                prism_grad64(c, flags >> 16, dj, di, &gj, &gi);
-            } else {
-                const double w = c[5] - fma(fma(c[0], dj, fma(c[1], di, c[3])), dj, fma(c[2], di, c[4]) * di);
-                const double r = w > 0.0 ? 0.5 * rsqrt(w) : 0.0;  // (the record's K = dn T0 supplies T0)
-                gj = -(2.0 * c[0] * dj + c[1] * di + c[3]) * r;
-                gi = -(c[1] * dj + 2.0 * c[2] * di + c[4]) * r;
+        int i = i0 + lane / bw, j = j0 + lane % bw;
+        if (flags & kFlagPrism) {
+            double2 uv[6], xn[6];                                // the record's slabs in registers for the whole walk
+#pragma unroll
+            for (int q = 0; q < 6; ++q) {
+                uv[q] = *reinterpret_cast<const double2*>(c + 4 * q);
+                xn[q] = *reinterpret_cast<const double2*>(c + 4 * q + 2);
             }
-            const double gv = (double)g[(size_t)i * W + j];
-            ax = fma(gv, gj, ax);
-            ay = fma(gv, gi, ay);
+            const uint32_t vmask = flags >> 16;
+            if (lane < 6) s_uv[wid][lane] = *reinterpret_cast<const double2*>(c + 4 * lane);
+            __syncwarp();
+            auto walk = [&](auto vert) {                         // vert: the prism has a vertical slab (rare; its tests leave the common loop)
+            for (int q = lane; q < np; q += 32) {
+                const double dj = (double)(j - h3.x), di = (double)(i - h3.y);
+                const double gv = (double)g[(size_t)i * W + j];
+                j += 32;
+                while (j > j1) { j -= bw; ++i; }
+                // t = exit - enter on the active planes (arg min / arg max), exit_k = Cx_k - U_k dj - V_k di:
+                // dt/ddj = -(U_e - U_f), dt/ddi = -(V_e - V_f); 0 where the chord is empty
+                double ex = 1.0e300, en = -1.0e300;
+                int ke = 0, kf = 0;                              // active slabs (their slopes are looked up in shared memory)
+                bool out = false;
+#pragma unroll
+                for (int s = 0; s < 6; ++s) {
+                    const double m = fma(uv[s].x, dj, uv[s].y * di);
+                    if (decltype(vert)::value && ((vmask >> s) & 1u)) {
+                        out = out || fabs(m + xn[s].x) > xn[s].y;
+                    } else {
+                        const double e = xn[s].x - m, f = xn[s].y - m;
+                        if (e < ex) { ex = e; ke = s; }
+                        if (f > en) { en = f; kf = s; }
+                    }
+                }
+                if (!out && ex - en > 0.0) {
+                    const double2 se = s_uv[wid][ke], sf = s_uv[wid][kf];
+                    ax = fma(gv, sf.x - se.x, ax);
+                    ay = fma(gv, sf.y - se.y, ay);
+                }
+            }
+            };
+            if (vmask) walk(std::true_type{}); else walk(std::false_type{});
+        } else {
+            const double c0 = c[0], c1 = c[1], c2 = c[2], c3 = c[3], c4 = c[4], c5 = c[5];
+            for (int q = lane; q < np; q += 32) {
+                const double dj = (double)(j - h3.x), di = (double)(i - h3.y);
+                const double gv = (double)g[(size_t)i * W + j];
+                j += 32;
+                while (j > j1) { j -= bw; ++i; }
+                const double w = c5 - fma(fma(c0, dj, fma(c1, di, c3)), dj, fma(c2, di, c4) * di);
+                const double r = w > 0.0 ? 0.5 * rsqrt(w) : 0.0;  // (the record's K = dn T0 supplies T0)
+                ax = fma(gv, -(2.0 * c0 * dj + c1 * di + c3) * r, ax);
+                ay = fma(gv, -(c1 * dj + 2.0 * c2 * di + c4) * r, ay);
+            }
         }
     }
 #pragma unroll
@@ -1278,6 +1326,7 @@ __global__ void __launch_bounds__(kPgThreads, 4) k_backward_params(const ParamGr
 #pragma unroll
             for (int m = 0; m < 36; ++m) mom[m][lane] = 0.0;
             int i = i0 + lane / bw, j = j0 + lane % bw;
+            auto walk = [&](auto vert) {                         // vert: the prism has a vertical slab (rare)
             for (int q = lane; q < np; q += 32) {
                 const double dx = (j + 0.5) * a.pitch - cx, dy = (i + 0.5) * a.pitch - cy;
                 const double gv = (double)g[(size_t)i * a.W + j];
@@ -1289,7 +1338,7 @@ __global__ void __launch_bounds__(kPgThreads, 4) k_backward_params(const ParamGr
 #pragma unroll
                 for (int sl = 0; sl < 6; ++sl) {
                     const double m = fma(su[sl], dx, sv[sl] * dy);
-                    if ((vmask >> sl) & 1u) {
+                    if (decltype(vert)::value && ((vmask >> sl) & 1u)) {
                         out = out || fabs(m) > sc[sl];
                     } else {
                         const double ze = sc[sl] - m, zn = -sc[sl] - m;
@@ -1304,6 +1353,8 @@ __global__ void __launch_bounds__(kPgThreads, 4) k_backward_params(const ParamGr
                 me[0] += gv; me[32] += gx; me[64] += gy;
                 mf[0] += gv; mf[32] += gx; mf[64] += gy;
             }
+            };
+            if (vmask) walk(std::true_type{}); else walk(std::false_type{});
             __syncwarp();
             // the 36 moments summed over the lanes (shuffle tree: a fixed order), then the parameters, slab by slab
 #pragma unroll
