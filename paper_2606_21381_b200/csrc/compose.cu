@@ -864,12 +864,13 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
             const uint32_t vmask = flags >> 16;
             double ex[4] = {1.0e300, 1.0e300, 1.0e300, 1.0e300}, en[4] = {-1.0e300, -1.0e300, -1.0e300, -1.0e300};
             bool out[4] = {false, false, false, false};
+            auto slabs = [&](auto vert) {                        // vert: the prism has a vertical slab (rare; its tests leave the common code)
 #pragma unroll
             for (int sl = 0; sl < 6; ++sl) {
                 const double2 uv = *reinterpret_cast<const double2*>(c + 4 * sl);
                 const double2 xn = *reinterpret_cast<const double2*>(c + 4 * sl + 2);
                 const double r = uv.y * di;
-                if ((vmask >> sl) & 1u) {                        // vertical slab (warp-uniform branch)
+                if (decltype(vert)::value && ((vmask >> sl) & 1u)) {   // vertical slab (warp-uniform branch)
 #pragma unroll
                     for (int q = 0; q < 4; ++q) out[q] = out[q] || fabs(fma(uv.x, dj0 + (double)q, r) + xn.x) > xn.y;
                 } else {
@@ -884,6 +885,8 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
                     }
                 }
             }
+            };
+            if (vmask) slabs(std::true_type{}); else slabs(std::false_type{});
 #pragma unroll
             for (int q = 0; q < 4; ++q) { hit[q] = !out[q] && ex[q] - en[q] > 0.0; zx[q] = ex[q]; }
         } else {
