@@ -143,7 +143,7 @@ __device__ __noinline__ double prism_t64(const double* r64, uint32_t vmask, doub
 
 // ---- preparation of one prism survivor by ONE lane (32 survivors are prepared at once, one per lane) --------------------
 // Evaluation classes of a prepared survivor:
-constexpr uint32_t kClsFull = 1u /* 1 + steep slabs: 1, 2, 3 */, kClsF64 = 4u, kClsPair = 5u, kClsNone = 7u;
+constexpr uint32_t kClsFull = 1u /* 1 + steep slabs: 1, 2, 3 */, kClsF64 = 4u, kClsPair = 5u, kClsLin = 6u, kClsNone = 7u;
 // For each of the 6 slabs: re-base its coefficients from the particle's reference pixel (jc, ic) to the warp's sub-tile
 // origin (wx0, wy0) and round to fp32 there: all later fp32 arithmetic uses pixel offsets 0..15 / 0..7 (DESIGN.md section
 // 6).  The re-basing itself runs in fp32 on the record's exact-grid (hi, lo) pairs (k_prepare; already scaled by the
@@ -210,6 +210,11 @@ __device__ __forceinline__ uint32_t prep_prism(float4* __restrict__ slot, const 
     if ((mx | mn) & ((1u << ns) - 1u)) return kClsFull + (uint32_t)ns; // a steep plane matters here: lo-part classes
     if (__popc(mx) > 2 || __popc(mn) > 2) return kClsFull;
     const int a0 = __ffs(mx) - 1, c0 = __ffs(mn) - 1;
+    if (__popc(mx) == 1 && __popc(mn) == 1) {                          // one exit and one entry plane: s t is one plane, clamped
+        const float4 sa = slot[a0], sc = slot[c0];
+        slot[7] = make_float4(sa.x - sc.y, sa.z - sc.z, sa.w - sc.w, 0.0f);
+        return kClsLin;
+    }
     const uint32_t mx1 = mx & (mx - 1u), mn1 = mn & (mn - 1u);
     const int a1 = mx1 ? __ffs(mx1) - 1 : a0, c1 = mn1 ? __ffs(mn1) - 1 : c0;      // a single plane is simply used twice
     const float4 sa = slot[a0], sb = slot[a1], sc = slot[c0], sd = slot[c1];
@@ -334,6 +339,23 @@ __device__ __forceinline__ void eval_prism_pair(const float4* __restrict__ slot,
         const float2 e = ffma2(xu, g.nlx[k], xr), n = ffma2(nu, g.nlx[k], nr);
         pend[k] = fmaf(sub_sat(fminf(e.x, e.y), fmaxf(n.x, n.y)), dn, pend[k]);
     }
+}
+
+// Prism of which one exit and one entry plane can be active in this sub-tile: s t = sat(D - Du lx - Dv ly), one saturating
+// FMA per pixel.
+__device__ __forceinline__ float ffma_sat(float a, float b, float c)
+{
+    float d;
+    asm("fma.rn.sat.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
+}
+__device__ __forceinline__ void eval_prism_lin(const float4* __restrict__ slot, const LaneGeom& g, float (&pend)[4])
+{
+    const float4 a = slot[7];
+    const float dn = slot[6].y;
+    const float r = fmaf(a.z, g.nly.x, a.x);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) pend[k] = fmaf(ffma_sat(a.y, g.nlx[k].x, r), dn, pend[k]);
 }
 
 // The evaluation loops add into fp32 partial sums; every kFlush survivors (and at the end of a class) these are widened
@@ -615,6 +637,7 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
                     cls = prep_prism(sl, recs4 + (size_t)spid * (kRecWords / 4),
                                      reinterpret_cast<const float4*>(a.rec2 + (size_t)spid * kPairWords), wx0, wy0);
             }
+            const unsigned ml = __ballot_sync(0xffffffffu, cls == kClsLin);
             const unsigned mp = __ballot_sync(0xffffffffu, cls == kClsPair);
             const unsigned m1 = __ballot_sync(0xffffffffu, cls == kClsFull);
             const unsigned m2 = __ballot_sync(0xffffffffu, cls == kClsFull + 1u);
@@ -625,6 +648,7 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
             __syncwarp();
             if (32 + lane < nqp) queue_p[lane] = moved;
             nqp -= n;
+            run_class(ml, my_slots, pend, acc, [&](const float4* slot) { eval_prism_lin(slot, g, pend); });
             run_class(mp, my_slots, pend, acc, [&](const float4* slot) { eval_prism_pair(slot, g, pend); });
             run_class(m1, my_slots, pend, acc, [&](const float4* slot) { eval_prism<0>(slot, g, pend); });
             run_class(m2, my_slots, pend, acc, [&](const float4* slot) { eval_prism<1>(slot, g, pend); });
