@@ -845,6 +845,7 @@ __global__ void __launch_bounds__(256) k_compose_atomic(const float* __restrict_
 // NORMAL: also the slope (dz/dx, dz/dy) of the owner's top surface (the analytic height gradient of the visible surface,
 // PAPER.md:76, 92): the active exit plane's -n_x / n_z = -U / p for a prism, the derivative of the upper root of the quadric
 // for an ellipsoid: d/ddj (Z0 + Zx dj + Zy di + T0 sqrt(w) / 2) / p.
+constexpr int kGbCap = 512;                        // longest list that k_gbuffer_tile ranks front to back (10 KB of shared memory)
 template <bool NORMAL>
 __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* __restrict__ recs, const uint32_t* __restrict__ offset,
                                                                 const uint32_t* __restrict__ list, const uint16_t* __restrict__ meta,
@@ -867,9 +868,48 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
     int32_t who[4] = {-1, -1, -1, -1};
     float2 slope[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
     float floor_all = __int_as_float(0xff800000);                // -inf: nothing can be skipped yet
+    // Front to back: the tile's entries are ranked by the upper bound cz + zmax of their tops (descending; ties in list order)
+    // in shared memory, so that a warp can STOP at the first entry whose bound lies below every top it has found, instead of
+    // skipping such entries one by one.  Lists longer than kGbCap keep the list order (the skip test still applies).
+    __shared__ uint32_t s_pid[2][kGbCap];
+    __shared__ float s_key[2][kGbCap];
+    __shared__ uint16_t s_meta[2][kGbCap];
+    const bool sorted = L <= (uint32_t)kGbCap;                   // CTA-uniform
+    if (sorted) {
+        for (uint32_t k = tid; k < L; k += kComposeThreads) {
+            const uint32_t pid = glist[k];
+            const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)pid * kRecWords);
+            const float czf = __ldg(rec + 2).z;
+            const float key = czf + __int_as_float(__ldg(reinterpret_cast<const int4*>(rec + 3)).z);
+            s_pid[0][k] = pid;
+            s_key[0][k] = fabsf(czf) <= 3.402823466e38f ? key : __int_as_float(0xff800000);   // non-finite height: last (and skipped below)
+            s_meta[0][k] = gmeta[k];
+        }
+        __syncthreads();
+        for (uint32_t k = tid; k < L; k += kComposeThreads) {
+            const float key = s_key[0][k];
+            uint32_t r = 0;
+            for (uint32_t q = 0; q < L; ++q) {
+                const float kq = s_key[0][q];
+                r += (kq > key || (kq == key && q < k)) ? 1u : 0u;
+            }
+            s_pid[1][r] = s_pid[0][k];
+            s_key[1][r] = key;
+            s_meta[1][r] = s_meta[0][k];
+        }
+        __syncthreads();
+    }
     for (uint32_t k = 0; k < L; ++k) {
-        if (((gmeta[k] >> wid) & 1u) == 0u) continue;           // warp-uniform
-        const uint32_t pid = glist[k];
+        uint32_t pid, mk;
+        if (sorted) {
+            if (s_key[1][k] < floor_all) break;                  // no later entry can reach any pixel of this warp
+            pid = s_pid[1][k];
+            mk = s_meta[1][k];
+        } else {
+            pid = glist[k];
+            mk = gmeta[k];
+        }
+        if (((mk >> wid) & 1u) == 0u) continue;                  // warp-uniform
         const float4* rec = reinterpret_cast<const float4*>(recs + (size_t)pid * kRecWords);
         const float4 h2 = __ldg(rec + 2);
         const int4 h3 = __ldg(reinterpret_cast<const int4*>(rec + 3));
@@ -931,7 +971,8 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const double top = (double)czf + zx[q];
-            if (hit[q] && (who[q] < 0 || top > best[q])) {
+            // strictly higher, or equally high with the smaller index (front-to-back order does not visit indices ascending)
+            if (hit[q] && (who[q] < 0 || top > best[q] || (top == best[q] && (int32_t)(pid - first) < who[q]))) {
                 best[q] = top; who[q] = (int32_t)(pid - first);
                 if (NORMAL) slope[q] = make_float2((float)(sxs[q] * inv_pitch), (float)(sys[q] * inv_pitch));
             }
