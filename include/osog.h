@@ -43,10 +43,11 @@
 extern "C" {
 #endif
 
-#define OSOG_API_VERSION 5   /* 2: osog_optics.defocus_um, osog_dic, osog_render_dic, osog_field_to_dic
+#define OSOG_API_VERSION 6   /* 2: osog_optics.defocus_um, osog_dic, osog_render_dic, osog_field_to_dic
                                 3: max_pairs is a TOTAL capacity (device scan + CSR lists), osog_status reports the exact need
                                 4: osog_optics.shot_noise_photons (Poisson shot noise), osog_debug_poisson, osog_debug_check_guards
-                                5: osog_optics.topography_amplitude (micro-topography), brightfield, backward_params, spectral loss */
+                                5: osog_optics.topography_amplitude (micro-topography), brightfield, backward_params, spectral loss
+                                6: osog_backward_particles */
 
 enum {
     OSOG_OK = 0,
@@ -246,6 +247,15 @@ int osog_backward_centre(osog_ctx* ctx, const osog_particles* p, int64_t N, cons
  * of a prism) and shares the caveat of osog_backward_centre for ellipsoids (it grows like 1 / sqrt(w) at the outline).
  * Works from the particle columns in fp64, same fixed-order gather as osog_backward_np. */
 int osog_backward_params(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gpar);
+
+/* The three gathers above in ONE pass over the pixels (the gradient "with respect to the initial state tensor"):
+ * d_gnp [N], d_gc [N, 2], d_gpar [N, 7] as defined for osog_backward_np / _centre / _params; any of them may be NULL, not all.
+ * dt/dtheta, grad t and t itself are linear in a few per-pixel quantities, so the pixel walk only accumulates moments (per active
+ * exit / entry plane of a prism: sum of G (1, dx, dy); for an ellipsoid: sum of G / sqrt(disc) times (1, dx, dy, dx^2, dx dy,
+ * dy^2) and sum of G sqrt(disc)) and all ten gradients are formed once per particle.  fp64, fixed order (reproducible bits); the
+ * values agree with the separate calls up to the rounding of a different fp64 summation order.  Same argument checks. */
+int osog_backward_particles(osog_ctx* ctx, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd,
+                            float* d_gnp, float* d_gc, float* d_gpar);
 
 /* Spectral loss of Eq. 8 (reading A28) and its gradient in the image: for every frame b,
  * d_loss[b] = sum over all FFT bins of (log(|F(I_b)| + eps) - log(|F(T_b)| + eps))^2 (DEVICE double [B]), F the unnormalised

@@ -87,6 +87,7 @@ def lib():
     L.osog_backward_intensity.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_spectral_loss.argtypes = [ctx, C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
     L.osog_backward_params.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
+    L.osog_backward_particles.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     L.osog_backward_centre.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_gbuffer.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p]
     L.osog_render_gbuffer_normals.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p,
@@ -111,7 +112,7 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_brightfield", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_gbuffer_normals", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_params", "osog_spectral_loss", "osog_backward_intensity", "osog_debug_recompose_field", "osog_debug_check_guards", "osog_debug_poisson", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_brightfield", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_gbuffer_normals", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_params", "osog_backward_particles", "osog_spectral_loss", "osog_backward_intensity", "osog_debug_recompose_field", "osog_debug_check_guards", "osog_debug_poisson", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
@@ -315,6 +316,19 @@ class Context:
         self._done(lib().osog_backward_params(self._ctx, C.byref(p.c), p.N, C.byref(o), gopd.data_ptr(), out.data_ptr()),
                    "osog_backward_params")
         return out
+
+    def backward_particles(self, p: Particles, o, gopd, np_=True, centre=True, params=True):
+        """(float32 [N] dL/dn_p, float32 [N, 2] dL/d(cx, cy), float32 [N, 7] dL/d(d0, d1, d2, qw, qx, qy, qz)) from ONE pass over
+        the pixels; an output that is switched off is None (osog_backward_particles)."""
+        t = self.torch
+        gnp = t.empty((p.N,), dtype=t.float32, device=self.device) if np_ else None
+        gc = t.empty((p.N, 2), dtype=t.float32, device=self.device) if centre else None
+        gpar = t.empty((p.N, 7), dtype=t.float32, device=self.device) if params else None
+        gopd = self._in(gopd, (o.B, self.H, self.W), "gopd")
+        ptr = lambda x: x.data_ptr() if x is not None else None
+        self._done(lib().osog_backward_particles(self._ctx, C.byref(p.c), p.N, C.byref(o), gopd.data_ptr(), ptr(gnp), ptr(gc), ptr(gpar)),
+                   "osog_backward_particles")
+        return gnp, gc, gpar
 
     def spectral_loss(self, I, I_target, eps, grad=True):
         """(float64 [B] loss of Eq. 8, float32 [B, H, W] dL/dI or None) for images I, I_target (float32 [B, H, W]) (osog_spectral_loss)."""

@@ -1255,7 +1255,9 @@ struct ParamGradArgs {
     int H, W;
     double pitch, n_medium;
     const float* gopd;
-    float* gpar;                  // [N][7]
+    float* gpar;                  // [N][7], or nullptr
+    float* gnp;                   // [N] dL/dn_p, or nullptr    (osog_backward_particles: the same moments give all three)
+    float2* gc;                   // [N] dL/d(cx, cy), or nullptr
 };
 
 // body-frame plane k of the capped prism (0, 1: +-x; 2, 3: +-y; 4..7: (+-hc, 0, +-s/2); 8..11: (0, +-hc, +-s/2)) and its
@@ -1298,6 +1300,7 @@ __global__ void __launch_bounds__(kPgThreads, 4) k_backward_params(const ParamGr
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     if (n >= a.N) return;
     double acc[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    double gt = 0.0, gcx = 0.0, gcy = 0.0;          // sum G t, sum G dt/dcx, sum G dt/dcy
     double dn_idx = 0.0;
     if (a.tbox[n].x <= a.tbox[n].y) {              // listed: valid and on the canvas (else the gradient is 0)
         const float4* rec = reinterpret_cast<const float4*>(a.recs + (size_t)n * kRecWords);
@@ -1327,7 +1330,7 @@ __global__ void __launch_bounds__(kPgThreads, 4) k_backward_params(const ParamGr
 #pragma unroll
                 for (int k = 0; k < 3; ++k) M[c] += R[3 * ra[c] + k] * D[k] * R[3 * rb[c] + k];
             }
-            double m0 = 0.0, mxx = 0.0, mxy = 0.0, myy = 0.0, ms = 0.0;
+            double m0 = 0.0, mxx = 0.0, mxy = 0.0, myy = 0.0, ms = 0.0, mx = 0.0, my = 0.0;
             int i = i0 + lane / bw, j = j0 + lane % bw;
             for (int q = lane; q < np; q += 32) {
                 const double dx = (j + 0.5) * a.pitch - cx, dy = (i + 0.5) * a.pitch - cy;
@@ -1344,6 +1347,8 @@ __global__ void __launch_bounds__(kPgThreads, 4) k_backward_params(const ParamGr
                 mxy = fma(wq, dx * dy, mxy);
                 myy = fma(wq, dy * dy, myy);
                 ms = fma(gv, sq, ms);
+                mx = fma(wq, dx, mx);
+                my = fma(wq, dy, my);
             }
 #pragma unroll
             for (int d = 16; d > 0; d >>= 1) {
@@ -1352,9 +1357,16 @@ __global__ void __launch_bounds__(kPgThreads, 4) k_backward_params(const ParamGr
                 mxy += __shfl_xor_sync(0xffffffffu, mxy, d);
                 myy += __shfl_xor_sync(0xffffffffu, myy, d);
                 ms += __shfl_xor_sync(0xffffffffu, ms, d);
+                mx += __shfl_xor_sync(0xffffffffu, mx, d);
+                my += __shfl_xor_sync(0xffffffffu, my, d);
             }
             const double A = M[5], iA = 1.0 / A;
             const double qC = M[0] * mxx + 2.0 * M[1] * mxy + M[2] * myy - m0;                       // <C>
+            // t = 2 sqrt(disc) / A;  d(disc)/dcx = -2 M_xz Bq + 2 A (M_xx dx + M_xy dy)  (dx = x - cx)
+            const double qB = M[3] * mx + M[4] * my;                                                 // <Bq>
+            gt = 2.0 * ms * iA;
+            gcx = 2.0 * (A * (M[0] * mx + M[1] * my) - M[3] * qB) * iA;
+            gcy = 2.0 * (A * (M[1] * mx + M[2] * my) - M[4] * qB) * iA;
 #pragma unroll
             for (int p = 0; p < 7; ++p) {
                 double dM[6];
@@ -1441,6 +1453,9 @@ __global__ void __launch_bounds__(kPgThreads, 4) k_backward_params(const ParamGr
                 const double sg = nz > 0.0 ? 1.0 : -1.0, ianz = 1.0 / fabs(nz);
                 const double Sze = sc[sl] * S[0] - su[sl] * S[1] - sv[sl] * S[2];      // sum G z over the exit set
                 const double Szf = -sc[sl] * S[3] - su[sl] * S[4] - sv[sl] * S[5];     // ... over the entry set
+                gt += Sze - Szf;                                  // t = z_exit - z_entry
+                gcx = fma(su[sl], S[0] - S[3], gcx);              // dz/dcx = +u for both planes of the slab (dx = x - cx)
+                gcy = fma(sv[sl], S[0] - S[3], gcy);
 #pragma unroll
                 for (int p = 0; p < 7; ++p) {
                     double dnx, dny, dnz, dbk;                   // derivatives of plane A's normal and offset
@@ -1465,13 +1480,17 @@ __global__ void __launch_bounds__(kPgThreads, 4) k_backward_params(const ParamGr
         }
     }
     if (lane == 0) {
+        if (a.gpar != nullptr) {
 #pragma unroll
-        for (int p = 0; p < 7; ++p) a.gpar[(size_t)n * 7 + p] = (float)(dn_idx * acc[p]);
+            for (int p = 0; p < 7; ++p) a.gpar[(size_t)n * 7 + p] = (float)(dn_idx * acc[p]);
+        }
+        if (a.gnp != nullptr) a.gnp[n] = (float)gt;
+        if (a.gc != nullptr) a.gc[n] = make_float2((float)(dn_idx * gcx), (float)(dn_idx * gcy));
     }
 }
 
 cudaError_t launch_backward_params(osog_ctx* c, const osog_particles* p, long long N, double pitch, double n_medium,
-                                   const float* d_gopd, float* d_gpar)
+                                   const float* d_gopd, float* d_gpar, float* d_gnp, float* d_gc)
 {
     if (N == 0) return cudaSuccess;
     ParamGradArgs a;
@@ -1479,6 +1498,7 @@ cudaError_t launch_backward_params(osog_ctx* c, const osog_particles* p, long lo
     a.d0 = p->d0; a.d1 = p->d1; a.d2 = p->d2; a.n_p = p->n_p; a.kind = p->kind;
     a.recs = c->rec; a.tbox = c->tbox; a.pframe = c->pframe; a.N = N; a.H = c->H; a.W = c->W;
     a.pitch = pitch; a.n_medium = n_medium; a.gopd = d_gopd; a.gpar = d_gpar;
+    a.gnp = d_gnp; a.gc = reinterpret_cast<float2*>(d_gc);
     const long long threads = N * 32;
     k_backward_params<<<(unsigned)((threads + kPgThreads - 1) / kPgThreads), kPgThreads, 0, c->stream>>>(a);
     return cudaGetLastError();

@@ -560,6 +560,25 @@ int osog_backward_params(osog_ctx* c, const osog_particles* p, int64_t N, const 
     return OSOG_OK;
 }
 
+int osog_backward_particles(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, const float* d_gopd, float* d_gnp,
+                            float* d_gc, float* d_gpar)
+{
+    if (!d_gopd || !aligned16(d_gopd)) return OSOG_EINVAL;
+    float* first = d_gnp ? d_gnp : (d_gc ? d_gc : d_gpar);       // at least one output
+    if (!first) return OSOG_EINVAL;
+    if (d_gc && (reinterpret_cast<uintptr_t>(d_gc) & 7u)) return OSOG_EINVAL;
+    if (N == 0) return (c && p && o) ? OSOG_OK : OSOG_EINVAL;
+    const int r = check_call(c, p, N, o, first);
+    if (r != OSOG_OK) return r;
+    if (o->topography_amplitude != 0.0) return OSOG_EINVAL;   // the gathers differentiate the smooth bodies (see osog.h)
+    DeviceGuard g(c->device);
+    cudaError_t e = launch_binning(c, p, N, o);      // tile ranges, frames and pixel bounding boxes (the tile lists are not used)
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = launch_backward_params(c, p, N, o->pitch_um, o->n_medium, d_gopd, d_gpar, d_gnp, d_gc);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return OSOG_OK;
+}
+
 int osog_render_opd_smem_atomic(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd)
 {
     const int r = check_call(c, p, N, o, d_opd);

@@ -161,7 +161,7 @@ cudaError_t launch_compose_smem_atomic(osog_ctx* c, int B, float* d_opd);
 cudaError_t launch_backward_np(osog_ctx* c, long long N, const float* d_gopd, float* d_gnp);
 cudaError_t launch_backward_centre(osog_ctx* c, long long N, double pitch, const float* d_gopd, float* d_gc);
 cudaError_t launch_backward_params(osog_ctx* c, const osog_particles* p, long long N, double pitch, double n_medium,
-                                   const float* d_gopd, float* d_gpar);
+                                   const float* d_gopd, float* d_gpar, float* d_gnp = nullptr, float* d_gc = nullptr);
 cudaError_t launch_gbuffer(osog_ctx* c, int B, const int32_t* d_frame_start, double pitch, int32_t* d_top_id, float* d_depth,
                            float* d_normal);
 // optics.cu

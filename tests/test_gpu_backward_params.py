@@ -144,3 +144,35 @@ def test_gathers_refuse_micro_topography(og):
             call(P, opt, G)
         assert e.value.code == og.OSOG_EINVAL
     ctx.close()
+
+
+@pytest.mark.parametrize("k,n", [(2, None), (3, 1500), (4, 3000), (5, 240)])
+def test_backward_particles_one_pass_equals_the_three_gathers(og, o, k, n):
+    """osog_backward_particles forms dL/dn_p, dL/d(cx, cy) and dL/d(dims, q) from one set of moments: same numbers as the three
+    separate gathers up to a different float64 summation order, and the same bars against the oracle."""
+    import torch
+    sc = make_config(k, n_override=n)
+    rng = np.random.default_rng(70 + k)
+    G = rng.standard_normal((sc.B, sc.H, sc.W)).astype(np.float32)
+    ctx = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B)
+    P, opt = og.Particles.from_scene(sc), og.optics_from_scene(sc)
+    Gd = torch.from_numpy(G).cuda()
+    gnp, gc, gpar = ctx.backward_particles(P, opt, Gd)
+    again = ctx.backward_particles(P, opt, Gd)
+    assert all(torch.equal(a, b) for a, b in zip((gnp, gc, gpar), again))          # reproducible bits
+    only_c = ctx.backward_particles(P, opt, Gd, np_=False, params=False)
+    assert only_c[0] is None and only_c[2] is None and torch.equal(only_c[1], gc)
+    assert ctx.check_guards() == 0
+    absG = np.abs(G)
+    f64 = lambda t: t.cpu().numpy().astype(np.float64)
+    # dL/dn_p: the bar of test_backward_np_matches_oracle (relative to the sum of magnitudes)
+    ref, scale = o.backward_np(sc, G), o.backward_np(sc, absG)
+    assert np.all(np.abs(f64(gnp) - ref) <= 2e-7 * scale + 1e-6)
+    assert np.all(np.abs(f64(gnp) - f64(ctx.backward_np(P, opt, Gd))) <= 2e-7 * scale + 1e-6)
+    # dL/d(cx, cy) and dL/d(dims, q): the bars of their own parity tests (per particle, relative to the largest component's scale)
+    for got, sep, fn in ((gc, ctx.backward_centre(P, opt, Gd), o.backward_centre), (gpar, ctx.backward_params(P, opt, Gd), o.backward_params)):
+        ref = fn(sc, G)
+        big = np.maximum((np.abs(fn(sc, absG)) + np.abs(ref)).max(axis=1, keepdims=True), 1.0)
+        assert np.all(np.abs(f64(got) - ref) <= 5e-7 * big), float((np.abs(f64(got) - ref) / big).max())
+        assert np.all(np.abs(f64(got) - f64(sep)) <= 5e-7 * big), float((np.abs(f64(got) - f64(sep)) / big).max())
+    ctx.close()
