@@ -77,14 +77,6 @@ __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c)
     asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
     return d;
 }
-// float -> double (exact widening) with integer ops on the ALU pipe instead of an XU-pipe conversion (F2F, 8 cycles per
-// warp).  f must be normal or zero; +-0.0f maps to +-2^-126 (about 1e-38), harmless for a sum in micrometres.
-__device__ __forceinline__ double f2d(float f)
-{
-    const uint32_t u = __float_as_uint(f);
-    const uint32_t hi = (((u & 0x7fffffffu) >> 3) + 0x38000000u) | (u & 0x80000000u);
-    return __hiloint2double((int)hi, (int)(u << 29));
-}
 // saturating fp32 add / subtract: the result is clamped to [0, 1] by the FMA pipe (NaN -> 0), no separate min / max
 __device__ __forceinline__ float sub_sat(float a, float b)
 {
@@ -97,28 +89,6 @@ __device__ __forceinline__ float add_sat(float a, float b)
     float r;
     asm("add.sat.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
     return r;
-}
-// sin(pi x), cos(pi x) for |x| <= 1 (the reduced phase of the write-out, in half turns): k = nearest integer to 2 x,
-// r = x - k / 2 in [-1/4, 1/4], Taylor polynomials of sin(pi r) (through r^9) and cos(pi r) (through r^8): truncation
-// errors 2e-9 and 2.5e-8, far below the fp32 rounding of the result; then the quadrant rotation by k.
-__device__ __forceinline__ void sincospi_unit(float x, float* sn, float* cs)
-{
-    const float kf = rintf(x + x);
-    const int k = (int)kf;
-    const float r = fmaf(kf, -0.5f, x);
-    const float r2 = r * r;
-    float sp = fmaf(r2, 0.0821458866f, -0.599264529f);
-    sp = fmaf(r2, sp, 2.55016404f);
-    sp = fmaf(r2, sp, -5.16771278f);
-    sp = fmaf(r2, sp, 3.14159265f) * r;
-    float cp = fmaf(r2, 0.235330630f, -1.33526277f);
-    cp = fmaf(r2, cp, 4.05871213f);
-    cp = fmaf(r2, cp, -4.93480220f);
-    cp = fmaf(r2, cp, 1.0f);
-    if (k & 1) { const float t = sp; sp = cp; cp = -t; }
-    if (k & 2) { sp = -sp; cp = -cp; }
-    *sn = sp;
-    *cs = cp;
 }
 // ---- fp64 prism evaluation (refinement of flagged pixels, and the atomic variant) -------------------------------------
 // r64: 24 doubles (U, V, Cx, Cn per slab, relative to pixel (jc, ic)); dj, di: pixel offsets from (jc, ic).
@@ -733,7 +703,10 @@ __global__ void __launch_bounds__(kCtaWarps * 32, 4 * kCtaSplit) k_compose_tile(
             ramp_dx = fo->fx0_pitch;
             ramp0 = fma(ramp_dx, (double)j + 0.5, fo->fy0_pitch * ((double)i + 0.5));
         }
-        // packed Horner coefficients of sin(pi r) / r and cos(pi r), |r| <= 1/4
+        // sin(pi x), cos(pi x) for |x| <= 1 (the reduced phase, in half turns): k = nearest integer to 2 x, r = x - k / 2 in
+        // [-1/4, 1/4], Taylor polynomials of sin(pi r) (through r^9) and cos(pi r) (through r^8): truncation errors 2e-9 and
+        // 2.5e-8, far below the fp32 rounding of the result; then the quadrant rotation by k.  Packed Horner coefficients of
+        // sin(pi r) / r and cos(pi r):
         const float2 c3 = make_float2(0.0821458866f, 0.235330630f), c2 = make_float2(-0.599264529f, -1.33526277f);
         const float2 c1 = make_float2(2.55016404f, 4.05871213f), c0 = make_float2(-5.16771278f, -4.93480220f);
         const float2 cc = make_float2(3.14159265f, 1.0f);
