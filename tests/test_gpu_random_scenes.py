@@ -68,3 +68,28 @@ def test_random_scene_matches_oracle_full_mode(og, o, seed):
     assert np.abs(U - Uref).max() <= 1e-4, f"seed {seed}: field {np.abs(U - Uref).max():.3e}"
     oc, oo, ol = o.binning(sc, og.osog_tile_size())
     assert np.array_equal(off, oo) and np.array_equal(lst, ol)
+
+
+@pytest.mark.parametrize("seed", range(0, 24, 3))
+def test_random_scene_gbuffer_and_gradients(og, o, seed):
+    """The same adversarial scenes through the widened calls: depth / instance-id maps (front-to-back ranking, explicit
+    smallest-index rule) and all particle gradients from the one-pass gather, each at the bar of its own parity test."""
+    import torch
+    import test_gpu_gbuffer as G
+    sc = G.with_heights(_scene(seed), seed=500 + seed)
+    G.check(og, o, sc)
+    rng = np.random.default_rng(seed)
+    Gm = rng.standard_normal((sc.B, sc.H, sc.W)).astype(np.float32)
+    ctx = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B)
+    P, opt = og.Particles.from_scene(sc), og.optics_from_scene(sc)
+    gnp, gc, gpar = ctx.backward_particles(P, opt, torch.from_numpy(Gm).cuda())
+    assert ctx.check_guards() == 0
+    ctx.close()
+    absG = np.abs(Gm)
+    f64 = lambda t: t.cpu().numpy().astype(np.float64)
+    ref, scale = o.backward_np(sc, Gm), o.backward_np(sc, absG)
+    assert np.all(np.abs(f64(gnp) - ref) <= 2e-7 * scale + 1e-6)
+    for got, fn in ((gc, o.backward_centre), (gpar, o.backward_params)):
+        ref = fn(sc, Gm)
+        big = np.maximum((np.abs(fn(sc, absG)) + np.abs(ref)).max(axis=1, keepdims=True), 1.0)
+        assert np.all(np.abs(f64(got) - ref) <= 5e-7 * big), float((np.abs(f64(got) - ref) / big).max())
