@@ -43,18 +43,20 @@
 extern "C" {
 #endif
 
-#define OSOG_API_VERSION 6   /* 2: osog_optics.defocus_um, osog_dic, osog_render_dic, osog_field_to_dic
+#define OSOG_API_VERSION 7   /* 2: osog_optics.defocus_um, osog_dic, osog_render_dic, osog_field_to_dic
                                 3: max_pairs is a TOTAL capacity (device scan + CSR lists), osog_status reports the exact need
                                 4: osog_optics.shot_noise_photons (Poisson shot noise), osog_debug_poisson, osog_debug_check_guards
                                 5: osog_optics.topography_amplitude (micro-topography), brightfield, backward_params, spectral loss
-                                6: osog_backward_particles */
+                                6: osog_backward_particles
+                                7: osog_render_opd_static, OSOG_ELIMIT */
 
 enum {
     OSOG_OK = 0,
     OSOG_EINVAL = -1,     /* null / misaligned pointer, bad size, N > max_particles, B > max_frames, bad optics */
     OSOG_ECUDA = -2,      /* CUDA runtime, launch or cuFFT failure (osog_last_cuda_error gives the code)       */
     OSOG_ECAPACITY = -3,  /* the call produced more (particle, tile) pairs in total than max_pairs: its frames are zero-filled */
-    OSOG_ENOMEM = -4      /* allocation failure in osog_create                                                 */
+    OSOG_ENOMEM = -4,     /* allocation failure in osog_create                                                 */
+    OSOG_ELIMIT = -5      /* osog_render_opd_static: more particles, frames or tiles than its fixed scratch holds */
 };
 /* status bits returned by osog_status (sticky until the next render call) */
 #define OSOG_WBADPARTICLE 1u   /* at least one particle was skipped as invalid                    */
@@ -303,6 +305,32 @@ int osog_debug_poisson(osog_ctx* ctx, const float* d_lambda, int64_t n, uint64_t
  * osog_create.  Synchronises and returns the number of guard bands that no longer hold their pattern (0 = no kernel wrote
  * past the end of its scratch), or a negative error code.  (compute-sanitizer is not available on every pool.) */
 int osog_debug_check_guards(osog_ctx* ctx);
+
+/* The hot path for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): osog_render_opd (H1-H6, the same three kernels, the same bits) without a context.  All scratch of the call lives in
+ * ONE file-scope device array of OSOG_STATIC_SCRATCH_BYTES (about 2.5 MB) that every GPU loading the library holds until exit; the
+ * call itself calls no cudaMalloc / cudaFree / cudaMallocHost and no allocating library routine (no cuFFT).  Fixed limits, beyond
+ * which the call returns OSOG_ELIMIT and enqueues nothing:
+ *   N <= OSOG_STATIC_MAX_PARTICLES, o->B <= OSOG_STATIC_MAX_FRAMES, o->B * ceil(H / 32) * ceil(W / 32) <= OSOG_STATIC_MAX_TILES
+ *   (one 512 x 512 frame, four 256 x 256 frames, ...).
+ * A call that produces more than OSOG_STATIC_MAX_PAIRS (particle, tile) pairs zero-fills d_opd and sets OSOG_WOVERFLOW, as
+ * osog_render_opd does beyond max_pairs.
+ * device: CUDA device ordinal (the pointers below live there); stream: cudaStream_t the work is enqueued on (NULL = default).
+ * p, N, o: as for osog_render_opd (DEVICE columns, host structs; read only).  d_opd: DEVICE float [B, H, W], 16-byte aligned,
+ * overwritten.  d_status_bits: DEVICE uint32 [1] or NULL; receives the call's warning bits (OSOG_W*) by a 4-byte
+ * device-to-device copy enqueued behind the kernels (there is no osog_status for this call: read the word after the stream has
+ * finished).  Enqueue-only, never synchronises.
+ * EVERY call on a GPU shares the one array, which keeps the last call's contents: the call first clears what must start at zero
+ * (tile counters, scan ticket, status words; three small memsets on `stream`).  Two calls that OVERLAP on the GPU (different
+ * streams without an ordering between them, or a captured graph replayed concurrently with itself) RACE on the scratch and
+ * produce garbage: order them.  Host threads are serialised by a mutex for the duration of the enqueue only. */
+#define OSOG_STATIC_MAX_PARTICLES 4096
+#define OSOG_STATIC_MAX_FRAMES 4
+#define OSOG_STATIC_MAX_TILES 256
+#define OSOG_STATIC_MAX_PAIRS 65536
+#define OSOG_STATIC_SCRATCH_BYTES (2560 * 1024)
+int osog_render_opd_static(int device, void* stream, int H, int W, const osog_particles* p, int64_t N, const osog_optics* o,
+                           float* d_opd, uint32_t* d_status_bits);
 
 /* Tile edge T in pixels (build-time constant of the binning, B3). */
 int osog_tile_size(void);

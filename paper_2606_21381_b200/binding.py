@@ -13,7 +13,7 @@ import numpy as np
 
 from . import build as _build
 
-OSOG_OK, OSOG_EINVAL, OSOG_ECUDA, OSOG_ECAPACITY, OSOG_ENOMEM = 0, -1, -2, -3, -4
+OSOG_OK, OSOG_EINVAL, OSOG_ECUDA, OSOG_ECAPACITY, OSOG_ENOMEM, OSOG_ELIMIT = 0, -1, -2, -3, -4, -5
 OSOG_WBADPARTICLE, OSOG_WOVERFLOW = 1, 2
 
 _F32_COLS = ("cx", "cy", "cz", "qw", "qx", "qy", "qz", "d0", "d1", "d2", "n_p")
@@ -94,6 +94,8 @@ def lib():
                                               C.c_void_p]
     L.osog_render_height.argtypes = [ctx, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics), C.c_void_p, C.c_void_p,
                                      C.c_void_p]
+    L.osog_render_opd_static.argtypes = [C.c_int, C.c_void_p, C.c_int, C.c_int, C.POINTER(osog_particles), C.c_int64, C.POINTER(osog_optics),
+                                         C.c_void_p, C.c_void_p]
     L.osog_debug_recompose_field.argtypes = [ctx, C.c_void_p]
     L.osog_debug_check_guards.argtypes = [ctx]
     L.osog_debug_poisson.argtypes = [ctx, C.c_void_p, C.c_int64, C.c_uint64, C.c_uint32, C.c_void_p]
@@ -112,12 +114,35 @@ def lib():
 
 
 EXPORTS = ("osog_create", "osog_render_opd", "osog_render_field", "osog_render_intensity",
-           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_brightfield", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_gbuffer_normals", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_params", "osog_backward_particles", "osog_spectral_loss", "osog_backward_intensity", "osog_debug_recompose_field", "osog_debug_check_guards", "osog_debug_poisson", "osog_destroy", "osog_status",
+           "osog_field_to_intensity", "osog_render_dic", "osog_field_to_dic", "osog_render_brightfield", "osog_render_opd_atomic", "osog_render_opd_smem_atomic", "osog_particle_obbs", "osog_render_gbuffer", "osog_render_gbuffer_normals", "osog_render_height", "osog_backward_np", "osog_backward_centre", "osog_backward_params", "osog_backward_particles", "osog_spectral_loss", "osog_backward_intensity", "osog_render_opd_static", "osog_debug_recompose_field", "osog_debug_check_guards", "osog_debug_poisson", "osog_destroy", "osog_status",
            "osog_debug_bins", "osog_tile_size", "osog_last_cuda_error", "osog_strerror")
 
 
 def osog_tile_size() -> int:
     return lib().osog_tile_size()
+
+
+def lib_limits() -> dict:
+    """The fixed limits of osog_render_opd_static (OSOG_STATIC_MAX_* of include/osog.h)."""
+    return {"particles": 4096, "frames": 4, "tiles": 256, "pairs": 65536}
+
+
+def render_opd_static(p, o, H, W, out=None, status=None, stream=None):
+    """float32 [B, H, W] OPD through osog_render_opd_static: no context, no allocation inside the call (its scratch is a fixed
+    device array of the library; limits in osog.h, OSOG_ELIMIT beyond them).  `out` (float32 [B, H, W]) and `status` (a
+    1-element device tensor of 4-byte integers receiving the OSOG_W* bits) are the caller's; `out` is made here only when not
+    passed.  Enqueue-only on `stream` (default: torch's current stream); calls that overlap on the GPU race on the scratch."""
+    import torch
+    dev = p.device if p.device.index is not None else torch.device("cuda", torch.cuda.current_device())
+    if out is None:
+        out = torch.empty((o.B, int(H), int(W)), dtype=torch.float32, device=dev)
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    r = lib().osog_render_opd_static(dev.index if dev.index is not None else torch.cuda.current_device(), C.c_void_p(st.cuda_stream),
+                                     int(H), int(W), C.byref(p.c), p.N, C.byref(o), out.data_ptr(),
+                                     status.data_ptr() if status is not None else None)
+    if r != OSOG_OK:
+        raise OsogError(r, "osog_render_opd_static")
+    return out
 
 
 class Particles:

@@ -1,4 +1,5 @@
 // C ABI of libosog (include/osog.h): context management, argument checks, launch sequencing.
+#include <mutex>
 #include <new>
 #include <cstring>
 #include <vector>
@@ -183,6 +184,7 @@ const char* osog_strerror(int code)
         case OSOG_ECUDA: return "CUDA or cuFFT failure";
         case OSOG_ECAPACITY: return "particle-tile pair list overflow";
         case OSOG_ENOMEM: return "out of memory";
+        case OSOG_ELIMIT: return "beyond the fixed limits of osog_render_opd_static (particles, frames or tiles)";
         default: return "unknown error";
     }
 }
@@ -661,6 +663,101 @@ int osog_debug_bins(osog_ctx* c, uint32_t* h_offset, uint32_t* h_list, int64_t c
         if (e != cudaSuccess) return cuda_fail(c, e);
     }
     return r;
+}
+
+
+// ---- osog_render_opd_static: the hot path without any allocation (osog.h) --------------------------------------------------
+// All scratch of one call lives in ONE file-scope device array of a fixed, modest size; every GPU that loads the library
+// holds it until exit.  In host code the array's name is only a stand-in: the device address is asked for once per device
+// (cudaGetSymbolAddress with that device current) and carved into the scratch arrays of a static context, which is then
+// handed to the same launch functions as a context made by osog_create.
+constexpr long long kStaticMaxParticles = OSOG_STATIC_MAX_PARTICLES;
+constexpr long long kStaticMaxTiles = OSOG_STATIC_MAX_TILES;
+constexpr long long kStaticMaxPairs = OSOG_STATIC_MAX_PAIRS;
+constexpr int kStaticMaxFrames = OSOG_STATIC_MAX_FRAMES;
+constexpr int kStaticSliceCap = (int)(kStaticMaxPairs / kStaticMaxTiles);      // 256 entries per staging slice
+constexpr int kStaticMaxDevices = 64;
+constexpr size_t up256(size_t v) { return (v + 255) & ~(size_t)255; }
+constexpr size_t kSoRec = 0;
+constexpr size_t kSoRec2 = kSoRec + up256(sizeof(float) * kStaticMaxParticles * kRecWords);
+constexpr size_t kSoTbox = kSoRec2 + up256(sizeof(float) * kStaticMaxParticles * kPairWords);
+constexpr size_t kSoPframe = kSoTbox + up256(sizeof(int4) * kStaticMaxParticles);
+constexpr size_t kSoCount = kSoPframe + up256(sizeof(int) * kStaticMaxParticles);
+constexpr size_t kSoOffset = kSoCount + up256(sizeof(uint32_t) * 2 * kStaticMaxTiles);
+constexpr size_t kSoDone = kSoOffset + up256(sizeof(uint32_t) * (kStaticMaxTiles + 4));
+constexpr size_t kSoSlices = kSoDone + 256;
+constexpr size_t kSoList = kSoSlices + up256(sizeof(uint32_t) * kStaticMaxTiles * kStaticSliceCap);
+constexpr size_t kSoMeta = kSoList + up256(sizeof(uint32_t) * kStaticMaxPairs);
+constexpr size_t kSoOptics = kSoMeta + up256(sizeof(uint16_t) * kStaticMaxPairs);
+constexpr size_t kSoStatus = kSoOptics + up256(sizeof(FrameOptics) * kStaticMaxFrames);
+constexpr size_t kStaticBytes = kSoStatus + 256;
+static_assert(kStaticBytes <= OSOG_STATIC_SCRATCH_BYTES, "osog.h states the size of the static scratch");
+static_assert(kStaticMaxTiles % 4 == 0 && kStaticSliceCap >= 32 && kStaticSliceCap <= 1024, "slice / scan layout");
+
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+
+struct StaticSlot {
+    bool ready;
+    osog_ctx ctx;           // static storage: all zero until set up; never destroyed (it owns nothing)
+};
+static StaticSlot g_static_slot[kStaticMaxDevices];
+static std::mutex g_static_mutex;
+
+int osog_render_opd_static(int device, void* stream, int H, int W, const osog_particles* p, int64_t N, const osog_optics* o,
+                           float* d_opd, uint32_t* d_status_bits)
+{
+    if (!p || !o || !d_opd || H < 1 || W < 1 || device < 0 || device >= kStaticMaxDevices) return OSOG_EINVAL;
+    if (o->struct_size != sizeof(osog_optics) || o->B < 1 || N < 0) return OSOG_EINVAL;
+    if (d_status_bits && (reinterpret_cast<uintptr_t>(d_status_bits) & 3u)) return OSOG_EINVAL;
+    const long long ntx = ((long long)W + kTile - 1) / kTile, nty = ((long long)H + kTile - 1) / kTile;
+    if (N > kStaticMaxParticles || o->B > kStaticMaxFrames || (long long)o->B * ntx * nty > kStaticMaxTiles) return OSOG_ELIMIT;
+    std::lock_guard<std::mutex> lock(g_static_mutex);      // host side only: calls that overlap ON THE GPU still race (osog.h)
+    DeviceGuard g(device);
+    if (!g.ok) return OSOG_ECUDA;
+    StaticSlot& slot = g_static_slot[device];
+    osog_ctx* c = &slot.ctx;
+    if (!slot.ready) {
+        unsigned char* base = nullptr;                       // this device's copy of the array
+        const cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_static_scratch);
+        if (e != cudaSuccess || !base) { c->last_cuda_error = (int)e; cudaGetLastError(); return OSOG_ECUDA; }
+        c->device = device;
+        c->max_frames = kStaticMaxFrames;
+        c->max_particles = kStaticMaxParticles;
+        c->max_pairs = kStaticMaxPairs;
+        c->max_tiles = kStaticMaxTiles;
+        c->count_stride = kStaticMaxTiles;
+        c->slice_cap = kStaticSliceCap;
+        c->rec = reinterpret_cast<float*>(base + kSoRec);
+        c->rec2 = reinterpret_cast<float*>(base + kSoRec2);
+        c->tbox = reinterpret_cast<int4*>(base + kSoTbox);
+        c->pframe = reinterpret_cast<int*>(base + kSoPframe);
+        c->count = reinterpret_cast<uint32_t*>(base + kSoCount);
+        c->offset = reinterpret_cast<uint32_t*>(base + kSoOffset);
+        c->done = reinterpret_cast<uint32_t*>(base + kSoDone);
+        c->slices = reinterpret_cast<uint32_t*>(base + kSoSlices);
+        c->list = reinterpret_cast<uint32_t*>(base + kSoList);
+        c->meta = reinterpret_cast<uint16_t*>(base + kSoMeta);
+        c->optics = reinterpret_cast<FrameOptics*>(base + kSoOptics);
+        c->status = reinterpret_cast<DeviceStatus*>(base + kSoStatus);
+        slot.ready = true;
+    }
+    c->stream = static_cast<cudaStream_t>(stream);
+    c->H = H; c->W = W; c->ntx = (int)ntx; c->nty = (int)nty;
+    c->last_has_ramp = -1;
+    const int r = check_call(c, p, N, o, d_opd);
+    if (r != OSOG_OK) return r;
+    // The array keeps the last call's contents (possibly of another frame size, on another stream, or of a call that failed):
+    // the tile counters of both slots, the scan ticket and the status words are cleared on this call's stream first.
+    c->scratch_dirty = true;
+    cudaError_t e = launch_binning(c, p, N, o, nullptr, false);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = launch_compose(c, o->B, false, d_opd, nullptr);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    if (d_status_bits) {
+        e = cudaMemcpyAsync(d_status_bits, &(c->status + c->status_idx)->bits, sizeof(uint32_t), cudaMemcpyDeviceToDevice, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e);
+    }
+    return OSOG_OK;
 }
 
 }  // extern "C"
