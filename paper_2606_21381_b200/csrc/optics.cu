@@ -454,4 +454,412 @@ cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_o
     return cudaGetLastError();
 }
 
+
+// ---- L1-L3 fused and pruned (power-of-two frames): row FFT -> [column FFT, pupil, inverse column FFT] -> inverse row FFT + sensor ----
+// The pupil passes |m_x| <= r_x only (NA 0.65 on config 4: 487 of 2048 columns), so after the forward row transforms only
+// those columns are kept (written transposed, one contiguous column each), one kernel does the forward column transform,
+// the pupil and the inverse column transform of the kept columns, and the inverse row transforms read the kept columns back
+// into zero-filled rows and end in the sensor.  Three kernels and ~85 MB of traffic per 2048^2 frame instead of six (two
+// cuFFT launches of two kernels each, pupil, sensor) and 385 MB.
+// The transforms: n / 8 threads per row, 8 complex values per thread in registers, decimation in frequency with the radix
+// sequence r1, 8, 8, ... (r1 = 2, 4 or 8 takes what the power of two leaves), one shared-memory exchange between two stages.
+// The spectrum stays in digit-reversed order (the pupil only needs to know which frequency sits where) and the inverse runs
+// the conjugate-transposed stages in reverse order: no reordering pass, and the stage next to the pupil needs no exchange.
+constexpr int kFoThreads = 512;                     // threads per CTA (one row of 4096, two of 2048, ...)
+
+struct FoPlan {
+    int n, lg_n, lg_r1, nstage;       // n = 2^lg_n = 2^lg_r1 * 8^(nstage - 1)
+};
+
+static FoPlan fo_plan(int n)
+{
+    FoPlan p;
+    p.n = n;
+    p.lg_n = 0;
+    while ((1 << p.lg_n) < n) ++p.lg_n;
+    p.lg_r1 = p.lg_n % 3 == 0 ? 3 : p.lg_n % 3;
+    p.nstage = 1 + (p.lg_n - p.lg_r1) / 3;
+    return p;
+}
+
+// position p of the digit-reversed spectrum holds frequency k:  p = m1 n/r1 + m2 n/(r1 r2) + ...,  k = m1 + r1 (m2 + r2 (...))
+__device__ __forceinline__ int fo_freq_of_pos(const FoPlan& pl, int p)
+{
+    int lg_L = pl.lg_n - pl.lg_r1;
+    int k = p >> lg_L, sh = pl.lg_r1;
+    p &= (1 << lg_L) - 1;
+    for (int s = 1; s < pl.nstage; ++s) {
+        lg_L -= 3;
+        k += (p >> lg_L) << sh;
+        p &= (1 << lg_L) - 1;
+        sh += 3;
+    }
+    return k;
+}
+__device__ __forceinline__ int fo_pos_of_freq(const FoPlan& pl, int k)
+{
+    int lg_L = pl.lg_n - pl.lg_r1;
+    int p = (k & ((1 << pl.lg_r1) - 1)) << lg_L;
+    k >>= pl.lg_r1;
+    for (int s = 1; s < pl.nstage; ++s) {
+        lg_L -= 3;
+        p += (k & 7) << lg_L;
+        k >>= 3;
+    }
+    return p;
+}
+
+__device__ __forceinline__ float2 fo_cmul(float2 a, float2 w) { return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x); }
+__device__ __forceinline__ float2 fo_cmulc(float2 a, float2 w) { return make_float2(a.x * w.x + a.y * w.y, a.y * w.x - a.x * w.y); }   // a conj(w)
+__device__ __forceinline__ float2 fo_conj(float2 a) { return make_float2(a.x, -a.y); }
+// complex add / subtract as ONE packed instruction (Blackwell add.f32x2): the butterflies are issue bound
+__device__ __forceinline__ float2 fo_add(float2 a, float2 b)
+{
+    unsigned long long ra, rb, rd;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(b.x), "f"(b.y));
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
+    float2 d;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
+    return d;
+}
+__device__ __forceinline__ float2 fo_sub(float2 a, float2 b)
+{
+    unsigned long long ra, rb, rd;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(b.x), "f"(b.y));
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
+    float2 d;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
+    return d;
+}
+
+// y_m = sum_j a_j w4^{j m}, w4 = exp(-2 pi i / 4) = -i (forward), in place
+__device__ __forceinline__ void fo_r4(float2& a0, float2& a1, float2& a2, float2& a3)
+{
+    const float2 s02 = fo_add(a0, a2), d02 = fo_sub(a0, a2), s13 = fo_add(a1, a3), d13 = fo_sub(a1, a3);
+    a0 = fo_add(s02, s13);
+    a2 = fo_sub(s02, s13);
+    a1 = make_float2(d02.x + d13.y, d02.y - d13.x);               // d02 - i d13
+    a3 = make_float2(d02.x - d13.y, d02.y + d13.x);               // d02 + i d13
+}
+// y_m = sum_j a_j w8^{j m}, w8 = exp(-2 pi i / 8) (forward), in place: a[m] <- y_m
+__device__ __forceinline__ void fo_r8(float2 (&a)[8])
+{
+    const float h = 0.70710678118654752f;
+    float2 s0 = fo_add(a[0], a[4]), s1 = fo_add(a[1], a[5]), s2 = fo_add(a[2], a[6]), s3 = fo_add(a[3], a[7]);
+    float2 d0 = fo_sub(a[0], a[4]), d1 = fo_sub(a[1], a[5]), d2 = fo_sub(a[2], a[6]), d3 = fo_sub(a[3], a[7]);
+    d1 = make_float2((d1.x + d1.y) * h, (d1.y - d1.x) * h);       // d1 (1 - i) / sqrt 2
+    d2 = make_float2(d2.y, -d2.x);                                // -i d2
+    d3 = make_float2((d3.y - d3.x) * h, -(d3.x + d3.y) * h);      // d3 (-1 - i) / sqrt 2
+    fo_r4(s0, s1, s2, s3);                                        // even outputs y0 y2 y4 y6
+    fo_r4(d0, d1, d2, d3);                                        // odd outputs  y1 y3 y5 y7
+    a[0] = s0; a[2] = s1; a[4] = s2; a[6] = s3;
+    a[1] = d0; a[3] = d1; a[5] = d2; a[7] = d3;
+}
+
+// shared-memory index of row position p: one pad element per 8 keeps the strided exchanges (sub = 1, 8, 64 ...) off the same banks
+__device__ __forceinline__ int fo_phys(int p) { return p + (p >> 3); }
+// element stride of positions p0 + k sub (sub = 1 or a multiple of 8, p0 + 7 sub inside one block) in the padded layout
+__device__ __forceinline__ int fo_stride(int lg_sub) { return lg_sub >= 3 ? 9 << (lg_sub - 3) : 1; }
+
+// twiddles of one butterfly: a[m] *= w^m (forward) or its conjugate (inverse), w = tw[q << lg_step], tw[k] = exp(-2 pi i k / n);
+// w, w^2, w^4 come from the table, the other four powers by one multiplication each (error ~ 1e-7; three loads instead of seven)
+template <bool INV>
+__device__ __forceinline__ void fo_twiddle8(float2 (&a)[8], int q, int lg_step, const float2* __restrict__ tw)
+{
+    const int i1 = q << lg_step;
+    const float2 w1 = __ldg(tw + i1), w2 = __ldg(tw + 2 * i1), w4 = __ldg(tw + 4 * i1);
+    const float2 w3 = fo_cmul(w1, w2), w5 = fo_cmul(w4, w1), w6 = fo_cmul(w4, w2), w7 = fo_cmul(w4, w3);
+    const float2 w[8] = {make_float2(1.f, 0.f), w1, w2, w3, w4, w5, w6, w7};
+#pragma unroll
+    for (int m = 1; m < 8; ++m) a[m] = INV ? fo_cmulc(a[m], w[m]) : fo_cmul(a[m], w[m]);
+}
+
+// first forward stage (block length n, radix r1) on a[k] = x[t + k T], T = n / 8, in place (positions unchanged)
+__device__ __forceinline__ void fo_first_fwd(float2 (&a)[8], int t, const FoPlan& pl, const float2* __restrict__ tw)
+{
+    const int T = pl.n >> 3;
+    if (pl.lg_r1 == 3) {
+        fo_r8(a);
+        fo_twiddle8<false>(a, t, 0, tw);
+    } else if (pl.lg_r1 == 2) {
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int q = t + i * T;
+            fo_r4(a[i], a[i + 2], a[i + 4], a[i + 6]);
+            a[i + 2] = fo_cmul(a[i + 2], __ldg(tw + q));
+            a[i + 4] = fo_cmul(a[i + 4], __ldg(tw + 2 * q));
+            a[i + 6] = fo_cmul(a[i + 6], __ldg(tw + 3 * q));
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float2 d = fo_sub(a[i], a[i + 4]);
+            a[i] = fo_add(a[i], a[i + 4]);
+            a[i + 4] = fo_cmul(d, __ldg(tw + t + i * T));
+        }
+    }
+}
+// its conjugate transpose (last inverse stage)
+__device__ __forceinline__ void fo_first_inv(float2 (&a)[8], int t, const FoPlan& pl, const float2* __restrict__ tw)
+{
+    const int T = pl.n >> 3;
+    if (pl.lg_r1 == 3) {
+        fo_twiddle8<true>(a, t, 0, tw);
+#pragma unroll
+        for (int m = 0; m < 8; ++m) a[m] = fo_conj(a[m]);
+        fo_r8(a);
+#pragma unroll
+        for (int m = 0; m < 8; ++m) a[m] = fo_conj(a[m]);
+    } else if (pl.lg_r1 == 2) {
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int q = t + i * T;
+            float2 y0 = fo_conj(a[i]), y1 = fo_conj(fo_cmulc(a[i + 2], __ldg(tw + q)));
+            float2 y2 = fo_conj(fo_cmulc(a[i + 4], __ldg(tw + 2 * q))), y3 = fo_conj(fo_cmulc(a[i + 6], __ldg(tw + 3 * q)));
+            fo_r4(y0, y1, y2, y3);
+            a[i] = fo_conj(y0); a[i + 2] = fo_conj(y1); a[i + 4] = fo_conj(y2); a[i + 6] = fo_conj(y3);
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float2 y1 = fo_cmulc(a[i + 4], __ldg(tw + t + i * T));
+            const float2 y0 = a[i];
+            a[i] = fo_add(y0, y1);
+            a[i + 4] = fo_sub(y0, y1);
+        }
+    }
+}
+
+// Forward transform of one row held as a[k] = x[t + k T]; on return a[m] is the value at digit-reversed position 8 t + m.
+// xr: this row's exchange buffer in shared memory (9 n / 8 elements); every thread of the CTA must call (barriers inside).
+__device__ __forceinline__ void fo_forward(float2 (&a)[8], int t, const FoPlan& pl, const float2* __restrict__ tw, float2* xr)
+{
+    fo_first_fwd(a, t, pl, tw);
+    int lg_L = pl.lg_n, lg_sub = pl.lg_n - 3, blk = 0, q = t;    // positions of a[k]: (blk << lg_L) + q + (k << lg_sub)
+    int lg_Ln = pl.lg_n - pl.lg_r1;                               // block length of the next stage
+    for (int s = 1; s < pl.nstage; ++s) {
+        {
+            float2* w = xr + fo_phys((blk << lg_L) + q);
+            const int st = fo_stride(lg_sub);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) w[k * st] = a[k];
+        }
+        __syncthreads();
+        lg_L = lg_Ln; lg_sub = lg_L - 3;
+        blk = t >> lg_sub; q = t & ((1 << lg_sub) - 1);
+        {
+            const float2* rd = xr + fo_phys((blk << lg_L) + q);
+            const int st = fo_stride(lg_sub);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) a[k] = rd[k * st];
+        }
+        __syncthreads();
+        fo_r8(a);
+        if (lg_sub > 0) fo_twiddle8<false>(a, q, pl.lg_n - lg_L, tw);
+        lg_Ln = lg_sub;
+    }
+}
+// Inverse (unnormalised): a[m] at digit-reversed position 8 t + m on entry, a[k] = x[t + k T] on return.
+__device__ __forceinline__ void fo_inverse(float2 (&a)[8], int t, const FoPlan& pl, const float2* __restrict__ tw, float2* xr)
+{
+    int lg_L = 3, lg_sub = 0;
+    for (int s = pl.nstage - 1; s >= 1; --s) {
+        const int blk = t >> lg_sub, q = t & ((1 << lg_sub) - 1);
+        if (lg_sub > 0) fo_twiddle8<true>(a, q, pl.lg_n - lg_L, tw);
+#pragma unroll
+        for (int m = 0; m < 8; ++m) a[m] = fo_conj(a[m]);
+        fo_r8(a);
+#pragma unroll
+        for (int m = 0; m < 8; ++m) a[m] = fo_conj(a[m]);
+        {
+            float2* w = xr + fo_phys((blk << lg_L) + q);
+            const int st = fo_stride(lg_sub);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) w[k * st] = a[k];
+        }
+        __syncthreads();
+        // the stage before: block length 8 L (the first stage: n, whatever its radix; its threads hold x[t + k n / 8])
+        int lg_Lp, lg_subp;
+        if (s == 1) { lg_Lp = pl.lg_n; lg_subp = pl.lg_n - 3; }
+        else { lg_Lp = lg_L + 3; lg_subp = lg_L; }
+        const int blkp = t >> lg_subp, qp = t & ((1 << lg_subp) - 1);
+        {
+            const float2* rd = xr + fo_phys((blkp << lg_Lp) + qp);
+            const int st = fo_stride(lg_subp);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) a[k] = rd[k * st];
+        }
+        __syncthreads();
+        lg_L = lg_Lp; lg_sub = lg_subp;
+    }
+    fo_first_inv(a, t, pl, tw);
+}
+
+struct FoArgs {
+    FoPlan pw, ph;                 // row (length W) and column (length H) transforms
+    const float2* tw_w;            // exp(-2 pi i k / W)
+    const float2* tw_h;            // exp(-2 pi i k / H)
+    int H, W;
+    int nc, m_lo;                  // kept columns: signed frequency m_x = m_lo + c, c = 0 .. nc-1
+    float2* spec_t;                // [B][nc][H] kept columns, transposed
+};
+
+__device__ __forceinline__ int fo_kx(const FoArgs& a, int c)
+{
+    const int m = a.m_lo + c;
+    return m < 0 ? m + a.W : m;
+}
+
+// K1: forward row transforms, kFoThreads / (W / 8) rows per CTA; the kept columns are written transposed
+__global__ void __launch_bounds__(kFoThreads) k_fo_rows_fwd(const FoArgs a, const float2* __restrict__ field)
+{
+    extern __shared__ __align__(16) float2 fo_x[];
+    const int lgT = a.pw.lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, R = 1 << lgR, stride = a.W + (a.W >> 3);
+    const int r = threadIdx.x >> lgT, t = threadIdx.x & (T - 1), b = blockIdx.y, row0 = blockIdx.x << lgR;
+    float2* xr = fo_x + r * stride;
+    const float2* src = field + ((size_t)b * a.H + row0 + r) * a.W + t;
+    float2 v[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = src[k << lgT];
+    fo_forward(v, t, a.pw, a.tw_w, xr);
+#pragma unroll
+    for (int m = 0; m < 8; ++m) xr[(m << lgT) + t] = v[m];          // position 8 t + m, stored transposed (conflict free)
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < (a.nc << lgR); idx += kFoThreads) {
+        const int rr = idx & (R - 1), c = idx >> lgR;
+        const int p = fo_pos_of_freq(a.pw, fo_kx(a, c));
+        a.spec_t[((size_t)b * a.nc + c) * a.H + row0 + rr] = fo_x[rr * stride + ((p & 7) << lgT) + (p >> 3)];
+    }
+}
+
+// K2: kept columns: forward transform along y, pupil (times 1 / (H W)), inverse transform along y, in place
+template <bool DEFOCUS>
+__global__ void __launch_bounds__(kFoThreads) k_fo_cols(const FoArgs a, const FrameOptics* __restrict__ optics, double inv_wp,
+                                                        double inv_hp, float scale)
+{
+    extern __shared__ __align__(16) float2 fo_x[];
+    const int lgT = a.ph.lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, stride = a.H + (a.H >> 3);
+    const int r = threadIdx.x >> lgT, t = threadIdx.x & (T - 1), b = blockIdx.y, c = (blockIdx.x << lgR) + r;
+    const bool valid = c < a.nc;
+    float2* xr = fo_x + r * stride;
+    float2* col = a.spec_t + ((size_t)b * a.nc + (valid ? c : 0)) * a.H + t;
+    float2 v[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = valid ? col[k << lgT] : make_float2(0.f, 0.f);
+    fo_forward(v, t, a.ph, a.tw_h, xr);
+    const int kx = fo_kx(a, valid ? c : 0);
+    const FrameOptics fo = optics[b];
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+        const float2 pv = pupil_value<DEFOCUS>(fo, kx, fo_freq_of_pos(a.ph, 8 * t + m), a.H, a.W, inv_wp, inv_hp, scale);
+        v[m] = DEFOCUS ? fo_cmul(v[m], pv) : make_float2(v[m].x * pv.x, v[m].y * pv.x);
+    }
+    fo_inverse(v, t, a.ph, a.tw_h, xr);
+    if (valid) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) col[k << lgT] = v[k];
+    }
+}
+
+// K3: inverse row transforms from the kept columns (all other bins are zero), then the sensor
+template <bool SHOT>
+__global__ void __launch_bounds__(kFoThreads) k_fo_rows_inv(const FoArgs a, float* __restrict__ out, float sigma, double photons,
+                                                            uint64_t seed)
+{
+    extern __shared__ __align__(16) float2 fo_x[];
+    const int lgT = a.pw.lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, R = 1 << lgR, stride = a.W + (a.W >> 3);
+    const int r = threadIdx.x >> lgT, t = threadIdx.x & (T - 1), b = blockIdx.y, row0 = blockIdx.x << lgR;
+    float2* xr = fo_x + r * stride;
+    for (int k = threadIdx.x; k < R * stride; k += kFoThreads) fo_x[k] = make_float2(0.f, 0.f);
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < (a.nc << lgR); idx += kFoThreads) {
+        const int rr = idx & (R - 1), c = idx >> lgR;
+        const int p = fo_pos_of_freq(a.pw, fo_kx(a, c));
+        fo_x[rr * stride + ((p & 7) << lgT) + (p >> 3)] = a.spec_t[((size_t)b * a.nc + c) * a.H + row0 + rr];
+    }
+    __syncthreads();
+    float2 v[8];
+#pragma unroll
+    for (int m = 0; m < 8; ++m) v[m] = xr[(m << lgT) + t];
+    __syncthreads();
+    fo_inverse(v, t, a.pw, a.tw_w, xr);
+    const size_t pix0 = (size_t)(row0 + r) * a.W + t;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const size_t pix = pix0 + (k << lgT);
+        float I = v[k].x * v[k].x + v[k].y * v[k].y;
+        if (SHOT) I = (float)(poisson_draw(photons * fmax((double)I, 0.0), seed, (uint32_t)b, (uint32_t)pix) / photons);
+        if (sigma != 0.0f) I = fmaf(sigma, read_noise_z(seed, (uint32_t)b, (uint32_t)pix), I);
+        out[(size_t)b * a.H * a.W + pix] = I;
+    }
+}
+
+__global__ void k_fo_twiddles(float2* tw, int n)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    double s, c;
+    sincospi(-2.0 * (double)k / (double)n, &s, &c);
+    tw[k] = make_float2((float)c, (float)s);
+}
+
+cudaError_t launch_fo_twiddles(osog_ctx* c, float2* tw, int n)
+{
+    k_fo_twiddles<<<(n + 255) / 256, 256, 0, c->stream>>>(tw, n);
+    return cudaGetLastError();
+}
+
+bool fused_optics_applies(const osog_ctx* c)
+{
+    auto pow2 = [](int v) { return v >= 64 && v <= 4096 && (v & (v - 1)) == 0; };
+    return pow2(c->H) && pow2(c->W);
+}
+
+// field: [B, H, W] exit wave (read only); spec_t: scratch of B * W * H complex values; tw_w / tw_h: twiddle tables of W / H
+cudaError_t launch_fused_optics(osog_ctx* c, const osog_optics* o, const float2* field, float2* spec_t, const float2* tw_w,
+                                const float2* tw_h, float* d_intensity)
+{
+    const int B = o->B, H = c->H, W = c->W;
+    FoArgs a;
+    a.pw = fo_plan(W); a.ph = fo_plan(H);
+    a.tw_w = tw_w; a.tw_h = tw_h; a.H = H; a.W = W;
+    a.spec_t = spec_t;
+    // widest pupil of the batch in x: m_x^2 H^2 <= floor((NA p / lambda)^2 H^2 W^2)  =>  |m_x| <= NA p W / lambda
+    long long rx = 0;
+    for (int b = 0; b < B; ++b) {
+        long long rb = W;                                         // all-pass
+        if (o->pupil_enabled && o->NA != nullptr) {
+            const double r = o->NA[b] * o->pitch_um / o->lambda_um[b] * (double)W;
+            if (r < (double)W) rb = (long long)floor(r) + 1;
+        }
+        rx = rb > rx ? rb : rx;
+    }
+    const int m_hi = (int)(rx < W / 2 - 1 ? rx : W / 2 - 1);
+    a.m_lo = -(int)(rx < W / 2 ? rx : W / 2);
+    a.nc = m_hi - a.m_lo + 1;
+    const bool defocus = o->defocus_um != 0.0;
+    const double inv_wp = 1.0 / ((double)W * o->pitch_um), inv_hp = 1.0 / ((double)H * o->pitch_um);
+    const float scale = (float)(1.0 / ((double)H * W));
+    const int Rw = kFoThreads / (W / 8), Rh = kFoThreads / (H / 8);           // rows / columns per CTA
+    const size_t smem_rows = (size_t)Rw * (W + W / 8) * sizeof(float2), smem_cols = (size_t)Rh * (H + H / 8) * sizeof(float2);
+    cudaError_t e;
+    k_fo_rows_fwd<<<dim3(H / Rw, B), kFoThreads, smem_rows, c->stream>>>(a, field);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    const dim3 gcol((a.nc + Rh - 1) / Rh, B);
+    if (defocus) k_fo_cols<true><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale);
+    else k_fo_cols<false><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    const float sigma = (float)o->read_noise_sigma;
+    if (o->shot_noise_photons != 0.0)
+        k_fo_rows_inv<true><<<dim3(H / Rw, B), kFoThreads, smem_rows, c->stream>>>(a, d_intensity, sigma, o->shot_noise_photons, o->seed);
+    else
+        k_fo_rows_inv<false><<<dim3(H / Rw, B), kFoThreads, smem_rows, c->stream>>>(a, d_intensity, sigma, o->shot_noise_photons, o->seed);
+    return cudaGetLastError();
+}
+
+
+
+
 }  // namespace osog

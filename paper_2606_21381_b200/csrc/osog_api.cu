@@ -110,6 +110,26 @@ int fft_frames(osog_ctx* c, float2* buf, int B, int sign, const float2* src = nu
 int optics_stage(osog_ctx* c, const osog_optics* o, float2* buf, float* d_intensity, const float2* src = nullptr)
 {
     const int B = o->B;
+    if (fused_optics_applies(c)) {
+        // power-of-two frames: row FFT -> [column FFT, pupil, inverse column FFT] of the columns the pupil keeps -> inverse row
+        // FFT + sensor, three kernels of this library (optics.cu); the field is only read
+        if (!c->fo_ready) {                          // first call: the kept-column scratch and the twiddle tables
+            cudaError_t ea = cudaSuccess;
+            if (!c->spec_t) ea = dalloc(&c->spec_t, (size_t)c->max_frames * c->H * c->W, c);
+            if (ea == cudaSuccess && !c->tw_w) ea = dalloc(&c->tw_w, (size_t)c->W, c);
+            if (ea == cudaSuccess && c->H != c->W && !c->tw_h) ea = dalloc(&c->tw_h, (size_t)c->H, c);
+            if (ea == cudaSuccess) ea = launch_fo_twiddles(c, c->tw_w, c->W);
+            if (ea == cudaSuccess && c->H != c->W) ea = launch_fo_twiddles(c, c->tw_h, c->H);
+            if (ea != cudaSuccess) {                 // (what was allocated stays with the context and is reused by the next call)
+                cudaGetLastError();
+                return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea);
+            }
+            if (c->H == c->W) c->tw_h = c->tw_w;
+            c->fo_ready = true;
+        }
+        const cudaError_t ef = launch_fused_optics(c, o, src ? src : buf, c->spec_t, c->tw_w, c->tw_h, d_intensity);
+        return ef == cudaSuccess ? OSOG_OK : cuda_fail(c, ef);
+    }
     int r = fft_frames(c, buf, B, CUFFT_FORWARD, src);
     if (r != OSOG_OK) return r;
     cudaError_t e = launch_pupil(c, B, buf, o->pitch_um, o->defocus_um != 0.0);
@@ -200,6 +220,7 @@ int osog_destroy(osog_ctx* c)
     cudaFree(c->rec); cudaFree(c->rec2); cudaFree(c->tbox); cudaFree(c->pframe); cudaFree(c->count);
     cudaFree(c->list); cudaFree(c->meta); cudaFree(c->slices); cudaFree(c->offset); cudaFree(c->done); cudaFree(c->optics);
     cudaFree(c->status); cudaFree(c->field); cudaFree(c->work); cudaFree(c->otf); cudaFree(c->bf_h); cudaFree(c->spec_partial);
+    cudaFree(c->spec_t); cudaFree(c->tw_w); if (c->tw_h != c->tw_w) cudaFree(c->tw_h);
     delete c->otf_key;
     delete c->guards;
     if (c->h_status) cudaFreeHost(c->h_status);

@@ -89,6 +89,10 @@ struct osog_ctx {
     float2* work;                   // [max_frames][H][W] second complex batch (DIC path; allocated by the first DIC call)
     double* spec_partial;           // [max_frames][ceil(H W / 256)] block sums of the spectral loss (allocated by its first call)
     float* bf_h;                    // [max_frames][H][W] height map of the brightfield path (allocated by its first call)
+    float2* spec_t;                 // [max_frames][W][H] kept columns of the fused optics stage (allocated by its first call)
+    float2* tw_w;                   // [W] exp(-2 pi i k / W), and [H] (the same table if H == W): fused optics stage
+    float2* tw_h;
+    bool fo_ready;
     float2* otf;                    // [max_frames][H][W] optical transfer function F{|F^-1{P}|^2} of the last DIC call
     std::vector<double>* otf_key;   // optics the cached OTF was built for (B, pitch, n_medium, defocus, pupil, lambda[], NA[])
     osog::DeviceStatus* h_status;   // pinned host mirror
@@ -181,6 +185,10 @@ cudaError_t launch_real_part(osog_ctx* c, int B, const float2* in, float* out);
 cudaError_t launch_height_stencil(osog_ctx* c, int B, const float* d_h, double pitch, float* d_grad, float* d_lap);
 cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_out, double sigma, double photons, uint64_t seed);
 cudaError_t launch_sensor(osog_ctx* c, int B, const float2* img, float* d_intensity, double sigma, double photons, uint64_t seed);
+bool fused_optics_applies(const osog_ctx* c);       // power-of-two frames, 64 .. 4096
+cudaError_t launch_fo_twiddles(osog_ctx* c, float2* tw, int n);
+cudaError_t launch_fused_optics(osog_ctx* c, const osog_optics* o, const float2* field, float2* spec_t, const float2* tw_w,
+                                const float2* tw_h, float* d_intensity);
 cudaError_t launch_poisson(osog_ctx* c, const float* d_lam, size_t n, uint64_t seed, uint32_t frame, int32_t* d_counts);
 
 }  // namespace osog
