@@ -737,7 +737,7 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_rows_fwd(const FoArgs a, cons
 // K2: kept columns: forward transform along y, pupil (times 1 / (H W)), inverse transform along y, in place
 template <bool DEFOCUS>
 __global__ void __launch_bounds__(kFoThreads) k_fo_cols(const FoArgs a, const FrameOptics* __restrict__ optics, double inv_wp,
-                                                        double inv_hp, float scale)
+                                                        double inv_hp, float scale, float imag_sign)
 {
     extern __shared__ __align__(16) float2 fo_x[];
     const int lgT = a.ph.lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, stride = a.H + (a.H >> 3);
@@ -753,7 +753,8 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_cols(const FoArgs a, const Fr
     const FrameOptics fo = optics[b];
 #pragma unroll
     for (int m = 0; m < 8; ++m) {
-        const float2 pv = pupil_value<DEFOCUS>(fo, kx, fo_freq_of_pos(a.ph, 8 * t + m), a.H, a.W, inv_wp, inv_hp, scale);
+        float2 pv = pupil_value<DEFOCUS>(fo, kx, fo_freq_of_pos(a.ph, 8 * t + m), a.H, a.W, inv_wp, inv_hp, scale);
+        if (DEFOCUS) pv.y *= imag_sign;                              // -1: conj(P), the adjoint of the stage
         v[m] = DEFOCUS ? fo_cmul(v[m], pv) : make_float2(v[m].x * pv.x, v[m].y * pv.x);
     }
     fo_inverse(v, t, a.ph, a.tw_h, xr);
@@ -763,10 +764,23 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_cols(const FoArgs a, const Fr
     }
 }
 
-// K3: inverse row transforms from the kept columns (all other bins are zero), then the sensor
-template <bool SHOT>
-__global__ void __launch_bounds__(kFoThreads) k_fo_rows_inv(const FoArgs a, float* __restrict__ out, float sigma, double photons,
-                                                            uint64_t seed)
+// what K3 does with the image V it has transformed back
+enum { kFoSensor = 0, kFoSensorShot = 1, kFoTimesReal = 2, kFoGopd = 3 };
+struct FoEpi {
+    float* out;                    // sensor: intensity [B, H, W]; kFoGopd: dL/dOPD [B, H, W]
+    float2* cout;                  // kFoTimesReal: g_V = g V [B, H, W] complex
+    const float* g;                // kFoTimesReal: the real factor (dL/dI)
+    const float2* u;               // kFoGopd: the exit wave U
+    const FrameOptics* optics;     // kFoGopd: 1 / lambda per frame
+    float sigma;
+    double photons;
+    uint64_t seed;
+};
+
+// K3: inverse row transforms from the kept columns (all other bins are zero), then the sensor (I = |V|^2, shot and read noise),
+// or, for the adjoint of the stage (osog_backward_intensity), g_V = (dL/dI) V  resp.  dL/dOPD = (4 pi / lambda) Im(g_U conj U)
+template <int MODE>
+__global__ void __launch_bounds__(kFoThreads) k_fo_rows_inv(const FoArgs a, const FoEpi ep)
 {
     extern __shared__ __align__(16) float2 fo_x[];
     const int lgT = a.pw.lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, R = 1 << lgR, stride = a.W + (a.W >> 3);
@@ -788,11 +802,21 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_rows_inv(const FoArgs a, floa
     const size_t pix0 = (size_t)(row0 + r) * a.W + t;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-        const size_t pix = pix0 + (k << lgT);
-        float I = v[k].x * v[k].x + v[k].y * v[k].y;
-        if (SHOT) I = (float)(poisson_draw(photons * fmax((double)I, 0.0), seed, (uint32_t)b, (uint32_t)pix) / photons);
-        if (sigma != 0.0f) I = fmaf(sigma, read_noise_z(seed, (uint32_t)b, (uint32_t)pix), I);
-        out[(size_t)b * a.H * a.W + pix] = I;
+        const size_t pix = pix0 + (k << lgT), gpix = (size_t)b * a.H * a.W + pix;
+        if (MODE == kFoTimesReal) {
+            const float gv = ep.g[gpix];
+            ep.cout[gpix] = make_float2(v[k].x * gv, v[k].y * gv);
+        } else if (MODE == kFoGopd) {
+            const float2 w = ep.u[gpix];
+            const float kk = (float)(12.566370614359172 * ep.optics[b].inv_lambda);
+            ep.out[gpix] = kk * (v[k].y * w.x - v[k].x * w.y);
+        } else {
+            float I = v[k].x * v[k].x + v[k].y * v[k].y;
+            if (MODE == kFoSensorShot)
+                I = (float)(poisson_draw(ep.photons * fmax((double)I, 0.0), ep.seed, (uint32_t)b, (uint32_t)pix) / ep.photons);
+            if (ep.sigma != 0.0f) I = fmaf(ep.sigma, read_noise_z(ep.seed, (uint32_t)b, (uint32_t)pix), I);
+            ep.out[gpix] = I;
+        }
     }
 }
 
@@ -817,9 +841,9 @@ bool fused_optics_applies(const osog_ctx* c)
     return pow2(c->H) && pow2(c->W);
 }
 
-// field: [B, H, W] exit wave (read only); spec_t: scratch of B * W * H complex values; tw_w / tw_h: twiddle tables of W / H
-cudaError_t launch_fused_optics(osog_ctx* c, const osog_optics* o, const float2* field, float2* spec_t, const float2* tw_w,
-                                const float2* tw_h, float* d_intensity)
+// in: [B, H, W] complex frames (read only); spec_t: scratch of B * W * H complex values; tw_w / tw_h: twiddle tables of W / H
+static cudaError_t fo_run(osog_ctx* c, const osog_optics* o, const float2* in, float2* spec_t, const float2* tw_w, const float2* tw_h,
+                          int mode, float imag_sign, const FoEpi& ep)
 {
     const int B = o->B, H = c->H, W = c->W;
     FoArgs a;
@@ -845,21 +869,41 @@ cudaError_t launch_fused_optics(osog_ctx* c, const osog_optics* o, const float2*
     const int Rw = kFoThreads / (W / 8), Rh = kFoThreads / (H / 8);           // rows / columns per CTA
     const size_t smem_rows = (size_t)Rw * (W + W / 8) * sizeof(float2), smem_cols = (size_t)Rh * (H + H / 8) * sizeof(float2);
     cudaError_t e;
-    k_fo_rows_fwd<<<dim3(H / Rw, B), kFoThreads, smem_rows, c->stream>>>(a, field);
+    k_fo_rows_fwd<<<dim3(H / Rw, B), kFoThreads, smem_rows, c->stream>>>(a, in);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    const dim3 gcol((a.nc + Rh - 1) / Rh, B);
-    if (defocus) k_fo_cols<true><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale);
-    else k_fo_cols<false><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale);
+    const dim3 gcol((a.nc + Rh - 1) / Rh, B), grow(H / Rw, B);
+    if (defocus) k_fo_cols<true><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign);
+    else k_fo_cols<false><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    const float sigma = (float)o->read_noise_sigma;
-    if (o->shot_noise_photons != 0.0)
-        k_fo_rows_inv<true><<<dim3(H / Rw, B), kFoThreads, smem_rows, c->stream>>>(a, d_intensity, sigma, o->shot_noise_photons, o->seed);
-    else
-        k_fo_rows_inv<false><<<dim3(H / Rw, B), kFoThreads, smem_rows, c->stream>>>(a, d_intensity, sigma, o->shot_noise_photons, o->seed);
+    if (mode == kFoSensorShot) k_fo_rows_inv<kFoSensorShot><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
+    else if (mode == kFoTimesReal) k_fo_rows_inv<kFoTimesReal><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
+    else if (mode == kFoGopd) k_fo_rows_inv<kFoGopd><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
+    else k_fo_rows_inv<kFoSensor><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
     return cudaGetLastError();
 }
 
+// L1-L3: intensity (with the sensor's noise) of the exit wave `field`
+cudaError_t launch_fused_optics(osog_ctx* c, const osog_optics* o, const float2* field, float2* spec_t, const float2* tw_w,
+                                const float2* tw_h, float* d_intensity)
+{
+    FoEpi ep = {};
+    ep.out = d_intensity;
+    ep.sigma = (float)o->read_noise_sigma; ep.photons = o->shot_noise_photons; ep.seed = o->seed;
+    return fo_run(c, o, field, spec_t, tw_w, tw_h, o->shot_noise_photons != 0.0 ? kFoSensorShot : kFoSensor, 1.0f, ep);
+}
 
-
+// Adjoint of L1-L3 (osog_backward_intensity): V = U * h_obj, g_V = (dL/dI) V into `work`; g_U = F^-1{conj(P) F{g_V}},
+// dL/dOPD = (4 pi / lambda) Im(g_U conj U) into d_gopd.  Two passes of the same three kernels; `field` (U) is only read.
+cudaError_t launch_fused_optics_adjoint(osog_ctx* c, const osog_optics* o, const float2* field, float2* work, float2* spec_t,
+                                        const float2* tw_w, const float2* tw_h, const float* d_gI, float* d_gopd)
+{
+    FoEpi ep = {};
+    ep.cout = work; ep.g = d_gI;
+    cudaError_t e = fo_run(c, o, field, spec_t, tw_w, tw_h, kFoTimesReal, 1.0f, ep);
+    if (e != cudaSuccess) return e;
+    FoEpi eq = {};
+    eq.out = d_gopd; eq.u = field; eq.optics = c->optics;
+    return fo_run(c, o, work, spec_t, tw_w, tw_h, kFoGopd, -1.0f, eq);
+}
 
 }  // namespace osog

@@ -105,6 +105,25 @@ int fft_frames(osog_ctx* c, float2* buf, int B, int sign, const float2* src = nu
     return OSOG_OK;
 }
 
+// first use of the fused library stage by this context: the kept-column scratch and the twiddle tables
+int ensure_fused_optics(osog_ctx* c)
+{
+    if (c->fo_ready) return OSOG_OK;
+    cudaError_t ea = cudaSuccess;
+    if (!c->spec_t) ea = dalloc(&c->spec_t, (size_t)c->max_frames * c->H * c->W, c);
+    if (ea == cudaSuccess && !c->tw_w) ea = dalloc(&c->tw_w, (size_t)c->W, c);
+    if (ea == cudaSuccess && c->H != c->W && !c->tw_h) ea = dalloc(&c->tw_h, (size_t)c->H, c);
+    if (ea == cudaSuccess) ea = launch_fo_twiddles(c, c->tw_w, c->W);
+    if (ea == cudaSuccess && c->H != c->W) ea = launch_fo_twiddles(c, c->tw_h, c->H);
+    if (ea != cudaSuccess) {                         // (what was allocated stays with the context and is reused by the next call)
+        cudaGetLastError();
+        return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea);
+    }
+    if (c->H == c->W) c->tw_h = c->tw_w;
+    c->fo_ready = true;
+    return OSOG_OK;
+}
+
 // forward FFT of the B frames of `src` into `buf` (src == nullptr: `buf` in place), pupil function, inverse FFT, then the
 // sensor into d_intensity
 int optics_stage(osog_ctx* c, const osog_optics* o, float2* buf, float* d_intensity, const float2* src = nullptr)
@@ -113,20 +132,8 @@ int optics_stage(osog_ctx* c, const osog_optics* o, float2* buf, float* d_intens
     if (fused_optics_applies(c)) {
         // power-of-two frames: row FFT -> [column FFT, pupil, inverse column FFT] of the columns the pupil keeps -> inverse row
         // FFT + sensor, three kernels of this library (optics.cu); the field is only read
-        if (!c->fo_ready) {                          // first call: the kept-column scratch and the twiddle tables
-            cudaError_t ea = cudaSuccess;
-            if (!c->spec_t) ea = dalloc(&c->spec_t, (size_t)c->max_frames * c->H * c->W, c);
-            if (ea == cudaSuccess && !c->tw_w) ea = dalloc(&c->tw_w, (size_t)c->W, c);
-            if (ea == cudaSuccess && c->H != c->W && !c->tw_h) ea = dalloc(&c->tw_h, (size_t)c->H, c);
-            if (ea == cudaSuccess) ea = launch_fo_twiddles(c, c->tw_w, c->W);
-            if (ea == cudaSuccess && c->H != c->W) ea = launch_fo_twiddles(c, c->tw_h, c->H);
-            if (ea != cudaSuccess) {                 // (what was allocated stays with the context and is reused by the next call)
-                cudaGetLastError();
-                return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea);
-            }
-            if (c->H == c->W) c->tw_h = c->tw_w;
-            c->fo_ready = true;
-        }
+        const int rs = ensure_fused_optics(c);
+        if (rs != OSOG_OK) return rs;
         const cudaError_t ef = launch_fused_optics(c, o, src ? src : buf, c->spec_t, c->tw_w, c->tw_h, d_intensity);
         return ef == cudaSuccess ? OSOG_OK : cuda_fail(c, ef);
     }
@@ -492,6 +499,11 @@ int osog_backward_intensity(osog_ctx* c, const osog_particles* p, int64_t N, con
     if (!c->work) {                                  // first call of this kind: a second complex batch
         const cudaError_t ea = dalloc(&c->work, (size_t)c->max_frames * c->H * c->W, c);
         if (ea != cudaSuccess) { cudaGetLastError(); c->work = nullptr; return ea == cudaErrorMemoryAllocation ? OSOG_ENOMEM : cuda_fail(c, ea); }
+    }
+    if (fused_optics_applies(c)) {                   // power-of-two frames: two passes of the three fused kernels (optics.cu)
+        if ((r = ensure_fused_optics(c)) != OSOG_OK) return r;
+        const cudaError_t ef = launch_fused_optics_adjoint(c, o, c->field, c->work, c->spec_t, c->tw_w, c->tw_h, d_gI, d_gopd);
+        return ef == cudaSuccess ? OSOG_OK : cuda_fail(c, ef);
     }
     const int B = o->B;
     const bool defocus = o->defocus_um != 0.0;

@@ -89,3 +89,24 @@ def test_fused_stage_batch_with_different_pupils_defocus_and_noise(og, o):
 def test_other_frame_sizes_keep_the_cufft_path(og, o):
     _check(og, o, _scene(96, 160, seed=3, NA=0.6))               # not powers of two
     _check(og, o, _scene(32, 64, seed=4, NA=0.6))                # below the smallest fused row
+
+
+@pytest.mark.parametrize("H,W,B,dz", [(256, 128, 3, 0.0), (128, 512, 1, 2.0), (64, 4096, 1, 0.0), (96, 160, 1, 1.0)])
+def test_adjoint_of_the_stage_fused_and_cufft_paths(og, o, H, W, B, dz):
+    """osog_backward_intensity runs the same three kernels twice on power-of-two frames (epilogues g_V = G V and
+    dL/dOPD = (4 pi / lambda) Im(g_U conj U), conjugated pupil) and keeps cuFFT elsewhere (96 x 160): the bar of
+    tests/test_gpu_backward.py."""
+    import torch
+    kw = dict(NA=[0.3, 0.8, 0.5][:B], lam=[0.45, 0.6, 0.55][:B]) if B > 1 else dict(NA=0.6, lam=0.5)
+    sc = replace(_scene(H, W, seed=7 * H + W, B=B, tilt_y_rad=-0.02, **kw), defocus_um=dz)
+    rng = np.random.default_rng(H + W)
+    GI = rng.standard_normal((sc.B, sc.H, sc.W)).astype(np.float32)
+    ctx = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B)
+    P, opt = og.Particles.from_scene(sc), og.optics_from_scene(sc)
+    g = ctx.backward_intensity(P, opt, torch.from_numpy(GI).cuda())
+    assert torch.equal(g, ctx.backward_intensity(P, opt, torch.from_numpy(GI).cuda()))
+    assert ctx.check_guards() == 0
+    ctx.close()
+    ref = o.backward_intensity(sc, GI)
+    err = np.abs(g.cpu().numpy().astype(np.float64) - ref).max()
+    assert err <= 2e-4 * np.abs(ref).max(), (err, np.abs(ref).max())
