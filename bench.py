@@ -419,6 +419,20 @@ def run_ours(args):
 
     t_steps, t_e2e = max_over_ranks([t_steps, t_e2e], dev)
     peak, peak_src = _peaks()
+    # library stage (L1-L3): bytes this design has to move on a power-of-two frame: field read, the kept
+    # columns written / read / written / read, intensity written; other frames (cuFFT path): SURVEY 8(d)'s 92 bytes per pixel
+    pow2 = all(v >= 64 and v <= 4096 and (v & (v - 1)) == 0 for v in (H, W))
+    if pow2:
+        rx = max(int(np.floor(float(scene.NA[b]) * scene.pitch_um / float(scene.lambda_um[b]) * W)) + 1 for b in range(B))
+        ncol = min(rx, W // 2 - 1) + min(rx, W // 2) + 1
+        lib_bytes = 8 * B * H * W + 4 * 8 * B * ncol * H + 4 * B * H * W
+    else:
+        ncol, lib_bytes = W, 92 * B * H * W
+    lib_gbs = lib_bytes / (ms_optics * 1e-3) / 1e9
+    lib_roof = {"bound": "hbm", "achieved": lib_gbs, "peak": peak, "unit": "GB/s", "frac": lib_gbs / peak,
+                "algorithmic_bytes": int(lib_bytes), "kept_columns": int(ncol), "stage_ms": ms_optics,
+                "what": "osog_field_to_intensity: k_fo_rows_fwd, k_fo_cols, k_fo_rows_inv" if pow2 else "osog_field_to_intensity: cuFFT x 2, k_pupil, k_sensor",
+                "note": "bytes of THIS design (pruned to the pupil's columns); SURVEY 8(d) counts 92 bytes per pixel for the unpruned stage"}
     alg_bytes = 48 * N + 8 * pairs + 8 * B * H * W      # SoA read + list write/read + complex64 write
     ms_step = t_steps / args.steps * 1e3
     step_gbs = alg_bytes / (ms_step * 1e-3) / 1e9
@@ -472,6 +486,7 @@ def run_ours(args):
         "roofline": roof, "roofline_hbm": hbm,
         "roofline_step": {"achieved": step_gbs, "frac": step_gbs / peak, "algorithmic_bytes": int(alg_bytes),
                           "what": "whole hot path: k_prepare, k_sort_cull, k_compose_tile"},
+        "roofline_library": lib_roof,
         "library_stage_ms": ms_optics, "dic_stage_ms": ms_dic, "gbuffer_ms": ms_gbuffer, "height_grad_lap_ms": ms_height, "backward_np_ms": ms_backward, "backward_centre_ms": ms_backward_c, "backward_params_ms": ms_backward_p, "backward_particles_ms": ms_backward_all, "backward_intensity_ms": ms_backward_i, "opd_only_ms": ms_opd, "atomic_alternative_opd_ms": ms_atomic, "smem_atomic_alternative_opd_ms": ms_smem_atomic,
         "paper_context": "PAPER.md:195: 40,000 particles < 50 ms on one A100 at 1024^2 (whole pipeline); context only",
         "clocks": clk.summary(),
