@@ -712,17 +712,44 @@ __device__ __forceinline__ int fo_kx(const FoArgs& a, int c)
     return m < 0 ? m + a.W : m;
 }
 
-// K1: forward row transforms, kFoThreads / (W / 8) rows per CTA; the kept columns are written transposed
-__global__ void __launch_bounds__(kFoThreads) k_fo_rows_fwd(const FoArgs a, const float2* __restrict__ field)
+struct FoShear {                   // DIC prologue of K1 (Eq. 5): D = |U(r + ds) e^{i theta} - U(r - ds) e^{-i theta}|^2
+    int sx, sy;
+    float2 e;                      // (cos theta, sin theta)
+};
+
+// K1: forward row transforms, kFoThreads / (W / 8) rows per CTA; the kept columns are written transposed.
+// SHEAR: the row that is transformed is the DIC interference image D of the field (real), formed on the fly.
+template <bool SHEAR>
+__global__ void __launch_bounds__(kFoThreads) k_fo_rows_fwd(const FoArgs a, const float2* __restrict__ field, const FoShear sh)
 {
     extern __shared__ __align__(16) float2 fo_x[];
     const int lgT = a.pw.lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, R = 1 << lgR, stride = a.W + (a.W >> 3);
     const int r = threadIdx.x >> lgT, t = threadIdx.x & (T - 1), b = blockIdx.y, row0 = blockIdx.x << lgR;
     float2* xr = fo_x + r * stride;
-    const float2* src = field + ((size_t)b * a.H + row0 + r) * a.W + t;
     float2 v[8];
+    if (!SHEAR) {
+        const float2* src = field + ((size_t)b * a.H + row0 + r) * a.W + t;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) v[k] = src[k << lgT];
+        for (int k = 0; k < 8; ++k) v[k] = src[k << lgT];
+    } else {
+        const int i = row0 + r;
+        int ip = i + sh.sy, im = i - sh.sy;                          // |sy| < H, |sx| < W: one wrap each (readings A21, A22)
+        ip += ip < 0 ? a.H : (ip >= a.H ? -a.H : 0);
+        im += im < 0 ? a.H : (im >= a.H ? -a.H : 0);
+        const float2* fp = field + ((size_t)b * a.H + ip) * a.W;
+        const float2* fm = field + ((size_t)b * a.H + im) * a.W;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int j = t + (k << lgT);
+            int jp = j + sh.sx, jm = j - sh.sx;
+            jp += jp < 0 ? a.W : (jp >= a.W ? -a.W : 0);
+            jm += jm < 0 ? a.W : (jm >= a.W ? -a.W : 0);
+            const float2 up = fp[jp], um = fm[jm];
+            const float dr = (up.x * sh.e.x - up.y * sh.e.y) - (um.x * sh.e.x + um.y * sh.e.y);
+            const float di = (up.x * sh.e.y + up.y * sh.e.x) - (um.y * sh.e.x - um.x * sh.e.y);
+            v[k] = make_float2(dr * dr + di * di, 0.0f);
+        }
+    }
     fo_forward(v, t, a.pw, a.tw_w, xr);
 #pragma unroll
     for (int m = 0; m < 8; ++m) xr[(m << lgT) + t] = v[m];          // position 8 t + m, stored transposed (conflict free)
@@ -734,10 +761,12 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_rows_fwd(const FoArgs a, cons
     }
 }
 
-// K2: kept columns: forward transform along y, pupil (times 1 / (H W)), inverse transform along y, in place
-template <bool DEFOCUS>
+// K2: kept columns: forward transform along y, multiplication, inverse transform along y, in place.
+// MUL = 0 / 1: the pupil function (without / with the defocus phase) times scale = 1 / (H W); MUL = 2: scale times the
+// transfer-function array tf[B][H][W] (natural FFT order; the DIC stage's OTF)
+template <int MUL>
 __global__ void __launch_bounds__(kFoThreads) k_fo_cols(const FoArgs a, const FrameOptics* __restrict__ optics, double inv_wp,
-                                                        double inv_hp, float scale, float imag_sign)
+                                                        double inv_hp, float scale, float imag_sign, const float2* __restrict__ tf)
 {
     extern __shared__ __align__(16) float2 fo_x[];
     const int lgT = a.ph.lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, stride = a.H + (a.H >> 3);
@@ -753,9 +782,15 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_cols(const FoArgs a, const Fr
     const FrameOptics fo = optics[b];
 #pragma unroll
     for (int m = 0; m < 8; ++m) {
-        float2 pv = pupil_value<DEFOCUS>(fo, kx, fo_freq_of_pos(a.ph, 8 * t + m), a.H, a.W, inv_wp, inv_hp, scale);
-        if (DEFOCUS) pv.y *= imag_sign;                              // -1: conj(P), the adjoint of the stage
-        v[m] = DEFOCUS ? fo_cmul(v[m], pv) : make_float2(v[m].x * pv.x, v[m].y * pv.x);
+        const int ky = fo_freq_of_pos(a.ph, 8 * t + m);
+        if (MUL == 2) {
+            const float2 w = __ldg(tf + ((size_t)b * a.H + ky) * a.W + kx);
+            v[m] = fo_cmul(v[m], make_float2(w.x * scale, w.y * scale));
+        } else {
+            float2 pv = pupil_value<MUL == 1>(fo, kx, ky, a.H, a.W, inv_wp, inv_hp, scale);
+            if (MUL == 1) pv.y *= imag_sign;                         // -1: conj(P), the adjoint of the stage
+            v[m] = MUL == 1 ? fo_cmul(v[m], pv) : make_float2(v[m].x * pv.x, v[m].y * pv.x);
+        }
     }
     fo_inverse(v, t, a.ph, a.tw_h, xr);
     if (valid) {
@@ -765,7 +800,7 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_cols(const FoArgs a, const Fr
 }
 
 // what K3 does with the image V it has transformed back
-enum { kFoSensor = 0, kFoSensorShot = 1, kFoTimesReal = 2, kFoGopd = 3 };
+enum { kFoSensor = 0, kFoSensorShot = 1, kFoTimesReal = 2, kFoGopd = 3, kFoRealSensor = 4, kFoRealSensorShot = 5 };
 struct FoEpi {
     float* out;                    // sensor: intensity [B, H, W]; kFoGopd: dL/dOPD [B, H, W]
     float2* cout;                  // kFoTimesReal: g_V = g V [B, H, W] complex
@@ -811,8 +846,8 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_rows_inv(const FoArgs a, cons
             const float kk = (float)(12.566370614359172 * ep.optics[b].inv_lambda);
             ep.out[gpix] = kk * (v[k].y * w.x - v[k].x * w.y);
         } else {
-            float I = v[k].x * v[k].x + v[k].y * v[k].y;
-            if (MODE == kFoSensorShot)
+            float I = (MODE == kFoRealSensor || MODE == kFoRealSensorShot) ? v[k].x : v[k].x * v[k].x + v[k].y * v[k].y;
+            if (MODE == kFoSensorShot || MODE == kFoRealSensorShot)
                 I = (float)(poisson_draw(ep.photons * fmax((double)I, 0.0), ep.seed, (uint32_t)b, (uint32_t)pix) / ep.photons);
             if (ep.sigma != 0.0f) I = fmaf(ep.sigma, read_noise_z(ep.seed, (uint32_t)b, (uint32_t)pix), I);
             ep.out[gpix] = I;
@@ -842,8 +877,10 @@ bool fused_optics_applies(const osog_ctx* c)
 }
 
 // in: [B, H, W] complex frames (read only); spec_t: scratch of B * W * H complex values; tw_w / tw_h: twiddle tables of W / H
+// tf == nullptr: multiply by the pupil function; else by the transfer-function array tf (support: twice the pupil's radius);
+// sh != nullptr: K1 transforms the DIC interference image of `in`
 static cudaError_t fo_run(osog_ctx* c, const osog_optics* o, const float2* in, float2* spec_t, const float2* tw_w, const float2* tw_h,
-                          int mode, float imag_sign, const FoEpi& ep)
+                          int mode, float imag_sign, const FoEpi& ep, const float2* tf = nullptr, const FoShear* sh = nullptr)
 {
     const int B = o->B, H = c->H, W = c->W;
     FoArgs a;
@@ -856,7 +893,7 @@ static cudaError_t fo_run(osog_ctx* c, const osog_optics* o, const float2* in, f
         long long rb = W;                                         // all-pass
         if (o->pupil_enabled && o->NA != nullptr) {
             const double r = o->NA[b] * o->pitch_um / o->lambda_um[b] * (double)W;
-            if (r < (double)W) rb = (long long)floor(r) + 1;
+            if (r < (double)W) rb = (long long)floor(tf ? 2.0 * r : r) + (tf ? 2 : 1);    // (the autocorrelation of the pupil)
         }
         rx = rb > rx ? rb : rx;
     }
@@ -869,15 +906,19 @@ static cudaError_t fo_run(osog_ctx* c, const osog_optics* o, const float2* in, f
     const int Rw = kFoThreads / (W / 8), Rh = kFoThreads / (H / 8);           // rows / columns per CTA
     const size_t smem_rows = (size_t)Rw * (W + W / 8) * sizeof(float2), smem_cols = (size_t)Rh * (H + H / 8) * sizeof(float2);
     cudaError_t e;
-    k_fo_rows_fwd<<<dim3(H / Rw, B), kFoThreads, smem_rows, c->stream>>>(a, in);
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
     const dim3 gcol((a.nc + Rh - 1) / Rh, B), grow(H / Rw, B);
-    if (defocus) k_fo_cols<true><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign);
-    else k_fo_cols<false><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign);
+    if (sh) k_fo_rows_fwd<true><<<grow, kFoThreads, smem_rows, c->stream>>>(a, in, *sh);
+    else k_fo_rows_fwd<false><<<grow, kFoThreads, smem_rows, c->stream>>>(a, in, FoShear{0, 0, make_float2(1.f, 0.f)});
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if (tf) k_fo_cols<2><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign, tf);
+    else if (defocus) k_fo_cols<1><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign, nullptr);
+    else k_fo_cols<0><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign, nullptr);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     if (mode == kFoSensorShot) k_fo_rows_inv<kFoSensorShot><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
     else if (mode == kFoTimesReal) k_fo_rows_inv<kFoTimesReal><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
     else if (mode == kFoGopd) k_fo_rows_inv<kFoGopd><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
+    else if (mode == kFoRealSensor) k_fo_rows_inv<kFoRealSensor><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
+    else if (mode == kFoRealSensorShot) k_fo_rows_inv<kFoRealSensorShot><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
     else k_fo_rows_inv<kFoSensor><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
     return cudaGetLastError();
 }
@@ -890,6 +931,19 @@ cudaError_t launch_fused_optics(osog_ctx* c, const osog_optics* o, const float2*
     ep.out = d_intensity;
     ep.sigma = (float)o->read_noise_sigma; ep.photons = o->shot_noise_photons; ep.seed = o->seed;
     return fo_run(c, o, field, spec_t, tw_w, tw_h, o->shot_noise_photons != 0.0 ? kFoSensorShot : kFoSensor, 1.0f, ep);
+}
+
+// DIC stage (Eq. 5) with a ready transfer function: I = Re F^-1{ F{D} OTF / (H W) }, D the interference image of `field`
+cudaError_t launch_fused_dic(osog_ctx* c, const osog_optics* o, const float2* field, const float2* otf, float2* spec_t,
+                             const float2* tw_w, const float2* tw_h, int sx, int sy, double bias_rad, float* d_dic)
+{
+    FoEpi ep = {};
+    ep.out = d_dic;
+    ep.sigma = (float)o->read_noise_sigma; ep.photons = o->shot_noise_photons; ep.seed = o->seed;
+    FoShear sh;
+    sh.sx = sx; sh.sy = sy;
+    sh.e = make_float2((float)cos(bias_rad), (float)sin(bias_rad));
+    return fo_run(c, o, field, spec_t, tw_w, tw_h, o->shot_noise_photons != 0.0 ? kFoRealSensorShot : kFoRealSensor, 1.0f, ep, otf, &sh);
 }
 
 // Adjoint of L1-L3 (osog_backward_intensity): V = U * h_obj, g_V = (dL/dI) V into `work`; g_U = F^-1{conj(P) F{g_V}},

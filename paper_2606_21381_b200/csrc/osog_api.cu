@@ -156,8 +156,10 @@ int check_dic(const osog_ctx* c, const osog_dic* d)
 }
 
 // Eq. 5 on the B frames of U held in c->field (overwritten): see include/osog.h, osog_render_dic
-int dic_stage(osog_ctx* c, const osog_optics* o, const osog_dic* d, float* d_dic)
+// field: the exit wave (only read); nullptr = the context's own frame batch
+int dic_stage(osog_ctx* c, const osog_optics* o, const osog_dic* d, float* d_dic, const float2* field = nullptr)
 {
+    if (!field) field = c->field;
     const int B = o->B;
     const double hw = (double)c->H * c->W;
     if (!c->work || !c->otf) {                       // first DIC call of this context: two more complex batches
@@ -172,9 +174,12 @@ int dic_stage(osog_ctx* c, const osog_optics* o, const osog_dic* d, float* d_dic
     const bool defocus = o->defocus_um != 0.0;
     cudaError_t e;
     int r;
+    const bool fused = fused_optics_applies(c);      // power-of-two frames: the three fused kernels of optics.cu (below)
     // D = |U(r+ds) e^{i theta} - U(r-ds) e^{-i theta}|^2 and its spectrum
-    if ((e = launch_dic_shear(c, B, c->field, c->work, d->shear_x_px, d->shear_y_px, d->bias_rad)) != cudaSuccess) return cuda_fail(c, e);
-    if ((r = fft_frames(c, c->work, B, CUFFT_FORWARD)) != OSOG_OK) return r;
+    if (!fused) {
+        if ((e = launch_dic_shear(c, B, field, c->work, d->shear_x_px, d->shear_y_px, d->bias_rad)) != cudaSuccess) return cuda_fail(c, e);
+        if ((r = fft_frames(c, c->work, B, CUFFT_FORWARD)) != OSOG_OK) return r;
+    }
     // optical transfer function: P -> h_obj = F^-1{P} -> |h_obj|^2 -> F{.}; it depends on the optics alone, so it is kept
     // and rebuilt only when they change (the same stream orders the rebuild against earlier readers)
     std::vector<double> key = {(double)B, o->pitch_um, o->n_medium, o->defocus_um, (double)(o->pupil_enabled != 0)};
@@ -191,6 +196,13 @@ int dic_stage(osog_ctx* c, const osog_optics* o, const osog_dic* d, float* d_dic
         *c->otf_key = key;
     }
     // I = F^-1{ F{D} OTF }
+    if (fused) {
+        // row FFT of D (formed on the fly from the field) -> [column FFT, x OTF / (H W), inverse column FFT] of the columns inside
+        // the OTF's support (twice the pupil's radius) -> inverse row FFT, real part, sensor
+        if ((r = ensure_fused_optics(c)) != OSOG_OK) return r;
+        e = launch_fused_dic(c, o, field, c->otf, c->spec_t, c->tw_w, c->tw_h, d->shear_x_px, d->shear_y_px, d->bias_rad, d_dic);
+        return e == cudaSuccess ? OSOG_OK : cuda_fail(c, e);
+    }
     if ((e = launch_cmul(c, B, c->work, c->otf, 1.0 / hw)) != cudaSuccess) return cuda_fail(c, e);
     if ((r = fft_frames(c, c->work, B, CUFFT_INVERSE)) != OSOG_OK) return r;
     if ((e = launch_sensor_real(c, B, c->work, d_dic, o->read_noise_sigma, o->shot_noise_photons, o->seed)) != cudaSuccess) return cuda_fail(c, e);
@@ -418,9 +430,7 @@ int osog_field_to_dic(osog_ctx* c, const osog_optics* o, const osog_dic* d, cons
     DeviceGuard g(c->device);
     cudaError_t e = upload_optics(c, o, nullptr);
     if (e != cudaSuccess) return cuda_fail(c, e);
-    e = cudaMemcpyAsync(c->field, d_field, sizeof(float2) * (size_t)o->B * c->H * c->W, cudaMemcpyDeviceToDevice, c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e);
-    return dic_stage(c, o, d, d_dic);
+    return dic_stage(c, o, d, d_dic, reinterpret_cast<const float2*>(d_field));      // (the stage only reads the field: no copy)
 }
 
 int osog_render_opd_atomic(osog_ctx* c, const osog_particles* p, int64_t N, const osog_optics* o, float* d_opd)

@@ -189,6 +189,8 @@ bool fused_optics_applies(const osog_ctx* c);       // power-of-two frames, 64 .
 cudaError_t launch_fo_twiddles(osog_ctx* c, float2* tw, int n);
 cudaError_t launch_fused_optics(osog_ctx* c, const osog_optics* o, const float2* field, float2* spec_t, const float2* tw_w,
                                 const float2* tw_h, float* d_intensity);
+cudaError_t launch_fused_dic(osog_ctx* c, const osog_optics* o, const float2* field, const float2* otf, float2* spec_t,
+                             const float2* tw_w, const float2* tw_h, int sx, int sy, double bias_rad, float* d_dic);
 cudaError_t launch_fused_optics_adjoint(osog_ctx* c, const osog_optics* o, const float2* field, float2* work, float2* spec_t,
                                         const float2* tw_w, const float2* tw_h, const float* d_gI, float* d_gopd);
 cudaError_t launch_poisson(osog_ctx* c, const float* d_lam, size_t n, uint64_t seed, uint32_t frame, int32_t* d_counts);

@@ -110,3 +110,22 @@ def test_adjoint_of_the_stage_fused_and_cufft_paths(og, o, H, W, B, dz):
     ref = o.backward_intensity(sc, GI)
     err = np.abs(g.cpu().numpy().astype(np.float64) - ref).max()
     assert err <= 2e-4 * np.abs(ref).max(), (err, np.abs(ref).max())
+
+
+@pytest.mark.parametrize("H,W,B,shear,dz,pupil", [(128, 512, 1, (3, -2), 1.0, True), (256, 64, 2, (-30, 100), 0.0, True),
+                                                  (64, 128, 1, (1, 1), 0.0, False)])
+def test_dic_stage_fused_path(og, o, H, W, B, shear, dz, pupil):
+    """The DIC image on power-of-two frames: K1 forms the interference image on the fly, K2 multiplies the kept columns (twice the
+    pupil's radius: the support of the transfer function) by the cached OTF.  Bar of tests/test_gpu_defocus_dic.py."""
+    kw = dict(NA=[0.35, 0.8][:B], lam=[0.5, 0.62][:B]) if B > 1 else dict(NA=0.6, lam=0.5)
+    sc = replace(_scene(H, W, seed=11 * H + W, B=B, tilt_x_rad=0.02, **kw), defocus_um=dz)
+    ctx = og.Context(sc.H, sc.W, sc.N, max_frames=sc.B)
+    P, opt = og.Particles.from_scene(sc), og.optics_from_scene(sc, pupil_enabled=pupil)
+    dic = og.make_dic(shear[0], shear[1], 0.4)
+    g = ctx.render_dic(P, opt, dic).clone()
+    assert bool((g == ctx.render_dic(P, opt, dic)).all()) and ctx.check_guards() == 0
+    ctx.close()
+    ref = o.render_dic(sc, shear, 0.4, pupil_enabled=pupil)
+    tol = 1e-4 * max(ref.mean(), 1e-3)
+    err = np.abs(g.cpu().numpy().astype(np.float64) - ref).max()
+    assert err <= tol, (err, tol)
