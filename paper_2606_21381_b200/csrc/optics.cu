@@ -467,28 +467,24 @@ cudaError_t launch_sensor_real(osog_ctx* c, int B, const float2* img, float* d_o
 // the conjugate-transposed stages in reverse order: no reordering pass, and the stage next to the pupil needs no exchange.
 constexpr int kFoThreads = 512;                     // threads per CTA (one row of 4096, two of 2048, ...)
 
+// compile-time plan of a transform of length n = 2^LG = 2^lg_r1 * 8^(nstage - 1): every shift below is a constant and every
+// stage loop unrolls (the run-time version of this code spent two thirds of its instructions on index arithmetic)
+template <int LG>
 struct FoPlan {
-    int n, lg_n, lg_r1, nstage;       // n = 2^lg_n = 2^lg_r1 * 8^(nstage - 1)
+    static constexpr int lg_n = LG, n = 1 << LG;
+    static constexpr int lg_r1 = LG % 3 == 0 ? 3 : LG % 3;
+    static constexpr int nstage = 1 + (LG - lg_r1) / 3;
 };
 
-static FoPlan fo_plan(int n)
-{
-    FoPlan p;
-    p.n = n;
-    p.lg_n = 0;
-    while ((1 << p.lg_n) < n) ++p.lg_n;
-    p.lg_r1 = p.lg_n % 3 == 0 ? 3 : p.lg_n % 3;
-    p.nstage = 1 + (p.lg_n - p.lg_r1) / 3;
-    return p;
-}
-
 // position p of the digit-reversed spectrum holds frequency k:  p = m1 n/r1 + m2 n/(r1 r2) + ...,  k = m1 + r1 (m2 + r2 (...))
-__device__ __forceinline__ int fo_freq_of_pos(const FoPlan& pl, int p)
+template <class PL>
+__device__ __forceinline__ int fo_freq_of_pos(int p)
 {
-    int lg_L = pl.lg_n - pl.lg_r1;
-    int k = p >> lg_L, sh = pl.lg_r1;
+    int lg_L = PL::lg_n - PL::lg_r1;
+    int k = p >> lg_L, sh = PL::lg_r1;
     p &= (1 << lg_L) - 1;
-    for (int s = 1; s < pl.nstage; ++s) {
+#pragma unroll
+    for (int s = 1; s < PL::nstage; ++s) {
         lg_L -= 3;
         k += (p >> lg_L) << sh;
         p &= (1 << lg_L) - 1;
@@ -496,12 +492,14 @@ __device__ __forceinline__ int fo_freq_of_pos(const FoPlan& pl, int p)
     }
     return k;
 }
-__device__ __forceinline__ int fo_pos_of_freq(const FoPlan& pl, int k)
+template <class PL>
+__device__ __forceinline__ int fo_pos_of_freq(int k)
 {
-    int lg_L = pl.lg_n - pl.lg_r1;
-    int p = (k & ((1 << pl.lg_r1) - 1)) << lg_L;
-    k >>= pl.lg_r1;
-    for (int s = 1; s < pl.nstage; ++s) {
+    int lg_L = PL::lg_n - PL::lg_r1;
+    int p = (k & ((1 << PL::lg_r1) - 1)) << lg_L;
+    k >>= PL::lg_r1;
+#pragma unroll
+    for (int s = 1; s < PL::nstage; ++s) {
         lg_L -= 3;
         p += (k & 7) << lg_L;
         k >>= 3;
@@ -577,13 +575,14 @@ __device__ __forceinline__ void fo_twiddle8(float2 (&a)[8], int q, int lg_step, 
 }
 
 // first forward stage (block length n, radix r1) on a[k] = x[t + k T], T = n / 8, in place (positions unchanged)
-__device__ __forceinline__ void fo_first_fwd(float2 (&a)[8], int t, const FoPlan& pl, const float2* __restrict__ tw)
+template <class PL>
+__device__ __forceinline__ void fo_first_fwd(float2 (&a)[8], int t, const float2* __restrict__ tw)
 {
-    const int T = pl.n >> 3;
-    if (pl.lg_r1 == 3) {
+    const int T = PL::n >> 3;
+    if (PL::lg_r1 == 3) {
         fo_r8(a);
         fo_twiddle8<false>(a, t, 0, tw);
-    } else if (pl.lg_r1 == 2) {
+    } else if (PL::lg_r1 == 2) {
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
             const int q = t + i * T;
@@ -602,17 +601,18 @@ __device__ __forceinline__ void fo_first_fwd(float2 (&a)[8], int t, const FoPlan
     }
 }
 // its conjugate transpose (last inverse stage)
-__device__ __forceinline__ void fo_first_inv(float2 (&a)[8], int t, const FoPlan& pl, const float2* __restrict__ tw)
+template <class PL>
+__device__ __forceinline__ void fo_first_inv(float2 (&a)[8], int t, const float2* __restrict__ tw)
 {
-    const int T = pl.n >> 3;
-    if (pl.lg_r1 == 3) {
+    const int T = PL::n >> 3;
+    if (PL::lg_r1 == 3) {
         fo_twiddle8<true>(a, t, 0, tw);
 #pragma unroll
         for (int m = 0; m < 8; ++m) a[m] = fo_conj(a[m]);
         fo_r8(a);
 #pragma unroll
         for (int m = 0; m < 8; ++m) a[m] = fo_conj(a[m]);
-    } else if (pl.lg_r1 == 2) {
+    } else if (PL::lg_r1 == 2) {
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
             const int q = t + i * T;
@@ -634,12 +634,14 @@ __device__ __forceinline__ void fo_first_inv(float2 (&a)[8], int t, const FoPlan
 
 // Forward transform of one row held as a[k] = x[t + k T]; on return a[m] is the value at digit-reversed position 8 t + m.
 // xr: this row's exchange buffer in shared memory (9 n / 8 elements); every thread of the CTA must call (barriers inside).
-__device__ __forceinline__ void fo_forward(float2 (&a)[8], int t, const FoPlan& pl, const float2* __restrict__ tw, float2* xr)
+template <class PL>
+__device__ __forceinline__ void fo_forward(float2 (&a)[8], int t, const float2* __restrict__ tw, float2* xr)
 {
-    fo_first_fwd(a, t, pl, tw);
-    int lg_L = pl.lg_n, lg_sub = pl.lg_n - 3, blk = 0, q = t;    // positions of a[k]: (blk << lg_L) + q + (k << lg_sub)
-    int lg_Ln = pl.lg_n - pl.lg_r1;                               // block length of the next stage
-    for (int s = 1; s < pl.nstage; ++s) {
+    fo_first_fwd<PL>(a, t, tw);
+    int lg_L = PL::lg_n, lg_sub = PL::lg_n - 3, blk = 0, q = t;    // positions of a[k]: (blk << lg_L) + q + (k << lg_sub)
+    int lg_Ln = PL::lg_n - PL::lg_r1;                               // block length of the next stage
+#pragma unroll
+    for (int s = 1; s < PL::nstage; ++s) {
         {
             float2* w = xr + fo_phys((blk << lg_L) + q);
             const int st = fo_stride(lg_sub);
@@ -657,17 +659,19 @@ __device__ __forceinline__ void fo_forward(float2 (&a)[8], int t, const FoPlan& 
         }
         __syncthreads();
         fo_r8(a);
-        if (lg_sub > 0) fo_twiddle8<false>(a, q, pl.lg_n - lg_L, tw);
+        if (lg_sub > 0) fo_twiddle8<false>(a, q, PL::lg_n - lg_L, tw);
         lg_Ln = lg_sub;
     }
 }
 // Inverse (unnormalised): a[m] at digit-reversed position 8 t + m on entry, a[k] = x[t + k T] on return.
-__device__ __forceinline__ void fo_inverse(float2 (&a)[8], int t, const FoPlan& pl, const float2* __restrict__ tw, float2* xr)
+template <class PL>
+__device__ __forceinline__ void fo_inverse(float2 (&a)[8], int t, const float2* __restrict__ tw, float2* xr)
 {
     int lg_L = 3, lg_sub = 0;
-    for (int s = pl.nstage - 1; s >= 1; --s) {
+#pragma unroll
+    for (int s = PL::nstage - 1; s >= 1; --s) {
         const int blk = t >> lg_sub, q = t & ((1 << lg_sub) - 1);
-        if (lg_sub > 0) fo_twiddle8<true>(a, q, pl.lg_n - lg_L, tw);
+        if (lg_sub > 0) fo_twiddle8<true>(a, q, PL::lg_n - lg_L, tw);
 #pragma unroll
         for (int m = 0; m < 8; ++m) a[m] = fo_conj(a[m]);
         fo_r8(a);
@@ -682,7 +686,7 @@ __device__ __forceinline__ void fo_inverse(float2 (&a)[8], int t, const FoPlan& 
         __syncthreads();
         // the stage before: block length 8 L (the first stage: n, whatever its radix; its threads hold x[t + k n / 8])
         int lg_Lp, lg_subp;
-        if (s == 1) { lg_Lp = pl.lg_n; lg_subp = pl.lg_n - 3; }
+        if (s == 1) { lg_Lp = PL::lg_n; lg_subp = PL::lg_n - 3; }
         else { lg_Lp = lg_L + 3; lg_subp = lg_L; }
         const int blkp = t >> lg_subp, qp = t & ((1 << lg_subp) - 1);
         {
@@ -694,11 +698,10 @@ __device__ __forceinline__ void fo_inverse(float2 (&a)[8], int t, const FoPlan& 
         __syncthreads();
         lg_L = lg_Lp; lg_sub = lg_subp;
     }
-    fo_first_inv(a, t, pl, tw);
+    fo_first_inv<PL>(a, t, tw);
 }
 
 struct FoArgs {
-    FoPlan pw, ph;                 // row (length W) and column (length H) transforms
     const float2* tw_w;            // exp(-2 pi i k / W)
     const float2* tw_h;            // exp(-2 pi i k / H)
     int H, W;
@@ -719,11 +722,11 @@ struct FoShear {                   // DIC prologue of K1 (Eq. 5): D = |U(r + ds)
 
 // K1: forward row transforms, kFoThreads / (W / 8) rows per CTA; the kept columns are written transposed.
 // SHEAR: the row that is transformed is the DIC interference image D of the field (real), formed on the fly.
-template <bool SHEAR>
+template <class PL, bool SHEAR>
 __global__ void __launch_bounds__(kFoThreads) k_fo_rows_fwd(const FoArgs a, const float2* __restrict__ field, const FoShear sh)
 {
     extern __shared__ __align__(16) float2 fo_x[];
-    const int lgT = a.pw.lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, R = 1 << lgR, stride = a.W + (a.W >> 3);
+    constexpr int lgT = PL::lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, R = 1 << lgR, stride = PL::n + (PL::n >> 3);
     const int r = threadIdx.x >> lgT, t = threadIdx.x & (T - 1), b = blockIdx.y, row0 = blockIdx.x << lgR;
     float2* xr = fo_x + r * stride;
     float2 v[8];
@@ -750,13 +753,13 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_rows_fwd(const FoArgs a, cons
             v[k] = make_float2(dr * dr + di * di, 0.0f);
         }
     }
-    fo_forward(v, t, a.pw, a.tw_w, xr);
+    fo_forward<PL>(v, t, a.tw_w, xr);
 #pragma unroll
     for (int m = 0; m < 8; ++m) xr[(m << lgT) + t] = v[m];          // position 8 t + m, stored transposed (conflict free)
     __syncthreads();
     for (int idx = threadIdx.x; idx < (a.nc << lgR); idx += kFoThreads) {
         const int rr = idx & (R - 1), c = idx >> lgR;
-        const int p = fo_pos_of_freq(a.pw, fo_kx(a, c));
+        const int p = fo_pos_of_freq<PL>(fo_kx(a, c));
         a.spec_t[((size_t)b * a.nc + c) * a.H + row0 + rr] = fo_x[rr * stride + ((p & 7) << lgT) + (p >> 3)];
     }
 }
@@ -764,12 +767,12 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_rows_fwd(const FoArgs a, cons
 // K2: kept columns: forward transform along y, multiplication, inverse transform along y, in place.
 // MUL = 0 / 1: the pupil function (without / with the defocus phase) times scale = 1 / (H W); MUL = 2: scale times the
 // transfer-function array tf[B][H][W] (natural FFT order; the DIC stage's OTF)
-template <int MUL>
+template <class PL, int MUL>
 __global__ void __launch_bounds__(kFoThreads) k_fo_cols(const FoArgs a, const FrameOptics* __restrict__ optics, double inv_wp,
                                                         double inv_hp, float scale, float imag_sign, const float2* __restrict__ tf)
 {
     extern __shared__ __align__(16) float2 fo_x[];
-    const int lgT = a.ph.lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, stride = a.H + (a.H >> 3);
+    constexpr int lgT = PL::lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, stride = PL::n + (PL::n >> 3);
     const int r = threadIdx.x >> lgT, t = threadIdx.x & (T - 1), b = blockIdx.y, c = (blockIdx.x << lgR) + r;
     const bool valid = c < a.nc;
     float2* xr = fo_x + r * stride;
@@ -777,12 +780,12 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_cols(const FoArgs a, const Fr
     float2 v[8];
 #pragma unroll
     for (int k = 0; k < 8; ++k) v[k] = valid ? col[k << lgT] : make_float2(0.f, 0.f);
-    fo_forward(v, t, a.ph, a.tw_h, xr);
+    fo_forward<PL>(v, t, a.tw_h, xr);
     const int kx = fo_kx(a, valid ? c : 0);
     const FrameOptics fo = optics[b];
 #pragma unroll
     for (int m = 0; m < 8; ++m) {
-        const int ky = fo_freq_of_pos(a.ph, 8 * t + m);
+        const int ky = fo_freq_of_pos<PL>(8 * t + m);
         if (MUL == 2) {
             const float2 w = __ldg(tf + ((size_t)b * a.H + ky) * a.W + kx);
             v[m] = fo_cmul(v[m], make_float2(w.x * scale, w.y * scale));
@@ -792,7 +795,7 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_cols(const FoArgs a, const Fr
             v[m] = MUL == 1 ? fo_cmul(v[m], pv) : make_float2(v[m].x * pv.x, v[m].y * pv.x);
         }
     }
-    fo_inverse(v, t, a.ph, a.tw_h, xr);
+    fo_inverse<PL>(v, t, a.tw_h, xr);
     if (valid) {
 #pragma unroll
         for (int k = 0; k < 8; ++k) col[k << lgT] = v[k];
@@ -814,18 +817,18 @@ struct FoEpi {
 
 // K3: inverse row transforms from the kept columns (all other bins are zero), then the sensor (I = |V|^2, shot and read noise),
 // or, for the adjoint of the stage (osog_backward_intensity), g_V = (dL/dI) V  resp.  dL/dOPD = (4 pi / lambda) Im(g_U conj U)
-template <int MODE>
+template <class PL, int MODE>
 __global__ void __launch_bounds__(kFoThreads) k_fo_rows_inv(const FoArgs a, const FoEpi ep)
 {
     extern __shared__ __align__(16) float2 fo_x[];
-    const int lgT = a.pw.lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, R = 1 << lgR, stride = a.W + (a.W >> 3);
+    constexpr int lgT = PL::lg_n - 3, T = 1 << lgT, lgR = 9 - lgT, R = 1 << lgR, stride = PL::n + (PL::n >> 3);
     const int r = threadIdx.x >> lgT, t = threadIdx.x & (T - 1), b = blockIdx.y, row0 = blockIdx.x << lgR;
     float2* xr = fo_x + r * stride;
     for (int k = threadIdx.x; k < R * stride; k += kFoThreads) fo_x[k] = make_float2(0.f, 0.f);
     __syncthreads();
     for (int idx = threadIdx.x; idx < (a.nc << lgR); idx += kFoThreads) {
         const int rr = idx & (R - 1), c = idx >> lgR;
-        const int p = fo_pos_of_freq(a.pw, fo_kx(a, c));
+        const int p = fo_pos_of_freq<PL>(fo_kx(a, c));
         fo_x[rr * stride + ((p & 7) << lgT) + (p >> 3)] = a.spec_t[((size_t)b * a.nc + c) * a.H + row0 + rr];
     }
     __syncthreads();
@@ -833,7 +836,7 @@ __global__ void __launch_bounds__(kFoThreads) k_fo_rows_inv(const FoArgs a, cons
 #pragma unroll
     for (int m = 0; m < 8; ++m) v[m] = xr[(m << lgT) + t];
     __syncthreads();
-    fo_inverse(v, t, a.pw, a.tw_w, xr);
+    fo_inverse<PL>(v, t, a.tw_w, xr);
     const size_t pix0 = (size_t)(row0 + r) * a.W + t;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
@@ -884,7 +887,6 @@ static cudaError_t fo_run(osog_ctx* c, const osog_optics* o, const float2* in, f
 {
     const int B = o->B, H = c->H, W = c->W;
     FoArgs a;
-    a.pw = fo_plan(W); a.ph = fo_plan(H);
     a.tw_w = tw_w; a.tw_h = tw_h; a.H = H; a.W = W;
     a.spec_t = spec_t;
     // widest pupil of the batch in x: m_x^2 H^2 <= floor((NA p / lambda)^2 H^2 W^2)  =>  |m_x| <= NA p W / lambda
@@ -905,21 +907,37 @@ static cudaError_t fo_run(osog_ctx* c, const osog_optics* o, const float2* in, f
     const float scale = (float)(1.0 / ((double)H * W));
     const int Rw = kFoThreads / (W / 8), Rh = kFoThreads / (H / 8);           // rows / columns per CTA
     const size_t smem_rows = (size_t)Rw * (W + W / 8) * sizeof(float2), smem_cols = (size_t)Rh * (H + H / 8) * sizeof(float2);
-    cudaError_t e;
     const dim3 gcol((a.nc + Rh - 1) / Rh, B), grow(H / Rw, B);
-    if (sh) k_fo_rows_fwd<true><<<grow, kFoThreads, smem_rows, c->stream>>>(a, in, *sh);
-    else k_fo_rows_fwd<false><<<grow, kFoThreads, smem_rows, c->stream>>>(a, in, FoShear{0, 0, make_float2(1.f, 0.f)});
+    int lg_w = 0, lg_h = 0;
+    while ((1 << lg_w) < W) ++lg_w;
+    while ((1 << lg_h) < H) ++lg_h;
+    const FoShear shv = sh ? *sh : FoShear{0, 0, make_float2(1.f, 0.f)};
+    cudaStream_t st = c->stream;
+// one instantiation per transform length 64 .. 4096
+#define FO_BY_LENGTH(lg, CALL) \
+    switch (lg) { \
+        case 6: { using PL = FoPlan<6>; CALL; } break;   case 7: { using PL = FoPlan<7>; CALL; } break; \
+        case 8: { using PL = FoPlan<8>; CALL; } break;   case 9: { using PL = FoPlan<9>; CALL; } break; \
+        case 10: { using PL = FoPlan<10>; CALL; } break; case 11: { using PL = FoPlan<11>; CALL; } break; \
+        case 12: { using PL = FoPlan<12>; CALL; } break; default: return cudaErrorInvalidValue; \
+    }
+    if (sh) { FO_BY_LENGTH(lg_w, (k_fo_rows_fwd<PL, true><<<grow, kFoThreads, smem_rows, st>>>(a, in, shv))) }
+    else { FO_BY_LENGTH(lg_w, (k_fo_rows_fwd<PL, false><<<grow, kFoThreads, smem_rows, st>>>(a, in, shv))) }
+    cudaError_t e;
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    if (tf) k_fo_cols<2><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign, tf);
-    else if (defocus) k_fo_cols<1><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign, nullptr);
-    else k_fo_cols<0><<<gcol, kFoThreads, smem_cols, c->stream>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign, nullptr);
+    if (tf) { FO_BY_LENGTH(lg_h, (k_fo_cols<PL, 2><<<gcol, kFoThreads, smem_cols, st>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign, tf))) }
+    else if (defocus) { FO_BY_LENGTH(lg_h, (k_fo_cols<PL, 1><<<gcol, kFoThreads, smem_cols, st>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign, tf))) }
+    else { FO_BY_LENGTH(lg_h, (k_fo_cols<PL, 0><<<gcol, kFoThreads, smem_cols, st>>>(a, c->optics, inv_wp, inv_hp, scale, imag_sign, tf))) }
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    if (mode == kFoSensorShot) k_fo_rows_inv<kFoSensorShot><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
-    else if (mode == kFoTimesReal) k_fo_rows_inv<kFoTimesReal><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
-    else if (mode == kFoGopd) k_fo_rows_inv<kFoGopd><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
-    else if (mode == kFoRealSensor) k_fo_rows_inv<kFoRealSensor><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
-    else if (mode == kFoRealSensorShot) k_fo_rows_inv<kFoRealSensorShot><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
-    else k_fo_rows_inv<kFoSensor><<<grow, kFoThreads, smem_rows, c->stream>>>(a, ep);
+    switch (mode) {
+        case kFoSensorShot: FO_BY_LENGTH(lg_w, (k_fo_rows_inv<PL, kFoSensorShot><<<grow, kFoThreads, smem_rows, st>>>(a, ep))) break;
+        case kFoTimesReal: FO_BY_LENGTH(lg_w, (k_fo_rows_inv<PL, kFoTimesReal><<<grow, kFoThreads, smem_rows, st>>>(a, ep))) break;
+        case kFoGopd: FO_BY_LENGTH(lg_w, (k_fo_rows_inv<PL, kFoGopd><<<grow, kFoThreads, smem_rows, st>>>(a, ep))) break;
+        case kFoRealSensor: FO_BY_LENGTH(lg_w, (k_fo_rows_inv<PL, kFoRealSensor><<<grow, kFoThreads, smem_rows, st>>>(a, ep))) break;
+        case kFoRealSensorShot: FO_BY_LENGTH(lg_w, (k_fo_rows_inv<PL, kFoRealSensorShot><<<grow, kFoThreads, smem_rows, st>>>(a, ep))) break;
+        default: FO_BY_LENGTH(lg_w, (k_fo_rows_inv<PL, kFoSensor><<<grow, kFoThreads, smem_rows, st>>>(a, ep))) break;
+    }
+#undef FO_BY_LENGTH
     return cudaGetLastError();
 }
 
