@@ -893,6 +893,26 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
         const uint32_t flags = __float_as_uint(h2.x);
         const double* c = reinterpret_cast<const double*>(rec + 4);
         const double di = (double)(i - h3.y), dj0 = (double)(j - h3.x);
+        // Bound of this particle's top over THIS sub-tile (16 x 8 pixels): a prism's top is the lowest exit plane, so it lies
+        // below every exit plane's maximum over the rectangle (lanes 0..5 take one slab each); an ellipsoid's top is the chord's
+        // midplane plus at most half the longest chord.  Tighter than cz + zmax wherever the sub-tile only sees the particle's flank.
+        if (floor_all > __int_as_float(0xff800000)) {
+            const double djc = (double)(tx * kTile + (wid & 1) * 16 - h3.x) + 7.5, dic = (double)(ty * kTile + (wid >> 1) * 8 - h3.y) + 3.5;
+            double bnd;
+            if (flags & kFlagPrism) {
+                bnd = 1.0e300;
+                if (lane < 6 && (((flags >> 16) >> lane) & 1u) == 0u) {
+                    const double2 uv = *reinterpret_cast<const double2*>(c + 4 * lane);
+                    bnd = c[4 * lane + 2] - uv.x * djc - uv.y * dic + 7.5 * fabs(uv.x) + 3.5 * fabs(uv.y);
+                }
+#pragma unroll
+                for (int d = 1; d < 8; d <<= 1) bnd = fmin(bnd, __shfl_xor_sync(0xffffffffu, bnd, d));
+                bnd = __shfl_sync(0xffffffffu, bnd, 0);
+            } else {
+                bnd = c[8] + c[9] * djc + c[10] * dic + 7.5 * fabs(c[9]) + 3.5 * fabs(c[10]) + 0.5 * c[11];
+            }
+            if ((double)czf + bnd + 1.0e-9 * (1.0 + fabs(bnd)) < (double)floor_all) continue;
+        }
         double zx[4];
         bool hit[4];
         double sxs[4] = {0.0, 0.0, 0.0, 0.0}, sys[4] = {0.0, 0.0, 0.0, 0.0};    // slope of this particle's top (NORMAL only)
