@@ -973,7 +973,8 @@ __global__ void __launch_bounds__(kComposeThreads) k_gbuffer_tile(const float* _
         // lowest top over the warp's 128 pixels, rounded down (-inf while some pixel has no owner)
         float lo = __int_as_float(0x7f800000);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) lo = fminf(lo, who[q] < 0 ? __int_as_float(0xff800000) : __double2float_rd(best[q]));
+        for (int q = 0; q < 4; ++q)                             // (pixels outside the frame never get an owner: they do not count)
+            if (j + q < W && i < H) lo = fminf(lo, who[q] < 0 ? __int_as_float(0xff800000) : __double2float_rd(best[q]));
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, d));
         floor_all = lo - 1.0e-5f;                                // margin for the float sum cz + zmax
