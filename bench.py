@@ -321,6 +321,8 @@ def run_ours(args):
     e1.record(stream)
     torch.cuda.synchronize()
     ms_dic = e0.elapsed_time(e1) / 5
+    ctx.render_opd(P, opt, out=inten)                  # (first use of this instantiation: module load outside the timed loop)
+    torch.cuda.synchronize()
     e0.record(stream)
     for _ in range(5):
         ctx.render_opd(P, opt, out=inten)
