@@ -1,7 +1,9 @@
-// Library stage around cuFFT (timed separately from the hot path, L1-L3):
+// Library stage (timed separately from the hot path, L1-L3):
 // pupil function circ(|k| / (NA / lambda)) exp(i dz k_z) with the 1/(HW) normalisation (Eq. 3),
 // the DIC shear-and-interfere step and the element-wise helpers of its incoherent convolution (Eq. 5),
-// and the sensor: I = |.|^2 plus optional Gaussian read noise from Philox4x32-10.
+// and the sensor: I = |.|^2 plus optional Poisson shot noise and Gaussian read noise from
+// Philox4x32-10.  First half of the file: the element-wise kernels that go around cuFFT (any frame size).  Second half
+// ("L1-L3 fused and pruned"): the whole stage as three FFT kernels of this library for power-of-two frames.
 #include "osog_internal.cuh"
 
 namespace osog {
